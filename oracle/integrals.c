@@ -1,0 +1,468 @@
+/* ORACLE -- test infrastructure, NOT the product.  Plain, slow, CPU-only McMurchie-Davidson
+ * integrals for contracted Cartesian s/p Gaussians, written from the textbook definitions the
+ * paper cites (refs 88-91) and DESIGN.md section "Oracle".  Shares no code with
+ * paper_2601_16949_b200/csrc.  Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline /
+ * --impl reference legs may call it.
+ *
+ * Conventions: AO order = shell order, p components x, y, z.  `ncoef[k]` are the FINAL
+ * coefficients multiplying the bare primitive  x^i y^j z^k exp(-a r^2)  (primitive norm,
+ * contraction coefficient and the contracted-shell renormalisation already folded in by
+ * oracle/integrals.py, which computes them from this file's own overlap routine).
+ *
+ * Every function follows the definitions step by step; there is no blocking or reordering.
+ */
+#define _GNU_SOURCE
+#include <math.h>
+#include <stdlib.h>
+#include <string.h>
+#include <stdint.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+#define LMAX_TOT 4 /* l_a+l_b+l_c+l_d <= 4 for s/p */
+
+typedef struct {
+    int nshells;
+    const double *centers; /* [ncenters][3] */
+    const int32_t *sh_center, *sh_l, *sh_nprim, *sh_off, *ao_off;
+    const double *exps, *ncoef;
+} basis_t;
+
+/* ---- Boys function F_n(T) = int_0^1 t^(2n) exp(-T t^2) dt, n = 0..nmax -------------------- */
+/* T <= 35: series F_m(T) = exp(-T) sum_k (2T)^k / ((2m+1)(2m+3)...(2m+2k+1)) at m = nmax,
+ *          then downward F_(n-1) = (2T F_n + exp(-T)) / (2n-1).
+ * T  > 35: F_0 = 1/2 sqrt(pi/T) erf(sqrt T), upward F_(n+1) = ((2n+1) F_n - exp(-T)) / (2T). */
+void oracle_boys(int nmax, double T, double *F)
+{
+    if (T <= 35.0) {
+        long double term = 1.0L / (2 * nmax + 1), sum = term;
+        for (int k = 1; k < 2000; ++k) {
+            term *= 2.0L * T / (2 * nmax + 2 * k + 1);
+            sum += term;
+            if (term < 1e-19L * sum) break;
+        }
+        long double emt = expl(-(long double)T);
+        long double f = emt * sum;
+        F[nmax] = (double)f;
+        for (int n = nmax; n >= 1; --n) {
+            f = (2.0L * T * f + emt) / (2 * n - 1);
+            F[n - 1] = (double)f;
+        }
+    } else {
+        long double emt = expl(-(long double)T);
+        long double f = 0.5L * sqrtl(M_PIl / T) * erfl(sqrtl((long double)T));
+        F[0] = (double)f;
+        for (int n = 0; n < nmax; ++n) {
+            f = ((2 * n + 1) * f - emt) / (2.0L * T);
+            F[n + 1] = (double)f;
+        }
+    }
+}
+
+/* ---- 1-D Hermite expansion coefficients E_t^{ij}, i,j <= 1, t <= 2 ------------------------ */
+/* E_0^{00} = exp(-mu X_AB^2);
+ * E_t^{i+1,j} = E_{t-1}^{ij}/(2p) + X_PA E_t^{ij} + (t+1) E_{t+1}^{ij}
+ * E_t^{i,j+1} = E_{t-1}^{ij}/(2p) + X_PB E_t^{ij} + (t+1) E_{t+1}^{ij};  E_t = 0 for t<0, t>i+j */
+static void hermite_E(double a, double b, double Ax, double Bx, double E[2][2][3])
+{
+    double p = a + b, mu = a * b / p, XAB = Ax - Bx;
+    double Px = (a * Ax + b * Bx) / p, XPA = Px - Ax, XPB = Px - Bx;
+    memset(E, 0, sizeof(double) * 12);
+    E[0][0][0] = exp(-mu * XAB * XAB);
+    /* i: 0 -> 1 at j = 0 */
+    for (int t = 0; t <= 1; ++t) {
+        double em = (t - 1 >= 0) ? E[0][0][t - 1] : 0.0;
+        double e0 = E[0][0][t];
+        double ep = (t + 1 <= 0) ? E[0][0][t + 1] : 0.0; /* E_t^{00} = 0 for t > 0 */
+        E[1][0][t] = em / (2 * p) + XPA * e0 + (t + 1) * ep;
+    }
+    /* j: 0 -> 1 at i = 0 and i = 1 */
+    for (int i = 0; i <= 1; ++i)
+        for (int t = 0; t <= i + 1; ++t) {
+            double em = (t - 1 >= 0) ? E[i][0][t - 1] : 0.0;
+            double e0 = (t <= i) ? E[i][0][t] : 0.0;
+            double ep = (t + 1 <= i) ? E[i][0][t + 1] : 0.0;
+            E[i][1][t] = em / (2 * p) + XPB * e0 + (t + 1) * ep;
+        }
+}
+
+/* Cartesian powers of component c of a shell with angular momentum l (s: 000; p: x, y, z). */
+static void cart_pow(int l, int c, int pw[3])
+{
+    pw[0] = pw[1] = pw[2] = 0;
+    if (l == 1) pw[c] = 1;
+}
+
+/* ---- one-electron: overlap and dipole (origin O) for one shell pair ----------------------- */
+/* <g_a|g_b> = E_0^x E_0^y E_0^z (pi/p)^{3/2};
+ * <g_a| x-O_x |g_b> = (E_1^x + (P_x - O_x) E_0^x) E_0^y E_0^z (pi/p)^{3/2}. */
+static void shell_pair_1e(const basis_t *B, int sa, int sb, const double *O,
+                          double *S, double *D /* [3][na*nb] or NULL */)
+{
+    int la = B->sh_l[sa], lb = B->sh_l[sb], na = 2 * la + 1, nb = 2 * lb + 1;
+    const double *A = B->centers + 3 * B->sh_center[sa], *Bc = B->centers + 3 * B->sh_center[sb];
+    for (int i = 0; i < na * nb; ++i) {
+        S[i] = 0.0;
+        if (D) D[i] = D[na * nb + i] = D[2 * na * nb + i] = 0.0;
+    }
+    for (int ka = 0; ka < B->sh_nprim[sa]; ++ka)
+        for (int kb = 0; kb < B->sh_nprim[sb]; ++kb) {
+            double a = B->exps[B->sh_off[sa] + ka], b = B->exps[B->sh_off[sb] + kb];
+            double cc = B->ncoef[B->sh_off[sa] + ka] * B->ncoef[B->sh_off[sb] + kb];
+            double p = a + b, pref = pow(M_PI / p, 1.5);
+            double E[3][2][2][3], P[3];
+            for (int x = 0; x < 3; ++x) {
+                hermite_E(a, b, A[x], Bc[x], E[x]);
+                P[x] = (a * A[x] + b * Bc[x]) / p;
+            }
+            for (int ca = 0; ca < na; ++ca)
+                for (int cb = 0; cb < nb; ++cb) {
+                    int pa[3], pb[3];
+                    cart_pow(la, ca, pa);
+                    cart_pow(lb, cb, pb);
+                    double e0[3], e1[3];
+                    for (int x = 0; x < 3; ++x) {
+                        e0[x] = E[x][pa[x]][pb[x]][0];
+                        e1[x] = E[x][pa[x]][pb[x]][1];
+                    }
+                    S[ca * nb + cb] += cc * pref * e0[0] * e0[1] * e0[2];
+                    if (D)
+                        for (int x = 0; x < 3; ++x) {
+                            double m = e1[x] + (P[x] - O[x]) * e0[x];
+                            int y = (x + 1) % 3, z = (x + 2) % 3;
+                            D[x * na * nb + ca * nb + cb] += cc * pref * m * e0[y] * e0[z];
+                        }
+                }
+        }
+}
+
+static basis_t mk_basis(int nshells, const double *centers, const int32_t *sh_center,
+                        const int32_t *sh_l, const int32_t *sh_nprim, const int32_t *sh_off,
+                        const int32_t *ao_off, const double *exps, const double *ncoef)
+{
+    basis_t B = {nshells, centers, sh_center, sh_l, sh_nprim, sh_off, ao_off, exps, ncoef};
+    return B;
+}
+
+#define BASIS_ARGS int nshells, const double *centers, const int32_t *sh_center, \
+    const int32_t *sh_l, const int32_t *sh_nprim, const int32_t *sh_off,       \
+    const int32_t *ao_off, const double *exps, const double *ncoef
+#define BASIS_MK mk_basis(nshells, centers, sh_center, sh_l, sh_nprim, sh_off, ao_off, exps, ncoef)
+
+/* S [nao][nao], D [3][nao][nao] (D may be NULL); origin O[3]. */
+void oracle_one_electron(BASIS_ARGS, int nao, const double *O, double *S, double *D)
+{
+    basis_t B = BASIS_MK;
+    for (int sa = 0; sa < nshells; ++sa)
+        for (int sb = 0; sb < nshells; ++sb) {
+            double s[9], d[27];
+            int na = 2 * sh_l[sa] + 1, nb = 2 * sh_l[sb] + 1;
+            shell_pair_1e(&B, sa, sb, O, s, D ? d : NULL);
+            for (int ca = 0; ca < na; ++ca)
+                for (int cb = 0; cb < nb; ++cb) {
+                    size_t idx = (size_t)(ao_off[sa] + ca) * nao + ao_off[sb] + cb;
+                    S[idx] = s[ca * nb + cb];
+                    if (D)
+                        for (int x = 0; x < 3; ++x)
+                            D[(size_t)x * nao * nao + idx] = d[x * na * nb + ca * nb + cb];
+                }
+        }
+}
+
+/* ---- Hermite Coulomb integrals R^n_{tuv}(alpha, R_PQ) -------------------------------------- */
+/* R^n_{000} = (-2 alpha)^n F_n(alpha |R|^2);
+ * R^n_{t+1,u,v} = t R^{n+1}_{t-1,u,v} + X R^{n+1}_{t,u,v}  (same in u with Y, v with Z). */
+static void hermite_R(int L, double alpha, const double *R, double Rt[5][5][5][5] /* [n][t][u][v] */)
+{
+    double F[LMAX_TOT + 1];
+    double T = alpha * (R[0] * R[0] + R[1] * R[1] + R[2] * R[2]);
+    oracle_boys(L, T, F);
+    memset(Rt, 0, sizeof(double) * 625);
+    double m2a = 1.0;
+    for (int n = 0; n <= L; ++n) {
+        Rt[n][0][0][0] = m2a * F[n];
+        m2a *= -2.0 * alpha;
+    }
+    for (int N = 1; N <= L; ++N) /* total order t+u+v = N needs n <= L-N */
+        for (int t = 0; t <= N; ++t)
+            for (int u = 0; u <= N - t; ++u) {
+                int v = N - t - u;
+                for (int n = 0; n <= L - N; ++n) {
+                    double val;
+                    if (t > 0)
+                        val = (t - 1 > 0 ? (t - 1) * Rt[n + 1][t - 2][u][v] : 0.0) +
+                              R[0] * Rt[n + 1][t - 1][u][v];
+                    else if (u > 0)
+                        val = (u - 1 > 0 ? (u - 1) * Rt[n + 1][t][u - 2][v] : 0.0) +
+                              R[1] * Rt[n + 1][t][u - 1][v];
+                    else
+                        val = (v - 1 > 0 ? (v - 1) * Rt[n + 1][t][u][v - 2] : 0.0) +
+                              R[2] * Rt[n + 1][t][u][v - 1];
+                    Rt[n][t][u][v] = val;
+                }
+            }
+}
+
+/* ---- contracted shell quartet (ab|cd): out[na][nb][nc][nd] --------------------------------- */
+/* primitive: (ab|cd) = 2 pi^{5/2} / (p q sqrt(p+q)) sum_{tuv} E^{ab}_{tuv}
+ *                       sum_{t'u'v'} (-1)^{t'+u'+v'} E^{cd}_{t'u'v'} R^0_{t+t',u+u',v+v'}          */
+static void shell_quartet(const basis_t *B, int sa, int sb, int sc, int sd, double *out)
+{
+    int l[4] = {B->sh_l[sa], B->sh_l[sb], B->sh_l[sc], B->sh_l[sd]};
+    int n[4] = {2 * l[0] + 1, 2 * l[1] + 1, 2 * l[2] + 1, 2 * l[3] + 1};
+    int L = l[0] + l[1] + l[2] + l[3];
+    const double *A = B->centers + 3 * B->sh_center[sa], *Bc = B->centers + 3 * B->sh_center[sb];
+    const double *C = B->centers + 3 * B->sh_center[sc], *D = B->centers + 3 * B->sh_center[sd];
+    int ntot = n[0] * n[1] * n[2] * n[3];
+    long double acc[81];
+    for (int i = 0; i < ntot; ++i) acc[i] = 0.0L;
+    for (int ka = 0; ka < B->sh_nprim[sa]; ++ka)
+    for (int kb = 0; kb < B->sh_nprim[sb]; ++kb) {
+        double a = B->exps[B->sh_off[sa] + ka], b = B->exps[B->sh_off[sb] + kb];
+        double cab = B->ncoef[B->sh_off[sa] + ka] * B->ncoef[B->sh_off[sb] + kb];
+        double p = a + b, P[3], Eab[3][2][2][3];
+        for (int x = 0; x < 3; ++x) {
+            P[x] = (a * A[x] + b * Bc[x]) / p;
+            hermite_E(a, b, A[x], Bc[x], Eab[x]);
+        }
+        for (int kc = 0; kc < B->sh_nprim[sc]; ++kc)
+        for (int kd = 0; kd < B->sh_nprim[sd]; ++kd) {
+            double c = B->exps[B->sh_off[sc] + kc], d = B->exps[B->sh_off[sd] + kd];
+            double ccd = B->ncoef[B->sh_off[sc] + kc] * B->ncoef[B->sh_off[sd] + kd];
+            double q = c + d, Q[3], Ecd[3][2][2][3], RPQ[3];
+            for (int x = 0; x < 3; ++x) {
+                Q[x] = (c * C[x] + d * D[x]) / q;
+                hermite_E(c, d, C[x], D[x], Ecd[x]);
+                RPQ[x] = P[x] - Q[x];
+            }
+            double alpha = p * q / (p + q);
+            double Rt[5][5][5][5];
+            hermite_R(L, alpha, RPQ, Rt);
+            double pref = 2.0 * pow(M_PI, 2.5) / (p * q * sqrt(p + q)) * cab * ccd;
+            int idx = 0;
+            for (int ca = 0; ca < n[0]; ++ca)
+            for (int cb = 0; cb < n[1]; ++cb)
+            for (int cc = 0; cc < n[2]; ++cc)
+            for (int cd = 0; cd < n[3]; ++cd, ++idx) {
+                int pa[3], pb[3], pc[3], pd[3];
+                cart_pow(l[0], ca, pa); cart_pow(l[1], cb, pb);
+                cart_pow(l[2], cc, pc); cart_pow(l[3], cd, pd);
+                double s = 0.0;
+                for (int t = 0; t <= pa[0] + pb[0]; ++t)
+                for (int u = 0; u <= pa[1] + pb[1]; ++u)
+                for (int v = 0; v <= pa[2] + pb[2]; ++v) {
+                    double eab = Eab[0][pa[0]][pb[0]][t] * Eab[1][pa[1]][pb[1]][u] *
+                                 Eab[2][pa[2]][pb[2]][v];
+                    for (int t2 = 0; t2 <= pc[0] + pd[0]; ++t2)
+                    for (int u2 = 0; u2 <= pc[1] + pd[1]; ++u2)
+                    for (int v2 = 0; v2 <= pc[2] + pd[2]; ++v2) {
+                        double ecd = Ecd[0][pc[0]][pd[0]][t2] * Ecd[1][pc[1]][pd[1]][u2] *
+                                     Ecd[2][pc[2]][pd[2]][v2];
+                        double sgn = ((t2 + u2 + v2) & 1) ? -1.0 : 1.0;
+                        s += eab * sgn * ecd * Rt[0][t + t2][u + u2][v + v2];
+                    }
+                }
+                acc[idx] += (long double)(pref * s);
+            }
+        }
+    }
+    for (int i = 0; i < ntot; ++i) out[i] = (double)acc[i];
+}
+
+void oracle_shell_quartet(BASIS_ARGS, int sa, int sb, int sc, int sd, double *out)
+{
+    basis_t B = BASIS_MK;
+    shell_quartet(&B, sa, sb, sc, sd, out);
+}
+
+/* One primitive (un-contracted, coefficient 1) ERI class block, for the pins: centres and exponents
+ * given directly.  out[na][nb][nc][nd]. */
+void oracle_primitive_eri(const double *ctr /* [4][3] */, const double *ex /* [4] */,
+                          const int32_t *l4, double *out)
+{
+    int32_t sh_center[4] = {0, 1, 2, 3}, sh_nprim[4] = {1, 1, 1, 1}, sh_off[4] = {0, 1, 2, 3};
+    int32_t ao_off[4];
+    double ncoef[4] = {1.0, 1.0, 1.0, 1.0};
+    int o = 0;
+    for (int i = 0; i < 4; ++i) { ao_off[i] = o; o += 2 * l4[i] + 1; }
+    basis_t B = mk_basis(4, ctr, sh_center, l4, sh_nprim, sh_off, ao_off, ex, ncoef);
+    shell_quartet(&B, 0, 1, 2, 3, out);
+}
+
+/* Full AO tensor (mu nu|lam sig), [nao]^4, NO symmetry used (tiny systems only). */
+void oracle_eri_tensor(BASIS_ARGS, int nao, double *eri)
+{
+    basis_t B = BASIS_MK;
+    #pragma omp parallel for schedule(dynamic) collapse(2)
+    for (int sa = 0; sa < nshells; ++sa)
+    for (int sb = 0; sb < nshells; ++sb)
+        for (int sc = 0; sc < nshells; ++sc)
+        for (int sd = 0; sd < nshells; ++sd) {
+            double blk[81];
+            shell_quartet(&B, sa, sb, sc, sd, blk);
+            int n0 = 2 * sh_l[sa] + 1, n1 = 2 * sh_l[sb] + 1, n2 = 2 * sh_l[sc] + 1,
+                n3 = 2 * sh_l[sd] + 1, idx = 0;
+            for (int ca = 0; ca < n0; ++ca)
+            for (int cb = 0; cb < n1; ++cb)
+            for (int cc = 0; cc < n2; ++cc)
+            for (int cd = 0; cd < n3; ++cd, ++idx) {
+                size_t m = ao_off[sa] + ca, nu = ao_off[sb] + cb, la = ao_off[sc] + cc,
+                       si = ao_off[sd] + cd;
+                eri[((m * nao + nu) * nao + la) * nao + si] = blk[idx];
+            }
+        }
+}
+
+/* Schwarz bounds Q_ab = sqrt(max_{mu in a, nu in b} (mu nu|mu nu)), [nshells][nshells] (R14). */
+void oracle_schwarz(BASIS_ARGS, double *Q)
+{
+    basis_t B = BASIS_MK;
+    #pragma omp parallel for schedule(dynamic)
+    for (int sa = 0; sa < nshells; ++sa)
+        for (int sb = 0; sb <= sa; ++sb) {
+            double blk[81];
+            shell_quartet(&B, sa, sb, sa, sb, blk);
+            int na = 2 * sh_l[sa] + 1, nb = 2 * sh_l[sb] + 1;
+            double m = 0.0;
+            for (int ca = 0; ca < na; ++ca)
+                for (int cb = 0; cb < nb; ++cb) {
+                    double v = blk[((ca * nb + cb) * na + ca) * nb + cb];
+                    if (v > m) m = v;
+                }
+            Q[(size_t)sa * nshells + sb] = Q[(size_t)sb * nshells + sa] = sqrt(m);
+        }
+}
+
+/* ---- matrix-free J[T], K[T] over Schwarz-screened unique shell quartets -------------------- */
+/* Definitions: J_{mu nu} = sum_{lam sig} (mu nu|lam sig) T_{lam sig},
+ *                          K_{mu lam} = sum_{nu sig} (mu nu|lam sig) T_{nu sig},  T NOT symmetric.
+ * Unique quartets: a>=b, c>=d, pair(ab) >= pair(cd); each integral is applied through all 8
+ * index images with weight 1/2 per coincidence (a==b, c==d, ab==cd), the standard degeneracy
+ * rule; tests pin this against the plain N^4 contraction of oracle_eri_tensor.
+ * T, J, K: [nvec][nao][nao].  Returns the number of unique shell quartets with Q_ab Q_cd >= tau
+ * (R14) through *nquartets, primitive quartets through *nprimq.  tau <= 0 disables screening. */
+void oracle_jk(BASIS_ARGS, int nao, int nvec, const double *T, double tau, const double *Qs,
+               double *J, double *K, int64_t *nquartets, int64_t *nprimq)
+{
+    basis_t B = BASIS_MK;
+    size_t nn = (size_t)nao * nao;
+    memset(J, 0, sizeof(double) * nn * nvec);
+    memset(K, 0, sizeof(double) * nn * nvec);
+    int64_t nq_tot = 0, npq_tot = 0;
+    int npair = nshells * (nshells + 1) / 2;
+    #pragma omp parallel
+    {
+        double *Jl = calloc(nn * nvec, sizeof(double)), *Kl = calloc(nn * nvec, sizeof(double));
+        int64_t nq = 0, npq = 0;
+        #pragma omp for schedule(dynamic, 4)
+        for (int ab = npair - 1; ab >= 0; --ab) {
+            int sa = (int)((sqrt(8.0 * ab + 1.0) - 1.0) / 2.0);
+            while ((sa + 1) * (sa + 2) / 2 <= ab) ++sa;
+            while (sa * (sa + 1) / 2 > ab) --sa;
+            int sb = ab - sa * (sa + 1) / 2;
+            double qab = Qs[(size_t)sa * nshells + sb];
+            for (int cd = 0; cd <= ab; ++cd) {
+                int sc = (int)((sqrt(8.0 * cd + 1.0) - 1.0) / 2.0);
+                while ((sc + 1) * (sc + 2) / 2 <= cd) ++sc;
+                while (sc * (sc + 1) / 2 > cd) --sc;
+                int sd = cd - sc * (sc + 1) / 2;
+                if (tau > 0.0 && qab * Qs[(size_t)sc * nshells + sd] < tau) continue;
+                ++nq;
+                npq += (int64_t)sh_nprim[sa] * sh_nprim[sb] * sh_nprim[sc] * sh_nprim[sd];
+                double blk[81];
+                shell_quartet(&B, sa, sb, sc, sd, blk);
+                double w = 1.0;
+                if (sa == sb) w *= 0.5;
+                if (sc == sd) w *= 0.5;
+                if (ab == cd) w *= 0.5;
+                int n0 = 2 * sh_l[sa] + 1, n1 = 2 * sh_l[sb] + 1, n2 = 2 * sh_l[sc] + 1,
+                    n3 = 2 * sh_l[sd] + 1, idx = 0;
+                for (int ca = 0; ca < n0; ++ca)
+                for (int cb = 0; cb < n1; ++cb)
+                for (int cc = 0; cc < n2; ++cc)
+                for (int cdd = 0; cdd < n3; ++cdd, ++idx) {
+                    double I = w * blk[idx];
+                    size_t m = ao_off[sa] + ca, n = ao_off[sb] + cb, l = ao_off[sc] + cc,
+                           s = ao_off[sd] + cdd;
+                    /* the 8 images (m n|l s) (n m|l s) (m n|s l) (n m|s l) and bra<->ket */
+                    size_t im[8][4] = {{m, n, l, s}, {n, m, l, s}, {m, n, s, l}, {n, m, s, l},
+                                       {l, s, m, n}, {s, l, m, n}, {l, s, n, m}, {s, l, n, m}};
+                    for (int v = 0; v < nvec; ++v) {
+                        const double *Tv = T + v * nn;
+                        double *Jv = Jl + v * nn, *Kv = Kl + v * nn;
+                        for (int g = 0; g < 8; ++g) {
+                            size_t i0 = im[g][0], i1 = im[g][1], i2 = im[g][2], i3 = im[g][3];
+                            Jv[i0 * nao + i1] += I * Tv[i2 * nao + i3];
+                            Kv[i0 * nao + i2] += I * Tv[i1 * nao + i3];
+                        }
+                    }
+                }
+            }
+        }
+        #pragma omp critical
+        {
+            for (size_t i = 0; i < nn * nvec; ++i) { J[i] += Jl[i]; K[i] += Kl[i]; }
+            nq_tot += nq;
+            npq_tot += npq;
+        }
+        free(Jl);
+        free(Kl);
+    }
+    if (nquartets) *nquartets = nq_tot;
+    if (nprimq) *nprimq = npq_tot;
+}
+
+/* Sampled elements of J[T] and K[T] straight from the definitions (no symmetry, no screening):
+ * for each sample s with AO pair (mu, nu): J = sum_{lam sig} (mu nu|lam sig) T[lam][sig],
+ * K = sum_{lam sig} (mu lam|nu sig) T[lam][sig].  Jout, Kout: [nsamp][nvec]. */
+void oracle_jk_samples(BASIS_ARGS, int nao, int nvec, const double *T, int nsamp,
+                       const int32_t *smu, const int32_t *snu, double *Jout, double *Kout)
+{
+    basis_t B = BASIS_MK;
+    size_t nn = (size_t)nao * nao;
+    int32_t *ao2sh = malloc(sizeof(int32_t) * nao);
+    for (int s = 0; s < nshells; ++s)
+        for (int c = 0; c < 2 * sh_l[s] + 1; ++c) ao2sh[ao_off[s] + c] = s;
+    #pragma omp parallel for schedule(dynamic)
+    for (int smp = 0; smp < nsamp; ++smp) {
+        int mu = smu[smp], nu = snu[smp], sa = ao2sh[mu], sb = ao2sh[nu];
+        int ca = mu - ao_off[sa], cb = nu - ao_off[sb];
+        int na = 2 * sh_l[sa] + 1, nb = 2 * sh_l[sb] + 1;
+        (void)na;
+        long double Jacc[64], Kacc[64];
+        for (int v = 0; v < nvec; ++v) Jacc[v] = Kacc[v] = 0.0L;
+        for (int sc = 0; sc < nshells; ++sc)
+            for (int sd = 0; sd < nshells; ++sd) {
+                int nc = 2 * sh_l[sc] + 1, nd = 2 * sh_l[sd] + 1;
+                double bj[81], bk[81];
+                shell_quartet(&B, sa, sb, sc, sd, bj); /* (mu nu|lam sig) */
+                shell_quartet(&B, sa, sc, sb, sd, bk); /* (mu lam|nu sig) */
+                for (int cc = 0; cc < nc; ++cc)
+                    for (int cd = 0; cd < nd; ++cd) {
+                        size_t lam = ao_off[sc] + cc, sig = ao_off[sd] + cd;
+                        double ij = bj[((ca * nb + cb) * nc + cc) * nd + cd];
+                        double ik = bk[((ca * nc + cc) * nb + cb) * nd + cd];
+                        for (int v = 0; v < nvec; ++v) {
+                            double t = T[v * nn + lam * nao + sig];
+                            Jacc[v] += (long double)(ij * t);
+                            Kacc[v] += (long double)(ik * t);
+                        }
+                    }
+            }
+        for (int v = 0; v < nvec; ++v) {
+            Jout[(size_t)smp * nvec + v] = (double)Jacc[v];
+            Kout[(size_t)smp * nvec + v] = (double)Kacc[v];
+        }
+    }
+    free(ao2sh);
+}
+
+int oracle_num_threads(void)
+{
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}

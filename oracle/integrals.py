@@ -1,0 +1,167 @@
+"""ORACLE (test infrastructure, not the product): ctypes front-end of oracle/integrals.c.
+
+Builds liboracle.so with gcc on first use.  Inputs are the plain arrays of `workloads.Basis`
+(duck-typed: this package imports neither `workloads` nor the CUDA package).
+"""
+from __future__ import annotations
+
+import ctypes as ct
+import os
+import subprocess
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "integrals.c")
+_LIB = os.path.join(_HERE, "liboracle.so")
+_lib = None
+
+_dp = ct.POINTER(ct.c_double)
+_ip = ct.POINTER(ct.c_int32)
+
+
+def build(force: bool = False) -> str:
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        subprocess.check_call(["gcc", "-O2", "-fopenmp", "-fPIC", "-shared", "-o", _LIB, _SRC, "-lm"])
+    return _LIB
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        _lib = ct.CDLL(build())
+    return _lib
+
+
+def _d(a):
+    a = np.ascontiguousarray(a, dtype=np.float64)
+    return a, a.ctypes.data_as(_dp)
+
+
+def _i(a):
+    a = np.ascontiguousarray(a, dtype=np.int32)
+    return a, a.ctypes.data_as(_ip)
+
+
+def boys(nmax: int, T: float) -> np.ndarray:
+    F = np.zeros(nmax + 1)
+    lib().oracle_boys(ct.c_int(nmax), ct.c_double(T), F.ctypes.data_as(_dp))
+    return F
+
+
+def primitive_norm(a, l):
+    """N(a,0) = (2a/pi)^(3/4); N(a,1) = (2a/pi)^(3/4) 2 sqrt(a)  (definitions)."""
+    a = np.asarray(a, dtype=np.float64)
+    n = (2.0 * a / np.pi) ** 0.75
+    return n * np.where(np.asarray(l) == 1, 2.0 * np.sqrt(a), 1.0)
+
+
+class OracleBasis:
+    """Holds the basis arrays + final coefficients (R11: each contracted AO scaled to <phi|phi>=1,
+    the scale taken from this oracle's own overlap routine)."""
+
+    def __init__(self, basis):
+        self.centers, self._pc = _d(basis.centers)
+        self.sh_center, self._psc = _i(basis.sh_center)
+        self.sh_l, self._pl = _i(basis.sh_l)
+        self.sh_nprim, self._pn = _i(basis.sh_nprim)
+        self.sh_off, self._po = _i(basis.sh_off)
+        self.nshells = int(self.sh_l.shape[0])
+        n = 2 * self.sh_l.astype(np.int64) + 1
+        self.ao_off, self._pa = _i(np.concatenate([[0], np.cumsum(n)[:-1]]))
+        self.nao = int(n.sum())
+        self.exps, self._pe = _d(basis.exps)
+        l_of_prim = np.repeat(self.sh_l, self.sh_nprim)
+        raw = np.asarray(basis.coefs, dtype=np.float64) * primitive_norm(self.exps, l_of_prim)
+        self.ncoef, self._pk = _d(raw)
+        S = self.overlap()
+        scale = 1.0 / np.sqrt(np.diag(S))
+        sh_scale = scale[self.ao_off]          # x, y, z of a p shell share the radial part
+        self.ncoef, self._pk = _d(raw * np.repeat(sh_scale, self.sh_nprim))
+
+    def _args(self):
+        return (ct.c_int(self.nshells), self._pc, self._psc, self._pl, self._pn, self._po,
+                self._pa, self._pe, self._pk)
+
+    def overlap(self) -> np.ndarray:
+        S = np.zeros((self.nao, self.nao))
+        O = np.zeros(3)
+        lib().oracle_one_electron(*self._args(), ct.c_int(self.nao), O.ctypes.data_as(_dp),
+                                  S.ctypes.data_as(_dp), None)
+        return S
+
+    def dipole(self, origin=(0.0, 0.0, 0.0)):
+        S = np.zeros((self.nao, self.nao))
+        D = np.zeros((3, self.nao, self.nao))
+        O = np.asarray(origin, dtype=np.float64)
+        lib().oracle_one_electron(*self._args(), ct.c_int(self.nao), O.ctypes.data_as(_dp),
+                                  S.ctypes.data_as(_dp), D.ctypes.data_as(_dp))
+        return D
+
+    def shell_quartet(self, a, b, c, d) -> np.ndarray:
+        n = [2 * int(self.sh_l[s]) + 1 for s in (a, b, c, d)]
+        out = np.zeros(n)
+        lib().oracle_shell_quartet(*self._args(), ct.c_int(a), ct.c_int(b), ct.c_int(c),
+                                   ct.c_int(d), out.ctypes.data_as(_dp))
+        return out
+
+    def eri_tensor(self) -> np.ndarray:
+        N = self.nao
+        if N > 64:
+            raise ValueError("full N^4 tensor only for tiny systems")
+        eri = np.zeros((N, N, N, N))
+        lib().oracle_eri_tensor(*self._args(), ct.c_int(N), eri.ctypes.data_as(_dp))
+        return eri
+
+    def schwarz(self) -> np.ndarray:
+        Q = np.zeros((self.nshells, self.nshells))
+        lib().oracle_schwarz(*self._args(), Q.ctypes.data_as(_dp))
+        return Q
+
+    def jk(self, T: np.ndarray, tau: float = 0.0, Q: np.ndarray | None = None):
+        """Matrix-free J[T], K[T] for T [nvec][N][N]; returns J, K, n_shell_quartets, n_prim_quartets."""
+        T = np.ascontiguousarray(T, dtype=np.float64)
+        if T.ndim == 2:
+            T = T[None]
+        nvec, N = T.shape[0], self.nao
+        if Q is None:
+            Q = self.schwarz()
+        Q = np.ascontiguousarray(Q)
+        J = np.zeros_like(T)
+        K = np.zeros_like(T)
+        nq = ct.c_int64(0)
+        npq = ct.c_int64(0)
+        lib().oracle_jk(*self._args(), ct.c_int(N), ct.c_int(nvec), T.ctypes.data_as(_dp),
+                        ct.c_double(tau), Q.ctypes.data_as(_dp), J.ctypes.data_as(_dp),
+                        K.ctypes.data_as(_dp), ct.byref(nq), ct.byref(npq))
+        return J, K, nq.value, npq.value
+
+    def jk_samples(self, T: np.ndarray, mu, nu):
+        """J[T]_{mu nu}, K[T]_{mu nu} at sampled AO pairs, from the definitions (no screening)."""
+        T = np.ascontiguousarray(T, dtype=np.float64)
+        if T.ndim == 2:
+            T = T[None]
+        nvec = T.shape[0]
+        assert nvec <= 64
+        mu_a, pm = _i(mu)
+        nu_a, pn = _i(nu)
+        ns = mu_a.shape[0]
+        J = np.zeros((ns, nvec))
+        K = np.zeros((ns, nvec))
+        lib().oracle_jk_samples(*self._args(), ct.c_int(self.nao), ct.c_int(nvec),
+                                T.ctypes.data_as(_dp), ct.c_int(ns), pm, pn,
+                                J.ctypes.data_as(_dp), K.ctypes.data_as(_dp))
+        return J, K
+
+
+def primitive_eri(centers4, exps4, l4) -> np.ndarray:
+    """Un-normalised primitive ERI block (ab|cd) with unit coefficients, for the pins."""
+    c, pc = _d(np.asarray(centers4).reshape(4, 3))
+    e, pe = _d(exps4)
+    l, pl = _i(l4)
+    out = np.zeros([2 * int(x) + 1 for x in l])
+    lib().oracle_primitive_eri(pc, pe, pl, out.ctypes.data_as(_dp))
+    return out
+
+
+def num_threads() -> int:
+    return int(lib().oracle_num_threads())

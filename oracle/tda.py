@@ -1,0 +1,221 @@
+"""ORACLE (test infrastructure, not the product): the RT-TDA definitions in plain numpy, fp64.
+
+Follows PAPER.md section 2 in the paper's order and notation; every reading of an ambiguous passage
+is listed in DESIGN.md ("Readings").  Nothing here is blocked, fused or reordered.
+
+  A_{ia,jb} = delta_ij delta_ab (eps_a - eps_i) + 2 (ia|jb) - c_x (ij|ab)        eq. 3, R1
+  index ia = i*nvirt + a (virtuals run fastest)
+  sigma = A X                                                                      eq. 11
+  extended vector: element 0 = KS ground state, A_00 = 0, A_0,ia = 0               P:102, R2
+  X = q + i p, (q', p') = (H p, -H q)                                              eq. 12-15
+  H(t) = A_ext + E(t) M,  M = CSF matrix of the position operator along d          eq. 16, R5
+  M from MO-basis dipoles via the Slater-Condon rules                              eq. 19a-f
+  pulses                                                                           eq. 18a-d
+  R(t) = X(eps)^dagger X(eps + t)                                                  eq. 20
+"""
+from __future__ import annotations
+
+import numpy as np
+
+SQRT2 = np.sqrt(2.0)
+
+
+# ---------------------------------------------------------------- A matrix and sigma (dense route)
+def mo_eri_blocks(eri, C_o, C_v):
+    """(ia|jb) and (ij|ab) from the AO tensor (mu nu|lam sig) by four quarter transforms (eq. 4)."""
+    ovov = np.einsum("mnls,mi,na,lj,sb->iajb", eri, C_o, C_v, C_o, C_v, optimize=True)
+    oovv = np.einsum("mnls,mi,nj,la,sb->ijab", eri, C_o, C_o, C_v, C_v, optimize=True)
+    return ovov, oovv
+
+
+def build_A(eri, C_o, C_v, eps, cx=1.0):
+    """Dense singles block of A (eq. 3 under R1), shape [nocc*nvirt][nocc*nvirt]."""
+    no, nv = C_o.shape[1], C_v.shape[1]
+    ovov, oovv = mo_eri_blocks(eri, C_o, C_v)
+    A = 2.0 * ovov - cx * np.transpose(oovv, (0, 2, 1, 3))     # (ij|ab) -> [i][a][j][b]
+    A = A.reshape(no * nv, no * nv).copy()
+    de = (eps[no:][None, :] - eps[:no][:, None]).reshape(-1)    # eps_a - eps_i at ia = i*nv + a
+    A[np.diag_indices(no * nv)] += de
+    return A
+
+
+def extend_A(A):
+    """A_ext = diag(A_00 = 0, A), no coupling between element 0 and the singles (R2)."""
+    n = A.shape[0]
+    Ae = np.zeros((n + 1, n + 1))
+    Ae[1:, 1:] = A
+    return Ae
+
+
+def sigma_dense(A, X):
+    """sigma_v = A x_v for X [nvec][ncsf] (eq. 11)."""
+    return X @ A.T
+
+
+def transition_density(X, C_o, C_v):
+    """T_v = C_o X_v C_v^T  (T_{lam sig} = sum_jb C_{lam j} X_jb C_{sig b}); NOT symmetric."""
+    no, nv = C_o.shape[1], C_v.shape[1]
+    return np.einsum("lj,vjb,sb->vls", C_o, X.reshape(-1, no, nv), C_v, optimize=True)
+
+
+def sigma_from_jk(X, J, K, C_o, C_v, eps, cx=1.0):
+    """sigma = d_eps o X + C_o^T (2 J - c_x K) C_v  (matrix-free identity of DESIGN.md)."""
+    no, nv = C_o.shape[1], C_v.shape[1]
+    de = (eps[no:][None, :] - eps[:no][:, None]).reshape(-1)
+    F = 2.0 * J - cx * K
+    S = np.einsum("mi,vmn,na->via", C_o, F, C_v, optimize=True).reshape(X.shape[0], no * nv)
+    return de[None, :] * X + S
+
+
+def sigma_matrix_free(ob, X, C_o, C_v, eps, cx=1.0, tau=0.0, Q=None):
+    """sigma through the oracle's own J/K (ob: oracle.integrals.OracleBasis)."""
+    T = transition_density(X, C_o, C_v)
+    J, K, nq, npq = ob.jk(T, tau=tau, Q=Q)
+    return sigma_from_jk(X, J, K, C_o, C_v, eps, cx), nq, npq
+
+
+# ---------------------------------------------------------------- dipole operator in the CSF basis
+def mo_dipoles(D_ao, C_o, C_v, d):
+    """D_d = sum_k d_k D^k in the MO basis: D_oo, D_vv, D_ov and D_00 = 2 tr D_oo (R3)."""
+    Dd = np.einsum("k,kmn->mn", np.asarray(d, dtype=np.float64), D_ao)
+    D_oo = C_o.T @ Dd @ C_o
+    D_vv = C_v.T @ Dd @ C_v
+    D_ov = C_o.T @ Dd @ C_v
+    return D_oo, D_vv, D_ov, 2.0 * np.trace(D_oo)
+
+
+def build_M_explicit(D_oo, D_vv, D_ov, D_00):
+    """The six Slater-Condon rules of eq. 19, element by element (R3, R4)."""
+    no, nv = D_ov.shape
+    n = no * nv
+    M = np.zeros((n + 1, n + 1))
+    M[0, 0] = D_00                                                    # 19a
+    for i in range(no):
+        for a in range(nv):
+            ia = 1 + i * nv + a
+            M[0, ia] = M[ia, 0] = SQRT2 * D_ov[i, a]                  # 19b
+            for j in range(no):
+                for b in range(nv):
+                    jb = 1 + j * nv + b
+                    if i == j and a == b:
+                        M[ia, jb] = D_00 - D_oo[i, i] + D_vv[a, a]    # 19c
+                    elif i == j:
+                        M[ia, jb] = D_vv[a, b]                        # 19d
+                    elif a == b:
+                        M[ia, jb] = -D_oo[i, j]                       # 19e
+                    # else 0: differ by more than one electron       # 19f
+    return M
+
+
+def apply_M(y, D_oo, D_vv, D_ov, D_00):
+    """Matrix-free M y:  (My)_0 = D_00 y_0 + sqrt2 sum D_ov Y;  (My)_ia = [sqrt2 D_ov y_0 + D_00 Y
+    + Y D_vv - D_oo Y]_ia.  y may be complex, shape [1+ncsf]."""
+    no, nv = D_ov.shape
+    Y = y[1:].reshape(no, nv)
+    out = np.empty_like(y)
+    out[0] = D_00 * y[0] + SQRT2 * np.sum(D_ov * Y)
+    out[1:] = (SQRT2 * D_ov * y[0] + D_00 * Y + Y @ D_vv - D_oo @ Y).reshape(-1)
+    return out
+
+
+# ---------------------------------------------------------------- pulses (eq. 18) and propagation
+def field_value(f: dict, t: float) -> float:
+    """Scalar E(t).  'delta' is applied as a kick by `kick`, its E(t) is 0 (R8)."""
+    typ = f.get("type", "none")
+    if typ in ("none", "delta"):
+        return 0.0
+    E0, w = f["E0"], f.get("omega", 0.0)
+    if typ == "cw":                                                   # 18b
+        return E0 * np.sin(w * t)
+    if typ == "tl":                                                   # 18c
+        s = t - f["t0"]
+        return E0 * np.exp(-s * s / (2.0 * f["sigma"] ** 2)) * np.sin(w * s)
+    if typ == "chirp":                                                # 18d
+        s = t - f["t0"]
+        return E0 * np.exp(-s * s / (2.0 * f["sigma"] ** 2)) * np.sin((w + 0.5 * f["beta"] * s) * s)
+    if typ == "sin2":                                                 # R9
+        Te = f["T_env"]
+        if t < 0.0 or t > Te:
+            return 0.0
+        return E0 * np.sin(np.pi * t / Te) ** 2 * np.sin(w * t)
+    raise ValueError(typ)
+
+
+def kick(y, f, apply_Md):
+    """Linearised delta kick y(0+) = (1 - i kappa M_d) y(0), kappa = E0 (R8)."""
+    return y - 1j * f["E0"] * apply_Md(y)
+
+
+def rk4_propagate(apply_A_ext, apply_Md, y0, f, t_start, dt, nsteps, log=True):
+    """Classical RK4 on y' = -i H(t) y, H(t) y = A_ext y + E(t) M_d y (eq. 1, 14-16; R7).
+
+    Stage times t, t+dt/2, t+dt/2, t+dt; weights 1/6, 1/3, 1/3, 1/6.  A 'delta' field is applied
+    as the linearised kick at t_start and the run is then field-free.  Returns (y, log) with
+    log[n] = (|y|^2, Re R, Im R), R = y(t_start+)^dagger y(t_{n+1}) (eq. 20)."""
+    y = np.array(y0, dtype=np.complex128)
+    if f.get("type") == "delta":
+        y = kick(y, f, apply_Md)
+    yref = y.copy()
+
+    def rhs(t, z):
+        E = field_value(f, t)
+        h = apply_A_ext(z)
+        if E != 0.0:
+            h = h + E * apply_Md(z)
+        return -1j * h
+
+    out = np.zeros((nsteps, 3))
+    t = t_start
+    for n in range(nsteps):
+        k1 = rhs(t, y)
+        k2 = rhs(t + 0.5 * dt, y + 0.5 * dt * k1)
+        k3 = rhs(t + 0.5 * dt, y + 0.5 * dt * k2)
+        k4 = rhs(t + dt, y + dt * k3)
+        y = y + (dt / 6.0) * (k1 + 2.0 * k2 + 2.0 * k3 + k4)
+        t = t_start + (n + 1) * dt
+        if log:
+            R = np.vdot(yref, y)
+            out[n] = (np.vdot(y, y).real, R.real, R.imag)
+    return y, out
+
+
+def rk4_dense(A, D_oo, D_vv, D_ov, D_00, y0, f, t_start, dt, nsteps):
+    """RK4 with the dense singles block A (element 0 decoupled, A_00 = 0)."""
+    def apply_A_ext(z):
+        o = np.empty_like(z)
+        o[0] = 0.0
+        o[1:] = A @ z[1:]
+        return o
+    return rk4_propagate(apply_A_ext, lambda z: apply_M(z, D_oo, D_vv, D_ov, D_00), y0, f,
+                         t_start, dt, nsteps)
+
+
+def rk4_matrix_free(ob, C_o, C_v, eps, cx, tau, Q, D_oo, D_vv, D_ov, D_00, y0, f, t_start, dt,
+                    nsteps):
+    """RK4 where A_ext z is applied through the oracle's matrix-free sigma (real and imaginary
+    parts as two vectors of one J/K pass)."""
+    def apply_A_ext(z):
+        X = np.stack([z[1:].real, z[1:].imag])
+        s, _, _ = sigma_matrix_free(ob, X, C_o, C_v, eps, cx, tau, Q)
+        o = np.empty_like(z)
+        o[0] = 0.0
+        o[1:] = s[0] + 1j * s[1]
+        return o
+    return rk4_propagate(apply_A_ext, lambda z: apply_M(z, D_oo, D_vv, D_ov, D_00), y0, f,
+                         t_start, dt, nsteps)
+
+
+# ---------------------------------------------------------------- spectrum (harness for the pins)
+def spectrum(R, dt, pad=50000):
+    """omega * F[R(t)] with mirroring R(-t) = R(t)^*, Hann window, zero padding (eq. 21).
+
+    R holds R(t_n) for n = 0..n-1 (R[0] = R(0)).  Returns (omega, intensity)."""
+    R = np.asarray(R, dtype=np.complex128)
+    full = np.concatenate([np.conj(R[:0:-1]), R])                   # t = -(n-1)dt .. (n-1)dt
+    full = full * np.hanning(full.shape[0])
+    npad = full.shape[0] + pad
+    ft = np.fft.fft(full, n=npad)
+    om = 2.0 * np.pi * np.fft.fftfreq(npad, d=dt)
+    # R(t) = sum |c_I|^2 exp(-i w_I t): peaks sit at om = -w_I in numpy's sign convention
+    keep = om < 0
+    return -om[keep][::-1], (-om[keep] * np.abs(ft[keep]))[::-1]

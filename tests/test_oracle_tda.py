@@ -1,0 +1,301 @@
+"""Pins for oracle/tda.py: A, the CSF dipole matrix, RK4, kick, spectrum, the paper's Rabi value."""
+import os
+
+import numpy as np
+import pytest
+
+from oracle import tda
+from oracle.integrals import OracleBasis, primitive_eri, primitive_norm
+from workloads import Basis, make_vectors
+
+GOLD = os.path.join(os.path.dirname(__file__), "golden", "paper_values.txt")
+
+
+def paper_values():
+    out = {}
+    for line in open(GOLD):
+        line = line.split("#")[0].split()
+        if len(line) >= 2:
+            out[line[0]] = float(line[1])
+    return out
+
+
+AU_TIME_FS = 2.4188843265857e-2     # CODATA, 1 au of time in fs
+HARTREE_EV = 27.211386245988
+H_EV_S = 4.135667696e-15            # Planck constant in eV s
+I_AU_WCM2 = 3.50944758e16           # intensity of a 1 au field amplitude, W/cm^2
+
+
+# ------------------------------------------------------------------------------------ A
+def test_A_symmetric_and_psd_blocks(tiny):
+    A = tiny["A"]
+    assert np.max(np.abs(A - A.T)) < 1e-13
+    ovov, oovv = tda.mo_eri_blocks(tiny["eri"], tiny["C_o"], tiny["C_v"])
+    n = A.shape[0]
+    assert np.linalg.eigvalsh(ovov.reshape(n, n))[0] > -1e-12            # x^T (ia|jb) x = (rho|rho) >= 0
+    assert np.linalg.eigvalsh(oovv.transpose(0, 2, 1, 3).reshape(n, n))[0] > -1e-12
+    x, y = make_vectors(tiny["cfg"], 2)
+    assert abs(x @ A @ y - y @ A @ x) < 1e-14
+
+
+def test_A_affine_in_cx(tiny):
+    args = (tiny["eri"], tiny["C_o"], tiny["C_v"], tiny["eps"])
+    A0, A1, A2 = tda.build_A(*args, 0.0), tda.build_A(*args, 1.0), tda.build_A(*args, 2.0)
+    assert np.max(np.abs(A2 - 2 * A1 + A0)) < 1e-13
+
+
+def test_A_1x1_closed_form():
+    """2 centres, one s primitive each, nocc = nvirt = 1: A = eps_a - eps_i + 2(ia|ia) - (ii|aa),
+    with every AO integral from the independent (ss|ss) closed form."""
+    from scipy.special import erf
+    R, a, b = 1.4, 0.9, 0.5
+    ctr = np.array([[0, 0, 0], [0, 0, R]], dtype=float)
+    basis = Basis(ctr, np.array([0, 1], dtype=np.int32), np.zeros(2, dtype=np.int32),
+                  np.ones(2, dtype=np.int32), np.array([0, 1], dtype=np.int32),
+                  np.array([a, b]), np.ones(2))
+    ob = OracleBasis(basis)
+    ex, nrm = np.array([a, b]), primitive_norm(np.array([a, b]), 0)
+
+    def F0(T):
+        return 1.0 if T < 1e-14 else 0.5 * np.sqrt(np.pi / T) * erf(np.sqrt(T))
+
+    def ssss(i, j, k, l):
+        p, q = ex[i] + ex[j], ex[k] + ex[l]
+        P = (ex[i] * ctr[i] + ex[j] * ctr[j]) / p
+        Qc = (ex[k] * ctr[k] + ex[l] * ctr[l]) / q
+        Kab = np.exp(-ex[i] * ex[j] / p * np.sum((ctr[i] - ctr[j]) ** 2))
+        Kcd = np.exp(-ex[k] * ex[l] / q * np.sum((ctr[k] - ctr[l]) ** 2))
+        return (2 * np.pi ** 2.5 / (p * q * np.sqrt(p + q)) * Kab * Kcd
+                * F0(p * q / (p + q) * np.sum((P - Qc) ** 2)) * nrm[i] * nrm[j] * nrm[k] * nrm[l])
+
+    eri = np.array([[[[ssss(i, j, k, l) for l in range(2)] for k in range(2)] for j in range(2)]
+                    for i in range(2)])
+    s = (np.pi / (a + b)) ** 1.5 * np.exp(-a * b / (a + b) * R * R) * nrm[0] * nrm[1]
+    co = np.array([1.0, 1.0]) / np.sqrt(2 + 2 * s)                    # bonding / antibonding MOs
+    cv = np.array([1.0, -1.0]) / np.sqrt(2 - 2 * s)
+    iaia = np.einsum("mnls,m,n,l,s->", eri, co, cv, co, cv)
+    iiaa = np.einsum("mnls,m,n,l,s->", eri, co, co, cv, cv)
+    eps = np.array([-0.5, 0.4])
+    A = tda.build_A(ob.eri_tensor(), co[:, None], cv[:, None], eps, 1.0)
+    assert abs(A[0, 0] - (0.9 + 2 * iaia - iiaa)) < 1e-14
+
+
+def test_sigma_matrix_free_equals_dense(tiny):
+    X = make_vectors(tiny["cfg"], 4)
+    s_d = tda.sigma_dense(tiny["A"], X)
+    s_m, nq, npq = tda.sigma_matrix_free(tiny["ob"], X, tiny["C_o"], tiny["C_v"], tiny["eps"], 1.0)
+    assert np.max(np.abs(s_d - s_m)) / np.max(np.abs(s_d)) < 1e-13
+    s_t, nq2, _ = tda.sigma_matrix_free(tiny["ob"], X, tiny["C_o"], tiny["C_v"], tiny["eps"], 1.0, tau=1e-12)
+    assert nq2 <= nq and np.max(np.abs(s_t - s_d)) / np.max(np.abs(s_d)) < 1e-10
+
+
+# ------------------------------------------------------------------------------------ M (eq. 19)
+def test_M_explicit_equals_matrix_free(tiny):
+    d = np.array([0.3, -0.5, 0.8]); d /= np.linalg.norm(d)
+    Doo, Dvv, Dov, D00 = tda.mo_dipoles(tiny["D"], tiny["C_o"], tiny["C_v"], d)
+    M = tda.build_M_explicit(Doo, Dvv, Dov, D00)
+    assert np.max(np.abs(M - M.T)) < 1e-14
+    rng = np.random.default_rng(1)
+    y = rng.standard_normal(M.shape[0]) + 1j * rng.standard_normal(M.shape[0])
+    assert np.max(np.abs(M @ y - tda.apply_M(y, Doo, Dvv, Dov, D00))) < 1e-13
+    # origin shift c changes M only by the multiple 2 nocc (-c.d) of the identity (R6)
+    c = np.array([1.0, 2.0, -0.5])
+    Doo2, Dvv2, Dov2, D002 = tda.mo_dipoles(tiny["ob"].dipole(c), tiny["C_o"], tiny["C_v"], d)
+    M2 = tda.build_M_explicit(Doo2, Dvv2, Dov2, D002)
+    assert np.max(np.abs(M2 - M + 2 * 5 * (c @ d) * np.eye(M.shape[0]))) < 1e-11
+
+
+def test_M_is_slater_condon_of_one_electron_operator():
+    """Independent check of the rules incl. the sqrt(2) (19b) and D_00 = 2 tr D_oo (R3): build singlet
+    CSFs as explicit spin-orbital determinant combinations for 2 occupied + 2 virtual orbitals and
+    evaluate <Phi|sum_i d(i)|Phi'> by brute force over determinants."""
+    import itertools
+    no, nv = 2, 2
+    n = no + nv
+    rng = np.random.default_rng(4)
+    d = rng.standard_normal((n, n)); d = d + d.T                         # spatial one-electron matrix
+    nso = 2 * n                                                           # spin orbital = 2*p + spin
+
+    def det_element(bra, ket):
+        """<bra| sum_i h(i) |ket> for ordered occupation tuples of spin orbitals (Slater-Condon
+        rules by explicit sign-counting through second quantisation)."""
+        tot = 0.0
+        for p in range(nso):
+            for q in range(nso):
+                if p % 2 != q % 2:
+                    continue
+                h = d[p // 2, q // 2]
+                if q not in ket:
+                    continue
+                lst = list(ket)
+                sgn = (-1) ** lst.index(q)
+                lst.remove(q)
+                if p in lst:
+                    continue
+                pos = sum(1 for x in lst if x < p)
+                sgn *= (-1) ** pos
+                lst.insert(pos, p)
+                if tuple(lst) == tuple(bra):
+                    tot += sgn * h
+        return tot
+
+    ground = tuple(range(2 * no))
+
+    def excite(i, a, spin):                                               # a^+_{a s} a_{i s} |0>, sorted
+        lst = list(ground)
+        k = lst.index(2 * i + spin)
+        sgn = (-1) ** k
+        lst.remove(2 * i + spin)
+        new = 2 * (no + a) + spin
+        pos = sum(1 for x in lst if x < new)
+        sgn *= (-1) ** pos
+        lst.insert(pos, new)
+        return sgn, tuple(lst)
+
+    states = [[(1.0, ground)]]
+    for i in range(no):
+        for a in range(nv):
+            sa, da = excite(i, a, 0)
+            sb, db = excite(i, a, 1)
+            states.append([(sa / np.sqrt(2), da), (sb / np.sqrt(2), db)])
+    dim = len(states)
+    Mref = np.zeros((dim, dim))
+    for I in range(dim):
+        for Jx in range(dim):
+            Mref[I, Jx] = sum(ci * cj * det_element(bi, bj) for ci, bi in states[I] for cj, bj in states[Jx])
+    Doo, Dvv, Dov = d[:no, :no], d[no:, no:], d[:no, no:]
+    M = tda.build_M_explicit(Doo, Dvv, Dov, 2 * np.trace(Doo))
+    assert np.max(np.abs(M - Mref)) < 1e-13
+
+
+# ------------------------------------------------------------------------------------ RK4
+def _g(z):
+    return 1 - 1j * z - z ** 2 / 2 + 1j * z ** 3 / 6 + z ** 4 / 24
+
+
+def test_rk4_field_free_eigenvector_closed_form(tiny):
+    A = tiny["A"]
+    w, U = np.linalg.eigh(A)
+    Doo, Dvv, Dov, D00 = tda.mo_dipoles(tiny["D"], tiny["C_o"], tiny["C_v"], (0, 0, 1.0))
+    dt, n = 0.1, 25
+    for I in (0, 7, len(w) - 1):
+        y0 = np.zeros(A.shape[0] + 1, dtype=complex); y0[1:] = U[:, I]
+        y, log = tda.rk4_dense(A, Doo, Dvv, Dov, D00, y0, {"type": "none"}, 0.0, dt, n)
+        z = w[I] * dt
+        assert np.max(np.abs(y[1:] - _g(z) ** n * U[:, I])) < 1e-13
+        # norm drift law |g|^2 - 1 = -z^6/72 + z^8/576
+        assert abs(log[0, 0] - (1 - z ** 6 / 72 + z ** 8 / 576)) < 1e-14
+        assert abs(log[-1, 1] + 1j * log[-1, 2] - _g(z) ** n) < 1e-13
+
+
+def test_rk4_ground_state_stationary_and_order(tiny):
+    A = tiny["A"]
+    Doo, Dvv, Dov, D00 = tda.mo_dipoles(tiny["D"], tiny["C_o"], tiny["C_v"], (0, 0, 1.0))
+    y0 = np.zeros(A.shape[0] + 1, dtype=complex); y0[0] = 1.0
+    y, _ = tda.rk4_dense(A, Doo, Dvv, Dov, D00, y0, {"type": "none"}, 0.0, 0.05, 10)
+    assert np.array_equal(y, y0)                                  # zero field: e_0 stays exactly
+    # with a cw field: halving dt divides the error against a much finer run by ~16
+    f = {"type": "cw", "E0": 0.05, "omega": 0.3}
+    ref, _ = tda.rk4_dense(A, Doo, Dvv, Dov, D00, y0, f, 0.0, 0.0125, 160)
+    e1 = np.max(np.abs(tda.rk4_dense(A, Doo, Dvv, Dov, D00, y0, f, 0.0, 0.1, 20)[0] - ref))
+    e2 = np.max(np.abs(tda.rk4_dense(A, Doo, Dvv, Dov, D00, y0, f, 0.0, 0.05, 40)[0] - ref))
+    assert 12 < e1 / e2 < 20
+
+
+def test_rk4_against_matrix_exponential(tiny):
+    from scipy.linalg import expm
+    A = tiny["A"]
+    Doo, Dvv, Dov, D00 = tda.mo_dipoles(tiny["D"], tiny["C_o"], tiny["C_v"], (0, 0, 1.0))
+    rng = np.random.default_rng(9)
+    y0 = rng.standard_normal(A.shape[0] + 1) + 1j * rng.standard_normal(A.shape[0] + 1)
+    y0 /= np.linalg.norm(y0)
+    y, _ = tda.rk4_dense(A, Doo, Dvv, Dov, D00, y0, {"type": "none"}, 0.0, 0.01, 100)
+    ref = expm(-1j * tda.extend_A(A) * 1.0) @ y0
+    assert np.max(np.abs(y - ref)) < 5e-9        # local error (w dt)^5/120 per step, w <= ~3.5
+
+
+def test_matrix_free_propagation_equals_dense(tiny):
+    A, cfg = tiny["A"], tiny["cfg"]
+    f = dict(cfg.fields[0])
+    Doo, Dvv, Dov, D00 = tda.mo_dipoles(tiny["D"], tiny["C_o"], tiny["C_v"], f["dir"])
+    y0 = np.zeros(A.shape[0] + 1, dtype=complex); y0[0] = 1.0
+    yd, ld = tda.rk4_dense(A, Doo, Dvv, Dov, D00, y0, f, 0.0, cfg.dt, 3)
+    ym, lm = tda.rk4_matrix_free(tiny["ob"], tiny["C_o"], tiny["C_v"], tiny["eps"], 1.0, 0.0, None,
+                                 Doo, Dvv, Dov, D00, y0, f, 0.0, cfg.dt, 3)
+    assert np.max(np.abs(yd - ym)) < 1e-14 and np.max(np.abs(ld - lm)) < 1e-14
+
+
+# ------------------------------------------------------------------------------------ paper pins
+def test_paper_unit_conversions():
+    pv = paper_values()
+    assert abs(0.1 * AU_TIME_FS * 1e3 - pv["dt_01_au_in_as"]) < 0.005
+    assert abs(3000 * AU_TIME_FS - pv["t_3000_au_in_fs"]) < 0.1
+    assert abs(2 * np.pi / 3000 * HARTREE_EV - pv["resolution_ev"]) < 5e-4
+    assert abs(pv["rabi_freq_hz"] * H_EV_S - pv["rabi_freq_ev"]) < 0.01         # nu, not omega
+    assert abs(pv["freq_2p_hz"] * H_EV_S - pv["freq_2p_ev"]) < 0.001
+    assert abs(2 * np.sqrt(2 * np.log(2)) - pv["fwhm_factor"]) < 1e-5
+
+
+def test_rabi_period_matches_paper_table2():
+    """Two-level limit of propagator + field coupling (eq. 16, 18b): resonant cw field,
+    mu = 1.5624 au, I = 1e12 W/cm^2  =>  T = 2 pi/(mu E0) = 18.22 fs (Table 2)."""
+    pv = paper_values()
+    mu = pv["rabi_mu_au"]
+    E0 = np.sqrt(pv["rabi_intensity_wcm2"] / I_AU_WCM2)
+    w0 = pv["rabi_freq_ev"] / HARTREE_EV
+    T_exact_fs = 2 * np.pi / (mu * E0) * AU_TIME_FS
+    assert abs(T_exact_fs - pv["rabi_period_exact_1"]) < 0.01
+    for k in range(1, 6):
+        assert abs(k * T_exact_fs - pv["rabi_period_exact_%d" % k]) < 0.03
+    # propagate the 2-level model with the oracle's RK4 through its generic interface
+    Amat = np.array([[0.0, 0.0], [0.0, w0]])
+    Mmat = np.array([[0.0, mu], [mu, 0.0]])
+    dt = pv["rabi_dt_au"]
+    nsteps = int(1.05 * 2 * np.pi / (mu * E0) / dt)
+    f = {"type": "cw", "E0": E0, "omega": w0}
+    y = np.array([1.0, 0.0], dtype=complex)
+    pops = np.zeros(nsteps)
+    # step one at a time through the same routine to record populations (eq. 22)
+    yk, t = y, 0.0
+    for n in range(nsteps):
+        yk, _ = tda.rk4_propagate(lambda z: Amat @ z, lambda z: Mmat @ z, yk, f, t, dt, 1, log=False)
+        t = (n + 1) * dt
+        pops[n] = abs(yk[0]) ** 2
+    # first full return of the ground-state population after the inversion
+    half = np.argmin(pops)
+    assert pops[half] < 5e-3                                      # complete inversion
+    ret = half + np.argmax(pops[half:])
+    T_fs = (ret + 1) * dt * AU_TIME_FS
+    assert abs(T_fs - pv["rabi_period_exact_1"]) < 0.1            # paper's RT-TDA: 18.26 vs 18.22
+    assert abs(T_fs - pv["rabi_period_rttda_1"]) < 0.1
+
+
+def test_delta_kick_correlation_closed_form_and_spectrum(tiny):
+    """Linear kick + field-free RK4 (R8): R(t_n) = 1 + k^2 D00^2 + 2 k^2 sum_I |d_I|^2 g(w_I dt)^n,
+    and the spectrum (eq. 21) peaks at eigenvalues of A within 2 pi/T (Table 1)."""
+    A = tiny["A"]
+    w, U = np.linalg.eigh(A)
+    Doo, Dvv, Dov, D00 = tda.mo_dipoles(tiny["D"], tiny["C_o"], tiny["C_v"], (0, 0, 1.0))
+    kappa, dt, n = 1e-4, 0.1, 3000
+    y0 = np.zeros(A.shape[0] + 1, dtype=complex); y0[0] = 1.0
+    f = {"type": "delta", "E0": kappa}
+    # propagate in the eigenbasis through the same generic RK4 (dense A would be the same numbers)
+    y, log = tda.rk4_dense(A, Doo, Dvv, Dov, D00, y0, f, 0.0, dt, 200)
+    dI = U.T @ Dov.reshape(-1)
+    ns = np.arange(1, 201)
+    Rref = 1 + kappa ** 2 * D00 ** 2 + 2 * kappa ** 2 * np.sum(
+        (dI ** 2)[None, :] * _g(w * dt)[None, :] ** ns[:, None], axis=1)
+    R = log[:, 1] + 1j * log[:, 2]
+    assert np.max(np.abs(R - Rref)) < 1e-15 + 1e-9 * kappa ** 2
+    # spectrum of the closed-form series over a long run: strongest peaks sit at eigenvalues
+    ns = np.arange(0, n)
+    Rlong = 2 * kappa ** 2 * np.sum((dI ** 2)[None, :] * _g(w * dt)[None, :] ** ns[:, None], axis=1)
+    om, inten = tda.spectrum(Rlong, dt)
+    res = 2 * np.pi / (n * dt)
+    strongest = np.argsort(w * dI ** 2)[::-1][:3]
+    sel = (om > 0.02) & (om < w.max() + 0.5)
+    om, inten = om[sel], inten[sel]
+    peaks = [i for i in range(1, len(om) - 1) if inten[i] > inten[i - 1] and inten[i] > inten[i + 1]]
+    peaks = sorted(peaks, key=lambda i: -inten[i])[:6]
+    for I in strongest[:2]:
+        assert min(abs(om[p] - w[I]) for p in peaks) < res
