@@ -1,0 +1,156 @@
+/* rttda.h -- C-ABI boundary of the B200-native RT-TDA sigma-vector / propagation library.
+ *
+ * What it computes (citations: P:NNN = /root/reference/PAPER.md line NNN, arXiv 2601.16949;
+ * Rn = reading n in DESIGN.md):
+ *   sigma = A X,  A_{ia,jb} = d_ij d_ab (eps_a - eps_i) + 2 (ia|jb) - c_x (ij|ab)     eq. 3 P:59 (R1), eq. 11
+ *   index ia = i*nvirt + a (virtuals run fastest)
+ *   direct CI through AO-basis Coulomb/exchange builds on the GPU
+ *   i dC/dt = H(t) C,  H(t) = A_ext + E(t) M_d  (M_d from MO dipoles, Slater-Condon)    eq. 1, eq. 16 P:134,
+ *                                                                                       eq. 19 P:161-173 (R3-R5)
+ *   C = q + i p, ground-state element first                                             eq. 12
+ *   pulses                                                                              eq. 18a-d P:146-153 (R8, R9)
+ *   R(t) = C(t0+)^dagger C(t)                                                           eq. 20
+ *
+ * Conventions
+ *   - every call returns RTTDA_OK (0) or a negative RTTDA_E* code; the message of the last failure of the
+ *     calling thread is available from rttda_last_error().  No C++ exception crosses the boundary.
+ *   - "DEVICE" pointers are CUDA device memory on the handle's device; "host" pointers are ordinary host
+ *     memory.  The caller owns every buffer it passes; the handle copies what it keeps.
+ *   - rttda_sigma / rttda_fock / rttda_propagate only ENQUEUE work on `stream` (a cudaStream_t cast to void*,
+ *     NULL = the legacy default stream) and return without synchronising; the *_host variants copy in,
+ *     run, copy out and synchronise the stream before returning.
+ *   - all floating point is IEEE binary64; all matrices are row-major.
+ *   - a handle is bound to the device current at rttda_create; concurrent calls on one handle are not supported.
+ *   - there is no CPU fallback: without a CUDA device every compute call fails with RTTDA_ECUDA.
+ */
+#ifndef RTTDA_H
+#define RTTDA_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define RTTDA_OK      0
+#define RTTDA_EINVAL -1   /* bad shapes, l > 1, nocc + nvirt != nao, nvec < 1, NULL pointer, ... */
+#define RTTDA_ENOMEM -2
+#define RTTDA_ECUDA  -3   /* CUDA runtime error; string in rttda_last_error() */
+
+typedef struct rttda_handle_s* rttda_handle_t;   /* opaque; owns all internal device memory */
+
+/* One contracted Cartesian Gaussian shell: l = 0 (s) or 1 (p: components x, y, z).  AO order = shell order. */
+typedef struct {
+    int32_t center;     /* index into centers */
+    int32_t l;          /* 0 or 1 */
+    int32_t nprim;      /* 1..RTTDA_MAX_NPRIM */
+    int32_t prim_off;   /* offset of this shell's primitives in exps / coefs */
+} rttda_shell_t;
+
+#define RTTDA_MAX_NPRIM 3
+
+typedef struct {
+    const double* centers;        /* host, [ncenters][3], bohr */
+    int32_t ncenters, nshells;
+    const rttda_shell_t* shells;  /* host, [nshells] */
+    const double* exps;           /* host, [sum nprim] Gaussian exponents */
+    const double* coefs;          /* host, [sum nprim]; multiply NORMALISED primitives; the library rescales
+                                     each contracted function to <phi|phi> = 1 (R11) */
+} rttda_basis_t;
+
+/* Pulse shapes, eq. 18a-d.  SIN2 is config 4's envelope (R9):
+ *   DELTA  linearised kick of area E0 applied at t_start: C <- (1 - i E0 M_d) C, then field free (R8)
+ *   CW     E0 sin(omega t)
+ *   TL     E0 exp(-(t-t0)^2 / (2 sigma^2)) sin(omega (t-t0))
+ *   CHIRP  E0 exp(-(t-t0)^2 / (2 sigma^2)) sin((omega + beta (t-t0)/2)(t-t0))
+ *   SIN2   E0 sin^2(pi t / T_env) sin(omega t) for 0 <= t <= T_env, else 0 */
+typedef enum { RTTDA_NONE = 0, RTTDA_DELTA = 1, RTTDA_CW = 2, RTTDA_TL = 3, RTTDA_CHIRP = 4,
+               RTTDA_SIN2 = 5 } rttda_pulse_t;
+
+typedef struct {
+    int32_t type;                               /* rttda_pulse_t */
+    int32_t reserved;
+    double E0, omega, t0, sigma, beta, T_env;
+    double dir[3];                              /* polarisation d (used as given, not renormalised) */
+} rttda_field_t;
+
+/* ---- host-only helpers (no GPU needed) ------------------------------------------------------------ */
+
+/* Overlap matrix S [nao][nao] (host) of the renormalised contracted basis; used by callers to build
+ * orthonormal MOs (C = S^-1/2 Q).  EINVAL if nao does not match the shell table. */
+int rttda_overlap(const rttda_basis_t* basis, int32_t nao, double* S);
+
+/* Position-operator matrices D^k_{mu nu} = <mu| r_k |nu>, origin (0,0,0) (R6); D host [3][nao][nao]. */
+int rttda_dipole_ao(const rttda_basis_t* basis, int32_t nao, double* D);
+
+/* ---- handle -------------------------------------------------------------------------------------- */
+
+/* Once per molecule: normalise shells, build the Schwarz-sorted shell-pair tables and work lists,
+ * MO-basis dipole blocks and eps_a - eps_i.  Synchronises `stream` before returning.
+ *   C_occ  DEVICE [nao][nocc], C_virt DEVICE [nao][nvirt] (copied), eps host [nocc+nvirt] occupied first,
+ *   cx = exact-exchange fraction c_x (1.0 in every config), schwarz_tau: a shell quartet (ab|cd) is skipped
+ *   iff Q_ab Q_cd < tau, Q_ab = sqrt(max (mu nu|mu nu)) (R14); tau = 0 keeps everything. */
+int rttda_create(rttda_handle_t* h, const rttda_basis_t* basis, int32_t nao, int32_t nocc, int32_t nvirt,
+                 const double* C_occ, const double* C_virt, const double* eps, double cx,
+                 double schwarz_tau, void* stream);
+
+int rttda_destroy(rttda_handle_t h);
+
+/* sigma_v = A x_v for v < nvec (singles block only, R16).  X, sigma DEVICE [nvec][nocc*nvirt]; must not
+ * alias.  Steps a1-a5 of DESIGN.md: MO->AO transform (FP64 tensor-core GEMM), Schwarz-screened direct J/K
+ * (one ERI pass per chunk of densities), AO->MO transform + (eps_a - eps_i) x. */
+int rttda_sigma(rttda_handle_t h, int32_t nvec, const double* X, double* sigma, void* stream);
+
+/* Same with HOST buffers: H2D copy of X, sigma build, D2H copy of sigma, stream synchronised. */
+int rttda_sigma_host(rttda_handle_t h, int32_t nvec, const double* X, double* sigma, void* stream);
+
+/* The AO-direct build alone (steps a3-a4): F_v = 2 J[T_v] - c_x K[T_v] for arbitrary (non-symmetric)
+ * AO matrices T_v; J_{mn} = sum_{ls} (mn|ls) T_ls, K_{ml} = sum_{ns} (mn|ls) T_ns.
+ * T, F DEVICE [nvec][nao][nao]. */
+int rttda_fock(rttda_handle_t h, int32_t nvec, const double* T, double* F, void* stream);
+
+/* Fixed-step RK4 (R7) on i dC/dt = H(t) C for ntraj independent trajectories sharing every ERI pass.
+ *   C      DEVICE in/out [ntraj][2][1 + nocc*nvirt]: plane 0 = q (Re), plane 1 = p (Im); element 0 = KS
+ *          ground state
+ *   fields host [ntraj]
+ *   log    DEVICE or NULL, [nsteps][ntraj][3]: |C|^2, Re R, Im R after each step, R relative to the state
+ *          at t_start (after the kick, if any)
+ * Re-entrant in time: call again with t_start += nsteps*dt to continue. */
+int rttda_propagate(rttda_handle_t h, int32_t ntraj, double* C, const rttda_field_t* fields,
+                    double t_start, double dt, int32_t nsteps, double* log, void* stream);
+
+/* Same with HOST buffers for C and log (copies inside, stream synchronised on return). */
+int rttda_propagate_host(rttda_handle_t h, int32_t ntraj, double* C, const rttda_field_t* fields,
+                         double t_start, double dt, int32_t nsteps, double* log, void* stream);
+
+/* Counters and timings.  Keys: */
+#define RTTDA_INFO_NPAIRS_TOTAL      0   /* unique shell pairs a >= b */
+#define RTTDA_INFO_NPAIRS_KEPT       1   /* pairs with Q_ab Q_max >= tau */
+#define RTTDA_INFO_NQUARTETS         2   /* unique shell quartets with Q_ab Q_cd >= tau (R14) */
+#define RTTDA_INFO_NPRIM_QUARTETS    3   /* primitive quartets inside those */
+#define RTTDA_INFO_NQUARTETS_EVAL    4   /* contracted quartet evaluations the kernels perform per ERI pass */
+#define RTTDA_INFO_NPRIM_EVAL        5   /* primitive quartet evaluations per ERI pass */
+#define RTTDA_INFO_FLOPS_EVAL        6   /* FP64 flop model of one ERI pass, evaluation part */
+#define RTTDA_INFO_FLOPS_DIGEST_PER_VEC 7 /* FP64 flop model, digestion per density */
+#define RTTDA_INFO_JK_LAUNCHES       8   /* kernel launches of one ERI pass */
+#define RTTDA_INFO_KERNEL_LAUNCHES   9   /* kernels launched by this handle so far (all entry points) */
+#define RTTDA_INFO_CREATE_MS        10   /* wall time of rttda_create */
+#define RTTDA_INFO_QMAX             11   /* largest Schwarz bound */
+#define RTTDA_INFO_NVEC_CHUNK       12   /* densities served by one ERI pass */
+int rttda_get_info(rttda_handle_t h, int32_t key, double* out);
+
+/* Time the last rttda_sigma/rttda_fock call spent in the J/K kernels, from CUDA events recorded on its
+ * stream (synchronises those events).  ms_out[0] = J/K build, [1] = MO->AO GEMMs, [2] = AO->MO GEMMs. */
+int rttda_last_timings(rttda_handle_t h, double* ms_out);
+
+/* Sustained FP64 FMA throughput of the device (TFLOP/s) from a dependent-chain DFMA kernel run for about
+ * `seconds`; the roofline denominator of the ALU-bound J/K kernels. */
+int rttda_fp64_peak(double seconds, double* tflops_out, void* stream);
+
+const char* rttda_last_error(void);
+const char* rttda_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* RTTDA_H */

@@ -1,0 +1,237 @@
+// C-ABI entry points (include/rttda.h).  Argument checking and marshalling only; every step of the path
+// runs in the kernels of this library.
+#include <chrono>
+#include <cstring>
+#include "common.cuh"
+
+namespace rttda {
+
+static thread_local std::string g_err;
+void set_error(const std::string& msg) { g_err = msg; }
+
+int create_impl(Handle* h, const rttda_basis_t* basis, const double* C_occ, const double* C_virt,
+                const double* eps, cudaStream_t st);
+int overlap_host(const rttda_basis_t* basis, int nao, double* S, double* D);
+
+// [v][N][N] <-> [N][N][v]
+__global__ void interleave_kernel(long long nn, int nvec, const double* __restrict__ in, double* __restrict__ out,
+                                  int to_interleaved)
+{
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= nn * nvec) return;
+    if (to_interleaved) {
+        const long long e = i / nvec; const int v = (int)(i % nvec);
+        out[i] = in[(long long)v * nn + e];
+    } else {
+        const int v = (int)(i / nn); const long long e = i % nn;
+        out[i] = in[e * nvec + v];
+    }
+}
+
+// dependent DFMA chains: 8 independent accumulators per thread, 2 flops per FMA
+__global__ void fp64_peak_kernel(double* out, int iters, double a, double b)
+{
+    double x0 = threadIdx.x, x1 = x0 + 1, x2 = x0 + 2, x3 = x0 + 3, x4 = x0 + 4, x5 = x0 + 5, x6 = x0 + 6, x7 = x0 + 7;
+    for (int i = 0; i < iters; ++i) {
+#pragma unroll
+        for (int u = 0; u < 16; ++u) {
+            x0 = fma(x0, a, b); x1 = fma(x1, a, b); x2 = fma(x2, a, b); x3 = fma(x3, a, b);
+            x4 = fma(x4, a, b); x5 = fma(x5, a, b); x6 = fma(x6, a, b); x7 = fma(x7, a, b);
+        }
+    }
+    out[(size_t)blockIdx.x * blockDim.x + threadIdx.x] = x0 + x1 + x2 + x3 + x4 + x5 + x6 + x7;
+}
+
+}  // namespace rttda
+
+using namespace rttda;
+
+extern "C" {
+
+const char* rttda_last_error(void) { return g_err.c_str(); }
+const char* rttda_version(void) { return "rttda-b200 0.1 (sm_100a)"; }
+
+int rttda_overlap(const rttda_basis_t* basis, int32_t nao, double* S)
+{
+    RT_CHECK(S != nullptr, "rttda_overlap: NULL output");
+    return overlap_host(basis, nao, S, nullptr);
+}
+
+int rttda_dipole_ao(const rttda_basis_t* basis, int32_t nao, double* D)
+{
+    RT_CHECK(D != nullptr, "rttda_dipole_ao: NULL output");
+    return overlap_host(basis, nao, nullptr, D);
+}
+
+int rttda_create(rttda_handle_t* out, const rttda_basis_t* basis, int32_t nao, int32_t nocc, int32_t nvirt,
+                 const double* C_occ, const double* C_virt, const double* eps, double cx, double schwarz_tau,
+                 void* stream)
+{
+    RT_CHECK(out && basis && C_occ && C_virt && eps, "rttda_create: NULL pointer");
+    RT_CHECK(nao > 0 && nocc > 0 && nvirt > 0 && nocc + nvirt == nao, "rttda_create: need nocc + nvirt == nao > 0");
+    RT_CHECK(schwarz_tau >= 0.0, "rttda_create: negative Schwarz threshold");
+    int ndev = 0;
+    cudaError_t e = cudaGetDeviceCount(&ndev);
+    if (e != cudaSuccess || ndev == 0) {
+        set_error(std::string("rttda_create: no CUDA device (") + cudaGetErrorString(e) + "); there is no CPU fallback");
+        return RTTDA_ECUDA;
+    }
+    Handle* h = new (std::nothrow) Handle();
+    if (!h) { set_error("rttda_create: out of host memory"); return RTTDA_ENOMEM; }
+    RT_CUDA(cudaGetDevice(&h->device));
+    h->nao = nao; h->nocc = nocc; h->nvirt = nvirt; h->ncsf = nocc * nvirt;
+    h->cx = cx; h->tau = schwarz_tau;
+    const int r = create_impl(h, basis, C_occ, C_virt, eps, (cudaStream_t)stream);
+    if (r != RTTDA_OK) { rttda_destroy((rttda_handle_t)h); return r; }
+    *out = (rttda_handle_t)h;
+    return RTTDA_OK;
+}
+
+int rttda_destroy(rttda_handle_t hh)
+{
+    Handle* h = (Handle*)hh;
+    if (!h) return RTTDA_OK;
+    cudaDeviceSynchronize();
+    for (void* p : h->dev_allocs) cudaFree(p);
+    for (double* p : {h->wsY, h->wsT, h->wsF, h->wsZ, h->prop_ws}) if (p) cudaFree(p);
+    for (auto& e : h->ev) if (e) cudaEventDestroy(e);
+    delete h;
+    return RTTDA_OK;
+}
+
+int rttda_sigma(rttda_handle_t hh, int32_t nvec, const double* X, double* sigma, void* stream)
+{
+    Handle* h = (Handle*)hh;
+    RT_CHECK(h && X && sigma, "rttda_sigma: NULL pointer");
+    RT_CHECK(nvec >= 1, "rttda_sigma: nvec < 1");
+    RT_CHECK(X != sigma, "rttda_sigma: X and sigma must not alias");
+    return sigma_impl(h, nvec, X, h->ncsf, sigma, h->ncsf, (cudaStream_t)stream);
+}
+
+int rttda_sigma_host(rttda_handle_t hh, int32_t nvec, const double* X, double* sigma, void* stream)
+{
+    Handle* h = (Handle*)hh;
+    RT_CHECK(h && X && sigma, "rttda_sigma_host: NULL pointer");
+    RT_CHECK(nvec >= 1, "rttda_sigma_host: nvec < 1");
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t n = (size_t)nvec * h->ncsf;
+    RT_TRY(ensure_ws(h, &h->wsZ, &h->wsZ_n, 2 * n));
+    RT_CUDA(cudaMemcpyAsync(h->wsZ, X, n * sizeof(double), cudaMemcpyHostToDevice, st));
+    RT_TRY(sigma_impl(h, nvec, h->wsZ, h->ncsf, h->wsZ + n, h->ncsf, st));
+    RT_CUDA(cudaMemcpyAsync(sigma, h->wsZ + n, n * sizeof(double), cudaMemcpyDeviceToHost, st));
+    RT_CUDA(cudaStreamSynchronize(st));
+    return RTTDA_OK;
+}
+
+int rttda_fock(rttda_handle_t hh, int32_t nvec, const double* T, double* F, void* stream)
+{
+    Handle* h = (Handle*)hh;
+    RT_CHECK(h && T && F, "rttda_fock: NULL pointer");
+    RT_CHECK(nvec >= 1, "rttda_fock: nvec < 1");
+    cudaStream_t st = (cudaStream_t)stream;
+    const long long nn = (long long)h->nao * h->nao;
+    RT_TRY(ensure_ws(h, &h->wsT, &h->wsT_n, (size_t)nvec * nn));
+    RT_TRY(ensure_ws(h, &h->wsF, &h->wsF_n, (size_t)nvec * nn));
+    const unsigned grid = (unsigned)((nn * nvec + 255) / 256);
+    RT_CUDA(cudaEventRecord(h->ev[0], st));
+    interleave_kernel<<<grid, 256, 0, st>>>(nn, nvec, T, h->wsT, 1);
+    RT_CUDA(cudaGetLastError());
+    RT_CUDA(cudaEventRecord(h->ev[1], st));
+    RT_CUDA(cudaMemsetAsync(h->wsF, 0, (size_t)nvec * nn * sizeof(double), st));
+    const int chunk = jk_nvec_chunk();
+    for (int v0 = 0; v0 < nvec; v0 += chunk)
+        RT_TRY(jk_build(h, nvec, v0, std::min(chunk, nvec - v0), h->wsT, h->wsF, st));
+    RT_CUDA(cudaEventRecord(h->ev[2], st));
+    interleave_kernel<<<grid, 256, 0, st>>>(nn, nvec, h->wsF, F, 0);
+    RT_CUDA(cudaGetLastError());
+    RT_CUDA(cudaEventRecord(h->ev[3], st));
+    h->ev_valid = true;
+    h->kernel_launches += 2;
+    return RTTDA_OK;
+}
+
+int rttda_propagate(rttda_handle_t hh, int32_t ntraj, double* C, const rttda_field_t* fields, double t_start,
+                    double dt, int32_t nsteps, double* log, void* stream)
+{
+    Handle* h = (Handle*)hh;
+    RT_CHECK(h && C && fields, "rttda_propagate: NULL pointer");
+    RT_CHECK(ntraj >= 1 && ntraj <= 8, "rttda_propagate: ntraj must be in 1..8");
+    RT_CHECK(nsteps >= 0, "rttda_propagate: negative step count");
+    for (int t = 0; t < ntraj; ++t)
+        RT_CHECK(fields[t].type >= RTTDA_NONE && fields[t].type <= RTTDA_SIN2, "rttda_propagate: bad pulse type");
+    return propagate_impl(h, ntraj, C, fields, t_start, dt, nsteps, log, (cudaStream_t)stream);
+}
+
+int rttda_propagate_host(rttda_handle_t hh, int32_t ntraj, double* C, const rttda_field_t* fields,
+                         double t_start, double dt, int32_t nsteps, double* log, void* stream)
+{
+    Handle* h = (Handle*)hh;
+    RT_CHECK(h && C && fields, "rttda_propagate_host: NULL pointer");
+    RT_CHECK(ntraj >= 1 && ntraj <= 8 && nsteps >= 0, "rttda_propagate_host: bad ntraj / nsteps");
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t ns = (size_t)ntraj * 2 * ((size_t)h->ncsf + 1), nl = (size_t)nsteps * ntraj * 3;
+    RT_TRY(ensure_ws(h, &h->wsZ, &h->wsZ_n, ns + nl));
+    RT_CUDA(cudaMemcpyAsync(h->wsZ, C, ns * sizeof(double), cudaMemcpyHostToDevice, st));
+    RT_TRY(rttda_propagate(hh, ntraj, h->wsZ, fields, t_start, dt, nsteps, log ? h->wsZ + ns : nullptr, stream));
+    RT_CUDA(cudaMemcpyAsync(C, h->wsZ, ns * sizeof(double), cudaMemcpyDeviceToHost, st));
+    if (log && nl) RT_CUDA(cudaMemcpyAsync(log, h->wsZ + ns, nl * sizeof(double), cudaMemcpyDeviceToHost, st));
+    RT_CUDA(cudaStreamSynchronize(st));
+    return RTTDA_OK;
+}
+
+int rttda_get_info(rttda_handle_t hh, int32_t key, double* out)
+{
+    Handle* h = (Handle*)hh;
+    RT_CHECK(h && out, "rttda_get_info: NULL pointer");
+    RT_CHECK(key >= 0 && key < 16, "rttda_get_info: unknown key");
+    *out = (key == RTTDA_INFO_KERNEL_LAUNCHES) ? (double)h->kernel_launches : h->info[key];
+    return RTTDA_OK;
+}
+
+int rttda_last_timings(rttda_handle_t hh, double* ms)
+{
+    Handle* h = (Handle*)hh;
+    RT_CHECK(h && ms, "rttda_last_timings: NULL pointer");
+    RT_CHECK(h->ev_valid, "rttda_last_timings: no sigma/fock call yet");
+    RT_CUDA(cudaEventSynchronize(h->ev[3]));
+    float a = 0, b = 0, c = 0;
+    RT_CUDA(cudaEventElapsedTime(&a, h->ev[1], h->ev[2]));
+    RT_CUDA(cudaEventElapsedTime(&b, h->ev[0], h->ev[1]));
+    RT_CUDA(cudaEventElapsedTime(&c, h->ev[2], h->ev[3]));
+    ms[0] = a; ms[1] = b; ms[2] = c;
+    return RTTDA_OK;
+}
+
+int rttda_fp64_peak(double seconds, double* tflops, void* stream)
+{
+    RT_CHECK(tflops && seconds > 0.0, "rttda_fp64_peak: bad arguments");
+    cudaStream_t st = (cudaStream_t)stream;
+    int dev = 0, nsm = 0;
+    RT_CUDA(cudaGetDevice(&dev));
+    RT_CUDA(cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev));
+    const int blocks = nsm * 8, threads = 256, iters = 4096;
+    double* buf = nullptr;
+    RT_CUDA(cudaMalloc((void**)&buf, (size_t)blocks * threads * sizeof(double)));
+    cudaEvent_t e0, e1;
+    RT_CUDA(cudaEventCreate(&e0));
+    RT_CUDA(cudaEventCreate(&e1));
+    fp64_peak_kernel<<<blocks, threads, 0, st>>>(buf, 64, 0.999999, 1e-9);   // warm-up
+    RT_CUDA(cudaStreamSynchronize(st));
+    const double flops_per_launch = (double)blocks * threads * iters * 16.0 * 8.0 * 2.0;
+    double best = 0.0, elapsed = 0.0;
+    while (elapsed < seconds) {
+        RT_CUDA(cudaEventRecord(e0, st));
+        fp64_peak_kernel<<<blocks, threads, 0, st>>>(buf, iters, 0.999999, 1e-9);
+        RT_CUDA(cudaEventRecord(e1, st));
+        RT_CUDA(cudaEventSynchronize(e1));
+        float ms = 0;
+        RT_CUDA(cudaEventElapsedTime(&ms, e0, e1));
+        elapsed += ms * 1e-3;
+        best = flops_per_launch / (ms * 1e-3) * 1e-12;   // sustained: keep the LAST launch's rate
+    }
+    *tflops = best;
+    cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(buf);
+    return RTTDA_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,159 @@
+// Shared declarations of the rttda CUDA library (product path; shares nothing with oracle/).
+#pragma once
+#include <cuda_runtime.h>
+#include <cstdint>
+#include <cstdio>
+#include <string>
+#include <vector>
+#include "../../include/rttda.h"
+
+namespace rttda {
+
+void set_error(const std::string& msg);
+
+#define RT_CUDA(call)                                                                         \
+    do {                                                                                      \
+        cudaError_t e__ = (call);                                                             \
+        if (e__ != cudaSuccess) {                                                             \
+            ::rttda::set_error(std::string(#call) + ": " + cudaGetErrorString(e__));          \
+            return RTTDA_ECUDA;                                                               \
+        }                                                                                     \
+    } while (0)
+
+#define RT_CHECK(cond, msg)                                                                   \
+    do {                                                                                      \
+        if (!(cond)) {                                                                        \
+            ::rttda::set_error(msg);                                                          \
+            return RTTDA_EINVAL;                                                              \
+        }                                                                                     \
+    } while (0)
+
+#define RT_TRY(expr)                                                                          \
+    do {                                                                                      \
+        int r__ = (expr);                                                                     \
+        if (r__ != RTTDA_OK) return r__;                                                      \
+    } while (0)
+
+// ---------------------------------------------------------------------------------------------
+// Shell-pair tables.
+//
+// A primitive pair record (12 doubles, one 96-byte row) of an ORDERED shell pair (first, second):
+//   [0] p = a+b   [1..3] P   [4] c = sqrt(2) pi^(5/4) / p * coefA coefB exp(-mu |AB|^2)
+//   [5] 1/(2p)    [6..8] P - A(first)   [9..11] P - B(second)
+// so that c_bra * c_ket / sqrt(p+q) = 2 pi^(5/2) / (p q sqrt(p+q)) * K_ab K_cd * coefficients.
+constexpr int PRIM_STRIDE = 12;
+
+// Pair classes: 0 = ss, 1 = ps (p first), 2 = pp; contraction sub-class by number of primitive pairs.
+constexpr int NSUB = 3;                       // nprim pairs in {1, 3, 9}
+constexpr int NKETCLASS = 3 * NSUB;           // ket class id = pairclass * NSUB + sub
+__host__ __device__ inline int sub_to_np(int sub) { return sub == 0 ? 1 : (sub == 1 ? 3 : 9); }
+
+// Unique (unordered) pairs of one ket class, sorted by Schwarz bound descending; thread-owned side.
+// Primitive data is SoA: prim[(k * PRIM_STRIDE + f) * n + q] so that consecutive kets coalesce.
+struct KetClass {
+    int n;                 // number of pairs
+    int np;                // primitive pairs per pair (1, 3, 9)
+    const double* Q;       // [n] Schwarz bounds, descending
+    const int* ao_c;       // [n] AO offset of the first (higher-l) shell
+    const int* ao_d;       // [n] AO offset of the second shell
+    const int* same;       // [n] 1 if both shells are the same shell
+    const double* prim;    // [np][PRIM_STRIDE][n]
+};
+
+// Ordered bra record (block-uniform side): shell a fixed by the list, partner b varies.
+struct BraRec {
+    double Q;              // Schwarz bound of the pair
+    int ao_b;              // AO offset of partner shell b
+    int prim_off;          // first primitive-pair row in bra_prim (oriented a first)
+    int pos;               // position of the unordered pair inside its ket class list
+    int flags;             // bit0: canonical orientation (does the J work), bit1: a == b
+};
+
+// All partners b of shell a with given l_b and contraction sub-class, sorted by Q descending.
+struct AList {
+    double Qmax;
+    int ao_a;
+    int rec_begin, rec_end;   // into BraRec array
+    int ketclass;             // ket class id of the (unordered) pairs in this list
+    int np;                   // primitive pairs per record
+};
+
+struct WorkItem {
+    int alist;
+    int ket0;                 // first ket (thread 0) of this block
+};
+
+struct JKLaunch {             // one kernel instantiation: ordered bra class x ket class
+    int la, lb, lc, ld, ketclass;
+    int nwork;
+    const WorkItem* work;     // device
+};
+
+struct JKTables {
+    KetClass kets[NKETCLASS];
+    const BraRec* recs;
+    const AList* alists;
+    const double* bra_prim;   // [nrows][PRIM_STRIDE] AoS
+    const double* boys;       // Boys table
+    double tau;
+    int nao;
+};
+
+constexpr int JK_BLOCK = 128;
+
+// Boys table: rows at T0 = j / 8, j = 0..BOYS_NROW-1; row = F_0..F_11(T0), exp(-T0), padding.
+constexpr int BOYS_ROW = 16;
+constexpr double BOYS_TMAX = 48.0;
+constexpr int BOYS_NROW = 385 + 1;
+void boys_table_host(std::vector<double>& tab);
+
+// ---------------------------------------------------------------------------------------------
+struct Handle {
+    int device = 0;
+    int nao = 0, nocc = 0, nvirt = 0, ncsf = 0, nshells = 0;
+    double cx = 1.0, tau = 0.0;
+    // device-resident inputs
+    double *C_occ = nullptr, *C_virt = nullptr, *deps = nullptr;
+    double* D_ao = nullptr;                    // [3][nao][nao]
+    double *D_oo = nullptr, *D_vv = nullptr, *D_ov = nullptr;   // [3][..]
+    double D_00[3] = {0, 0, 0};
+    // J/K tables
+    JKTables tabs{};
+    std::vector<JKLaunch> launches;
+    std::vector<void*> dev_allocs;             // everything to free
+    // workspaces (grown on demand)
+    double *wsY = nullptr, *wsT = nullptr, *wsF = nullptr, *wsZ = nullptr;
+    size_t wsY_n = 0, wsT_n = 0, wsF_n = 0, wsZ_n = 0;
+    double* prop_ws = nullptr;
+    size_t prop_ws_n = 0;
+    // info
+    double info[16] = {0};
+    long long kernel_launches = 0;
+    cudaEvent_t ev[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
+    bool ev_valid = false;
+};
+
+// jk_kernels.cu
+int jk_build(Handle* h, int nvec_total, int v0, int nv, const double* Tq, double* Fq, cudaStream_t st);
+int jk_nvec_chunk();
+int schwarz_device(int pairclass, int npairs, const int* d_np, const int* d_off, const double* d_prim,
+                   const double* d_boys, double* d_Q, cudaStream_t st);
+
+// gemm_f64.cu: C(m,n) = alpha * sum_k A(m,k) B(k,n) + beta * C(m,n), fully strided, batched.
+struct GemmDesc {
+    int M, N, K, batch;
+    const double* A; long long sam, sak, sabatch;
+    const double* B; long long sbk, sbn, sbbatch;
+    double* C;       long long scm, scn, scbatch;
+    double alpha, beta;
+};
+int gemm_f64(const GemmDesc& g, cudaStream_t st);
+
+// propagate.cu
+int propagate_impl(Handle* h, int ntraj, double* C, const rttda_field_t* fields, double t_start,
+                   double dt, int nsteps, double* log, cudaStream_t st);
+int sigma_impl(Handle* h, int nvec, const double* X, long long ldx, double* sigma, long long lds,
+               cudaStream_t st);
+int ensure_ws(Handle* h, double** p, size_t* cur, size_t need);
+
+}  // namespace rttda

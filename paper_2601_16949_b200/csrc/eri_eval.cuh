@@ -1,0 +1,213 @@
+// Primitive s/p electron-repulsion integrals in registers (McMurchie-Davidson form, cf. P:130 refs 88-91).
+//
+// (ab|cd) = 2 pi^(5/2) / (p q sqrt(p+q)) K_ab K_cd * [ O_a O_b O_c O_d R ](0),  where R_{tuv} are the Hermite
+// Coulomb integrals R^0_{tuv}(alpha, P-Q) and every p function is the operator (X_PA + (1/2p) d/dP_x) acting
+// on the s-type result (for ket functions d/dQ = -d/dP, hence the minus sign).  Everything is unrolled at
+// compile time; Hermite tables live in registers.
+#pragma once
+#include "common.cuh"
+
+namespace rttda {
+
+__host__ __device__ constexpr int nherm(int L) { return (L + 1) * (L + 2) * (L + 3) / 6; }
+// index of Hermite component (t,u,v): ordered by total order N, then s = N - t, then v
+__host__ __device__ constexpr int hidx(int t, int u, int v)
+{
+    return nherm(t + u + v - 1) + (u + v) * (u + v + 1) / 2 + v;
+}
+__host__ __device__ constexpr int hidx_plus(int t, int u, int v, int axis)
+{
+    return axis == 0 ? hidx(t + 1, u, v) : (axis == 1 ? hidx(t, u + 1, v) : hidx(t, u, v + 1));
+}
+
+// ---- Boys function F_0..F_L(T), pre-multiplied by `scale` ---------------------------------------------
+// T < 48: 8-term Taylor expansion of F_L about the nearest grid point T0 = j/8 (dF_n/dT = -F_{n+1}), then
+// downward recursion F_{n-1} = (2T F_n + e^-T)/(2n-1) with e^-T = e^-T0 e^(T0-T) (8-term Taylor).
+// T >= 48: F_0 = sqrt(pi/T)/2, F_{n+1} = (2n+1) F_n / (2T) (the e^-T term is < 1e-20).
+template <int L>
+__device__ __forceinline__ void boys(double T, const double* __restrict__ tab, double (&F)[L + 1])
+{
+    if (T < BOYS_TMAX) {
+        const int j = __double2int_rn(T * 8.0);
+        const double dx = (double)j * 0.125 - T;             // T0 - T, |dx| <= 1/16
+        const double* row = tab + j * BOYS_ROW;
+        double f = __ldg(row + L + 7) * (1.0 / 5040.0);
+        f = fma(f, dx, __ldg(row + L + 6) * (1.0 / 720.0));
+        f = fma(f, dx, __ldg(row + L + 5) * (1.0 / 120.0));
+        f = fma(f, dx, __ldg(row + L + 4) * (1.0 / 24.0));
+        f = fma(f, dx, __ldg(row + L + 3) * (1.0 / 6.0));
+        f = fma(f, dx, __ldg(row + L + 2) * 0.5);
+        f = fma(f, dx, __ldg(row + L + 1));
+        f = fma(f, dx, __ldg(row + L));
+        F[L] = f;
+        if (L > 0) {
+            double e = 1.0 / 40320.0;
+            e = fma(e, dx, 1.0 / 5040.0);
+            e = fma(e, dx, 1.0 / 720.0);
+            e = fma(e, dx, 1.0 / 120.0);
+            e = fma(e, dx, 1.0 / 24.0);
+            e = fma(e, dx, 1.0 / 6.0);
+            e = fma(e, dx, 0.5);
+            e = fma(e, dx, 1.0);
+            e = fma(e, dx, 1.0);
+            e *= __ldg(row + 12);
+            const double t2 = 2.0 * T;
+#pragma unroll
+            for (int n = L; n >= 1; --n) F[n - 1] = fma(t2, F[n], e) * (1.0 / (2 * n - 1));
+        }
+    } else {
+        const double rs = rsqrt(T);
+        F[0] = 0.88622692545275801365 * rs;                  // sqrt(pi)/2
+        const double h = 0.5 * rs * rs;
+#pragma unroll
+        for (int n = 0; n < L; ++n) F[n + 1] = (2 * n + 1) * h * F[n];
+    }
+}
+
+// ---- Hermite Coulomb integrals R^0_{tuv}, |tuv| <= L, scaled by pref -----------------------------------
+template <int L>
+__device__ __forceinline__ void hermite_R(double pref, double alpha, double X, double Y, double Z,
+                                          const double* __restrict__ tab, double (&R0)[nherm(L)])
+{
+    double F[L + 1];
+    boys<L>(alpha * (X * X + Y * Y + Z * Z), tab, F);
+    double r[L + 1][nherm(L)];
+    double s = pref;
+#pragma unroll
+    for (int n = 0; n <= L; ++n) {
+        r[n][0] = s * F[n];
+        s *= -2.0 * alpha;
+    }
+#pragma unroll
+    for (int N = 1; N <= L; ++N)
+#pragma unroll
+        for (int n = 0; n <= L - N; ++n)
+#pragma unroll
+            for (int t = N; t >= 0; --t)
+#pragma unroll
+                for (int u = N - t; u >= 0; --u) {
+                    const int v = N - t - u;
+                    double val;
+                    if (t > 0) {
+                        val = X * r[n + 1][hidx(t - 1, u, v)];
+                        if (t > 1) val = fma((double)(t - 1), r[n + 1][hidx(t - 2, u, v)], val);
+                    } else if (u > 0) {
+                        val = Y * r[n + 1][hidx(t, u - 1, v)];
+                        if (u > 1) val = fma((double)(u - 1), r[n + 1][hidx(t, u - 2, v)], val);
+                    } else {
+                        val = Z * r[n + 1][hidx(t, u, v - 1)];
+                        if (v > 1) val = fma((double)(v - 1), r[n + 1][hidx(t, u, v - 2)], val);
+                    }
+                    r[n][hidx(t, u, v)] = val;
+                }
+#pragma unroll
+    for (int i = 0; i < nherm(L); ++i) R0[i] = r[0][i];
+}
+
+// One operator application: out[c][h] = X[c] * in[h] + g * in[h + e_c] for |h| <= LOUT (g = +1/2p for bra
+// functions, -1/2q for ket functions).  NC = 1 means "s function": plain copy of the first nherm(LOUT).
+template <int NC, int LOUT, int NBLK>
+__device__ __forceinline__ void apply_p(const double (&in)[NBLK][nherm(LOUT + (NC == 3 ? 1 : 0))],
+                                        const double* X, double g, double (&out)[NBLK * NC][nherm(LOUT)])
+{
+#pragma unroll
+    for (int b = 0; b < NBLK; ++b) {
+        if (NC == 1) {
+#pragma unroll
+            for (int h = 0; h < nherm(LOUT); ++h) out[b][h] = in[b][h];
+        } else {
+#pragma unroll
+            for (int c = 0; c < 3; ++c)
+#pragma unroll
+                for (int t = LOUT; t >= 0; --t)
+#pragma unroll
+                    for (int u = LOUT - t; u >= 0; --u)
+#pragma unroll
+                        for (int v = LOUT - t - u; v >= 0; --v)
+                            out[b * 3 + c][hidx(t, u, v)] =
+                                fma(X[c], in[b][hidx(t, u, v)], g * in[b][hidx_plus(t, u, v, c)]);
+        }
+    }
+}
+
+// Primitive pair view (registers or pointers already resolved by the caller).
+struct PrimPair {
+    double p, Px, Py, Pz, c, inv2p;
+    double XA[3];   // P - (first centre)
+    double XB[3];   // P - (second centre)
+};
+
+// Accumulate the primitive block into I[ia][ib][ic][id] (flattened, d fastest).
+// Order of operator application: d, c (ket; g = -1/2q), then b, a (bra; g = +1/2p).  The flattened block
+// index after the four stages is ((d*NC + c)*NB + b)*NA + a, so the caller reads I through eri_index().
+template <int LA, int LB, int LC, int LD>
+__device__ __forceinline__ void eri_prim_accum(const PrimPair& br, const PrimPair& kt,
+                                               const double* __restrict__ tab,
+                                               double (&I)[(2 * LA + 1) * (2 * LB + 1) * (2 * LC + 1) * (2 * LD + 1)])
+{
+    constexpr int L = LA + LB + LC + LD;
+    constexpr int NA = 2 * LA + 1, NB = 2 * LB + 1, NC = 2 * LC + 1, ND = 2 * LD + 1;
+    const double s = br.p + kt.p;
+    const double rs = rsqrt(s);
+    const double alpha = br.p * kt.p * (rs * rs);
+    const double pref = br.c * kt.c * rs;
+    double V0[1][nherm(L)];
+    hermite_R<L>(pref, alpha, br.Px - kt.Px, br.Py - kt.Py, br.Pz - kt.Pz, tab, V0[0]);
+    double VD[ND][nherm(L - LD)];
+    apply_p<ND, L - LD, 1>(V0, kt.XB, -kt.inv2p, VD);
+    double VC[ND * NC][nherm(L - LD - LC)];
+    apply_p<NC, L - LD - LC, ND>(VD, kt.XA, -kt.inv2p, VC);
+    // The operators above treat X_QC, X_QD as constants; two p functions on one pair with the SAME Cartesian
+    // component pick up the extra term of E_0^{11} = X_PA X_PB + 1/2p (x_P Lambda_1 = Lambda_2/2p + Lambda_0).
+    if constexpr (LC == 1 && LD == 1) {
+#pragma unroll
+        for (int c = 0; c < 3; ++c)
+#pragma unroll
+            for (int hh = 0; hh < nherm(L - LD - LC); ++hh)
+                VC[c * NC + c][hh] = fma(kt.inv2p, V0[0][hh], VC[c * NC + c][hh]);
+    }
+    double VB[ND * NC * NB][nherm(LA)];
+    apply_p<NB, LA, ND * NC>(VC, br.XB, br.inv2p, VB);
+    double VA[ND * NC * NB * NA][1];
+    apply_p<NA, 0, ND * NC * NB>(VB, br.XA, br.inv2p, VA);
+    if constexpr (LA == 1 && LB == 1) {
+#pragma unroll
+        for (int dc = 0; dc < ND * NC; ++dc)
+#pragma unroll
+            for (int a = 0; a < 3; ++a)
+                VA[(dc * NB + a) * NA + a][0] = fma(br.inv2p, VC[dc][0], VA[(dc * NB + a) * NA + a][0]);
+    }
+#pragma unroll
+    for (int i = 0; i < NA * NB * NC * ND; ++i) I[i] += VA[i][0];
+}
+
+// flattened index of component (a, b, c, d) in the block produced by eri_prim_accum
+template <int LA, int LB, int LC, int LD>
+__host__ __device__ constexpr int eri_index(int a, int b, int c, int d)
+{
+    return ((d * (2 * LC + 1) + c) * (2 * LB + 1) + b) * (2 * LA + 1) + a;
+}
+
+__device__ __forceinline__ PrimPair load_prim_aos(const double* __restrict__ row)
+{
+    PrimPair r;
+    r.p = __ldg(row + 0); r.Px = __ldg(row + 1); r.Py = __ldg(row + 2); r.Pz = __ldg(row + 3);
+    r.c = __ldg(row + 4); r.inv2p = __ldg(row + 5);
+    r.XA[0] = __ldg(row + 6); r.XA[1] = __ldg(row + 7); r.XA[2] = __ldg(row + 8);
+    r.XB[0] = __ldg(row + 9); r.XB[1] = __ldg(row + 10); r.XB[2] = __ldg(row + 11);
+    return r;
+}
+
+// SoA: element f of primitive k of ket q sits at prim[(k*PRIM_STRIDE + f)*n + q]
+__device__ __forceinline__ PrimPair load_prim_soa(const double* __restrict__ prim, int n, int k, int q)
+{
+    const double* b = prim + (size_t)k * PRIM_STRIDE * n + q;
+    PrimPair r;
+    r.p = __ldg(b); r.Px = __ldg(b + n); r.Py = __ldg(b + 2 * (size_t)n); r.Pz = __ldg(b + 3 * (size_t)n);
+    r.c = __ldg(b + 4 * (size_t)n); r.inv2p = __ldg(b + 5 * (size_t)n);
+    r.XA[0] = __ldg(b + 6 * (size_t)n); r.XA[1] = __ldg(b + 7 * (size_t)n); r.XA[2] = __ldg(b + 8 * (size_t)n);
+    r.XB[0] = __ldg(b + 9 * (size_t)n); r.XB[1] = __ldg(b + 10 * (size_t)n); r.XB[2] = __ldg(b + 11 * (size_t)n);
+    return r;
+}
+
+}  // namespace rttda

@@ -1,0 +1,320 @@
+// sigma = A X (steps a1-a5), field coupling (a6, eq. 16/19) and the RK4 propagator (a7, eq. 1, 12-15).
+#include <cmath>
+#include "common.cuh"
+
+namespace rttda {
+
+int ensure_ws(Handle* h, double** p, size_t* cur, size_t need)
+{
+    if (*cur >= need) return RTTDA_OK;
+    if (*p) cudaFree(*p);
+    *p = nullptr; *cur = 0;
+    cudaError_t e = cudaMalloc((void**)p, need * sizeof(double));
+    if (e != cudaSuccess) { set_error(std::string("workspace cudaMalloc: ") + cudaGetErrorString(e)); return RTTDA_ENOMEM; }
+    *cur = need;
+    return RTTDA_OK;
+}
+
+// sigma[v][ia] = deps[ia] * X[v][ia]   (the diagonal term of eq. 3; the GEMM then accumulates onto it)
+__global__ void diag_kernel(int ncsf, int nvec, const double* __restrict__ deps, const double* __restrict__ X,
+                            long long ldx, double* __restrict__ S, long long lds)
+{
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= (long long)ncsf * nvec) return;
+    const int v = (int)(i / ncsf), k = (int)(i % ncsf);
+    S[v * lds + k] = deps[k] * X[v * ldx + k];
+}
+
+int sigma_impl(Handle* h, int nvec, const double* X, long long ldx, double* sigma, long long lds,
+               cudaStream_t st)
+{
+    const size_t N = h->nao, no = h->nocc, nv = h->nvirt;
+    RT_TRY(ensure_ws(h, &h->wsY, &h->wsY_n, (size_t)nvec * no * N));
+    RT_TRY(ensure_ws(h, &h->wsT, &h->wsT_n, (size_t)nvec * N * N));
+    RT_TRY(ensure_ws(h, &h->wsF, &h->wsF_n, (size_t)nvec * N * N));
+    RT_CUDA(cudaEventRecord(h->ev[0], st));
+    // a1: Y_v = X_v C_v^T  [no][N];  T[mu][nu][v] = sum_j C_o[mu][j] Y_v[j][nu]
+    GemmDesc g{};
+    g.alpha = 1.0; g.beta = 0.0; g.batch = nvec;
+    g.M = (int)no; g.N = (int)N; g.K = (int)nv;
+    g.A = X; g.sam = nv; g.sak = 1; g.sabatch = ldx;
+    g.B = h->C_virt; g.sbk = 1; g.sbn = nv; g.sbbatch = 0;
+    g.C = h->wsY; g.scm = N; g.scn = 1; g.scbatch = no * N;
+    RT_TRY(gemm_f64(g, st));
+    g.M = (int)N; g.N = (int)N; g.K = (int)no;
+    g.A = h->C_occ; g.sam = no; g.sak = 1; g.sabatch = 0;
+    g.B = h->wsY; g.sbk = N; g.sbn = 1; g.sbbatch = no * N;
+    g.C = h->wsT; g.scm = N * nvec; g.scn = nvec; g.scbatch = 1;
+    RT_TRY(gemm_f64(g, st));
+    RT_CUDA(cudaEventRecord(h->ev[1], st));
+    // a3-a4: F = 2 J[T] - cx K[T], interleaved layout, chunks of densities per ERI pass
+    RT_CUDA(cudaMemsetAsync(h->wsF, 0, (size_t)nvec * N * N * sizeof(double), st));
+    const int chunk = jk_nvec_chunk();
+    for (int v0 = 0; v0 < nvec; v0 += chunk)
+        RT_TRY(jk_build(h, nvec, v0, std::min(chunk, nvec - v0), h->wsT, h->wsF, st));
+    RT_CUDA(cudaEventRecord(h->ev[2], st));
+    // a5: Z_v = C_o^T F_v [no][N];  sigma_v = deps o X_v + Z_v C_v
+    g.M = (int)no; g.N = (int)N; g.K = (int)N; g.batch = nvec;
+    g.A = h->C_occ; g.sam = 1; g.sak = no; g.sabatch = 0;
+    g.B = h->wsF; g.sbk = N * nvec; g.sbn = nvec; g.sbbatch = 1;
+    g.C = h->wsY; g.scm = N; g.scn = 1; g.scbatch = no * N;
+    RT_TRY(gemm_f64(g, st));
+    const long long tot = (long long)h->ncsf * nvec;
+    diag_kernel<<<(unsigned)((tot + 255) / 256), 256, 0, st>>>(h->ncsf, nvec, h->deps, X, ldx, sigma, lds);
+    RT_CUDA(cudaGetLastError());
+    g.M = (int)no; g.N = (int)nv; g.K = (int)N; g.beta = 1.0;
+    g.A = h->wsY; g.sam = N; g.sak = 1; g.sabatch = no * N;
+    g.B = h->C_virt; g.sbk = nv; g.sbn = 1; g.sbbatch = 0;
+    g.C = sigma; g.scm = nv; g.scn = 1; g.scbatch = lds;
+    RT_TRY(gemm_f64(g, st));
+    RT_CUDA(cudaEventRecord(h->ev[3], st));
+    h->ev_valid = true;
+    h->kernel_launches += 5;
+    return RTTDA_OK;
+}
+
+// ---------------------------------------------------------------------------------------------- field
+static double field_value(const rttda_field_t& f, double t)
+{
+    switch (f.type) {
+        case RTTDA_CW: return f.E0 * std::sin(f.omega * t);
+        case RTTDA_TL: {
+            const double s = t - f.t0;
+            return f.E0 * std::exp(-s * s / (2.0 * f.sigma * f.sigma)) * std::sin(f.omega * s);
+        }
+        case RTTDA_CHIRP: {
+            const double s = t - f.t0;
+            return f.E0 * std::exp(-s * s / (2.0 * f.sigma * f.sigma)) * std::sin((f.omega + 0.5 * f.beta * s) * s);
+        }
+        case RTTDA_SIN2: {
+            if (t < 0.0 || t > f.T_env) return 0.0;
+            const double e = std::sin(M_PI * t / f.T_env);
+            return f.E0 * e * e * std::sin(f.omega * t);
+        }
+        default: return 0.0;
+    }
+}
+
+// out[i] = d0 in0[i] + d1 in1[i] + d2 in2[i]   (D_d = sum_k d_k D^k)
+__global__ void combine3_kernel(long long n, const double* __restrict__ in, double d0, double d1, double d2,
+                                double* __restrict__ out)
+{
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) out[i] = d0 * in[i] + d1 * in[n + i] + d2 * in[2 * n + i];
+}
+
+struct FieldArgs {
+    double E[8];        // E(t) (or kick area) per trajectory
+    double D00[8];      // D_00 along the trajectory's polarisation
+};
+
+// One block per (trajectory, plane): element 0 and the elementwise part of E * M y (eq. 19a-c):
+//   hy_0  (+)= E (D_00 y_0 + sqrt2 sum_ia D_ov[ia] Y[ia])
+//   hy_ia  += E (sqrt2 D_ov[ia] y_0 + D_00 Y[ia])
+// `assign0`: hy_0 is assigned (sigma never writes element 0), singles are always accumulated.
+__global__ void __launch_bounds__(1024)
+field_elem_kernel(int ncsf, const double* __restrict__ ys, double* __restrict__ hy,
+                  const double* __restrict__ Dov /* [ntraj][ncsf] */, FieldArgs fa)
+{
+    const int b = blockIdx.x, traj = b >> 1;
+    const long long n1 = (long long)ncsf + 1;
+    const double* y = ys + b * n1;
+    double* h = hy + b * n1;
+    const double* d = Dov + (long long)traj * ncsf;
+    const double E = fa.E[traj], D00 = fa.D00[traj], y0 = y[0];
+    const double s2 = 1.41421356237309504880;
+    double dot = 0.0;
+    if (E != 0.0) {
+        for (int i = threadIdx.x; i < ncsf; i += blockDim.x) {
+            const double Y = y[1 + i], dv = d[i];
+            dot = fma(dv, Y, dot);
+            h[1 + i] += E * fma(s2 * dv, y0, D00 * Y);
+        }
+    }
+    __shared__ double red[32];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) dot += __shfl_xor_sync(0xffffffffu, dot, o);
+    if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = dot;
+    __syncthreads();
+    if (threadIdx.x < 32) {
+        double v = threadIdx.x < (blockDim.x >> 5) ? red[threadIdx.x] : 0.0;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+        if (threadIdx.x == 0) h[0] = E * fma(D00, y0, s2 * v);
+    }
+}
+
+// hy (+)= E_traj * M_d ys for all trajectories/planes.  Singles of hy must already hold A ys (or zeros).
+static int apply_field(Handle* h, int ntraj, const double* ys, double* hy, const double* Dd_oo,
+                       const double* Dd_vv, const double* Dd_ov, const FieldArgs& fa, cudaStream_t st)
+{
+    const size_t no = h->nocc, nv = h->nvirt, n1 = (size_t)h->ncsf + 1;
+    field_elem_kernel<<<2 * ntraj, 1024, 0, st>>>(h->ncsf, ys, hy, Dd_ov, fa);
+    RT_CUDA(cudaGetLastError());
+    h->kernel_launches++;
+    for (int t = 0; t < ntraj; ++t) {
+        if (fa.E[t] == 0.0) continue;
+        GemmDesc g{};
+        g.batch = 2; g.beta = 1.0;
+        // + E Y D_vv
+        g.alpha = fa.E[t];
+        g.M = (int)no; g.N = (int)nv; g.K = (int)nv;
+        g.A = ys + (size_t)t * 2 * n1 + 1; g.sam = nv; g.sak = 1; g.sabatch = n1;
+        g.B = Dd_vv + (size_t)t * nv * nv; g.sbk = nv; g.sbn = 1; g.sbbatch = 0;
+        g.C = hy + (size_t)t * 2 * n1 + 1; g.scm = nv; g.scn = 1; g.scbatch = n1;
+        RT_TRY(gemm_f64(g, st));
+        // - E D_oo Y
+        g.alpha = -fa.E[t];
+        g.M = (int)no; g.N = (int)nv; g.K = (int)no;
+        g.A = Dd_oo + (size_t)t * no * no; g.sam = no; g.sak = 1; g.sabatch = 0;
+        g.B = ys + (size_t)t * 2 * n1 + 1; g.sbk = nv; g.sbn = 1; g.sbbatch = n1;
+        RT_TRY(gemm_f64(g, st));
+        h->kernel_launches += 2;
+    }
+    return RTTDA_OK;
+}
+
+// ---------------------------------------------------------------------------------------------- RK4
+// k = -i H ys: (k_q, k_p) = (hy_p, -hy_q)  (eq. 14-15).  One fused pass per stage:
+//   ksum  = (first ? 0 : ksum) + w k
+//   ys    = y + c k                      (next stage input)       if !last
+//   y     = y + (dt/6) ksum                                       if last
+__global__ void rk4_stage_kernel(long long n1, int ntraj, const double* __restrict__ hy, double* __restrict__ y,
+                                 double* __restrict__ ys, double* __restrict__ ksum, double w, double c,
+                                 double dt6, int first, int last)
+{
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n1 * ntraj) return;
+    const long long t = i / n1, e = i % n1;
+    const long long iq = (2 * t) * n1 + e, ip = (2 * t + 1) * n1 + e;
+    const double kq = hy[ip], kp = -hy[iq];
+    double sq = w * kq, sp = w * kp;
+    if (!first) { sq += ksum[iq]; sp += ksum[ip]; }
+    if (last) {
+        y[iq] = fma(dt6, sq, y[iq]);
+        y[ip] = fma(dt6, sp, y[ip]);
+    } else {
+        ksum[iq] = sq; ksum[ip] = sp;
+        ys[iq] = fma(c, kq, y[iq]);
+        ys[ip] = fma(c, kp, y[ip]);
+    }
+}
+
+// delta kick (R8): y <- y - i kappa M y, hy holds kappa M y:  q += hy_p, p -= hy_q
+__global__ void kick_kernel(long long n1, int ntraj, const double* __restrict__ hy, double* __restrict__ y,
+                            FieldArgs fa)
+{
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n1 * ntraj) return;
+    const long long t = i / n1, e = i % n1;
+    if (fa.E[t] == 0.0) return;
+    const long long iq = (2 * t) * n1 + e, ip = (2 * t + 1) * n1 + e;
+    y[iq] += hy[ip];
+    y[ip] -= hy[iq];
+}
+
+// log[traj] = (|y|^2, Re <yref|y>, Im <yref|y>)   (eq. 20)
+__global__ void __launch_bounds__(1024)
+observe_kernel(long long n1, const double* __restrict__ y, const double* __restrict__ yref, double* __restrict__ out)
+{
+    const int t = blockIdx.x;
+    const double *q = y + 2 * t * n1, *p = q + n1, *qr = yref + 2 * t * n1, *pr = qr + n1;
+    double a = 0, b = 0, c = 0;
+    for (long long i = threadIdx.x; i < n1; i += blockDim.x) {
+        const double qi = q[i], pi = p[i], qri = qr[i], pri = pr[i];
+        a = fma(qi, qi, fma(pi, pi, a));
+        b = fma(qri, qi, fma(pri, pi, b));
+        c = fma(qri, pi, fma(-pri, qi, c));
+    }
+    __shared__ double red[3][32];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        a += __shfl_xor_sync(0xffffffffu, a, o);
+        b += __shfl_xor_sync(0xffffffffu, b, o);
+        c += __shfl_xor_sync(0xffffffffu, c, o);
+    }
+    if ((threadIdx.x & 31) == 0) { red[0][threadIdx.x >> 5] = a; red[1][threadIdx.x >> 5] = b; red[2][threadIdx.x >> 5] = c; }
+    __syncthreads();
+    if (threadIdx.x < 32) {
+        const int nw = blockDim.x >> 5;
+        a = threadIdx.x < nw ? red[0][threadIdx.x] : 0.0;
+        b = threadIdx.x < nw ? red[1][threadIdx.x] : 0.0;
+        c = threadIdx.x < nw ? red[2][threadIdx.x] : 0.0;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            a += __shfl_xor_sync(0xffffffffu, a, o);
+            b += __shfl_xor_sync(0xffffffffu, b, o);
+            c += __shfl_xor_sync(0xffffffffu, c, o);
+        }
+        if (threadIdx.x == 0) { out[3 * t] = a; out[3 * t + 1] = b; out[3 * t + 2] = c; }
+    }
+}
+
+int propagate_impl(Handle* h, int ntraj, double* y, const rttda_field_t* fields, double t_start, double dt,
+                   int nsteps, double* log, cudaStream_t st)
+{
+    const size_t no = h->nocc, nv = h->nvirt, ncsf = h->ncsf, n1 = ncsf + 1;
+    const size_t nstate = (size_t)ntraj * 2 * n1;
+    const size_t need = 4 * nstate + (size_t)ntraj * (no * no + nv * nv + no * nv);
+    RT_TRY(ensure_ws(h, &h->prop_ws, &h->prop_ws_n, need));
+    double* ys = h->prop_ws;
+    double* hy = ys + nstate;
+    double* ksum = hy + nstate;
+    double* yref = ksum + nstate;
+    double* Dd_oo = yref + nstate;
+    double* Dd_vv = Dd_oo + (size_t)ntraj * no * no;
+    double* Dd_ov = Dd_vv + (size_t)ntraj * nv * nv;
+    FieldArgs fa{};
+    for (int t = 0; t < ntraj; ++t) {
+        const double* d = fields[t].dir;
+        fa.D00[t] = d[0] * h->D_00[0] + d[1] * h->D_00[1] + d[2] * h->D_00[2];
+        const long long a = no * no, b = nv * nv, c = no * nv;
+        combine3_kernel<<<(unsigned)((a + 255) / 256), 256, 0, st>>>(a, h->D_oo, d[0], d[1], d[2], Dd_oo + t * a);
+        combine3_kernel<<<(unsigned)((b + 255) / 256), 256, 0, st>>>(b, h->D_vv, d[0], d[1], d[2], Dd_vv + t * b);
+        combine3_kernel<<<(unsigned)((c + 255) / 256), 256, 0, st>>>(c, h->D_ov, d[0], d[1], d[2], Dd_ov + t * c);
+        h->kernel_launches += 3;
+    }
+    RT_CUDA(cudaGetLastError());
+    const unsigned eg = (unsigned)((n1 * ntraj + 255) / 256);
+    // delta kick at t_start (R8)
+    bool any_kick = false;
+    for (int t = 0; t < ntraj; ++t) {
+        fa.E[t] = fields[t].type == RTTDA_DELTA ? fields[t].E0 : 0.0;
+        any_kick |= fa.E[t] != 0.0;
+    }
+    if (any_kick) {
+        RT_CUDA(cudaMemsetAsync(hy, 0, nstate * sizeof(double), st));
+        RT_TRY(apply_field(h, ntraj, y, hy, Dd_oo, Dd_vv, Dd_ov, fa, st));
+        kick_kernel<<<eg, 256, 0, st>>>((long long)n1, ntraj, hy, y, fa);
+        RT_CUDA(cudaGetLastError());
+        h->kernel_launches++;
+    }
+    RT_CUDA(cudaMemcpyAsync(yref, y, nstate * sizeof(double), cudaMemcpyDeviceToDevice, st));
+
+    const double ts_off[4] = {0.0, 0.5, 0.5, 1.0};
+    const double wgt[4] = {1.0, 2.0, 2.0, 1.0};
+    const double cnext[4] = {0.5 * dt, 0.5 * dt, dt, 0.0};
+    for (int n = 0; n < nsteps; ++n) {
+        const double t0 = t_start + n * dt;
+        for (int s = 0; s < 4; ++s) {
+            const double* in = (s == 0) ? y : ys;
+            // hy singles = A in (both planes of every trajectory in one batched sigma)
+            RT_TRY(sigma_impl(h, 2 * ntraj, in + 1, (long long)n1, hy + 1, (long long)n1, st));
+            const double ts = t0 + ts_off[s] * dt;
+            for (int t = 0; t < ntraj; ++t) fa.E[t] = field_value(fields[t], ts);
+            RT_TRY(apply_field(h, ntraj, in, hy, Dd_oo, Dd_vv, Dd_ov, fa, st));
+            rk4_stage_kernel<<<eg, 256, 0, st>>>((long long)n1, ntraj, hy, y, ys, ksum, wgt[s], cnext[s],
+                                                 dt / 6.0, s == 0, s == 3);
+            RT_CUDA(cudaGetLastError());
+            h->kernel_launches++;
+        }
+        if (log) {
+            observe_kernel<<<ntraj, 1024, 0, st>>>((long long)n1, y, yref, log + (size_t)n * ntraj * 3);
+            RT_CUDA(cudaGetLastError());
+            h->kernel_launches++;
+        }
+    }
+    return RTTDA_OK;
+}
+
+}  // namespace rttda

@@ -1,0 +1,522 @@
+// Host-side setup of a handle (DESIGN.md step a0): shell normalisation (R11), primitive-pair tables,
+// Schwarz bounds (R14, computed on the device), class/bound sorting, a-lists and work lists, one-electron
+// integrals (overlap for callers, dipoles for eq. 19), Boys table.
+#include <algorithm>
+#include <chrono>
+#include <cmath>
+#include <cstring>
+#include <map>
+#include <numeric>
+#include "common.cuh"
+
+namespace rttda {
+
+// ---------------------------------------------------------------------------------------------- Boys table
+// F_n(T0), n = 0..11, by the series at n = 11 + downward recursion (T0 <= 48), in long double.
+void boys_table_host(std::vector<double>& tab)
+{
+    tab.assign((size_t)BOYS_NROW * BOYS_ROW, 0.0);
+    for (int j = 0; j < BOYS_NROW; ++j) {
+        const long double T = (long double)j / 8.0L;
+        const int nmax = 11;
+        long double term = 1.0L / (2 * nmax + 1), sum = term;
+        for (int k = 1; k < 4000; ++k) {
+            term *= 2.0L * T / (2 * nmax + 2 * k + 1);
+            sum += term;
+            if (term < 1e-21L * sum) break;
+        }
+        const long double emt = expl(-T);
+        long double f = emt * sum;
+        tab[(size_t)j * BOYS_ROW + nmax] = (double)f;
+        for (int n = nmax; n >= 1; --n) {
+            f = (2.0L * T * f + emt) / (2 * n - 1);
+            tab[(size_t)j * BOYS_ROW + n - 1] = (double)f;
+        }
+        tab[(size_t)j * BOYS_ROW + 12] = (double)emt;
+    }
+}
+
+// ---------------------------------------------------------------------------------------------- basis
+struct HostBasis {
+    int nshells = 0, nao = 0;
+    std::vector<int> l, np, off, ao, center;
+    std::vector<double> ex, cf;          // cf: final coefficient of the bare primitive
+    std::vector<double> xyz;             // [ncenters][3]
+};
+
+static int load_basis(const rttda_basis_t* b, HostBasis& H)
+{
+    RT_CHECK(b && b->centers && b->shells && b->exps && b->coefs, "basis: NULL pointer");
+    RT_CHECK(b->nshells > 0 && b->ncenters > 0, "basis: empty");
+    H.nshells = b->nshells;
+    H.xyz.assign(b->centers, b->centers + 3 * (size_t)b->ncenters);
+    int ao = 0;
+    for (int s = 0; s < b->nshells; ++s) {
+        const rttda_shell_t& sh = b->shells[s];
+        RT_CHECK(sh.l == 0 || sh.l == 1, "basis: only s and p shells are supported");
+        RT_CHECK(sh.nprim >= 1 && sh.nprim <= RTTDA_MAX_NPRIM, "basis: nprim out of range");
+        RT_CHECK(sh.center >= 0 && sh.center < b->ncenters, "basis: bad centre index");
+        H.l.push_back(sh.l); H.np.push_back(sh.nprim); H.off.push_back((int)H.ex.size());
+        H.center.push_back(sh.center); H.ao.push_back(ao);
+        ao += 2 * sh.l + 1;
+        // coefficient on the normalised primitive -> coefficient on the bare primitive
+        std::vector<double> c(sh.nprim);
+        for (int k = 0; k < sh.nprim; ++k) {
+            const double a = b->exps[sh.prim_off + k];
+            RT_CHECK(a > 0.0, "basis: non-positive exponent");
+            double nrm = std::pow(2.0 * a / M_PI, 0.75);
+            if (sh.l == 1) nrm *= 2.0 * std::sqrt(a);
+            c[k] = b->coefs[sh.prim_off + k] * nrm;
+            H.ex.push_back(a);
+        }
+        // self overlap of the contracted function: s: sum c c (pi/p)^1.5 ; p: sum c c (pi/p)^1.5 / (2p)
+        double self = 0.0;
+        for (int k = 0; k < sh.nprim; ++k)
+            for (int m = 0; m < sh.nprim; ++m) {
+                const double p = b->exps[sh.prim_off + k] + b->exps[sh.prim_off + m];
+                double t = c[k] * c[m] * std::pow(M_PI / p, 1.5);
+                if (sh.l == 1) t /= 2.0 * p;
+                self += t;
+            }
+        RT_CHECK(self > 0.0, "basis: contracted function has zero norm");
+        for (int k = 0; k < sh.nprim; ++k) H.cf.push_back(c[k] / std::sqrt(self));
+    }
+    H.nao = ao;
+    return RTTDA_OK;
+}
+
+// One-electron block of a shell pair: S[na*nb] and D[3][na*nb] (origin 0).
+static void pair_1e(const HostBasis& H, int sa, int sb, double* S, double* D)
+{
+    const int la = H.l[sa], lb = H.l[sb], na = 2 * la + 1, nb = 2 * lb + 1;
+    const double* A = &H.xyz[3 * H.center[sa]];
+    const double* B = &H.xyz[3 * H.center[sb]];
+    std::fill(S, S + na * nb, 0.0);
+    std::fill(D, D + 3 * na * nb, 0.0);
+    const double ab2 = (A[0] - B[0]) * (A[0] - B[0]) + (A[1] - B[1]) * (A[1] - B[1]) + (A[2] - B[2]) * (A[2] - B[2]);
+    for (int ka = 0; ka < H.np[sa]; ++ka)
+        for (int kb = 0; kb < H.np[sb]; ++kb) {
+            const double a = H.ex[H.off[sa] + ka], b = H.ex[H.off[sb] + kb], p = a + b;
+            const double base = H.cf[H.off[sa] + ka] * H.cf[H.off[sb] + kb] * std::pow(M_PI / p, 1.5) *
+                                std::exp(-a * b / p * ab2);
+            double P[3], e0[3][2][2], e1[3][2][2];   // [axis][i][j]: Hermite E_0 and E_1 (K factored out)
+            for (int x = 0; x < 3; ++x) {
+                P[x] = (a * A[x] + b * B[x]) / p;
+                const double xa = P[x] - A[x], xb = P[x] - B[x], h = 0.5 / p;
+                e0[x][0][0] = 1.0;            e1[x][0][0] = 0.0;
+                e0[x][1][0] = xa;             e1[x][1][0] = h;
+                e0[x][0][1] = xb;             e1[x][0][1] = h;
+                e0[x][1][1] = xa * xb + h;    e1[x][1][1] = (xa + xb) * h;
+            }
+            for (int ca = 0; ca < na; ++ca)
+                for (int cb = 0; cb < nb; ++cb) {
+                    int pa[3] = {0, 0, 0}, pb[3] = {0, 0, 0};
+                    if (la) pa[ca] = 1;
+                    if (lb) pb[cb] = 1;
+                    const double f0 = e0[0][pa[0]][pb[0]], f1 = e0[1][pa[1]][pb[1]], f2 = e0[2][pa[2]][pb[2]];
+                    S[ca * nb + cb] += base * f0 * f1 * f2;
+                    const double m0 = e1[0][pa[0]][pb[0]] + P[0] * f0, m1 = e1[1][pa[1]][pb[1]] + P[1] * f1,
+                                 m2 = e1[2][pa[2]][pb[2]] + P[2] * f2;
+                    D[0 * na * nb + ca * nb + cb] += base * m0 * f1 * f2;
+                    D[1 * na * nb + ca * nb + cb] += base * f0 * m1 * f2;
+                    D[2 * na * nb + ca * nb + cb] += base * f0 * f1 * m2;
+                }
+        }
+}
+
+static void one_electron_host(const HostBasis& H, double* S, double* D)
+{
+    const size_t N = H.nao;
+    for (int sa = 0; sa < H.nshells; ++sa)
+        for (int sb = 0; sb < H.nshells; ++sb) {
+            double s[9], d[27];
+            pair_1e(H, sa, sb, s, d);
+            const int na = 2 * H.l[sa] + 1, nb = 2 * H.l[sb] + 1;
+            for (int ca = 0; ca < na; ++ca)
+                for (int cb = 0; cb < nb; ++cb) {
+                    const size_t idx = (size_t)(H.ao[sa] + ca) * N + H.ao[sb] + cb;
+                    if (S) S[idx] = s[ca * nb + cb];
+                    if (D)
+                        for (int x = 0; x < 3; ++x) D[x * N * N + idx] = d[x * na * nb + ca * nb + cb];
+                }
+        }
+}
+
+// Primitive-pair rows of the ordered shell pair (first, second).
+static void prim_rows(const HostBasis& H, int s1, int s2, std::vector<double>& rows)
+{
+    const double* A = &H.xyz[3 * H.center[s1]];
+    const double* B = &H.xyz[3 * H.center[s2]];
+    const double ab2 = (A[0] - B[0]) * (A[0] - B[0]) + (A[1] - B[1]) * (A[1] - B[1]) + (A[2] - B[2]) * (A[2] - B[2]);
+    const double c0 = std::sqrt(2.0) * std::pow(M_PI, 1.25);
+    for (int k1 = 0; k1 < H.np[s1]; ++k1)
+        for (int k2 = 0; k2 < H.np[s2]; ++k2) {
+            const double a = H.ex[H.off[s1] + k1], b = H.ex[H.off[s2] + k2], p = a + b;
+            double r[PRIM_STRIDE];
+            r[0] = p;
+            for (int x = 0; x < 3; ++x) {
+                r[1 + x] = (a * A[x] + b * B[x]) / p;
+                r[6 + x] = r[1 + x] - A[x];
+                r[9 + x] = r[1 + x] - B[x];
+            }
+            r[4] = c0 / p * H.cf[H.off[s1] + k1] * H.cf[H.off[s2] + k2] * std::exp(-a * b / p * ab2);
+            r[5] = 0.5 / p;
+            rows.insert(rows.end(), r, r + PRIM_STRIDE);
+        }
+}
+
+struct Pair {
+    int s1, s2;          // first (higher l, or larger index at equal l), second
+    int pc, sub, np;     // pair class, contraction sub-class, primitive pairs
+    int row;             // first row in the per-class candidate prim table
+    double Q;
+    int pos;             // position in its ket class after sorting
+};
+
+template <class T>
+static int upload(Handle* h, const std::vector<T>& v, const T** out)
+{
+    void* d = nullptr;
+    const size_t bytes = std::max<size_t>(v.size(), 1) * sizeof(T);
+    RT_CUDA(cudaMalloc(&d, bytes));
+    h->dev_allocs.push_back(d);
+    if (!v.empty()) RT_CUDA(cudaMemcpy(d, v.data(), v.size() * sizeof(T), cudaMemcpyHostToDevice));
+    *out = (const T*)d;
+    return RTTDA_OK;
+}
+
+static int np_to_sub(int np) { return np == 1 ? 0 : (np == 3 ? 1 : 2); }
+
+// Flop model of one primitive quartet of total angular momentum L, bra/ket split irrelevant at this
+// granularity: geometry + prefactor, Boys, R recursion, operator stages.
+static double flops_prim(int la, int lb, int lc, int ld)
+{
+    const int L = la + lb + lc + ld;
+    auto nh = [](int n) { return (n + 1) * (n + 2) * (n + 3) / 6; };
+    double fma = 0.0, other = 0.0;
+    other += 16;                       // P-Q, |PQ|^2, p+q, rsqrt (counted as 4), alpha, prefactor
+    fma += 8 + (L > 0 ? 9 + L : 0);    // Boys Taylor (+ exp Taylor + downward recursion)
+    other += L + 1;                    // (-2 alpha)^n scaling
+    for (int N = 1; N <= L; ++N) fma += (double)(L - N + 1) * (nh(N) - nh(N - 1)) * 1.5;
+    int ord = L, blk = 1;
+    const int ls[4] = {ld, lc, lb, la};
+    for (int s = 0; s < 4; ++s)
+        if (ls[s]) { ord -= 1; fma += 2.0 * 3 * blk * nh(ord) * 0.75; blk *= 3; }
+    return 2.0 * fma + other;
+}
+
+int create_impl(Handle* h, const rttda_basis_t* basis, const double* C_occ, const double* C_virt,
+                const double* eps, cudaStream_t st)
+{
+    auto t0 = std::chrono::steady_clock::now();
+    HostBasis H;
+    RT_TRY(load_basis(basis, H));
+    RT_CHECK(H.nao == h->nao, "nao does not match the shell table");
+    h->nshells = H.nshells;
+    const size_t N = h->nao;
+
+    // ---- Boys table
+    std::vector<double> boys;
+    boys_table_host(boys);
+    RT_TRY(upload(h, boys, &h->tabs.boys));
+
+    // ---- candidate pairs and their primitive rows (canonical orientation), per pair class
+    std::vector<Pair> pairs;
+    std::vector<double> rows[3];
+    std::vector<int> cand_np[3], cand_off[3], cand_id[3];
+    long long npairs_total = 0;
+    for (int i = 0; i < H.nshells; ++i)
+        for (int j = 0; j <= i; ++j) {
+            ++npairs_total;
+            int s1 = i, s2 = j;
+            if (H.l[s2] > H.l[s1]) std::swap(s1, s2);
+            Pair P;
+            P.s1 = s1; P.s2 = s2; P.pc = H.l[s1] + H.l[s2]; P.np = H.np[s1] * H.np[s2];
+            RT_CHECK(P.np == 1 || P.np == 3 || P.np == 9 || P.np == 2 || P.np == 4 || P.np == 6,
+                     "unsupported contraction depth");
+            RT_CHECK(P.np == 1 || P.np == 3 || P.np == 9,
+                     "contraction depths other than 1 and 3 primitives per shell are not supported yet");
+            P.sub = np_to_sub(P.np);
+            const size_t before = rows[P.pc].size();
+            prim_rows(H, s1, s2, rows[P.pc]);
+            double cmax = 0.0;
+            for (size_t r = before; r < rows[P.pc].size(); r += PRIM_STRIDE) cmax = std::max(cmax, std::fabs(rows[P.pc][r + 4]));
+            if (cmax < 1e-30) {                 // Gaussian product vanishes: contributes < 1e-30 everywhere
+                rows[P.pc].resize(before);
+                continue;
+            }
+            P.row = (int)(before / PRIM_STRIDE);
+            P.Q = 0.0; P.pos = -1;
+            cand_np[P.pc].push_back(P.np);
+            cand_off[P.pc].push_back(P.row);
+            cand_id[P.pc].push_back((int)pairs.size());
+            pairs.push_back(P);
+        }
+
+    // ---- Schwarz bounds on the device
+    for (int pc = 0; pc < 3; ++pc) {
+        const int n = (int)cand_np[pc].size();
+        if (!n) continue;
+        int *d_np = nullptr, *d_off = nullptr;
+        double *d_prim = nullptr, *d_Q = nullptr;
+        RT_CUDA(cudaMalloc(&d_np, n * sizeof(int)));
+        RT_CUDA(cudaMalloc(&d_off, n * sizeof(int)));
+        RT_CUDA(cudaMalloc(&d_prim, rows[pc].size() * sizeof(double)));
+        RT_CUDA(cudaMalloc(&d_Q, n * sizeof(double)));
+        RT_CUDA(cudaMemcpyAsync(d_np, cand_np[pc].data(), n * sizeof(int), cudaMemcpyHostToDevice, st));
+        RT_CUDA(cudaMemcpyAsync(d_off, cand_off[pc].data(), n * sizeof(int), cudaMemcpyHostToDevice, st));
+        RT_CUDA(cudaMemcpyAsync(d_prim, rows[pc].data(), rows[pc].size() * sizeof(double), cudaMemcpyHostToDevice, st));
+        RT_TRY(schwarz_device(pc, n, d_np, d_off, d_prim, h->tabs.boys, d_Q, st));
+        h->kernel_launches++;
+        std::vector<double> Q(n);
+        RT_CUDA(cudaMemcpyAsync(Q.data(), d_Q, n * sizeof(double), cudaMemcpyDeviceToHost, st));
+        RT_CUDA(cudaStreamSynchronize(st));
+        for (int k = 0; k < n; ++k) pairs[cand_id[pc][k]].Q = Q[k];
+        cudaFree(d_np); cudaFree(d_off); cudaFree(d_prim); cudaFree(d_Q);
+    }
+    double Qmax = 0.0;
+    for (const Pair& P : pairs) Qmax = std::max(Qmax, P.Q);
+    RT_CHECK(Qmax > 0.0 && std::isfinite(Qmax), "Schwarz bounds are not finite/positive");
+    const double tau = h->tau;
+
+    // ---- keep, classify, sort by bound
+    std::vector<int> cls[NKETCLASS];
+    for (int k = 0; k < (int)pairs.size(); ++k) {
+        const Pair& P = pairs[k];
+        if (!(P.Q > 0.0) || P.Q * Qmax < tau) continue;
+        cls[P.pc * NSUB + P.sub].push_back(k);
+    }
+    long long nkept = 0;
+    std::vector<std::vector<double>> hQ(NKETCLASS);
+    for (int kc = 0; kc < NKETCLASS; ++kc) {
+        std::vector<int>& v = cls[kc];
+        std::sort(v.begin(), v.end(), [&](int x, int y) {
+            if (pairs[x].Q != pairs[y].Q) return pairs[x].Q > pairs[y].Q;
+            return x < y;
+        });
+        const int n = (int)v.size(), np = sub_to_np(kc % NSUB), pc = kc / NSUB;
+        nkept += n;
+        std::vector<double> soa((size_t)np * PRIM_STRIDE * std::max(n, 1), 0.0);
+        std::vector<int> aoc(std::max(n, 1), 0), aod(std::max(n, 1), 0), same(std::max(n, 1), 0);
+        hQ[kc].assign(std::max(n, 1), 0.0);
+        for (int q = 0; q < n; ++q) {
+            Pair& P = pairs[v[q]];
+            P.pos = q;
+            hQ[kc][q] = P.Q;
+            aoc[q] = H.ao[P.s1]; aod[q] = H.ao[P.s2]; same[q] = (P.s1 == P.s2);
+            for (int k = 0; k < np; ++k)
+                for (int f = 0; f < PRIM_STRIDE; ++f)
+                    soa[((size_t)k * PRIM_STRIDE + f) * n + q] = rows[pc][(size_t)(P.row + k) * PRIM_STRIDE + f];
+        }
+        KetClass& K = h->tabs.kets[kc];
+        K.n = n; K.np = np;
+        RT_TRY(upload(h, hQ[kc], &K.Q));
+        RT_TRY(upload(h, aoc, &K.ao_c));
+        RT_TRY(upload(h, aod, &K.ao_d));
+        RT_TRY(upload(h, same, &K.same));
+        RT_TRY(upload(h, soa, &K.prim));
+    }
+
+    // ---- ordered bra records grouped into a-lists keyed by (shell a, l_b, sub)
+    struct Rec { int a, b, pair, canonical; };
+    std::map<std::tuple<int, int, int>, std::vector<Rec>> groups;
+    for (int kc = 0; kc < NKETCLASS; ++kc)
+        for (int k : cls[kc]) {
+            const Pair& P = pairs[k];
+            groups[{P.s1, H.l[P.s2], P.sub}].push_back({P.s1, P.s2, k, 1});
+            if (P.s1 != P.s2) groups[{P.s2, H.l[P.s1], P.sub}].push_back({P.s2, P.s1, k, 0});
+        }
+    std::vector<BraRec> recs;
+    std::vector<AList> alists;
+    std::vector<double> bra_rows;
+    std::vector<int> alist_la, alist_lb;
+    for (auto& g : groups) {
+        std::vector<Rec>& v = g.second;
+        std::sort(v.begin(), v.end(), [&](const Rec& x, const Rec& y) { return pairs[x.pair].pos < pairs[y.pair].pos; });
+        AList al;
+        al.ao_a = H.ao[std::get<0>(g.first)];
+        al.rec_begin = (int)recs.size();
+        al.ketclass = pairs[v[0].pair].pc * NSUB + pairs[v[0].pair].sub;
+        al.np = pairs[v[0].pair].np;
+        al.Qmax = pairs[v[0].pair].Q;
+        for (const Rec& r : v) {
+            const Pair& P = pairs[r.pair];
+            BraRec br;
+            br.Q = P.Q; br.ao_b = H.ao[r.b]; br.pos = P.pos;
+            br.flags = (r.canonical ? 1 : 0) | (r.a == r.b ? 2 : 0);
+            br.prim_off = (int)(bra_rows.size() / PRIM_STRIDE);
+            prim_rows(H, r.a, r.b, bra_rows);
+            recs.push_back(br);
+        }
+        al.rec_end = (int)recs.size();
+        alists.push_back(al);
+        alist_la.push_back(H.l[std::get<0>(g.first)]);
+        alist_lb.push_back(std::get<1>(g.first));
+    }
+    RT_TRY(upload(h, recs, &h->tabs.recs));
+    RT_TRY(upload(h, alists, &h->tabs.alists));
+    RT_TRY(upload(h, bra_rows, &h->tabs.bra_prim));
+    h->tabs.tau = tau;
+    h->tabs.nao = h->nao;
+
+    // ---- work lists, one per kernel instantiation
+    auto count_ge = [&](int kc, double thr) {       // kets with Q >= thr (Q sorted descending)
+        const std::vector<double>& q = hQ[kc];
+        const int n = h->tabs.kets[kc].n;
+        return (int)(std::upper_bound(q.begin(), q.begin() + n, thr, [](double t, double x) { return t > x; }) - q.begin());
+    };
+    double n_eval = 0, nprim_eval = 0, flops_eval_kernel = 0;
+    const int bra_classes[4][2] = {{0, 0}, {1, 0}, {0, 1}, {1, 1}};
+    h->launches.clear();
+    for (int bc = 3; bc >= 0; --bc) {
+        const int la = bra_classes[bc][0], lb = bra_classes[bc][1], pcb = la + lb;
+        for (int kc = NKETCLASS - 1; kc >= 0; --kc) {
+            const int pck = kc / NSUB;
+            if (pck > pcb || h->tabs.kets[kc].n == 0) continue;
+            const int lc = pck >= 1 ? 1 : 0, ld = pck == 2 ? 1 : 0;
+            std::vector<std::pair<double, WorkItem>> items;
+            for (int ai = 0; ai < (int)alists.size(); ++ai) {
+                if (alist_la[ai] != la || alist_lb[ai] != lb) continue;
+                const AList& al = alists[ai];
+                if (pck == pcb && al.ketclass > kc) continue;
+                const int nk = tau > 0.0 ? count_ge(kc, tau / al.Qmax) : h->tabs.kets[kc].n;
+                int q0 = 0;
+                if (al.ketclass == kc) q0 = (recs[al.rec_begin].pos / JK_BLOCK) * JK_BLOCK;
+                // exact evaluation counts of this a-list against this ket class
+                for (int r = al.rec_begin; r < al.rec_end; ++r) {
+                    const int nkr = tau > 0.0 ? count_ge(kc, tau / recs[r].Q) : h->tabs.kets[kc].n;
+                    const int lo = (al.ketclass == kc) ? recs[r].pos : 0;
+                    if (nkr > lo) {
+                        n_eval += nkr - lo;
+                        nprim_eval += (double)(nkr - lo) * al.np * h->tabs.kets[kc].np;
+                        flops_eval_kernel += (double)(nkr - lo) * al.np * h->tabs.kets[kc].np * flops_prim(la, lb, lc, ld);
+                    }
+                }
+                const double len = al.rec_end - al.rec_begin;
+                for (int k0 = q0; k0 < nk; k0 += JK_BLOCK)
+                    items.push_back({len * al.np, WorkItem{ai, k0}});
+            }
+            std::stable_sort(items.begin(), items.end(), [](const auto& x, const auto& y) { return x.first > y.first; });
+            std::vector<WorkItem> w;
+            w.reserve(items.size());
+            for (auto& it : items) w.push_back(it.second);
+            JKLaunch L;
+            L.la = la; L.lb = lb; L.lc = lc; L.ld = ld; L.ketclass = kc; L.nwork = (int)w.size();
+            RT_TRY(upload(h, w, &L.work));
+            if (L.nwork) h->launches.push_back(L);
+        }
+    }
+
+    // ---- R14 counts: unique quartets with Q_ab Q_cd >= tau, and the flop model on them
+    {
+        double ordered = 0, ordered_prim = 0, diag = 0, diag_prim = 0, fl_ord = 0, fl_diag = 0, nint_ord = 0, nint_diag = 0;
+        for (int kc1 = 0; kc1 < NKETCLASS; ++kc1)
+            for (int k : cls[kc1]) {
+                const Pair& P = pairs[k];
+                const int l1 = P.pc >= 1, l2 = P.pc == 2;
+                for (int kc2 = 0; kc2 < NKETCLASS; ++kc2) {
+                    const int n2 = tau > 0.0 ? count_ge(kc2, tau / P.Q) : h->tabs.kets[kc2].n;
+                    const int pc2 = kc2 / NSUB, l3 = pc2 >= 1, l4 = pc2 == 2;
+                    const double npq = (double)P.np * h->tabs.kets[kc2].np;
+                    ordered += n2;
+                    ordered_prim += n2 * npq;
+                    fl_ord += n2 * npq * flops_prim(l1, l2, l3, l4);
+                    nint_ord += (double)n2 * (2 * l1 + 1) * (2 * l2 + 1) * (2 * l3 + 1) * (2 * l4 + 1);
+                }
+                if (P.Q * P.Q >= tau) {
+                    diag += 1; diag_prim += (double)P.np * P.np;
+                    fl_diag += (double)P.np * P.np * flops_prim(l1, l2, l1, l2);
+                    nint_diag += (double)(2 * l1 + 1) * (2 * l2 + 1) * (2 * l1 + 1) * (2 * l2 + 1);
+                }
+            }
+        h->info[RTTDA_INFO_NQUARTETS] = 0.5 * (ordered + diag);
+        h->info[RTTDA_INFO_NPRIM_QUARTETS] = 0.5 * (ordered_prim + diag_prim);
+        h->info[RTTDA_INFO_FLOPS_EVAL] = 0.5 * (fl_ord + fl_diag);
+        h->info[RTTDA_INFO_FLOPS_DIGEST_PER_VEC] = 20.0 * 0.5 * (nint_ord + nint_diag);
+    }
+    h->info[RTTDA_INFO_NPAIRS_TOTAL] = (double)npairs_total;
+    h->info[RTTDA_INFO_NPAIRS_KEPT] = (double)nkept;
+    h->info[RTTDA_INFO_NQUARTETS_EVAL] = n_eval;
+    h->info[RTTDA_INFO_NPRIM_EVAL] = nprim_eval;
+    h->info[RTTDA_INFO_JK_LAUNCHES] = (double)h->launches.size();
+    h->info[RTTDA_INFO_QMAX] = Qmax;
+    h->info[RTTDA_INFO_NVEC_CHUNK] = jk_nvec_chunk();
+
+    // ---- MO coefficients, eps differences, dipoles
+    auto dalloc = [&](double** p, size_t n) -> int {
+        RT_CUDA(cudaMalloc((void**)p, std::max<size_t>(n, 1) * sizeof(double)));
+        h->dev_allocs.push_back(*p);
+        return RTTDA_OK;
+    };
+    const size_t no = h->nocc, nv = h->nvirt;
+    RT_TRY(dalloc(&h->C_occ, N * no));
+    RT_TRY(dalloc(&h->C_virt, N * nv));
+    RT_CUDA(cudaMemcpyAsync(h->C_occ, C_occ, N * no * sizeof(double), cudaMemcpyDeviceToDevice, st));
+    RT_CUDA(cudaMemcpyAsync(h->C_virt, C_virt, N * nv * sizeof(double), cudaMemcpyDeviceToDevice, st));
+    std::vector<double> de(no * nv);
+    for (size_t i = 0; i < no; ++i)
+        for (size_t a = 0; a < nv; ++a) de[i * nv + a] = eps[no + a] - eps[i];
+    RT_TRY(dalloc(&h->deps, no * nv));
+    RT_CUDA(cudaMemcpyAsync(h->deps, de.data(), de.size() * sizeof(double), cudaMemcpyHostToDevice, st));
+    std::vector<double> D(3 * N * N);
+    one_electron_host(H, nullptr, D.data());
+    RT_TRY(dalloc(&h->D_ao, 3 * N * N));
+    RT_CUDA(cudaMemcpyAsync(h->D_ao, D.data(), D.size() * sizeof(double), cudaMemcpyHostToDevice, st));
+    RT_TRY(dalloc(&h->D_oo, 3 * no * no));
+    RT_TRY(dalloc(&h->D_vv, 3 * nv * nv));
+    RT_TRY(dalloc(&h->D_ov, 3 * no * nv));
+    double* tmp = nullptr;                      // D C_v | D C_o, [3][N][max(no,nv)]
+    const size_t nm = std::max(no, nv);
+    RT_CUDA(cudaMalloc((void**)&tmp, 3 * N * nm * sizeof(double)));
+    // tmp = D^k C_v ; D_vv = C_v^T tmp ; D_ov = C_o^T tmp ; then tmp = D^k C_o ; D_oo = C_o^T tmp
+    GemmDesc g{};
+    g.alpha = 1.0; g.beta = 0.0; g.batch = 3;
+    g.M = (int)N; g.N = (int)nv; g.K = (int)N;
+    g.A = h->D_ao; g.sam = N; g.sak = 1; g.sabatch = N * N;
+    g.B = h->C_virt; g.sbk = nv; g.sbn = 1; g.sbbatch = 0;
+    g.C = tmp; g.scm = nv; g.scn = 1; g.scbatch = N * nv;
+    RT_TRY(gemm_f64(g, st));
+    g.M = (int)nv; g.N = (int)nv; g.K = (int)N;
+    g.A = h->C_virt; g.sam = 1; g.sak = nv; g.sabatch = 0;
+    g.B = tmp; g.sbk = nv; g.sbn = 1; g.sbbatch = N * nv;
+    g.C = h->D_vv; g.scm = nv; g.scn = 1; g.scbatch = nv * nv;
+    RT_TRY(gemm_f64(g, st));
+    g.M = (int)no; g.A = h->C_occ; g.sam = 1; g.sak = no;
+    g.C = h->D_ov; g.scm = nv; g.scbatch = no * nv;
+    RT_TRY(gemm_f64(g, st));
+    g.M = (int)N; g.N = (int)no; g.K = (int)N;
+    g.A = h->D_ao; g.sam = N; g.sak = 1; g.sabatch = N * N;
+    g.B = h->C_occ; g.sbk = no; g.sbn = 1; g.sbbatch = 0;
+    g.C = tmp; g.scm = no; g.scn = 1; g.scbatch = N * no;
+    RT_TRY(gemm_f64(g, st));
+    g.M = (int)no; g.N = (int)no; g.K = (int)N;
+    g.A = h->C_occ; g.sam = 1; g.sak = no; g.sabatch = 0;
+    g.B = tmp; g.sbk = no; g.sbn = 1; g.sbbatch = N * no;
+    g.C = h->D_oo; g.scm = no; g.scn = 1; g.scbatch = no * no;
+    RT_TRY(gemm_f64(g, st));
+    h->kernel_launches += 5;
+    std::vector<double> doo(3 * no * no);
+    RT_CUDA(cudaMemcpyAsync(doo.data(), h->D_oo, doo.size() * sizeof(double), cudaMemcpyDeviceToHost, st));
+    RT_CUDA(cudaStreamSynchronize(st));
+    cudaFree(tmp);
+    for (int k = 0; k < 3; ++k) {
+        double tr = 0.0;
+        for (size_t i = 0; i < no; ++i) tr += doo[k * no * no + i * no + i];
+        h->D_00[k] = 2.0 * tr;                 // R3: sum over spin orbitals
+    }
+    for (auto& e : h->ev) RT_CUDA(cudaEventCreate(&e));
+    h->info[RTTDA_INFO_CREATE_MS] =
+        std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - t0).count();
+    return RTTDA_OK;
+}
+
+int overlap_host(const rttda_basis_t* basis, int nao, double* S, double* D)
+{
+    HostBasis H;
+    RT_TRY(load_basis(basis, H));
+    RT_CHECK(H.nao == nao, "nao does not match the shell table");
+    one_electron_host(H, S, D);
+    return RTTDA_OK;
+}
+
+}  // namespace rttda

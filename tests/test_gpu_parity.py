@@ -1,0 +1,170 @@
+"""-m gpu parity tests: the CUDA library (through the C-ABI binding) against the oracle, element by element.
+
+Tolerances (BASELINE.json north_star): sigma  ||s_gpu - s_ref||_inf / ||s_ref||_inf <= 1e-10,
+amplitudes after the run <= 1e-8 absolute.  Integer work (quartet counts) is compared exactly.
+"""
+import numpy as np
+import pytest
+
+from gpu_common import gpu_fock, gpu_sigma, rel_inf, setup_config
+
+pytestmark = pytest.mark.gpu
+
+SIGMA_TOL = 1e-10
+AMP_TOL = 1e-8
+
+
+def test_fock_tiny_all_classes_nonsymmetric_density():
+    ctx = setup_config(1, tau=0.0, dense=True)
+    ob, N = ctx["ob"], ctx["basis"].nao
+    eri = ob.eri_tensor()
+    T = np.random.default_rng(0).standard_normal((3, N, N))          # 3 = one full chunk + a ragged one
+    Fref = 2 * np.einsum("mnls,vls->vmn", eri, T) - np.einsum("mnls,vns->vml", eri, T)
+    F = gpu_fock(ctx, T)
+    assert rel_inf(F, Fref) < 1e-12
+
+
+def test_fock_tiny_unit_densities_hit_every_integral():
+    """T = e_lam e_sig^T isolates single columns of the integral tensor: catches any index slip."""
+    ctx = setup_config(1, tau=0.0, dense=True)
+    eri, N = ctx["ob"].eri_tensor(), ctx["basis"].nao
+    rng = np.random.default_rng(1)
+    for _ in range(6):
+        lam, sig = rng.integers(0, N, size=2)
+        T = np.zeros((1, N, N)); T[0, lam, sig] = 1.0
+        Fref = 2 * eri[:, :, lam, sig] - eri[:, lam, :, sig]
+        F = gpu_fock(ctx, T)[0]
+        assert np.max(np.abs(F - Fref)) < 1e-13
+
+
+@pytest.mark.parametrize("nvec", [1, 2, 5, 8])
+def test_sigma_tiny_vs_dense_A(nvec):
+    from workloads import make_vectors
+    from oracle import tda
+    ctx = setup_config(1, dense=True)
+    X = make_vectors(ctx["cfg"], nvec)
+    ref = tda.sigma_dense(ctx["A"], X)
+    got = gpu_sigma(ctx, X)
+    assert rel_inf(got, ref) < SIGMA_TOL
+    assert rel_inf(got, ref) < 1e-12        # in practice rounding level
+
+
+def test_sigma_symmetry_and_linearity_tiny():
+    from workloads import make_vectors
+    ctx = setup_config(1, dense=True)
+    X = make_vectors(ctx["cfg"], 2)
+    s = gpu_sigma(ctx, X)
+    assert abs(X[0] @ s[1] - X[1] @ s[0]) < 1e-12                     # x^T A y = y^T A x
+    s2 = gpu_sigma(ctx, np.stack([2.0 * X[0] - 0.5 * X[1], X[1]]))
+    assert np.max(np.abs(s2[0] - (2.0 * s[0] - 0.5 * s[1]))) < 1e-12
+
+
+def test_quartet_counts_match_oracle_exactly():
+    for k, tau in ((1, 1e-12), (1, 1e-6), (2, 1e-12)):
+        ctx = setup_config(k, tau=tau)
+        ob, N = ctx["ob"], ctx["basis"].nao
+        _, _, nq, npq = ob.jk(np.zeros((1, N, N)), tau=tau)
+        assert int(ctx["h"].rttda_get_info("nquartets")) == nq
+        assert int(ctx["h"].rttda_get_info("nprim_quartets")) == npq
+
+
+def test_sigma_config2_vs_matrix_free_oracle():
+    from workloads import make_vectors
+    from oracle import tda
+    ctx = setup_config(2)
+    X = make_vectors(ctx["cfg"], 6)
+    ref, nq, _ = tda.sigma_matrix_free(ctx["ob"], X, ctx["C_o"], ctx["C_v"], ctx["eps"], 1.0, tau=1e-20)
+    got = gpu_sigma(ctx, X)
+    assert rel_inf(got, ref) < SIGMA_TOL
+    assert abs(X[0] @ got[1] - X[1] @ got[0]) < 1e-11
+
+
+def _state0(ntraj, ncsf):
+    y = np.zeros((ntraj, 2, 1 + ncsf))
+    y[:, 0, 0] = 1.0                                                  # q_0 = 1
+    return y
+
+
+def test_propagate_tiny_cw_10_steps():
+    import torch
+    from oracle import tda
+    ctx = setup_config(1, dense=True)
+    cfg, h = ctx["cfg"], ctx["h"]
+    f = dict(cfg.fields[0])
+    D = ctx["ob"].dipole()
+    Doo, Dvv, Dov, D00 = tda.mo_dipoles(D, ctx["C_o"], ctx["C_v"], f["dir"])
+    n = ctx["A"].shape[0]
+    y0 = np.zeros(n + 1, dtype=complex); y0[0] = 1.0
+    yref, logref = tda.rk4_dense(ctx["A"], Doo, Dvv, Dov, D00, y0, f, 0.0, cfg.dt, cfg.nsteps)
+    y = torch.from_numpy(_state0(1, n)).to(ctx["dev"])
+    log = torch.zeros((cfg.nsteps, 1, 3), dtype=torch.float64, device=ctx["dev"])
+    h.rttda_propagate(y, [f], 0.0, cfg.dt, cfg.nsteps, log)
+    torch.cuda.synchronize()
+    y = y.cpu().numpy()
+    assert np.max(np.abs(y[0, 0] - yref.real)) < AMP_TOL and np.max(np.abs(y[0, 1] - yref.imag)) < AMP_TOL
+    assert np.max(np.abs(y[0, 0] - yref.real)) < 1e-12
+    assert np.max(np.abs(log.cpu().numpy()[:, 0, :] - logref)) < 1e-12
+    # zero field: the ground state stays exactly stationary
+    y = torch.from_numpy(_state0(1, n)).to(ctx["dev"])
+    h.rttda_propagate(y, [{"type": "none"}], 0.0, cfg.dt, 5, None)
+    torch.cuda.synchronize()
+    assert np.array_equal(y.cpu().numpy(), _state0(1, n))
+
+
+def test_propagate_tiny_batched_kicks_and_pulses_and_reentry():
+    """Three trajectories with different pulse types in one call; continue in a second call."""
+    import torch
+    from oracle import tda
+    ctx = setup_config(1, dense=True)
+    h, n = ctx["h"], ctx["A"].shape[0]
+    D = ctx["ob"].dipole()
+    fields = [{"type": "delta", "E0": 1e-4, "dir": (1.0, 0.0, 0.0)},
+              {"type": "tl", "E0": 0.02, "omega": 0.4, "t0": 1.0, "sigma": 0.6, "dir": (0.0, 1.0, 0.0)},
+              {"type": "sin2", "E0": 0.03, "omega": 0.5, "T_env": 1.5, "dir": (0.3, 0.1, 0.9)}]
+    dt, n1, n2 = 0.05, 12, 9
+    y = torch.from_numpy(_state0(3, n)).to(ctx["dev"])
+    log = torch.zeros((n1, 3, 3), dtype=torch.float64, device=ctx["dev"])
+    h.rttda_propagate(y, fields, 0.0, dt, n1, log)
+    cont = [dict(f) for f in fields]
+    cont[0] = {"type": "none"}                                       # the kick is applied once
+    h.rttda_propagate(y, cont, n1 * dt, dt, n2, None)
+    torch.cuda.synchronize()
+    y, log = y.cpu().numpy(), log.cpu().numpy()
+    for t, f in enumerate(fields):
+        Doo, Dvv, Dov, D00 = tda.mo_dipoles(D, ctx["C_o"], ctx["C_v"], f["dir"])
+        y0 = np.zeros(n + 1, dtype=complex); y0[0] = 1.0
+        ya, la = tda.rk4_dense(ctx["A"], Doo, Dvv, Dov, D00, y0, f, 0.0, dt, n1)
+        assert np.max(np.abs(log[:, t, :] - la)) < 1e-12
+        yb, _ = tda.rk4_dense(ctx["A"], Doo, Dvv, Dov, D00, ya, cont[t], n1 * dt, dt, n2)
+        assert np.max(np.abs(y[t, 0] - yb.real)) < 1e-12 and np.max(np.abs(y[t, 1] - yb.imag)) < 1e-12
+
+
+def test_host_buffer_entry_points():
+    from workloads import make_vectors
+    from oracle import tda
+    ctx = setup_config(1, dense=True)
+    X = make_vectors(ctx["cfg"], 3)
+    out = np.zeros_like(X)
+    ctx["h"].rttda_sigma_host(X, out)
+    assert rel_inf(out, tda.sigma_dense(ctx["A"], X)) < 1e-12
+    n = ctx["A"].shape[0]
+    y = _state0(1, n)
+    log = np.zeros((4, 1, 3))
+    ctx["h"].rttda_propagate_host(y, [dict(ctx["cfg"].fields[0])], 0.0, 0.05, 4, log)
+    assert abs(log[-1, 0, 0] - 1.0) < 1e-6 and y[0, 0, 0] != 1.0
+
+
+def test_error_codes():
+    import torch
+    import paper_2601_16949_b200 as R
+    ctx = setup_config(1)
+    h = ctx["h"]
+    X = torch.zeros((1, h.ncsf), dtype=torch.float64, device=ctx["dev"])
+    with pytest.raises(R.RttdaError):
+        h.rttda_sigma(X, X)                                           # aliasing
+    with pytest.raises(R.RttdaError):
+        h.rttda_propagate(torch.zeros((9, 2, 1 + h.ncsf), dtype=torch.float64, device=ctx["dev"]),
+                          [{"type": "none"}] * 9, 0.0, 0.1, 1)        # ntraj > 8
+    with pytest.raises(R.RttdaError):
+        R.Rttda(ctx["basis"], torch.zeros((30, 4), dtype=torch.float64, device=ctx["dev"]),
+                torch.zeros((30, 25), dtype=torch.float64, device=ctx["dev"]), ctx["eps"])   # nocc+nvirt != nao
