@@ -1,0 +1,355 @@
+#!/usr/bin/env python
+"""bench.py -- RT-TDA hot path at the 1280-AO molecule (BASELINE.json metric: sigma-vectors/s and RT-TDA
+steps/s at 1280 AO; FP64 pipe % of peak).
+
+    python bench.py --gpus N --steps K --warmup W [--config 4] [--ntraj 3] [--impl reference]
+
+One *step* = one RK4 step of `rttda_propagate` on config 4: every row a1-a7 of
+the hot path -- 4 ERI passes, each serving the 2*ntraj real vectors of the batch, the MO<->AO GEMMs, the
+field coupling and the RK4 combine.  value = sigma-vectors/s = 8*ntraj*N_gpus / t_step (one sigma-vector =
+A x for one real x).  Inputs are seeded synthetic (workloads/), resident in HBM before the timed
+region; the `e2e` number goes through `rttda_propagate_host` (host buffers, copies inside the timed region).
+Multi-GPU (N > 1): replicas only -- every rank runs the same batch of trajectories on
+its own GPU, no data-path collective, "weak" scaling; time = max over ranks.
+
+`--impl reference` times the CPU oracle (oracle/, as it stands) on the host cores for the same metric.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "sigma_vectors_per_s_1280ao"
+UNIT = "sigma-vectors/s"
+FP64_NOMINAL_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12      # 148 SMs x 64 DFMA/clk/SM x 2 x max SM clock
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--config", type=int, default=4, help="workload (4 = the 1280-AO molecule; 2, 3 smaller)")
+    ap.add_argument("--ntraj", type=int, default=0, help="trajectories per call (0 = all of the config's fields)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--cpu-seconds", type=float, default=20.0, help="CPU budget of the cpu_baseline sample")
+    ap.add_argument("--sweep", action="store_true", help="also run the config-5 sigma sweep -> gpurun_out/sweep.json")
+    return ap.parse_args()
+
+
+def dist_env():
+    return int(os.environ.get("RANK", 0)), int(os.environ.get("LOCAL_RANK", 0)), int(os.environ.get("WORLD_SIZE", 1))
+
+
+# ------------------------------------------------------------------------------------------ workload
+def build_inputs(k: int, overlap_fn):
+    """Seeded synthetic molecule of config k.  overlap_fn(basis) -> S comes from the side being timed."""
+    from workloads import get_config, make_basis, make_mos
+    cfg = get_config(k)
+    bump = 0
+    while True:
+        basis = make_basis(cfg, bump)
+        S = overlap_fn(basis)
+        C_o, C_v, eps, cond = make_mos(cfg, S, bump)
+        if cond <= 1e5:
+            break
+        bump += 1
+    return cfg, basis, C_o, C_v, eps, cond, bump
+
+
+def fields_for(cfg, ntraj, omega):
+    fs = [dict(f) for f in cfg.fields]
+    if ntraj:
+        fs = [dict(fs[i % len(fs)]) for i in range(ntraj)]
+    for f in fs:
+        if f.get("omega", 0.0) is None:
+            f["omega"] = omega
+    return fs
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons DURING the timed region (B200_PROFILING.md recipe)."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.proc, self.lines = index, None, []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "200"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            threading.Thread(target=self._read, daemon=True).start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.lines.append(line.strip())
+
+    def stop(self) -> dict:
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        sm, smax, pw, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for ln in self.lines:
+            p = [x.strip() for x in ln.split(",")]
+            if len(p) < 8:
+                continue
+            try:
+                sm.append(float(p[1])); smax.append(float(p[2])); pw.append(float(p[3]))
+            except ValueError:
+                continue
+            for nm, v in zip(names, p[4:8]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        return {"sm_mhz": float(np.median(sm)), "sm_max_mhz": float(max(smax)), "power_w_max": float(max(pw)),
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# ------------------------------------------------------------------------------------------ CPU oracle legs
+def count_unique_quartets(Q: np.ndarray, sh_nprim: np.ndarray, tau: float):
+    """Unique shell quartets (a>=b, c>=d, ab>=cd) with Q_ab Q_cd >= tau (R14) and the primitive quartets in
+    them, from the Schwarz matrix alone (pure counting; used to scale the CPU sample to one full pass)."""
+    ns = Q.shape[0]
+    ia, ib = np.tril_indices(ns)
+    q = Q[ia, ib]
+    w = (sh_nprim[ia].astype(np.float64) * sh_nprim[ib])
+    order = np.argsort(-q, kind="stable")
+    qs, ws = q[order], w[order]
+    cw = np.concatenate([[0.0], np.cumsum(ws)])
+    with np.errstate(divide="ignore"):
+        thr = np.where(qs > 0, tau / qs, np.inf)
+    n = np.searchsorted(-qs, -thr, side="right")          # kets with Q_cd >= tau / Q_ab
+    ordered, ordered_p = float(np.sum(n)), float(np.sum(ws * cw[n]))
+    dmask = qs * qs >= tau
+    return 0.5 * (ordered + float(np.sum(dmask))), 0.5 * (ordered_p + float(np.sum(ws[dmask] ** 2)))
+
+
+def oracle_sample(cfg_k: int, nvec: int, cpu_seconds: float):
+    """Time the oracle's matrix-free J/K (oracle/, as it stands, all host cores) on a bounded sample of the
+    bra shell pairs of config cfg_k and scale by the primitive-quartet fraction of the sample.
+    Returns (sigma_vectors_per_s, cores, description, seconds per full ERI pass)."""
+    from oracle.integrals import OracleBasis, num_threads
+    from oracle import tda
+    from workloads import make_vectors
+    cfg, basis, C_o, C_v, eps, _, _ = build_inputs(cfg_k, lambda b: OracleBasis(b).overlap())
+    ob = OracleBasis(basis)
+    Q = ob.schwarz()
+    nq_total, nprim_total = count_unique_quartets(Q, np.asarray(basis.sh_nprim), cfg.tau)
+    X = make_vectors(cfg, nvec)
+    T = np.stack([tda.transition_density(x.reshape(cfg.nocc, cfg.nvirt), C_o, C_v) for x in X])
+    npair = ob.nshells * (ob.nshells + 1) // 2
+    # pilot: a thin sample to learn the rate, then one sample sized for the CPU budget
+    stride = max(1, npair // 256)
+    t0 = time.perf_counter()
+    _, _, nq, npq = ob.jk_strided(T, cfg.tau, Q, stride, stride // 2)
+    dt = time.perf_counter() - t0
+    rate = max(npq, 1) / max(dt, 1e-6)
+    stride2 = int(max(1, min(stride, round(nprim_total / max(rate * cpu_seconds, 1.0)))))
+    t0 = time.perf_counter()
+    _, _, nq2, npq2 = ob.jk_strided(T, cfg.tau, Q, stride2, stride2 // 2)
+    dt2 = time.perf_counter() - t0
+    frac = npq2 / nprim_total
+    t_pass = dt2 / frac
+    desc = ("oracle_jk over bra shell pairs ab %% %d == %d of config %d: %d of %.4g unique shell quartets, %.4g of "
+            "%.4g primitive quartets (fraction %.5f of one ERI pass, tau=%g, nvec=%d) in %.1f s, scaled to one "
+            "pass; MO<->AO transforms (<1%% of the flops) not included"
+            % (stride2, stride2 // 2, cfg_k, nq2, nq_total, npq2, nprim_total, frac, cfg.tau, nvec, dt2))
+    return nvec / t_pass, num_threads(), desc, t_pass
+
+
+def run_reference(args):
+    rank, _, world = dist_env()
+    if rank != 0:
+        return
+    k = args.config
+    from workloads import get_config
+    cfg = get_config(k)
+    ntraj = args.ntraj or len(cfg.fields)
+    nvec = 2 * ntraj
+    vals, desc, cores = [], "", 0
+    per = max(5.0, min(30.0, 120.0 / max(args.steps + args.warmup, 1)))
+    for i in range(args.warmup + args.steps):
+        v, cores, desc, t_pass = oracle_sample(k, nvec, per)
+        if i >= args.warmup:
+            vals.append((v, t_pass))
+    v = float(np.mean([x[0] for x in vals]))
+    t_step = 4.0 * float(np.mean([x[1] for x in vals]))
+    out = {"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus,
+           "steps": args.steps, "warmup": args.warmup, "ms_per_step": t_step * 1e3, "higher_is_better": True,
+           "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+           "config": {"workload": "config %d (%s): %d AO, nocc %d, nvirt %d, ntraj %d (nvec %d), tau %g; one step = "
+                                  "one RK4 step = 4 ERI passes" % (k, cfg.name, cfg.nocc + cfg.nvirt, cfg.nocc,
+                                                                  cfg.nvirt, ntraj, nvec, cfg.tau)},
+           "cpu_baseline": {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc},
+           "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+           "gpu_launches": 0}
+    print(json.dumps(out))
+
+
+# ------------------------------------------------------------------------------------------ B200 arm
+def run_b200(args):
+    import torch
+    import paper_2601_16949_b200 as R
+    rank, local_rank, world = dist_env()
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: the product path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=dev)
+
+    def barrier():
+        if world > 1:
+            torch.distributed.barrier()
+        torch.cuda.synchronize()
+
+    k = args.config
+    t0 = time.perf_counter()
+    cfg, basis, C_o, C_v, eps, cond, bump = build_inputs(k, R.rttda_overlap)
+    st = torch.cuda.current_stream()
+    h = R.Rttda(basis, torch.from_numpy(C_o).to(dev), torch.from_numpy(C_v).to(dev), eps, 1.0, cfg.tau, st)
+    torch.cuda.synchronize()
+    setup_s = time.perf_counter() - t0
+    info = h.info()
+    ncsf, n1 = h.ncsf, h.ncsf + 1
+
+    # carrier frequency (R9/R10 leave it to the harness; any recorded omega serves the timing): Rayleigh
+    # quotient of A on the normalised z-dipole vector through rttda_sigma, halved for config 4
+    D = R.rttda_dipole_ao(basis)
+    dz = (C_o.T @ D[2] @ C_v).reshape(1, -1)
+    dz /= np.linalg.norm(dz)
+    xd = torch.from_numpy(dz).to(dev)
+    sd = torch.empty_like(xd)
+    h.rttda_sigma(xd, sd, st)
+    torch.cuda.synchronize()
+    omega = float((xd * sd).sum().item()) * (0.5 if k == 4 else 1.0)
+    fields = fields_for(cfg, args.ntraj, omega)
+    ntraj = len(fields)
+    nvec = 2 * ntraj
+
+    y0 = np.zeros((ntraj, 2, n1))
+    y0[:, 0, 0] = 1.0
+    y = torch.from_numpy(y0).to(dev)
+    log = torch.zeros((1, ntraj, 3), dtype=torch.float64, device=dev)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)     # > 126 MB L2
+    dt = cfg.dt if cfg.dt > 0 else 0.1
+
+    def step(i):
+        h.rttda_propagate(y, fields if i == 0 else cont, i * dt, dt, 1, log, st)
+
+    cont = [dict(f) if f["type"] != "delta" else {"type": "none"} for f in fields]
+    for i in range(args.warmup):
+        step(i)
+        flush.zero_()
+    barrier()
+    h.rttda_jk_time()
+    l0 = h.rttda_get_info("kernel_launches")
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    barrier()
+    for i in range(args.steps):
+        ev[i][0].record(st)
+        step(args.warmup + i)
+        ev[i][1].record(st)
+        flush.zero_()
+    barrier()
+    clocks = sampler.stop()
+    ms = [a.elapsed_time(b) for a, b in ev]
+    total_ms = float(sum(ms))
+    jk_ms, jk_n = h.rttda_jk_time()
+    launches = int(h.rttda_get_info("kernel_launches") - l0)
+    if world > 1:
+        t = torch.tensor([total_ms], dtype=torch.float64, device=dev)
+        torch.distributed.all_reduce(t, op=torch.distributed.ReduceOp.MAX)
+        total_ms = float(t.item())
+    ms_per_step = total_ms / args.steps
+    value = 8.0 * ntraj * world / (ms_per_step * 1e-3)
+
+    # end to end: host buffers through rttda_propagate_host (H2D of the state, D2H of state + log inside)
+    yh = torch.from_numpy(y0.copy()).pin_memory()
+    lh = torch.zeros((1, ntraj, 3), dtype=torch.float64).pin_memory()
+    h.rttda_propagate_host(yh.numpy(), fields, 0.0, dt, 1, lh.numpy(), st)
+    barrier()
+    e0 = time.perf_counter()
+    for i in range(args.steps):
+        h.rttda_propagate_host(yh.numpy(), cont, (i + 1) * dt, dt, 1, lh.numpy(), st)
+    barrier()
+    e2e_s = time.perf_counter() - e0
+    if world > 1:
+        t = torch.tensor([e2e_s], dtype=torch.float64, device=dev)
+        torch.distributed.all_reduce(t, op=torch.distributed.ReduceOp.MAX)
+        e2e_s = float(t.item())
+    e2e_val = 8.0 * ntraj * world * args.steps / e2e_s
+    h2d = yh.numel() * 8
+    d2h = yh.numel() * 8 + lh.numel() * 8
+
+    # roofline of the dominant kernel group (the J/K ERI pass): algorithmic flops / measured device time
+    flops_pass = info["flops_eval"] + nvec * info["flops_digest_per_vec"]
+    jk_avg_ms = jk_ms / max(jk_n, 1)
+    achieved = flops_pass / (jk_avg_ms * 1e-3) / 1e12
+    peak = R.rttda_fp64_peak(1.0, st)
+    out = None
+    if rank == 0:
+        out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+               "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
+               "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+               "config": {"workload": "config %d (%s): %d AO, nocc %d, nvirt %d, %d singles, ntraj %d (nvec %d per ERI "
+                                      "pass), tau %g, dt %g; one step = one RK4 step of rttda_propagate = 4 ERI passes "
+                                      "+ 16 GEMM launches + field + combine" % (k, cfg.name, h.nao, h.nocc, h.nvirt,
+                                                                               ncsf, ntraj, nvec, cfg.tau, dt),
+                          "l2": "256 MiB buffer written between timed steps (L2 flush)",
+                          "parallelism": "replicas" if world > 1 else "1 GPU", "omega": omega,
+                          "cond_S": cond, "seed_bump": bump},
+               "rt_tda_steps_per_s": world * 1e3 / ms_per_step,
+               "eri_quartets_per_s": info["nquartets"] / (jk_avg_ms * 1e-3),
+               "counts": {"shell_pairs_kept": info["npairs_kept"], "unique_shell_quartets": info["nquartets"],
+                          "primitive_quartets": info["nprim_quartets"], "quartets_evaluated": info["nquartets_eval"],
+                          "primitive_evaluated": info["nprim_eval"], "nvec_chunk": info["nvec_chunk"]},
+               "setup_s": setup_s, "create_ms": info["create_ms"],
+               "jk_ms_per_pass": jk_avg_ms, "jk_share_of_step": jk_ms / (sum(ms) if sum(ms) else 1.0),
+               "roofline": {"bound": "alu", "kernel": "jk_kernel<*> (all class launches of one ERI pass)",
+                            "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
+                            "traffic": None, "peak_source": "measured live: rttda_fp64_peak DFMA chain, 1 s "
+                            "(MEASURED_PEAKS.json has no FP64 entry; nominal %.1f)" % FP64_NOMINAL_TFLOPS,
+                            "flops_per_launch_group": flops_pass},
+               "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
+               "gpu_launches": launches, "clocks": clocks}
+    h.close()
+    if rank == 0:
+        if not args.no_cpu_baseline and world == 1:
+            v, cores, desc, _ = oracle_sample(k, nvec, args.cpu_seconds)
+            out["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc}
+        else:
+            out["cpu_baseline"] = None
+        print(json.dumps(out))
+    if world > 1:
+        torch.distributed.destroy_process_group()
+
+
+if __name__ == "__main__":
+    a = parse()
+    if a.impl == "reference":
+        run_reference(a)
+    else:
+        run_b200(a)

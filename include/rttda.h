@@ -143,6 +143,12 @@ int rttda_get_info(rttda_handle_t h, int32_t key, double* out);
  * stream (synchronises those events).  ms_out[0] = J/K build, [1] = MO->AO GEMMs, [2] = AO->MO GEMMs. */
 int rttda_last_timings(rttda_handle_t h, double* ms_out);
 
+/* Device time spent in the J/K builds (steps a3-a4) of every rttda_sigma / rttda_fock / rttda_propagate call
+ * since the previous query: *sum_ms = total of the CUDA-event intervals recorded on the callers' streams
+ * around each ERI pass, *count = number of passes.  Synchronises on those events and resets the log (which
+ * holds at most 32768 passes; later ones are not recorded). */
+int rttda_jk_time(rttda_handle_t h, double* sum_ms, double* count);
+
 /* Sustained FP64 FMA throughput of the device (TFLOP/s) from a dependent-chain DFMA kernel run for about
  * `seconds`; the roofline denominator of the ALU-bound J/K kernels. */
 int rttda_fp64_peak(double seconds, double* tflops_out, void* stream);

@@ -342,8 +342,12 @@ void oracle_schwarz(BASIS_ARGS, double *Q)
  * rule; tests pin this against the plain N^4 contraction of oracle_eri_tensor.
  * T, J, K: [nvec][nao][nao].  Returns the number of unique shell quartets with Q_ab Q_cd >= tau
  * (R14) through *nquartets, primitive quartets through *nprimq.  tau <= 0 disables screening. */
-void oracle_jk(BASIS_ARGS, int nao, int nvec, const double *T, double tau, const double *Qs,
-               double *J, double *K, int64_t *nquartets, int64_t *nprimq)
+/* oracle_jk_strided visits only the bra pairs ab with ab % ab_stride == ab_phase (all their kets): a
+ * BOUNDED SAMPLE of the same loop, used only to time the oracle on workloads whose full pass takes
+ * tens of minutes (bench.py cpu_baseline); its J/K are then partial sums.  oracle_jk = stride 1. */
+void oracle_jk_strided(BASIS_ARGS, int nao, int nvec, const double *T, double tau, const double *Qs,
+                       int ab_stride, int ab_phase,
+                       double *J, double *K, int64_t *nquartets, int64_t *nprimq)
 {
     basis_t B = BASIS_MK;
     size_t nn = (size_t)nao * nao;
@@ -357,6 +361,7 @@ void oracle_jk(BASIS_ARGS, int nao, int nvec, const double *T, double tau, const
         int64_t nq = 0, npq = 0;
         #pragma omp for schedule(dynamic, 4)
         for (int ab = npair - 1; ab >= 0; --ab) {
+            if (ab_stride > 1 && ab % ab_stride != ab_phase) continue;
             int sa = (int)((sqrt(8.0 * ab + 1.0) - 1.0) / 2.0);
             while ((sa + 1) * (sa + 2) / 2 <= ab) ++sa;
             while (sa * (sa + 1) / 2 > ab) --sa;
@@ -411,6 +416,13 @@ void oracle_jk(BASIS_ARGS, int nao, int nvec, const double *T, double tau, const
     }
     if (nquartets) *nquartets = nq_tot;
     if (nprimq) *nprimq = npq_tot;
+}
+
+void oracle_jk(BASIS_ARGS, int nao, int nvec, const double *T, double tau, const double *Qs,
+               double *J, double *K, int64_t *nquartets, int64_t *nprimq)
+{
+    oracle_jk_strided(nshells, centers, sh_center, sh_l, sh_nprim, sh_off, ao_off, exps, ncoef, nao, nvec, T,
+                      tau, Qs, 1, 0, J, K, nquartets, nprimq);
 }
 
 /* Sampled elements of J[T] and K[T] straight from the definitions (no symmetry, no screening):

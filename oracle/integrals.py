@@ -135,6 +135,23 @@ class OracleBasis:
                         K.ctypes.data_as(_dp), ct.byref(nq), ct.byref(npq))
         return J, K, nq.value, npq.value
 
+    def jk_strided(self, T: np.ndarray, tau: float, Q: np.ndarray, stride: int, phase: int = 0):
+        """Bounded SAMPLE of jk(): only bra pairs ab with ab % stride == phase.  Returns the partial
+        J, K and the shell / primitive quartet counts of the sample (for timing extrapolation only)."""
+        T = np.ascontiguousarray(T, dtype=np.float64)
+        if T.ndim == 2:
+            T = T[None]
+        Q = np.ascontiguousarray(Q)
+        J = np.zeros_like(T)
+        K = np.zeros_like(T)
+        nq = ct.c_int64(0)
+        npq = ct.c_int64(0)
+        lib().oracle_jk_strided(*self._args(), ct.c_int(self.nao), ct.c_int(T.shape[0]),
+                                T.ctypes.data_as(_dp), ct.c_double(tau), Q.ctypes.data_as(_dp),
+                                ct.c_int(stride), ct.c_int(phase), J.ctypes.data_as(_dp),
+                                K.ctypes.data_as(_dp), ct.byref(nq), ct.byref(npq))
+        return J, K, nq.value, npq.value
+
     def jk_samples(self, T: np.ndarray, mu, nu):
         """J[T]_{mu nu}, K[T]_{mu nu} at sampled AO pairs, from the definitions (no screening)."""
         T = np.ascontiguousarray(T, dtype=np.float64)

@@ -20,7 +20,7 @@ INFO = dict(npairs_total=0, npairs_kept=1, nquartets=2, nprim_quartets=3, nquart
 PULSE = dict(none=0, delta=1, cw=2, tl=3, chirp=4, sin2=5)
 EXPORTS = ["rttda_overlap", "rttda_dipole_ao", "rttda_create", "rttda_destroy", "rttda_sigma",
            "rttda_sigma_host", "rttda_fock", "rttda_propagate", "rttda_propagate_host",
-           "rttda_get_info", "rttda_last_timings", "rttda_fp64_peak", "rttda_last_error",
+           "rttda_get_info", "rttda_last_timings", "rttda_jk_time", "rttda_fp64_peak", "rttda_last_error",
            "rttda_version"]
 
 
@@ -197,6 +197,11 @@ class Rttda:
         ms = (ct.c_double * 3)()
         _check(lib().rttda_last_timings(self._h, ms), "rttda_last_timings")
         return dict(jk_ms=ms[0], mo2ao_ms=ms[1], ao2mo_ms=ms[2])
+
+    def rttda_jk_time(self):
+        s, c = ct.c_double(0.0), ct.c_double(0.0)
+        _check(lib().rttda_jk_time(self._h, ct.byref(s), ct.byref(c)), "rttda_jk_time")
+        return s.value, int(c.value)
 
     def info(self) -> dict:
         return {k: self.rttda_get_info(k) for k in INFO}

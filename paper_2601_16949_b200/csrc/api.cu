@@ -95,6 +95,7 @@ int rttda_destroy(rttda_handle_t hh)
     for (void* p : h->dev_allocs) cudaFree(p);
     for (double* p : {h->wsY, h->wsT, h->wsF, h->wsZ, h->prop_ws}) if (p) cudaFree(p);
     for (auto& e : h->ev) if (e) cudaEventDestroy(e);
+    for (auto& e : h->jk_ev) cudaEventDestroy(e);
     delete h;
     return RTTDA_OK;
 }
@@ -137,10 +138,12 @@ int rttda_fock(rttda_handle_t hh, int32_t nvec, const double* T, double* F, void
     interleave_kernel<<<grid, 256, 0, st>>>(nn, nvec, T, h->wsT, 1);
     RT_CUDA(cudaGetLastError());
     RT_CUDA(cudaEventRecord(h->ev[1], st));
+    RT_TRY(jk_mark(h, st));
     RT_CUDA(cudaMemsetAsync(h->wsF, 0, (size_t)nvec * nn * sizeof(double), st));
     const int chunk = jk_nvec_chunk();
     for (int v0 = 0; v0 < nvec; v0 += chunk)
         RT_TRY(jk_build(h, nvec, v0, std::min(chunk, nvec - v0), h->wsT, h->wsF, st));
+    RT_TRY(jk_mark(h, st));
     RT_CUDA(cudaEventRecord(h->ev[2], st));
     interleave_kernel<<<grid, 256, 0, st>>>(nn, nvec, h->wsF, F, 0);
     RT_CUDA(cudaGetLastError());
@@ -199,6 +202,23 @@ int rttda_last_timings(rttda_handle_t hh, double* ms)
     RT_CUDA(cudaEventElapsedTime(&b, h->ev[0], h->ev[1]));
     RT_CUDA(cudaEventElapsedTime(&c, h->ev[2], h->ev[3]));
     ms[0] = a; ms[1] = b; ms[2] = c;
+    return RTTDA_OK;
+}
+
+int rttda_jk_time(rttda_handle_t hh, double* sum_ms, double* count)
+{
+    Handle* h = (Handle*)hh;
+    RT_CHECK(h && sum_ms && count, "rttda_jk_time: NULL pointer");
+    double tot = 0.0;
+    const size_t n = h->jk_ev_used / 2;
+    for (size_t i = 0; i < n; ++i) {
+        RT_CUDA(cudaEventSynchronize(h->jk_ev[2 * i + 1]));
+        float ms = 0;
+        RT_CUDA(cudaEventElapsedTime(&ms, h->jk_ev[2 * i], h->jk_ev[2 * i + 1]));
+        tot += ms;
+    }
+    *sum_ms = tot; *count = (double)n;
+    h->jk_ev_used = 0;
     return RTTDA_OK;
 }
 

@@ -131,7 +131,12 @@ struct Handle {
     long long kernel_launches = 0;
     cudaEvent_t ev[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
     bool ev_valid = false;
+    // pairs of events around every J/K build since the last rttda_jk_time query
+    std::vector<cudaEvent_t> jk_ev;
+    size_t jk_ev_used = 0;
 };
+
+int jk_mark(Handle* h, cudaStream_t st);   // record the next event of the J/K timing log
 
 // jk_kernels.cu
 int jk_build(Handle* h, int nvec_total, int v0, int nv, const double* Tq, double* Fq, cudaStream_t st);

@@ -25,6 +25,19 @@ __global__ void diag_kernel(int ncsf, int nvec, const double* __restrict__ deps,
     S[v * lds + k] = deps[k] * X[v * ldx + k];
 }
 
+int jk_mark(Handle* h, cudaStream_t st)
+{
+    constexpr size_t CAP = 1 << 16;
+    if (h->jk_ev_used >= CAP) return RTTDA_OK;
+    if (h->jk_ev_used == h->jk_ev.size()) {
+        cudaEvent_t e;
+        RT_CUDA(cudaEventCreate(&e));
+        h->jk_ev.push_back(e);
+    }
+    RT_CUDA(cudaEventRecord(h->jk_ev[h->jk_ev_used++], st));
+    return RTTDA_OK;
+}
+
 int sigma_impl(Handle* h, int nvec, const double* X, long long ldx, double* sigma, long long lds,
                cudaStream_t st)
 {
@@ -47,11 +60,13 @@ int sigma_impl(Handle* h, int nvec, const double* X, long long ldx, double* sigm
     g.C = h->wsT; g.scm = N * nvec; g.scn = nvec; g.scbatch = 1;
     RT_TRY(gemm_f64(g, st));
     RT_CUDA(cudaEventRecord(h->ev[1], st));
+    RT_TRY(jk_mark(h, st));
     // a3-a4: F = 2 J[T] - cx K[T], interleaved layout, chunks of densities per ERI pass
     RT_CUDA(cudaMemsetAsync(h->wsF, 0, (size_t)nvec * N * N * sizeof(double), st));
     const int chunk = jk_nvec_chunk();
     for (int v0 = 0; v0 < nvec; v0 += chunk)
         RT_TRY(jk_build(h, nvec, v0, std::min(chunk, nvec - v0), h->wsT, h->wsF, st));
+    RT_TRY(jk_mark(h, st));
     RT_CUDA(cudaEventRecord(h->ev[2], st));
     // a5: Z_v = C_o^T F_v [no][N];  sigma_v = deps o X_v + Z_v C_v
     g.M = (int)no; g.N = (int)N; g.K = (int)N; g.batch = nvec;
