@@ -136,7 +136,8 @@ int rttda_propagate_host(rttda_handle_t h, int32_t ntraj, double* C, const rttda
 #define RTTDA_INFO_KERNEL_LAUNCHES   9   /* kernels launched by this handle so far (all entry points) */
 #define RTTDA_INFO_CREATE_MS        10   /* wall time of rttda_create */
 #define RTTDA_INFO_QMAX             11   /* largest Schwarz bound */
-#define RTTDA_INFO_NVEC_CHUNK       12   /* densities served by one ERI pass */
+#define RTTDA_INFO_NVEC_CHUNK       12   /* 0: every ERI pass serves all densities of the call */
+#define RTTDA_INFO_ERI_BUF_BYTES    13   /* HBM staging buffer between ERI evaluation and J/K digestion */
 int rttda_get_info(rttda_handle_t h, int32_t key, double* out);
 
 /* Time the last rttda_sigma/rttda_fock call spent in the J/K kernels, from CUDA events recorded on its

@@ -16,7 +16,7 @@ _lib = None
 
 INFO = dict(npairs_total=0, npairs_kept=1, nquartets=2, nprim_quartets=3, nquartets_eval=4,
             nprim_eval=5, flops_eval=6, flops_digest_per_vec=7, jk_launches=8, kernel_launches=9,
-            create_ms=10, qmax=11, nvec_chunk=12)
+            create_ms=10, qmax=11, nvec_chunk=12, eri_buf_bytes=13)
 PULSE = dict(none=0, delta=1, cw=2, tl=3, chirp=4, sin2=5)
 EXPORTS = ["rttda_overlap", "rttda_dipole_ao", "rttda_create", "rttda_destroy", "rttda_sigma",
            "rttda_sigma_host", "rttda_fock", "rttda_propagate", "rttda_propagate_host",

@@ -13,18 +13,19 @@ int create_impl(Handle* h, const rttda_basis_t* basis, const double* C_occ, cons
                 const double* eps, cudaStream_t st);
 int overlap_host(const rttda_basis_t* basis, int nao, double* S, double* D);
 
-// [v][N][N] <-> [N][N][v]
-__global__ void interleave_kernel(long long nn, int nvec, const double* __restrict__ in, double* __restrict__ out,
-                                  int to_interleaved)
+// [nvec][N][N] <-> [N][N][nvt] (nvt >= nvec slots per element; the padding slots are written as zeros)
+__global__ void interleave_kernel(long long nn, int nvec, int nvt, const double* __restrict__ in,
+                                  double* __restrict__ out, int to_interleaved)
 {
     const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= nn * nvec) return;
     if (to_interleaved) {
-        const long long e = i / nvec; const int v = (int)(i % nvec);
-        out[i] = in[(long long)v * nn + e];
+        if (i >= nn * nvt) return;
+        const long long e = i / nvt; const int v = (int)(i % nvt);
+        out[i] = v < nvec ? in[(long long)v * nn + e] : 0.0;
     } else {
+        if (i >= nn * nvec) return;
         const int v = (int)(i / nn); const long long e = i % nn;
-        out[i] = in[e * nvec + v];
+        out[i] = in[e * nvt + v];
     }
 }
 
@@ -93,7 +94,7 @@ int rttda_destroy(rttda_handle_t hh)
     if (!h) return RTTDA_OK;
     cudaDeviceSynchronize();
     for (void* p : h->dev_allocs) cudaFree(p);
-    for (double* p : {h->wsY, h->wsT, h->wsF, h->wsZ, h->prop_ws}) if (p) cudaFree(p);
+    for (double* p : {h->wsY, h->wsT, h->wsF, h->wsZ, h->prop_ws, h->eri_buf}) if (p) cudaFree(p);
     for (auto& e : h->ev) if (e) cudaEventDestroy(e);
     for (auto& e : h->jk_ev) cudaEventDestroy(e);
     delete h;
@@ -131,21 +132,19 @@ int rttda_fock(rttda_handle_t hh, int32_t nvec, const double* T, double* F, void
     RT_CHECK(nvec >= 1, "rttda_fock: nvec < 1");
     cudaStream_t st = (cudaStream_t)stream;
     const long long nn = (long long)h->nao * h->nao;
-    RT_TRY(ensure_ws(h, &h->wsT, &h->wsT_n, (size_t)nvec * nn));
-    RT_TRY(ensure_ws(h, &h->wsF, &h->wsF_n, (size_t)nvec * nn));
-    const unsigned grid = (unsigned)((nn * nvec + 255) / 256);
+    const int nvt = (nvec + 1) & ~1;
+    RT_TRY(ensure_ws(h, &h->wsT, &h->wsT_n, (size_t)nvt * nn));
+    RT_TRY(ensure_ws(h, &h->wsF, &h->wsF_n, (size_t)nvt * nn));
     RT_CUDA(cudaEventRecord(h->ev[0], st));
-    interleave_kernel<<<grid, 256, 0, st>>>(nn, nvec, T, h->wsT, 1);
+    interleave_kernel<<<(unsigned)((nn * nvt + 255) / 256), 256, 0, st>>>(nn, nvec, nvt, T, h->wsT, 1);
     RT_CUDA(cudaGetLastError());
     RT_CUDA(cudaEventRecord(h->ev[1], st));
     RT_TRY(jk_mark(h, st));
-    RT_CUDA(cudaMemsetAsync(h->wsF, 0, (size_t)nvec * nn * sizeof(double), st));
-    const int chunk = jk_nvec_chunk();
-    for (int v0 = 0; v0 < nvec; v0 += chunk)
-        RT_TRY(jk_build(h, nvec, v0, std::min(chunk, nvec - v0), h->wsT, h->wsF, st));
+    RT_CUDA(cudaMemsetAsync(h->wsF, 0, (size_t)nvt * nn * sizeof(double), st));
+    RT_TRY(jk_build(h, nvt, h->wsT, h->wsF, st));
     RT_TRY(jk_mark(h, st));
     RT_CUDA(cudaEventRecord(h->ev[2], st));
-    interleave_kernel<<<grid, 256, 0, st>>>(nn, nvec, h->wsF, F, 0);
+    interleave_kernel<<<(unsigned)((nn * nvec + 255) / 256), 256, 0, st>>>(nn, nvec, nvt, h->wsF, F, 0);
     RT_CUDA(cudaGetLastError());
     RT_CUDA(cudaEventRecord(h->ev[3], st));
     h->ev_valid = true;

@@ -48,8 +48,10 @@ constexpr int NSUB = 3;                       // nprim pairs in {1, 3, 9}
 constexpr int NKETCLASS = 3 * NSUB;           // ket class id = pairclass * NSUB + sub
 __host__ __device__ inline int sub_to_np(int sub) { return sub == 0 ? 1 : (sub == 1 ? 3 : 9); }
 
-// Unique (unordered) pairs of one ket class, sorted by Schwarz bound descending; thread-owned side.
-// Primitive data is SoA: prim[(k * PRIM_STRIDE + f) * n + q] so that consecutive kets coalesce.
+// Unique (unordered) pairs of one pair class (pair type x contraction sub-class), sorted by Schwarz bound
+// descending.  The same list serves as the BRA list of the evaluation kernels (block-uniform side, AoS rows
+// staged in shared memory) and as the KET list (thread-owned side, SoA so that consecutive kets coalesce).
+// Primitive data SoA: prim[(k * PRIM_STRIDE + f) * n + q]; AoS: prim_aos[(q * np + k) * PRIM_STRIDE + f].
 struct KetClass {
     int n;                 // number of pairs
     int np;                // primitive pairs per pair (1, 3, 9)
@@ -58,15 +60,16 @@ struct KetClass {
     const int* ao_d;       // [n] AO offset of the second shell
     const int* same;       // [n] 1 if both shells are the same shell
     const double* prim;    // [np][PRIM_STRIDE][n]
+    const double* prim_aos;// [n][np][PRIM_STRIDE]
 };
 
-// Ordered bra record (block-uniform side): shell a fixed by the list, partner b varies.
+// Ordered bra record of the digestion kernels (block-uniform side): shell a fixed by the list, partner b varies.
 struct BraRec {
     double Q;              // Schwarz bound of the pair
     int ao_b;              // AO offset of partner shell b
-    int prim_off;          // first primitive-pair row in bra_prim (oriented a first)
-    int pos;               // position of the unordered pair inside its ket class list
-    int flags;             // bit0: canonical orientation (does the J work), bit1: a == b
+    int pos;               // position of the unordered pair inside its class list
+    int flags;             // bit0: canonical orientation (a is the pair's first shell; does the J work), bit1: a == b
+    int pad;
 };
 
 // All partners b of shell a with given l_b and contraction sub-class, sorted by Q descending.
@@ -74,7 +77,7 @@ struct AList {
     double Qmax;
     int ao_a;
     int rec_begin, rec_end;   // into BraRec array
-    int ketclass;             // ket class id of the (unordered) pairs in this list
+    int ketclass;             // class id of the (unordered) pairs in this list
     int np;                   // primitive pairs per record
 };
 
@@ -83,8 +86,31 @@ struct WorkItem {
     int ket0;                 // first ket (thread 0) of this block
 };
 
-struct JKLaunch {             // one kernel instantiation: ordered bra class x ket class
+// One block of the evaluation kernel: JK_BLOCK consecutive kets x bra pairs [p_begin, p_end) of the bra list.
+struct EvalItem {
+    int k0, p_begin, p_end;
+};
+
+// A segment = all unique quartets (bra pair class x ket pair class).  The evaluation kernel writes the
+// contracted integrals of the segment to the staging buffer in HBM, batch by batch; a batch is one bra pair
+// x 32 consecutive kets, laid out [component][lane] so that both sides coalesce:
+//   value(pair p, ket q, component i) at  ((batch_base[p] + (q >> 5) - (same ? p >> 5 : 0)) * NI + i) * 32 + (q & 31)
+// A quartet exists iff Q_p Q_q >= tau and (bra class != ket class or p <= q).
+struct Segment {
+    int kc_bra, kc_ket;       // class ids (pair type * NSUB + sub) of the bra and ket lists
+    int la, lb, lc, ld;       // canonical angular momenta (la >= lb, lc >= ld)
+    int ni;                   // integrals per quartet
+    long long nbatch;         // 32-ket batches in the segment
+    long long nquartets;      // quartets actually evaluated (unique, screened)
+    const long long* batch_base;   // device [n_bra]
+    const EvalItem* items;    // device
+    int nitems;
+    int first_launch, nlaunch;     // digestion launches that read this segment
+};
+
+struct JKLaunch {             // one digestion kernel instantiation: ordered bra class x ket class
     int la, lb, lc, ld, ketclass;
+    int seg;
     int nwork;
     const WorkItem* work;     // device
 };
@@ -93,19 +119,18 @@ struct JKTables {
     KetClass kets[NKETCLASS];
     const BraRec* recs;
     const AList* alists;
-    const double* bra_prim;   // [nrows][PRIM_STRIDE] AoS
-    const double* boys;       // Boys table
+    const double2* boys[5];   // per total angular momentum L: rows {F_{L+7}(j/8), exp(-j/8)}
     double tau;
     int nao;
 };
 
 constexpr int JK_BLOCK = 128;
+constexpr int EVAL_MAX_ROWS = 288;     // bra primitive rows staged per evaluation block (32 pairs x 9 prims)
 
-// Boys table: rows at T0 = j / 8, j = 0..BOYS_NROW-1; row = F_0..F_11(T0), exp(-T0), padding.
-constexpr int BOYS_ROW = 16;
+// Boys grid: T0 = j / 8, j = 0..BOYS_NROW-1
 constexpr double BOYS_TMAX = 48.0;
 constexpr int BOYS_NROW = 385 + 1;
-void boys_table_host(std::vector<double>& tab);
+void boys_table_host(int L, std::vector<double>& tab);
 
 // ---------------------------------------------------------------------------------------------
 struct Handle {
@@ -120,6 +145,10 @@ struct Handle {
     // J/K tables
     JKTables tabs{};
     std::vector<JKLaunch> launches;
+    std::vector<Segment> segments;
+    double* eri_buf = nullptr;                 // HBM staging buffer of one segment's integrals
+    size_t eri_buf_n = 0;                      // doubles allocated
+    size_t eri_buf_need = 0;                   // doubles needed by the largest segment
     std::vector<void*> dev_allocs;             // everything to free
     // workspaces (grown on demand)
     double *wsY = nullptr, *wsT = nullptr, *wsF = nullptr, *wsZ = nullptr;
@@ -138,11 +167,14 @@ struct Handle {
 
 int jk_mark(Handle* h, cudaStream_t st);   // record the next event of the J/K timing log
 
-// jk_kernels.cu
-int jk_build(Handle* h, int nvec_total, int v0, int nv, const double* Tq, double* Fq, cudaStream_t st);
-int jk_nvec_chunk();
+// jk_eval.cu / jk_digest.cu
+// F += 2 J[T] - cx K[T] for all nvt (even) interleaved densities; F zeroed by the caller.
+int jk_build(Handle* h, int nvt, const double* Tq, double* Fq, cudaStream_t st);
+int eval_segment(Handle* h, const Segment& sg, cudaStream_t st);
+int digest_launch(Handle* h, const JKLaunch& L, const Segment& sg, int nvt, const double* Tq, double* Fq,
+                  cudaStream_t st);
 int schwarz_device(int pairclass, int npairs, const int* d_np, const int* d_off, const double* d_prim,
-                   const double* d_boys, double* d_Q, cudaStream_t st);
+                   const double2* d_boys /* table for L = 2 * pairclass */, double* d_Q, cudaStream_t st);
 
 // gemm_f64.cu: C(m,n) = alpha * sum_k A(m,k) B(k,n) + beta * C(m,n), fully strided, batched.
 struct GemmDesc {

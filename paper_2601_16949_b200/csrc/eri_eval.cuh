@@ -20,25 +20,33 @@ __host__ __device__ constexpr int hidx_plus(int t, int u, int v, int axis)
     return axis == 0 ? hidx(t + 1, u, v) : (axis == 1 ? hidx(t, u + 1, v) : hidx(t, u, v + 1));
 }
 
-// ---- Boys function F_0..F_L(T), pre-multiplied by `scale` ---------------------------------------------
-// T < 48: 8-term Taylor expansion of F_L about the nearest grid point T0 = j/8 (dF_n/dT = -F_{n+1}), then
-// downward recursion F_{n-1} = (2T F_n + e^-T)/(2n-1) with e^-T = e^-T0 e^(T0-T) (8-term Taylor).
+// ---- Boys function F_0..F_L(T) -------------------------------------------------------------------------
+// T < 48: nearest grid point T0 = j/8; ONE 16-byte table row {F_{L+7}(T0), e^-T0} (shared memory gather);
+//   the lower orders at T0 follow from the (stable) downward recursion F_{n-1} = (2 T0 F_n + e^-T0)/(2n-1),
+//   carried in the scaled form h_k = F_{L+k}(T0)/k! so that the Taylor sum F_L(T) = sum_k h_k (T0-T)^k
+//   (dF_n/dT = -F_{n+1}) is a plain Horner chain; then downward recursion at T with
+//   e^-T = e^-T0 e^(T0-T) (degree-8 Taylor, |T0-T| <= 1/16).
 // T >= 48: F_0 = sqrt(pi/T)/2, F_{n+1} = (2n+1) F_n / (2T) (the e^-T term is < 1e-20).
 template <int L>
-__device__ __forceinline__ void boys(double T, const double* __restrict__ tab, double (&F)[L + 1])
+__device__ __forceinline__ void boys(double T, const double2* __restrict__ tab, double (&F)[L + 1])
 {
     if (T < BOYS_TMAX) {
-        const int j = __double2int_rn(T * 8.0);
-        const double dx = (double)j * 0.125 - T;             // T0 - T, |dx| <= 1/16
-        const double* row = tab + j * BOYS_ROW;
-        double f = __ldg(row + L + 7) * (1.0 / 5040.0);
-        f = fma(f, dx, __ldg(row + L + 6) * (1.0 / 720.0));
-        f = fma(f, dx, __ldg(row + L + 5) * (1.0 / 120.0));
-        f = fma(f, dx, __ldg(row + L + 4) * (1.0 / 24.0));
-        f = fma(f, dx, __ldg(row + L + 3) * (1.0 / 6.0));
-        f = fma(f, dx, __ldg(row + L + 2) * 0.5);
-        f = fma(f, dx, __ldg(row + L + 1));
-        f = fma(f, dx, __ldg(row + L));
+        constexpr double MAGIC = 6755399441055744.0;          // 1.5 * 2^52: rounds to nearest integer
+        const double t = fma(T, 8.0, MAGIC);
+        const int j = __double2loint(t);
+        const double jd = t - MAGIC;
+        const double dx = fma(jd, 0.125, -T);                 // T0 - T, |dx| <= 1/16
+        const double2 row = tab[j];
+        const double twoT0 = jd * 0.25, e0 = row.y;
+        constexpr double fact[8] = {1.0, 1.0, 2.0, 6.0, 24.0, 120.0, 720.0, 5040.0};
+        double h = row.x * (1.0 / fact[7]);
+        double f = h;
+#pragma unroll
+        for (int k = 7; k >= 1; --k) {
+            const double den = 2.0 * (L + k) - 1.0;
+            h = fma(twoT0 * ((double)k / den), h, e0 * (1.0 / (den * fact[k - 1])));
+            f = fma(f, dx, h);
+        }
         F[L] = f;
         if (L > 0) {
             double e = 1.0 / 40320.0;
@@ -50,7 +58,7 @@ __device__ __forceinline__ void boys(double T, const double* __restrict__ tab, d
             e = fma(e, dx, 0.5);
             e = fma(e, dx, 1.0);
             e = fma(e, dx, 1.0);
-            e *= __ldg(row + 12);
+            e *= e0;
             const double t2 = 2.0 * T;
 #pragma unroll
             for (int n = L; n >= 1; --n) F[n - 1] = fma(t2, F[n], e) * (1.0 / (2 * n - 1));
@@ -67,7 +75,7 @@ __device__ __forceinline__ void boys(double T, const double* __restrict__ tab, d
 // ---- Hermite Coulomb integrals R^0_{tuv}, |tuv| <= L, scaled by pref -----------------------------------
 template <int L>
 __device__ __forceinline__ void hermite_R(double pref, double alpha, double X, double Y, double Z,
-                                          const double* __restrict__ tab, double (&R0)[nherm(L)])
+                                          const double2* __restrict__ tab, double (&R0)[nherm(L)])
 {
     double F[L + 1];
     boys<L>(alpha * (X * X + Y * Y + Z * Z), tab, F);
@@ -142,7 +150,7 @@ struct PrimPair {
 // index after the four stages is ((d*NC + c)*NB + b)*NA + a, so the caller reads I through eri_index().
 template <int LA, int LB, int LC, int LD>
 __device__ __forceinline__ void eri_prim_accum(const PrimPair& br, const PrimPair& kt,
-                                               const double* __restrict__ tab,
+                                               const double2* __restrict__ tab,
                                                double (&I)[(2 * LA + 1) * (2 * LB + 1) * (2 * LC + 1) * (2 * LD + 1)])
 {
     constexpr int L = LA + LB + LC + LD;

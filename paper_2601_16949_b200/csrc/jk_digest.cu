@@ -1,0 +1,370 @@
+// J/K digestion (DESIGN.md step a4; "Coulomb and Exchange terms" P:130): F += 2 J[T] - cx K[T] from the
+// contracted integrals the evaluation kernels staged in HBM (jk_eval.cu), for NV densities per launch.
+//
+// Work decomposition ("shell a fixed per block, ket pair owned by a thread"):
+//   block  = one a-list (all ordered bra pairs (a,b) for one shell a, one l_b, one contraction sub-class,
+//            sorted by Schwarz bound) x JK_BLOCK consecutive kets of one ket class
+//   thread = one unordered ket pair {c,d}; it walks the a-list while Q_ab Q_cd >= tau, streams the stored
+//            block (ab|cd) (coalesced, read-once) and digests it for NV densities:
+//              K_ac += I T_bd, K_ad += I T_bc, K_ca += I T_db, K_da += I T_cb      (registers, whole b loop)
+//              J_cd += I (T_ab + T_ba)                                             (registers, canonical bras)
+//              J_ab += I (T_cd + T_dc)                                             (warp butterfly reduce)
+//   Both orientations (a,b), (b,a) of a bra pair are separate records reading the SAME stored block, which
+//   keeps every exchange update in registers: no per-quartet global atomics, and no second evaluation.
+// Densities and results use the interleaved layout Tq[mu][nu][v] (v fastest), F likewise.
+#include <cstdlib>
+#include "common.cuh"
+
+namespace rttda {
+
+template <int NV>
+__device__ __forceinline__ void red_add(double* p, const double (&v)[NV], double s)
+{
+#pragma unroll
+    for (int i = 0; i < NV; ++i) atomicAdd(p + i, s * v[i]);
+}
+
+// Sum N (power of two <= 32) per-lane values over the warp with a transposing butterfly: at each of the first
+// log2(N) steps a lane keeps one half of its values and hands the other half to its partner, so N values cost
+// N - 1 + (5 - log2 N) shuffles instead of 5 N.  On return v[0] of lane l is the warp total of value index
+// warp_reduce_owner_index<N>(l); lanes that differ only in their low (5 - log2 N) bits hold the same total.
+template <int N, int W, int OFF>
+__device__ __forceinline__ void warp_reduce_step(double (&v)[N], int lane)
+{
+    if constexpr (OFF >= 1) {
+        if constexpr (W > 1) {
+            constexpr int half = W / 2;
+            const bool upper = (lane & OFF) != 0;
+#pragma unroll
+            for (int j = 0; j < half; ++j) {
+                const double send = upper ? v[j] : v[j + half];
+                const double keep = upper ? v[j + half] : v[j];
+                v[j] = keep + __shfl_xor_sync(0xffffffffu, send, OFF);
+            }
+            warp_reduce_step<N, half, OFF / 2>(v, lane);
+        } else {
+            v[0] += __shfl_xor_sync(0xffffffffu, v[0], OFF);
+            warp_reduce_step<N, 1, OFF / 2>(v, lane);
+        }
+    }
+}
+template <int N>
+__device__ __forceinline__ double warp_reduce_multi(double (&v)[N], int lane)
+{
+    static_assert(N == 1 || N == 2 || N == 4 || N == 8 || N == 16 || N == 32, "N must be a power of two");
+    warp_reduce_step<N, N, 16>(v, lane);
+    return v[0];
+}
+template <int N>
+__device__ __forceinline__ int warp_reduce_owner_index(int lane)
+{
+    int idx = 0;
+    if (N >= 2 && (lane & 16)) idx += N / 2;
+    if (N >= 4 && (lane & 8)) idx += N / 4;
+    if (N >= 8 && (lane & 4)) idx += N / 8;
+    if (N >= 16 && (lane & 2)) idx += N / 16;
+    if (N >= 32 && (lane & 1)) idx += N / 32;
+    return idx;
+}
+
+constexpr int next_pow2(int n) { return n <= 1 ? 1 : (n <= 2 ? 2 : (n <= 4 ? 4 : (n <= 8 ? 8 : (n <= 16 ? 16 : 32)))); }
+
+struct DigestArgs {
+    JKTables tb;
+    const WorkItem* work;
+    const long long* batch_base;
+    const double* buf;
+    const double* Tq;
+    double* Fq;
+    double cx;
+    int ketclass, same, nvt, v0;
+};
+
+template <int NV>
+struct VecLoad {
+    __device__ static __forceinline__ void ld(const double* __restrict__ p, double (&out)[NV])
+    {
+        if (NV % 2 == 0) {
+            const double2* p2 = reinterpret_cast<const double2*>(p);
+#pragma unroll
+            for (int i = 0; i < NV / 2; ++i) {
+                const double2 x = __ldg(p2 + i);
+                out[2 * i] = x.x; out[2 * i + 1] = x.y;
+            }
+        } else {
+#pragma unroll
+            for (int i = 0; i < NV; ++i) out[i] = __ldg(p + i);
+        }
+    }
+};
+
+// Stored component order (jk_eval.cu): canonical pair orientation (first shell = higher l), eri_index of
+// eri_eval.cuh: ((d * NC + c) * N2 + c2) * N1 + c1 with (c1, c2) the components of the canonical first/second
+// shell.
+template <int LA, int LB, int LC, int LD, int NV>
+__global__ void __launch_bounds__(JK_BLOCK)
+digest_kernel(DigestArgs g)
+{
+    constexpr int NA = 2 * LA + 1, NB = 2 * LB + 1, NC = 2 * LC + 1, ND = 2 * LD + 1;
+    constexpr int NI = NA * NB * NC * ND;
+    const JKTables& tb = g.tb;
+    const WorkItem wi = g.work[blockIdx.x];
+    const AList al = tb.alists[wi.alist];
+    const KetClass& kc = tb.kets[g.ketclass];
+    const int q = wi.ket0 + threadIdx.x;
+    const bool active = q < kc.n;
+    const int qq = active ? q : kc.n - 1;
+    const double Qq = active ? __ldg(kc.Q + qq) : 0.0;
+    const int aoC = __ldg(kc.ao_c + qq), aoD = __ldg(kc.ao_d + qq);
+    const bool cd_same = __ldg(kc.same + qq) != 0;
+    const bool same_class = g.same != 0;
+    const int aoA = al.ao_a;
+    const size_t nao = tb.nao;
+    const int nvt = g.nvt;
+    const double* Tv = g.Tq + g.v0;
+    double* Fv = g.Fq + g.v0;
+    const size_t rs = nao * nvt;          // row stride of Tq / Fq
+    const int lane = threadIdx.x & 31;
+#define TQ(mu, nu) (Tv + (size_t)(mu) * rs + (size_t)(nu) * nvt)
+
+    // S_cd = T_cd + T_dc for the J_ab update
+    double Scd[NC][ND][NV];
+#pragma unroll
+    for (int c = 0; c < NC; ++c)
+#pragma unroll
+        for (int d = 0; d < ND; ++d) {
+            double x[NV], y[NV];
+            VecLoad<NV>::ld(TQ(aoC + c, aoD + d), x);
+            VecLoad<NV>::ld(TQ(aoD + d, aoC + c), y);
+#pragma unroll
+            for (int v = 0; v < NV; ++v) Scd[c][d][v] = x[v] + y[v];
+        }
+
+    double Kac[NA][NC][NV], Kad[NA][ND][NV], Kca[NC][NA][NV], Kda[ND][NA][NV], Jcd[NC][ND][NV];
+#pragma unroll
+    for (int v = 0; v < NV; ++v) {
+#pragma unroll
+        for (int a = 0; a < NA; ++a) {
+#pragma unroll
+            for (int c = 0; c < NC; ++c) Kac[a][c][v] = Kca[c][a][v] = 0.0;
+#pragma unroll
+            for (int d = 0; d < ND; ++d) Kad[a][d][v] = Kda[d][a][v] = 0.0;
+        }
+#pragma unroll
+        for (int c = 0; c < NC; ++c)
+#pragma unroll
+            for (int d = 0; d < ND; ++d) Jcd[c][d][v] = 0.0;
+    }
+
+    for (int r = al.rec_begin; r < al.rec_end; ++r) {
+        const BraRec br = tb.recs[r];
+        const bool ok = active && (br.Q * Qq >= tb.tau) && (!same_class || br.pos <= q);
+        if (!__any_sync(0xffffffffu, ok)) break;
+        const bool canonical = (br.flags & 1) != 0;
+        const bool ab_same = (br.flags & 2) != 0;
+        const int aoB = br.ao_b;
+        const long long batch = __ldg(g.batch_base + br.pos) + (q >> 5) - (same_class ? (br.pos >> 5) : 0);
+        const double* src = g.buf + (size_t)batch * (NI * 32) + lane;
+        // degeneracy weights: 1/2 if the ket is a diagonal pair, 1/2 if bra pair == ket pair
+        const double wsame = (same_class && br.pos == q) ? 0.5 : 1.0;
+        const double wk = ok ? wsame * (cd_same ? 0.5 : 1.0) : 0.0;
+        // J_cd needs wsame * w_ab instead of wk
+        const double fix = (cd_same ? 2.0 : 1.0) * (ab_same ? 0.5 : 1.0);
+        // stored block is (first, second | c d) of the canonical orientation
+        const bool flip = (LA < LB) || (LA == LB && !canonical);
+
+#pragma unroll
+        for (int b = 0; b < NB; ++b) {
+            double tbd[ND][NV], tdb[ND][NV], tbc[NC][NV], tcb[NC][NV];
+            if (ok) {
+#pragma unroll
+                for (int d = 0; d < ND; ++d) {
+                    VecLoad<NV>::ld(TQ(aoB + b, aoD + d), tbd[d]);
+                    VecLoad<NV>::ld(TQ(aoD + d, aoB + b), tdb[d]);
+                }
+#pragma unroll
+                for (int c = 0; c < NC; ++c) {
+                    VecLoad<NV>::ld(TQ(aoB + b, aoC + c), tbc[c]);
+                    VecLoad<NV>::ld(TQ(aoC + c, aoB + b), tcb[c]);
+                }
+            } else {
+#pragma unroll
+                for (int v = 0; v < NV; ++v) {
+#pragma unroll
+                    for (int d = 0; d < ND; ++d) tbd[d][v] = tdb[d][v] = 0.0;
+#pragma unroll
+                    for (int c = 0; c < NC; ++c) tbc[c][v] = tcb[c][v] = 0.0;
+                }
+            }
+#pragma unroll
+            for (int a = 0; a < NA; ++a) {
+                double sab[NV], jab[next_pow2(NV)];
+                if (canonical) {
+                    double x[NV], y[NV];
+                    VecLoad<NV>::ld(TQ(aoA + a, aoB + b), x);
+                    VecLoad<NV>::ld(TQ(aoB + b, aoA + a), y);
+#pragma unroll
+                    for (int v = 0; v < NV; ++v) sab[v] = fix * (x[v] + y[v]);
+                } else {
+#pragma unroll
+                    for (int v = 0; v < NV; ++v) sab[v] = 0.0;
+                }
+#pragma unroll
+                for (int v = 0; v < next_pow2(NV); ++v) jab[v] = 0.0;
+                // stored index of (a, b, c, d): first-shell component runs fastest
+                const int i_ab = flip ? (a * NB + b) : (b * NA + a);   // = c2 * N1 + c1
+#pragma unroll
+                for (int d = 0; d < ND; ++d)
+#pragma unroll
+                    for (int c = 0; c < NC; ++c) {
+                        const int i = (d * NC + c) * (NA * NB) + i_ab;
+                        const double x = ok ? wk * __ldcs(src + i * 32) : 0.0;
+#pragma unroll
+                        for (int v = 0; v < NV; ++v) {
+                            Kac[a][c][v] = fma(x, tbd[d][v], Kac[a][c][v]);
+                            Kca[c][a][v] = fma(x, tdb[d][v], Kca[c][a][v]);
+                            Kad[a][d][v] = fma(x, tbc[c][v], Kad[a][d][v]);
+                            Kda[d][a][v] = fma(x, tcb[c][v], Kda[d][a][v]);
+                            Jcd[c][d][v] = fma(x, sab[v], Jcd[c][d][v]);
+                            jab[v] = fma(x, Scd[c][d][v], jab[v]);
+                        }
+                    }
+                // ---- Coulomb J_ab: only the canonical orientation of the bra pair does it (uniform branch)
+                if (canonical) {
+                    constexpr int NP = next_pow2(NV);
+                    const double tot = warp_reduce_multi<NP>(jab, lane);
+                    const int v = warp_reduce_owner_index<NP>(lane);
+                    if (v < NV && tot != 0.0 && (lane & (32 / NP - 1)) == 0) {
+                        atomicAdd(Fv + (size_t)(aoA + a) * rs + (size_t)(aoB + b) * nvt + v, 2.0 * tot);
+                        if (!ab_same)
+                            atomicAdd(Fv + (size_t)(aoB + b) * rs + (size_t)(aoA + a) * nvt + v, 2.0 * tot);
+                    }
+                }
+            }
+        }
+    }
+#undef TQ
+    if (!active) return;
+    // ---- flush the register accumulators: F += 2 J - cx K
+    const double cx = g.cx;
+#pragma unroll
+    for (int a = 0; a < NA; ++a) {
+#pragma unroll
+        for (int c = 0; c < NC; ++c) {
+            red_add<NV>(Fv + (size_t)(aoA + a) * rs + (size_t)(aoC + c) * nvt, Kac[a][c], -cx);
+            red_add<NV>(Fv + (size_t)(aoC + c) * rs + (size_t)(aoA + a) * nvt, Kca[c][a], -cx);
+        }
+#pragma unroll
+        for (int d = 0; d < ND; ++d) {
+            red_add<NV>(Fv + (size_t)(aoA + a) * rs + (size_t)(aoD + d) * nvt, Kad[a][d], -cx);
+            red_add<NV>(Fv + (size_t)(aoD + d) * rs + (size_t)(aoA + a) * nvt, Kda[d][a], -cx);
+        }
+    }
+#pragma unroll
+    for (int c = 0; c < NC; ++c)
+#pragma unroll
+        for (int d = 0; d < ND; ++d) {
+            red_add<NV>(Fv + (size_t)(aoC + c) * rs + (size_t)(aoD + d) * nvt, Jcd[c][d], 2.0);
+            if (!cd_same) red_add<NV>(Fv + (size_t)(aoD + d) * rs + (size_t)(aoC + c) * nvt, Jcd[c][d], 2.0);
+        }
+}
+
+// ---------------------------------------------------------------------------------------------------
+// Densities per digestion launch: as many as the register file holds for the class (accumulators per density:
+// 2 NA (NC + ND) + 2 NC ND doubles).  More launches only re-read the staged integrals.
+static int class_nv_max(int la, int lb, int lc, int ld)
+{
+    const int na = 2 * la + 1, nc = 2 * lc + 1, nd = 2 * ld + 1;
+    (void)lb;
+    const int per_v = 2 * na * (nc + nd) + 2 * nc * nd;
+    static int cap[3] = {0, 0, 0};
+    if (cap[0] == 0) {                 // tuning knobs (defaults measured on B200)
+        const char* e0 = getenv("RTTDA_NV_A"); const char* e1 = getenv("RTTDA_NV_B"); const char* e2 = getenv("RTTDA_NV_C");
+        cap[0] = e0 ? atoi(e0) : 6; cap[1] = e1 ? atoi(e1) : 4; cap[2] = e2 ? atoi(e2) : 2;
+    }
+    if (per_v <= 8) return cap[0];     // ss|ss, sp|ss
+    if (per_v <= 16) return cap[1];    // ps|ss, pp|ss, sp|ps
+    if (per_v <= 32) return cap[2];    // ps|ps, pp|ps
+    return 1;                          // pp|pp
+}
+
+template <int LA, int LB, int LC, int LD, int NV>
+static int launch_digest_nv(Handle* h, const JKLaunch& L, const Segment& sg, int nvt, int v0, const double* Tq,
+                            double* Fq, cudaStream_t st)
+{
+    DigestArgs g;
+    g.tb = h->tabs;
+    g.work = L.work;
+    g.batch_base = sg.batch_base;
+    g.buf = h->eri_buf;
+    g.Tq = Tq; g.Fq = Fq; g.cx = h->cx;
+    g.ketclass = L.ketclass; g.same = (sg.kc_bra == sg.kc_ket); g.nvt = nvt; g.v0 = v0;
+    digest_kernel<LA, LB, LC, LD, NV><<<dim3(L.nwork), dim3(JK_BLOCK), 0, st>>>(g);
+    h->kernel_launches++;
+    RT_CUDA(cudaGetLastError());
+    return RTTDA_OK;
+}
+
+template <int LA, int LB, int LC, int LD>
+static int launch_digest(Handle* h, const JKLaunch& L, const Segment& sg, int nvt, const double* Tq, double* Fq,
+                         cudaStream_t st)
+{
+    constexpr int NA = 2 * LA + 1, NC = 2 * LC + 1, ND = 2 * LD + 1;
+    constexpr int PER_V = 2 * NA * (NC + ND) + 2 * NC * ND;
+    const int nvmax = class_nv_max(LA, LB, LC, LD);
+    int v0 = 0;
+    while (v0 < nvt) {
+        const int left = nvt - v0;
+        int nv = left < nvmax ? left : nvmax;
+        if (nv == 7) nv = 6;
+        if (nv == 5 || nv == 3) nv -= 1;
+        if constexpr (PER_V <= 8) {
+            if (nv == 8) { RT_TRY((launch_digest_nv<LA, LB, LC, LD, 8>(h, L, sg, nvt, v0, Tq, Fq, st))); v0 += 8; continue; }
+        }
+        if constexpr (PER_V <= 16) {
+            if (nv >= 6) { RT_TRY((launch_digest_nv<LA, LB, LC, LD, 6>(h, L, sg, nvt, v0, Tq, Fq, st))); v0 += 6; continue; }
+            if (nv >= 4) { RT_TRY((launch_digest_nv<LA, LB, LC, LD, 4>(h, L, sg, nvt, v0, Tq, Fq, st))); v0 += 4; continue; }
+        }
+        if constexpr (PER_V <= 32) {
+            if (nv >= 2) { RT_TRY((launch_digest_nv<LA, LB, LC, LD, 2>(h, L, sg, nvt, v0, Tq, Fq, st))); v0 += 2; continue; }
+        }
+        RT_TRY((launch_digest_nv<LA, LB, LC, LD, 1>(h, L, sg, nvt, v0, Tq, Fq, st)));
+        v0 += 1;
+    }
+    return RTTDA_OK;
+}
+
+int digest_launch(Handle* h, const JKLaunch& L, const Segment& sg, int nvt, const double* Tq, double* Fq,
+                  cudaStream_t st)
+{
+    if (L.nwork == 0) return RTTDA_OK;
+    const int key = L.la * 8 + L.lb * 4 + L.lc * 2 + L.ld;
+    switch (key) {
+        case 0:  return launch_digest<0, 0, 0, 0>(h, L, sg, nvt, Tq, Fq, st);
+        case 8:  return launch_digest<1, 0, 0, 0>(h, L, sg, nvt, Tq, Fq, st);
+        case 4:  return launch_digest<0, 1, 0, 0>(h, L, sg, nvt, Tq, Fq, st);
+        case 10: return launch_digest<1, 0, 1, 0>(h, L, sg, nvt, Tq, Fq, st);
+        case 6:  return launch_digest<0, 1, 1, 0>(h, L, sg, nvt, Tq, Fq, st);
+        case 12: return launch_digest<1, 1, 0, 0>(h, L, sg, nvt, Tq, Fq, st);
+        case 14: return launch_digest<1, 1, 1, 0>(h, L, sg, nvt, Tq, Fq, st);
+        case 15: return launch_digest<1, 1, 1, 1>(h, L, sg, nvt, Tq, Fq, st);
+        default: set_error("digest: unsupported class"); return RTTDA_EINVAL;
+    }
+}
+
+// One ERI pass: for every segment, evaluate its quartets once into the staging buffer, then digest them for all
+// nvt densities.  Fq must be zeroed by the caller; nvt must be even (16-byte density slots).
+int jk_build(Handle* h, int nvt, const double* Tq, double* Fq, cudaStream_t st)
+{
+    RT_CHECK(nvt >= 2 && nvt % 2 == 0, "jk_build: the interleaved density count must be even");
+    RT_TRY(ensure_ws(h, &h->eri_buf, &h->eri_buf_n, h->eri_buf_need));
+    for (const Segment& sg : h->segments) {
+        if (sg.nitems == 0) continue;
+        RT_TRY(eval_segment(h, sg, st));
+        for (int l = sg.first_launch; l < sg.first_launch + sg.nlaunch; ++l)
+            RT_TRY(digest_launch(h, h->launches[l], sg, nvt, Tq, Fq, st));
+    }
+    return RTTDA_OK;
+}
+
+}  // namespace rttda

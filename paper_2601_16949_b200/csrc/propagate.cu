@@ -42,10 +42,12 @@ int sigma_impl(Handle* h, int nvec, const double* X, long long ldx, double* sigm
                cudaStream_t st)
 {
     const size_t N = h->nao, no = h->nocc, nv = h->nvirt;
+    const int nvt = (nvec + 1) & ~1;            // interleaved density slots are 16-byte multiples
     RT_TRY(ensure_ws(h, &h->wsY, &h->wsY_n, (size_t)nvec * no * N));
-    RT_TRY(ensure_ws(h, &h->wsT, &h->wsT_n, (size_t)nvec * N * N));
-    RT_TRY(ensure_ws(h, &h->wsF, &h->wsF_n, (size_t)nvec * N * N));
+    RT_TRY(ensure_ws(h, &h->wsT, &h->wsT_n, (size_t)nvt * N * N));
+    RT_TRY(ensure_ws(h, &h->wsF, &h->wsF_n, (size_t)nvt * N * N));
     RT_CUDA(cudaEventRecord(h->ev[0], st));
+    if (nvt != nvec) RT_CUDA(cudaMemsetAsync(h->wsT, 0, (size_t)nvt * N * N * sizeof(double), st));
     // a1: Y_v = X_v C_v^T  [no][N];  T[mu][nu][v] = sum_j C_o[mu][j] Y_v[j][nu]
     GemmDesc g{};
     g.alpha = 1.0; g.beta = 0.0; g.batch = nvec;
@@ -57,21 +59,19 @@ int sigma_impl(Handle* h, int nvec, const double* X, long long ldx, double* sigm
     g.M = (int)N; g.N = (int)N; g.K = (int)no;
     g.A = h->C_occ; g.sam = no; g.sak = 1; g.sabatch = 0;
     g.B = h->wsY; g.sbk = N; g.sbn = 1; g.sbbatch = no * N;
-    g.C = h->wsT; g.scm = N * nvec; g.scn = nvec; g.scbatch = 1;
+    g.C = h->wsT; g.scm = N * nvt; g.scn = nvt; g.scbatch = 1;
     RT_TRY(gemm_f64(g, st));
     RT_CUDA(cudaEventRecord(h->ev[1], st));
     RT_TRY(jk_mark(h, st));
-    // a3-a4: F = 2 J[T] - cx K[T], interleaved layout, chunks of densities per ERI pass
-    RT_CUDA(cudaMemsetAsync(h->wsF, 0, (size_t)nvec * N * N * sizeof(double), st));
-    const int chunk = jk_nvec_chunk();
-    for (int v0 = 0; v0 < nvec; v0 += chunk)
-        RT_TRY(jk_build(h, nvec, v0, std::min(chunk, nvec - v0), h->wsT, h->wsF, st));
+    // a3-a4: F = 2 J[T] - cx K[T], interleaved layout; one ERI pass serves all densities
+    RT_CUDA(cudaMemsetAsync(h->wsF, 0, (size_t)nvt * N * N * sizeof(double), st));
+    RT_TRY(jk_build(h, nvt, h->wsT, h->wsF, st));
     RT_TRY(jk_mark(h, st));
     RT_CUDA(cudaEventRecord(h->ev[2], st));
     // a5: Z_v = C_o^T F_v [no][N];  sigma_v = deps o X_v + Z_v C_v
     g.M = (int)no; g.N = (int)N; g.K = (int)N; g.batch = nvec;
     g.A = h->C_occ; g.sam = 1; g.sak = no; g.sabatch = 0;
-    g.B = h->wsF; g.sbk = N * nvec; g.sbn = nvec; g.sbbatch = 1;
+    g.B = h->wsF; g.sbk = N * nvt; g.sbn = nvt; g.sbbatch = 1;
     g.C = h->wsY; g.scm = N; g.scn = 1; g.scbatch = no * N;
     RT_TRY(gemm_f64(g, st));
     const long long tot = (long long)h->ncsf * nvec;

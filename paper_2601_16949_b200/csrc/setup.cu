@@ -12,27 +12,22 @@
 namespace rttda {
 
 // ---------------------------------------------------------------------------------------------- Boys table
-// F_n(T0), n = 0..11, by the series at n = 11 + downward recursion (T0 <= 48), in long double.
-void boys_table_host(std::vector<double>& tab)
+// Rows {F_{L+7}(T0), exp(-T0)} at T0 = j/8 (eri_eval.cuh boys<L>): series for F_{L+7} (T0 <= 48), in long double.
+void boys_table_host(int L, std::vector<double>& tab)
 {
-    tab.assign((size_t)BOYS_NROW * BOYS_ROW, 0.0);
+    tab.assign((size_t)BOYS_NROW * 2, 0.0);
+    const int n = L + 7;
     for (int j = 0; j < BOYS_NROW; ++j) {
         const long double T = (long double)j / 8.0L;
-        const int nmax = 11;
-        long double term = 1.0L / (2 * nmax + 1), sum = term;
+        long double term = 1.0L / (2 * n + 1), sum = term;
         for (int k = 1; k < 4000; ++k) {
-            term *= 2.0L * T / (2 * nmax + 2 * k + 1);
+            term *= 2.0L * T / (2 * n + 2 * k + 1);
             sum += term;
             if (term < 1e-21L * sum) break;
         }
         const long double emt = expl(-T);
-        long double f = emt * sum;
-        tab[(size_t)j * BOYS_ROW + nmax] = (double)f;
-        for (int n = nmax; n >= 1; --n) {
-            f = (2.0L * T * f + emt) / (2 * n - 1);
-            tab[(size_t)j * BOYS_ROW + n - 1] = (double)f;
-        }
-        tab[(size_t)j * BOYS_ROW + 12] = (double)emt;
+        tab[2 * (size_t)j] = (double)(emt * sum);
+        tab[2 * (size_t)j + 1] = (double)emt;
     }
 }
 
@@ -216,9 +211,13 @@ int create_impl(Handle* h, const rttda_basis_t* basis, const double* C_occ, cons
     const size_t N = h->nao;
 
     // ---- Boys table
-    std::vector<double> boys;
-    boys_table_host(boys);
-    RT_TRY(upload(h, boys, &h->tabs.boys));
+    for (int L = 0; L <= 4; ++L) {
+        std::vector<double> boys;
+        boys_table_host(L, boys);
+        const double* d = nullptr;
+        RT_TRY(upload(h, boys, &d));
+        h->tabs.boys[L] = reinterpret_cast<const double2*>(d);
+    }
 
     // ---- candidate pairs and their primitive rows (canonical orientation), per pair class
     std::vector<Pair> pairs;
@@ -266,7 +265,7 @@ int create_impl(Handle* h, const rttda_basis_t* basis, const double* C_occ, cons
         RT_CUDA(cudaMemcpyAsync(d_np, cand_np[pc].data(), n * sizeof(int), cudaMemcpyHostToDevice, st));
         RT_CUDA(cudaMemcpyAsync(d_off, cand_off[pc].data(), n * sizeof(int), cudaMemcpyHostToDevice, st));
         RT_CUDA(cudaMemcpyAsync(d_prim, rows[pc].data(), rows[pc].size() * sizeof(double), cudaMemcpyHostToDevice, st));
-        RT_TRY(schwarz_device(pc, n, d_np, d_off, d_prim, h->tabs.boys, d_Q, st));
+        RT_TRY(schwarz_device(pc, n, d_np, d_off, d_prim, h->tabs.boys[2 * pc], d_Q, st));
         h->kernel_launches++;
         std::vector<double> Q(n);
         RT_CUDA(cudaMemcpyAsync(Q.data(), d_Q, n * sizeof(double), cudaMemcpyDeviceToHost, st));
@@ -297,6 +296,7 @@ int create_impl(Handle* h, const rttda_basis_t* basis, const double* C_occ, cons
         const int n = (int)v.size(), np = sub_to_np(kc % NSUB), pc = kc / NSUB;
         nkept += n;
         std::vector<double> soa((size_t)np * PRIM_STRIDE * std::max(n, 1), 0.0);
+        std::vector<double> aos((size_t)np * PRIM_STRIDE * std::max(n, 1), 0.0);
         std::vector<int> aoc(std::max(n, 1), 0), aod(std::max(n, 1), 0), same(std::max(n, 1), 0);
         hQ[kc].assign(std::max(n, 1), 0.0);
         for (int q = 0; q < n; ++q) {
@@ -306,7 +306,10 @@ int create_impl(Handle* h, const rttda_basis_t* basis, const double* C_occ, cons
             aoc[q] = H.ao[P.s1]; aod[q] = H.ao[P.s2]; same[q] = (P.s1 == P.s2);
             for (int k = 0; k < np; ++k)
                 for (int f = 0; f < PRIM_STRIDE; ++f)
+                {
                     soa[((size_t)k * PRIM_STRIDE + f) * n + q] = rows[pc][(size_t)(P.row + k) * PRIM_STRIDE + f];
+                    aos[((size_t)q * np + k) * PRIM_STRIDE + f] = rows[pc][(size_t)(P.row + k) * PRIM_STRIDE + f];
+                }
         }
         KetClass& K = h->tabs.kets[kc];
         K.n = n; K.np = np;
@@ -315,6 +318,7 @@ int create_impl(Handle* h, const rttda_basis_t* basis, const double* C_occ, cons
         RT_TRY(upload(h, aod, &K.ao_d));
         RT_TRY(upload(h, same, &K.same));
         RT_TRY(upload(h, soa, &K.prim));
+        RT_TRY(upload(h, aos, &K.prim_aos));
     }
 
     // ---- ordered bra records grouped into a-lists keyed by (shell a, l_b, sub)
@@ -328,7 +332,6 @@ int create_impl(Handle* h, const rttda_basis_t* basis, const double* C_occ, cons
         }
     std::vector<BraRec> recs;
     std::vector<AList> alists;
-    std::vector<double> bra_rows;
     std::vector<int> alist_la, alist_lb;
     for (auto& g : groups) {
         std::vector<Rec>& v = g.second;
@@ -344,8 +347,7 @@ int create_impl(Handle* h, const rttda_basis_t* basis, const double* C_occ, cons
             BraRec br;
             br.Q = P.Q; br.ao_b = H.ao[r.b]; br.pos = P.pos;
             br.flags = (r.canonical ? 1 : 0) | (r.a == r.b ? 2 : 0);
-            br.prim_off = (int)(bra_rows.size() / PRIM_STRIDE);
-            prim_rows(H, r.a, r.b, bra_rows);
+            br.pad = 0;
             recs.push_back(br);
         }
         al.rec_end = (int)recs.size();
@@ -355,57 +357,93 @@ int create_impl(Handle* h, const rttda_basis_t* basis, const double* C_occ, cons
     }
     RT_TRY(upload(h, recs, &h->tabs.recs));
     RT_TRY(upload(h, alists, &h->tabs.alists));
-    RT_TRY(upload(h, bra_rows, &h->tabs.bra_prim));
     h->tabs.tau = tau;
     h->tabs.nao = h->nao;
 
-    // ---- work lists, one per kernel instantiation
-    auto count_ge = [&](int kc, double thr) {       // kets with Q >= thr (Q sorted descending)
+    // ---- segments (bra pair class x ket pair class, unique quartets), their staging-buffer maps and the
+    //      evaluation / digestion work lists
+    auto count_ge = [&](int kc, double thr) {       // pairs of class kc with Q >= thr (Q sorted descending)
         const std::vector<double>& q = hQ[kc];
         const int n = h->tabs.kets[kc].n;
         return (int)(std::upper_bound(q.begin(), q.begin() + n, thr, [](double t, double x) { return t > x; }) - q.begin());
     };
-    double n_eval = 0, nprim_eval = 0, flops_eval_kernel = 0;
-    const int bra_classes[4][2] = {{0, 0}, {1, 0}, {0, 1}, {1, 1}};
+    auto nkets_of = [&](int kc_ket, double Qp) {    // kets q (a prefix of the list) with Qp Q_q >= tau
+        return tau > 0.0 ? count_ge(kc_ket, tau / Qp) : h->tabs.kets[kc_ket].n;
+    };
+    double n_eval = 0, nprim_eval = 0;
+    size_t buf_need = 1;
     h->launches.clear();
-    for (int bc = 3; bc >= 0; --bc) {
-        const int la = bra_classes[bc][0], lb = bra_classes[bc][1], pcb = la + lb;
-        for (int kc = NKETCLASS - 1; kc >= 0; --kc) {
-            const int pck = kc / NSUB;
-            if (pck > pcb || h->tabs.kets[kc].n == 0) continue;
-            const int lc = pck >= 1 ? 1 : 0, ld = pck == 2 ? 1 : 0;
-            std::vector<std::pair<double, WorkItem>> items;
-            for (int ai = 0; ai < (int)alists.size(); ++ai) {
-                if (alist_la[ai] != la || alist_lb[ai] != lb) continue;
-                const AList& al = alists[ai];
-                if (pck == pcb && al.ketclass > kc) continue;
-                const int nk = tau > 0.0 ? count_ge(kc, tau / al.Qmax) : h->tabs.kets[kc].n;
-                int q0 = 0;
-                if (al.ketclass == kc) q0 = (recs[al.rec_begin].pos / JK_BLOCK) * JK_BLOCK;
-                // exact evaluation counts of this a-list against this ket class
-                for (int r = al.rec_begin; r < al.rec_end; ++r) {
-                    const int nkr = tau > 0.0 ? count_ge(kc, tau / recs[r].Q) : h->tabs.kets[kc].n;
-                    const int lo = (al.ketclass == kc) ? recs[r].pos : 0;
-                    if (nkr > lo) {
-                        n_eval += nkr - lo;
-                        nprim_eval += (double)(nkr - lo) * al.np * h->tabs.kets[kc].np;
-                        flops_eval_kernel += (double)(nkr - lo) * al.np * h->tabs.kets[kc].np * flops_prim(la, lb, lc, ld);
-                    }
+    h->segments.clear();
+    for (int kcb = NKETCLASS - 1; kcb >= 0; --kcb)
+        for (int kck = NKETCLASS - 1; kck >= 0; --kck) {
+            const int pcb = kcb / NSUB, pck = kck / NSUB;
+            // unique quartets: higher pair type is the bra; within a type the lower class id; within a class p <= q
+            if (pck > pcb || (pck == pcb && kcb > kck)) continue;
+            const int nb = h->tabs.kets[kcb].n, nk = h->tabs.kets[kck].n;
+            if (nb == 0 || nk == 0) continue;
+            const bool same = (kcb == kck);
+            Segment sg{};
+            sg.kc_bra = kcb; sg.kc_ket = kck;
+            sg.la = pcb >= 1; sg.lb = pcb == 2; sg.lc = pck >= 1; sg.ld = pck == 2;
+            sg.ni = (2 * sg.la + 1) * (2 * sg.lb + 1) * (2 * sg.lc + 1) * (2 * sg.ld + 1);
+            // staging map: pair p owns the 32-ket batches covering kets [same ? p : 0, nk_p)
+            std::vector<long long> base(nb, 0);
+            long long nbatch = 0, nquart = 0;
+            for (int p = 0; p < nb; ++p) {
+                base[p] = nbatch;
+                const int nkp = nkets_of(kck, hQ[kcb][p]);
+                const int lo = same ? p : 0;
+                if (nkp > lo) {
+                    nbatch += ((nkp - 1) >> 5) - (lo >> 5) + 1;
+                    nquart += nkp - lo;
                 }
-                const double len = al.rec_end - al.rec_begin;
-                for (int k0 = q0; k0 < nk; k0 += JK_BLOCK)
-                    items.push_back({len * al.np, WorkItem{ai, k0}});
             }
-            std::stable_sort(items.begin(), items.end(), [](const auto& x, const auto& y) { return x.first > y.first; });
-            std::vector<WorkItem> w;
-            w.reserve(items.size());
-            for (auto& it : items) w.push_back(it.second);
-            JKLaunch L;
-            L.la = la; L.lb = lb; L.lc = lc; L.ld = ld; L.ketclass = kc; L.nwork = (int)w.size();
-            RT_TRY(upload(h, w, &L.work));
-            if (L.nwork) h->launches.push_back(L);
+            sg.nbatch = nbatch; sg.nquartets = nquart;
+            if (nquart == 0) continue;
+            n_eval += (double)nquart;
+            nprim_eval += (double)nquart * h->tabs.kets[kcb].np * h->tabs.kets[kck].np;
+            buf_need = std::max(buf_need, (size_t)nbatch * sg.ni * 32);
+            RT_TRY(upload(h, base, &sg.batch_base));
+            // evaluation blocks: JK_BLOCK kets x a run of bra pairs (rows staged in shared memory)
+            const int npb = h->tabs.kets[kcb].np;
+            const int G = std::min(JK_BLOCK, EVAL_MAX_ROWS / npb);
+            std::vector<EvalItem> items;
+            for (int k0 = 0; k0 < nk; k0 += JK_BLOCK) {
+                int hi = tau > 0.0 ? count_ge(kcb, tau / hQ[kck][k0]) : nb;   // bra pairs reaching this chunk
+                if (same) hi = std::min(hi, std::min(nb, k0 + JK_BLOCK));
+                for (int p0 = 0; p0 < hi; p0 += G) items.push_back(EvalItem{k0, p0, std::min(hi, p0 + G)});
+            }
+            sg.nitems = (int)items.size();
+            RT_TRY(upload(h, items, &sg.items));
+            // digestion launches: ordered bra classes (a-lists) of this bra pair class against the ket class
+            sg.first_launch = (int)h->launches.size();
+            for (int orient = 0; orient < 2; ++orient) {
+                if (orient == 1 && sg.la == sg.lb) break;          // ss and pp pairs: one ordered class
+                const int la = orient == 0 ? sg.la : sg.lb, lb = orient == 0 ? sg.lb : sg.la;
+                std::vector<std::pair<double, WorkItem>> witems;
+                for (int ai = 0; ai < (int)alists.size(); ++ai) {
+                    if (alist_la[ai] != la || alist_lb[ai] != lb || alists[ai].ketclass != kcb) continue;
+                    const AList& al = alists[ai];
+                    const int nkmax = nkets_of(kck, al.Qmax);
+                    const int q0 = same ? (recs[al.rec_begin].pos / JK_BLOCK) * JK_BLOCK : 0;
+                    const double len = al.rec_end - al.rec_begin;
+                    for (int k0 = q0; k0 < nkmax; k0 += JK_BLOCK) witems.push_back({len, WorkItem{ai, k0}});
+                }
+                std::stable_sort(witems.begin(), witems.end(), [](const auto& x, const auto& y) { return x.first > y.first; });
+                std::vector<WorkItem> w;
+                w.reserve(witems.size());
+                for (auto& it : witems) w.push_back(it.second);
+                JKLaunch L{};
+                L.la = la; L.lb = lb; L.lc = sg.lc; L.ld = sg.ld; L.ketclass = kck;
+                L.seg = (int)h->segments.size();
+                L.nwork = (int)w.size();
+                RT_TRY(upload(h, w, &L.work));
+                h->launches.push_back(L);
+            }
+            sg.nlaunch = (int)h->launches.size() - sg.first_launch;
+            h->segments.push_back(sg);
         }
-    }
+    h->eri_buf_need = buf_need;
 
     // ---- R14 counts: unique quartets with Q_ab Q_cd >= tau, and the flop model on them
     {
@@ -440,7 +478,8 @@ int create_impl(Handle* h, const rttda_basis_t* basis, const double* C_occ, cons
     h->info[RTTDA_INFO_NPRIM_EVAL] = nprim_eval;
     h->info[RTTDA_INFO_JK_LAUNCHES] = (double)h->launches.size();
     h->info[RTTDA_INFO_QMAX] = Qmax;
-    h->info[RTTDA_INFO_NVEC_CHUNK] = jk_nvec_chunk();
+    h->info[RTTDA_INFO_NVEC_CHUNK] = 0.0;
+    h->info[RTTDA_INFO_ERI_BUF_BYTES] = (double)buf_need * sizeof(double);
 
     // ---- MO coefficients, eps differences, dipoles
     auto dalloc = [&](double** p, size_t n) -> int {
