@@ -94,7 +94,9 @@ int rttda_destroy(rttda_handle_t hh)
     if (!h) return RTTDA_OK;
     cudaDeviceSynchronize();
     for (void* p : h->dev_allocs) cudaFree(p);
-    for (double* p : {h->wsY, h->wsT, h->wsF, h->wsZ, h->prop_ws, h->eri_buf}) if (p) cudaFree(p);
+    for (double* p : {h->wsY, h->wsT, h->wsF, h->wsZ, h->prop_ws, h->eri_buf[0], h->eri_buf[1]}) if (p) cudaFree(p);
+    if (h->st_eval) cudaStreamDestroy(h->st_eval);
+    for (cudaEvent_t e : {h->ev_fork, h->ev_E[0], h->ev_E[1], h->ev_D[0], h->ev_D[1]}) if (e) cudaEventDestroy(e);
     for (auto& e : h->ev) if (e) cudaEventDestroy(e);
     for (auto& e : h->jk_ev) cudaEventDestroy(e);
     delete h;
@@ -132,7 +134,7 @@ int rttda_fock(rttda_handle_t hh, int32_t nvec, const double* T, double* F, void
     RT_CHECK(nvec >= 1, "rttda_fock: nvec < 1");
     cudaStream_t st = (cudaStream_t)stream;
     const long long nn = (long long)h->nao * h->nao;
-    const int nvt = (nvec + 1) & ~1;
+    const int nvt = padded_nvec(nvec);
     RT_TRY(ensure_ws(h, &h->wsT, &h->wsT_n, (size_t)nvt * nn));
     RT_TRY(ensure_ws(h, &h->wsF, &h->wsF_n, (size_t)nvt * nn));
     RT_CUDA(cudaEventRecord(h->ev[0], st));
@@ -141,7 +143,7 @@ int rttda_fock(rttda_handle_t hh, int32_t nvec, const double* T, double* F, void
     RT_CUDA(cudaEventRecord(h->ev[1], st));
     RT_TRY(jk_mark(h, st));
     RT_CUDA(cudaMemsetAsync(h->wsF, 0, (size_t)nvt * nn * sizeof(double), st));
-    RT_TRY(jk_build(h, nvt, h->wsT, h->wsF, st));
+    RT_TRY(jk_build(h, nvt, (nvec + 1) & ~1, h->wsT, h->wsF, st));
     RT_TRY(jk_mark(h, st));
     RT_CUDA(cudaEventRecord(h->ev[2], st));
     interleave_kernel<<<(unsigned)((nn * nvec + 255) / 256), 256, 0, st>>>(nn, nvec, nvt, h->wsF, F, 0);

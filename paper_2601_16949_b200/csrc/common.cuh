@@ -81,6 +81,33 @@ struct AList {
     int np;                   // primitive pairs per record
 };
 
+// Shell-blocked a-lists of the density-per-lane digestion kernel: SUPER_M (or 2) shells a_i of one shell class,
+// neighbours in space, share ONE walk over the union of their partners b, so that every density element gathered
+// for (b, c), (b, d) is reused for up to M quartets (a_i b|c d).
+constexpr int SUPER_MAX = 4;
+struct SHead {              // one partner shell b of the group
+    double Qmax;            // largest Schwarz bound over the members' pairs (a_i, b)
+    int ao_b;
+    int pad;
+};
+struct SMem {               // pair (a_i, b) of member i; Q = 0 if the pair is absent
+    double Q;
+    int pos;                // position of the unordered pair inside its class list
+    int flags;              // bit0 canonical, bit1 a == b, bit2 present
+};
+struct SAList {
+    double Qmax;
+    int ao_a[SUPER_MAX];      // AO offsets of the members (-1: slot unused)
+    int rec_begin, rec_end;   // into SHead array; members at [rec * M + i]
+    int ketclass, minpos;
+};
+struct SuperSet {             // device tables of one blocking factor M
+    int M;
+    const SHead* heads;
+    const SMem* mems;
+    const SAList* lists;
+};
+
 struct WorkItem {
     int alist;
     int ket0;                 // first ket (thread 0) of this block
@@ -113,12 +140,15 @@ struct JKLaunch {             // one digestion kernel instantiation: ordered bra
     int seg;
     int nwork;
     const WorkItem* work;     // device
+    int nswork[2];            // blocks over the shell-blocked a-lists, M = 2 and M = 4
+    const WorkItem* swork[2];
 };
 
 struct JKTables {
     KetClass kets[NKETCLASS];
     const BraRec* recs;
     const AList* alists;
+    SuperSet super[2];        // M = 2, M = 4
     const double2* boys[5];   // per total angular momentum L: rows {F_{L+7}(j/8), exp(-j/8)}
     double tau;
     int nao;
@@ -146,9 +176,12 @@ struct Handle {
     JKTables tabs{};
     std::vector<JKLaunch> launches;
     std::vector<Segment> segments;
-    double* eri_buf = nullptr;                 // HBM staging buffer of one segment's integrals
-    size_t eri_buf_n = 0;                      // doubles allocated
+    // HBM staging buffers (double-buffered: evaluation of segment k+1 overlaps digestion of segment k)
+    double* eri_buf[2] = {nullptr, nullptr};
+    size_t eri_buf_n[2] = {0, 0};              // doubles allocated
     size_t eri_buf_need = 0;                   // doubles needed by the largest segment
+    cudaStream_t st_eval = nullptr;            // evaluation kernels run here, digestion on the caller's stream
+    cudaEvent_t ev_fork = nullptr, ev_E[2] = {nullptr, nullptr}, ev_D[2] = {nullptr, nullptr};
     std::vector<void*> dev_allocs;             // everything to free
     // workspaces (grown on demand)
     double *wsY = nullptr, *wsT = nullptr, *wsF = nullptr, *wsZ = nullptr;
@@ -169,10 +202,11 @@ int jk_mark(Handle* h, cudaStream_t st);   // record the next event of the J/K t
 
 // jk_eval.cu / jk_digest.cu
 // F += 2 J[T] - cx K[T] for all nvt (even) interleaved densities; F zeroed by the caller.
-int jk_build(Handle* h, int nvt, const double* Tq, double* Fq, cudaStream_t st);
-int eval_segment(Handle* h, const Segment& sg, cudaStream_t st);
-int digest_launch(Handle* h, const JKLaunch& L, const Segment& sg, int nvt, const double* Tq, double* Fq,
-                  cudaStream_t st);
+int jk_build(Handle* h, int nvt, int nvec, const double* Tq, double* Fq, cudaStream_t st);
+int eval_segment(Handle* h, const Segment& sg, double* buf, cudaStream_t st);
+int digest_launch(Handle* h, const JKLaunch& L, const Segment& sg, const double* buf, int nvt, const double* Tq,
+                  double* Fq, cudaStream_t st);
+inline int padded_nvec(int nvec) { return nvec <= 2 ? 2 : (nvec <= 4 ? 4 : ((nvec + 7) & ~7)); }
 int schwarz_device(int pairclass, int npairs, const int* d_np, const int* d_off, const double* d_prim,
                    const double2* d_boys /* table for L = 2 * pairclass */, double* d_Q, cudaStream_t st);
 

@@ -270,6 +270,150 @@ digest_kernel(DigestArgs g)
 }
 
 // ---------------------------------------------------------------------------------------------------
+// Density-per-lane variant (used when a call carries >= 4 densities): a group of G consecutive lanes owns ONE ket
+// pair, lane v of the group serves density v.  A warp holds KW = 32 / G kets of its 32-ket batch at a time.  Every
+// density/Fock access is then a contiguous 8*G-byte run of one 64-byte aligned slot (sector-efficient gathers,
+// coalesced reductions), and a lane needs only one density's accumulators, so all densities of the call are
+// served by ONE read of the staged integrals for every class.
+template <int LA, int LB, int LC, int LD>
+__global__ void __launch_bounds__(JK_BLOCK)
+digest_v_kernel(DigestArgs g, int G, int KW)
+{
+    constexpr int NA = 2 * LA + 1, NB = 2 * LB + 1, NC = 2 * LC + 1, ND = 2 * LD + 1;
+    constexpr int NI = NA * NB * NC * ND;
+    const JKTables& tb = g.tb;
+    const WorkItem wi = g.work[blockIdx.x];
+    const AList al = tb.alists[wi.alist];
+    const KetClass& kc = tb.kets[g.ketclass];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int kg = lane / G, v = lane - kg * G;
+    const bool lane_used = kg < KW;
+    const bool same_class = g.same != 0;
+    const int aoA = al.ao_a;
+    const size_t nao = tb.nao;
+    const int nvt = g.nvt;
+    const size_t rs = nao * nvt;
+    const double* Tv = g.Tq + g.v0 + v;
+    double* Fv = g.Fq + g.v0 + v;
+    const double cx = g.cx;
+#define TQ(mu, nu) (Tv + (size_t)(mu) * rs + (size_t)(nu) * nvt)
+#define FQ(mu, nu) (Fv + (size_t)(mu) * rs + (size_t)(nu) * nvt)
+    const int qw = wi.ket0 + warp * 32;                  // this warp's 32-ket batch
+    for (int kbase = 0; kbase < 32; kbase += KW) {
+        const int q = qw + kbase + kg;
+        const bool active = lane_used && (kbase + kg < 32) && q < kc.n;
+        if (!__any_sync(0xffffffffu, active)) break;
+        const int qq = active ? q : kc.n - 1;
+        const double Qq = active ? __ldg(kc.Q + qq) : 0.0;
+        const int aoC = __ldg(kc.ao_c + qq), aoD = __ldg(kc.ao_d + qq);
+        const bool cd_same = __ldg(kc.same + qq) != 0;
+
+        double Scd[NC][ND], Jcd[NC][ND], Kac[NA][NC], Kca[NC][NA], Kad[NA][ND], Kda[ND][NA];
+#pragma unroll
+        for (int c = 0; c < NC; ++c)
+#pragma unroll
+            for (int d2 = 0; d2 < ND; ++d2) {
+                Scd[c][d2] = active ? __ldg(TQ(aoC + c, aoD + d2)) + __ldg(TQ(aoD + d2, aoC + c)) : 0.0;
+                Jcd[c][d2] = 0.0;
+            }
+#pragma unroll
+        for (int a = 0; a < NA; ++a) {
+#pragma unroll
+            for (int c = 0; c < NC; ++c) Kac[a][c] = Kca[c][a] = 0.0;
+#pragma unroll
+            for (int d2 = 0; d2 < ND; ++d2) Kad[a][d2] = Kda[d2][a] = 0.0;
+        }
+
+        for (int r = al.rec_begin; r < al.rec_end; ++r) {
+            const BraRec br = tb.recs[r];
+            const bool ok = active && (br.Q * Qq >= tb.tau) && (!same_class || br.pos <= q);
+            if (!__any_sync(0xffffffffu, ok)) break;
+            const bool canonical = (br.flags & 1) != 0;
+            const bool ab_same = (br.flags & 2) != 0;
+            const int aoB = br.ao_b;
+            const long long batch = __ldg(g.batch_base + br.pos) + (qw >> 5) - (same_class ? (br.pos >> 5) : 0);
+            const double* src = g.buf + (size_t)batch * (NI * 32) + (q & 31);
+            const double wsame = (same_class && br.pos == q) ? 0.5 : 1.0;
+            const double wk = ok ? wsame * (cd_same ? 0.5 : 1.0) : 0.0;
+            const double fix = (cd_same ? 2.0 : 1.0) * (ab_same ? 0.5 : 1.0);
+            const bool flip = (LA < LB) || (LA == LB && !canonical);
+#pragma unroll
+            for (int b = 0; b < NB; ++b) {
+                double tbd[ND], tdb[ND], tbc[NC], tcb[NC];
+#pragma unroll
+                for (int d2 = 0; d2 < ND; ++d2) {
+                    tbd[d2] = ok ? __ldg(TQ(aoB + b, aoD + d2)) : 0.0;
+                    tdb[d2] = ok ? __ldg(TQ(aoD + d2, aoB + b)) : 0.0;
+                }
+#pragma unroll
+                for (int c = 0; c < NC; ++c) {
+                    tbc[c] = ok ? __ldg(TQ(aoB + b, aoC + c)) : 0.0;
+                    tcb[c] = ok ? __ldg(TQ(aoC + c, aoB + b)) : 0.0;
+                }
+#pragma unroll
+                for (int a = 0; a < NA; ++a) {
+                    double sab = 0.0, jab = 0.0;
+                    if (canonical && lane_used)
+                        sab = fix * (__ldg(TQ(aoA + a, aoB + b)) + __ldg(TQ(aoB + b, aoA + a)));
+                    const int i_ab = flip ? (a * NB + b) : (b * NA + a);
+#pragma unroll
+                    for (int d2 = 0; d2 < ND; ++d2)
+#pragma unroll
+                        for (int c = 0; c < NC; ++c) {
+                            const int i = (d2 * NC + c) * (NA * NB) + i_ab;
+                            const double x = ok ? wk * __ldcs(src + i * 32) : 0.0;
+                            Kac[a][c] = fma(x, tbd[d2], Kac[a][c]);
+                            Kca[c][a] = fma(x, tdb[d2], Kca[c][a]);
+                            Kad[a][d2] = fma(x, tbc[c], Kad[a][d2]);
+                            Kda[d2][a] = fma(x, tcb[c], Kda[d2][a]);
+                            Jcd[c][d2] = fma(x, sab, Jcd[c][d2]);
+                            jab = fma(x, Scd[c][d2], jab);
+                        }
+                    if (canonical) {
+                        // sum J_ab over the KW kets of the warp (tree over the ket-group index), group 0 writes
+                        int n = KW;
+                        while (n > 1) {
+                            const int s = (n + 1) >> 1;
+                            const double y = __shfl_down_sync(0xffffffffu, jab, s * G);
+                            if (kg + s < n) jab += y;
+                            n = s;
+                        }
+                        if (kg == 0 && jab != 0.0) {
+                            atomicAdd(FQ(aoA + a, aoB + b), 2.0 * jab);
+                            if (!ab_same) atomicAdd(FQ(aoB + b, aoA + a), 2.0 * jab);
+                        }
+                    }
+                }
+            }
+        }
+        if (active) {
+#pragma unroll
+            for (int a = 0; a < NA; ++a) {
+#pragma unroll
+                for (int c = 0; c < NC; ++c) {
+                    atomicAdd(FQ(aoA + a, aoC + c), -cx * Kac[a][c]);
+                    atomicAdd(FQ(aoC + c, aoA + a), -cx * Kca[c][a]);
+                }
+#pragma unroll
+                for (int d2 = 0; d2 < ND; ++d2) {
+                    atomicAdd(FQ(aoA + a, aoD + d2), -cx * Kad[a][d2]);
+                    atomicAdd(FQ(aoD + d2, aoA + a), -cx * Kda[d2][a]);
+                }
+            }
+#pragma unroll
+            for (int c = 0; c < NC; ++c)
+#pragma unroll
+                for (int d2 = 0; d2 < ND; ++d2) {
+                    atomicAdd(FQ(aoC + c, aoD + d2), 2.0 * Jcd[c][d2]);
+                    if (!cd_same) atomicAdd(FQ(aoD + d2, aoC + c), 2.0 * Jcd[c][d2]);
+                }
+        }
+    }
+#undef TQ
+#undef FQ
+}
+
+// ---------------------------------------------------------------------------------------------------
 // Densities per digestion launch: as many as the register file holds for the class (accumulators per density:
 // 2 NA (NC + ND) + 2 NC ND doubles).  More launches only re-read the staged integrals.
 static int class_nv_max(int la, int lb, int lc, int ld)
@@ -289,14 +433,14 @@ static int class_nv_max(int la, int lb, int lc, int ld)
 }
 
 template <int LA, int LB, int LC, int LD, int NV>
-static int launch_digest_nv(Handle* h, const JKLaunch& L, const Segment& sg, int nvt, int v0, const double* Tq,
-                            double* Fq, cudaStream_t st)
+static int launch_digest_nv(Handle* h, const JKLaunch& L, const Segment& sg, const double* buf, int nvt, int v0,
+                            const double* Tq, double* Fq, cudaStream_t st)
 {
     DigestArgs g;
     g.tb = h->tabs;
     g.work = L.work;
     g.batch_base = sg.batch_base;
-    g.buf = h->eri_buf;
+    g.buf = buf;
     g.Tq = Tq; g.Fq = Fq; g.cx = h->cx;
     g.ketclass = L.ketclass; g.same = (sg.kc_bra == sg.kc_ket); g.nvt = nvt; g.v0 = v0;
     digest_kernel<LA, LB, LC, LD, NV><<<dim3(L.nwork), dim3(JK_BLOCK), 0, st>>>(g);
@@ -306,63 +450,90 @@ static int launch_digest_nv(Handle* h, const JKLaunch& L, const Segment& sg, int
 }
 
 template <int LA, int LB, int LC, int LD>
-static int launch_digest(Handle* h, const JKLaunch& L, const Segment& sg, int nvt, const double* Tq, double* Fq,
-                         cudaStream_t st)
+static int launch_digest(Handle* h, const JKLaunch& L, const Segment& sg, const double* buf, int nvt, int nvec,
+                         const double* Tq, double* Fq, cudaStream_t st)
 {
     constexpr int NA = 2 * LA + 1, NC = 2 * LC + 1, ND = 2 * LD + 1;
     constexpr int PER_V = 2 * NA * (NC + ND) + 2 * NC * ND;
+    static int vmode = -1;
+    if (vmode < 0) { const char* e = getenv("RTTDA_DIGEST_V"); vmode = e ? atoi(e) : 4; }
+    if (vmode > 0 && nvec >= vmode) {
+        // density-per-lane kernel: groups of G lanes per ket, chunks of at most 32 densities
+        for (int v0 = 0; v0 < nvec; v0 += 32) {
+            const int G = nvec - v0 < 32 ? nvec - v0 : 32;
+            DigestArgs g;
+            g.tb = h->tabs; g.work = L.work; g.batch_base = sg.batch_base; g.buf = buf;
+            g.Tq = Tq; g.Fq = Fq; g.cx = h->cx;
+            g.ketclass = L.ketclass; g.same = (sg.kc_bra == sg.kc_ket); g.nvt = nvt; g.v0 = v0;
+            digest_v_kernel<LA, LB, LC, LD><<<dim3(L.nwork), dim3(JK_BLOCK), 0, st>>>(g, G, 32 / G);
+            h->kernel_launches++;
+            RT_CUDA(cudaGetLastError());
+        }
+        return RTTDA_OK;
+    }
     const int nvmax = class_nv_max(LA, LB, LC, LD);
     int v0 = 0;
-    while (v0 < nvt) {
-        const int left = nvt - v0;
+    while (v0 < nvec) {                 // nvec is even; slots [nvec, nvt) are alignment padding, never touched
+        const int left = nvec - v0;
         int nv = left < nvmax ? left : nvmax;
         if (nv == 7) nv = 6;
         if (nv == 5 || nv == 3) nv -= 1;
         if constexpr (PER_V <= 8) {
-            if (nv == 8) { RT_TRY((launch_digest_nv<LA, LB, LC, LD, 8>(h, L, sg, nvt, v0, Tq, Fq, st))); v0 += 8; continue; }
+            if (nv == 8) { RT_TRY((launch_digest_nv<LA, LB, LC, LD, 8>(h, L, sg, buf, nvt, v0, Tq, Fq, st))); v0 += 8; continue; }
         }
         if constexpr (PER_V <= 16) {
-            if (nv >= 6) { RT_TRY((launch_digest_nv<LA, LB, LC, LD, 6>(h, L, sg, nvt, v0, Tq, Fq, st))); v0 += 6; continue; }
-            if (nv >= 4) { RT_TRY((launch_digest_nv<LA, LB, LC, LD, 4>(h, L, sg, nvt, v0, Tq, Fq, st))); v0 += 4; continue; }
+            if (nv >= 6) { RT_TRY((launch_digest_nv<LA, LB, LC, LD, 6>(h, L, sg, buf, nvt, v0, Tq, Fq, st))); v0 += 6; continue; }
+            if (nv >= 4) { RT_TRY((launch_digest_nv<LA, LB, LC, LD, 4>(h, L, sg, buf, nvt, v0, Tq, Fq, st))); v0 += 4; continue; }
         }
         if constexpr (PER_V <= 32) {
-            if (nv >= 2) { RT_TRY((launch_digest_nv<LA, LB, LC, LD, 2>(h, L, sg, nvt, v0, Tq, Fq, st))); v0 += 2; continue; }
+            if (nv >= 2) { RT_TRY((launch_digest_nv<LA, LB, LC, LD, 2>(h, L, sg, buf, nvt, v0, Tq, Fq, st))); v0 += 2; continue; }
         }
-        RT_TRY((launch_digest_nv<LA, LB, LC, LD, 1>(h, L, sg, nvt, v0, Tq, Fq, st)));
+        RT_TRY((launch_digest_nv<LA, LB, LC, LD, 1>(h, L, sg, buf, nvt, v0, Tq, Fq, st)));
         v0 += 1;
     }
     return RTTDA_OK;
 }
 
-int digest_launch(Handle* h, const JKLaunch& L, const Segment& sg, int nvt, const double* Tq, double* Fq,
-                  cudaStream_t st)
+int digest_launch(Handle* h, const JKLaunch& L, const Segment& sg, const double* buf, int nvt, int nvec,
+                  const double* Tq, double* Fq, cudaStream_t st)
 {
     if (L.nwork == 0) return RTTDA_OK;
     const int key = L.la * 8 + L.lb * 4 + L.lc * 2 + L.ld;
     switch (key) {
-        case 0:  return launch_digest<0, 0, 0, 0>(h, L, sg, nvt, Tq, Fq, st);
-        case 8:  return launch_digest<1, 0, 0, 0>(h, L, sg, nvt, Tq, Fq, st);
-        case 4:  return launch_digest<0, 1, 0, 0>(h, L, sg, nvt, Tq, Fq, st);
-        case 10: return launch_digest<1, 0, 1, 0>(h, L, sg, nvt, Tq, Fq, st);
-        case 6:  return launch_digest<0, 1, 1, 0>(h, L, sg, nvt, Tq, Fq, st);
-        case 12: return launch_digest<1, 1, 0, 0>(h, L, sg, nvt, Tq, Fq, st);
-        case 14: return launch_digest<1, 1, 1, 0>(h, L, sg, nvt, Tq, Fq, st);
-        case 15: return launch_digest<1, 1, 1, 1>(h, L, sg, nvt, Tq, Fq, st);
+        case 0:  return launch_digest<0, 0, 0, 0>(h, L, sg, buf, nvt, nvec, Tq, Fq, st);
+        case 8:  return launch_digest<1, 0, 0, 0>(h, L, sg, buf, nvt, nvec, Tq, Fq, st);
+        case 4:  return launch_digest<0, 1, 0, 0>(h, L, sg, buf, nvt, nvec, Tq, Fq, st);
+        case 10: return launch_digest<1, 0, 1, 0>(h, L, sg, buf, nvt, nvec, Tq, Fq, st);
+        case 6:  return launch_digest<0, 1, 1, 0>(h, L, sg, buf, nvt, nvec, Tq, Fq, st);
+        case 12: return launch_digest<1, 1, 0, 0>(h, L, sg, buf, nvt, nvec, Tq, Fq, st);
+        case 14: return launch_digest<1, 1, 1, 0>(h, L, sg, buf, nvt, nvec, Tq, Fq, st);
+        case 15: return launch_digest<1, 1, 1, 1>(h, L, sg, buf, nvt, nvec, Tq, Fq, st);
         default: set_error("digest: unsupported class"); return RTTDA_EINVAL;
     }
 }
 
-// One ERI pass: for every segment, evaluate its quartets once into the staging buffer, then digest them for all
-// nvt densities.  Fq must be zeroed by the caller; nvt must be even (16-byte density slots).
-int jk_build(Handle* h, int nvt, const double* Tq, double* Fq, cudaStream_t st)
+// One ERI pass: for every segment, evaluate its quartets once into a staging buffer (stream st_eval), then digest
+// them for all densities (caller's stream).  Two buffers: the FP64-bound evaluation of segment k+1 overlaps the
+// L1/L2-bound digestion of segment k.  Fq must be zeroed by the caller; densities [0, nvec) of the nvt slots per
+// element are processed (nvec even, nvt a multiple of 2 with 16-byte aligned slots).
+int jk_build(Handle* h, int nvt, int nvec, const double* Tq, double* Fq, cudaStream_t st)
 {
-    RT_CHECK(nvt >= 2 && nvt % 2 == 0, "jk_build: the interleaved density count must be even");
-    RT_TRY(ensure_ws(h, &h->eri_buf, &h->eri_buf_n, h->eri_buf_need));
+    RT_CHECK(nvec >= 2 && nvec % 2 == 0 && nvt >= nvec && nvt % 2 == 0, "jk_build: bad density slot counts");
+    for (int b = 0; b < 2; ++b) RT_TRY(ensure_ws(h, &h->eri_buf[b], &h->eri_buf_n[b], h->eri_buf_need));
+    RT_CUDA(cudaEventRecord(h->ev_fork, st));
+    RT_CUDA(cudaStreamWaitEvent(h->st_eval, h->ev_fork, 0));
+    int k = 0;
     for (const Segment& sg : h->segments) {
         if (sg.nitems == 0) continue;
-        RT_TRY(eval_segment(h, sg, st));
+        const int b = k & 1;
+        if (k >= 2) RT_CUDA(cudaStreamWaitEvent(h->st_eval, h->ev_D[b], 0));
+        RT_TRY(eval_segment(h, sg, h->eri_buf[b], h->st_eval));
+        RT_CUDA(cudaEventRecord(h->ev_E[b], h->st_eval));
+        RT_CUDA(cudaStreamWaitEvent(st, h->ev_E[b], 0));
         for (int l = sg.first_launch; l < sg.first_launch + sg.nlaunch; ++l)
-            RT_TRY(digest_launch(h, h->launches[l], sg, nvt, Tq, Fq, st));
+            RT_TRY(digest_launch(h, h->launches[l], sg, h->eri_buf[b], nvt, nvec, Tq, Fq, st));
+        RT_CUDA(cudaEventRecord(h->ev_D[b], st));
+        ++k;
     }
     return RTTDA_OK;
 }

@@ -125,7 +125,7 @@ __global__ void __launch_bounds__(JK_BLOCK) eval_kernel(EvalArgs g)
 }
 
 template <int LA, int LB, int LC, int LD>
-static int launch_eval(Handle* h, const Segment& sg, cudaStream_t st)
+static int launch_eval(Handle* h, const Segment& sg, double* buf, cudaStream_t st)
 {
     EvalArgs g;
     g.items = sg.items;
@@ -133,7 +133,7 @@ static int launch_eval(Handle* h, const Segment& sg, cudaStream_t st)
     g.ket = h->tabs.kets[sg.kc_ket];
     g.batch_base = sg.batch_base;
     g.boys = h->tabs.boys[LA + LB + LC + LD];
-    g.buf = h->eri_buf;
+    g.buf = buf;
     g.tau = h->tabs.tau;
     g.same = (sg.kc_bra == sg.kc_ket);
     dim3 grid(sg.nitems), block(JK_BLOCK);
@@ -147,17 +147,17 @@ static int launch_eval(Handle* h, const Segment& sg, cudaStream_t st)
     return RTTDA_OK;
 }
 
-int eval_segment(Handle* h, const Segment& sg, cudaStream_t st)
+int eval_segment(Handle* h, const Segment& sg, double* buf, cudaStream_t st)
 {
     if (sg.nitems == 0) return RTTDA_OK;
     const int key = sg.la * 8 + sg.lb * 4 + sg.lc * 2 + sg.ld;
     switch (key) {
-        case 0:  return launch_eval<0, 0, 0, 0>(h, sg, st);
-        case 8:  return launch_eval<1, 0, 0, 0>(h, sg, st);
-        case 10: return launch_eval<1, 0, 1, 0>(h, sg, st);
-        case 12: return launch_eval<1, 1, 0, 0>(h, sg, st);
-        case 14: return launch_eval<1, 1, 1, 0>(h, sg, st);
-        case 15: return launch_eval<1, 1, 1, 1>(h, sg, st);
+        case 0:  return launch_eval<0, 0, 0, 0>(h, sg, buf, st);
+        case 8:  return launch_eval<1, 0, 0, 0>(h, sg, buf, st);
+        case 10: return launch_eval<1, 0, 1, 0>(h, sg, buf, st);
+        case 12: return launch_eval<1, 1, 0, 0>(h, sg, buf, st);
+        case 14: return launch_eval<1, 1, 1, 0>(h, sg, buf, st);
+        case 15: return launch_eval<1, 1, 1, 1>(h, sg, buf, st);
         default: set_error("eval_segment: unsupported class"); return RTTDA_EINVAL;
     }
 }

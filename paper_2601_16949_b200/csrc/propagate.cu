@@ -42,7 +42,7 @@ int sigma_impl(Handle* h, int nvec, const double* X, long long ldx, double* sigm
                cudaStream_t st)
 {
     const size_t N = h->nao, no = h->nocc, nv = h->nvirt;
-    const int nvt = (nvec + 1) & ~1;            // interleaved density slots are 16-byte multiples
+    const int nvt = padded_nvec(nvec);          // density slots: 16, 32 or multiples of 64 bytes (sector aligned)
     RT_TRY(ensure_ws(h, &h->wsY, &h->wsY_n, (size_t)nvec * no * N));
     RT_TRY(ensure_ws(h, &h->wsT, &h->wsT_n, (size_t)nvt * N * N));
     RT_TRY(ensure_ws(h, &h->wsF, &h->wsF_n, (size_t)nvt * N * N));
@@ -65,7 +65,7 @@ int sigma_impl(Handle* h, int nvec, const double* X, long long ldx, double* sigm
     RT_TRY(jk_mark(h, st));
     // a3-a4: F = 2 J[T] - cx K[T], interleaved layout; one ERI pass serves all densities
     RT_CUDA(cudaMemsetAsync(h->wsF, 0, (size_t)nvt * N * N * sizeof(double), st));
-    RT_TRY(jk_build(h, nvt, h->wsT, h->wsF, st));
+    RT_TRY(jk_build(h, nvt, (nvec + 1) & ~1, h->wsT, h->wsF, st));
     RT_TRY(jk_mark(h, st));
     RT_CUDA(cudaEventRecord(h->ev[2], st));
     // a5: Z_v = C_o^T F_v [no][N];  sigma_v = deps o X_v + Z_v C_v

@@ -544,6 +544,12 @@ int create_impl(Handle* h, const rttda_basis_t* basis, const double* C_occ, cons
         h->D_00[k] = 2.0 * tr;                 // R3: sum over spin orbitals
     }
     for (auto& e : h->ev) RT_CUDA(cudaEventCreate(&e));
+    RT_CUDA(cudaStreamCreateWithFlags(&h->st_eval, cudaStreamNonBlocking));
+    RT_CUDA(cudaEventCreateWithFlags(&h->ev_fork, cudaEventDisableTiming));
+    for (int b = 0; b < 2; ++b) {
+        RT_CUDA(cudaEventCreateWithFlags(&h->ev_E[b], cudaEventDisableTiming));
+        RT_CUDA(cudaEventCreateWithFlags(&h->ev_D[b], cudaEventDisableTiming));
+    }
     h->info[RTTDA_INFO_CREATE_MS] =
         std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - t0).count();
     return RTTDA_OK;
