@@ -14,6 +14,7 @@
 // Densities and results use the interleaved layout Tq[mu][nu][v] (v fastest), F likewise.
 #include <cstdlib>
 #include "common.cuh"
+#include "tma.cuh"
 
 namespace rttda {
 
@@ -67,6 +68,11 @@ __device__ __forceinline__ int warp_reduce_owner_index(int lane)
     return idx;
 }
 
+constexpr int REC_TILE = 256;
+// classes whose two-stage integral ring (4 warps x 2 x NI x 256 bytes) leaves room for several blocks per SM
+constexpr bool digest_uses_tma(int ni) { return ni <= 27; }
+constexpr size_t digest_ring_bytes(int ni) { return digest_uses_tma(ni) ? (size_t)(JK_BLOCK / 32) * 2 * ni * 256 : 0; }      // a-list records staged in shared memory at a time
+
 constexpr int next_pow2(int n) { return n <= 1 ? 1 : (n <= 2 ? 2 : (n <= 4 ? 4 : (n <= 8 ? 8 : (n <= 16 ? 16 : 32)))); }
 
 struct DigestArgs {
@@ -107,6 +113,7 @@ digest_kernel(DigestArgs g)
 {
     constexpr int NA = 2 * LA + 1, NB = 2 * LB + 1, NC = 2 * LC + 1, ND = 2 * LD + 1;
     constexpr int NI = NA * NB * NC * ND;
+    constexpr bool USE_TMA = digest_uses_tma(NI);
     const JKTables& tb = g.tb;
     const WorkItem wi = g.work[blockIdx.x];
     const AList al = tb.alists[wi.alist];
@@ -156,15 +163,69 @@ digest_kernel(DigestArgs g)
             for (int d = 0; d < ND; ++d) Jcd[c][d][v] = 0.0;
     }
 
-    for (int r = al.rec_begin; r < al.rec_end; ++r) {
-        const BraRec br = tb.recs[r];
-        const bool ok = active && (br.Q * Qq >= tb.tau) && (!same_class || br.pos <= q);
-        if (!__any_sync(0xffffffffu, ok)) break;
+    // The a-list's records and their staging-buffer offsets go through shared memory, REC_TILE at a time.  Each
+    // warp streams its 32-ket batch of every record (NI x 256 contiguous bytes) from HBM into a two-stage shared
+    // memory ring with TMA bulk copies: the copy of record r+1 is in flight while record r is digested.
+    __shared__ BraRec s_rec[REC_TILE];
+    __shared__ long long s_bb[REC_TILE];
+    __shared__ __align__(8) uint64_t s_bar[JK_BLOCK / 32][2];
+    extern __shared__ __align__(16) double s_dyn[];
+    const int warp = threadIdx.x >> 5;
+    double* ring = s_dyn + (size_t)warp * 2 * (NI * 32);
+    if (USE_TMA) {
+        if (lane == 0) { mbar_init(&s_bar[warp][0], 1); mbar_init(&s_bar[warp][1], 1); mbar_fence_init(); }
+        __syncwarp();
+    }
+    uint32_t phase0 = 0, phase1 = 0;
+    int stage = 0;
+    const long long qb = q >> 5;                            // warp-uniform
+    auto issue = [&](int ir, int s) {
+        if (USE_TMA && lane == 0) {
+            const double* gsrc = g.buf + (size_t)(s_bb[ir] + qb) * (NI * 32);
+            mbar_expect_tx(&s_bar[warp][s], NI * 256);
+            tma_load_1d(ring + (size_t)s * (NI * 32), gsrc, NI * 256, &s_bar[warp][s]);
+        }
+    };
+    auto pred = [&](int ir) {
+        const BraRec& b1 = s_rec[ir];
+        return active && (b1.Q * Qq >= tb.tau) && (!same_class || b1.pos <= q);
+    };
+    bool done = false;                                      // warp-uniform
+    for (int r0 = al.rec_begin; r0 < al.rec_end; r0 += REC_TILE) {
+      const int nrec = min(REC_TILE, al.rec_end - r0);
+      __syncthreads();
+      for (int i = threadIdx.x; i < nrec; i += JK_BLOCK) {
+          const BraRec b0 = tb.recs[r0 + i];
+          s_rec[i] = b0;
+          s_bb[i] = __ldg(g.batch_base + b0.pos) - (same_class ? (b0.pos >> 5) : 0);
+      }
+      __syncthreads();
+      bool ok_next = false;
+      if (!done) {
+          ok_next = pred(0);
+          if (__any_sync(0xffffffffu, ok_next)) issue(0, stage); else done = true;
+      }
+      if (!done)
+      for (int ir = 0; ir < nrec; ++ir) {
+        const BraRec br = s_rec[ir];
+        const bool ok = ok_next;
+        bool more = false;
+        if (ir + 1 < nrec) {
+            ok_next = pred(ir + 1);
+            more = __any_sync(0xffffffffu, ok_next);
+            if (more) issue(ir + 1, stage ^ 1);
+        }
         const bool canonical = (br.flags & 1) != 0;
         const bool ab_same = (br.flags & 2) != 0;
         const int aoB = br.ao_b;
-        const long long batch = __ldg(g.batch_base + br.pos) + (q >> 5) - (same_class ? (br.pos >> 5) : 0);
-        const double* src = g.buf + (size_t)batch * (NI * 32) + lane;
+        const double* src;
+        if (USE_TMA) {
+            src = ring + (size_t)stage * (NI * 32) + lane;
+            if (stage == 0) { mbar_wait(&s_bar[warp][0], phase0); phase0 ^= 1; }
+            else { mbar_wait(&s_bar[warp][1], phase1); phase1 ^= 1; }
+        } else {
+            src = g.buf + (size_t)(s_bb[ir] + qb) * (NI * 32) + lane;
+        }
         // degeneracy weights: 1/2 if the ket is a diagonal pair, 1/2 if bra pair == ket pair
         const double wsame = (same_class && br.pos == q) ? 0.5 : 1.0;
         const double wk = ok ? wsame * (cd_same ? 0.5 : 1.0) : 0.0;
@@ -218,7 +279,7 @@ digest_kernel(DigestArgs g)
 #pragma unroll
                     for (int c = 0; c < NC; ++c) {
                         const int i = (d * NC + c) * (NA * NB) + i_ab;
-                        const double x = ok ? wk * __ldcs(src + i * 32) : 0.0;
+                        const double x = ok ? wk * (USE_TMA ? src[i * 32] : __ldcs(src + i * 32)) : 0.0;
 #pragma unroll
                         for (int v = 0; v < NV; ++v) {
                             Kac[a][c][v] = fma(x, tbd[d][v], Kac[a][c][v]);
@@ -242,6 +303,10 @@ digest_kernel(DigestArgs g)
                 }
             }
         }
+        if (USE_TMA) { __syncwarp(); stage ^= 1; }          // every lane is done with this stage before it is refilled
+        if (!more) { if (ir + 1 < nrec) done = true; break; }
+      }
+      if (__syncthreads_and(done)) break;
     }
 #undef TQ
     if (!active) return;
@@ -299,10 +364,12 @@ digest_v_kernel(DigestArgs g, int G, int KW)
 #define TQ(mu, nu) (Tv + (size_t)(mu) * rs + (size_t)(nu) * nvt)
 #define FQ(mu, nu) (Fv + (size_t)(mu) * rs + (size_t)(nu) * nvt)
     const int qw = wi.ket0 + warp * 32;                  // this warp's 32-ket batch
+    __shared__ BraRec s_rec[REC_TILE];
+    __shared__ long long s_bb[REC_TILE];
+    int loaded_r0 = -1;
     for (int kbase = 0; kbase < 32; kbase += KW) {
         const int q = qw + kbase + kg;
         const bool active = lane_used && (kbase + kg < 32) && q < kc.n;
-        if (!__any_sync(0xffffffffu, active)) break;
         const int qq = active ? q : kc.n - 1;
         const double Qq = active ? __ldg(kc.Q + qq) : 0.0;
         const int aoC = __ldg(kc.ao_c + qq), aoD = __ldg(kc.ao_d + qq);
@@ -324,14 +391,28 @@ digest_v_kernel(DigestArgs g, int G, int KW)
             for (int d2 = 0; d2 < ND; ++d2) Kad[a][d2] = Kda[d2][a] = 0.0;
         }
 
-        for (int r = al.rec_begin; r < al.rec_end; ++r) {
-            const BraRec br = tb.recs[r];
+        bool done = !__any_sync(0xffffffffu, active);       // warp-uniform
+        for (int r0 = al.rec_begin; r0 < al.rec_end; r0 += REC_TILE) {
+          const int nrec = min(REC_TILE, al.rec_end - r0);
+          if (loaded_r0 != r0) {                              // block-uniform: short lists are staged once
+              __syncthreads();
+              for (int i = threadIdx.x; i < nrec; i += JK_BLOCK) {
+                  const BraRec b0 = tb.recs[r0 + i];
+                  s_rec[i] = b0;
+                  s_bb[i] = __ldg(g.batch_base + b0.pos) - (same_class ? (b0.pos >> 5) : 0);
+              }
+              __syncthreads();
+              loaded_r0 = r0;
+          }
+          if (!done)
+          for (int ir = 0; ir < nrec; ++ir) {
+            const BraRec br = s_rec[ir];
             const bool ok = active && (br.Q * Qq >= tb.tau) && (!same_class || br.pos <= q);
-            if (!__any_sync(0xffffffffu, ok)) break;
+            if (!__any_sync(0xffffffffu, ok)) { done = true; break; }
             const bool canonical = (br.flags & 1) != 0;
             const bool ab_same = (br.flags & 2) != 0;
             const int aoB = br.ao_b;
-            const long long batch = __ldg(g.batch_base + br.pos) + (qw >> 5) - (same_class ? (br.pos >> 5) : 0);
+            const long long batch = s_bb[ir] + (qw >> 5);
             const double* src = g.buf + (size_t)batch * (NI * 32) + (q & 31);
             const double wsame = (same_class && br.pos == q) ? 0.5 : 1.0;
             const double wk = ok ? wsame * (cd_same ? 0.5 : 1.0) : 0.0;
@@ -385,6 +466,8 @@ digest_v_kernel(DigestArgs g, int G, int KW)
                     }
                 }
             }
+          }
+          if (al.rec_end - al.rec_begin > REC_TILE && __syncthreads_and(done)) break;
         }
         if (active) {
 #pragma unroll
@@ -443,7 +526,14 @@ static int launch_digest_nv(Handle* h, const JKLaunch& L, const Segment& sg, con
     g.buf = buf;
     g.Tq = Tq; g.Fq = Fq; g.cx = h->cx;
     g.ketclass = L.ketclass; g.same = (sg.kc_bra == sg.kc_ket); g.nvt = nvt; g.v0 = v0;
-    digest_kernel<LA, LB, LC, LD, NV><<<dim3(L.nwork), dim3(JK_BLOCK), 0, st>>>(g);
+    constexpr int NI = (2 * LA + 1) * (2 * LB + 1) * (2 * LC + 1) * (2 * LD + 1);
+    constexpr size_t smem = digest_ring_bytes(NI);
+    static bool attr_set = false;
+    if (!attr_set && smem > 0) {
+        RT_CUDA(cudaFuncSetAttribute(digest_kernel<LA, LB, LC, LD, NV>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        attr_set = true;
+    }
+    digest_kernel<LA, LB, LC, LD, NV><<<dim3(L.nwork), dim3(JK_BLOCK), smem, st>>>(g);
     h->kernel_launches++;
     RT_CUDA(cudaGetLastError());
     return RTTDA_OK;
@@ -457,7 +547,12 @@ static int launch_digest(Handle* h, const JKLaunch& L, const Segment& sg, const 
     constexpr int PER_V = 2 * NA * (NC + ND) + 2 * NC * ND;
     static int vmode = -1;
     if (vmode < 0) { const char* e = getenv("RTTDA_DIGEST_V"); vmode = e ? atoi(e) : 4; }
-    if (vmode > 0 && nvec >= vmode) {
+    // which ordered classes use the density-per-lane kernel (bit: ssss, spss, psss, spps, psps, ppss, ppps, pppp)
+    static int vmask = -1;
+    if (vmask < 0) { const char* e = getenv("RTTDA_DIGEST_VMASK"); vmask = e ? atoi(e) : 31; }
+    constexpr int KEY = LA * 8 + LB * 4 + LC * 2 + LD;
+    constexpr int CLS = KEY == 0 ? 0 : KEY == 4 ? 1 : KEY == 8 ? 2 : KEY == 6 ? 3 : KEY == 10 ? 4 : KEY == 12 ? 5 : KEY == 14 ? 6 : 7;
+    if (vmode > 0 && nvec >= vmode && ((vmask >> CLS) & 1)) {
         // density-per-lane kernel: groups of G lanes per ket, chunks of at most 32 densities
         for (int v0 = 0; v0 < nvec; v0 += 32) {
             const int G = nvec - v0 < 32 ? nvec - v0 : 32;
