@@ -49,6 +49,21 @@ def parse():
     return ap.parse_args()
 
 
+def reduce_max(x: float, world: int, device) -> float:
+    """Time of the slowest replica: the one collective of the N > 1 path (replicas only)."""
+    if world <= 1:
+        return float(x)
+    import torch
+    t = torch.tensor([x], dtype=torch.float64, device=device)
+    torch.distributed.all_reduce(t, op=torch.distributed.ReduceOp.MAX)
+    return float(t.item())
+
+
+def aggregate_value(ntraj: int, world: int, ms_per_step: float) -> float:
+    """Whole-job sigma-vectors/s: every replica builds 8*ntraj sigma-vectors per RK4 step."""
+    return 8.0 * ntraj * world / (ms_per_step * 1e-3)
+
+
 def dist_env():
     return int(os.environ.get("RANK", 0)), int(os.environ.get("LOCAL_RANK", 0)), int(os.environ.get("WORLD_SIZE", 1))
 
@@ -279,12 +294,9 @@ def run_b200(args):
     total_ms = float(sum(ms))
     jk_ms, jk_n = h.rttda_jk_time()
     launches = int(h.rttda_get_info("kernel_launches") - l0)
-    if world > 1:
-        t = torch.tensor([total_ms], dtype=torch.float64, device=dev)
-        torch.distributed.all_reduce(t, op=torch.distributed.ReduceOp.MAX)
-        total_ms = float(t.item())
+    total_ms = reduce_max(total_ms, world, dev)
     ms_per_step = total_ms / args.steps
-    value = 8.0 * ntraj * world / (ms_per_step * 1e-3)
+    value = aggregate_value(ntraj, world, ms_per_step)
 
     # end to end: host buffers through rttda_propagate_host (H2D of the state, D2H of state + log inside)
     yh = torch.from_numpy(y0.copy()).pin_memory()
@@ -296,11 +308,8 @@ def run_b200(args):
         h.rttda_propagate_host(yh.numpy(), cont, (i + 1) * dt, dt, 1, lh.numpy(), st)
     barrier()
     e2e_s = time.perf_counter() - e0
-    if world > 1:
-        t = torch.tensor([e2e_s], dtype=torch.float64, device=dev)
-        torch.distributed.all_reduce(t, op=torch.distributed.ReduceOp.MAX)
-        e2e_s = float(t.item())
-    e2e_val = 8.0 * ntraj * world * args.steps / e2e_s
+    e2e_s = reduce_max(e2e_s, world, dev)
+    e2e_val = aggregate_value(ntraj, world, e2e_s * 1e3 / args.steps)
     h2d = yh.numel() * 8
     d2h = yh.numel() * 8 + lh.numel() * 8
 
@@ -325,10 +334,12 @@ def run_b200(args):
                "eri_quartets_per_s": info["nquartets"] / (jk_avg_ms * 1e-3),
                "counts": {"shell_pairs_kept": info["npairs_kept"], "unique_shell_quartets": info["nquartets"],
                           "primitive_quartets": info["nprim_quartets"], "quartets_evaluated": info["nquartets_eval"],
-                          "primitive_evaluated": info["nprim_eval"], "nvec_chunk": info["nvec_chunk"]},
+                          "primitive_evaluated": info["nprim_eval"], "flops_eval_per_pass": info["flops_eval"],
+                          "flops_digest_per_vec": info["flops_digest_per_vec"],
+                          "eri_staging_buffer_bytes": info["eri_buf_bytes"]},
                "setup_s": setup_s, "create_ms": info["create_ms"],
                "jk_ms_per_pass": jk_avg_ms, "jk_share_of_step": jk_ms / (sum(ms) if sum(ms) else 1.0),
-               "roofline": {"bound": "alu", "kernel": "jk_kernel<*> (all class launches of one ERI pass)",
+               "roofline": {"bound": "alu", "kernel": "eval_kernel<*> + digest_kernel<*>/digest_v_kernel<*> (all launches of one ERI pass)",
                             "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
                             "traffic": None, "peak_source": "measured live: rttda_fp64_peak DFMA chain, 1 s "
                             "(MEASURED_PEAKS.json has no FP64 entry; nominal %.1f)" % FP64_NOMINAL_TFLOPS,

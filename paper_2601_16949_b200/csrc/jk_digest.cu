@@ -547,9 +547,10 @@ static int launch_digest(Handle* h, const JKLaunch& L, const Segment& sg, const 
     constexpr int PER_V = 2 * NA * (NC + ND) + 2 * NC * ND;
     static int vmode = -1;
     if (vmode < 0) { const char* e = getenv("RTTDA_DIGEST_V"); vmode = e ? atoi(e) : 4; }
-    // which ordered classes use the density-per-lane kernel (bit: ssss, spss, psss, spps, psps, ppss, ppps, pppp)
+    // which ordered classes use the density-per-lane kernel (bit: ssss, spss, psss, spps, psps, ppss, ppps, pppp);
+    // default = the classes where it measured faster on B200 (ss|ss, sp|ss, sp|ps), see profiles/
     static int vmask = -1;
-    if (vmask < 0) { const char* e = getenv("RTTDA_DIGEST_VMASK"); vmask = e ? atoi(e) : 31; }
+    if (vmask < 0) { const char* e = getenv("RTTDA_DIGEST_VMASK"); vmask = e ? atoi(e) : 11; }
     constexpr int KEY = LA * 8 + LB * 4 + LC * 2 + LD;
     constexpr int CLS = KEY == 0 ? 0 : KEY == 4 ? 1 : KEY == 8 ? 2 : KEY == 6 ? 3 : KEY == 10 ? 4 : KEY == 12 ? 5 : KEY == 14 ? 6 : 7;
     if (vmode > 0 && nvec >= vmode && ((vmask >> CLS) & 1)) {

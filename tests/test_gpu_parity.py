@@ -168,3 +168,69 @@ def test_error_codes():
     with pytest.raises(R.RttdaError):
         R.Rttda(ctx["basis"], torch.zeros((30, 4), dtype=torch.float64, device=ctx["dev"]),
                 torch.zeros((30, 25), dtype=torch.float64, device=ctx["dev"]), ctx["eps"])   # nocc+nvirt != nao
+
+
+# ---------------------------------------------------------------------------------------------------
+# wider batches: odd counts, more than one 32-density chunk, every digestion kernel variant
+@pytest.mark.parametrize("nvec", [3, 4, 7, 12, 33])
+def test_fock_tiny_wide_batches(nvec):
+    ctx = setup_config(1, tau=0.0, dense=True)
+    eri, N = ctx["ob"].eri_tensor(), ctx["basis"].nao
+    T = np.random.default_rng(100 + nvec).standard_normal((nvec, N, N))
+    Fref = 2 * np.einsum("mnls,vls->vmn", eri, T) - np.einsum("mnls,vns->vml", eri, T)
+    F = gpu_fock(ctx, T)
+    assert rel_inf(F, Fref) < 1e-12
+
+
+def test_sigma_config2_screened_matches_unscreened_and_counts():
+    """tau = 1e-12 (the config's value) against tau = 0 on the GPU: the screening error stays below the
+    sigma tolerance, and the two handles count different quartets."""
+    import paper_2601_16949_b200 as R
+    import torch
+    from workloads import make_vectors
+    ctx = setup_config(2)
+    X = make_vectors(ctx["cfg"], 4)
+    got = gpu_sigma(ctx, X)
+    h0 = R.Rttda(ctx["basis"], torch.from_numpy(ctx["C_o"]).to(ctx["dev"]), torch.from_numpy(ctx["C_v"]).to(ctx["dev"]),
+                 ctx["eps"], 1.0, 0.0)
+    Xd = torch.from_numpy(X).to(ctx["dev"])
+    out = torch.empty_like(Xd)
+    h0.rttda_sigma(Xd, out)
+    torch.cuda.synchronize()
+    assert rel_inf(got, out.cpu().numpy()) < SIGMA_TOL
+    assert h0.rttda_get_info("nquartets") > ctx["h"].rttda_get_info("nquartets")
+    h0.close()
+
+
+def test_sigma_config3_vs_matrix_free_oracle():
+    from workloads import make_vectors
+    from oracle import tda
+    ctx = setup_config(3)
+    X = make_vectors(ctx["cfg"], 2)
+    ref, _, _ = tda.sigma_matrix_free(ctx["ob"], X, ctx["C_o"], ctx["C_v"], ctx["eps"], 1.0, tau=1e-20)
+    got = gpu_sigma(ctx, X)
+    assert rel_inf(got, ref) < SIGMA_TOL
+
+
+def test_fock_config4_full_size_sampled_elements():
+    """The 1280-AO molecule in the launch configuration bench.py times (nvec = 6, tau = 1e-12): F elements at
+    sampled AO pairs against the oracle's definition-level J and K (unscreened), plus properties that hold at
+    any size (J part symmetric for symmetric T, linearity)."""
+    ctx = setup_config(4)
+    ob, N = ctx["ob"], ctx["basis"].nao
+    rng = np.random.default_rng(4)
+    X = rng.standard_normal((6, ctx["cfg"].nocc, ctx["cfg"].nvirt))
+    X /= np.linalg.norm(X.reshape(6, -1), axis=1)[:, None, None]
+    T = np.einsum("mi,via,na->vmn", ctx["C_o"], X, ctx["C_v"])           # transition densities, non-symmetric
+    F = gpu_fock(ctx, T)
+    mu = rng.integers(0, N, size=5)                                       # ~15-30 s of oracle time per sample
+    nu = rng.integers(0, N, size=5)
+    mu[:2] = [0, N - 1]; nu[:2] = [0, 700]                                # a diagonal element and an s-p element
+    J, K = ob.jk_samples(T, mu, nu)
+    ref = 2 * J - K                                                       # [sample][v]
+    got = F[:, mu, nu].T
+    scale = np.max(np.abs(F))
+    assert np.max(np.abs(got - ref)) / scale < SIGMA_TOL
+    F2 = gpu_fock(ctx, np.stack([T[0] + T[0].T, 2.0 * T[1] - 0.5 * T[2]]))
+    assert np.max(np.abs(F2[0] - (F[0] + F[0].T))) / scale < 1e-12        # F[T^T] = F[T]^T
+    assert np.max(np.abs(F2[1] - (2.0 * F[1] - 0.5 * F[2]))) / scale < 1e-12
