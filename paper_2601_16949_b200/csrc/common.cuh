@@ -81,6 +81,33 @@ struct AList {
     int np;                   // primitive pairs per record
 };
 
+// Shell-blocked a-lists of the block-per-batch digestion kernel: M (2 or 4) shells a_i of one shell class,
+// neighbours in space (consecutive along a Morton curve), share ONE walk over the union of their partners b, so
+// that every density element gathered for (b, c), (b, d) is reused for up to M quartets (a_i b|c d).
+constexpr int SUPER_MAX = 4;
+struct SHead {              // one partner shell b of the group
+    double Qmax;            // largest Schwarz bound over the members' pairs (a_i, b)
+    int ao_b;
+    int pad;
+};
+struct SMem {               // pair (a_i, b) of member i
+    double Q;               // 0 if the pair is absent
+    int pos;                // position of the unordered pair inside its class list
+    int flags;              // bit0 canonical, bit1 a == b, bit2 present
+};
+struct SAList {
+    double Qmax;
+    int ao_a[SUPER_MAX];      // AO offsets of the members (-1: slot unused)
+    int rec_begin, rec_end;   // into SHead array; members at [rec * M + i]
+    int ketclass, minpos;
+};
+struct SuperSet {             // device tables of one blocking factor M
+    int M;
+    const SHead* heads;
+    const SMem* mems;
+    const SAList* lists;
+};
+
 struct WorkItem {
     int alist;
     int ket0;                 // first ket (thread 0) of this block
@@ -113,21 +140,25 @@ struct JKLaunch {             // one digestion kernel instantiation: ordered bra
     int seg;
     int nwork;
     const WorkItem* work;     // device
+    int nswork[2];            // blocks over the shell-blocked a-lists, M = 2 and M = 4
+    const WorkItem* swork[2];
 };
 
 struct JKTables {
     KetClass kets[NKETCLASS];
     const BraRec* recs;
     const AList* alists;
-    const double2* boys[5];   // per total angular momentum L: rows {F_{L+7}(j/8), exp(-j/8)}
+    SuperSet super[2];        // M = 2, M = 4
+    const double2* boys[5];   // per total angular momentum L: rows {F_{L+k}(j/8)/k!, k < 8; exp(-j/8); pad}
     double tau;
     int nao;
 };
 
 constexpr int JK_BLOCK = 128;
-constexpr int EVAL_MAX_ROWS = 288;     // bra primitive rows staged per evaluation block (32 pairs x 9 prims)
+constexpr int EVAL_MAX_ROWS = 144;     // bra primitive rows staged per evaluation block (16 pairs x 9 prims)
 
-// Boys grid: T0 = j / 8, j = 0..BOYS_NROW-1
+// Boys grid: T0 = j / 8, j = 0..BOYS_NROW-1; BOYS_ROW doubles per row (eri_eval.cuh)
+constexpr int BOYS_ROW = 10;
 constexpr double BOYS_TMAX = 48.0;
 constexpr int BOYS_NROW = 385 + 1;
 void boys_table_host(int L, std::vector<double>& tab);

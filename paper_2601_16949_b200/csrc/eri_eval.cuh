@@ -21,11 +21,11 @@ __host__ __device__ constexpr int hidx_plus(int t, int u, int v, int axis)
 }
 
 // ---- Boys function F_0..F_L(T) -------------------------------------------------------------------------
-// T < 48: nearest grid point T0 = j/8; ONE 16-byte table row {F_{L+7}(T0), e^-T0} (shared memory gather);
-//   the lower orders at T0 follow from the (stable) downward recursion F_{n-1} = (2 T0 F_n + e^-T0)/(2n-1),
-//   carried in the scaled form h_k = F_{L+k}(T0)/k! so that the Taylor sum F_L(T) = sum_k h_k (T0-T)^k
-//   (dF_n/dT = -F_{n+1}) is a plain Horner chain; then downward recursion at T with
-//   e^-T = e^-T0 e^(T0-T) (degree-8 Taylor, |T0-T| <= 1/16).
+// T < 48: nearest grid point T0 = j/8; one 80-byte table row {h_0..h_7, e^-T0, pad}, h_k = F_{L+k}(T0)/k!, so
+//   that F_L(T) = sum_k h_k (T0-T)^k (dF_n/dT = -F_{n+1}) is a 7-FMA Horner chain; then downward recursion
+//   F_{n-1} = (2T F_n + e^-T)/(2n-1) with e^-T = e^-T0 e^(T0-T) (degree-8 Taylor, |T0-T| <= 1/16).
+//   The row is a shared-memory gather; in the workloads of DESIGN.md only ~1 primitive quartet in 8 takes this
+//   branch (few active lanes), so its cost is its instruction count, not its shared-memory traffic.
 // T >= 48: F_0 = sqrt(pi/T)/2, F_{n+1} = (2n+1) F_n / (2T) (the e^-T term is < 1e-20).
 template <int L>
 __device__ __forceinline__ void boys(double T, const double2* __restrict__ tab, double (&F)[L + 1])
@@ -34,21 +34,20 @@ __device__ __forceinline__ void boys(double T, const double2* __restrict__ tab, 
         constexpr double MAGIC = 6755399441055744.0;          // 1.5 * 2^52: rounds to nearest integer
         const double t = fma(T, 8.0, MAGIC);
         const int j = __double2loint(t);
-        const double jd = t - MAGIC;
-        const double dx = fma(jd, 0.125, -T);                 // T0 - T, |dx| <= 1/16
-        const double2 row = tab[j];
-        const double twoT0 = jd * 0.25, e0 = row.y;
-        constexpr double fact[8] = {1.0, 1.0, 2.0, 6.0, 24.0, 120.0, 720.0, 5040.0};
-        double h = row.x * (1.0 / fact[7]);
-        double f = h;
-#pragma unroll
-        for (int k = 7; k >= 1; --k) {
-            const double den = 2.0 * (L + k) - 1.0;
-            h = fma(twoT0 * ((double)k / den), h, e0 * (1.0 / (den * fact[k - 1])));
-            f = fma(f, dx, h);
-        }
+        const double dx = fma(t - MAGIC, 0.125, -T);          // T0 - T, |dx| <= 1/16
+        const double2* row = tab + j * (BOYS_ROW / 2);
+        const double2 h01 = row[0], h23 = row[1], h45 = row[2], h67 = row[3];
+        double f = h67.y;
+        f = fma(f, dx, h67.x);
+        f = fma(f, dx, h45.y);
+        f = fma(f, dx, h45.x);
+        f = fma(f, dx, h23.y);
+        f = fma(f, dx, h23.x);
+        f = fma(f, dx, h01.y);
+        f = fma(f, dx, h01.x);
         F[L] = f;
         if (L > 0) {
+            const double e0 = row[4].x;
             double e = 1.0 / 40320.0;
             e = fma(e, dx, 1.0 / 5040.0);
             e = fma(e, dx, 1.0 / 720.0);

@@ -12,6 +12,9 @@
 //   Both orientations (a,b), (b,a) of a bra pair are separate records reading the SAME stored block, which
 //   keeps every exchange update in registers: no per-quartet global atomics, and no second evaluation.
 // Densities and results use the interleaved layout Tq[mu][nu][v] (v fastest), F likewise.
+// Two kernels share that decomposition: digest_kernel (thread = ket, NV densities in registers; calls with < 4
+// densities and the ps|ss, pp|ss classes) and digest_b_kernel (block = one 32-ket batch, a group of lanes per ket,
+// lane = density; the other classes).  Both are bound by the density gathers through L1/L2.
 #include <cstdlib>
 #include "common.cuh"
 #include "tma.cuh"
@@ -335,24 +338,29 @@ digest_kernel(DigestArgs g)
 }
 
 // ---------------------------------------------------------------------------------------------------
-// Density-per-lane variant (used when a call carries >= 4 densities): a group of G consecutive lanes owns ONE ket
-// pair, lane v of the group serves density v.  A warp holds KW = 32 / G kets of its 32-ket batch at a time.  Every
-// density/Fock access is then a contiguous 8*G-byte run of one 64-byte aligned slot (sector-efficient gathers,
-// coalesced reductions), and a lane needs only one density's accumulators, so all densities of the call are
-// served by ONE read of the staged integrals for every class.
+// Block-per-batch, density-per-lane kernel: the block owns ONE 32-ket batch and walks an a-list; warp w holds
+// KW = 32 / G kets of the batch, a group of G lanes per ket, lane v of the group serves density v.  The batch's
+// integrals of each record (NI x 256 contiguous bytes) are fetched ONCE by a TMA bulk copy into a two-stage shared
+// memory ring shared by all warps (the copy of record r+1 flies while record r is digested); every density access
+// is a contiguous 8*G-byte run of an aligned slot; a lane carries one density's accumulators only, so all
+// densities of the call are served by one read of the staged integrals.
 template <int LA, int LB, int LC, int LD>
-__global__ void __launch_bounds__(JK_BLOCK)
-digest_v_kernel(DigestArgs g, int G, int KW)
+__global__ void __launch_bounds__(256)
+digest_b_kernel(DigestArgs g, int G, int KW)
 {
     constexpr int NA = 2 * LA + 1, NB = 2 * LB + 1, NC = 2 * LC + 1, ND = 2 * LD + 1;
     constexpr int NI = NA * NB * NC * ND;
     const JKTables& tb = g.tb;
-    const WorkItem wi = g.work[blockIdx.x];
+    const WorkItem wi = g.work[blockIdx.x >> 2];
     const AList al = tb.alists[wi.alist];
     const KetClass& kc = tb.kets[g.ketclass];
+    const int q0 = wi.ket0 + 32 * (blockIdx.x & 3);      // first ket of this block's batch
+    if (q0 >= kc.n) return;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int kg = lane / G, v = lane - kg * G;
-    const bool lane_used = kg < KW;
+    const int kb = warp * KW + kg;                       // ket index inside the batch
+    const int q = q0 + kb;
+    const bool active = kg < KW && kb < 32 && q < kc.n;
     const bool same_class = g.same != 0;
     const int aoA = al.ao_a;
     const size_t nao = tb.nao;
@@ -363,134 +371,153 @@ digest_v_kernel(DigestArgs g, int G, int KW)
     const double cx = g.cx;
 #define TQ(mu, nu) (Tv + (size_t)(mu) * rs + (size_t)(nu) * nvt)
 #define FQ(mu, nu) (Fv + (size_t)(mu) * rs + (size_t)(nu) * nvt)
-    const int qw = wi.ket0 + warp * 32;                  // this warp's 32-ket batch
     __shared__ BraRec s_rec[REC_TILE];
     __shared__ long long s_bb[REC_TILE];
-    int loaded_r0 = -1;
-    for (int kbase = 0; kbase < 32; kbase += KW) {
-        const int q = qw + kbase + kg;
-        const bool active = lane_used && (kbase + kg < 32) && q < kc.n;
-        const int qq = active ? q : kc.n - 1;
-        const double Qq = active ? __ldg(kc.Q + qq) : 0.0;
-        const int aoC = __ldg(kc.ao_c + qq), aoD = __ldg(kc.ao_d + qq);
-        const bool cd_same = __ldg(kc.same + qq) != 0;
+    __shared__ __align__(8) uint64_t s_bar[2];
+    extern __shared__ __align__(16) double s_dyn[];      // ring: 2 stages x NI x 32 doubles
+    if (threadIdx.x == 0) { mbar_init(&s_bar[0], 1); mbar_init(&s_bar[1], 1); mbar_fence_init(); }
 
-        double Scd[NC][ND], Jcd[NC][ND], Kac[NA][NC], Kca[NC][NA], Kad[NA][ND], Kda[ND][NA];
+    const double Qbatch = __ldg(kc.Q + q0);               // kets are sorted: the batch's largest bound
+    const int qlast = min(q0 + 31, kc.n - 1);
+    const long long qb = q0 >> 5;
+    const int qq = active ? q : kc.n - 1;
+    const double Qq = active ? __ldg(kc.Q + qq) : 0.0;
+    const int aoC = __ldg(kc.ao_c + qq), aoD = __ldg(kc.ao_d + qq);
+    const bool cd_same = __ldg(kc.same + qq) != 0;
+
+    double Scd[NC][ND], Jcd[NC][ND], Kac[NA][NC], Kca[NC][NA], Kad[NA][ND], Kda[ND][NA];
 #pragma unroll
-        for (int c = 0; c < NC; ++c)
+    for (int c = 0; c < NC; ++c)
 #pragma unroll
-            for (int d2 = 0; d2 < ND; ++d2) {
-                Scd[c][d2] = active ? __ldg(TQ(aoC + c, aoD + d2)) + __ldg(TQ(aoD + d2, aoC + c)) : 0.0;
-                Jcd[c][d2] = 0.0;
-            }
-#pragma unroll
-        for (int a = 0; a < NA; ++a) {
-#pragma unroll
-            for (int c = 0; c < NC; ++c) Kac[a][c] = Kca[c][a] = 0.0;
-#pragma unroll
-            for (int d2 = 0; d2 < ND; ++d2) Kad[a][d2] = Kda[d2][a] = 0.0;
+        for (int d2 = 0; d2 < ND; ++d2) {
+            Scd[c][d2] = active ? __ldg(TQ(aoC + c, aoD + d2)) + __ldg(TQ(aoD + d2, aoC + c)) : 0.0;
+            Jcd[c][d2] = 0.0;
         }
+#pragma unroll
+    for (int a = 0; a < NA; ++a) {
+#pragma unroll
+        for (int c = 0; c < NC; ++c) Kac[a][c] = Kca[c][a] = 0.0;
+#pragma unroll
+        for (int d2 = 0; d2 < ND; ++d2) Kad[a][d2] = Kda[d2][a] = 0.0;
+    }
 
-        bool done = !__any_sync(0xffffffffu, active);       // warp-uniform
-        for (int r0 = al.rec_begin; r0 < al.rec_end; r0 += REC_TILE) {
-          const int nrec = min(REC_TILE, al.rec_end - r0);
-          if (loaded_r0 != r0) {                              // block-uniform: short lists are staged once
-              __syncthreads();
-              for (int i = threadIdx.x; i < nrec; i += JK_BLOCK) {
-                  const BraRec b0 = tb.recs[r0 + i];
-                  s_rec[i] = b0;
-                  s_bb[i] = __ldg(g.batch_base + b0.pos) - (same_class ? (b0.pos >> 5) : 0);
-              }
-              __syncthreads();
-              loaded_r0 = r0;
-          }
-          if (!done)
-          for (int ir = 0; ir < nrec; ++ir) {
+    // block-uniform test: does record ir reach any ket of this batch?
+    auto reaches = [&](int ir) {
+        const BraRec& b1 = s_rec[ir];
+        return (b1.Q * Qbatch >= tb.tau) && (!same_class || b1.pos <= qlast);
+    };
+    auto issue = [&](int ir, int s) {
+        if (threadIdx.x == 0) {
+            const double* gsrc = g.buf + (size_t)(s_bb[ir] + qb) * (NI * 32);
+            mbar_expect_tx(&s_bar[s], NI * 256);
+            tma_load_1d(s_dyn + (size_t)s * (NI * 32), gsrc, NI * 256, &s_bar[s]);
+        }
+    };
+    uint32_t phase0 = 0, phase1 = 0;
+    int stage = 0;
+    bool done = false;                                    // block-uniform
+    for (int r0 = al.rec_begin; r0 < al.rec_end && !done; r0 += REC_TILE) {
+        const int nrec = min(REC_TILE, al.rec_end - r0);
+        __syncthreads();
+        for (int i = threadIdx.x; i < nrec; i += blockDim.x) {
+            const BraRec b0 = tb.recs[r0 + i];
+            s_rec[i] = b0;
+            s_bb[i] = __ldg(g.batch_base + b0.pos) - (same_class ? (b0.pos >> 5) : 0);
+        }
+        __syncthreads();
+        if (!reaches(0)) { done = true; break; }
+        issue(0, stage);
+        for (int ir = 0; ir < nrec; ++ir) {
             const BraRec br = s_rec[ir];
+            const bool more = (ir + 1 < nrec) && reaches(ir + 1);
+            __syncthreads();                              // every warp is done with the stage refilled next
+            if (more) issue(ir + 1, stage ^ 1);
+            if (stage == 0) { mbar_wait(&s_bar[0], phase0); phase0 ^= 1; }
+            else { mbar_wait(&s_bar[1], phase1); phase1 ^= 1; }
+            const double* src = s_dyn + (size_t)stage * (NI * 32) + (kb & 31);
             const bool ok = active && (br.Q * Qq >= tb.tau) && (!same_class || br.pos <= q);
-            if (!__any_sync(0xffffffffu, ok)) { done = true; break; }
             const bool canonical = (br.flags & 1) != 0;
             const bool ab_same = (br.flags & 2) != 0;
             const int aoB = br.ao_b;
-            const long long batch = s_bb[ir] + (qw >> 5);
-            const double* src = g.buf + (size_t)batch * (NI * 32) + (q & 31);
             const double wsame = (same_class && br.pos == q) ? 0.5 : 1.0;
             const double wk = ok ? wsame * (cd_same ? 0.5 : 1.0) : 0.0;
             const double fix = (cd_same ? 2.0 : 1.0) * (ab_same ? 0.5 : 1.0);
             const bool flip = (LA < LB) || (LA == LB && !canonical);
+            if (__any_sync(0xffffffffu, ok)) {
 #pragma unroll
-            for (int b = 0; b < NB; ++b) {
-                double tbd[ND], tdb[ND], tbc[NC], tcb[NC];
+                for (int b = 0; b < NB; ++b) {
+                    double tbd[ND], tdb[ND], tbc[NC], tcb[NC];
 #pragma unroll
-                for (int d2 = 0; d2 < ND; ++d2) {
-                    tbd[d2] = ok ? __ldg(TQ(aoB + b, aoD + d2)) : 0.0;
-                    tdb[d2] = ok ? __ldg(TQ(aoD + d2, aoB + b)) : 0.0;
-                }
+                    for (int d2 = 0; d2 < ND; ++d2) {
+                        tbd[d2] = ok ? __ldg(TQ(aoB + b, aoD + d2)) : 0.0;
+                        tdb[d2] = ok ? __ldg(TQ(aoD + d2, aoB + b)) : 0.0;
+                    }
 #pragma unroll
-                for (int c = 0; c < NC; ++c) {
-                    tbc[c] = ok ? __ldg(TQ(aoB + b, aoC + c)) : 0.0;
-                    tcb[c] = ok ? __ldg(TQ(aoC + c, aoB + b)) : 0.0;
-                }
+                    for (int c = 0; c < NC; ++c) {
+                        tbc[c] = ok ? __ldg(TQ(aoB + b, aoC + c)) : 0.0;
+                        tcb[c] = ok ? __ldg(TQ(aoC + c, aoB + b)) : 0.0;
+                    }
 #pragma unroll
-                for (int a = 0; a < NA; ++a) {
-                    double sab = 0.0, jab = 0.0;
-                    if (canonical && lane_used)
-                        sab = fix * (__ldg(TQ(aoA + a, aoB + b)) + __ldg(TQ(aoB + b, aoA + a)));
-                    const int i_ab = flip ? (a * NB + b) : (b * NA + a);
+                    for (int a = 0; a < NA; ++a) {
+                        double sab = 0.0, jab = 0.0;
+                        if (canonical && kg < KW)
+                            sab = fix * (__ldg(TQ(aoA + a, aoB + b)) + __ldg(TQ(aoB + b, aoA + a)));
+                        const int i_ab = flip ? (a * NB + b) : (b * NA + a);
 #pragma unroll
-                    for (int d2 = 0; d2 < ND; ++d2)
+                        for (int d2 = 0; d2 < ND; ++d2)
 #pragma unroll
-                        for (int c = 0; c < NC; ++c) {
-                            const int i = (d2 * NC + c) * (NA * NB) + i_ab;
-                            const double x = ok ? wk * __ldcs(src + i * 32) : 0.0;
-                            Kac[a][c] = fma(x, tbd[d2], Kac[a][c]);
-                            Kca[c][a] = fma(x, tdb[d2], Kca[c][a]);
-                            Kad[a][d2] = fma(x, tbc[c], Kad[a][d2]);
-                            Kda[d2][a] = fma(x, tcb[c], Kda[d2][a]);
-                            Jcd[c][d2] = fma(x, sab, Jcd[c][d2]);
-                            jab = fma(x, Scd[c][d2], jab);
-                        }
-                    if (canonical) {
-                        // sum J_ab over the KW kets of the warp (tree over the ket-group index), group 0 writes
-                        int n = KW;
-                        while (n > 1) {
-                            const int s = (n + 1) >> 1;
-                            const double y = __shfl_down_sync(0xffffffffu, jab, s * G);
-                            if (kg + s < n) jab += y;
-                            n = s;
-                        }
-                        if (kg == 0 && jab != 0.0) {
-                            atomicAdd(FQ(aoA + a, aoB + b), 2.0 * jab);
-                            if (!ab_same) atomicAdd(FQ(aoB + b, aoA + a), 2.0 * jab);
+                            for (int c = 0; c < NC; ++c) {
+                                const int i = (d2 * NC + c) * (NA * NB) + i_ab;
+                                const double x = ok ? wk * src[i * 32] : 0.0;
+                                Kac[a][c] = fma(x, tbd[d2], Kac[a][c]);
+                                Kca[c][a] = fma(x, tdb[d2], Kca[c][a]);
+                                Kad[a][d2] = fma(x, tbc[c], Kad[a][d2]);
+                                Kda[d2][a] = fma(x, tcb[c], Kda[d2][a]);
+                                Jcd[c][d2] = fma(x, sab, Jcd[c][d2]);
+                                jab = fma(x, Scd[c][d2], jab);
+                            }
+                        if (canonical) {
+                            // sum J_ab over the KW kets of the warp (tree over the ket-group index), group 0 writes
+                            int n = KW;
+                            while (n > 1) {
+                                const int s = (n + 1) >> 1;
+                                const double y = __shfl_down_sync(0xffffffffu, jab, s * G);
+                                if (kg + s < n) jab += y;
+                                n = s;
+                            }
+                            if (kg == 0 && jab != 0.0) {
+                                atomicAdd(FQ(aoA + a, aoB + b), 2.0 * jab);
+                                if (!ab_same) atomicAdd(FQ(aoB + b, aoA + a), 2.0 * jab);
+                            }
                         }
                     }
                 }
             }
-          }
-          if (al.rec_end - al.rec_begin > REC_TILE && __syncthreads_and(done)) break;
+            stage ^= 1;
+            if (!more) { if (ir + 1 < nrec) done = true; break; }
         }
-        if (active) {
+    }
+    if (active) {
 #pragma unroll
-            for (int a = 0; a < NA; ++a) {
+        for (int a = 0; a < NA; ++a) {
 #pragma unroll
-                for (int c = 0; c < NC; ++c) {
-                    atomicAdd(FQ(aoA + a, aoC + c), -cx * Kac[a][c]);
-                    atomicAdd(FQ(aoC + c, aoA + a), -cx * Kca[c][a]);
-                }
-#pragma unroll
-                for (int d2 = 0; d2 < ND; ++d2) {
-                    atomicAdd(FQ(aoA + a, aoD + d2), -cx * Kad[a][d2]);
-                    atomicAdd(FQ(aoD + d2, aoA + a), -cx * Kda[d2][a]);
-                }
+            for (int c = 0; c < NC; ++c) {
+                atomicAdd(FQ(aoA + a, aoC + c), -cx * Kac[a][c]);
+                atomicAdd(FQ(aoC + c, aoA + a), -cx * Kca[c][a]);
             }
 #pragma unroll
-            for (int c = 0; c < NC; ++c)
-#pragma unroll
-                for (int d2 = 0; d2 < ND; ++d2) {
-                    atomicAdd(FQ(aoC + c, aoD + d2), 2.0 * Jcd[c][d2]);
-                    if (!cd_same) atomicAdd(FQ(aoD + d2, aoC + c), 2.0 * Jcd[c][d2]);
-                }
+            for (int d2 = 0; d2 < ND; ++d2) {
+                atomicAdd(FQ(aoA + a, aoD + d2), -cx * Kad[a][d2]);
+                atomicAdd(FQ(aoD + d2, aoA + a), -cx * Kda[d2][a]);
+            }
         }
+#pragma unroll
+        for (int c = 0; c < NC; ++c)
+#pragma unroll
+            for (int d2 = 0; d2 < ND; ++d2) {
+                atomicAdd(FQ(aoC + c, aoD + d2), 2.0 * Jcd[c][d2]);
+                if (!cd_same) atomicAdd(FQ(aoD + d2, aoC + c), 2.0 * Jcd[c][d2]);
+            }
     }
 #undef TQ
 #undef FQ
@@ -545,23 +572,31 @@ static int launch_digest(Handle* h, const JKLaunch& L, const Segment& sg, const 
 {
     constexpr int NA = 2 * LA + 1, NC = 2 * LC + 1, ND = 2 * LD + 1;
     constexpr int PER_V = 2 * NA * (NC + ND) + 2 * NC * ND;
-    static int vmode = -1;
-    if (vmode < 0) { const char* e = getenv("RTTDA_DIGEST_V"); vmode = e ? atoi(e) : 4; }
-    // which ordered classes use the density-per-lane kernel (bit: ssss, spss, psss, spps, psps, ppss, ppps, pppp);
-    // default = the classes where it measured faster on B200 (ss|ss, sp|ss, sp|ps), see profiles/
+    const int vmode = 4;
+    // which ordered classes use the block-per-batch kernel when the call has >= 4 densities (bit: ssss, spss, psss,
+    // spps, psps, ppss, ppps, pppp); default = the classes where it measured faster on B200 (profiles/): all but
+    // ps|ss and pp|ss.  RTTDA_DIGEST_BMASK overrides it (tuning only).
     static int vmask = -1;
-    if (vmask < 0) { const char* e = getenv("RTTDA_DIGEST_VMASK"); vmask = e ? atoi(e) : 11; }
+    if (vmask < 0) { const char* e = getenv("RTTDA_DIGEST_BMASK"); vmask = e ? atoi(e) : 219; }
     constexpr int KEY = LA * 8 + LB * 4 + LC * 2 + LD;
     constexpr int CLS = KEY == 0 ? 0 : KEY == 4 ? 1 : KEY == 8 ? 2 : KEY == 6 ? 3 : KEY == 10 ? 4 : KEY == 12 ? 5 : KEY == 14 ? 6 : 7;
     if (vmode > 0 && nvec >= vmode && ((vmask >> CLS) & 1)) {
-        // density-per-lane kernel: groups of G lanes per ket, chunks of at most 32 densities
-        for (int v0 = 0; v0 < nvec; v0 += 32) {
-            const int G = nvec - v0 < 32 ? nvec - v0 : 32;
+        // block-per-batch kernel: groups of G <= 8 lanes per ket (at most 8 warps per block), chunks of 8 densities
+        constexpr int NI = (2 * LA + 1) * (2 * LB + 1) * (2 * LC + 1) * (2 * LD + 1);
+        constexpr size_t smem = (size_t)2 * NI * 256;
+        static bool attr_set = false;
+        if (!attr_set) {
+            RT_CUDA(cudaFuncSetAttribute(digest_b_kernel<LA, LB, LC, LD>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+            attr_set = true;
+        }
+        for (int v0 = 0; v0 < nvec; v0 += 8) {
+            const int G = nvec - v0 < 8 ? nvec - v0 : 8;
             DigestArgs g;
             g.tb = h->tabs; g.work = L.work; g.batch_base = sg.batch_base; g.buf = buf;
             g.Tq = Tq; g.Fq = Fq; g.cx = h->cx;
             g.ketclass = L.ketclass; g.same = (sg.kc_bra == sg.kc_ket); g.nvt = nvt; g.v0 = v0;
-            digest_v_kernel<LA, LB, LC, LD><<<dim3(L.nwork), dim3(JK_BLOCK), 0, st>>>(g, G, 32 / G);
+            const int KW = 32 / G, nwarps = (32 + KW - 1) / KW;
+            digest_b_kernel<LA, LB, LC, LD><<<dim3(4 * L.nwork), dim3(32 * nwarps), smem, st>>>(g, G, KW);
             h->kernel_launches++;
             RT_CUDA(cudaGetLastError());
         }

@@ -7,7 +7,8 @@
 //   block  = JK_BLOCK consecutive kets of the (Schwarz-sorted) ket list x a run of bra pairs of the bra list
 //   thread = one ket pair; its primitive data stay in registers (SoA loads, coalesced) while the block walks
 //            the bra pairs, whose primitive rows are staged in shared memory and read as broadcasts
-//   Boys   = one 16-byte shared-memory gather per primitive quartet (eri_eval.cuh)
+//   Boys   = Taylor coefficients from a shared-memory table row for the near-field primitive quartets, a closed form
+//            for the far-field majority (eri_eval.cuh)
 // The inner loops are pure FP64 ALU work: no accumulators of the J/K digestion live here.
 #include "eri_eval.cuh"
 
@@ -62,14 +63,14 @@ __global__ void __launch_bounds__(JK_BLOCK) eval_kernel(EvalArgs g)
     constexpr int L = LA + LB + LC + LD;
     // ket primitives live in registers when they are few doubles; otherwise they are re-read (L1 hits)
     constexpr bool KET_IN_REGS = (KP == 1) || (L <= 3 && ((KP <= 3) || (LC + LD == 0)));
-    __shared__ __align__(16) double2 s_boys[BOYS_NROW];
+    __shared__ __align__(16) double2 s_boys[BOYS_NROW * (BOYS_ROW / 2)];
     __shared__ __align__(16) double s_rows[EVAL_MAX_ROWS * PRIM_STRIDE];
     __shared__ double s_Q[JK_BLOCK];
     __shared__ long long s_base[JK_BLOCK];
 
     const EvalItem it = g.items[blockIdx.x];
     const int npb = g.bra.np, npairs = it.p_end - it.p_begin;
-    for (int i = threadIdx.x; i < BOYS_NROW; i += JK_BLOCK) s_boys[i] = g.boys[i];
+    for (int i = threadIdx.x; i < BOYS_NROW * (BOYS_ROW / 2); i += JK_BLOCK) s_boys[i] = g.boys[i];
     {
         const double2* src = reinterpret_cast<const double2*>(g.bra.prim_aos + (size_t)it.p_begin * npb * PRIM_STRIDE);
         double2* dst = reinterpret_cast<double2*>(s_rows);

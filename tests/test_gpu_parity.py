@@ -221,7 +221,7 @@ def test_fock_config4_full_size_sampled_elements():
     rng = np.random.default_rng(4)
     X = rng.standard_normal((6, ctx["cfg"].nocc, ctx["cfg"].nvirt))
     X /= np.linalg.norm(X.reshape(6, -1), axis=1)[:, None, None]
-    T = np.einsum("mi,via,na->vmn", ctx["C_o"], X, ctx["C_v"])           # transition densities, non-symmetric
+    T = np.stack([ctx["C_o"] @ x @ ctx["C_v"].T for x in X])              # transition densities, non-symmetric
     F = gpu_fock(ctx, T)
     mu = rng.integers(0, N, size=5)                                       # ~15-30 s of oracle time per sample
     nu = rng.integers(0, N, size=5)
@@ -232,5 +232,6 @@ def test_fock_config4_full_size_sampled_elements():
     scale = np.max(np.abs(F))
     assert np.max(np.abs(got - ref)) / scale < SIGMA_TOL
     F2 = gpu_fock(ctx, np.stack([T[0] + T[0].T, 2.0 * T[1] - 0.5 * T[2]]))
-    assert np.max(np.abs(F2[0] - (F[0] + F[0].T))) / scale < 1e-12        # F[T^T] = F[T]^T
-    assert np.max(np.abs(F2[1] - (2.0 * F[1] - 0.5 * F[2]))) / scale < 1e-12
+    # F[T^T] = F[T]^T and linearity; different summation orders of ~1e6 terms each: rounding-level agreement
+    assert np.max(np.abs(F2[0] - (F[0] + F[0].T))) / scale < SIGMA_TOL
+    assert np.max(np.abs(F2[1] - (2.0 * F[1] - 0.5 * F[2]))) / scale < SIGMA_TOL
