@@ -77,35 +77,9 @@ struct AList {
     double Qmax;
     int ao_a;
     int rec_begin, rec_end;   // into BraRec array
+    int jrec_begin, jrec_end; // into the array of canonical records only (J-only digestion)
     int ketclass;             // class id of the (unordered) pairs in this list
     int np;                   // primitive pairs per record
-};
-
-// Shell-blocked a-lists of the block-per-batch digestion kernel: M (2 or 4) shells a_i of one shell class,
-// neighbours in space (consecutive along a Morton curve), share ONE walk over the union of their partners b, so
-// that every density element gathered for (b, c), (b, d) is reused for up to M quartets (a_i b|c d).
-constexpr int SUPER_MAX = 4;
-struct SHead {              // one partner shell b of the group
-    double Qmax;            // largest Schwarz bound over the members' pairs (a_i, b)
-    int ao_b;
-    int pad;
-};
-struct SMem {               // pair (a_i, b) of member i
-    double Q;               // 0 if the pair is absent
-    int pos;                // position of the unordered pair inside its class list
-    int flags;              // bit0 canonical, bit1 a == b, bit2 present
-};
-struct SAList {
-    double Qmax;
-    int ao_a[SUPER_MAX];      // AO offsets of the members (-1: slot unused)
-    int rec_begin, rec_end;   // into SHead array; members at [rec * M + i]
-    int ketclass, minpos;
-};
-struct SuperSet {             // device tables of one blocking factor M
-    int M;
-    const SHead* heads;
-    const SMem* mems;
-    const SAList* lists;
 };
 
 struct WorkItem {
@@ -140,15 +114,13 @@ struct JKLaunch {             // one digestion kernel instantiation: ordered bra
     int seg;
     int nwork;
     const WorkItem* work;     // device
-    int nswork[2];            // blocks over the shell-blocked a-lists, M = 2 and M = 4
-    const WorkItem* swork[2];
 };
 
 struct JKTables {
     KetClass kets[NKETCLASS];
     const BraRec* recs;
+    const BraRec* jrecs;      // the canonical records of every a-list, in the same order
     const AList* alists;
-    SuperSet super[2];        // M = 2, M = 4
     const double2* boys[5];   // per total angular momentum L: rows {F_{L+k}(j/8)/k!, k < 8; exp(-j/8); pad}
     double tau;
     int nao;

@@ -110,10 +110,12 @@ struct VecLoad {
 // Stored component order (jk_eval.cu): canonical pair orientation (first shell = higher l), eri_index of
 // eri_eval.cuh: ((d * NC + c) * N2 + c2) * N1 + c1 with (c1, c2) the components of the canonical first/second
 // shell.
-template <int LA, int LB, int LC, int LD, int NV>
+// MODE 0: J and K; 1: J only (walks the canonical records of the a-list, no density gathers); 2: K only.
+template <int LA, int LB, int LC, int LD, int NV, int MODE>
 __global__ void __launch_bounds__(JK_BLOCK)
 digest_kernel(DigestArgs g)
 {
+    constexpr bool DO_J = MODE != 2, DO_K = MODE != 1;
     constexpr int NA = 2 * LA + 1, NB = 2 * LB + 1, NC = 2 * LC + 1, ND = 2 * LD + 1;
     constexpr int NI = NA * NB * NC * ND;
     constexpr bool USE_TMA = digest_uses_tma(NI);
@@ -194,11 +196,13 @@ digest_kernel(DigestArgs g)
         return active && (b1.Q * Qq >= tb.tau) && (!same_class || b1.pos <= q);
     };
     bool done = false;                                      // warp-uniform
-    for (int r0 = al.rec_begin; r0 < al.rec_end; r0 += REC_TILE) {
-      const int nrec = min(REC_TILE, al.rec_end - r0);
+    const BraRec* recs = MODE == 1 ? tb.jrecs : tb.recs;
+    const int rec_begin = MODE == 1 ? al.jrec_begin : al.rec_begin, rec_end = MODE == 1 ? al.jrec_end : al.rec_end;
+    for (int r0 = rec_begin; r0 < rec_end; r0 += REC_TILE) {
+      const int nrec = min(REC_TILE, rec_end - r0);
       __syncthreads();
       for (int i = threadIdx.x; i < nrec; i += JK_BLOCK) {
-          const BraRec b0 = tb.recs[r0 + i];
+          const BraRec b0 = recs[r0 + i];
           s_rec[i] = b0;
           s_bb[i] = __ldg(g.batch_base + b0.pos) - (same_class ? (b0.pos >> 5) : 0);
       }
@@ -240,7 +244,7 @@ digest_kernel(DigestArgs g)
 #pragma unroll
         for (int b = 0; b < NB; ++b) {
             double tbd[ND][NV], tdb[ND][NV], tbc[NC][NV], tcb[NC][NV];
-            if (ok) {
+            if (DO_K && ok) {
 #pragma unroll
                 for (int d = 0; d < ND; ++d) {
                     VecLoad<NV>::ld(TQ(aoB + b, aoD + d), tbd[d]);
@@ -263,7 +267,7 @@ digest_kernel(DigestArgs g)
 #pragma unroll
             for (int a = 0; a < NA; ++a) {
                 double sab[NV], jab[next_pow2(NV)];
-                if (canonical) {
+                if (DO_J && canonical) {
                     double x[NV], y[NV];
                     VecLoad<NV>::ld(TQ(aoA + a, aoB + b), x);
                     VecLoad<NV>::ld(TQ(aoB + b, aoA + a), y);
@@ -285,16 +289,20 @@ digest_kernel(DigestArgs g)
                         const double x = ok ? wk * (USE_TMA ? src[i * 32] : __ldcs(src + i * 32)) : 0.0;
 #pragma unroll
                         for (int v = 0; v < NV; ++v) {
-                            Kac[a][c][v] = fma(x, tbd[d][v], Kac[a][c][v]);
-                            Kca[c][a][v] = fma(x, tdb[d][v], Kca[c][a][v]);
-                            Kad[a][d][v] = fma(x, tbc[c][v], Kad[a][d][v]);
-                            Kda[d][a][v] = fma(x, tcb[c][v], Kda[d][a][v]);
-                            Jcd[c][d][v] = fma(x, sab[v], Jcd[c][d][v]);
-                            jab[v] = fma(x, Scd[c][d][v], jab[v]);
+                            if (DO_K) {
+                                Kac[a][c][v] = fma(x, tbd[d][v], Kac[a][c][v]);
+                                Kca[c][a][v] = fma(x, tdb[d][v], Kca[c][a][v]);
+                                Kad[a][d][v] = fma(x, tbc[c][v], Kad[a][d][v]);
+                                Kda[d][a][v] = fma(x, tcb[c][v], Kda[d][a][v]);
+                            }
+                            if (DO_J) {
+                                Jcd[c][d][v] = fma(x, sab[v], Jcd[c][d][v]);
+                                jab[v] = fma(x, Scd[c][d][v], jab[v]);
+                            }
                         }
                     }
                 // ---- Coulomb J_ab: only the canonical orientation of the bra pair does it (uniform branch)
-                if (canonical) {
+                if (DO_J && canonical) {
                     constexpr int NP = next_pow2(NV);
                     const double tot = warp_reduce_multi<NP>(jab, lane);
                     const int v = warp_reduce_owner_index<NP>(lane);
@@ -315,26 +323,30 @@ digest_kernel(DigestArgs g)
     if (!active) return;
     // ---- flush the register accumulators: F += 2 J - cx K
     const double cx = g.cx;
+    if (DO_K) {
 #pragma unroll
-    for (int a = 0; a < NA; ++a) {
+        for (int a = 0; a < NA; ++a) {
 #pragma unroll
-        for (int c = 0; c < NC; ++c) {
-            red_add<NV>(Fv + (size_t)(aoA + a) * rs + (size_t)(aoC + c) * nvt, Kac[a][c], -cx);
-            red_add<NV>(Fv + (size_t)(aoC + c) * rs + (size_t)(aoA + a) * nvt, Kca[c][a], -cx);
-        }
+            for (int c = 0; c < NC; ++c) {
+                red_add<NV>(Fv + (size_t)(aoA + a) * rs + (size_t)(aoC + c) * nvt, Kac[a][c], -cx);
+                red_add<NV>(Fv + (size_t)(aoC + c) * rs + (size_t)(aoA + a) * nvt, Kca[c][a], -cx);
+            }
 #pragma unroll
-        for (int d = 0; d < ND; ++d) {
-            red_add<NV>(Fv + (size_t)(aoA + a) * rs + (size_t)(aoD + d) * nvt, Kad[a][d], -cx);
-            red_add<NV>(Fv + (size_t)(aoD + d) * rs + (size_t)(aoA + a) * nvt, Kda[d][a], -cx);
+            for (int d = 0; d < ND; ++d) {
+                red_add<NV>(Fv + (size_t)(aoA + a) * rs + (size_t)(aoD + d) * nvt, Kad[a][d], -cx);
+                red_add<NV>(Fv + (size_t)(aoD + d) * rs + (size_t)(aoA + a) * nvt, Kda[d][a], -cx);
+            }
         }
     }
+    if (DO_J) {
 #pragma unroll
-    for (int c = 0; c < NC; ++c)
+        for (int c = 0; c < NC; ++c)
 #pragma unroll
-        for (int d = 0; d < ND; ++d) {
-            red_add<NV>(Fv + (size_t)(aoC + c) * rs + (size_t)(aoD + d) * nvt, Jcd[c][d], 2.0);
-            if (!cd_same) red_add<NV>(Fv + (size_t)(aoD + d) * rs + (size_t)(aoC + c) * nvt, Jcd[c][d], 2.0);
-        }
+            for (int d = 0; d < ND; ++d) {
+                red_add<NV>(Fv + (size_t)(aoC + c) * rs + (size_t)(aoD + d) * nvt, Jcd[c][d], 2.0);
+                if (!cd_same) red_add<NV>(Fv + (size_t)(aoD + d) * rs + (size_t)(aoC + c) * nvt, Jcd[c][d], 2.0);
+            }
+    }
 }
 
 // ---------------------------------------------------------------------------------------------------
@@ -344,7 +356,7 @@ digest_kernel(DigestArgs g)
 // memory ring shared by all warps (the copy of record r+1 flies while record r is digested); every density access
 // is a contiguous 8*G-byte run of an aligned slot; a lane carries one density's accumulators only, so all
 // densities of the call are served by one read of the staged integrals.
-template <int LA, int LB, int LC, int LD>
+template <int LA, int LB, int LC, int LD, bool DO_J>
 __global__ void __launch_bounds__(256)
 digest_b_kernel(DigestArgs g, int G, int KW)
 {
@@ -390,7 +402,7 @@ digest_b_kernel(DigestArgs g, int G, int KW)
     for (int c = 0; c < NC; ++c)
 #pragma unroll
         for (int d2 = 0; d2 < ND; ++d2) {
-            Scd[c][d2] = active ? __ldg(TQ(aoC + c, aoD + d2)) + __ldg(TQ(aoD + d2, aoC + c)) : 0.0;
+            Scd[c][d2] = (DO_J && active) ? __ldg(TQ(aoC + c, aoD + d2)) + __ldg(TQ(aoD + d2, aoC + c)) : 0.0;
             Jcd[c][d2] = 0.0;
         }
 #pragma unroll
@@ -460,7 +472,7 @@ digest_b_kernel(DigestArgs g, int G, int KW)
 #pragma unroll
                     for (int a = 0; a < NA; ++a) {
                         double sab = 0.0, jab = 0.0;
-                        if (canonical && kg < KW)
+                        if (DO_J && canonical && kg < KW)
                             sab = fix * (__ldg(TQ(aoA + a, aoB + b)) + __ldg(TQ(aoB + b, aoA + a)));
                         const int i_ab = flip ? (a * NB + b) : (b * NA + a);
 #pragma unroll
@@ -473,10 +485,12 @@ digest_b_kernel(DigestArgs g, int G, int KW)
                                 Kca[c][a] = fma(x, tdb[d2], Kca[c][a]);
                                 Kad[a][d2] = fma(x, tbc[c], Kad[a][d2]);
                                 Kda[d2][a] = fma(x, tcb[c], Kda[d2][a]);
-                                Jcd[c][d2] = fma(x, sab, Jcd[c][d2]);
-                                jab = fma(x, Scd[c][d2], jab);
+                                if (DO_J) {
+                                    Jcd[c][d2] = fma(x, sab, Jcd[c][d2]);
+                                    jab = fma(x, Scd[c][d2], jab);
+                                }
                             }
-                        if (canonical) {
+                        if (DO_J && canonical) {
                             // sum J_ab over the KW kets of the warp (tree over the ket-group index), group 0 writes
                             int n = KW;
                             while (n > 1) {
@@ -511,13 +525,15 @@ digest_b_kernel(DigestArgs g, int G, int KW)
                 atomicAdd(FQ(aoD + d2, aoA + a), -cx * Kda[d2][a]);
             }
         }
+        if (DO_J) {
 #pragma unroll
-        for (int c = 0; c < NC; ++c)
+            for (int c = 0; c < NC; ++c)
 #pragma unroll
-            for (int d2 = 0; d2 < ND; ++d2) {
-                atomicAdd(FQ(aoC + c, aoD + d2), 2.0 * Jcd[c][d2]);
-                if (!cd_same) atomicAdd(FQ(aoD + d2, aoC + c), 2.0 * Jcd[c][d2]);
-            }
+                for (int d2 = 0; d2 < ND; ++d2) {
+                    atomicAdd(FQ(aoC + c, aoD + d2), 2.0 * Jcd[c][d2]);
+                    if (!cd_same) atomicAdd(FQ(aoD + d2, aoC + c), 2.0 * Jcd[c][d2]);
+                }
+        }
     }
 #undef TQ
 #undef FQ
@@ -542,7 +558,7 @@ static int class_nv_max(int la, int lb, int lc, int ld)
     return 1;                          // pp|pp
 }
 
-template <int LA, int LB, int LC, int LD, int NV>
+template <int LA, int LB, int LC, int LD, int NV, int MODE = 0>
 static int launch_digest_nv(Handle* h, const JKLaunch& L, const Segment& sg, const double* buf, int nvt, int v0,
                             const double* Tq, double* Fq, cudaStream_t st)
 {
@@ -557,10 +573,10 @@ static int launch_digest_nv(Handle* h, const JKLaunch& L, const Segment& sg, con
     constexpr size_t smem = digest_ring_bytes(NI);
     static bool attr_set = false;
     if (!attr_set && smem > 0) {
-        RT_CUDA(cudaFuncSetAttribute(digest_kernel<LA, LB, LC, LD, NV>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        RT_CUDA(cudaFuncSetAttribute(digest_kernel<LA, LB, LC, LD, NV, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         attr_set = true;
     }
-    digest_kernel<LA, LB, LC, LD, NV><<<dim3(L.nwork), dim3(JK_BLOCK), smem, st>>>(g);
+    digest_kernel<LA, LB, LC, LD, NV, MODE><<<dim3(L.nwork), dim3(JK_BLOCK), smem, st>>>(g);
     h->kernel_launches++;
     RT_CUDA(cudaGetLastError());
     return RTTDA_OK;
@@ -574,19 +590,35 @@ static int launch_digest(Handle* h, const JKLaunch& L, const Segment& sg, const 
     constexpr int PER_V = 2 * NA * (NC + ND) + 2 * NC * ND;
     const int vmode = 4;
     // which ordered classes use the block-per-batch kernel when the call has >= 4 densities (bit: ssss, spss, psss,
-    // spps, psps, ppss, ppps, pppp); default = the classes where it measured faster on B200 (profiles/): all but
-    // ps|ss and pp|ss.  RTTDA_DIGEST_BMASK overrides it (tuning only).
+    // spps, psps, ppss, ppps, pppp); default = all (with the Coulomb part split off it measured faster for every
+    // class on B200, profiles/).  RTTDA_DIGEST_BMASK overrides it (tuning only).
     static int vmask = -1;
-    if (vmask < 0) { const char* e = getenv("RTTDA_DIGEST_BMASK"); vmask = e ? atoi(e) : 219; }
+    if (vmask < 0) { const char* e = getenv("RTTDA_DIGEST_BMASK"); vmask = e ? atoi(e) : 255; }
     constexpr int KEY = LA * 8 + LB * 4 + LC * 2 + LD;
     constexpr int CLS = KEY == 0 ? 0 : KEY == 4 ? 1 : KEY == 8 ? 2 : KEY == 6 ? 3 : KEY == 10 ? 4 : KEY == 12 ? 5 : KEY == 14 ? 6 : 7;
     if (vmode > 0 && nvec >= vmode && ((vmask >> CLS) & 1)) {
-        // block-per-batch kernel: groups of G <= 8 lanes per ket (at most 8 warps per block), chunks of 8 densities
+        // Coulomb part: thread-per-ket kernel in J-only mode over the canonical records (no density gathers, the
+        // J_ab sums amortise one warp butterfly over 32 kets); launches of the flipped orientation (la < lb) hold
+        // no canonical record.  Exchange part: block-per-batch kernel, lane = density, K only.
+        static int jsplit = -1;
+        if (jsplit < 0) { const char* e = getenv("RTTDA_DIGEST_JSPLIT"); jsplit = e ? atoi(e) : 1; }
+        if (jsplit && LA >= LB) {
+            constexpr int NVJ = (NC * ND <= 3) ? 8 : 4;
+            int v0 = 0;
+            while (v0 < nvec) {
+                const int left = nvec - v0;
+                if (left >= NVJ) { RT_TRY((launch_digest_nv<LA, LB, LC, LD, NVJ, 1>(h, L, sg, buf, nvt, v0, Tq, Fq, st))); v0 += NVJ; }
+                else if (NVJ == 8 && left >= 6) { RT_TRY((launch_digest_nv<LA, LB, LC, LD, 6, 1>(h, L, sg, buf, nvt, v0, Tq, Fq, st))); v0 += 6; }
+                else if (left >= 4) { RT_TRY((launch_digest_nv<LA, LB, LC, LD, 4, 1>(h, L, sg, buf, nvt, v0, Tq, Fq, st))); v0 += 4; }
+                else { RT_TRY((launch_digest_nv<LA, LB, LC, LD, 2, 1>(h, L, sg, buf, nvt, v0, Tq, Fq, st))); v0 += 2; }
+            }
+        }
         constexpr int NI = (2 * LA + 1) * (2 * LB + 1) * (2 * LC + 1) * (2 * LD + 1);
         constexpr size_t smem = (size_t)2 * NI * 256;
         static bool attr_set = false;
         if (!attr_set) {
-            RT_CUDA(cudaFuncSetAttribute(digest_b_kernel<LA, LB, LC, LD>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+            RT_CUDA(cudaFuncSetAttribute(digest_b_kernel<LA, LB, LC, LD, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+            RT_CUDA(cudaFuncSetAttribute(digest_b_kernel<LA, LB, LC, LD, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
             attr_set = true;
         }
         for (int v0 = 0; v0 < nvec; v0 += 8) {
@@ -596,7 +628,10 @@ static int launch_digest(Handle* h, const JKLaunch& L, const Segment& sg, const 
             g.Tq = Tq; g.Fq = Fq; g.cx = h->cx;
             g.ketclass = L.ketclass; g.same = (sg.kc_bra == sg.kc_ket); g.nvt = nvt; g.v0 = v0;
             const int KW = 32 / G, nwarps = (32 + KW - 1) / KW;
-            digest_b_kernel<LA, LB, LC, LD><<<dim3(4 * L.nwork), dim3(32 * nwarps), smem, st>>>(g, G, KW);
+            if (jsplit)
+                digest_b_kernel<LA, LB, LC, LD, false><<<dim3(4 * L.nwork), dim3(32 * nwarps), smem, st>>>(g, G, KW);
+            else
+                digest_b_kernel<LA, LB, LC, LD, true><<<dim3(4 * L.nwork), dim3(32 * nwarps), smem, st>>>(g, G, KW);
             h->kernel_launches++;
             RT_CUDA(cudaGetLastError());
         }

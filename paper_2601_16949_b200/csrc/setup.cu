@@ -338,7 +338,7 @@ int create_impl(Handle* h, const rttda_basis_t* basis, const double* C_occ, cons
             groups[{P.s1, H.l[P.s2], P.sub}].push_back({P.s1, P.s2, k, 1});
             if (P.s1 != P.s2) groups[{P.s2, H.l[P.s1], P.sub}].push_back({P.s2, P.s1, k, 0});
         }
-    std::vector<BraRec> recs;
+    std::vector<BraRec> recs, jrecs;
     std::vector<AList> alists;
     std::vector<int> alist_la, alist_lb;
     for (auto& g : groups) {
@@ -347,6 +347,7 @@ int create_impl(Handle* h, const rttda_basis_t* basis, const double* C_occ, cons
         AList al;
         al.ao_a = H.ao[std::get<0>(g.first)];
         al.rec_begin = (int)recs.size();
+        al.jrec_begin = (int)jrecs.size();
         al.ketclass = pairs[v[0].pair].pc * NSUB + pairs[v[0].pair].sub;
         al.np = pairs[v[0].pair].np;
         al.Qmax = pairs[v[0].pair].Q;
@@ -357,106 +358,17 @@ int create_impl(Handle* h, const rttda_basis_t* basis, const double* C_occ, cons
             br.flags = (r.canonical ? 1 : 0) | (r.a == r.b ? 2 : 0);
             br.pad = 0;
             recs.push_back(br);
+            if (r.canonical) jrecs.push_back(br);
         }
         al.rec_end = (int)recs.size();
+        al.jrec_end = (int)jrecs.size();
         alists.push_back(al);
         alist_la.push_back(H.l[std::get<0>(g.first)]);
         alist_lb.push_back(std::get<1>(g.first));
     }
     RT_TRY(upload(h, recs, &h->tabs.recs));
+    RT_TRY(upload(h, jrecs, &h->tabs.jrecs));
     RT_TRY(upload(h, alists, &h->tabs.alists));
-
-    // ---- shell-blocked a-lists: M shells of one shell class, consecutive along a Morton curve through their
-    //      centres, share one walk over the union of their partners
-    struct SuperHost {
-        std::vector<SHead> heads; std::vector<SMem> mems; std::vector<SAList> lists;
-        std::vector<int> la, lb;
-    };
-    SuperHost superh[2];
-    {
-        double lo[3] = {1e300, 1e300, 1e300}, hi[3] = {-1e300, -1e300, -1e300};
-        for (size_t c = 0; c < H.xyz.size() / 3; ++c)
-            for (int x = 0; x < 3; ++x) { lo[x] = std::min(lo[x], H.xyz[3 * c + x]); hi[x] = std::max(hi[x], H.xyz[3 * c + x]); }
-        auto morton = [&](int shell) {
-            unsigned long long code = 0;
-            unsigned v[3];
-            for (int x = 0; x < 3; ++x) {
-                const double t = (H.xyz[3 * H.center[shell] + x] - lo[x]) / std::max(hi[x] - lo[x], 1e-12);
-                v[x] = (unsigned)std::min(1023.0, std::max(0.0, t * 1023.0));
-            }
-            for (int bit = 9; bit >= 0; --bit)
-                for (int x = 0; x < 3; ++x) code = (code << 1) | ((v[x] >> bit) & 1u);
-            return code;
-        };
-        std::map<std::pair<int, int>, std::vector<int>> shell_classes;      // (l, nprim) -> shells in Morton order
-        for (int sidx = 0; sidx < H.nshells; ++sidx) shell_classes[{H.l[sidx], H.np[sidx]}].push_back(sidx);
-        for (auto& sc : shell_classes)
-            std::stable_sort(sc.second.begin(), sc.second.end(), [&](int x, int y) {
-                const unsigned long long mx = morton(x), my = morton(y);
-                return mx != my ? mx < my : x < y;
-            });
-        for (int ms = 0; ms < 2; ++ms) {
-            const int M = ms == 0 ? 2 : 4;
-            SuperHost& S = superh[ms];
-            for (auto& sc : shell_classes) {
-                const std::vector<int>& sh = sc.second;
-                for (size_t g0 = 0; g0 < sh.size(); g0 += M) {
-                    const int nm = (int)std::min<size_t>(M, sh.size() - g0);
-                    std::map<std::pair<int, int>, std::map<int, std::vector<const Rec*>>> by_class;   // (l_b, sub) -> b -> members
-                    for (int i = 0; i < nm; ++i) {
-                        auto it = groups.lower_bound(std::make_tuple(sh[g0 + i], -1, -1));
-                        for (; it != groups.end() && std::get<0>(it->first) == sh[g0 + i]; ++it) {
-                            auto& dst = by_class[{std::get<1>(it->first), std::get<2>(it->first)}];
-                            for (const Rec& r : it->second) {
-                                auto& v = dst[r.b];
-                                if (v.empty()) v.assign(M, nullptr);
-                                v[i] = &r;
-                            }
-                        }
-                    }
-                    for (auto& bc : by_class) {
-                        struct Tmp { double Qmax; int b; const std::vector<const Rec*>* v; };
-                        std::vector<Tmp> tmp;
-                        for (auto& e : bc.second) {
-                            double qm = 0.0;
-                            for (const Rec* r : e.second) if (r) qm = std::max(qm, pairs[r->pair].Q);
-                            tmp.push_back({qm, e.first, &e.second});
-                        }
-                        std::sort(tmp.begin(), tmp.end(), [](const Tmp& x, const Tmp& y) { return x.Qmax != y.Qmax ? x.Qmax > y.Qmax : x.b < y.b; });
-                        SAList sl{};
-                        for (int i = 0; i < SUPER_MAX; ++i) sl.ao_a[i] = i < nm ? H.ao[sh[g0 + i]] : -1;
-                        sl.rec_begin = (int)S.heads.size();
-                        sl.Qmax = tmp[0].Qmax;
-                        sl.minpos = 1 << 30;
-                        sl.ketclass = -1;
-                        for (const Tmp& t : tmp) {
-                            S.heads.push_back(SHead{t.Qmax, H.ao[t.b], 0});
-                            for (int i = 0; i < M; ++i) {
-                                const Rec* r = (*t.v)[i];
-                                SMem m{0.0, 0, 0};
-                                if (r) {
-                                    const Pair& P = pairs[r->pair];
-                                    m.Q = P.Q; m.pos = P.pos;
-                                    m.flags = (r->canonical ? 1 : 0) | (r->a == r->b ? 2 : 0) | 4;
-                                    sl.minpos = std::min(sl.minpos, P.pos);
-                                    sl.ketclass = P.pc * NSUB + P.sub;
-                                }
-                                S.mems.push_back(m);
-                            }
-                        }
-                        sl.rec_end = (int)S.heads.size();
-                        S.lists.push_back(sl);
-                        S.la.push_back(sc.first.first);
-                        S.lb.push_back(bc.first.first);
-                    }
-                }
-            }
-            h->tabs.super[ms].M = M;
-            RT_TRY(upload(h, S.heads, &h->tabs.super[ms].heads));
-            RT_TRY(upload(h, S.mems, &h->tabs.super[ms].mems));
-            RT_TRY(upload(h, S.lists, &h->tabs.super[ms].lists));
-        }
-    }
     h->tabs.tau = tau;
     h->tabs.nao = h->nao;
 
@@ -538,24 +450,6 @@ int create_impl(Handle* h, const rttda_basis_t* basis, const double* C_occ, cons
                 L.seg = (int)h->segments.size();
                 L.nwork = (int)w.size();
                 RT_TRY(upload(h, w, &L.work));
-                for (int ms = 0; ms < 2; ++ms) {
-                    const SuperHost& S = superh[ms];
-                    std::vector<std::pair<double, WorkItem>> sitems;
-                    for (int ai = 0; ai < (int)S.lists.size(); ++ai) {
-                        if (S.la[ai] != la || S.lb[ai] != lb || S.lists[ai].ketclass != kcb) continue;
-                        const SAList& sl = S.lists[ai];
-                        const int nkmax = nkets_of(kck, sl.Qmax);
-                        const int q0 = same ? (sl.minpos / JK_BLOCK) * JK_BLOCK : 0;
-                        const double len = sl.rec_end - sl.rec_begin;
-                        for (int k0 = q0; k0 < nkmax; k0 += JK_BLOCK) sitems.push_back({len, WorkItem{ai, k0}});
-                    }
-                    std::stable_sort(sitems.begin(), sitems.end(), [](const auto& x, const auto& y) { return x.first > y.first; });
-                    std::vector<WorkItem> sw;
-                    sw.reserve(sitems.size());
-                    for (auto& it : sitems) sw.push_back(it.second);
-                    L.nswork[ms] = (int)sw.size();
-                    RT_TRY(upload(h, sw, &L.swork[ms]));
-                }
                 h->launches.push_back(L);
             }
             sg.nlaunch = (int)h->launches.size() - sg.first_launch;
