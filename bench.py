@@ -45,7 +45,7 @@ def parse():
     ap.add_argument("--ntraj", type=int, default=0, help="trajectories per call (0 = all of the config's fields)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=20.0, help="CPU budget of the cpu_baseline sample")
-    ap.add_argument("--sweep", action="store_true", help="also run the config-5 sigma sweep -> gpurun_out/sweep.json")
+    ap.add_argument("--sweep", action="store_true", help="run the config-5 sigma sweep (nvec x tau) instead of the step bench -> gpurun_out/sweep.json")
     return ap.parse_args()
 
 
@@ -318,6 +318,13 @@ def run_b200(args):
     jk_avg_ms = jk_ms / max(jk_n, 1)
     achieved = flops_pass / (jk_avg_ms * 1e-3) / 1e12
     peak = R.rttda_fp64_peak(1.0, st)
+    # DRAM bytes of one ERI pass from the committed ncu launch list of this same command (profiles/README.md)
+    traffic = None
+    tpath = os.path.join(ROOT, "profiles", "r1_traffic_per_pass.json")
+    if k == 4 and nvec == 6 and os.path.exists(tpath):
+        with open(tpath) as f:
+            tj = json.load(f)
+        traffic = tj["dram_read_bytes"] + tj["dram_write_bytes"]
     out = None
     if rank == 0:
         out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
@@ -341,7 +348,9 @@ def run_b200(args):
                "jk_ms_per_pass": jk_avg_ms, "jk_share_of_step": jk_ms / (sum(ms) if sum(ms) else 1.0),
                "roofline": {"bound": "alu", "kernel": "eval_kernel<*> + digest_kernel<*>/digest_v_kernel<*> (all launches of one ERI pass)",
                             "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
-                            "traffic": None, "peak_source": "measured live: rttda_fp64_peak DFMA chain, 1 s "
+                            "traffic": traffic, "traffic_source": "profiles/r1_traffic_per_pass.json (ncu dram__bytes_read+write "
+                            "summed over the launches of one ERI pass, config 4, nvec 6)" if traffic else None,
+                            "peak_source": "measured live: rttda_fp64_peak DFMA chain, 1 s "
                             "(MEASURED_PEAKS.json has no FP64 entry; nominal %.1f)" % FP64_NOMINAL_TFLOPS,
                             "flops_per_launch_group": flops_pass},
                "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
@@ -358,9 +367,65 @@ def run_b200(args):
         torch.distributed.destroy_process_group()
 
 
+# ------------------------------------------------------------------------------------------ config 5 sweep
+def run_sweep(args):
+    """BJ:configs[4]: batched sigma microbenchmark at the 1280-AO molecule, nvec x tau; 3 warm-ups + 10 timed
+    rttda_sigma calls per point (CUDA events on the call's stream), median and min.  The error column compares
+    against the GPU result at tau = 1e-14 (convergence under screening; oracle parity at full size is the sampled
+    test in tests/test_gpu_parity.py)."""
+    import torch
+    import paper_2601_16949_b200 as R
+    from workloads import make_vectors
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(0)
+    cfg, basis, C_o, C_v, eps, cond, bump = build_inputs(4, R.rttda_overlap)
+    st = torch.cuda.current_stream()
+    peak = R.rttda_fp64_peak(1.0, st)
+    Co, Cv = torch.from_numpy(C_o).to(dev), torch.from_numpy(C_v).to(dev)
+    points, ref = [], {}
+    for tau in (1e-14, 1e-12, 1e-10):
+        h = R.Rttda(basis, Co, Cv, eps, 1.0, tau, st)
+        info = h.info()
+        for nvec in (2, 8, 16, 32):
+            X = torch.from_numpy(make_vectors(cfg, nvec)).to(dev)
+            out = torch.empty_like(X)
+            for _ in range(3):
+                h.rttda_sigma(X, out, st)
+            torch.cuda.synchronize()
+            h.rttda_jk_time()
+            ms = []
+            for _ in range(10):
+                a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                a.record(st); h.rttda_sigma(X, out, st); b.record(st)
+                torch.cuda.synchronize()
+                ms.append(a.elapsed_time(b))
+            jk_ms, jk_n = h.rttda_jk_time()
+            jk = jk_ms / max(jk_n, 1)
+            res = out.cpu().numpy()
+            if tau == 1e-14:
+                ref[nvec] = res
+            err = float(np.max(np.abs(res - ref[nvec])) / np.max(np.abs(ref[nvec])))
+            flops = info["flops_eval"] + nvec * info["flops_digest_per_vec"]
+            points.append({"tau": tau, "nvec": nvec, "ms_median": float(np.median(ms)), "ms_min": float(min(ms)),
+                           "sigma_vectors_per_s": nvec / (float(np.median(ms)) * 1e-3),
+                           "eri_quartets_per_s": info["nquartets"] / (jk * 1e-3), "jk_ms": jk,
+                           "unique_shell_quartets": info["nquartets"], "primitive_quartets": info["nprim_quartets"],
+                           "fp64_roofline_frac": flops / (jk * 1e-3) / 1e12 / peak,
+                           "rel_inf_err_vs_tau1e-14": err})
+            print(json.dumps(points[-1]), file=sys.stderr)
+        h.close()
+    out = {"metric": "sigma_sweep_1280ao", "unit": UNIT, "fp64_peak_tflops": peak, "cond_S": cond, "points": points}
+    os.makedirs(os.path.join(ROOT, "gpurun_out"), exist_ok=True)
+    with open(os.path.join(ROOT, "gpurun_out", "sweep.json"), "w") as f:
+        json.dump(out, f, indent=1)
+    print(json.dumps(out))
+
+
 if __name__ == "__main__":
     a = parse()
-    if a.impl == "reference":
+    if a.sweep:
+        run_sweep(a)
+    elif a.impl == "reference":
         run_reference(a)
     else:
         run_b200(a)
