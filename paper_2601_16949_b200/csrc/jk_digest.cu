@@ -547,14 +547,9 @@ static int class_nv_max(int la, int lb, int lc, int ld)
     const int na = 2 * la + 1, nc = 2 * lc + 1, nd = 2 * ld + 1;
     (void)lb;
     const int per_v = 2 * na * (nc + nd) + 2 * nc * nd;
-    static int cap[3] = {0, 0, 0};
-    if (cap[0] == 0) {                 // tuning knobs (defaults measured on B200)
-        const char* e0 = getenv("RTTDA_NV_A"); const char* e1 = getenv("RTTDA_NV_B"); const char* e2 = getenv("RTTDA_NV_C");
-        cap[0] = e0 ? atoi(e0) : 6; cap[1] = e1 ? atoi(e1) : 4; cap[2] = e2 ? atoi(e2) : 2;
-    }
-    if (per_v <= 8) return cap[0];     // ss|ss, sp|ss
-    if (per_v <= 16) return cap[1];    // ps|ss, pp|ss, sp|ps
-    if (per_v <= 32) return cap[2];    // ps|ps, pp|ps
+    if (per_v <= 8) return 6;          // ss|ss, sp|ss
+    if (per_v <= 16) return 4;         // ps|ss, pp|ss, sp|ps
+    if (per_v <= 32) return 2;         // ps|ps, pp|ps
     return 1;                          // pp|pp
 }
 
@@ -600,9 +595,7 @@ static int launch_digest(Handle* h, const JKLaunch& L, const Segment& sg, const 
         // Coulomb part: thread-per-ket kernel in J-only mode over the canonical records (no density gathers, the
         // J_ab sums amortise one warp butterfly over 32 kets); launches of the flipped orientation (la < lb) hold
         // no canonical record.  Exchange part: block-per-batch kernel, lane = density, K only.
-        static int jsplit = -1;
-        if (jsplit < 0) { const char* e = getenv("RTTDA_DIGEST_JSPLIT"); jsplit = e ? atoi(e) : 1; }
-        if (jsplit && LA >= LB) {
+        if (LA >= LB) {
             constexpr int NVJ = (NC * ND <= 3) ? 8 : 4;
             int v0 = 0;
             while (v0 < nvec) {
@@ -617,7 +610,6 @@ static int launch_digest(Handle* h, const JKLaunch& L, const Segment& sg, const 
         constexpr size_t smem = (size_t)2 * NI * 256;
         static bool attr_set = false;
         if (!attr_set) {
-            RT_CUDA(cudaFuncSetAttribute(digest_b_kernel<LA, LB, LC, LD, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
             RT_CUDA(cudaFuncSetAttribute(digest_b_kernel<LA, LB, LC, LD, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
             attr_set = true;
         }
@@ -628,10 +620,7 @@ static int launch_digest(Handle* h, const JKLaunch& L, const Segment& sg, const 
             g.Tq = Tq; g.Fq = Fq; g.cx = h->cx;
             g.ketclass = L.ketclass; g.same = (sg.kc_bra == sg.kc_ket); g.nvt = nvt; g.v0 = v0;
             const int KW = 32 / G, nwarps = (32 + KW - 1) / KW;
-            if (jsplit)
-                digest_b_kernel<LA, LB, LC, LD, false><<<dim3(4 * L.nwork), dim3(32 * nwarps), smem, st>>>(g, G, KW);
-            else
-                digest_b_kernel<LA, LB, LC, LD, true><<<dim3(4 * L.nwork), dim3(32 * nwarps), smem, st>>>(g, G, KW);
+            digest_b_kernel<LA, LB, LC, LD, false><<<dim3(4 * L.nwork), dim3(32 * nwarps), smem, st>>>(g, G, KW);
             h->kernel_launches++;
             RT_CUDA(cudaGetLastError());
         }
