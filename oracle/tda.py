@@ -205,6 +205,56 @@ def rk4_matrix_free(ob, C_o, C_v, eps, cx, tau, Q, D_oo, D_vv, D_ov, D_00, y0, f
                          t_start, dt, nsteps)
 
 
+# ---------------------------------------------------------------- SSO propagator (NEXT-1; reading R22)
+def sso_propagate(apply_A_ext, apply_Md, y0, f, t_start, dt, nsteps, log=True):
+    """Second-order symplectic split-operator step on (q', p') = (H p, -H q) (eq. 14-15; "SSO").
+
+    The paper names the integrator and its cost (2 sigma builds per step, P:130) but prints no update formulas;
+    reading R22 takes the Stoermer-Verlet splitting with H evaluated at the time of each sub-step:
+        p_half  = p_n    - (dt/2) H(t_n)        q_n
+        q_{n+1} = q_n    +  dt    H(t_n + dt/2) p_half
+        p_{n+1} = p_half - (dt/2) H(t_{n+1})    q_{n+1}
+    H(t_{n+1}) q_{n+1} is reused as the first half-kick of the next step: two applications of H to a REAL vector
+    per step.  A 'delta' field is the linearised kick of R8 at t_start.  Returns (y, log) as rk4_propagate."""
+    y = np.array(y0, dtype=np.complex128)
+    if f.get("type") == "delta":
+        y = kick(y, f, apply_Md)
+    yref = y.copy()
+
+    def H(t, x):                                    # x real; A_ext and M_d are real operators
+        E = field_value(f, t)
+        h = apply_A_ext(x.astype(np.complex128)).real
+        if E != 0.0:
+            h = h + E * apply_Md(x.astype(np.complex128)).real
+        return h
+
+    q, p = y.real.copy(), y.imag.copy()
+    out = np.zeros((nsteps, 3))
+    hq = H(t_start, q)
+    for n in range(nsteps):
+        t = t_start + n * dt
+        p = p - 0.5 * dt * hq
+        q = q + dt * H(t + 0.5 * dt, p)
+        hq = H(t + dt, q)
+        p = p - 0.5 * dt * hq
+        if log:
+            yy = q + 1j * p
+            R = np.vdot(yref, yy)
+            out[n] = (np.vdot(yy, yy).real, R.real, R.imag)
+    return q + 1j * p, out
+
+
+def sso_dense(A, D_oo, D_vv, D_ov, D_00, y0, f, t_start, dt, nsteps):
+    """SSO with the dense singles block A (element 0 decoupled, A_00 = 0)."""
+    def apply_A_ext(z):
+        o = np.empty_like(z)
+        o[0] = 0.0
+        o[1:] = A @ z[1:]
+        return o
+    return sso_propagate(apply_A_ext, lambda z: apply_M(z, D_oo, D_vv, D_ov, D_00), y0, f,
+                         t_start, dt, nsteps)
+
+
 # ---------------------------------------------------------------- spectrum (harness for the pins)
 def spectrum(R, dt, pad=50000):
     """omega * F[R(t)] with mirroring R(-t) = R(t)^*, Hann window, zero padding (eq. 21).

@@ -225,6 +225,49 @@ def test_matrix_free_propagation_equals_dense(tiny):
     assert np.max(np.abs(yd - ym)) < 1e-14 and np.max(np.abs(ld - lm)) < 1e-14
 
 
+# ------------------------------------------------------------------------------------ SSO (NEXT-1, reading R22)
+def test_sso_field_free_eigenvector_is_the_leapfrog_map(tiny):
+    """For H u = w u one SSO step acts on the (q, p) coefficients of u as the 2x2 leapfrog matrix
+    [[1 - z^2/2, z], [-z (1 - z^2/4), 1 - z^2/2]], z = w dt, of determinant 1: n steps = its n-th power."""
+    A = tiny["A"]
+    w, U = np.linalg.eigh(A)
+    Doo, Dvv, Dov, D00 = tda.mo_dipoles(tiny["D"], tiny["C_o"], tiny["C_v"], (0, 0, 1.0))
+    dt, n = 0.1, 40
+    for I in (0, 5, len(w) - 1):
+        y0 = np.zeros(A.shape[0] + 1, dtype=complex); y0[1:] = (0.8 - 0.6j) * U[:, I]
+        y, log = tda.sso_dense(A, Doo, Dvv, Dov, D00, y0, {"type": "none"}, 0.0, dt, n)
+        z = w[I] * dt
+        M = np.array([[1 - z * z / 2, z], [-z * (1 - z * z / 4), 1 - z * z / 2]])
+        assert abs(np.linalg.det(M) - 1.0) < 1e-14
+        qn, pn = np.linalg.matrix_power(M, n) @ np.array([0.8, -0.6])
+        assert np.max(np.abs(y[1:] - (qn + 1j * pn) * U[:, I])) < 1e-12
+        assert abs(log[-1, 0] - (qn * qn + pn * pn)) < 1e-12
+
+
+def test_sso_second_order_stationary_ground_state_and_bounded_norm(tiny):
+    from scipy.linalg import expm
+    A = tiny["A"]
+    Doo, Dvv, Dov, D00 = tda.mo_dipoles(tiny["D"], tiny["C_o"], tiny["C_v"], (0, 0, 1.0))
+    y0 = np.zeros(A.shape[0] + 1, dtype=complex); y0[0] = 1.0
+    y, _ = tda.sso_dense(A, Doo, Dvv, Dov, D00, y0, {"type": "none"}, 0.0, 0.05, 10)
+    assert np.array_equal(y, y0)                                  # zero field: e_0 stays exactly
+    rng = np.random.default_rng(11)
+    y1 = rng.standard_normal(A.shape[0] + 1) + 1j * rng.standard_normal(A.shape[0] + 1)
+    y1 /= np.linalg.norm(y1)
+    ref = expm(-1j * tda.extend_A(A) * 1.0) @ y1
+    e1 = np.max(np.abs(tda.sso_dense(A, Doo, Dvv, Dov, D00, y1, {"type": "none"}, 0.0, 0.02, 50)[0] - ref))
+    e2 = np.max(np.abs(tda.sso_dense(A, Doo, Dvv, Dov, D00, y1, {"type": "none"}, 0.0, 0.01, 100)[0] - ref))
+    assert 3.5 < e1 / e2 < 4.5                                    # second order (P:285-289: slope 2)
+    _, log = tda.sso_dense(A, Doo, Dvv, Dov, D00, y1, {"type": "none"}, 0.0, 0.05, 400)
+    assert np.max(np.abs(log[:, 0] - 1.0)) < 0.02                 # symplectic: the norm error stays bounded
+    # driven: converges to the RK4 result of a much finer step, again with ratio 4
+    f = {"type": "cw", "E0": 0.05, "omega": 0.3}
+    fine, _ = tda.rk4_dense(A, Doo, Dvv, Dov, D00, y0, f, 0.0, 0.0125, 160)
+    d1 = np.max(np.abs(tda.sso_dense(A, Doo, Dvv, Dov, D00, y0, f, 0.0, 0.05, 40)[0] - fine))
+    d2 = np.max(np.abs(tda.sso_dense(A, Doo, Dvv, Dov, D00, y0, f, 0.0, 0.025, 80)[0] - fine))
+    assert 3.5 < d1 / d2 < 4.5
+
+
 # ------------------------------------------------------------------------------------ paper pins
 def test_paper_unit_conversions():
     pv = paper_values()
