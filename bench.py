@@ -45,6 +45,9 @@ def parse():
     ap.add_argument("--ntraj", type=int, default=0, help="trajectories per call (0 = all of the config's fields)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=20.0, help="CPU budget of the cpu_baseline sample")
+    ap.add_argument("--propagator", default="rk4", choices=["rk4", "sso"],
+                    help="rk4 (BASELINE.json configs; 8 sigma-vectors per trajectory and step) or the paper's SSO "
+                         "(NEXT-1; 2 per trajectory and step)")
     ap.add_argument("--sweep", action="store_true", help="run the config-5 sigma sweep (nvec x tau) instead of the step bench -> gpurun_out/sweep.json")
     return ap.parse_args()
 
@@ -59,9 +62,9 @@ def reduce_max(x: float, world: int, device) -> float:
     return float(t.item())
 
 
-def aggregate_value(ntraj: int, world: int, ms_per_step: float) -> float:
-    """Whole-job sigma-vectors/s: every replica builds 8*ntraj sigma-vectors per RK4 step."""
-    return 8.0 * ntraj * world / (ms_per_step * 1e-3)
+def aggregate_value(ntraj: int, world: int, ms_per_step: float, per_traj: float = 8.0) -> float:
+    """Whole-job sigma-vectors/s: every replica builds per_traj*ntraj sigma-vectors per step (RK4: 8, SSO: 2)."""
+    return per_traj * ntraj * world / (ms_per_step * 1e-3)
 
 
 def dist_env():
@@ -269,8 +272,14 @@ def run_b200(args):
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)     # > 126 MB L2
     dt = cfg.dt if cfg.dt > 0 else 0.1
 
+    sso = args.propagator == "sso"
+    per_traj = 2.0 if sso else 8.0
+    if sso:
+        nvec = ntraj                      # one real plane per sigma build
+    prop = h.rttda_propagate_sso if sso else h.rttda_propagate
+
     def step(i):
-        h.rttda_propagate(y, fields if i == 0 else cont, i * dt, dt, 1, log, st)
+        prop(y, fields if i == 0 else cont, i * dt, dt, 1, log, st)
 
     cont = [dict(f) if f["type"] != "delta" else {"type": "none"} for f in fields]
     for i in range(args.warmup):
@@ -296,7 +305,7 @@ def run_b200(args):
     launches = int(h.rttda_get_info("kernel_launches") - l0)
     total_ms = reduce_max(total_ms, world, dev)
     ms_per_step = total_ms / args.steps
-    value = aggregate_value(ntraj, world, ms_per_step)
+    value = aggregate_value(ntraj, world, ms_per_step, per_traj)
 
     # end to end: host buffers through rttda_propagate_host (H2D of the state, D2H of state + log inside)
     yh = torch.from_numpy(y0.copy()).pin_memory()
@@ -309,7 +318,7 @@ def run_b200(args):
     barrier()
     e2e_s = time.perf_counter() - e0
     e2e_s = reduce_max(e2e_s, world, dev)
-    e2e_val = aggregate_value(ntraj, world, e2e_s * 1e3 / args.steps)
+    e2e_val = aggregate_value(ntraj, world, e2e_s * 1e3 / args.steps, 8.0)
     h2d = yh.numel() * 8
     d2h = yh.numel() * 8 + lh.numel() * 8
 
@@ -336,6 +345,8 @@ def run_b200(args):
                                                                                ncsf, ntraj, nvec, cfg.tau, dt),
                           "l2": "256 MiB buffer written between timed steps (L2 flush)",
                           "parallelism": "replicas" if world > 1 else "1 GPU", "omega": omega,
+                          "propagator": args.propagator + (" (one call per step: H(t0) q is recomputed, 3 sigma builds "
+                                                           "of ntraj vectors per timed step)" if sso else ""),
                           "cond_S": cond, "seed_bump": bump},
                "rt_tda_steps_per_s": world * 1e3 / ms_per_step,
                "eri_quartets_per_s": info["nquartets"] / (jk_avg_ms * 1e-3),

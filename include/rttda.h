@@ -119,6 +119,14 @@ int rttda_fock(rttda_handle_t h, int32_t nvec, const double* T, double* F, void*
 int rttda_propagate(rttda_handle_t h, int32_t ntraj, double* C, const rttda_field_t* fields,
                     double t_start, double dt, int32_t nsteps, double* log, void* stream);
 
+/* The paper's own propagator (NEXT-1 of DESIGN.md): second-order symplectic split operator, P:126-130, 2 sigma
+ * builds per step.  The text names it without formulas; reading R22 = Stoermer-Verlet on (q', p') = (H p, -H q):
+ *   p_half = p_n - dt/2 H(t_n) q_n;  q_{n+1} = q_n + dt H(t_n + dt/2) p_half;  p_{n+1} = p_half - dt/2 H(t_{n+1}) q_{n+1},
+ * H(t_{n+1}) q_{n+1} being reused by the next step.  Arguments, layout, kick (R8), log and re-entrancy as
+ * rttda_propagate (a continued call recomputes H(t_start) q once). */
+int rttda_propagate_sso(rttda_handle_t h, int32_t ntraj, double* C, const rttda_field_t* fields,
+                        double t_start, double dt, int32_t nsteps, double* log, void* stream);
+
 /* Same with HOST buffers for C and log (copies inside, stream synchronised on return). */
 int rttda_propagate_host(rttda_handle_t h, int32_t ntraj, double* C, const rttda_field_t* fields,
                          double t_start, double dt, int32_t nsteps, double* log, void* stream);

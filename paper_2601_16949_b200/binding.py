@@ -19,7 +19,7 @@ INFO = dict(npairs_total=0, npairs_kept=1, nquartets=2, nprim_quartets=3, nquart
             create_ms=10, qmax=11, nvec_chunk=12, eri_buf_bytes=13)
 PULSE = dict(none=0, delta=1, cw=2, tl=3, chirp=4, sin2=5)
 EXPORTS = ["rttda_overlap", "rttda_dipole_ao", "rttda_create", "rttda_destroy", "rttda_sigma",
-           "rttda_sigma_host", "rttda_fock", "rttda_propagate", "rttda_propagate_host",
+           "rttda_sigma_host", "rttda_fock", "rttda_propagate", "rttda_propagate_sso", "rttda_propagate_host",
            "rttda_get_info", "rttda_last_timings", "rttda_jk_time", "rttda_fp64_peak", "rttda_last_error",
            "rttda_version"]
 
@@ -178,6 +178,12 @@ class Rttda:
         arr = self._fields(fields)
         _check(lib().rttda_propagate(self._h, len(fields), _dptr(C), arr, ct.c_double(t_start), ct.c_double(dt),
                                      int(nsteps), _dptr(log), _stream(stream)), "rttda_propagate")
+        return C
+
+    def rttda_propagate_sso(self, C, fields, t_start, dt, nsteps, log=None, stream=None):
+        arr = self._fields(fields)
+        _check(lib().rttda_propagate_sso(self._h, len(fields), _dptr(C), arr, ct.c_double(t_start), ct.c_double(dt),
+                                         int(nsteps), _dptr(log), _stream(stream)), "rttda_propagate_sso")
         return C
 
     def rttda_propagate_host(self, C: np.ndarray, fields, t_start, dt, nsteps, log=None, stream=None):

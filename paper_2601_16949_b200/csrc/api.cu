@@ -166,6 +166,18 @@ int rttda_propagate(rttda_handle_t hh, int32_t ntraj, double* C, const rttda_fie
     return propagate_impl(h, ntraj, C, fields, t_start, dt, nsteps, log, (cudaStream_t)stream);
 }
 
+int rttda_propagate_sso(rttda_handle_t hh, int32_t ntraj, double* C, const rttda_field_t* fields, double t_start,
+                        double dt, int32_t nsteps, double* log, void* stream)
+{
+    Handle* h = (Handle*)hh;
+    RT_CHECK(h && C && fields, "rttda_propagate_sso: NULL pointer");
+    RT_CHECK(ntraj >= 1 && ntraj <= 8, "rttda_propagate_sso: ntraj must be in 1..8");
+    RT_CHECK(nsteps >= 0, "rttda_propagate_sso: negative step count");
+    for (int t = 0; t < ntraj; ++t)
+        RT_CHECK(fields[t].type >= RTTDA_NONE && fields[t].type <= RTTDA_SIN2, "rttda_propagate_sso: bad pulse type");
+    return propagate_sso_impl(h, ntraj, C, fields, t_start, dt, nsteps, log, (cudaStream_t)stream);
+}
+
 int rttda_propagate_host(rttda_handle_t hh, int32_t ntraj, double* C, const rttda_field_t* fields,
                          double t_start, double dt, int32_t nsteps, double* log, void* stream)
 {

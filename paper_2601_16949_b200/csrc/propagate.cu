@@ -332,4 +332,88 @@ int propagate_impl(Handle* h, int ntraj, double* y, const rttda_field_t* fields,
     return RTTDA_OK;
 }
 
+// ---------------------------------------------------------------------------------------------- SSO
+// y[t][dst_plane][e] += c * hy[t][src_plane][e]
+__global__ void plane_axpy_kernel(long long n1, int ntraj, double c, const double* __restrict__ hy, int src_plane,
+                                  double* __restrict__ y, int dst_plane)
+{
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n1 * ntraj) return;
+    const long long t = i / n1, e = i % n1;
+    y[(2 * t + dst_plane) * n1 + e] = fma(c, hy[(2 * t + src_plane) * n1 + e], y[(2 * t + dst_plane) * n1 + e]);
+}
+
+// Second-order symplectic split-operator propagator (the paper's SSO; Stoermer-Verlet reading R22 of
+// DESIGN.md): p_half = p - dt/2 H(t_n) q; q += dt H(t_n + dt/2) p_half; p = p_half - dt/2 H(t_n + dt) q, with the
+// last H q reused by the next step: two applications of H to one REAL plane per step, i.e. two sigma builds of
+// ntraj vectors each (RK4: four builds of 2 ntraj).
+int propagate_sso_impl(Handle* h, int ntraj, double* y, const rttda_field_t* fields, double t_start, double dt,
+                       int nsteps, double* log, cudaStream_t st)
+{
+    const size_t no = h->nocc, nv = h->nvirt, ncsf = h->ncsf, n1 = ncsf + 1;
+    const size_t nstate = (size_t)ntraj * 2 * n1;
+    const size_t need = 4 * nstate + (size_t)ntraj * (no * no + nv * nv + no * nv);
+    RT_TRY(ensure_ws(h, &h->prop_ws, &h->prop_ws_n, need));
+    double* hy = h->prop_ws + nstate;              // same carving as propagate_impl
+    double* yref = h->prop_ws + 3 * nstate;
+    double* Dd_oo = yref + nstate;
+    double* Dd_vv = Dd_oo + (size_t)ntraj * no * no;
+    double* Dd_ov = Dd_vv + (size_t)ntraj * nv * nv;
+    FieldArgs fa{};
+    for (int t = 0; t < ntraj; ++t) {
+        const double* d = fields[t].dir;
+        fa.D00[t] = d[0] * h->D_00[0] + d[1] * h->D_00[1] + d[2] * h->D_00[2];
+        const long long a = no * no, b = nv * nv, c = no * nv;
+        combine3_kernel<<<(unsigned)((a + 255) / 256), 256, 0, st>>>(a, h->D_oo, d[0], d[1], d[2], Dd_oo + t * a);
+        combine3_kernel<<<(unsigned)((b + 255) / 256), 256, 0, st>>>(b, h->D_vv, d[0], d[1], d[2], Dd_vv + t * b);
+        combine3_kernel<<<(unsigned)((c + 255) / 256), 256, 0, st>>>(c, h->D_ov, d[0], d[1], d[2], Dd_ov + t * c);
+        h->kernel_launches += 3;
+    }
+    RT_CUDA(cudaGetLastError());
+    const unsigned eg = (unsigned)((n1 * ntraj + 255) / 256);
+    bool any_kick = false;
+    for (int t = 0; t < ntraj; ++t) {
+        fa.E[t] = fields[t].type == RTTDA_DELTA ? fields[t].E0 : 0.0;
+        any_kick |= fa.E[t] != 0.0;
+    }
+    if (any_kick) {
+        RT_CUDA(cudaMemsetAsync(hy, 0, nstate * sizeof(double), st));
+        RT_TRY(apply_field(h, ntraj, y, hy, Dd_oo, Dd_vv, Dd_ov, fa, st));
+        kick_kernel<<<eg, 256, 0, st>>>((long long)n1, ntraj, hy, y, fa);
+        RT_CUDA(cudaGetLastError());
+        h->kernel_launches++;
+    }
+    RT_CUDA(cudaMemcpyAsync(yref, y, nstate * sizeof(double), cudaMemcpyDeviceToDevice, st));
+
+    // hy[:, plane, :] = H(t) y[:, plane, :]; the other plane of hy is scratch of the field kernels
+    auto apply_H = [&](int plane, double t) -> int {
+        RT_CUDA(cudaMemsetAsync(hy, 0, nstate * sizeof(double), st));
+        RT_TRY(sigma_impl(h, ntraj, y + plane * n1 + 1, (long long)(2 * n1), hy + plane * n1 + 1, (long long)(2 * n1), st));
+        for (int k = 0; k < ntraj; ++k) fa.E[k] = field_value(fields[k], t);
+        RT_TRY(apply_field(h, ntraj, y, hy, Dd_oo, Dd_vv, Dd_ov, fa, st));
+        return RTTDA_OK;
+    };
+    auto axpy = [&](double c, int src_plane, int dst_plane) -> int {
+        plane_axpy_kernel<<<eg, 256, 0, st>>>((long long)n1, ntraj, c, hy, src_plane, y, dst_plane);
+        RT_CUDA(cudaGetLastError());
+        h->kernel_launches++;
+        return RTTDA_OK;
+    };
+    if (nsteps > 0) RT_TRY(apply_H(0, t_start));                         // H(t_0) q_0
+    for (int n = 0; n < nsteps; ++n) {
+        const double t0 = t_start + n * dt;
+        RT_TRY(axpy(-0.5 * dt, 0, 1));                                   // p_half = p - dt/2 H q
+        RT_TRY(apply_H(1, t0 + 0.5 * dt));
+        RT_TRY(axpy(dt, 1, 0));                                          // q += dt H p_half
+        RT_TRY(apply_H(0, t0 + dt));
+        RT_TRY(axpy(-0.5 * dt, 0, 1));                                   // p = p_half - dt/2 H q   (H q kept for the next step)
+        if (log) {
+            observe_kernel<<<ntraj, 1024, 0, st>>>((long long)n1, y, yref, log + (size_t)n * ntraj * 3);
+            RT_CUDA(cudaGetLastError());
+            h->kernel_launches++;
+        }
+    }
+    return RTTDA_OK;
+}
+
 }  // namespace rttda

@@ -277,3 +277,32 @@ def test_sigma_config4_vs_stored_oracle_samples():
     print("config-4 sigma error vs unscreened oracle:", errs)
     assert errs[1e-14] < SIGMA_TOL
     assert errs[1e-12] < 1e-8
+
+
+def test_propagate_sso_tiny_vs_oracle():
+    """The paper's SSO propagator (reading R22) against the oracle's, three pulse types in one batch, with a
+    continued second call; and its cost: two sigma builds of ntraj vectors per step."""
+    import torch
+    from oracle import tda
+    ctx = setup_config(1, dense=True)
+    h, n = ctx["h"], ctx["A"].shape[0]
+    D = ctx["ob"].dipole()
+    fields = [{"type": "delta", "E0": 1e-4, "dir": (1.0, 0.0, 0.0)},
+              {"type": "cw", "E0": 0.02, "omega": 0.4, "dir": (0.0, 1.0, 0.0)},
+              {"type": "sin2", "E0": 0.03, "omega": 0.5, "T_env": 1.5, "dir": (0.3, 0.1, 0.9)}]
+    dt, n1, n2 = 0.05, 15, 10
+    y = torch.from_numpy(_state0(3, n)).to(ctx["dev"])
+    log = torch.zeros((n1, 3, 3), dtype=torch.float64, device=ctx["dev"])
+    h.rttda_propagate_sso(y, fields, 0.0, dt, n1, log)
+    cont = [dict(f) for f in fields]
+    cont[0] = {"type": "none"}
+    h.rttda_propagate_sso(y, cont, n1 * dt, dt, n2, None)
+    torch.cuda.synchronize()
+    y, log = y.cpu().numpy(), log.cpu().numpy()
+    for t, f in enumerate(fields):
+        Doo, Dvv, Dov, D00 = tda.mo_dipoles(D, ctx["C_o"], ctx["C_v"], f["dir"])
+        y0 = np.zeros(n + 1, dtype=complex); y0[0] = 1.0
+        ya, la = tda.sso_dense(ctx["A"], Doo, Dvv, Dov, D00, y0, f, 0.0, dt, n1)
+        assert np.max(np.abs(log[:, t, :] - la)) < 1e-12
+        yb, _ = tda.sso_dense(ctx["A"], Doo, Dvv, Dov, D00, ya, cont[t], n1 * dt, dt, n2)
+        assert np.max(np.abs(y[t, 0] - yb.real)) < 1e-12 and np.max(np.abs(y[t, 1] - yb.imag)) < 1e-12
