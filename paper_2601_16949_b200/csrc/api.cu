@@ -94,7 +94,7 @@ int rttda_destroy(rttda_handle_t hh)
     if (!h) return RTTDA_OK;
     cudaDeviceSynchronize();
     for (void* p : h->dev_allocs) cudaFree(p);
-    for (double* p : {h->wsY, h->wsT, h->wsF, h->wsZ, h->prop_ws, h->eri_buf[0], h->eri_buf[1]}) if (p) cudaFree(p);
+    for (double* p : {h->wsY, h->wsT, h->wsF, h->wsZ, h->wsP, h->prop_ws, h->eri_buf[0], h->eri_buf[1]}) if (p) cudaFree(p);
     if (h->st_eval) cudaStreamDestroy(h->st_eval);
     for (cudaEvent_t e : {h->ev_fork, h->ev_E[0], h->ev_E[1], h->ev_D[0], h->ev_D[1]}) if (e) cudaEventDestroy(e);
     for (auto& e : h->ev) if (e) cudaEventDestroy(e);

@@ -157,8 +157,8 @@ struct Handle {
     cudaEvent_t ev_fork = nullptr, ev_E[2] = {nullptr, nullptr}, ev_D[2] = {nullptr, nullptr};
     std::vector<void*> dev_allocs;             // everything to free
     // workspaces (grown on demand)
-    double *wsY = nullptr, *wsT = nullptr, *wsF = nullptr, *wsZ = nullptr;
-    size_t wsY_n = 0, wsT_n = 0, wsF_n = 0, wsZ_n = 0;
+    double *wsY = nullptr, *wsT = nullptr, *wsF = nullptr, *wsZ = nullptr, *wsP = nullptr;
+    size_t wsY_n = 0, wsT_n = 0, wsF_n = 0, wsZ_n = 0, wsP_n = 0;
     double* prop_ws = nullptr;
     size_t prop_ws_n = 0;
     // info

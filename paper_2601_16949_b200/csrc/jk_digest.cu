@@ -84,6 +84,7 @@ struct DigestArgs {
     const long long* batch_base;
     const double* buf;
     const double* Tq;
+    const double* PPq;      // symmetric / antisymmetric density pairs {T + T^T, T - T^T}, [mu][nu][v][2] (K-only kernel)
     double* Fq;
     double cx;
     int ketclass, same, nvt, v0;
@@ -360,6 +361,7 @@ template <int LA, int LB, int LC, int LD, bool DO_J>
 __global__ void __launch_bounds__(256)
 digest_b_kernel(DigestArgs g, int G, int KW)
 {
+    static_assert(!DO_J, "the block-per-batch kernel reads the {Ps, Pa} density pairs: exchange part only");
     constexpr int NA = 2 * LA + 1, NB = 2 * LB + 1, NC = 2 * LC + 1, ND = 2 * LD + 1;
     constexpr int NI = NA * NB * NC * ND;
     const JKTables& tb = g.tb;
@@ -383,6 +385,9 @@ digest_b_kernel(DigestArgs g, int G, int KW)
     const double cx = g.cx;
 #define TQ(mu, nu) (Tv + (size_t)(mu) * rs + (size_t)(nu) * nvt)
 #define FQ(mu, nu) (Fv + (size_t)(mu) * rs + (size_t)(nu) * nvt)
+    // {Ps, Pa}(mu, nu)[v]: one 16-byte load gives T_mn + T_nm and T_mn - T_nm, i.e. both T_mn and T_nm
+    const double2* PPv = reinterpret_cast<const double2*>(g.PPq) + g.v0 + v;
+#define PQ(mu, nu) (PPv + (size_t)(mu) * rs + (size_t)(nu) * nvt)
     __shared__ BraRec s_rec[REC_TILE];
     __shared__ long long s_bb[REC_TILE];
     __shared__ __align__(8) uint64_t s_bar[2];
@@ -458,16 +463,17 @@ digest_b_kernel(DigestArgs g, int G, int KW)
             if (__any_sync(0xffffffffu, ok)) {
 #pragma unroll
                 for (int b = 0; b < NB; ++b) {
+                    // tbd = Ps_bd, tdb = Pa_bd (and likewise for c): K_ac = (U + V)/2, K_ca = (U - V)/2 at the flush
                     double tbd[ND], tdb[ND], tbc[NC], tcb[NC];
 #pragma unroll
                     for (int d2 = 0; d2 < ND; ++d2) {
-                        tbd[d2] = ok ? __ldg(TQ(aoB + b, aoD + d2)) : 0.0;
-                        tdb[d2] = ok ? __ldg(TQ(aoD + d2, aoB + b)) : 0.0;
+                        const double2 pp = ok ? __ldg(PQ(aoB + b, aoD + d2)) : make_double2(0.0, 0.0);
+                        tbd[d2] = pp.x; tdb[d2] = pp.y;
                     }
 #pragma unroll
                     for (int c = 0; c < NC; ++c) {
-                        tbc[c] = ok ? __ldg(TQ(aoB + b, aoC + c)) : 0.0;
-                        tcb[c] = ok ? __ldg(TQ(aoC + c, aoB + b)) : 0.0;
+                        const double2 pp = ok ? __ldg(PQ(aoB + b, aoC + c)) : make_double2(0.0, 0.0);
+                        tbc[c] = pp.x; tcb[c] = pp.y;
                     }
 #pragma unroll
                     for (int a = 0; a < NA; ++a) {
@@ -516,13 +522,13 @@ digest_b_kernel(DigestArgs g, int G, int KW)
         for (int a = 0; a < NA; ++a) {
 #pragma unroll
             for (int c = 0; c < NC; ++c) {
-                atomicAdd(FQ(aoA + a, aoC + c), -cx * Kac[a][c]);
-                atomicAdd(FQ(aoC + c, aoA + a), -cx * Kca[c][a]);
+                atomicAdd(FQ(aoA + a, aoC + c), -0.5 * cx * (Kac[a][c] + Kca[c][a]));
+                atomicAdd(FQ(aoC + c, aoA + a), -0.5 * cx * (Kac[a][c] - Kca[c][a]));
             }
 #pragma unroll
             for (int d2 = 0; d2 < ND; ++d2) {
-                atomicAdd(FQ(aoA + a, aoD + d2), -cx * Kad[a][d2]);
-                atomicAdd(FQ(aoD + d2, aoA + a), -cx * Kda[d2][a]);
+                atomicAdd(FQ(aoA + a, aoD + d2), -0.5 * cx * (Kad[a][d2] + Kda[d2][a]));
+                atomicAdd(FQ(aoD + d2, aoA + a), -0.5 * cx * (Kad[a][d2] - Kda[d2][a]));
             }
         }
         if (DO_J) {
@@ -537,6 +543,7 @@ digest_b_kernel(DigestArgs g, int G, int KW)
     }
 #undef TQ
 #undef FQ
+#undef PQ
 }
 
 // ---------------------------------------------------------------------------------------------------
@@ -562,7 +569,7 @@ static int launch_digest_nv(Handle* h, const JKLaunch& L, const Segment& sg, con
     g.work = L.work;
     g.batch_base = sg.batch_base;
     g.buf = buf;
-    g.Tq = Tq; g.Fq = Fq; g.cx = h->cx;
+    g.Tq = Tq; g.PPq = nullptr; g.Fq = Fq; g.cx = h->cx;
     g.ketclass = L.ketclass; g.same = (sg.kc_bra == sg.kc_ket); g.nvt = nvt; g.v0 = v0;
     constexpr int NI = (2 * LA + 1) * (2 * LB + 1) * (2 * LC + 1) * (2 * LD + 1);
     constexpr size_t smem = digest_ring_bytes(NI);
@@ -617,7 +624,7 @@ static int launch_digest(Handle* h, const JKLaunch& L, const Segment& sg, const 
             const int G = nvec - v0 < 8 ? nvec - v0 : 8;
             DigestArgs g;
             g.tb = h->tabs; g.work = L.work; g.batch_base = sg.batch_base; g.buf = buf;
-            g.Tq = Tq; g.Fq = Fq; g.cx = h->cx;
+            g.Tq = Tq; g.PPq = h->wsP; g.Fq = Fq; g.cx = h->cx;
             g.ketclass = L.ketclass; g.same = (sg.kc_bra == sg.kc_ket); g.nvt = nvt; g.v0 = v0;
             const int KW = 32 / G, nwarps = (32 + KW - 1) / KW;
             digest_b_kernel<LA, LB, LC, LD, false><<<dim3(4 * L.nwork), dim3(32 * nwarps), smem, st>>>(g, G, KW);
@@ -667,6 +674,19 @@ int digest_launch(Handle* h, const JKLaunch& L, const Segment& sg, const double*
     }
 }
 
+// PP[mu][nu][v] = {T[mu][nu][v] + T[nu][mu][v], T[mu][nu][v] - T[nu][mu][v]}  (step a2 of DESIGN.md)
+__global__ void symsplit_kernel(int nao, int nvt, const double* __restrict__ T, double2* __restrict__ PP)
+{
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const long long n = (long long)nao * nao * nvt;
+    if (i >= n) return;
+    const int v = (int)(i % nvt);
+    const long long e = i / nvt;
+    const int mu = (int)(e / nao), nu = (int)(e % nao);
+    const double a = T[i], b = T[((long long)nu * nao + mu) * nvt + v];
+    PP[i] = make_double2(a + b, a - b);
+}
+
 // One ERI pass: for every segment, evaluate its quartets once into a staging buffer (stream st_eval), then digest
 // them for all densities (caller's stream).  Two buffers: the FP64-bound evaluation of segment k+1 overlaps the
 // L1/L2-bound digestion of segment k.  Fq must be zeroed by the caller; densities [0, nvec) of the nvt slots per
@@ -675,6 +695,13 @@ int jk_build(Handle* h, int nvt, int nvec, const double* Tq, double* Fq, cudaStr
 {
     RT_CHECK(nvec >= 2 && nvec % 2 == 0 && nvt >= nvec && nvt % 2 == 0, "jk_build: bad density slot counts");
     for (int b = 0; b < 2; ++b) RT_TRY(ensure_ws(h, &h->eri_buf[b], &h->eri_buf_n[b], h->eri_buf_need));
+    if (nvec >= 4) {                    // the K-only kernel gathers {Ps, Pa} pairs: one 16-byte load per (T_mn, T_nm)
+        const long long n = (long long)h->nao * h->nao * nvt;
+        RT_TRY(ensure_ws(h, &h->wsP, &h->wsP_n, (size_t)2 * n));
+        symsplit_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(h->nao, nvt, Tq, reinterpret_cast<double2*>(h->wsP));
+        RT_CUDA(cudaGetLastError());
+        h->kernel_launches++;
+    }
     RT_CUDA(cudaEventRecord(h->ev_fork, st));
     RT_CUDA(cudaStreamWaitEvent(h->st_eval, h->ev_fork, 0));
     int k = 0;
