@@ -12,9 +12,11 @@
 //   Both orientations (a,b), (b,a) of a bra pair are separate records reading the SAME stored block, which
 //   keeps every exchange update in registers: no per-quartet global atomics, and no second evaluation.
 // Densities and results use the interleaved layout Tq[mu][nu][v] (v fastest), F likewise.
-// Two kernels share that decomposition: digest_kernel (thread = ket, NV densities in registers; calls with < 4
-// densities and the ps|ss, pp|ss classes) and digest_b_kernel (block = one 32-ket batch, a group of lanes per ket,
-// lane = density; the other classes).  Both are bound by the density gathers through L1/L2.
+// Two kernels share that decomposition: digest_kernel (thread = ket, NV densities in registers): J and K for calls
+// with < 4 densities, and the Coulomb part alone (MODE 1: canonical records, no density gathers) otherwise;
+// digest_b_kernel (block = one 32-ket batch, a group of lanes per ket, lane = density): the exchange part for
+// calls with >= 4 densities, gathering {T + T^T, T - T^T} pairs (symsplit_kernel) so that one 16-byte load yields
+// both T_mn and T_nm.  DESIGN.md section 5 has the rooflines, profiles/ the ncu evidence.
 #include <cstdlib>
 #include "common.cuh"
 #include "tma.cuh"
@@ -355,13 +357,13 @@ digest_kernel(DigestArgs g)
 // KW = 32 / G kets of the batch, a group of G lanes per ket, lane v of the group serves density v.  The batch's
 // integrals of each record (NI x 256 contiguous bytes) are fetched ONCE by a TMA bulk copy into a two-stage shared
 // memory ring shared by all warps (the copy of record r+1 flies while record r is digested); every density access
-// is a contiguous 8*G-byte run of an aligned slot; a lane carries one density's accumulators only, so all
-// densities of the call are served by one read of the staged integrals.
-template <int LA, int LB, int LC, int LD, bool DO_J>
+// is a contiguous 16*G-byte run of an aligned slot of {Ps, Pa} pairs; a lane carries one density's accumulators
+// only, so all densities of a chunk are served by one read of the staged integrals.  Exchange part only: with
+//   U_ac = sum I Ps_bd, V_ac = sum I Pa_bd (Ps = T + T^T, Pa = T - T^T):  K_ac = (U + V)/2,  K_ca = (U - V)/2.
+template <int LA, int LB, int LC, int LD>
 __global__ void __launch_bounds__(256)
 digest_b_kernel(DigestArgs g, int G, int KW)
 {
-    static_assert(!DO_J, "the block-per-batch kernel reads the {Ps, Pa} density pairs: exchange part only");
     constexpr int NA = 2 * LA + 1, NB = 2 * LB + 1, NC = 2 * LC + 1, ND = 2 * LD + 1;
     constexpr int NI = NA * NB * NC * ND;
     const JKTables& tb = g.tb;
@@ -402,14 +404,8 @@ digest_b_kernel(DigestArgs g, int G, int KW)
     const int aoC = __ldg(kc.ao_c + qq), aoD = __ldg(kc.ao_d + qq);
     const bool cd_same = __ldg(kc.same + qq) != 0;
 
-    double Scd[NC][ND], Jcd[NC][ND], Kac[NA][NC], Kca[NC][NA], Kad[NA][ND], Kda[ND][NA];
-#pragma unroll
-    for (int c = 0; c < NC; ++c)
-#pragma unroll
-        for (int d2 = 0; d2 < ND; ++d2) {
-            Scd[c][d2] = (DO_J && active) ? __ldg(TQ(aoC + c, aoD + d2)) + __ldg(TQ(aoD + d2, aoC + c)) : 0.0;
-            Jcd[c][d2] = 0.0;
-        }
+    // Kac/Kad accumulate against Ps (symmetric part), Kca/Kda against Pa (antisymmetric part) of the density
+    double Kac[NA][NC], Kca[NC][NA], Kad[NA][ND], Kda[ND][NA];
 #pragma unroll
     for (int a = 0; a < NA; ++a) {
 #pragma unroll
@@ -454,11 +450,9 @@ digest_b_kernel(DigestArgs g, int G, int KW)
             const double* src = s_dyn + (size_t)stage * (NI * 32) + (kb & 31);
             const bool ok = active && (br.Q * Qq >= tb.tau) && (!same_class || br.pos <= q);
             const bool canonical = (br.flags & 1) != 0;
-            const bool ab_same = (br.flags & 2) != 0;
             const int aoB = br.ao_b;
             const double wsame = (same_class && br.pos == q) ? 0.5 : 1.0;
             const double wk = ok ? wsame * (cd_same ? 0.5 : 1.0) : 0.0;
-            const double fix = (cd_same ? 2.0 : 1.0) * (ab_same ? 0.5 : 1.0);
             const bool flip = (LA < LB) || (LA == LB && !canonical);
             if (__any_sync(0xffffffffu, ok)) {
 #pragma unroll
@@ -477,9 +471,6 @@ digest_b_kernel(DigestArgs g, int G, int KW)
                     }
 #pragma unroll
                     for (int a = 0; a < NA; ++a) {
-                        double sab = 0.0, jab = 0.0;
-                        if (DO_J && canonical && kg < KW)
-                            sab = fix * (__ldg(TQ(aoA + a, aoB + b)) + __ldg(TQ(aoB + b, aoA + a)));
                         const int i_ab = flip ? (a * NB + b) : (b * NA + a);
 #pragma unroll
                         for (int d2 = 0; d2 < ND; ++d2)
@@ -491,25 +482,7 @@ digest_b_kernel(DigestArgs g, int G, int KW)
                                 Kca[c][a] = fma(x, tdb[d2], Kca[c][a]);
                                 Kad[a][d2] = fma(x, tbc[c], Kad[a][d2]);
                                 Kda[d2][a] = fma(x, tcb[c], Kda[d2][a]);
-                                if (DO_J) {
-                                    Jcd[c][d2] = fma(x, sab, Jcd[c][d2]);
-                                    jab = fma(x, Scd[c][d2], jab);
-                                }
                             }
-                        if (DO_J && canonical) {
-                            // sum J_ab over the KW kets of the warp (tree over the ket-group index), group 0 writes
-                            int n = KW;
-                            while (n > 1) {
-                                const int s = (n + 1) >> 1;
-                                const double y = __shfl_down_sync(0xffffffffu, jab, s * G);
-                                if (kg + s < n) jab += y;
-                                n = s;
-                            }
-                            if (kg == 0 && jab != 0.0) {
-                                atomicAdd(FQ(aoA + a, aoB + b), 2.0 * jab);
-                                if (!ab_same) atomicAdd(FQ(aoB + b, aoA + a), 2.0 * jab);
-                            }
-                        }
                     }
                 }
             }
@@ -530,15 +503,6 @@ digest_b_kernel(DigestArgs g, int G, int KW)
                 atomicAdd(FQ(aoA + a, aoD + d2), -0.5 * cx * (Kad[a][d2] + Kda[d2][a]));
                 atomicAdd(FQ(aoD + d2, aoA + a), -0.5 * cx * (Kad[a][d2] - Kda[d2][a]));
             }
-        }
-        if (DO_J) {
-#pragma unroll
-            for (int c = 0; c < NC; ++c)
-#pragma unroll
-                for (int d2 = 0; d2 < ND; ++d2) {
-                    atomicAdd(FQ(aoC + c, aoD + d2), 2.0 * Jcd[c][d2]);
-                    if (!cd_same) atomicAdd(FQ(aoD + d2, aoC + c), 2.0 * Jcd[c][d2]);
-                }
         }
     }
 #undef TQ
@@ -617,7 +581,7 @@ static int launch_digest(Handle* h, const JKLaunch& L, const Segment& sg, const 
         constexpr size_t smem = (size_t)2 * NI * 256;
         static bool attr_set = false;
         if (!attr_set) {
-            RT_CUDA(cudaFuncSetAttribute(digest_b_kernel<LA, LB, LC, LD, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+            RT_CUDA(cudaFuncSetAttribute(digest_b_kernel<LA, LB, LC, LD>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
             attr_set = true;
         }
         for (int v0 = 0; v0 < nvec; v0 += 8) {
@@ -627,7 +591,7 @@ static int launch_digest(Handle* h, const JKLaunch& L, const Segment& sg, const 
             g.Tq = Tq; g.PPq = h->wsP; g.Fq = Fq; g.cx = h->cx;
             g.ketclass = L.ketclass; g.same = (sg.kc_bra == sg.kc_ket); g.nvt = nvt; g.v0 = v0;
             const int KW = 32 / G, nwarps = (32 + KW - 1) / KW;
-            digest_b_kernel<LA, LB, LC, LD, false><<<dim3(4 * L.nwork), dim3(32 * nwarps), smem, st>>>(g, G, KW);
+            digest_b_kernel<LA, LB, LC, LD><<<dim3(4 * L.nwork), dim3(32 * nwarps), smem, st>>>(g, G, KW);
             h->kernel_launches++;
             RT_CUDA(cudaGetLastError());
         }
