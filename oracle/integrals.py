@@ -106,8 +106,8 @@ class OracleBasis:
 
     def eri_tensor(self) -> np.ndarray:
         N = self.nao
-        if N > 64:
-            raise ValueError("full N^4 tensor only for tiny systems")
+        if N > 256:                       # memory guard only: 256^4 doubles = 34 GB (config 2 needs 200^4 = 12.8 GB)
+            raise ValueError("full N^4 tensor only for small systems (N <= 256)")
         eri = np.zeros((N, N, N, N))
         lib().oracle_eri_tensor(*self._args(), ct.c_int(N), eri.ctypes.data_as(_dp))
         return eri

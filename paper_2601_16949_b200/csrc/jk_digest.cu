@@ -426,6 +426,20 @@ digest_b_kernel(DigestArgs g, int G, int KW)
             tma_load_1d(s_dyn + (size_t)s * (NI * 32), gsrc, NI * 256, &s_bar[s]);
         }
     };
+    auto lane_ok = [&](int ir) {
+        const BraRec& b1 = s_rec[ir];
+        return active && (b1.Q * Qq >= tb.tau) && (!same_class || b1.pos <= q);
+    };
+    auto gather = [&](int ir, bool okx, double2 (&bd)[NB][ND], double2 (&bc)[NB][NC]) {
+        const int aoBx = s_rec[ir].ao_b;
+#pragma unroll
+        for (int b = 0; b < NB; ++b) {
+#pragma unroll
+            for (int d2 = 0; d2 < ND; ++d2) bd[b][d2] = okx ? __ldg(PQ(aoBx + b, aoD + d2)) : make_double2(0.0, 0.0);
+#pragma unroll
+            for (int c = 0; c < NC; ++c) bc[b][c] = okx ? __ldg(PQ(aoBx + b, aoC + c)) : make_double2(0.0, 0.0);
+        }
+    };
     uint32_t phase0 = 0, phase1 = 0;
     int stage = 0;
     bool done = false;                                    // block-uniform
@@ -440,6 +454,11 @@ digest_b_kernel(DigestArgs g, int G, int KW)
         __syncthreads();
         if (!reaches(0)) { done = true; break; }
         issue(0, stage);
+        // the density pairs of a record are gathered right after the previous record's arithmetic, i.e. before the
+        // block barrier and the TMA wait of their own record: the L2 latency of the gathers overlaps both
+        bool ok_cur = lane_ok(0);
+        double2 cur_bd[NB][ND], cur_bc[NB][NC];
+        gather(0, ok_cur, cur_bd, cur_bc);
         for (int ir = 0; ir < nrec; ++ir) {
             const BraRec br = s_rec[ir];
             const bool more = (ir + 1 < nrec) && reaches(ir + 1);
@@ -448,9 +467,8 @@ digest_b_kernel(DigestArgs g, int G, int KW)
             if (stage == 0) { mbar_wait(&s_bar[0], phase0); phase0 ^= 1; }
             else { mbar_wait(&s_bar[1], phase1); phase1 ^= 1; }
             const double* src = s_dyn + (size_t)stage * (NI * 32) + (kb & 31);
-            const bool ok = active && (br.Q * Qq >= tb.tau) && (!same_class || br.pos <= q);
+            const bool ok = ok_cur;
             const bool canonical = (br.flags & 1) != 0;
-            const int aoB = br.ao_b;
             const double wsame = (same_class && br.pos == q) ? 0.5 : 1.0;
             const double wk = ok ? wsame * (cd_same ? 0.5 : 1.0) : 0.0;
             const bool flip = (LA < LB) || (LA == LB && !canonical);
@@ -460,15 +478,9 @@ digest_b_kernel(DigestArgs g, int G, int KW)
                     // tbd = Ps_bd, tdb = Pa_bd (and likewise for c): K_ac = (U + V)/2, K_ca = (U - V)/2 at the flush
                     double tbd[ND], tdb[ND], tbc[NC], tcb[NC];
 #pragma unroll
-                    for (int d2 = 0; d2 < ND; ++d2) {
-                        const double2 pp = ok ? __ldg(PQ(aoB + b, aoD + d2)) : make_double2(0.0, 0.0);
-                        tbd[d2] = pp.x; tdb[d2] = pp.y;
-                    }
+                    for (int d2 = 0; d2 < ND; ++d2) { tbd[d2] = cur_bd[b][d2].x; tdb[d2] = cur_bd[b][d2].y; }
 #pragma unroll
-                    for (int c = 0; c < NC; ++c) {
-                        const double2 pp = ok ? __ldg(PQ(aoB + b, aoC + c)) : make_double2(0.0, 0.0);
-                        tbc[c] = pp.x; tcb[c] = pp.y;
-                    }
+                    for (int c = 0; c < NC; ++c) { tbc[c] = cur_bc[b][c].x; tcb[c] = cur_bc[b][c].y; }
 #pragma unroll
                     for (int a = 0; a < NA; ++a) {
                         const int i_ab = flip ? (a * NB + b) : (b * NA + a);
@@ -488,6 +500,8 @@ digest_b_kernel(DigestArgs g, int G, int KW)
             }
             stage ^= 1;
             if (!more) { if (ir + 1 < nrec) done = true; break; }
+            ok_cur = lane_ok(ir + 1);
+            gather(ir + 1, ok_cur, cur_bd, cur_bc);
         }
     }
     if (active) {
