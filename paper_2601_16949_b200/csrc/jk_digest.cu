@@ -12,12 +12,11 @@
 //   Both orientations (a,b), (b,a) of a bra pair are separate records reading the SAME stored block, which
 //   keeps every exchange update in registers: no per-quartet global atomics, and no second evaluation.
 // Densities and results use the interleaved layout Tq[mu][nu][v] (v fastest), F likewise.
-// Two kernels share that decomposition: digest_kernel (thread = ket, NV densities in registers): J and K for calls
-// with < 4 densities, and the Coulomb part alone (MODE 1: canonical records, no density gathers) otherwise;
-// digest_b_kernel (block = one 32-ket batch, a group of lanes per ket, lane = density): the exchange part for
-// calls with >= 4 densities, gathering {T + T^T, T - T^T} pairs (symsplit_kernel) so that one 16-byte load yields
-// both T_mn and T_nm.  DESIGN.md section 5 has the rooflines, profiles/ the ncu evidence.
-#include <cstdlib>
+// Two kernels share that decomposition: digest_j_kernel (thread = ket, NV densities in registers) does the Coulomb
+// part over the canonical records without any per-lane density gather; digest_b_kernel (block = one 32-ket batch,
+// a group of lanes per ket, lane = density) does the exchange part, gathering {T + T^T, T - T^T} pairs
+// (symsplit_kernel) so that one 16-byte load yields both T_mn and T_nm.  DESIGN.md section 5 has the rooflines,
+// profiles/ the ncu evidence.
 #include "common.cuh"
 #include "tma.cuh"
 
@@ -113,12 +112,12 @@ struct VecLoad {
 // Stored component order (jk_eval.cu): canonical pair orientation (first shell = higher l), eri_index of
 // eri_eval.cuh: ((d * NC + c) * N2 + c2) * N1 + c1 with (c1, c2) the components of the canonical first/second
 // shell.
-// MODE 0: J and K; 1: J only (walks the canonical records of the a-list, no density gathers); 2: K only.
-template <int LA, int LB, int LC, int LD, int NV, int MODE>
+// Coulomb part: J_cd += I (T_ab + T_ba) in registers over the canonical records of the a-list, J_ab += I (T_cd + T_dc)
+// by one transposing warp butterfly per record; no per-lane density gathers at all.
+template <int LA, int LB, int LC, int LD, int NV>
 __global__ void __launch_bounds__(JK_BLOCK)
-digest_kernel(DigestArgs g)
+digest_j_kernel(DigestArgs g)
 {
-    constexpr bool DO_J = MODE != 2, DO_K = MODE != 1;
     constexpr int NA = 2 * LA + 1, NB = 2 * LB + 1, NC = 2 * LC + 1, ND = 2 * LD + 1;
     constexpr int NI = NA * NB * NC * ND;
     constexpr bool USE_TMA = digest_uses_tma(NI);
@@ -155,21 +154,13 @@ digest_kernel(DigestArgs g)
             for (int v = 0; v < NV; ++v) Scd[c][d][v] = x[v] + y[v];
         }
 
-    double Kac[NA][NC][NV], Kad[NA][ND][NV], Kca[NC][NA][NV], Kda[ND][NA][NV], Jcd[NC][ND][NV];
+    double Jcd[NC][ND][NV];
 #pragma unroll
-    for (int v = 0; v < NV; ++v) {
-#pragma unroll
-        for (int a = 0; a < NA; ++a) {
-#pragma unroll
-            for (int c = 0; c < NC; ++c) Kac[a][c][v] = Kca[c][a][v] = 0.0;
-#pragma unroll
-            for (int d = 0; d < ND; ++d) Kad[a][d][v] = Kda[d][a][v] = 0.0;
-        }
+    for (int v = 0; v < NV; ++v)
 #pragma unroll
         for (int c = 0; c < NC; ++c)
 #pragma unroll
             for (int d = 0; d < ND; ++d) Jcd[c][d][v] = 0.0;
-    }
 
     // The a-list's records and their staging-buffer offsets go through shared memory, REC_TILE at a time.  Each
     // warp streams its 32-ket batch of every record (NI x 256 contiguous bytes) from HBM into a two-stage shared
@@ -199,8 +190,8 @@ digest_kernel(DigestArgs g)
         return active && (b1.Q * Qq >= tb.tau) && (!same_class || b1.pos <= q);
     };
     bool done = false;                                      // warp-uniform
-    const BraRec* recs = MODE == 1 ? tb.jrecs : tb.recs;
-    const int rec_begin = MODE == 1 ? al.jrec_begin : al.rec_begin, rec_end = MODE == 1 ? al.jrec_end : al.rec_end;
+    const BraRec* recs = tb.jrecs;                          // the canonical records of the a-list
+    const int rec_begin = al.jrec_begin, rec_end = al.jrec_end;
     for (int r0 = rec_begin; r0 < rec_end; r0 += REC_TILE) {
       const int nrec = min(REC_TILE, rec_end - r0);
       __syncthreads();
@@ -225,7 +216,6 @@ digest_kernel(DigestArgs g)
             more = __any_sync(0xffffffffu, ok_next);
             if (more) issue(ir + 1, stage ^ 1);
         }
-        const bool canonical = (br.flags & 1) != 0;
         const bool ab_same = (br.flags & 2) != 0;
         const int aoB = br.ao_b;
         const double* src;
@@ -241,49 +231,23 @@ digest_kernel(DigestArgs g)
         const double wk = ok ? wsame * (cd_same ? 0.5 : 1.0) : 0.0;
         // J_cd needs wsame * w_ab instead of wk
         const double fix = (cd_same ? 2.0 : 1.0) * (ab_same ? 0.5 : 1.0);
-        // stored block is (first, second | c d) of the canonical orientation
-        const bool flip = (LA < LB) || (LA == LB && !canonical);
-
+        // canonical records: a is the pair's first shell, the stored block is (a b|c d), a fastest
 #pragma unroll
         for (int b = 0; b < NB; ++b) {
-            double tbd[ND][NV], tdb[ND][NV], tbc[NC][NV], tcb[NC][NV];
-            if (DO_K && ok) {
-#pragma unroll
-                for (int d = 0; d < ND; ++d) {
-                    VecLoad<NV>::ld(TQ(aoB + b, aoD + d), tbd[d]);
-                    VecLoad<NV>::ld(TQ(aoD + d, aoB + b), tdb[d]);
-                }
-#pragma unroll
-                for (int c = 0; c < NC; ++c) {
-                    VecLoad<NV>::ld(TQ(aoB + b, aoC + c), tbc[c]);
-                    VecLoad<NV>::ld(TQ(aoC + c, aoB + b), tcb[c]);
-                }
-            } else {
-#pragma unroll
-                for (int v = 0; v < NV; ++v) {
-#pragma unroll
-                    for (int d = 0; d < ND; ++d) tbd[d][v] = tdb[d][v] = 0.0;
-#pragma unroll
-                    for (int c = 0; c < NC; ++c) tbc[c][v] = tcb[c][v] = 0.0;
-                }
-            }
 #pragma unroll
             for (int a = 0; a < NA; ++a) {
                 double sab[NV], jab[next_pow2(NV)];
-                if (DO_J && canonical) {
+                {
                     double x[NV], y[NV];
                     VecLoad<NV>::ld(TQ(aoA + a, aoB + b), x);
                     VecLoad<NV>::ld(TQ(aoB + b, aoA + a), y);
 #pragma unroll
                     for (int v = 0; v < NV; ++v) sab[v] = fix * (x[v] + y[v]);
-                } else {
-#pragma unroll
-                    for (int v = 0; v < NV; ++v) sab[v] = 0.0;
                 }
 #pragma unroll
                 for (int v = 0; v < next_pow2(NV); ++v) jab[v] = 0.0;
                 // stored index of (a, b, c, d): first-shell component runs fastest
-                const int i_ab = flip ? (a * NB + b) : (b * NA + a);   // = c2 * N1 + c1
+                const int i_ab = b * NA + a;
 #pragma unroll
                 for (int d = 0; d < ND; ++d)
 #pragma unroll
@@ -292,20 +256,12 @@ digest_kernel(DigestArgs g)
                         const double x = ok ? wk * (USE_TMA ? src[i * 32] : __ldcs(src + i * 32)) : 0.0;
 #pragma unroll
                         for (int v = 0; v < NV; ++v) {
-                            if (DO_K) {
-                                Kac[a][c][v] = fma(x, tbd[d][v], Kac[a][c][v]);
-                                Kca[c][a][v] = fma(x, tdb[d][v], Kca[c][a][v]);
-                                Kad[a][d][v] = fma(x, tbc[c][v], Kad[a][d][v]);
-                                Kda[d][a][v] = fma(x, tcb[c][v], Kda[d][a][v]);
-                            }
-                            if (DO_J) {
-                                Jcd[c][d][v] = fma(x, sab[v], Jcd[c][d][v]);
-                                jab[v] = fma(x, Scd[c][d][v], jab[v]);
-                            }
+                            Jcd[c][d][v] = fma(x, sab[v], Jcd[c][d][v]);
+                            jab[v] = fma(x, Scd[c][d][v], jab[v]);
                         }
                     }
-                // ---- Coulomb J_ab: only the canonical orientation of the bra pair does it (uniform branch)
-                if (DO_J && canonical) {
+                // ---- J_ab: warp total of the kets' contributions
+                {
                     constexpr int NP = next_pow2(NV);
                     const double tot = warp_reduce_multi<NP>(jab, lane);
                     const int v = warp_reduce_owner_index<NP>(lane);
@@ -324,32 +280,14 @@ digest_kernel(DigestArgs g)
     }
 #undef TQ
     if (!active) return;
-    // ---- flush the register accumulators: F += 2 J - cx K
-    const double cx = g.cx;
-    if (DO_K) {
+    // ---- flush the register accumulators: F += 2 J_cd
 #pragma unroll
-        for (int a = 0; a < NA; ++a) {
+    for (int c = 0; c < NC; ++c)
 #pragma unroll
-            for (int c = 0; c < NC; ++c) {
-                red_add<NV>(Fv + (size_t)(aoA + a) * rs + (size_t)(aoC + c) * nvt, Kac[a][c], -cx);
-                red_add<NV>(Fv + (size_t)(aoC + c) * rs + (size_t)(aoA + a) * nvt, Kca[c][a], -cx);
-            }
-#pragma unroll
-            for (int d = 0; d < ND; ++d) {
-                red_add<NV>(Fv + (size_t)(aoA + a) * rs + (size_t)(aoD + d) * nvt, Kad[a][d], -cx);
-                red_add<NV>(Fv + (size_t)(aoD + d) * rs + (size_t)(aoA + a) * nvt, Kda[d][a], -cx);
-            }
+        for (int d = 0; d < ND; ++d) {
+            red_add<NV>(Fv + (size_t)(aoC + c) * rs + (size_t)(aoD + d) * nvt, Jcd[c][d], 2.0);
+            if (!cd_same) red_add<NV>(Fv + (size_t)(aoD + d) * rs + (size_t)(aoC + c) * nvt, Jcd[c][d], 2.0);
         }
-    }
-    if (DO_J) {
-#pragma unroll
-        for (int c = 0; c < NC; ++c)
-#pragma unroll
-            for (int d = 0; d < ND; ++d) {
-                red_add<NV>(Fv + (size_t)(aoC + c) * rs + (size_t)(aoD + d) * nvt, Jcd[c][d], 2.0);
-                if (!cd_same) red_add<NV>(Fv + (size_t)(aoD + d) * rs + (size_t)(aoC + c) * nvt, Jcd[c][d], 2.0);
-            }
-    }
 }
 
 // ---------------------------------------------------------------------------------------------------
@@ -525,21 +463,8 @@ digest_b_kernel(DigestArgs g, int G, int KW)
 }
 
 // ---------------------------------------------------------------------------------------------------
-// Densities per digestion launch: as many as the register file holds for the class (accumulators per density:
-// 2 NA (NC + ND) + 2 NC ND doubles).  More launches only re-read the staged integrals.
-static int class_nv_max(int la, int lb, int lc, int ld)
-{
-    const int na = 2 * la + 1, nc = 2 * lc + 1, nd = 2 * ld + 1;
-    (void)lb;
-    const int per_v = 2 * na * (nc + nd) + 2 * nc * nd;
-    if (per_v <= 8) return 6;          // ss|ss, sp|ss
-    if (per_v <= 16) return 4;         // ps|ss, pp|ss, sp|ps
-    if (per_v <= 32) return 2;         // ps|ps, pp|ps
-    return 1;                          // pp|pp
-}
-
-template <int LA, int LB, int LC, int LD, int NV, int MODE = 0>
-static int launch_digest_nv(Handle* h, const JKLaunch& L, const Segment& sg, const double* buf, int nvt, int v0,
+template <int LA, int LB, int LC, int LD, int NV>
+static int launch_digest_j(Handle* h, const JKLaunch& L, const Segment& sg, const double* buf, int nvt, int v0,
                             const double* Tq, double* Fq, cudaStream_t st)
 {
     DigestArgs g;
@@ -553,83 +478,52 @@ static int launch_digest_nv(Handle* h, const JKLaunch& L, const Segment& sg, con
     constexpr size_t smem = digest_ring_bytes(NI);
     static bool attr_set = false;
     if (!attr_set && smem > 0) {
-        RT_CUDA(cudaFuncSetAttribute(digest_kernel<LA, LB, LC, LD, NV, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        RT_CUDA(cudaFuncSetAttribute(digest_j_kernel<LA, LB, LC, LD, NV>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         attr_set = true;
     }
-    digest_kernel<LA, LB, LC, LD, NV, MODE><<<dim3(L.nwork), dim3(JK_BLOCK), smem, st>>>(g);
+    digest_j_kernel<LA, LB, LC, LD, NV><<<dim3(L.nwork), dim3(JK_BLOCK), smem, st>>>(g);
     h->kernel_launches++;
     RT_CUDA(cudaGetLastError());
     return RTTDA_OK;
 }
 
+// One digestion launch group (ordered bra class x ket class) for the nvec (even) densities of the call:
+//   Coulomb part  - digest_j_kernel over the canonical records, NVJ densities in registers per launch; launches of the
+//                   flipped orientation (la < lb) hold no canonical record;
+//   exchange part - digest_b_kernel, groups of G <= 8 lanes per ket (at most 8 warps per block), chunks of 8 densities.
 template <int LA, int LB, int LC, int LD>
 static int launch_digest(Handle* h, const JKLaunch& L, const Segment& sg, const double* buf, int nvt, int nvec,
                          const double* Tq, double* Fq, cudaStream_t st)
 {
-    constexpr int NA = 2 * LA + 1, NC = 2 * LC + 1, ND = 2 * LD + 1;
-    constexpr int PER_V = 2 * NA * (NC + ND) + 2 * NC * ND;
-    const int vmode = 4;
-    // which ordered classes use the block-per-batch kernel when the call has >= 4 densities (bit: ssss, spss, psss,
-    // spps, psps, ppss, ppps, pppp); default = all (with the Coulomb part split off it measured faster for every
-    // class on B200, profiles/).  RTTDA_DIGEST_BMASK overrides it (tuning only).
-    static int vmask = -1;
-    if (vmask < 0) { const char* e = getenv("RTTDA_DIGEST_BMASK"); vmask = e ? atoi(e) : 255; }
-    constexpr int KEY = LA * 8 + LB * 4 + LC * 2 + LD;
-    constexpr int CLS = KEY == 0 ? 0 : KEY == 4 ? 1 : KEY == 8 ? 2 : KEY == 6 ? 3 : KEY == 10 ? 4 : KEY == 12 ? 5 : KEY == 14 ? 6 : 7;
-    if (vmode > 0 && nvec >= vmode && ((vmask >> CLS) & 1)) {
-        // Coulomb part: thread-per-ket kernel in J-only mode over the canonical records (no density gathers, the
-        // J_ab sums amortise one warp butterfly over 32 kets); launches of the flipped orientation (la < lb) hold
-        // no canonical record.  Exchange part: block-per-batch kernel, lane = density, K only.
-        if (LA >= LB) {
-            constexpr int NVJ = (NC * ND <= 3) ? 8 : 4;
-            int v0 = 0;
-            while (v0 < nvec) {
-                const int left = nvec - v0;
-                if (left >= NVJ) { RT_TRY((launch_digest_nv<LA, LB, LC, LD, NVJ, 1>(h, L, sg, buf, nvt, v0, Tq, Fq, st))); v0 += NVJ; }
-                else if (NVJ == 8 && left >= 6) { RT_TRY((launch_digest_nv<LA, LB, LC, LD, 6, 1>(h, L, sg, buf, nvt, v0, Tq, Fq, st))); v0 += 6; }
-                else if (left >= 4) { RT_TRY((launch_digest_nv<LA, LB, LC, LD, 4, 1>(h, L, sg, buf, nvt, v0, Tq, Fq, st))); v0 += 4; }
-                else { RT_TRY((launch_digest_nv<LA, LB, LC, LD, 2, 1>(h, L, sg, buf, nvt, v0, Tq, Fq, st))); v0 += 2; }
-            }
+    constexpr int NC = 2 * LC + 1, ND = 2 * LD + 1;
+    if (LA >= LB) {
+        constexpr int NVJ = (NC * ND <= 3) ? 8 : 4;
+        int v0 = 0;
+        while (v0 < nvec) {
+            const int left = nvec - v0;
+            if (left >= NVJ) { RT_TRY((launch_digest_j<LA, LB, LC, LD, NVJ>(h, L, sg, buf, nvt, v0, Tq, Fq, st))); v0 += NVJ; }
+            else if (NVJ == 8 && left >= 6) { RT_TRY((launch_digest_j<LA, LB, LC, LD, 6>(h, L, sg, buf, nvt, v0, Tq, Fq, st))); v0 += 6; }
+            else if (left >= 4) { RT_TRY((launch_digest_j<LA, LB, LC, LD, 4>(h, L, sg, buf, nvt, v0, Tq, Fq, st))); v0 += 4; }
+            else { RT_TRY((launch_digest_j<LA, LB, LC, LD, 2>(h, L, sg, buf, nvt, v0, Tq, Fq, st))); v0 += 2; }
         }
-        constexpr int NI = (2 * LA + 1) * (2 * LB + 1) * (2 * LC + 1) * (2 * LD + 1);
-        constexpr size_t smem = (size_t)2 * NI * 256;
-        static bool attr_set = false;
-        if (!attr_set) {
-            RT_CUDA(cudaFuncSetAttribute(digest_b_kernel<LA, LB, LC, LD>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-            attr_set = true;
-        }
-        for (int v0 = 0; v0 < nvec; v0 += 8) {
-            const int G = nvec - v0 < 8 ? nvec - v0 : 8;
-            DigestArgs g;
-            g.tb = h->tabs; g.work = L.work; g.batch_base = sg.batch_base; g.buf = buf;
-            g.Tq = Tq; g.PPq = h->wsP; g.Fq = Fq; g.cx = h->cx;
-            g.ketclass = L.ketclass; g.same = (sg.kc_bra == sg.kc_ket); g.nvt = nvt; g.v0 = v0;
-            const int KW = 32 / G, nwarps = (32 + KW - 1) / KW;
-            digest_b_kernel<LA, LB, LC, LD><<<dim3(4 * L.nwork), dim3(32 * nwarps), smem, st>>>(g, G, KW);
-            h->kernel_launches++;
-            RT_CUDA(cudaGetLastError());
-        }
-        return RTTDA_OK;
     }
-    const int nvmax = class_nv_max(LA, LB, LC, LD);
-    int v0 = 0;
-    while (v0 < nvec) {                 // nvec is even; slots [nvec, nvt) are alignment padding, never touched
-        const int left = nvec - v0;
-        int nv = left < nvmax ? left : nvmax;
-        if (nv == 7) nv = 6;
-        if (nv == 5 || nv == 3) nv -= 1;
-        if constexpr (PER_V <= 8) {
-            if (nv == 8) { RT_TRY((launch_digest_nv<LA, LB, LC, LD, 8>(h, L, sg, buf, nvt, v0, Tq, Fq, st))); v0 += 8; continue; }
-        }
-        if constexpr (PER_V <= 16) {
-            if (nv >= 6) { RT_TRY((launch_digest_nv<LA, LB, LC, LD, 6>(h, L, sg, buf, nvt, v0, Tq, Fq, st))); v0 += 6; continue; }
-            if (nv >= 4) { RT_TRY((launch_digest_nv<LA, LB, LC, LD, 4>(h, L, sg, buf, nvt, v0, Tq, Fq, st))); v0 += 4; continue; }
-        }
-        if constexpr (PER_V <= 32) {
-            if (nv >= 2) { RT_TRY((launch_digest_nv<LA, LB, LC, LD, 2>(h, L, sg, buf, nvt, v0, Tq, Fq, st))); v0 += 2; continue; }
-        }
-        RT_TRY((launch_digest_nv<LA, LB, LC, LD, 1>(h, L, sg, buf, nvt, v0, Tq, Fq, st)));
-        v0 += 1;
+    constexpr int NI = (2 * LA + 1) * (2 * LB + 1) * (2 * LC + 1) * (2 * LD + 1);
+    constexpr size_t smem = (size_t)2 * NI * 256;
+    static bool attr_set = false;
+    if (!attr_set) {
+        RT_CUDA(cudaFuncSetAttribute(digest_b_kernel<LA, LB, LC, LD>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        attr_set = true;
+    }
+    for (int v0 = 0; v0 < nvec; v0 += 8) {
+        const int G = nvec - v0 < 8 ? nvec - v0 : 8;
+        DigestArgs g;
+        g.tb = h->tabs; g.work = L.work; g.batch_base = sg.batch_base; g.buf = buf;
+        g.Tq = Tq; g.PPq = h->wsP; g.Fq = Fq; g.cx = h->cx;
+        g.ketclass = L.ketclass; g.same = (sg.kc_bra == sg.kc_ket); g.nvt = nvt; g.v0 = v0;
+        const int KW = 32 / G, nwarps = (32 + KW - 1) / KW;
+        digest_b_kernel<LA, LB, LC, LD><<<dim3(4 * L.nwork), dim3(32 * nwarps), smem, st>>>(g, G, KW);
+        h->kernel_launches++;
+        RT_CUDA(cudaGetLastError());
     }
     return RTTDA_OK;
 }
@@ -673,7 +567,7 @@ int jk_build(Handle* h, int nvt, int nvec, const double* Tq, double* Fq, cudaStr
 {
     RT_CHECK(nvec >= 2 && nvec % 2 == 0 && nvt >= nvec && nvt % 2 == 0, "jk_build: bad density slot counts");
     for (int b = 0; b < 2; ++b) RT_TRY(ensure_ws(h, &h->eri_buf[b], &h->eri_buf_n[b], h->eri_buf_need));
-    if (nvec >= 4) {                    // the K-only kernel gathers {Ps, Pa} pairs: one 16-byte load per (T_mn, T_nm)
+    {                                   // the exchange kernel gathers {Ps, Pa} pairs: one 16-byte load per (T_mn, T_nm)
         const long long n = (long long)h->nao * h->nao * nvt;
         RT_TRY(ensure_ws(h, &h->wsP, &h->wsP_n, (size_t)2 * n));
         symsplit_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(h->nao, nvt, Tq, reinterpret_cast<double2*>(h->wsP));
