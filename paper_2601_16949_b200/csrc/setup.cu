@@ -374,13 +374,20 @@ int create_impl(Handle* h, const rttda_basis_t* basis, const double* C_occ, cons
 
     // ---- segments (bra pair class x ket pair class, unique quartets), their staging-buffer maps and the
     //      evaluation / digestion work lists
-    auto count_ge = [&](int kc, double thr) {       // pairs of class kc with Q >= thr (Q sorted descending)
+    // pairs q of class kc (Q sorted descending) with Q_q * Qother >= tau: the SAME product test the kernels apply
+    // per lane, so that the staging map and the kernels agree on which batches exist down to the last bit
+    auto count_prod_ge = [&](int kc, double Qother) {
         const std::vector<double>& q = hQ[kc];
         const int n = h->tabs.kets[kc].n;
-        return (int)(std::upper_bound(q.begin(), q.begin() + n, thr, [](double t, double x) { return t > x; }) - q.begin());
+        int lo = 0, hi = n;                         // first index whose product falls below tau
+        while (lo < hi) {
+            const int mid = (lo + hi) / 2;
+            if (q[mid] * Qother >= tau) lo = mid + 1; else hi = mid;
+        }
+        return lo;
     };
     auto nkets_of = [&](int kc_ket, double Qp) {    // kets q (a prefix of the list) with Qp Q_q >= tau
-        return tau > 0.0 ? count_ge(kc_ket, tau / Qp) : h->tabs.kets[kc_ket].n;
+        return tau > 0.0 ? count_prod_ge(kc_ket, Qp) : h->tabs.kets[kc_ket].n;
     };
     double n_eval = 0, nprim_eval = 0;
     size_t buf_need = 1;
@@ -421,7 +428,7 @@ int create_impl(Handle* h, const rttda_basis_t* basis, const double* C_occ, cons
             const int G = std::min(JK_BLOCK, EVAL_MAX_ROWS / npb);
             std::vector<EvalItem> items;
             for (int k0 = 0; k0 < nk; k0 += JK_BLOCK) {
-                int hi = tau > 0.0 ? count_ge(kcb, tau / hQ[kck][k0]) : nb;   // bra pairs reaching this chunk
+                int hi = tau > 0.0 ? count_prod_ge(kcb, hQ[kck][k0]) : nb;     // bra pairs reaching this chunk
                 if (same) hi = std::min(hi, std::min(nb, k0 + JK_BLOCK));
                 for (int p0 = 0; p0 < hi; p0 += G) items.push_back(EvalItem{k0, p0, std::min(hi, p0 + G)});
             }
@@ -465,7 +472,7 @@ int create_impl(Handle* h, const rttda_basis_t* basis, const double* C_occ, cons
                 const Pair& P = pairs[k];
                 const int l1 = P.pc >= 1, l2 = P.pc == 2;
                 for (int kc2 = 0; kc2 < NKETCLASS; ++kc2) {
-                    const int n2 = tau > 0.0 ? count_ge(kc2, tau / P.Q) : h->tabs.kets[kc2].n;
+                    const int n2 = tau > 0.0 ? count_prod_ge(kc2, P.Q) : h->tabs.kets[kc2].n;
                     const int pc2 = kc2 / NSUB, l3 = pc2 >= 1, l4 = pc2 == 2;
                     const double npq = (double)P.np * h->tabs.kets[kc2].np;
                     ordered += n2;
