@@ -62,21 +62,28 @@ static int load_basis(const rttda_basis_t* b, HostBasis& H)
         H.l.push_back(sh.l); H.np.push_back(sh.nprim); H.off.push_back((int)H.ex.size());
         H.center.push_back(sh.center); H.ao.push_back(ao);
         ao += 2 * sh.l + 1;
+        // Primitives are taken in order of ascending exponent: the contraction sums do not depend on the order, but
+        // with every shell sorted the same way a primitive-pair index means "diffuse x diffuse" ... "tight x tight"
+        // for all kets of a warp alike, which makes the near-field / far-field Boys branch of the evaluation kernels
+        // (eri_eval.cuh) far more uniform across the lanes.
+        std::vector<int> order(sh.nprim);
+        std::iota(order.begin(), order.end(), 0);
+        std::sort(order.begin(), order.end(), [&](int x, int y) { return b->exps[sh.prim_off + x] < b->exps[sh.prim_off + y]; });
         // coefficient on the normalised primitive -> coefficient on the bare primitive
         std::vector<double> c(sh.nprim);
         for (int k = 0; k < sh.nprim; ++k) {
-            const double a = b->exps[sh.prim_off + k];
+            const double a = b->exps[sh.prim_off + order[k]];
             RT_CHECK(a > 0.0, "basis: non-positive exponent");
             double nrm = std::pow(2.0 * a / M_PI, 0.75);
             if (sh.l == 1) nrm *= 2.0 * std::sqrt(a);
-            c[k] = b->coefs[sh.prim_off + k] * nrm;
+            c[k] = b->coefs[sh.prim_off + order[k]] * nrm;
             H.ex.push_back(a);
         }
         // self overlap of the contracted function: s: sum c c (pi/p)^1.5 ; p: sum c c (pi/p)^1.5 / (2p)
         double self = 0.0;
         for (int k = 0; k < sh.nprim; ++k)
             for (int m = 0; m < sh.nprim; ++m) {
-                const double p = b->exps[sh.prim_off + k] + b->exps[sh.prim_off + m];
+                const double p = H.ex[H.off.back() + k] + H.ex[H.off.back() + m];   // sorted order, as c[]
                 double t = c[k] * c[m] * std::pow(M_PI / p, 1.5);
                 if (sh.l == 1) t /= 2.0 * p;
                 self += t;
