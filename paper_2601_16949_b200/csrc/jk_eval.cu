@@ -104,16 +104,21 @@ __global__ void __launch_bounds__(JK_BLOCK) eval_kernel(EvalArgs g)
 #pragma unroll
         for (int i = 0; i < NI; ++i) I[i] = 0.0;
         const double* rows = s_rows + (size_t)ip * npb * PRIM_STRIDE;
+        if (KET_IN_REGS) {
 #pragma unroll 1
-        for (int kb = 0; kb < npb; ++kb) {
-            const PrimPair bp = load_bra_prim_smem(rows + kb * PRIM_STRIDE);
-            if (KET_IN_REGS) {
+            for (int kb = 0; kb < npb; ++kb) {
+                const PrimPair bp = load_bra_prim_smem(rows + kb * PRIM_STRIDE);
 #pragma unroll
                 for (int kk = 0; kk < KP; ++kk) eri_prim_accum<LA, LB, LC, LD>(bp, kp[kk], s_boys, I);
-            } else {
+            }
+        } else {
+            // ket primitive outermost: it is loaded once (coalesced, L1) and meets every bra primitive (shared memory)
 #pragma unroll 1
-                for (int kk = 0; kk < KP; ++kk) {
-                    const PrimPair k1 = load_ket_prim<LC, LD>(g.ket.prim, g.ket.n, kk, qq);
+            for (int kk = 0; kk < KP; ++kk) {
+                const PrimPair k1 = load_ket_prim<LC, LD>(g.ket.prim, g.ket.n, kk, qq);
+#pragma unroll 1
+                for (int kb = 0; kb < npb; ++kb) {
+                    const PrimPair bp = load_bra_prim_smem(rows + kb * PRIM_STRIDE);
                     eri_prim_accum<LA, LB, LC, LD>(bp, k1, s_boys, I);
                 }
             }
