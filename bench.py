@@ -322,6 +322,29 @@ def run_b200(args):
     h2d = yh.numel() * 8
     d2h = yh.numel() * 8 + lh.numel() * 8
 
+    # optional in-core mode (NOT the headline: the evaluation is skipped after the first pass; include/rttda.h)
+    incore = None
+    if world == 1 and not sso:
+        try:
+            h.rttda_set_option(R.OPT_INCORE, 1)
+            yi = torch.from_numpy(y0).to(dev)
+            h.rttda_propagate(yi, fields, 0.0, dt, 1, log, st)                   # fills the store
+            torch.cuda.synchronize()
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(st)
+            for i in range(args.steps):
+                h.rttda_propagate(yi, cont, (i + 1) * dt, dt, 1, log, st)
+            b.record(st)
+            torch.cuda.synchronize()
+            ms_i = a.elapsed_time(b) / args.steps
+            incore = {"sigma_vectors_per_s": 8.0 * ntraj / (ms_i * 1e-3), "ms_per_step": ms_i,
+                      "store_bytes": info["eri_all_bytes"],
+                      "note": "RTTDA_OPT_INCORE: integrals resident in HBM, evaluation skipped after the first pass; "
+                              "not the paper's direct method and not the headline value"}
+        except R.RttdaError as e:
+            incore = {"unavailable": str(e)}
+        finally:
+            h.rttda_set_option(R.OPT_INCORE, 0)
     # roofline of the dominant kernel group (the J/K ERI pass): algorithmic flops / measured device time
     flops_pass = info["flops_eval"] + nvec * info["flops_digest_per_vec"]
     jk_avg_ms = jk_ms / max(jk_n, 1)
@@ -365,7 +388,7 @@ def run_b200(args):
                             "(MEASURED_PEAKS.json has no FP64 entry; nominal %.1f)" % FP64_NOMINAL_TFLOPS,
                             "flops_per_launch_group": flops_pass},
                "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
-               "gpu_launches": launches, "clocks": clocks}
+               "incore_mode": incore, "gpu_launches": launches, "clocks": clocks}
     h.close()
     if rank == 0:
         if not args.no_cpu_baseline and world == 1:

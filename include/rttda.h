@@ -146,7 +146,17 @@ int rttda_propagate_host(rttda_handle_t h, int32_t ntraj, double* C, const rttda
 #define RTTDA_INFO_QMAX             11   /* largest Schwarz bound */
 #define RTTDA_INFO_NVEC_CHUNK       12   /* 0: every ERI pass serves all densities of the call */
 #define RTTDA_INFO_ERI_BUF_BYTES    13   /* HBM staging buffer between ERI evaluation and J/K digestion */
+#define RTTDA_INFO_ERI_ALL_BYTES    14   /* bytes of ALL contracted integrals of one pass (the in-core store) */
 int rttda_get_info(rttda_handle_t h, int32_t key, double* out);
+
+/* Options.  RTTDA_OPT_INCORE (value != 0 switches it on; default off): keep the contracted integrals of all
+ * segments resident in HBM (RTTDA_INFO_ERI_ALL_BYTES: 61 GB for the 1280-AO molecule at tau = 1e-12) so that, after
+ * the first ERI pass of the handle, later passes skip the evaluation and only digest.  This is NOT the paper's direct
+ * method (P:130 re-evaluates every integral in every sigma build; that is the default and what bench.py reports as
+ * `value`); it is offered because 180 GB of HBM3e can hold what the paper's GPUs could not.  RTTDA_ENOMEM if the
+ * store does not fit: the handle then stays in direct mode. */
+#define RTTDA_OPT_INCORE 1
+int rttda_set_option(rttda_handle_t h, int32_t option, double value);
 
 /* Time the last rttda_sigma/rttda_fock call spent in the J/K kernels, from CUDA events recorded on its
  * stream (synchronises those events).  ms_out[0] = J/K build, [1] = MO->AO GEMMs, [2] = AO->MO GEMMs. */

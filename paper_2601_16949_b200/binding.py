@@ -16,11 +16,12 @@ _lib = None
 
 INFO = dict(npairs_total=0, npairs_kept=1, nquartets=2, nprim_quartets=3, nquartets_eval=4,
             nprim_eval=5, flops_eval=6, flops_digest_per_vec=7, jk_launches=8, kernel_launches=9,
-            create_ms=10, qmax=11, nvec_chunk=12, eri_buf_bytes=13)
+            create_ms=10, qmax=11, nvec_chunk=12, eri_buf_bytes=13, eri_all_bytes=14)
+OPT_INCORE = 1
 PULSE = dict(none=0, delta=1, cw=2, tl=3, chirp=4, sin2=5)
 EXPORTS = ["rttda_overlap", "rttda_dipole_ao", "rttda_create", "rttda_destroy", "rttda_sigma",
            "rttda_sigma_host", "rttda_fock", "rttda_propagate", "rttda_propagate_sso", "rttda_propagate_host",
-           "rttda_get_info", "rttda_last_timings", "rttda_jk_time", "rttda_fp64_peak", "rttda_last_error",
+           "rttda_get_info", "rttda_set_option", "rttda_last_timings", "rttda_jk_time", "rttda_fp64_peak", "rttda_last_error",
            "rttda_version"]
 
 
@@ -192,6 +193,9 @@ class Rttda:
                                           ct.c_double(dt), int(nsteps), _dptr(log), _stream(stream)),
                "rttda_propagate_host")
         return C
+
+    def rttda_set_option(self, option: int, value: float):
+        _check(lib().rttda_set_option(self._h, int(option), ct.c_double(value)), "rttda_set_option")
 
     def rttda_get_info(self, key) -> float:
         out = ct.c_double(0.0)

@@ -94,7 +94,7 @@ int rttda_destroy(rttda_handle_t hh)
     if (!h) return RTTDA_OK;
     cudaDeviceSynchronize();
     for (void* p : h->dev_allocs) cudaFree(p);
-    for (double* p : {h->wsY, h->wsT, h->wsF, h->wsZ, h->wsP, h->prop_ws, h->eri_buf[0], h->eri_buf[1]}) if (p) cudaFree(p);
+    for (double* p : {h->wsY, h->wsT, h->wsF, h->wsZ, h->wsP, h->prop_ws, h->eri_buf[0], h->eri_buf[1], h->eri_all}) if (p) cudaFree(p);
     if (h->st_eval) cudaStreamDestroy(h->st_eval);
     for (cudaEvent_t e : {h->ev_fork, h->ev_E[0], h->ev_E[1], h->ev_D[0], h->ev_D[1]}) if (e) cudaEventDestroy(e);
     for (auto& e : h->ev) if (e) cudaEventDestroy(e);
@@ -192,6 +192,22 @@ int rttda_propagate_host(rttda_handle_t hh, int32_t ntraj, double* C, const rttd
     RT_CUDA(cudaMemcpyAsync(C, h->wsZ, ns * sizeof(double), cudaMemcpyDeviceToHost, st));
     if (log && nl) RT_CUDA(cudaMemcpyAsync(log, h->wsZ + ns, nl * sizeof(double), cudaMemcpyDeviceToHost, st));
     RT_CUDA(cudaStreamSynchronize(st));
+    return RTTDA_OK;
+}
+
+int rttda_set_option(rttda_handle_t hh, int32_t option, double value)
+{
+    Handle* h = (Handle*)hh;
+    RT_CHECK(h != nullptr, "rttda_set_option: NULL handle");
+    RT_CHECK(option == RTTDA_OPT_INCORE, "rttda_set_option: unknown option");
+    const bool on = value != 0.0;
+    if (on && !h->incore) {
+        const int r = ensure_ws(h, &h->eri_all, &h->eri_all_n, h->eri_all_need);
+        if (r != RTTDA_OK) return r;                       // not enough HBM: the handle stays in direct mode
+    }
+    if (!on && h->eri_all) { cudaDeviceSynchronize(); cudaFree(h->eri_all); h->eri_all = nullptr; h->eri_all_n = 0; }
+    h->incore = on;
+    h->incore_valid = false;
     return RTTDA_OK;
 }
 

@@ -102,6 +102,7 @@ struct Segment {
     int la, lb, lc, ld;       // canonical angular momenta (la >= lb, lc >= ld)
     int ni;                   // integrals per quartet
     long long nbatch;         // 32-ket batches in the segment
+    size_t incore_off;        // offset (doubles) of this segment in the in-core integral store
     long long nquartets;      // quartets actually evaluated (unique, screened)
     const long long* batch_base;   // device [n_bra]
     const EvalItem* items;    // device
@@ -153,6 +154,10 @@ struct Handle {
     double* eri_buf[2] = {nullptr, nullptr};
     size_t eri_buf_n[2] = {0, 0};              // doubles allocated
     size_t eri_buf_need = 0;                   // doubles needed by the largest segment
+    // optional in-core mode (rttda_set_option): all segments' integrals kept in HBM after the first pass
+    bool incore = false, incore_valid = false;
+    double* eri_all = nullptr;
+    size_t eri_all_n = 0, eri_all_need = 0;
     cudaStream_t st_eval = nullptr;            // evaluation kernels run here, digestion on the caller's stream
     cudaEvent_t ev_fork = nullptr, ev_E[2] = {nullptr, nullptr}, ev_D[2] = {nullptr, nullptr};
     std::vector<void*> dev_allocs;             // everything to free

@@ -566,13 +566,28 @@ __global__ void symsplit_kernel(int nao, int nvt, const double* __restrict__ T, 
 int jk_build(Handle* h, int nvt, int nvec, const double* Tq, double* Fq, cudaStream_t st)
 {
     RT_CHECK(nvec >= 2 && nvec % 2 == 0 && nvt >= nvec && nvt % 2 == 0, "jk_build: bad density slot counts");
-    for (int b = 0; b < 2; ++b) RT_TRY(ensure_ws(h, &h->eri_buf[b], &h->eri_buf_n[b], h->eri_buf_need));
+    if (!h->incore)
+        for (int b = 0; b < 2; ++b) RT_TRY(ensure_ws(h, &h->eri_buf[b], &h->eri_buf_n[b], h->eri_buf_need));
     {                                   // the exchange kernel gathers {Ps, Pa} pairs: one 16-byte load per (T_mn, T_nm)
         const long long n = (long long)h->nao * h->nao * nvt;
         RT_TRY(ensure_ws(h, &h->wsP, &h->wsP_n, (size_t)2 * n));
         symsplit_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(h->nao, nvt, Tq, reinterpret_cast<double2*>(h->wsP));
         RT_CUDA(cudaGetLastError());
         h->kernel_launches++;
+    }
+    if (h->incore) {
+        // In-core mode (optional, off by default): every segment owns its part of one resident store; the first
+        // pass fills it, later passes only digest.  This trades 8 bytes of HBM per integral for the evaluation.
+        RT_TRY(ensure_ws(h, &h->eri_all, &h->eri_all_n, h->eri_all_need));
+        for (const Segment& sg : h->segments) {
+            if (sg.nitems == 0) continue;
+            double* buf = h->eri_all + sg.incore_off;
+            if (!h->incore_valid) RT_TRY(eval_segment(h, sg, buf, st));
+            for (int l = sg.first_launch; l < sg.first_launch + sg.nlaunch; ++l)
+                RT_TRY(digest_launch(h, h->launches[l], sg, buf, nvt, nvec, Tq, Fq, st));
+        }
+        h->incore_valid = true;
+        return RTTDA_OK;
     }
     RT_CUDA(cudaEventRecord(h->ev_fork, st));
     RT_CUDA(cudaStreamWaitEvent(h->st_eval, h->ev_fork, 0));

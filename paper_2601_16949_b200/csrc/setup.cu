@@ -429,6 +429,8 @@ int create_impl(Handle* h, const rttda_basis_t* basis, const double* C_occ, cons
             n_eval += (double)nquart;
             nprim_eval += (double)nquart * h->tabs.kets[kcb].np * h->tabs.kets[kck].np;
             buf_need = std::max(buf_need, (size_t)nbatch * sg.ni * 32);
+            sg.incore_off = h->eri_all_need;
+            h->eri_all_need += (size_t)nbatch * sg.ni * 32;
             RT_TRY(upload(h, base, &sg.batch_base));
             // evaluation blocks: JK_BLOCK kets x a run of bra pairs (rows staged in shared memory)
             const int npb = h->tabs.kets[kcb].np;
@@ -506,6 +508,7 @@ int create_impl(Handle* h, const rttda_basis_t* basis, const double* C_occ, cons
     h->info[RTTDA_INFO_QMAX] = Qmax;
     h->info[RTTDA_INFO_NVEC_CHUNK] = 0.0;
     h->info[RTTDA_INFO_ERI_BUF_BYTES] = (double)buf_need * sizeof(double);
+    h->info[RTTDA_INFO_ERI_ALL_BYTES] = (double)h->eri_all_need * sizeof(double);
 
     // ---- MO coefficients, eps differences, dipoles
     auto dalloc = [&](double** p, size_t n) -> int {

@@ -348,3 +348,30 @@ def test_propagate_config2_full_2000_steps_vs_dense_A():
     norm_drift = float(np.max(np.abs(log.cpu().numpy()[:, :, 0] - log.cpu().numpy()[0, :, 0])))
     print("config 2, 2000 RK4 steps: max amplitude error %.3e, norm drift %.3e" % (err, norm_drift))
     assert err < AMP_TOL
+
+
+def test_incore_option_matches_direct_mode():
+    """RTTDA_OPT_INCORE: the first pass fills the resident integral store, later passes only digest; results are
+    those of the direct mode and the oracle, and the later passes launch fewer kernels."""
+    import paper_2601_16949_b200 as R
+    from workloads import make_vectors
+    from oracle import tda
+    ctx = setup_config(1, dense=True)
+    h = ctx["h"]
+    X = make_vectors(ctx["cfg"], 4)
+    ref = tda.sigma_dense(ctx["A"], X)
+    direct = gpu_sigma(ctx, X)
+    h.rttda_set_option(R.OPT_INCORE, 1)
+    try:
+        l0 = h.rttda_get_info("kernel_launches")
+        first = gpu_sigma(ctx, X)
+        l1 = h.rttda_get_info("kernel_launches")
+        second = gpu_sigma(ctx, 2.0 * X)
+        l2 = h.rttda_get_info("kernel_launches")
+    finally:
+        h.rttda_set_option(R.OPT_INCORE, 0)
+    assert rel_inf(first, ref) < 1e-12 and rel_inf(second, 2.0 * ref) < 1e-12
+    assert np.max(np.abs(first - direct)) < 1e-13
+    assert (l2 - l1) < (l1 - l0)                      # no evaluation launches in the second pass
+    again = gpu_sigma(ctx, X)                         # back in direct mode
+    assert np.max(np.abs(again - direct)) < 1e-13
