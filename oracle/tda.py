@@ -255,6 +255,14 @@ def sso_dense(A, D_oo, D_vv, D_ov, D_00, y0, f, t_start, dt, nsteps):
                          t_start, dt, nsteps)
 
 
+# ---------------------------------------------------------------- populations (NEXT-2)
+def populations(Xs, y):
+    """P_i = |X_i^dagger y|^2, eq. 22: projection of the time-dependent vector y (length 1 + N_CSF, complex)
+    onto stationary states X_i (rows of Xs, real or complex, same length; the ground state is e_0)."""
+    Xs = np.atleast_2d(np.asarray(Xs))
+    return np.abs(Xs.conj() @ np.asarray(y)) ** 2
+
+
 # ---------------------------------------------------------------- spectrum (harness for the pins)
 def spectrum(R, dt, pad=50000):
     """omega * F[R(t)] with mirroring R(-t) = R(t)^*, Hann window, zero padding (eq. 21).

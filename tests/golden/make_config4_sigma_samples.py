@@ -2,11 +2,13 @@
 """Writes tests/golden/config4_sigma_samples.txt: oracle sigma-vector elements of the 1280-AO molecule.
 
 Calls only oracle/ and workloads/ (never the CUDA path).  sigma = A x (eq. 3 / eq. 11, P:59 / P:97, R1) through the
-oracle's matrix-free route with tau_oracle = 1e-20 (effectively unscreened, S:8(c2) step 6) for the first two seeded
-trial vectors of config 4; 256 seeded sample positions per vector plus the position of the largest element.
-One pass over ~4e10 primitive quartets: 0.5-2 h of CPU time depending on the core count.
+oracle's matrix-free route with tau_oracle = 1e-15 for the first two seeded trial vectors of config 4; 256 seeded
+sample positions per vector plus the position of the largest element.  (tau_oracle = 1e-20, as used for the smaller
+configs, keeps ~1.4e12 primitive quartets at 1280 AOs - about a day of CPU time; at 1e-15 the neglected integrals
+are 1000 times smaller than those the GPU drops at its tightest tested threshold 1e-14, one pass over ~6e10
+primitive quartets: 0.5-1.5 h depending on the core count.)
 
-    python tests/golden/make_config4_sigma_samples.py
+    python tests/golden/make_config4_sigma_samples.py [output file]
 """
 import os
 import sys
@@ -20,7 +22,7 @@ from oracle import tda                      # noqa: E402
 from oracle.integrals import OracleBasis, num_threads  # noqa: E402
 from workloads import get_config, make_basis, make_mos, make_vectors  # noqa: E402
 
-NVEC, NSAMP, TAU_ORACLE = 2, 256, 1e-20
+NVEC, NSAMP, TAU_ORACLE = 2, 256, 1e-15
 
 
 def main():
@@ -34,7 +36,8 @@ def main():
     sig, nq, npq = tda.sigma_matrix_free(ob, X, C_o, C_v, eps, 1.0, tau=TAU_ORACLE)
     dt = time.time() - t0
     rng = np.random.default_rng(20260116949)
-    out = os.path.join(os.path.dirname(os.path.abspath(__file__)), "config4_sigma_samples.txt")
+    out = sys.argv[1] if len(sys.argv) > 1 else os.path.join(os.path.dirname(os.path.abspath(__file__)),
+                                                             "config4_sigma_samples.txt")
     with open(out, "w") as f:
         f.write("# oracle sigma samples, config 4 (1280 AO), written by tests/golden/make_config4_sigma_samples.py\n")
         f.write("# definition: sigma = A x, eq. 3 / eq. 11 (P:59, P:97, reading R1), matrix-free oracle route, tau_oracle = %g\n" % TAU_ORACLE)

@@ -268,6 +268,25 @@ def test_sso_second_order_stationary_ground_state_and_bounded_norm(tiny):
     assert 3.5 < d1 / d2 < 4.5
 
 
+# ------------------------------------------------------------------------------------ populations (eq. 22)
+def test_populations_completeness_and_stationary_states(tiny):
+    A = tiny["A"]
+    w, U = np.linalg.eigh(A)
+    n = A.shape[0]
+    Xs = np.zeros((n + 1, n + 1)); Xs[0, 0] = 1.0; Xs[1:, 1:] = U.T        # ground state + all TI-TDA states
+    rng = np.random.default_rng(3)
+    y = rng.standard_normal(n + 1) + 1j * rng.standard_normal(n + 1)
+    P = tda.populations(Xs, y)
+    assert abs(P.sum() - np.vdot(y, y).real) < 1e-12                       # Parseval over a complete basis
+    assert abs(P[0] - abs(y[0]) ** 2) < 1e-15
+    # a stationary state keeps population 1 (up to the RK4 norm drift) under field-free propagation
+    Doo, Dvv, Dov, D00 = tda.mo_dipoles(tiny["D"], tiny["C_o"], tiny["C_v"], (0, 0, 1.0))
+    y0 = np.zeros(n + 1, dtype=complex); y0[1:] = U[:, 3]
+    yt, _ = tda.rk4_dense(A, Doo, Dvv, Dov, D00, y0, {"type": "none"}, 0.0, 0.05, 50)
+    Pt = tda.populations(Xs, yt)
+    assert abs(Pt[4] - 1.0) < 1e-7 and np.max(np.delete(Pt, 4)) < 1e-20
+
+
 # ------------------------------------------------------------------------------------ paper pins
 def test_paper_unit_conversions():
     pv = paper_values()
