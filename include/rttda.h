@@ -149,6 +149,13 @@ int rttda_propagate_host(rttda_handle_t h, int32_t ntraj, double* C, const rttda
 #define RTTDA_INFO_ERI_ALL_BYTES    14   /* bytes of ALL contracted integrals of one pass (the in-core store) */
 int rttda_get_info(rttda_handle_t h, int32_t key, double* out);
 
+/* Populations of stationary states (NEXT-2 of DESIGN.md): P[t][i] = |X_i^dagger C_t|^2, eq. 22, the projection
+ * of every trajectory's vector onto supplied stationary states (e.g. TI-TDA eigenvectors; the ground state is e_0).
+ *   C  DEVICE [ntraj][2][1 + nocc*nvirt] (layout of rttda_propagate), Xs DEVICE [nstates][1 + nocc*nvirt] real,
+ *   P  DEVICE [ntraj][nstates].  Enqueued on `stream`. */
+int rttda_populations(rttda_handle_t h, int32_t ntraj, const double* C, int32_t nstates, const double* Xs, double* P,
+                      void* stream);
+
 /* Options.  RTTDA_OPT_INCORE (value != 0 switches it on; default off): keep the contracted integrals of all
  * segments resident in HBM (RTTDA_INFO_ERI_ALL_BYTES: 61 GB for the 1280-AO molecule at tau = 1e-12) so that, after
  * the first ERI pass of the handle, later passes skip the evaluation and only digest.  This is NOT the paper's direct

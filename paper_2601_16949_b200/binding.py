@@ -21,7 +21,7 @@ OPT_INCORE = 1
 PULSE = dict(none=0, delta=1, cw=2, tl=3, chirp=4, sin2=5)
 EXPORTS = ["rttda_overlap", "rttda_dipole_ao", "rttda_create", "rttda_destroy", "rttda_sigma",
            "rttda_sigma_host", "rttda_fock", "rttda_propagate", "rttda_propagate_sso", "rttda_propagate_host",
-           "rttda_get_info", "rttda_set_option", "rttda_last_timings", "rttda_jk_time", "rttda_fp64_peak", "rttda_last_error",
+           "rttda_get_info", "rttda_set_option", "rttda_populations", "rttda_last_timings", "rttda_jk_time", "rttda_fp64_peak", "rttda_last_error",
            "rttda_version"]
 
 
@@ -193,6 +193,11 @@ class Rttda:
                                           ct.c_double(dt), int(nsteps), _dptr(log), _stream(stream)),
                "rttda_propagate_host")
         return C
+
+    def rttda_populations(self, C, Xs, P, stream=None):
+        _check(lib().rttda_populations(self._h, int(C.shape[0]), _dptr(C), int(Xs.shape[0]), _dptr(Xs), _dptr(P),
+                                       _stream(stream)), "rttda_populations")
+        return P
 
     def rttda_set_option(self, option: int, value: float):
         _check(lib().rttda_set_option(self._h, int(option), ct.c_double(value)), "rttda_set_option")

@@ -195,6 +195,15 @@ int rttda_propagate_host(rttda_handle_t hh, int32_t ntraj, double* C, const rttd
     return RTTDA_OK;
 }
 
+int rttda_populations(rttda_handle_t hh, int32_t ntraj, const double* C, int32_t nstates, const double* Xs, double* P,
+                      void* stream)
+{
+    Handle* h = (Handle*)hh;
+    RT_CHECK(h && C && Xs && P, "rttda_populations: NULL pointer");
+    RT_CHECK(ntraj >= 1 && nstates >= 1, "rttda_populations: ntraj and nstates must be positive");
+    return populations_impl(h, ntraj, C, nstates, Xs, P, (cudaStream_t)stream);
+}
+
 int rttda_set_option(rttda_handle_t hh, int32_t option, double value)
 {
     Handle* h = (Handle*)hh;

@@ -416,4 +416,41 @@ int propagate_sso_impl(Handle* h, int ntraj, double* y, const rttda_field_t* fie
     return RTTDA_OK;
 }
 
+// ---------------------------------------------------------------------------------------------- populations
+// P[t][i] = |X_i^dagger y_t|^2 (eq. 22) for real stationary-state vectors X_i [nstates][n1]; one block per (t, i)
+__global__ void __launch_bounds__(256)
+populations_kernel(long long n1, int nstates, const double* __restrict__ y, const double* __restrict__ Xs,
+                   double* __restrict__ P)
+{
+    const int t = blockIdx.x / nstates, i = blockIdx.x % nstates;
+    const double *q = y + 2 * t * n1, *p = q + n1, *x = Xs + (long long)i * n1;
+    double re = 0.0, im = 0.0;
+    for (long long e = threadIdx.x; e < n1; e += blockDim.x) {
+        const double xv = x[e];
+        re = fma(xv, q[e], re);
+        im = fma(xv, p[e], im);
+    }
+    __shared__ double red[2][8];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        re += __shfl_xor_sync(0xffffffffu, re, o);
+        im += __shfl_xor_sync(0xffffffffu, im, o);
+    }
+    if ((threadIdx.x & 31) == 0) { red[0][threadIdx.x >> 5] = re; red[1][threadIdx.x >> 5] = im; }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double a = 0.0, b = 0.0;
+        for (int w = 0; w < (int)(blockDim.x >> 5); ++w) { a += red[0][w]; b += red[1][w]; }
+        P[blockIdx.x] = a * a + b * b;
+    }
+}
+
+int populations_impl(Handle* h, int ntraj, const double* y, int nstates, const double* Xs, double* P, cudaStream_t st)
+{
+    populations_kernel<<<ntraj * nstates, 256, 0, st>>>((long long)h->ncsf + 1, nstates, y, Xs, P);
+    RT_CUDA(cudaGetLastError());
+    h->kernel_launches++;
+    return RTTDA_OK;
+}
+
 }  // namespace rttda

@@ -375,3 +375,26 @@ def test_incore_option_matches_direct_mode():
     assert (l2 - l1) < (l1 - l0)                      # no evaluation launches in the second pass
     again = gpu_sigma(ctx, X)                         # back in direct mode
     assert np.max(np.abs(again - direct)) < 1e-13
+
+
+def test_populations_vs_oracle():
+    """eq. 22: populations of the ground state and the TI-TDA states (eigenvectors of the oracle's dense A) along a
+    driven trajectory, against the oracle's projection of the same state."""
+    import torch
+    from oracle import tda
+    ctx = setup_config(1, dense=True)
+    h, A = ctx["h"], ctx["A"]
+    n = A.shape[0]
+    w, U = np.linalg.eigh(A)
+    Xs = np.zeros((6, n + 1)); Xs[0, 0] = 1.0; Xs[1:, 1:] = U[:, :5].T
+    f = {"type": "cw", "E0": 0.05, "omega": float(w[0]), "dir": (0.0, 0.0, 1.0)}
+    y = torch.from_numpy(_state0(2, n)).to(ctx["dev"])
+    h.rttda_propagate(y, [f, dict(f, E0=0.1)], 0.0, 0.05, 40, None)
+    P = torch.zeros((2, 6), dtype=torch.float64, device=ctx["dev"])
+    h.rttda_populations(y, torch.from_numpy(Xs).to(ctx["dev"]), P)
+    torch.cuda.synchronize()
+    yh = y.cpu().numpy()
+    for t in range(2):
+        ref = tda.populations(Xs, yh[t, 0] + 1j * yh[t, 1])
+        assert np.max(np.abs(P.cpu().numpy()[t] - ref)) < 1e-14
+    assert P.cpu().numpy()[1, 0] < P.cpu().numpy()[0, 0] < 1.0          # the stronger field depletes the ground state more
