@@ -263,6 +263,30 @@ def populations(Xs, y):
     return np.abs(Xs.conj() @ np.asarray(y)) ** 2
 
 
+# ---------------------------------------------------------------- Lanczos on A (NEXT-3: TI-TDA eigenvalues, eq. 2)
+def lanczos(apply_A, v0, m, reorth=True):
+    """m steps of the symmetric Lanczos process on the singles block A (TI-TDA eigenproblem A X = omega X, eq. 2):
+        v_1 = v0/|v0|;  w = A v_j - beta_{j-1} v_{j-1};  alpha_j = v_j.w;  w -= alpha_j v_j;
+        (reorth: w -= V_j (V_j^T w), applied twice);  beta_j = |w|;  v_{j+1} = w / beta_j.
+    Returns alpha [m], beta [m], V [m+1][n]; the Ritz values are the eigenvalues of tridiag(alpha, beta[:-1])."""
+    n = v0.shape[0]
+    V = np.zeros((m + 1, n))
+    alpha, beta = np.zeros(m), np.zeros(m)
+    V[0] = v0 / np.linalg.norm(v0)
+    for j in range(m):
+        w = apply_A(V[j])
+        if j > 0:
+            w = w - beta[j - 1] * V[j - 1]
+        alpha[j] = V[j] @ w
+        w = w - alpha[j] * V[j]
+        if reorth:
+            for _ in range(2):
+                w = w - V[: j + 1].T @ (V[: j + 1] @ w)
+        beta[j] = np.linalg.norm(w)
+        V[j + 1] = w / beta[j]
+    return alpha, beta, V
+
+
 # ---------------------------------------------------------------- spectrum (harness for the pins)
 def spectrum(R, dt, pad=50000):
     """omega * F[R(t)] with mirroring R(-t) = R(t)^*, Hann window, zero padding (eq. 21).

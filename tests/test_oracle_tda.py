@@ -287,6 +287,31 @@ def test_populations_completeness_and_stationary_states(tiny):
     assert abs(Pt[4] - 1.0) < 1e-7 and np.max(np.delete(Pt, 4)) < 1e-20
 
 
+# ------------------------------------------------------------------------------------ Lanczos (eq. 2)
+def test_lanczos_relation_orthogonality_and_ritz_values(tiny):
+    A = tiny["A"]
+    n = A.shape[0]
+    rng = np.random.default_rng(5)
+    v0 = rng.standard_normal(n)
+    m = 40
+    al, be, V = tda.lanczos(lambda x: A @ x, v0, m)
+    T = np.diag(al) + np.diag(be[:-1], 1) + np.diag(be[:-1], -1)
+    Vm = V[:m].T
+    # Lanczos relation A V_m = V_m T_m + beta_m v_{m+1} e_m^T and orthonormal basis: checks of the recurrence itself
+    Rm = A @ Vm - Vm @ T
+    Rm[:, -1] -= be[-1] * V[m]
+    assert np.max(np.abs(Rm)) < 1e-12
+    assert np.max(np.abs(V @ V.T - np.eye(m + 1))) < 1e-12
+    # extremal Ritz values converge to the extremal eigenvalues of dense A
+    w = np.linalg.eigvalsh(A)
+    th = np.linalg.eigvalsh(T)
+    assert abs(th[0] - w[0]) < 1e-8 and abs(th[-1] - w[-1]) < 1e-8
+    # after n steps the Krylov space is the whole space: all eigenvalues
+    al, be, V = tda.lanczos(lambda x: A @ x, v0, n - 1)
+    T = np.diag(al) + np.diag(be[:-1], 1) + np.diag(be[:-1], -1)
+    assert np.max(np.abs(np.linalg.eigvalsh(T)[[0, -1]] - w[[0, -1]])) < 1e-10
+
+
 # ------------------------------------------------------------------------------------ paper pins
 def test_paper_unit_conversions():
     pv = paper_values()
