@@ -149,6 +149,13 @@ int rttda_propagate_host(rttda_handle_t h, int32_t ntraj, double* C, const rttda
 #define RTTDA_INFO_ERI_ALL_BYTES    14   /* bytes of ALL contracted integrals of one pass (the in-core store) */
 int rttda_get_info(rttda_handle_t h, int32_t key, double* out);
 
+/* TI-TDA eigenvalues through the same sigma builds (NEXT-3 of DESIGN.md): m steps of the symmetric Lanczos process on
+ * the singles block A (A X = omega X, eq. 2), one sigma vector per step, full reorthogonalisation.
+ *   v0 DEVICE [nocc*nvirt] start vector (any norm), alpha, beta HOST [m], V DEVICE [m+1][nocc*nvirt] (the Lanczos
+ *   vectors; must not alias v0).  The Ritz values are the eigenvalues of tridiag(alpha, beta[0..m-2]); the caller
+ *   diagonalises that small matrix.  Synchronises `stream` every step (alpha_j, beta_j are read back). */
+int rttda_lanczos(rttda_handle_t h, int32_t m, const double* v0, double* alpha, double* beta, double* V, void* stream);
+
 /* Populations of stationary states (NEXT-2 of DESIGN.md): P[t][i] = |X_i^dagger C_t|^2, eq. 22, the projection
  * of every trajectory's vector onto supplied stationary states (e.g. TI-TDA eigenvectors; the ground state is e_0).
  *   C  DEVICE [ntraj][2][1 + nocc*nvirt] (layout of rttda_propagate), Xs DEVICE [nstates][1 + nocc*nvirt] real,

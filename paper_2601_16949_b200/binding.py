@@ -21,7 +21,7 @@ OPT_INCORE = 1
 PULSE = dict(none=0, delta=1, cw=2, tl=3, chirp=4, sin2=5)
 EXPORTS = ["rttda_overlap", "rttda_dipole_ao", "rttda_create", "rttda_destroy", "rttda_sigma",
            "rttda_sigma_host", "rttda_fock", "rttda_propagate", "rttda_propagate_sso", "rttda_propagate_host",
-           "rttda_get_info", "rttda_set_option", "rttda_populations", "rttda_last_timings", "rttda_jk_time", "rttda_fp64_peak", "rttda_last_error",
+           "rttda_get_info", "rttda_set_option", "rttda_populations", "rttda_lanczos", "rttda_last_timings", "rttda_jk_time", "rttda_fp64_peak", "rttda_last_error",
            "rttda_version"]
 
 
@@ -193,6 +193,13 @@ class Rttda:
                                           ct.c_double(dt), int(nsteps), _dptr(log), _stream(stream)),
                "rttda_propagate_host")
         return C
+
+    def rttda_lanczos(self, m: int, v0, V, stream=None):
+        """Returns (alpha, beta) as numpy arrays; V (CUDA tensor [m+1][ncsf]) receives the Lanczos vectors."""
+        alpha, beta = np.zeros(m), np.zeros(m)
+        _check(lib().rttda_lanczos(self._h, int(m), _dptr(v0), _dptr(alpha), _dptr(beta), _dptr(V), _stream(stream)),
+               "rttda_lanczos")
+        return alpha, beta
 
     def rttda_populations(self, C, Xs, P, stream=None):
         _check(lib().rttda_populations(self._h, int(C.shape[0]), _dptr(C), int(Xs.shape[0]), _dptr(Xs), _dptr(P),

@@ -195,6 +195,15 @@ int rttda_propagate_host(rttda_handle_t hh, int32_t ntraj, double* C, const rttd
     return RTTDA_OK;
 }
 
+int rttda_lanczos(rttda_handle_t hh, int32_t m, const double* v0, double* alpha, double* beta, double* V, void* stream)
+{
+    Handle* h = (Handle*)hh;
+    RT_CHECK(h && v0 && alpha && beta && V, "rttda_lanczos: NULL pointer");
+    RT_CHECK(m >= 1 && m < h->ncsf, "rttda_lanczos: need 1 <= m < nocc*nvirt");
+    RT_CHECK(v0 < V || v0 >= V + (size_t)(m + 1) * h->ncsf, "rttda_lanczos: v0 must not alias V");
+    return lanczos_impl(h, m, v0, alpha, beta, V, (cudaStream_t)stream);
+}
+
 int rttda_populations(rttda_handle_t hh, int32_t ntraj, const double* C, int32_t nstates, const double* Xs, double* P,
                       void* stream)
 {

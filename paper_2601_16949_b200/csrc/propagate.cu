@@ -1,5 +1,6 @@
 // sigma = A X (steps a1-a5), field coupling (a6, eq. 16/19) and the RK4 propagator (a7, eq. 1, 12-15).
 #include <cmath>
+#include <vector>
 #include "common.cuh"
 
 namespace rttda {
@@ -450,6 +451,82 @@ int populations_impl(Handle* h, int ntraj, const double* y, int nstates, const d
     populations_kernel<<<ntraj * nstates, 256, 0, st>>>((long long)h->ncsf + 1, nstates, y, Xs, P);
     RT_CUDA(cudaGetLastError());
     h->kernel_launches++;
+    return RTTDA_OK;
+}
+
+// ---------------------------------------------------------------------------------------------- Lanczos
+// out[i] = sum_e V[i][e] w[e] for i < nv (one block per i)
+__global__ void __launch_bounds__(256)
+multi_dot_kernel(long long n, const double* __restrict__ V, const double* __restrict__ w, double* __restrict__ out)
+{
+    const double* v = V + (long long)blockIdx.x * n;
+    double s = 0.0;
+    for (long long e = threadIdx.x; e < n; e += blockDim.x) s = fma(v[e], w[e], s);
+    __shared__ double red[8];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+    if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = s;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double a = 0.0;
+        for (int k = 0; k < (int)(blockDim.x >> 5); ++k) a += red[k];
+        out[blockIdx.x] = a;
+    }
+}
+// w[e] -= sum_i c[i] V[i][e]
+__global__ void multi_axpy_kernel(long long n, int nv, const double* __restrict__ V, const double* __restrict__ c,
+                                  double* __restrict__ w)
+{
+    const long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (e >= n) return;
+    double s = w[e];
+    for (int i = 0; i < nv; ++i) s = fma(-c[i], V[(long long)i * n + e], s);
+    w[e] = s;
+}
+__global__ void scale_to_kernel(long long n, double a, const double* __restrict__ in, double* __restrict__ out)
+{
+    const long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (e < n) out[e] = a * in[e];
+}
+
+// m steps of symmetric Lanczos on the singles block A through sigma_impl (one sigma vector per step), with full
+// reorthogonalisation (twice) against all previous Lanczos vectors.  alpha, beta: host [m]; V: DEVICE [m+1][ncsf].
+int lanczos_impl(Handle* h, int m, const double* v0, double* alpha, double* beta, double* V, cudaStream_t st)
+{
+    const long long n = h->ncsf;
+    const unsigned eg = (unsigned)((n + 255) / 256);
+    RT_TRY(ensure_ws(h, &h->wsZ, &h->wsZ_n, (size_t)n + (size_t)m + 2));
+    double* w = h->wsZ;
+    double* dots = h->wsZ + n;                              // [m+1] device scalars
+    std::vector<double> hd((size_t)m + 2);
+    // v_1 = v0 / |v0|
+    multi_dot_kernel<<<1, 256, 0, st>>>(n, v0, v0, dots);
+    RT_CUDA(cudaMemcpyAsync(hd.data(), dots, sizeof(double), cudaMemcpyDeviceToHost, st));
+    RT_CUDA(cudaStreamSynchronize(st));
+    RT_CHECK(hd[0] > 0.0, "rttda_lanczos: zero start vector");
+    scale_to_kernel<<<eg, 256, 0, st>>>(n, 1.0 / std::sqrt(hd[0]), v0, V);
+    h->kernel_launches += 2;
+    for (int j = 0; j < m; ++j) {
+        double* vj = V + (size_t)j * n;
+        RT_TRY(sigma_impl(h, 1, vj, n, w, n, st));                              // w = A v_j
+        // one pass of coefficients against v_0..v_j removes alpha_j v_j and beta_{j-1} v_{j-1} (and, in exact
+        // arithmetic, nothing else); alpha_j is the coefficient of v_j in that first pass
+        for (int pass = 0; pass < 3; ++pass) {
+            multi_dot_kernel<<<j + 1, 256, 0, st>>>(n, V, w, dots);
+            if (pass == 0) RT_CUDA(cudaMemcpyAsync(hd.data(), dots + j, sizeof(double), cudaMemcpyDeviceToHost, st));
+            multi_axpy_kernel<<<eg, 256, 0, st>>>(n, j + 1, V, dots, w);
+            h->kernel_launches += 2;
+        }
+        multi_dot_kernel<<<1, 256, 0, st>>>(n, w, w, dots);
+        RT_CUDA(cudaMemcpyAsync(hd.data() + 1, dots, sizeof(double), cudaMemcpyDeviceToHost, st));
+        RT_CUDA(cudaStreamSynchronize(st));
+        alpha[j] = hd[0];
+        beta[j] = std::sqrt(hd[1]);
+        RT_CHECK(beta[j] > 0.0, "rttda_lanczos: breakdown (invariant subspace reached)");
+        scale_to_kernel<<<eg, 256, 0, st>>>(n, 1.0 / beta[j], w, V + (size_t)(j + 1) * n);
+        h->kernel_launches += 2;
+    }
+    RT_CUDA(cudaGetLastError());
     return RTTDA_OK;
 }
 

@@ -398,3 +398,26 @@ def test_populations_vs_oracle():
         ref = tda.populations(Xs, yh[t, 0] + 1j * yh[t, 1])
         assert np.max(np.abs(P.cpu().numpy()[t] - ref)) < 1e-14
     assert P.cpu().numpy()[1, 0] < P.cpu().numpy()[0, 0] < 1.0          # the stronger field depletes the ground state more
+
+
+def test_lanczos_vs_oracle_and_dense_eigenvalues():
+    """NEXT-3: Lanczos on A through the GPU sigma builds: coefficients against the oracle's Lanczos on dense A (same
+    start vector), Ritz values against eigh(A)."""
+    import torch
+    from oracle import tda
+    ctx = setup_config(1, dense=True)
+    h, A = ctx["h"], ctx["A"]
+    n = A.shape[0]
+    v0 = np.random.default_rng(8).standard_normal(n)
+    m = 30
+    V = torch.zeros((m + 1, n), dtype=torch.float64, device=ctx["dev"])
+    al, be = h.rttda_lanczos(m, torch.from_numpy(v0).to(ctx["dev"]), V)
+    torch.cuda.synchronize()
+    ral, rbe, rV = tda.lanczos(lambda x: A @ x, v0, m)
+    assert np.max(np.abs(al - ral)) < 1e-9 and np.max(np.abs(be - rbe)) < 1e-9
+    Vh = V.cpu().numpy()
+    assert np.max(np.abs(Vh @ Vh.T - np.eye(m + 1))) < 1e-12
+    T = np.diag(al) + np.diag(be[:-1], 1) + np.diag(be[:-1], -1)
+    w = np.linalg.eigvalsh(A)
+    th = np.linalg.eigvalsh(T)
+    assert abs(th[0] - w[0]) < 1e-8 and abs(th[-1] - w[-1]) < 1e-8
