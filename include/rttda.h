@@ -98,7 +98,7 @@ int rttda_destroy(rttda_handle_t h);
 
 /* sigma_v = A x_v for v < nvec (singles block only, R16).  X, sigma DEVICE [nvec][nocc*nvirt]; must not
  * alias.  Steps a1-a5 of DESIGN.md: MO->AO transform (FP64 tensor-core GEMM), Schwarz-screened direct J/K
- * (one ERI pass per chunk of densities), AO->MO transform + (eps_a - eps_i) x. */
+ * (ONE evaluation pass serves all densities of the call), AO->MO transform + (eps_a - eps_i) x. */
 int rttda_sigma(rttda_handle_t h, int32_t nvec, const double* X, double* sigma, void* stream);
 
 /* Same with HOST buffers: H2D copy of X, sigma build, D2H copy of sigma, stream synchronised. */
