@@ -380,7 +380,7 @@ def run_b200(args):
                           "eri_staging_buffer_bytes": info["eri_buf_bytes"]},
                "setup_s": setup_s, "create_ms": info["create_ms"],
                "jk_ms_per_pass": jk_avg_ms, "jk_share_of_step": jk_ms / (sum(ms) if sum(ms) else 1.0),
-               "roofline": {"bound": "alu", "kernel": "eval_kernel<*> + digest_kernel<*,1> + digest_b_kernel<*> (all launches of one ERI pass)",
+               "roofline": {"bound": "alu", "kernel": "eval_kernel<*> + digest_j_kernel<*> + digest_b_kernel<*> (all launches of one ERI pass)",
                             "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
                             "traffic": traffic, "traffic_source": "profiles/r1_traffic_per_pass.json (ncu dram__bytes_read+write "
                             "summed over the launches of one ERI pass, config 4, nvec 6)" if traffic else None,

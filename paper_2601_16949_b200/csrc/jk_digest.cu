@@ -1,20 +1,19 @@
 // J/K digestion (DESIGN.md step a4; "Coulomb and Exchange terms" P:130): F += 2 J[T] - cx K[T] from the
 // contracted integrals the evaluation kernels staged in HBM (jk_eval.cu), for NV densities per launch.
 //
-// Work decomposition ("shell a fixed per block, ket pair owned by a thread"):
-//   block  = one a-list (all ordered bra pairs (a,b) for one shell a, one l_b, one contraction sub-class,
-//            sorted by Schwarz bound) x JK_BLOCK consecutive kets of one ket class
-//   thread = one unordered ket pair {c,d}; it walks the a-list while Q_ab Q_cd >= tau, streams the stored
-//            block (ab|cd) (coalesced, read-once) and digests it for NV densities:
+// Work decomposition ("shell a fixed per block, ket pair owned by a thread or lane group"):
+//   block  = one a-list (all ordered bra pairs (a,b) for one shell a, one l_b, one contraction sub-class, sorted by
+//            Schwarz bound) x consecutive kets of one ket class; it walks the a-list while Q_ab Q_cd >= tau and
+//            streams the stored blocks (ab|cd) through TMA bulk-copy rings in shared memory:
 //              K_ac += I T_bd, K_ad += I T_bc, K_ca += I T_db, K_da += I T_cb      (registers, whole b loop)
 //              J_cd += I (T_ab + T_ba)                                             (registers, canonical bras)
 //              J_ab += I (T_cd + T_dc)                                             (warp butterfly reduce)
 //   Both orientations (a,b), (b,a) of a bra pair are separate records reading the SAME stored block, which
 //   keeps every exchange update in registers: no per-quartet global atomics, and no second evaluation.
 // Densities and results use the interleaved layout Tq[mu][nu][v] (v fastest), F likewise.
-// Two kernels share that decomposition: digest_j_kernel (thread = ket, NV densities in registers) does the Coulomb
-// part over the canonical records without any per-lane density gather; digest_b_kernel (block = one 32-ket batch,
-// a group of lanes per ket, lane = density) does the exchange part, gathering {T + T^T, T - T^T} pairs
+// Two kernels: digest_j_kernel (thread = ket, NV densities in registers, 128 kets per block) does the Coulomb part
+// over the canonical records without any per-lane density gather; digest_b_kernel (block = one 32-ket batch, a
+// group of lanes per ket, lane = density) does the exchange part, gathering {T + T^T, T - T^T} pairs
 // (symsplit_kernel) so that one 16-byte load yields both T_mn and T_nm.  DESIGN.md section 5 has the rooflines,
 // profiles/ the ncu evidence.
 #include "common.cuh"
