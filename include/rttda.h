@@ -5,7 +5,8 @@
  *   sigma = A X,  A_{ia,jb} = d_ij d_ab (eps_a - eps_i) + 2 (ia|jb) - c_x (ij|ab)     eq. 3 P:59 (R1), eq. 11
  *   index ia = i*nvirt + a (virtuals run fastest)
  *   direct CI through AO-basis Coulomb/exchange builds on the GPU
- *   i dC/dt = H(t) C,  H(t) = A_ext + E(t) M_d  (M_d from MO dipoles, Slater-Condon)    eq. 1, eq. 16 P:134,
+ *   i dC/dt = H(t) C,  H(t) = A_ext + E(t) M_d  (M_d from MO dipoles, Slater-Condon;    eq. 1, eq. 16 P:134,
+ *   dipole origin = electronic centroid of the ground state, R6)
  *                                                                                       eq. 19 P:161-173 (R3-R5)
  *   C = q + i p, ground-state element first                                             eq. 12
  *   pulses                                                                              eq. 18a-d P:146-153 (R8, R9)

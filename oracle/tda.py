@@ -76,11 +76,23 @@ def sigma_matrix_free(ob, X, C_o, C_v, eps, cx=1.0, tau=0.0, Q=None):
 
 # ---------------------------------------------------------------- dipole operator in the CSF basis
 def mo_dipoles(D_ao, C_o, C_v, d):
-    """D_d = sum_k d_k D^k in the MO basis: D_oo, D_vv, D_ov and D_00 = 2 tr D_oo (R3)."""
+    """D_d = sum_k d_k D^k in the MO basis: D_oo, D_vv, D_ov and D_00 = 2 tr D_oo (R3).
+
+    Dipole origin (reading R6): the electronic centroid of the ground state, c = tr(D_oo)/n_occ along d.  The paper's
+    dipole operator is the molecular one: for a neutral molecule it does not depend on the origin and its
+    ground-state expectation value (eq. 19a) is the permanent dipole moment, O(1) au.  The synthetic centres carry no
+    charges (R5), so the bare electronic D_00 = 2 sum_i <i|r|i> would grow with the distance of the molecule from
+    the coordinate origin (1e4 au for the 1280-AO molecule: a global phase rotating 500 times faster than any
+    excitation, which no fixed-step propagator at the configs' dt can follow).  With orthonormal MOs (C^T S C = 1,
+    checked by the tests) the shift r -> r - c acts as D_oo -> D_oo - c 1, D_vv -> D_vv - c 1, D_ov unchanged, and
+    D_00 -> 0; eq. 19a-f are applied unchanged to the shifted matrices."""
     Dd = np.einsum("k,kmn->mn", np.asarray(d, dtype=np.float64), D_ao)
     D_oo = C_o.T @ Dd @ C_o
     D_vv = C_v.T @ Dd @ C_v
     D_ov = C_o.T @ Dd @ C_v
+    c = np.trace(D_oo) / D_oo.shape[0]
+    D_oo = D_oo - c * np.eye(D_oo.shape[0])
+    D_vv = D_vv - c * np.eye(D_vv.shape[0])
     return D_oo, D_vv, D_ov, 2.0 * np.trace(D_oo)
 
 

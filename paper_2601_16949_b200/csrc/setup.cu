@@ -175,6 +175,12 @@ static void prim_rows(const HostBasis& H, int s1, int s2, std::vector<double>& r
         }
 }
 
+__global__ void shift_diag_kernel(int n, double c, double* __restrict__ A)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) A[(size_t)i * n + i] += c;
+}
+
 struct Pair {
     int s1, s2;          // first (higher l, or larger index at equal l), second
     int pc, sub, np;     // pair class, contraction sub-class, primitive pairs
@@ -567,11 +573,23 @@ int create_impl(Handle* h, const rttda_basis_t* basis, const double* C_occ, cons
     RT_CUDA(cudaMemcpyAsync(doo.data(), h->D_oo, doo.size() * sizeof(double), cudaMemcpyDeviceToHost, st));
     RT_CUDA(cudaStreamSynchronize(st));
     cudaFree(tmp);
+    // Dipole origin = electronic centroid of the ground state, c_k = tr(D_oo^k)/n_occ (R6): with orthonormal MOs the
+    // shift r -> r - c is D_oo -> D_oo - c 1, D_vv -> D_vv - c 1, D_ov unchanged, and D_00 = 2 tr D_oo (R3: sum
+    // over spin orbitals) becomes zero.  Without it D_00 grows with the molecule's distance from the coordinate
+    // origin (1e4 au at 1280 AOs) and E(t) D_00 is a global phase no fixed-step propagator can follow.
     for (int k = 0; k < 3; ++k) {
         double tr = 0.0;
         for (size_t i = 0; i < no; ++i) tr += doo[k * no * no + i * no + i];
-        h->D_00[k] = 2.0 * tr;                 // R3: sum over spin orbitals
+        const double c = tr / (double)no;
+        shift_diag_kernel<<<(unsigned)((no + 255) / 256), 256, 0, st>>>((int)no, -c, h->D_oo + (size_t)k * no * no);
+        shift_diag_kernel<<<(unsigned)((nv + 255) / 256), 256, 0, st>>>((int)nv, -c, h->D_vv + (size_t)k * nv * nv);
+        double tr2 = 0.0;
+        for (size_t i = 0; i < no; ++i) tr2 += doo[k * no * no + i * no + i] - c;
+        h->D_00[k] = 2.0 * tr2;
     }
+    RT_CUDA(cudaGetLastError());
+    RT_CUDA(cudaStreamSynchronize(st));
+    h->kernel_launches += 6;
     for (auto& e : h->ev) RT_CUDA(cudaEventCreate(&e));
     RT_CUDA(cudaStreamCreateWithFlags(&h->st_eval, cudaStreamNonBlocking));
     RT_CUDA(cudaEventCreateWithFlags(&h->ev_fork, cudaEventDisableTiming));

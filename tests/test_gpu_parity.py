@@ -423,3 +423,68 @@ def test_lanczos_vs_oracle_and_dense_eigenvalues():
     w = np.linalg.eigvalsh(A)
     th = np.linalg.eigvalsh(T)
     assert abs(th[0] - w[0]) < 1e-8 and abs(th[-1] - w[-1]) < 1e-8
+
+
+def _slow():
+    import os
+    if os.environ.get("RTTDA_SLOW_TESTS") != "1":
+        pytest.skip("set RTTDA_SLOW_TESTS=1 to run the slow trajectory checks (results recorded in DESIGN.md section 7)")
+
+
+def test_propagate_config3_prefix_vs_matrix_free_oracle():
+    """Config 3 (400 AO, dense A = 5.2 GB is not built): the first 3 RK4 steps of the resonant cw trajectory with
+    E0 = 0.02 against the oracle's matrix-free RK4 (12 oracle J/K passes, ~5 min)."""
+    _slow()
+    import torch
+    from oracle import tda
+    ctx = setup_config(3)
+    cfg, h = ctx["cfg"], ctx["h"]
+    f = dict(cfg.fields[1]); f["omega"] = 0.35                            # any recorded omega serves parity (R10)
+    D = ctx["ob"].dipole()
+    Doo, Dvv, Dov, D00 = tda.mo_dipoles(D, ctx["C_o"], ctx["C_v"], f["dir"])
+    n = cfg.nocc * cfg.nvirt
+    y0 = np.zeros(n + 1, dtype=complex); y0[0] = 1.0
+    Q = ctx["ob"].schwarz()
+    yref, _ = tda.rk4_matrix_free(ctx["ob"], ctx["C_o"], ctx["C_v"], ctx["eps"], 1.0, 1e-20, Q, Doo, Dvv, Dov, D00,
+                                  y0, f, 0.0, cfg.dt, 3)
+    y = torch.from_numpy(_state0(1, n)).to(ctx["dev"])
+    h.rttda_propagate(y, [f], 0.0, cfg.dt, 3, None)
+    torch.cuda.synchronize()
+    y = y.cpu().numpy()
+    err = max(float(np.max(np.abs(y[0, 0] - yref.real))), float(np.max(np.abs(y[0, 1] - yref.imag))))
+    print("config 3, 3 RK4 steps vs matrix-free oracle: max amplitude error %.3e" % err)
+    assert err < AMP_TOL
+
+
+def test_propagate_config4_indirect_checks():
+    """Config 4 (1280 AO): the oracle cannot follow a trajectory (one RK4 step = 4 passes of ~20 min), so the
+    checks are the indirect ones of S:8(c5): (5) dt-halving self-convergence of RK4 (ratio ~16) and the RK4
+    norm-drift law, (6) tau-convergence of the trajectory (1e-12 vs 1e-14)."""
+    _slow()
+    import torch
+    import paper_2601_16949_b200 as R
+    ctx = setup_config(4)
+    cfg, h = ctx["cfg"], ctx["h"]
+    n = cfg.nocc * cfg.nvirt
+    f = dict(cfg.fields[2]); f["omega"] = 0.4; f["T_env"] = 4.0          # strong, short pulse so that 2 au of time matter
+
+    def run(handle, dt, nsteps):
+        y = torch.from_numpy(_state0(1, n)).to(ctx["dev"])
+        log = torch.zeros((nsteps, 1, 3), dtype=torch.float64, device=ctx["dev"])
+        handle.rttda_propagate(y, [f], 0.0, dt, nsteps, log)
+        torch.cuda.synchronize()
+        y = y.cpu().numpy()
+        return y[0, 0] + 1j * y[0, 1], log.cpu().numpy()[:, 0, 0]
+    y1, n1 = run(h, 0.1, 20)                                           # lambda_max(A) dt = 1.3: inside RK4's stability region
+    y2, _ = run(h, 0.05, 40)
+    y4, _ = run(h, 0.025, 80)
+    ratio = np.max(np.abs(y1 - y2)) / np.max(np.abs(y2 - y4))
+    h14 = R.Rttda(ctx["basis"], torch.from_numpy(ctx["C_o"]).to(ctx["dev"]), torch.from_numpy(ctx["C_v"]).to(ctx["dev"]),
+                  ctx["eps"], 1.0, 1e-14)
+    y2t, _ = run(h14, 0.05, 40)
+    h14.close()
+    dtau = float(np.max(np.abs(y2 - y2t)))
+    print("config 4: dt-halving ratio %.2f, tau 1e-12 vs 1e-14 after 40 steps %.3e, norm drift (dt 0.1, 20 steps) %.3e"
+          % (ratio, dtau, float(np.max(np.abs(n1 - 1.0)))))
+    assert 10.0 < ratio < 24.0
+    assert dtau < 1e-9

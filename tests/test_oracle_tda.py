@@ -98,11 +98,20 @@ def test_M_explicit_equals_matrix_free(tiny):
     rng = np.random.default_rng(1)
     y = rng.standard_normal(M.shape[0]) + 1j * rng.standard_normal(M.shape[0])
     assert np.max(np.abs(M @ y - tda.apply_M(y, Doo, Dvv, Dov, D00))) < 1e-13
-    # origin shift c changes M only by the multiple 2 nocc (-c.d) of the identity (R6)
+    # R6: the dipole origin is the electronic centroid of the ground state, so M does not depend on where the AO
+    # dipole integrals were taken from (a bare origin shift c would add the multiple -2 nocc (c.d) of the identity),
+    # and the ground-state element D_00 vanishes
     c = np.array([1.0, 2.0, -0.5])
     Doo2, Dvv2, Dov2, D002 = tda.mo_dipoles(tiny["ob"].dipole(c), tiny["C_o"], tiny["C_v"], d)
     M2 = tda.build_M_explicit(Doo2, Dvv2, Dov2, D002)
-    assert np.max(np.abs(M2 - M + 2 * 5 * (c @ d) * np.eye(M.shape[0]))) < 1e-11
+    assert np.max(np.abs(M2 - M)) < 1e-11
+    assert abs(D00) < 1e-12 and abs(M[0, 0]) < 1e-12
+    # the shifted one-electron matrices are those of the operator (r - centroid).d
+    Dd = np.einsum("k,kmn->mn", d, tiny["D"])
+    cen = np.trace(tiny["C_o"].T @ Dd @ tiny["C_o"]) / tiny["C_o"].shape[1]
+    assert np.max(np.abs(Doo - tiny["C_o"].T @ (Dd - cen * tiny["S"]) @ tiny["C_o"])) < 1e-11
+    assert np.max(np.abs(Dvv - tiny["C_v"].T @ (Dd - cen * tiny["S"]) @ tiny["C_v"])) < 1e-11
+    assert np.max(np.abs(Dov - tiny["C_o"].T @ (Dd - cen * tiny["S"]) @ tiny["C_v"])) < 1e-11
 
 
 def test_M_is_slater_condon_of_one_electron_operator():
