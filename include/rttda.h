@@ -81,7 +81,8 @@ typedef struct {
  * orthonormal MOs (C = S^-1/2 Q).  EINVAL if nao does not match the shell table. */
 int rttda_overlap(const rttda_basis_t* basis, int32_t nao, double* S);
 
-/* Position-operator matrices D^k_{mu nu} = <mu| r_k |nu>, origin (0,0,0) (R6); D host [3][nao][nao]. */
+/* Position-operator matrices D^k_{mu nu} = <mu| r_k |nu> about the coordinate origin (0,0,0); D host [3][nao][nao].
+ * (A handle shifts its own copies to the electronic centroid of the ground state, R6.) */
 int rttda_dipole_ao(const rttda_basis_t* basis, int32_t nao, double* D);
 
 /* ---- handle -------------------------------------------------------------------------------------- */
