@@ -352,7 +352,7 @@ def run_b200(args):
     peak = R.rttda_fp64_peak(1.0, st)
     # DRAM bytes of one ERI pass from the committed ncu launch list of this same command (profiles/README.md)
     traffic = None
-    tpath = os.path.join(ROOT, "profiles", "r1_traffic_per_pass.json")
+    tpath = os.path.join(ROOT, "profiles", "r1_traffic_per_pass.txt")
     if k == 4 and nvec == 6 and os.path.exists(tpath):
         with open(tpath) as f:
             tj = json.load(f)
@@ -382,7 +382,7 @@ def run_b200(args):
                "jk_ms_per_pass": jk_avg_ms, "jk_share_of_step": jk_ms / (sum(ms) if sum(ms) else 1.0),
                "roofline": {"bound": "alu", "kernel": "eval_kernel<*> + digest_j_kernel<*> + digest_b_kernel<*> (all launches of one ERI pass)",
                             "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
-                            "traffic": traffic, "traffic_source": "profiles/r1_traffic_per_pass.json (ncu dram__bytes_read+write "
+                            "traffic": traffic, "traffic_source": "profiles/r1_traffic_per_pass.txt (ncu dram__bytes_read+write "
                             "summed over the launches of one ERI pass, config 4, nvec 6)" if traffic else None,
                             "peak_source": "measured live: rttda_fp64_peak DFMA chain, 1 s "
                             "(MEASURED_PEAKS.json has no FP64 entry; nominal %.1f)" % FP64_NOMINAL_TFLOPS,
