@@ -488,3 +488,77 @@ def test_propagate_config4_indirect_checks():
           % (ratio, dtau, float(np.max(np.abs(n1 - 1.0)))))
     assert 10.0 < ratio < 24.0
     assert dtau < 1e-9
+
+
+@pytest.mark.parametrize("seed", range(24))
+def test_sigma_random_small_molecules_and_degenerate_shapes(seed):
+    """Seeded random small systems covering the shapes the fixed configs do not: s-only and p-only bases, a single
+    occupied or virtual orbital, coincident centres (shell pairs with identical centres), loose screening that cuts
+    many quartets, one to four centres.  sigma and Fock matrices against the oracle's dense tensor."""
+    import torch
+    import paper_2601_16949_b200 as R
+    from workloads import Basis
+    from workloads.molecules import orthonormalizer
+    from oracle.integrals import OracleBasis
+    from oracle import tda
+    rng = np.random.default_rng(7000 + seed)
+    ncen = int(rng.integers(1, 5))
+    centers = rng.uniform(0.0, 4.0, size=(ncen, 3))
+    if seed % 4 == 3 and ncen > 1:
+        centers[1] = centers[0]                                        # two centres on top of each other
+    kinds = ["s", "p", "sp"][seed % 3]
+    sh_center, sh_l, sh_nprim, exps, coefs = [], [], [], [], []
+    for c in range(ncen):
+        shells = {"s": [(0, 3), (0, 1)], "p": [(1, 1), (1, 3)], "sp": [(0, 3), (1, 3), (0, 1), (1, 1)]}[kinds]
+        for l, npr in shells[: int(rng.integers(1, len(shells) + 1))]:
+            sh_center.append(c); sh_l.append(l); sh_nprim.append(npr)
+            exps.extend(np.exp(rng.uniform(np.log(0.15), np.log(8.0), size=npr)).tolist())
+            coefs.extend(rng.uniform(0.2, 1.0, size=npr).tolist())
+    sh_nprim = np.asarray(sh_nprim, dtype=np.int32)
+    basis = Basis(np.ascontiguousarray(centers), np.asarray(sh_center, dtype=np.int32), np.asarray(sh_l, dtype=np.int32),
+                  sh_nprim, np.concatenate([[0], np.cumsum(sh_nprim)[:-1]]).astype(np.int32),
+                  np.asarray(exps), np.asarray(coefs))
+    N = basis.nao
+    if N < 2:
+        pytest.skip("needs at least one occupied and one virtual orbital")
+    ob = OracleBasis(basis)
+    S = ob.overlap()
+    X12, cond = orthonormalizer(S)
+    if cond > 1e8:
+        pytest.skip("near-singular overlap (coincident identical shells)")
+    Q, Rq = np.linalg.qr(rng.standard_normal((N, N)))
+    C = X12 @ (Q * np.sign(np.diag(Rq)))
+    nocc = 1 if seed % 2 == 0 else max(1, N // 3)
+    nocc = min(nocc, N - 1)
+    nvirt = N - nocc
+    if seed == 5:
+        nocc, nvirt = N - 1, 1
+    C_o, C_v = np.ascontiguousarray(C[:, :nocc]), np.ascontiguousarray(C[:, nocc:])
+    eps = np.concatenate([np.sort(rng.uniform(-1.0, -0.3, nocc)), np.sort(rng.uniform(0.05, 2.0, nvirt))])
+    eri = ob.eri_tensor()
+    A = tda.build_A(eri, C_o, C_v, eps, 1.0)
+    dev = torch.device("cuda:0")
+    # The reference here is the oracle's DENSE A, built from four factors of C = S^-1/2 Q: with an ill-conditioned S
+    # (coincident centres) its own rounding error, amplified like the loss of orthonormality of C, sets the floor
+    # (the AO-level Fock check below has no such factor and stays at 1e-12)
+    orth = float(np.max(np.abs(C.T @ S @ C - np.eye(N))))
+    floor = max(1e-12, 3e3 * orth)
+    for tau, tol in ((0.0, floor), (1e-6, 5e-5 + floor)):
+        h = R.Rttda(basis, torch.from_numpy(C_o).to(dev), torch.from_numpy(C_v).to(dev), eps, 1.0, tau)
+        for nvec in (1, 6):
+            X = rng.standard_normal((nvec, nocc * nvirt))
+            Xd = torch.from_numpy(X).to(dev)
+            out = torch.empty_like(Xd)
+            h.rttda_sigma(Xd, out)
+            torch.cuda.synchronize()
+            ref = tda.sigma_dense(A, X)
+            assert rel_inf(out.cpu().numpy(), ref) < tol
+        if tau == 0.0:
+            T = rng.standard_normal((2, N, N))
+            Td = torch.from_numpy(T).to(dev)
+            F = torch.empty_like(Td)
+            h.rttda_fock(Td, F)
+            torch.cuda.synchronize()
+            Fref = 2 * np.einsum("mnls,vls->vmn", eri, T) - np.einsum("mnls,vns->vml", eri, T)
+            assert rel_inf(F.cpu().numpy(), Fref) < 1e-12          # AO level: no conditioning involved
+        h.close()
