@@ -20,70 +20,79 @@ __host__ __device__ constexpr int hidx_plus(int t, int u, int v, int axis)
     return axis == 0 ? hidx(t + 1, u, v) : (axis == 1 ? hidx(t, u + 1, v) : hidx(t, u, v + 1));
 }
 
-// ---- Boys function F_0..F_L(T) -------------------------------------------------------------------------
-// T < 48: nearest grid point T0 = j/8; one 80-byte table row {h_0..h_7, e^-T0, pad}, h_k = F_{L+k}(T0)/k!, so
-//   that F_L(T) = sum_k h_k (T0-T)^k (dF_n/dT = -F_{n+1}) is a 7-FMA Horner chain; then downward recursion
-//   F_{n-1} = (2T F_n + e^-T)/(2n-1) with e^-T = e^-T0 e^(T0-T) (degree-8 Taylor, |T0-T| <= 1/16).
+// ---- Boys function F_0..F_L(T), near field ------------------------------------------------------------
+// T < 48 (plus rounding slack of the caller's test): nearest grid point T0 = j/8; one 80-byte table row
+//   {h_0..h_7, e^-T0, pad}, h_k = F_{L+k}(T0)/k!, so that F_L(T) = sum_k h_k (T0-T)^k (dF_n/dT = -F_{n+1}) is a
+//   7-FMA Horner chain; then downward recursion F_{n-1} = (2T F_n + e^-T)/(2n-1) with e^-T = e^-T0 e^(T0-T)
+//   (degree-8 Taylor, |T0-T| <= 1/16).
 //   The row is a shared-memory gather; in the workloads of DESIGN.md only ~1 primitive quartet in 8 takes this
 //   branch (few active lanes), so its cost is its instruction count, not its shared-memory traffic.
-// T >= 48: F_0 = sqrt(pi/T)/2, F_{n+1} = (2n+1) F_n / (2T) (the e^-T term is < 1e-20).
+// The far field (T >= 48, e^-T < 1e-20) never forms F_n: see hermite_R.
 template <int L>
-__device__ __forceinline__ void boys(double T, const double2* __restrict__ tab, double (&F)[L + 1])
+__device__ __forceinline__ void boys_near(double T, const double2* __restrict__ tab, double (&F)[L + 1])
 {
-    if (T < BOYS_TMAX) {
-        constexpr double MAGIC = 6755399441055744.0;          // 1.5 * 2^52: rounds to nearest integer
-        const double t = fma(T, 8.0, MAGIC);
-        const int j = __double2loint(t);
-        const double dx = fma(t - MAGIC, 0.125, -T);          // T0 - T, |dx| <= 1/16
-        const double2* row = tab + j * (BOYS_ROW / 2);
-        const double2 h01 = row[0], h23 = row[1], h45 = row[2], h67 = row[3];
-        double f = h67.y;
-        f = fma(f, dx, h67.x);
-        f = fma(f, dx, h45.y);
-        f = fma(f, dx, h45.x);
-        f = fma(f, dx, h23.y);
-        f = fma(f, dx, h23.x);
-        f = fma(f, dx, h01.y);
-        f = fma(f, dx, h01.x);
-        F[L] = f;
-        if (L > 0) {
-            const double e0 = row[4].x;
-            double e = 1.0 / 40320.0;
-            e = fma(e, dx, 1.0 / 5040.0);
-            e = fma(e, dx, 1.0 / 720.0);
-            e = fma(e, dx, 1.0 / 120.0);
-            e = fma(e, dx, 1.0 / 24.0);
-            e = fma(e, dx, 1.0 / 6.0);
-            e = fma(e, dx, 0.5);
-            e = fma(e, dx, 1.0);
-            e = fma(e, dx, 1.0);
-            e *= e0;
-            const double t2 = 2.0 * T;
+    constexpr double MAGIC = 6755399441055744.0;          // 1.5 * 2^52: rounds to nearest integer
+    const double t = fma(T, 8.0, MAGIC);
+    const int j = __double2loint(t);
+    const double dx = fma(t - MAGIC, 0.125, -T);          // T0 - T, |dx| <= 1/16
+    const double2* row = tab + j * (BOYS_ROW / 2);
+    const double2 h01 = row[0], h23 = row[1], h45 = row[2], h67 = row[3];
+    double f = h67.y;
+    f = fma(f, dx, h67.x);
+    f = fma(f, dx, h45.y);
+    f = fma(f, dx, h45.x);
+    f = fma(f, dx, h23.y);
+    f = fma(f, dx, h23.x);
+    f = fma(f, dx, h01.y);
+    f = fma(f, dx, h01.x);
+    F[L] = f;
+    if (L > 0) {
+        const double e0 = row[4].x;
+        double e = 1.0 / 40320.0;
+        e = fma(e, dx, 1.0 / 5040.0);
+        e = fma(e, dx, 1.0 / 720.0);
+        e = fma(e, dx, 1.0 / 120.0);
+        e = fma(e, dx, 1.0 / 24.0);
+        e = fma(e, dx, 1.0 / 6.0);
+        e = fma(e, dx, 0.5);
+        e = fma(e, dx, 1.0);
+        e = fma(e, dx, 1.0);
+        e *= e0;
+        const double t2 = 2.0 * T;
 #pragma unroll
-            for (int n = L; n >= 1; --n) F[n - 1] = fma(t2, F[n], e) * (1.0 / (2 * n - 1));
-        }
-    } else {
-        const double rs = rsqrt(T);
-        F[0] = 0.88622692545275801365 * rs;                  // sqrt(pi)/2
-        const double h = 0.5 * rs * rs;
-#pragma unroll
-        for (int n = 0; n < L; ++n) F[n + 1] = (2 * n + 1) * h * F[n];
+        for (int n = L; n >= 1; --n) F[n - 1] = fma(t2, F[n], e) * (1.0 / (2 * n - 1));
     }
 }
 
-// ---- Hermite Coulomb integrals R^0_{tuv}, |tuv| <= L, scaled by pref -----------------------------------
+// ---- Hermite Coulomb integrals R^0_{tuv}, |tuv| <= L, times cc / sqrt(p+q) ---------------------------------
+// alpha = pq/(p+q), T = alpha R^2, r[n][0] = cc (p+q)^-1/2 (-2 alpha)^n F_n(T).
+// Far field (T >= 48, tested as pq R^2 >= 48 (p+q) without a division): F_0 = sqrt(pi/T)/2 and
+// F_{n+1} = (2n+1) F_n / 2T give r[0][0] = cc sqrt(pi)/2 (pq R^2)^-1/2 and r[n+1][0] = -(2n+1) r[n][0] / R^2:
+// alpha and (p+q)^-1/2 cancel, so the majority branch costs ONE rsqrt (1/R^2 = pq u^2) and no reciprocal.
 template <int L>
-__device__ __forceinline__ void hermite_R(double pref, double alpha, double X, double Y, double Z,
+__device__ __forceinline__ void hermite_R(double cc, double p, double q, double X, double Y, double Z,
                                           const double2* __restrict__ tab, double (&R0)[nherm(L)])
 {
-    double F[L + 1];
-    boys<L>(alpha * (X * X + Y * Y + Z * Z), tab, F);
     double r[L + 1][nherm(L)];
-    double s = pref;
+    const double R2 = X * X + Y * Y + Z * Z;
+    const double pq = p * q, s = p + q;
+    if (pq * R2 < BOYS_TMAX * s) {
+        const double rs = rsqrt(s);
+        const double alpha = pq * (rs * rs);
+        double F[L + 1];
+        boys_near<L>(alpha * R2, tab, F);
+        double sc = cc * rs;
 #pragma unroll
-    for (int n = 0; n <= L; ++n) {
-        r[n][0] = s * F[n];
-        s *= -2.0 * alpha;
+        for (int n = 0; n <= L; ++n) {
+            r[n][0] = sc * F[n];
+            sc *= -2.0 * alpha;
+        }
+    } else {
+        const double u = rsqrt(pq * R2);
+        r[0][0] = (0.88622692545275801365 * cc) * u;         // sqrt(pi)/2
+        const double w = -pq * (u * u);                      // -1/R^2
+#pragma unroll
+        for (int n = 0; n < L; ++n) r[n + 1][0] = ((2 * n + 1) * w) * r[n][0];
     }
 #pragma unroll
     for (int N = 1; N <= L; ++N)
@@ -154,12 +163,8 @@ __device__ __forceinline__ void eri_prim_accum(const PrimPair& br, const PrimPai
 {
     constexpr int L = LA + LB + LC + LD;
     constexpr int NA = 2 * LA + 1, NB = 2 * LB + 1, NC = 2 * LC + 1, ND = 2 * LD + 1;
-    const double s = br.p + kt.p;
-    const double rs = rsqrt(s);
-    const double alpha = br.p * kt.p * (rs * rs);
-    const double pref = br.c * kt.c * rs;
     double V0[1][nherm(L)];
-    hermite_R<L>(pref, alpha, br.Px - kt.Px, br.Py - kt.Py, br.Pz - kt.Pz, tab, V0[0]);
+    hermite_R<L>(br.c * kt.c, br.p, kt.p, br.Px - kt.Px, br.Py - kt.Py, br.Pz - kt.Pz, tab, V0[0]);
     double VD[ND][nherm(L - LD)];
     apply_p<ND, L - LD, 1>(V0, kt.XB, -kt.inv2p, VD);
     double VC[ND * NC][nherm(L - LD - LC)];
