@@ -165,6 +165,18 @@ int rttda_lanczos(rttda_handle_t h, int32_t m, const double* v0, double* alpha, 
 int rttda_populations(rttda_handle_t h, int32_t ntraj, const double* C, int32_t nstates, const double* Xs, double* P,
                       void* stream);
 
+/* Absorption spectrum from the time-correlation function (NEXT-2 of DESIGN.md): eq. 21 R(omega) ~ omega F[R(t)]
+ * with the recipe of P:212 (mirroring R(-t) = R(t)^*, Hann window over the 2n+1 mirrored points, `pad` zeros; the
+ * paper pads 50,000), and the angular average of eq. 23 over the ntraj trajectories.
+ *   log  DEVICE [n][ntraj][3], the log rttda_propagate wrote (entries 1, 2 of a row = Re, Im R((k+1) dt)); may be
+ *        NULL if n == 0.  R0 HOST [ntraj][2] = R(0) of each trajectory (1 + 0i for a normalised start).
+ *   omega DEVICE [nout], intensity DEVICE [ntraj + 1][nout] with nout = (2n + 1 + pad) / 2 (anything else is
+ *        RTTDA_EINVAL): omega[i] = 2 pi (i+1) / ((2n+1+pad) dt); row t < ntraj = omega |F_t|, row ntraj = their mean.
+ *   No normalisation to the highest peak (P:214 does that for plotting).  The transform is a direct DFT evaluated on
+ *   the device.  Needs no handle.  Enqueued on `stream`. */
+int rttda_spectrum(int32_t ntraj, int32_t n, const double* R0, const double* log, double dt, int32_t pad, int32_t nout,
+                   double* omega, double* intensity, void* stream);
+
 /* Options.  RTTDA_OPT_INCORE (value != 0 switches it on; default off): keep the contracted integrals of all
  * segments resident in HBM (RTTDA_INFO_ERI_ALL_BYTES: 61 GB for the 1280-AO molecule at tau = 1e-12) so that, after
  * the first ERI pass of the handle, later passes skip the evaluation and only digest.  This is NOT the paper's direct

@@ -21,7 +21,7 @@ OPT_INCORE = 1
 PULSE = dict(none=0, delta=1, cw=2, tl=3, chirp=4, sin2=5)
 EXPORTS = ["rttda_overlap", "rttda_dipole_ao", "rttda_create", "rttda_destroy", "rttda_sigma",
            "rttda_sigma_host", "rttda_fock", "rttda_propagate", "rttda_propagate_sso", "rttda_propagate_host",
-           "rttda_get_info", "rttda_set_option", "rttda_populations", "rttda_lanczos", "rttda_last_timings", "rttda_jk_time", "rttda_fp64_peak", "rttda_last_error",
+           "rttda_get_info", "rttda_set_option", "rttda_populations", "rttda_spectrum", "rttda_lanczos", "rttda_last_timings", "rttda_jk_time", "rttda_fp64_peak", "rttda_last_error",
            "rttda_version"]
 
 
@@ -128,6 +128,17 @@ def rttda_fp64_peak(seconds: float = 1.0, stream=None) -> float:
     out = ct.c_double(0.0)
     _check(lib().rttda_fp64_peak(ct.c_double(seconds), ct.byref(out), _stream(stream)), "rttda_fp64_peak")
     return out.value
+
+
+def rttda_spectrum(R0, log, dt: float, pad: int, omega, intensity, stream=None):
+    """eq. 21 / 23: log CUDA [n][ntraj][3] (rttda_propagate's log), R0 host [ntraj][2]; omega CUDA [nout],
+    intensity CUDA [ntraj + 1][nout], nout = (2n + 1 + pad) // 2."""
+    R0 = np.ascontiguousarray(R0, dtype=np.float64)
+    ntraj = int(R0.shape[0])
+    n = 0 if log is None else int(log.shape[0])
+    _check(lib().rttda_spectrum(ntraj, n, _dptr(R0), _dptr(log), ct.c_double(dt), int(pad), int(omega.shape[0]),
+                                _dptr(omega), _dptr(intensity), _stream(stream)), "rttda_spectrum")
+    return omega, intensity
 
 
 class Rttda:

@@ -213,6 +213,18 @@ int rttda_populations(rttda_handle_t hh, int32_t ntraj, const double* C, int32_t
     return populations_impl(h, ntraj, C, nstates, Xs, P, (cudaStream_t)stream);
 }
 
+int rttda_spectrum(int32_t ntraj, int32_t n, const double* R0, const double* log, double dt, int32_t pad, int32_t nout,
+                   double* omega, double* intensity, void* stream)
+{
+    RT_CHECK(ntraj >= 1 && n >= 0 && pad >= 0 && dt > 0.0, "rttda_spectrum: need ntraj >= 1, n >= 0, pad >= 0, dt > 0");
+    const long long npad = 2LL * n + 1 + pad;
+    RT_CHECK(npad < (1LL << 31), "rttda_spectrum: 2n + 1 + pad must be below 2^31");
+    RT_CHECK((long long)nout == npad / 2, "rttda_spectrum: nout must be (2n + 1 + pad) / 2");
+    if (nout == 0) return RTTDA_OK;                         // a single sample without padding has no frequency grid
+    RT_CHECK(R0 && omega && intensity && (log || n == 0), "rttda_spectrum: NULL pointer");
+    return spectrum_impl(ntraj, n, R0, log, dt, pad, nout, omega, intensity, (cudaStream_t)stream);
+}
+
 int rttda_set_option(rttda_handle_t hh, int32_t option, double value)
 {
     Handle* h = (Handle*)hh;

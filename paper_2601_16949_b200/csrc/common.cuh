@@ -204,6 +204,8 @@ int propagate_impl(Handle* h, int ntraj, double* C, const rttda_field_t* fields,
 int propagate_sso_impl(Handle* h, int ntraj, double* C, const rttda_field_t* fields, double t_start,
                        double dt, int nsteps, double* log, cudaStream_t st);
 int lanczos_impl(Handle* h, int m, const double* v0, double* alpha, double* beta, double* V, cudaStream_t st);
+int spectrum_impl(int ntraj, int n, const double* R0, const double* log, double dt, int pad, int nout, double* omega,
+                  double* inten, cudaStream_t st);
 int populations_impl(Handle* h, int ntraj, const double* y, int nstates, const double* Xs, double* P, cudaStream_t st);
 int sigma_impl(Handle* h, int nvec, const double* X, long long ldx, double* sigma, long long lds,
                cudaStream_t st);

@@ -62,7 +62,7 @@ __global__ void __launch_bounds__(JK_BLOCK) eval_kernel(EvalArgs g)
     constexpr int NI = (2 * LA + 1) * (2 * LB + 1) * (2 * LC + 1) * (2 * LD + 1);
     constexpr int L = LA + LB + LC + LD;
     // ket primitives live in registers when they are few doubles; otherwise they are re-read (L1 hits)
-    constexpr bool KET_IN_REGS = (KP == 1) || (L <= 3 && ((KP <= 3) || (LC + LD == 0)));
+    constexpr bool KET_IN_REGS = (KP == 1) || (L <= 3 && (KP <= 3 || (LC + LD == 0 && L <= 1)));
     __shared__ __align__(16) double2 s_boys[BOYS_NROW * (BOYS_ROW / 2)];
     __shared__ __align__(16) double s_rows[EVAL_MAX_ROWS * PRIM_STRIDE];
     __shared__ double s_Q[JK_BLOCK];

@@ -454,6 +454,91 @@ int populations_impl(Handle* h, int ntraj, const double* y, int nstates, const d
     return RTTDA_OK;
 }
 
+// ---------------------------------------------------------------------------------------------- spectrum
+// eq. 21 with the recipe of P:212: the correlation function of one trajectory, R(k dt) for k = 0..n, is
+// mirrored (R(-t) = R(t)^*), multiplied by the Hann window over its 2n+1 points, padded with `pad` zeros and Fourier
+// transformed; the spectrum is omega |F| on the grid omega_j = 2 pi j / (npad dt), j = 1..npad/2.  The transform is
+// a direct DFT (n is a few thousand steps: 1e8 phase factors): thread = one frequency, block = SPEC_TILE of them;
+// the windowed signal is built tile by tile in shared memory, the phase index (j m mod npad) is kept as an integer
+// so that sincospi sees an argument reduced exactly.
+constexpr int SPEC_TILE = 128;
+
+__global__ void __launch_bounds__(SPEC_TILE)
+spectrum_kernel(int ntraj, int n, const double* __restrict__ log, double r0re, double r0im, int traj0, double dt,
+                long long npad, int nout, double* __restrict__ omega, double* __restrict__ inten)
+{
+    __shared__ double2 s_x[SPEC_TILE];
+    const int traj = traj0 + blockIdx.y;
+    const long long M = 2LL * n + 1;
+    const int i = blockIdx.x * SPEC_TILE + threadIdx.x;
+    const long long j = (long long)i + 1;                      // frequency index; also the phase increment per sample
+    const double inv = 2.0 / (double)npad;
+    double re = 0.0, im = 0.0;
+    for (long long m0 = 0; m0 < M; m0 += SPEC_TILE) {
+        const long long m = m0 + threadIdx.x;
+        double2 x = make_double2(0.0, 0.0);
+        if (m < M) {
+            const long long k = m - n;                          // sample time k dt
+            const long long a = k < 0 ? -k : k;
+            double xr, xi;
+            if (a == 0) { xr = r0re; xi = r0im; }
+            else {
+                const double* e = log + ((a - 1) * ntraj + traj) * 3;
+                xr = e[1]; xi = e[2];
+            }
+            if (k < 0) xi = -xi;
+            const double w = (M > 1) ? 0.5 - 0.5 * cospi(2.0 * (double)m / (double)(M - 1)) : 1.0;
+            x = make_double2(w * xr, w * xi);
+        }
+        __syncthreads();
+        s_x[threadIdx.x] = x;
+        __syncthreads();
+        if (i < nout) {
+            const int cnt = (int)((M - m0 < SPEC_TILE) ? (M - m0) : SPEC_TILE);
+            long long r = (j * (m0 % npad)) % npad;             // j, m0 % npad < 2^31
+            for (int t = 0; t < cnt; ++t) {
+                double sn, cs;
+                sincospi((double)r * inv, &sn, &cs);            // exp(+2 pi i j m / npad): numpy's bin npad - j
+                const double2 v = s_x[t];
+                re = fma(v.x, cs, fma(-v.y, sn, re));
+                im = fma(v.x, sn, fma(v.y, cs, im));
+                r += j;
+                if (r >= npad) r -= npad;
+            }
+        }
+    }
+    if (i < nout) {
+        const double om = 6.283185307179586476925 * (double)j / ((double)npad * dt);
+        if (blockIdx.y == 0) omega[i] = om;
+        inten[(long long)traj * nout + i] = om * sqrt(re * re + im * im);
+    }
+}
+
+// eq. 23: mean of the ntraj spectra (x, y, z polarisation) into row ntraj
+__global__ void spectrum_mean_kernel(int ntraj, int nout, double* __restrict__ inten)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= nout) return;
+    double s = 0.0;
+    for (int t = 0; t < ntraj; ++t) s += inten[(long long)t * nout + i];
+    inten[(long long)ntraj * nout + i] = s / (double)ntraj;
+}
+
+int spectrum_impl(int ntraj, int n, const double* R0, const double* log, double dt, int pad, int nout, double* omega,
+                  double* inten, cudaStream_t st)
+{
+    const long long npad = 2LL * n + 1 + pad;
+    dim3 grid((nout + SPEC_TILE - 1) / SPEC_TILE, 1);
+    for (int t = 0; t < ntraj; ++t) {                           // R(0) of each trajectory is a kernel argument
+        spectrum_kernel<<<grid, SPEC_TILE, 0, st>>>(ntraj, n, log, R0[2 * t], R0[2 * t + 1], t, dt, npad, nout, omega,
+                                                    inten);
+        RT_CUDA(cudaGetLastError());
+    }
+    spectrum_mean_kernel<<<(nout + 255) / 256, 256, 0, st>>>(ntraj, nout, inten);
+    RT_CUDA(cudaGetLastError());
+    return RTTDA_OK;
+}
+
 // ---------------------------------------------------------------------------------------------- Lanczos
 // out[i] = sum_e V[i][e] w[e] for i < nv (one block per i)
 __global__ void __launch_bounds__(256)

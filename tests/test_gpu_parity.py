@@ -402,6 +402,105 @@ def test_populations_vs_oracle():
     assert P.cpu().numpy()[1, 0] < P.cpu().numpy()[0, 0] < 1.0          # the stronger field depletes the ground state more
 
 
+def _gpu_spectrum(R, dt, pad):
+    """R complex [ntraj][n+1] (R[:, 0] = R(0)) -> (omega, intensity[ntraj + 1]) through rttda_spectrum."""
+    import torch
+    from paper_2601_16949_b200 import binding
+    R = np.atleast_2d(R)
+    ntraj, n = R.shape[0], R.shape[1] - 1
+    dev = torch.device("cuda:0")
+    log = np.zeros((n, ntraj, 3))
+    log[:, :, 0] = 1.0
+    log[:, :, 1] = R[:, 1:].real.T
+    log[:, :, 2] = R[:, 1:].imag.T
+    R0 = np.stack([R[:, 0].real, R[:, 0].imag], axis=1)
+    nout = (2 * n + 1 + pad) // 2
+    om = torch.zeros(nout, dtype=torch.float64, device=dev)
+    inten = torch.zeros((ntraj + 1, nout), dtype=torch.float64, device=dev)
+    binding.rttda_spectrum(R0, torch.from_numpy(log).to(dev) if n else None, dt, pad, om, inten)
+    torch.cuda.synchronize()
+    return om.cpu().numpy(), inten.cpu().numpy()
+
+
+@pytest.mark.parametrize("n,pad,ntraj", [(0, 0, 1), (0, 7, 1), (1, 0, 1), (5, 2, 2), (130, 33, 3), (700, 5000, 3)])
+def test_spectrum_vs_oracle(n, pad, ntraj):
+    """eq. 21 / 23 with the recipe of P:212: the device DFT against the oracle's mirrored, Hann-windowed, zero-padded
+    FFT on synthetic correlation functions (sums of decaying oscillations plus noise); sizes span several tiles of
+    128 samples / frequencies with ragged tails, odd and even padded lengths, and the degenerate n = 0, 1."""
+    from oracle import tda
+    rng = np.random.default_rng(100 + n + pad)
+    dt = 0.2
+    t = np.arange(n + 1) * dt
+    R = np.zeros((ntraj, n + 1), dtype=complex)
+    for k in range(ntraj):
+        w = rng.uniform(0.1, 3.0, 6)
+        c = rng.uniform(0.0, 1.0, 6)
+        R[k] = (c[None, :] * np.exp(-1j * w[None, :] * t[:, None])).sum(1) * np.exp(-0.002 * t)
+        R[k] += 1e-3 * (rng.standard_normal(n + 1) + 1j * rng.standard_normal(n + 1))
+    om, inten = _gpu_spectrum(R, dt, pad)
+    assert om.shape[0] == (2 * n + 1 + pad) // 2
+    refs = []
+    for k in range(ntraj):
+        rom, rin = tda.spectrum(R[k], dt, pad=pad)
+        assert rom.shape == om.shape
+        if om.size:
+            assert np.max(np.abs(om - rom) / rom) < 1e-14
+            scale = max(np.max(rin), 1e-300)
+            assert np.max(np.abs(inten[k] - rin)) / scale < 1e-12
+        refs.append(rin)
+    if om.size:
+        mean = np.mean(refs, axis=0)
+        assert np.max(np.abs(inten[ntraj] - mean)) <= 1e-12 * max(np.max(mean), 1e-300)
+
+
+def test_spectrum_of_propagated_trajectory_peaks_at_eigenvalues():
+    """delta kick on config 1, rttda_propagate's own log fed to rttda_spectrum: parity with the oracle's spectrum of
+    the same log, and the strongest peak sits at an eigenvalue of A within the resolution 2 pi / T."""
+    import torch
+    from oracle import tda
+    from paper_2601_16949_b200 import binding
+    ctx = setup_config(1, dense=True)
+    h, A = ctx["h"], ctx["A"]
+    n = A.shape[0]
+    dt, nsteps, pad = 0.1, 1500, 4000
+    y = torch.from_numpy(_state0(1, n)).to(ctx["dev"])
+    log = torch.zeros((nsteps, 1, 3), dtype=torch.float64, device=ctx["dev"])
+    h.rttda_propagate(y, [{"type": "delta", "E0": 1e-2, "dir": (0.0, 0.0, 1.0)}], 0.0, dt, nsteps, log)
+    # the ground state (eigenvalue 0 of A_ext) contributes the constant |c_0|^2 to R(t): remove that DC line so
+    # that its window leakage does not bury the excited-state peaks
+    yh = y.cpu().numpy()
+    p0 = float(yh[0, 0, 0] ** 2 + yh[0, 1, 0] ** 2)
+    log[:, 0, 1] -= p0
+    R0 = np.array([[float(np.sum(yh[0] ** 2)) - p0, 0.0]])
+    nout = (2 * nsteps + 1 + pad) // 2
+    om = torch.zeros(nout, dtype=torch.float64, device=ctx["dev"])
+    inten = torch.zeros((2, nout), dtype=torch.float64, device=ctx["dev"])
+    binding.rttda_spectrum(R0, log, dt, pad, om, inten)
+    torch.cuda.synchronize()
+    lh = log.cpu().numpy()
+    R = np.concatenate([[R0[0, 0] + 0.0j], lh[:, 0, 1] + 1j * lh[:, 0, 2]])
+    rom, rin = tda.spectrum(R, dt, pad=pad)
+    ih = inten.cpu().numpy()
+    assert np.max(np.abs(ih[0] - rin)) < 1e-12 * np.max(rin)
+    assert np.array_equal(ih[0], ih[1])                       # mean of one trajectory
+    w = np.linalg.eigvalsh(A)
+    peak = om.cpu().numpy()[np.argmax(ih[0])]
+    assert np.min(np.abs(w - peak)) < 2 * np.pi / (nsteps * dt)
+
+
+def test_spectrum_rejects_bad_arguments():
+    import torch
+    from paper_2601_16949_b200 import binding
+    dev = torch.device("cuda:0")
+    om = torch.zeros(4, dtype=torch.float64, device=dev)
+    inten = torch.zeros((2, 4), dtype=torch.float64, device=dev)
+    log = torch.zeros((3, 1, 3), dtype=torch.float64, device=dev)
+    with pytest.raises(binding.RttdaError):
+        binding.rttda_spectrum(np.array([[1.0, 0.0]]), log, 0.1, 0, om, inten)       # nout must be 3
+    with pytest.raises(binding.RttdaError):
+        binding.rttda_spectrum(np.array([[1.0, 0.0]]), log, -0.1, 1, om, inten)      # dt <= 0
+
+
 def test_lanczos_vs_oracle_and_dense_eigenvalues():
     """NEXT-3: Lanczos on A through the GPU sigma builds: coefficients against the oracle's Lanczos on dense A (same
     start vector), Ritz values against eigh(A)."""
