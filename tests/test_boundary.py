@@ -70,6 +70,26 @@ def test_no_cpu_fallback(R):
     assert rc == -3 and b"no CUDA device" in R.lib().rttda_last_error()
 
 
+def test_spectrum_argument_errors_and_no_fallback_without_gpu(R):
+    """rttda_spectrum: argument errors are reported before any device work; with valid arguments and no CUDA device
+    the call fails (no host DFT behind it)."""
+    import torch
+    L = R.lib()
+    R0 = np.array([[1.0, 0.0]])
+    buf = np.zeros((3, 1, 3))
+    om, inten = np.zeros(3), np.zeros((2, 3))
+    args = lambda n, dt, pad, nout: (1, n, ct.c_void_p(R0.ctypes.data), ct.c_void_p(buf.ctypes.data), ct.c_double(dt),
+                                     pad, nout, ct.c_void_p(om.ctypes.data), ct.c_void_p(inten.ctypes.data),
+                                     ct.c_void_p(0))
+    assert L.rttda_spectrum(*args(3, 0.1, 0, 4)) == -1 and b"nout" in L.rttda_last_error()
+    assert L.rttda_spectrum(*args(3, 0.0, 0, 3)) == -1
+    assert L.rttda_spectrum(*args(-1, 0.1, 0, 0)) == -1
+    assert L.rttda_spectrum(*args(0, 0.1, 0, 0)) == 0            # one sample, no padding: empty frequency grid
+    if not torch.cuda.is_available():
+        assert L.rttda_spectrum(*args(3, 0.1, 0, 3)) != 0
+        assert np.all(om == 0.0) and np.all(inten == 0.0)
+
+
 def test_product_does_not_import_oracle():
     pkg = os.path.join(ROOT, "paper_2601_16949_b200")
     for dp, _, fs in os.walk(pkg):
