@@ -132,8 +132,8 @@ constexpr int EVAL_MAX_ROWS = 144;     // bra primitive rows staged per evaluati
 
 // Boys grid: T0 = j / 8, j = 0..BOYS_NROW-1; BOYS_ROW doubles per row (eri_eval.cuh)
 constexpr int BOYS_ROW = 10;
-constexpr double BOYS_TMAX = 48.0;
-constexpr int BOYS_NROW = 385 + 1;
+constexpr double BOYS_TMAX = 36.0;
+constexpr int BOYS_NROW = 289 + 1;
 void boys_table_host(int L, std::vector<double>& tab);
 
 // ---------------------------------------------------------------------------------------------

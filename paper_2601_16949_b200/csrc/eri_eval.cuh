@@ -21,13 +21,13 @@ __host__ __device__ constexpr int hidx_plus(int t, int u, int v, int axis)
 }
 
 // ---- Boys function F_0..F_L(T), near field ------------------------------------------------------------
-// T < 48 (plus rounding slack of the caller's test): nearest grid point T0 = j/8; one 80-byte table row
+// T < BOYS_TMAX = 36 (plus rounding slack of the caller's test): nearest grid point T0 = j/8; one 80-byte table row
 //   {h_0..h_7, e^-T0, pad}, h_k = F_{L+k}(T0)/k!, so that F_L(T) = sum_k h_k (T0-T)^k (dF_n/dT = -F_{n+1}) is a
 //   7-FMA Horner chain; then downward recursion F_{n-1} = (2T F_n + e^-T)/(2n-1) with e^-T = e^-T0 e^(T0-T)
 //   (degree-8 Taylor, |T0-T| <= 1/16).
 //   The row is a shared-memory gather; in the workloads of DESIGN.md only ~1 primitive quartet in 8 takes this
 //   branch (few active lanes), so its cost is its instruction count, not its shared-memory traffic.
-// The far field (T >= 48, e^-T < 1e-20) never forms F_n: see hermite_R.
+// The far field (T >= 36) never forms F_n: see hermite_R.
 template <int L>
 __device__ __forceinline__ void boys_near(double T, const double2* __restrict__ tab, double (&F)[L + 1])
 {
@@ -66,7 +66,9 @@ __device__ __forceinline__ void boys_near(double T, const double2* __restrict__ 
 
 // ---- Hermite Coulomb integrals R^0_{tuv}, |tuv| <= L, times cc / sqrt(p+q) ---------------------------------
 // alpha = pq/(p+q), T = alpha R^2, r[n][0] = cc (p+q)^-1/2 (-2 alpha)^n F_n(T).
-// Far field (T >= 48, tested as pq R^2 >= 48 (p+q) without a division): F_0 = sqrt(pi/T)/2 and
+// Far field (T >= 36, tested as pq R^2 >= 36 (p+q) without a division; erfc(6) = 2.2e-17 and every dropped term
+// e^-T/2T of the upward recursion is below 4e-18 of the (ss|ss)-like magnitude, since (2 alpha)^n / ((2p)^k (2q)^m)
+// <= 1 for n = k + m): F_0 = sqrt(pi/T)/2 and
 // F_{n+1} = (2n+1) F_n / 2T give r[0][0] = cc sqrt(pi)/2 (pq R^2)^-1/2 and r[n+1][0] = -(2n+1) r[n][0] / R^2:
 // alpha and (p+q)^-1/2 cancel, so the majority branch costs ONE rsqrt (1/R^2 = pq u^2) and no reciprocal.
 template <int L>

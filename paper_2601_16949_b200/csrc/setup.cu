@@ -12,7 +12,7 @@
 namespace rttda {
 
 // ---------------------------------------------------------------------------------------------- Boys table
-// Rows {F_{L+k}(T0)/k!, k = 0..7; exp(-T0); 0} at T0 = j/8 (eri_eval.cuh boys_near<L>): series for F_{L+7} (T0 <= 48),
+// Rows {F_{L+k}(T0)/k!, k = 0..7; exp(-T0); 0} at T0 = j/8 (eri_eval.cuh boys_near<L>): series for F_{L+7} (T0 <= BOYS_TMAX + 1/8),
 // downward recursion for the lower orders, all in long double.
 void boys_table_host(int L, std::vector<double>& tab)
 {
