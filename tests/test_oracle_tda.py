@@ -395,3 +395,24 @@ def test_delta_kick_correlation_closed_form_and_spectrum(tiny):
     peaks = sorted(peaks, key=lambda i: -inten[i])[:6]
     for I in strongest[:2]:
         assert min(abs(om[p] - w[I]) for p in peaks) < res
+
+
+def test_spectrum_pure_tone_closed_form():
+    """eq. 21 with the recipe of P:212 on R(t) = exp(-i w t), w on the padded frequency grid: the mirrored series
+    (R(-t) = R(t)^*) is the same pure tone on t = -n dt .. n dt, so the transform at w is the plain sum of the Hann
+    window, sum_m (1 - cos(2 pi m / (M - 1))) / 2 = (M - 1) / 2 with M = 2n + 1, and the spectrum there is w (M - 1) / 2.
+    A mirror without the conjugate, a transform with the opposite sign, a window over the padded length or a
+    padding before the window all change this value."""
+    n, pad, dt, j = 50, 99, 0.2, 20
+    npad = 2 * n + 1 + pad                                       # 200
+    w = 2.0 * np.pi * j / (npad * dt)
+    R = np.exp(-1j * w * dt * np.arange(n + 1))
+    om, inten = tda.spectrum(R, dt, pad=pad)
+    assert om.shape[0] == npad // 2
+    assert abs(om[j - 1] - w) < 1e-14 * w
+    assert int(np.argmax(inten)) == j - 1
+    assert abs(inten[j - 1] - w * n) < 1e-12 * w * n
+    # two bins away in units of the UNPADDED resolution the Hann transform has its first zero: 2 * npad / (M - 1)
+    # is not an integer here, so instead check the mirror symmetry of the line shape about the peak
+    assert np.allclose(inten[j - 1 - 5:j - 1] / om[j - 1 - 5:j - 1],
+                       (inten[j:j + 5] / om[j:j + 5])[::-1], rtol=1e-9, atol=1e-12)
