@@ -425,6 +425,81 @@ void oracle_jk(BASIS_ARGS, int nao, int nvec, const double *T, double tau, const
                       tau, Qs, 1, 0, J, K, nquartets, nprimq);
 }
 
+/* Extended-precision route of oracle_jk ("accumulate J/K sums ... in long double"): the same loop
+ * over unique screened quartets and the same 8-image rule, but the densities arrive as long double, every product
+ * I * T and every partial sum (per thread and across threads) is x87 80-bit long double, and J, K are returned as
+ * long double.  Only the integral values themselves are FP64 (shell_quartet).  Layout: T, J, K are [nao][nao][nvec]
+ * (vector index fastest) so that one integral meets the nvec densities at consecutive addresses.  Used for the
+ * stored samples at 1280 AOs and by the test that bounds the noise floor of the FP64 route above. */
+void oracle_jk_ld(BASIS_ARGS, int nao, int nvec, const long double *T, double tau, const double *Qs,
+                  long double *J, long double *K, int64_t *nquartets, int64_t *nprimq)
+{
+    basis_t B = BASIS_MK;
+    size_t nn = (size_t)nao * nao;
+    for (size_t i = 0; i < nn * nvec; ++i) J[i] = K[i] = 0.0L;
+    int64_t nq_tot = 0, npq_tot = 0;
+    int npair = nshells * (nshells + 1) / 2;
+    #pragma omp parallel
+    {
+        long double *Jl = calloc(nn * nvec, sizeof(long double)), *Kl = calloc(nn * nvec, sizeof(long double));
+        int64_t nq = 0, npq = 0;
+        #pragma omp for schedule(dynamic, 4)
+        for (int ab = npair - 1; ab >= 0; --ab) {
+            int sa = (int)((sqrt(8.0 * ab + 1.0) - 1.0) / 2.0);
+            while ((sa + 1) * (sa + 2) / 2 <= ab) ++sa;
+            while (sa * (sa + 1) / 2 > ab) --sa;
+            int sb = ab - sa * (sa + 1) / 2;
+            double qab = Qs[(size_t)sa * nshells + sb];
+            for (int cd = 0; cd <= ab; ++cd) {
+                int sc = (int)((sqrt(8.0 * cd + 1.0) - 1.0) / 2.0);
+                while ((sc + 1) * (sc + 2) / 2 <= cd) ++sc;
+                while (sc * (sc + 1) / 2 > cd) --sc;
+                int sd = cd - sc * (sc + 1) / 2;
+                if (tau > 0.0 && qab * Qs[(size_t)sc * nshells + sd] < tau) continue;
+                ++nq;
+                npq += (int64_t)sh_nprim[sa] * sh_nprim[sb] * sh_nprim[sc] * sh_nprim[sd];
+                double blk[81];
+                shell_quartet(&B, sa, sb, sc, sd, blk);
+                long double w = 1.0L;
+                if (sa == sb) w *= 0.5L;
+                if (sc == sd) w *= 0.5L;
+                if (ab == cd) w *= 0.5L;
+                int n0 = 2 * sh_l[sa] + 1, n1 = 2 * sh_l[sb] + 1, n2 = 2 * sh_l[sc] + 1,
+                    n3 = 2 * sh_l[sd] + 1, idx = 0;
+                for (int ca = 0; ca < n0; ++ca)
+                for (int cb = 0; cb < n1; ++cb)
+                for (int cc = 0; cc < n2; ++cc)
+                for (int cdd = 0; cdd < n3; ++cdd, ++idx) {
+                    long double I = w * (long double)blk[idx];
+                    size_t m = ao_off[sa] + ca, n = ao_off[sb] + cb, l = ao_off[sc] + cc,
+                           s = ao_off[sd] + cdd;
+                    size_t im[8][4] = {{m, n, l, s}, {n, m, l, s}, {m, n, s, l}, {n, m, s, l},
+                                       {l, s, m, n}, {s, l, m, n}, {l, s, n, m}, {s, l, n, m}};
+                    for (int g = 0; g < 8; ++g) {
+                        size_t i0 = im[g][0], i1 = im[g][1], i2 = im[g][2], i3 = im[g][3];
+                        long double *Jr = Jl + (i0 * nao + i1) * nvec, *Kr = Kl + (i0 * nao + i2) * nvec;
+                        const long double *Tj = T + (i2 * nao + i3) * nvec, *Tk = T + (i1 * nao + i3) * nvec;
+                        for (int v = 0; v < nvec; ++v) {
+                            Jr[v] += I * Tj[v];
+                            Kr[v] += I * Tk[v];
+                        }
+                    }
+                }
+            }
+        }
+        #pragma omp critical
+        {
+            for (size_t i = 0; i < nn * nvec; ++i) { J[i] += Jl[i]; K[i] += Kl[i]; }
+            nq_tot += nq;
+            npq_tot += npq;
+        }
+        free(Jl);
+        free(Kl);
+    }
+    if (nquartets) *nquartets = nq_tot;
+    if (nprimq) *nprimq = npq_tot;
+}
+
 /* Sampled elements of J[T] and K[T] straight from the definitions (no symmetry, no screening):
  * for each sample s with AO pair (mu, nu): J = sum_{lam sig} (mu nu|lam sig) T[lam][sig],
  * K = sum_{lam sig} (mu lam|nu sig) T[lam][sig].  Jout, Kout: [nsamp][nvec]. */

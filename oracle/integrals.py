@@ -135,6 +135,28 @@ class OracleBasis:
                         K.ctypes.data_as(_dp), ct.byref(nq), ct.byref(npq))
         return J, K, nq.value, npq.value
 
+    def jk_ld(self, T: np.ndarray, tau: float = 0.0, Q: np.ndarray | None = None):
+        """Extended-precision J[T], K[T] (oracle_jk_ld): T [nvec][N][N] as np.longdouble (x87 80-bit); every product
+        and sum past the FP64 integral values is long double.  Returns J, K as np.longdouble [nvec][N][N] + counts."""
+        assert np.finfo(np.longdouble).nmant >= 63, "needs x87 80-bit long double"
+        T = np.asarray(T, dtype=np.longdouble)
+        if T.ndim == 2:
+            T = T[None]
+        nvec, N = T.shape[0], self.nao
+        Tt = np.ascontiguousarray(np.transpose(T, (1, 2, 0)))          # [N][N][nvec]
+        if Q is None:
+            Q = self.schwarz()
+        Q = np.ascontiguousarray(Q)
+        J = np.zeros_like(Tt)
+        K = np.zeros_like(Tt)
+        nq = ct.c_int64(0)
+        npq = ct.c_int64(0)
+        lib().oracle_jk_ld(*self._args(), ct.c_int(N), ct.c_int(nvec), ct.c_void_p(Tt.ctypes.data),
+                           ct.c_double(tau), Q.ctypes.data_as(_dp), ct.c_void_p(J.ctypes.data),
+                           ct.c_void_p(K.ctypes.data), ct.byref(nq), ct.byref(npq))
+        return (np.ascontiguousarray(np.transpose(J, (2, 0, 1))), np.ascontiguousarray(np.transpose(K, (2, 0, 1))),
+                nq.value, npq.value)
+
     def jk_strided(self, T: np.ndarray, tau: float, Q: np.ndarray, stride: int, phase: int = 0):
         """Bounded SAMPLE of jk(): only bra pairs ab with ab % stride == phase.  Returns the partial
         J, K and the shell / primitive quartet counts of the sample (for timing extrapolation only)."""

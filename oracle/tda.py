@@ -74,6 +74,22 @@ def sigma_matrix_free(ob, X, C_o, C_v, eps, cx=1.0, tau=0.0, Q=None):
     return sigma_from_jk(X, J, K, C_o, C_v, eps, cx), nq, npq
 
 
+def sigma_matrix_free_ld(ob, X, C_o, C_v, eps, cx=1.0, tau=0.0, Q=None):
+    """The same matrix-free identity with every step past the FP64 integral values in x87 long double (SURVEY 8(c):
+    long-double J/K sums and MO transforms): T = C_o X C_v^T, J/K by `ob.jk_ld`, sigma = d_eps o X + C_o^T (2J - c_x K) C_v,
+    all as np.longdouble matrix products.  Returns (sigma as np.longdouble, n_shell_quartets, n_prim_quartets); the
+    difference to `sigma_matrix_free` is the rounding-noise floor of the FP64 route."""
+    ld = np.longdouble
+    no, nv = C_o.shape[1], C_v.shape[1]
+    Co, Cv, Xl = C_o.astype(ld), C_v.astype(ld), np.asarray(X, dtype=ld).reshape(-1, no, nv)
+    T = np.stack([Co @ x @ Cv.T for x in Xl])
+    J, K, nq, npq = ob.jk_ld(T, tau=tau, Q=Q)
+    de = (eps[no:].astype(ld)[None, :] - eps[:no].astype(ld)[:, None]).reshape(-1)
+    F = ld(2.0) * J - ld(cx) * K
+    S = np.stack([(Co.T @ f @ Cv).reshape(-1) for f in F])
+    return de[None, :] * Xl.reshape(-1, no * nv) + S, nq, npq
+
+
 # ---------------------------------------------------------------- dipole operator in the CSF basis
 def mo_dipoles(D_ao, C_o, C_v, d):
     """D_d = sum_k d_k D^k in the MO basis: D_oo, D_vv, D_ov and D_00 = 2 tr D_oo (R3).
