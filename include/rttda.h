@@ -196,6 +196,14 @@ int rttda_last_timings(rttda_handle_t h, double* ms_out);
  * holds at most 32768 passes; later ones are not recorded). */
 int rttda_jk_time(rttda_handle_t h, double* sum_ms, double* count);
 
+/* Timing instrumentation: runs ONE extra ERI pass (steps a3-a4) on the densities left by the last rttda_sigma /
+ * rttda_fock call of the same nvec, with the evaluation and the digestion of every segment (bra pair class x ket pair
+ * class) timed by CUDA events, serialised on `stream` (no overlap: the sum exceeds the time of a normal pass).
+ *   rows HOST [cap][16]: segment, bra class id, ket class id, la, lb, lc, ld, bra primitive pairs, ket primitive
+ *   pairs, quartets evaluated, 32-ket batches, evaluation ms, digestion ms, evaluation blocks, digestion launches, 0.
+ *   *nrows = rows written.  Synchronises.  The Fock workspace of the handle is overwritten. */
+int rttda_profile_pass(rttda_handle_t h, int32_t nvec, double* rows, int32_t cap, int32_t* nrows, void* stream);
+
 /* Sustained FP64 FMA throughput of the device (TFLOP/s) from a dependent-chain DFMA kernel run for about
  * `seconds`; the roofline denominator of the ALU-bound J/K kernels. */
 int rttda_fp64_peak(double seconds, double* tflops_out, void* stream);

@@ -21,7 +21,7 @@ OPT_INCORE = 1
 PULSE = dict(none=0, delta=1, cw=2, tl=3, chirp=4, sin2=5)
 EXPORTS = ["rttda_overlap", "rttda_dipole_ao", "rttda_create", "rttda_destroy", "rttda_sigma",
            "rttda_sigma_host", "rttda_fock", "rttda_propagate", "rttda_propagate_sso", "rttda_propagate_host",
-           "rttda_get_info", "rttda_set_option", "rttda_populations", "rttda_spectrum", "rttda_lanczos", "rttda_last_timings", "rttda_jk_time", "rttda_fp64_peak", "rttda_last_error",
+           "rttda_get_info", "rttda_set_option", "rttda_populations", "rttda_spectrum", "rttda_lanczos", "rttda_last_timings", "rttda_jk_time", "rttda_profile_pass", "rttda_fp64_peak", "rttda_last_error",
            "rttda_version"]
 
 
@@ -235,6 +235,14 @@ class Rttda:
         s, c = ct.c_double(0.0), ct.c_double(0.0)
         _check(lib().rttda_jk_time(self._h, ct.byref(s), ct.byref(c)), "rttda_jk_time")
         return s.value, int(c.value)
+
+    def rttda_profile_pass(self, nvec: int, stream=None) -> np.ndarray:
+        """One extra ERI pass with per-segment CUDA-event timings; rows as documented in include/rttda.h."""
+        rows = np.zeros((128, 16))
+        n = ct.c_int32(0)
+        _check(lib().rttda_profile_pass(self._h, int(nvec), _dptr(rows), 128, ct.byref(n), _stream(stream)),
+               "rttda_profile_pass")
+        return rows[: n.value]
 
     def info(self) -> dict:
         return {k: self.rttda_get_info(k) for k in INFO}

@@ -281,6 +281,20 @@ int rttda_jk_time(rttda_handle_t hh, double* sum_ms, double* count)
     return RTTDA_OK;
 }
 
+int rttda_profile_pass(rttda_handle_t hh, int32_t nvec, double* rows, int32_t cap, int32_t* nrows, void* stream)
+{
+    Handle* h = (Handle*)hh;
+    RT_CHECK(h && rows && nrows && cap > 0, "rttda_profile_pass: bad arguments");
+    RT_CHECK(nvec >= 1, "rttda_profile_pass: nvec < 1");
+    const int nvt = padded_nvec(nvec);
+    const size_t nn = (size_t)h->nao * h->nao;
+    RT_CHECK(h->wsT && h->wsT_n >= nn * nvt && h->wsF_n >= nn * nvt,
+             "rttda_profile_pass: call rttda_sigma / rttda_fock with the same nvec first (its densities are reused)");
+    cudaStream_t st = (cudaStream_t)stream;
+    RT_CUDA(cudaMemsetAsync(h->wsF, 0, nn * nvt * sizeof(double), st));
+    return jk_profile(h, nvt, (nvec + 1) & ~1, h->wsT, h->wsF, st, rows, cap, nrows);
+}
+
 int rttda_fp64_peak(double seconds, double* tflops, void* stream)
 {
     RT_CHECK(tflops && seconds > 0.0, "rttda_fp64_peak: bad arguments");

@@ -181,6 +181,7 @@ int jk_mark(Handle* h, cudaStream_t st);   // record the next event of the J/K t
 // jk_eval.cu / jk_digest.cu
 // F += 2 J[T] - cx K[T] for all nvt (even) interleaved densities; F zeroed by the caller.
 int jk_build(Handle* h, int nvt, int nvec, const double* Tq, double* Fq, cudaStream_t st);
+int jk_profile(Handle* h, int nvt, int nvec, const double* Tq, double* Fq, cudaStream_t st, double* rows, int cap, int* nrows);
 int eval_segment(Handle* h, const Segment& sg, double* buf, cudaStream_t st);
 int digest_launch(Handle* h, const JKLaunch& L, const Segment& sg, const double* buf, int nvt, const double* Tq,
                   double* Fq, cudaStream_t st);

@@ -64,37 +64,50 @@ __device__ __forceinline__ void boys_near(double T, const double2* __restrict__ 
     }
 }
 
-// ---- Hermite Coulomb integrals R^0_{tuv}, |tuv| <= L, times cc / sqrt(p+q) ---------------------------------
-// alpha = pq/(p+q), T = alpha R^2, r[n][0] = cc (p+q)^-1/2 (-2 alpha)^n F_n(T).
-// Far field (T >= 36, tested as pq R^2 >= 36 (p+q) without a division; erfc(6) = 2.2e-17 and every dropped term
-// e^-T/2T of the upward recursion is below 4e-18 of the (ss|ss)-like magnitude, since (2 alpha)^n / ((2p)^k (2q)^m)
-// <= 1 for n = k + m): F_0 = sqrt(pi/T)/2 and
-// F_{n+1} = (2n+1) F_n / 2T give r[0][0] = cc sqrt(pi)/2 (pq R^2)^-1/2 and r[n+1][0] = -(2n+1) r[n][0] / R^2:
-// alpha and (p+q)^-1/2 cancel, so the majority branch costs ONE rsqrt (1/R^2 = pq u^2) and no reciprocal.
+// ---- Hermite Coulomb integrals R^0_{tuv}, |tuv| <= L, times the prefactor 2 pi^(5/2) / (pq sqrt(p+q)) K_ab K_cd ------
+// r[n][0] = pref (-2 alpha)^n F_n(T), alpha = pq/(p+q), T = alpha R^2.  The kernels carry every primitive pair as
+//   c' = c pi^(1/4) / sqrt(2p)   (c = row entry [4], so that c_b c_k / sqrt(p+q) = c'_b c'_k (2/sqrt(pi)) sqrt(alpha))
+//   w  = 36 / p                  (so that alpha = 36 / (w_b + w_k) and T < 36  <=>  R^2 < w_b + w_k)
+// (PrimPair::c and PrimPair::p hold c' and w; see to_scaled).
+// Far field (T >= 36; erfc(6) = 2.2e-17 and every dropped term e^-T/2T of the upward recursion is below 4e-18 of the
+// (ss|ss)-like magnitude, since (2 alpha)^n / ((2p)^k (2q)^m) <= 1 for n = k + m): F_0 = sqrt(pi/T)/2 and
+// F_{n+1} = (2n+1) F_n / 2T give r[0][0] = c'_b c'_k / R and r[n+1][0] = -(2n+1) r[n][0] / R^2: alpha and (p+q)^-1/2
+// cancel, so the majority branch costs ONE rsqrt, no reciprocal, and the branch test is an add and a compare.
+// Near field: alpha = 36 / w needs one more rsqrt; pref = c'_b c'_k (12/sqrt(pi)) / sqrt(w).
+__device__ __forceinline__ double rsqrt_fast(double x)
+{
+    // MUFU.RSQ64H seed (2^-20) and one third-order step: error 1.6e-16 for normal positive x (measured); the library
+    // rsqrt() adds a slow-path call for subnormals / infinities that splits the scheduling region
+    double y;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+    const double e = fma(-x, y * y, 1.0);
+    return fma(y * e, fma(0.375, e, 0.5), y);
+}
+
 template <int L>
-__device__ __forceinline__ void hermite_R(double cc, double p, double q, double X, double Y, double Z,
+__device__ __forceinline__ void hermite_R(double cc, double wb, double wk, double X, double Y, double Z,
                                           const double2* __restrict__ tab, double (&R0)[nherm(L)])
 {
     double r[L + 1][nherm(L)];
-    const double R2 = X * X + Y * Y + Z * Z;
-    const double pq = p * q, s = p + q;
-    if (pq * R2 < BOYS_TMAX * s) {
-        const double rs = rsqrt(s);
-        const double alpha = pq * (rs * rs);
+    const double R2 = fma(X, X, fma(Y, Y, Z * Z));
+    const double w = wb + wk;
+    if (R2 < w) {
+        const double rw = rsqrt_fast(w);
+        const double alpha = 36.0 * (rw * rw);
         double F[L + 1];
         boys_near<L>(alpha * R2, tab, F);
-        double sc = cc * rs;
+        double sc = cc * 6.77027500257307544338 * rw;        // 12 / sqrt(pi)
 #pragma unroll
         for (int n = 0; n <= L; ++n) {
             r[n][0] = sc * F[n];
             sc *= -2.0 * alpha;
         }
     } else {
-        const double u = rsqrt(pq * R2);
-        r[0][0] = (0.88622692545275801365 * cc) * u;         // sqrt(pi)/2
-        const double w = -pq * (u * u);                      // -1/R^2
+        const double u = rsqrt_fast(R2);
+        r[0][0] = cc * u;
+        const double wn = -(u * u);                          // -1/R^2
 #pragma unroll
-        for (int n = 0; n < L; ++n) r[n + 1][0] = ((2 * n + 1) * w) * r[n][0];
+        for (int n = 0; n < L; ++n) r[n + 1][0] = ((2 * n + 1) * wn) * r[n][0];
     }
 #pragma unroll
     for (int N = 1; N <= L; ++N)
@@ -148,12 +161,19 @@ __device__ __forceinline__ void apply_p(const double (&in)[NBLK][nherm(LOUT + (N
     }
 }
 
-// Primitive pair view (registers or pointers already resolved by the caller).
+// Primitive pair view (registers or pointers already resolved by the caller).  p and c hold the SCALED quantities
+// w = 36/p and c' = c pi^(1/4)/sqrt(2p) (see hermite_R) once to_scaled() has been applied to a table row.
 struct PrimPair {
     double p, Px, Py, Pz, c, inv2p;
     double XA[3];   // P - (first centre)
     double XB[3];   // P - (second centre)
 };
+
+__device__ __forceinline__ void to_scaled(PrimPair& r)
+{
+    r.c *= 1.33133536380038971280 * rsqrt(2.0 * r.p);        // pi^(1/4)
+    r.p = 36.0 / r.p;
+}
 
 // Accumulate the primitive block into I[ia][ib][ic][id] (flattened, d fastest).
 // Order of operator application: d, c (ket; g = -1/2q), then b, a (bra; g = +1/2p).  The flattened block

@@ -72,6 +72,9 @@ __device__ __forceinline__ int warp_reduce_owner_index(int lane)
 }
 
 constexpr int REC_TILE = 256;
+#ifndef RTTDA_K_PP_MAXNI
+#define RTTDA_K_PP_MAXNI 27
+#endif
 // classes whose two-stage integral ring (4 warps x 2 x NI x 256 bytes) leaves room for several blocks per SM
 constexpr bool digest_uses_tma(int ni) { return ni <= 27; }
 constexpr size_t digest_ring_bytes(int ni) { return digest_uses_tma(ni) ? (size_t)(JK_BLOCK / 32) * 2 * ni * 256 : 0; }      // a-list records staged in shared memory at a time
@@ -88,6 +91,7 @@ struct DigestArgs {
     double* Fq;
     double cx;
     int ketclass, same, nvt, v0;
+    int nvleft;             // densities of this chunk (lanes v >= nvleft idle along)
 };
 
 template <int NV>
@@ -226,9 +230,8 @@ digest_j_kernel(DigestArgs g)
             src = g.buf + (size_t)(s_bb[ir] + qb) * (NI * 32) + lane;
         }
         // degeneracy weights: 1/2 if the ket is a diagonal pair, 1/2 if bra pair == ket pair
-        const double wsame = (same_class && br.pos == q) ? 0.5 : 1.0;
-        const double wk = ok ? wsame * (cd_same ? 0.5 : 1.0) : 0.0;
-        // J_cd needs wsame * w_ab instead of wk
+        // the stored values carry wsame * w_cd (jk_eval.cu) and are zero for lanes without a quartet;
+        // J_cd needs wsame * w_ab instead
         const double fix = (cd_same ? 2.0 : 1.0) * (ab_same ? 0.5 : 1.0);
         // canonical records: a is the pair's first shell, the stored block is (a b|c d), a fastest
 #pragma unroll
@@ -252,7 +255,7 @@ digest_j_kernel(DigestArgs g)
 #pragma unroll
                     for (int c = 0; c < NC; ++c) {
                         const int i = (d * NC + c) * (NA * NB) + i_ab;
-                        const double x = ok ? wk * (USE_TMA ? src[i * 32] : __ldcs(src + i * 32)) : 0.0;
+                        const double x = USE_TMA ? src[i * 32] : __ldcs(src + i * 32);
 #pragma unroll
                         for (int v = 0; v < NV; ++v) {
                             Jcd[c][d][v] = fma(x, sab[v], Jcd[c][d][v]);
@@ -313,7 +316,7 @@ digest_b_kernel(DigestArgs g, int G, int KW)
     const int kg = lane / G, v = lane - kg * G;
     const int kb = warp * KW + kg;                       // ket index inside the batch
     const int q = q0 + kb;
-    const bool active = kg < KW && kb < 32 && q < kc.n;
+    const bool active = kg < KW && kb < 32 && q < kc.n && v < g.nvleft;
     const bool same_class = g.same != 0;
     const int aoA = al.ao_a;
     const size_t nao = tb.nao;
@@ -406,8 +409,6 @@ digest_b_kernel(DigestArgs g, int G, int KW)
             const double* src = s_dyn + (size_t)stage * (NI * 32) + (kb & 31);
             const bool ok = ok_cur;
             const bool canonical = (br.flags & 1) != 0;
-            const double wsame = (same_class && br.pos == q) ? 0.5 : 1.0;
-            const double wk = ok ? wsame * (cd_same ? 0.5 : 1.0) : 0.0;
             const bool flip = (LA < LB) || (LA == LB && !canonical);
             if (__any_sync(0xffffffffu, ok)) {
 #pragma unroll
@@ -426,7 +427,7 @@ digest_b_kernel(DigestArgs g, int G, int KW)
 #pragma unroll
                             for (int c = 0; c < NC; ++c) {
                                 const int i = (d2 * NC + c) * (NA * NB) + i_ab;
-                                const double x = ok ? wk * src[i * 32] : 0.0;
+                                const double x = src[i * 32];
                                 Kac[a][c] = fma(x, tbd[d2], Kac[a][c]);
                                 Kca[c][a] = fma(x, tdb[d2], Kca[c][a]);
                                 Kad[a][d2] = fma(x, tbc[c], Kad[a][d2]);
@@ -462,6 +463,191 @@ digest_b_kernel(DigestArgs g, int G, int KW)
 }
 
 // ---------------------------------------------------------------------------------------------------
+// Exchange digestion, lean variant: same mapping as digest_b_kernel (block = one 32-ket batch x the a-list of one
+// shell, a group of G lanes per ket, lane = density; the batch's integrals arrive through a block-wide TMA ring), but
+//   * the stored integrals carry the degeneracy weights and are zero where no quartet exists (jk_eval.cu), so there
+//     is no per-lane test in the loop: the block walks the first `nreach` records of the a-list (those whose batch
+//     exists), found by one binary search per record tile;
+//   * a ring stage holds KR records (KR bulk copies on one mbarrier), so the block barrier and the mbarrier wait are
+//     paid once per KR records instead of once per record;
+//   * the density pairs of record r+1 are gathered while record r is digested (two register sets, loop unrolled by 2).
+constexpr int digest_k_recs(int ni) { return ni == 1 ? 16 : (ni == 3 ? 8 : (ni == 9 ? 4 : (ni == 27 ? 2 : 1))); }
+constexpr size_t digest_k_smem(int ni) { return (size_t)2 * digest_k_recs(ni) * ni * 256; }
+
+template <int NB, int NC, int ND>
+struct KRec {
+    double2 bd[NB][ND], bc[NB][NC];
+};
+
+template <int LA, int LB, int LC, int LD>
+__global__ void __launch_bounds__(256)
+digest_k_kernel(DigestArgs g, int G, int KW)
+{
+    constexpr int NA = 2 * LA + 1, NB = 2 * LB + 1, NC = 2 * LC + 1, ND = 2 * LD + 1;
+    constexpr int NI = NA * NB * NC * ND;
+    constexpr int NAB = NA * NB;
+    constexpr int KR = digest_k_recs(NI);
+    constexpr bool PP = (NI < RTTDA_K_PP_MAXNI);                        // two register sets for the gathered density pairs
+    const JKTables& tb = g.tb;
+    const WorkItem wi = g.work[blockIdx.x >> 2];
+    const AList al = tb.alists[wi.alist];
+    const KetClass& kc = tb.kets[g.ketclass];
+    const int q0 = wi.ket0 + 32 * (blockIdx.x & 3);      // first ket of this block's batch
+    if (q0 >= kc.n) return;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int kg = lane / G, v = lane - kg * G;
+    const int kb = warp * KW + kg;                       // ket index inside the batch
+    const int q = q0 + kb;
+    const bool active = kg < KW && kb < 32 && q < kc.n && v < g.nvleft;
+    const bool same_class = g.same != 0;
+    const size_t nao = tb.nao;
+    const int nvt = g.nvt;
+    const size_t rs = nao * nvt;
+    __shared__ unsigned long long s_ro[REC_TILE];        // row offset of shell b in the density-pair array | canonical bit
+    __shared__ long long s_bb[REC_TILE];                 // offset of the record's batch in the staging buffer
+    __shared__ double s_Q[REC_TILE];
+    __shared__ int s_pos[REC_TILE];
+    __shared__ __align__(8) uint64_t s_bar[2];
+    extern __shared__ __align__(16) double s_dyn[];      // ring: 2 stages x KR records x NI x 32 doubles
+    if (threadIdx.x == 0) { mbar_init(&s_bar[0], 1); mbar_init(&s_bar[1], 1); mbar_fence_init(); }
+
+    const int qlast = min(q0 + 31, kc.n - 1);
+    const double Qbatch = __ldg(kc.Q + q0);               // kets are sorted: the batch's largest bound
+    const int qq = active ? q : q0;                       // idle lanes shadow a real ket (their results are dropped)
+    const int aoC = __ldg(kc.ao_c + qq), aoD = __ldg(kc.ao_d + qq);
+    const double2* PPv = reinterpret_cast<const double2*>(g.PPq) + g.v0 + (active ? v : 0);
+    const double2* PD = PPv + (size_t)aoD * nvt;         // + (aoB + b) * rs + d2 * nvt
+    const double2* PC = PPv + (size_t)aoC * nvt;
+    const double* gbase = g.buf + (size_t)(q0 >> 5) * (NI * 32);
+    const int kcol = active ? kb : 0;
+
+    double Kac[NA][NC], Kca[NC][NA], Kad[NA][ND], Kda[ND][NA];
+#pragma unroll
+    for (int a = 0; a < NA; ++a) {
+#pragma unroll
+        for (int c = 0; c < NC; ++c) Kac[a][c] = Kca[c][a] = 0.0;
+#pragma unroll
+        for (int d2 = 0; d2 < ND; ++d2) Kad[a][d2] = Kda[d2][a] = 0.0;
+    }
+    using Rec = KRec<NB, NC, ND>;
+    auto fetch = [&](int ir, Rec& r) {
+        const size_t ro = (size_t)(s_ro[ir] >> 1);
+#pragma unroll
+        for (int b = 0; b < NB; ++b) {
+#pragma unroll
+            for (int d2 = 0; d2 < ND; ++d2) r.bd[b][d2] = __ldg(PD + ro + b * rs + d2 * nvt);
+#pragma unroll
+            for (int c = 0; c < NC; ++c) r.bc[b][c] = __ldg(PC + ro + b * rs + c * nvt);
+        }
+    };
+    auto digest = [&](int ir, const double* src, const Rec& r) {
+        const bool flip = (LA < LB) || (LA == LB && LA > 0 && !(s_ro[ir] & 1ull));
+#pragma unroll
+        for (int d2 = 0; d2 < ND; ++d2)
+#pragma unroll
+            for (int c = 0; c < NC; ++c) {
+                double x[NAB];
+#pragma unroll
+                for (int j = 0; j < NAB; ++j) x[j] = src[((d2 * NC + c) * NAB + j) * 32];
+#pragma unroll
+                for (int b = 0; b < NB; ++b)
+#pragma unroll
+                    for (int a = 0; a < NA; ++a) {
+                        const double xi = flip ? x[a * NB + b] : x[b * NA + a];
+                        Kac[a][c] = fma(xi, r.bd[b][d2].x, Kac[a][c]);
+                        Kca[c][a] = fma(xi, r.bd[b][d2].y, Kca[c][a]);
+                        Kad[a][d2] = fma(xi, r.bc[b][c].x, Kad[a][d2]);
+                        Kda[d2][a] = fma(xi, r.bc[b][c].y, Kda[d2][a]);
+                    }
+            }
+    };
+    auto issue = [&](int r_begin, int r_end, int sidx) {  // thread 0: records [r_begin, r_end) of the tile into ring stage sidx
+        mbar_expect_tx(&s_bar[sidx], (uint32_t)(r_end - r_begin) * NI * 256);
+        for (int r = r_begin; r < r_end; ++r)
+            tma_load_1d(s_dyn + ((size_t)sidx * KR + (r - r_begin)) * (NI * 32), gbase + s_bb[r], NI * 256, &s_bar[sidx]);
+    };
+    uint32_t phase0 = 0, phase1 = 0;
+    bool done = false;                                    // block-uniform
+    for (int r0 = al.rec_begin; r0 < al.rec_end && !done; r0 += REC_TILE) {
+        const int nrec = min(REC_TILE, al.rec_end - r0);
+        __syncthreads();
+        for (int i = threadIdx.x; i < nrec; i += blockDim.x) {
+            const BraRec b0 = tb.recs[r0 + i];
+            s_ro[i] = ((unsigned long long)((size_t)b0.ao_b * rs) << 1) | (unsigned long long)(b0.flags & 1);
+            s_bb[i] = (__ldg(g.batch_base + b0.pos) - (same_class ? (b0.pos >> 5) : 0)) * (long long)(NI * 32);
+            s_Q[i] = b0.Q;
+            s_pos[i] = b0.pos;
+        }
+        __syncthreads();
+        // Records are sorted (bound descending, position ascending).  The batch of record p exists iff some ket q of
+        // it has Q_p Q_q >= tau and (different classes or p <= q); the best candidate is q = max(p, q0), and
+        // Q[p] = Q_p inside one class.  The records whose batch exists are a prefix of the list.
+        int lo = 0, hi = nrec;
+        while (lo < hi) {
+            const int mid = (lo + hi) >> 1;
+            const double Qp = s_Q[mid];
+            const int pos = s_pos[mid];
+            const bool reach = same_class ? (pos <= qlast && Qp * (pos > q0 ? Qp : Qbatch) >= tb.tau)
+                                          : (Qp * Qbatch >= tb.tau);
+            if (reach) lo = mid + 1; else hi = mid;
+        }
+        const int nreach = lo;
+        if (nreach < nrec) done = true;
+        if (nreach == 0) break;
+        const int nst = (nreach + KR - 1) / KR;
+        if (threadIdx.x == 0) issue(0, min(KR, nreach), 0);
+        Rec A, B;
+        fetch(0, A);
+        for (int st = 0; st < nst; ++st) {
+            const int sidx = st & 1, rb = st * KR, re = min(rb + KR, nreach);
+            if (threadIdx.x == 0 && st + 1 < nst) issue(re, min(re + KR, nreach), sidx ^ 1);
+            if (sidx == 0) { mbar_wait(&s_bar[0], phase0); phase0 ^= 1; }
+            else { mbar_wait(&s_bar[1], phase1); phase1 ^= 1; }
+            const double* sbase = s_dyn + (size_t)sidx * KR * (NI * 32) + kcol;
+            if (PP) {
+                int ir = rb;
+                for (; ir + 1 < re; ir += 2) {
+                    fetch(ir + 1, B);
+                    digest(ir, sbase + (size_t)(ir - rb) * (NI * 32), A);
+                    if (ir + 2 < nreach) fetch(ir + 2, A);
+                    digest(ir + 1, sbase + (size_t)(ir + 1 - rb) * (NI * 32), B);
+                }
+                if (ir < re) {                            // odd tail of the stage (KR == 1 or the last stage)
+                    if (ir + 1 < nreach) fetch(ir + 1, B);
+                    digest(ir, sbase + (size_t)(ir - rb) * (NI * 32), A);
+                    if (ir + 1 < nreach) A = B;
+                }
+            } else {
+                for (int ir = rb; ir < re; ++ir) {
+                    if (ir > 0) fetch(ir, A);
+                    digest(ir, sbase + (size_t)(ir - rb) * (NI * 32), A);
+                }
+            }
+            __syncthreads();                              // every warp is done with this stage before it is refilled
+        }
+    }
+    if (active) {
+        const int aoA = al.ao_a;
+        const double cx = g.cx;
+        double* Fv = g.Fq + g.v0 + v;
+        double* FA = Fv + (size_t)aoA * rs;
+#pragma unroll
+        for (int a = 0; a < NA; ++a) {
+#pragma unroll
+            for (int c = 0; c < NC; ++c) {
+                atomicAdd(FA + a * rs + (size_t)(aoC + c) * nvt, -0.5 * cx * (Kac[a][c] + Kca[c][a]));
+                atomicAdd(Fv + (size_t)(aoC + c) * rs + (size_t)(aoA + a) * nvt, -0.5 * cx * (Kac[a][c] - Kca[c][a]));
+            }
+#pragma unroll
+            for (int d2 = 0; d2 < ND; ++d2) {
+                atomicAdd(FA + a * rs + (size_t)(aoD + d2) * nvt, -0.5 * cx * (Kad[a][d2] + Kda[d2][a]));
+                atomicAdd(Fv + (size_t)(aoD + d2) * rs + (size_t)(aoA + a) * nvt, -0.5 * cx * (Kad[a][d2] - Kda[d2][a]));
+            }
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------
 template <int LA, int LB, int LC, int LD, int NV>
 static int launch_digest_j(Handle* h, const JKLaunch& L, const Segment& sg, const double* buf, int nvt, int v0,
                             const double* Tq, double* Fq, cudaStream_t st)
@@ -475,11 +661,8 @@ static int launch_digest_j(Handle* h, const JKLaunch& L, const Segment& sg, cons
     g.ketclass = L.ketclass; g.same = (sg.kc_bra == sg.kc_ket); g.nvt = nvt; g.v0 = v0;
     constexpr int NI = (2 * LA + 1) * (2 * LB + 1) * (2 * LC + 1) * (2 * LD + 1);
     constexpr size_t smem = digest_ring_bytes(NI);
-    static bool attr_set = false;
-    if (!attr_set && smem > 0) {
+    if (smem > 0)     // per launch: the attribute belongs to the current device's context, not to the process
         RT_CUDA(cudaFuncSetAttribute(digest_j_kernel<LA, LB, LC, LD, NV>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        attr_set = true;
-    }
     digest_j_kernel<LA, LB, LC, LD, NV><<<dim3(L.nwork), dim3(JK_BLOCK), smem, st>>>(g);
     h->kernel_launches++;
     RT_CUDA(cudaGetLastError());
@@ -508,19 +691,23 @@ static int launch_digest(Handle* h, const JKLaunch& L, const Segment& sg, const 
     }
     constexpr int NI = (2 * LA + 1) * (2 * LB + 1) * (2 * LC + 1) * (2 * LD + 1);
     constexpr size_t smem = (size_t)2 * NI * 256;
-    static bool attr_set = false;
-    if (!attr_set) {
-        RT_CUDA(cudaFuncSetAttribute(digest_b_kernel<LA, LB, LC, LD>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        attr_set = true;
-    }
+    RT_CUDA(cudaFuncSetAttribute(digest_b_kernel<LA, LB, LC, LD>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    RT_CUDA(cudaFuncSetAttribute(digest_k_kernel<LA, LB, LC, LD>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)digest_k_smem(NI)));
     for (int v0 = 0; v0 < nvec; v0 += 8) {
-        const int G = nvec - v0 < 8 ? nvec - v0 : 8;
+        // lane groups of 2, 4 or 8 densities: a group then never straddles a quarter warp, so one 16-byte gather per
+        // lane costs one L1 wavefront per ket (groups of 6 cost ~1.6); lanes beyond the call's densities work on the
+        // zero padding slots and are not flushed
+        const int left = nvec - v0, G = left > 4 ? 8 : (left > 2 ? 4 : 2);
         DigestArgs g;
+        g.nvleft = left;
         g.tb = h->tabs; g.work = L.work; g.batch_base = sg.batch_base; g.buf = buf;
         g.Tq = Tq; g.PPq = h->wsP; g.Fq = Fq; g.cx = h->cx;
         g.ketclass = L.ketclass; g.same = (sg.kc_bra == sg.kc_ket); g.nvt = nvt; g.v0 = v0;
         const int KW = 32 / G, nwarps = (32 + KW - 1) / KW;
-        digest_b_kernel<LA, LB, LC, LD><<<dim3(4 * L.nwork), dim3(32 * nwarps), smem, st>>>(g, G, KW);
+        // one or three integrals per quartet: the multi-record ring (digest_k_kernel) wins; above that its larger
+        // register footprint costs more occupancy than the saved barriers bring (profiles/README.md)
+        if (NI > 3) digest_b_kernel<LA, LB, LC, LD><<<dim3(4 * L.nwork), dim3(32 * nwarps), smem, st>>>(g, G, KW);
+        else digest_k_kernel<LA, LB, LC, LD><<<dim3(4 * L.nwork), dim3(32 * nwarps), digest_k_smem(NI), st>>>(g, G, KW);
         h->kernel_launches++;
         RT_CUDA(cudaGetLastError());
     }
@@ -603,6 +790,44 @@ int jk_build(Handle* h, int nvt, int nvec, const double* Tq, double* Fq, cudaStr
         RT_CUDA(cudaEventRecord(h->ev_D[b], st));
         ++k;
     }
+    return RTTDA_OK;
+}
+
+// Timing instrumentation: ONE ERI pass with every segment's evaluation and digestion timed by its
+// own pair of CUDA events, everything serialised on `st`.  rows[k][16] (host) = {segment, bra class, ket class, la, lb,
+// lc, ld, bra primitive pairs, ket primitive pairs, quartets, 32-ket batches, evaluation ms, digestion ms, evaluation
+// blocks, digestion launches, 0}.
+int jk_profile(Handle* h, int nvt, int nvec, const double* Tq, double* Fq, cudaStream_t st, double* rows, int cap, int* nrows)
+{
+    for (int b = 0; b < 2; ++b) RT_TRY(ensure_ws(h, &h->eri_buf[b], &h->eri_buf_n[b], h->eri_buf_need));
+    const long long n = (long long)h->nao * h->nao * nvt;
+    RT_TRY(ensure_ws(h, &h->wsP, &h->wsP_n, (size_t)2 * n));
+    symsplit_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(h->nao, nvt, Tq, reinterpret_cast<double2*>(h->wsP));
+    RT_CUDA(cudaGetLastError());
+    cudaEvent_t e[3];
+    for (auto& x : e) RT_CUDA(cudaEventCreate(&x));
+    int k = 0;
+    for (size_t si = 0; si < h->segments.size(); ++si) {
+        const Segment& sg = h->segments[si];
+        if (sg.nitems == 0 || k >= cap) continue;
+        RT_CUDA(cudaEventRecord(e[0], st));
+        RT_TRY(eval_segment(h, sg, h->eri_buf[0], st));
+        RT_CUDA(cudaEventRecord(e[1], st));
+        for (int l = sg.first_launch; l < sg.first_launch + sg.nlaunch; ++l)
+            RT_TRY(digest_launch(h, h->launches[l], sg, h->eri_buf[0], nvt, nvec, Tq, Fq, st));
+        RT_CUDA(cudaEventRecord(e[2], st));
+        RT_CUDA(cudaEventSynchronize(e[2]));
+        float me = 0, md = 0;
+        RT_CUDA(cudaEventElapsedTime(&me, e[0], e[1]));
+        RT_CUDA(cudaEventElapsedTime(&md, e[1], e[2]));
+        double* r = rows + (size_t)k * 16;
+        r[0] = (double)si; r[1] = sg.kc_bra; r[2] = sg.kc_ket; r[3] = sg.la; r[4] = sg.lb; r[5] = sg.lc; r[6] = sg.ld;
+        r[7] = h->tabs.kets[sg.kc_bra].np; r[8] = h->tabs.kets[sg.kc_ket].np; r[9] = (double)sg.nquartets;
+        r[10] = (double)sg.nbatch; r[11] = me; r[12] = md; r[13] = sg.nitems; r[14] = sg.nlaunch; r[15] = 0.0;
+        ++k;
+    }
+    for (auto& x : e) cudaEventDestroy(x);
+    *nrows = k;
     return RTTDA_OK;
 }
 

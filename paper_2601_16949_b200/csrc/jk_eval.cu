@@ -43,6 +43,7 @@ __device__ __forceinline__ PrimPair load_ket_prim(const double* __restrict__ pri
     } else {
         r.XB[0] = r.XB[1] = r.XB[2] = 0.0;
     }
+    to_scaled(r);
     return r;
 }
 
@@ -76,6 +77,12 @@ __global__ void __launch_bounds__(JK_BLOCK) eval_kernel(EvalArgs g)
         double2* dst = reinterpret_cast<double2*>(s_rows);
         const int n2 = npairs * npb * (PRIM_STRIDE / 2);
         for (int i = threadIdx.x; i < n2; i += JK_BLOCK) dst[i] = src[i];
+        __syncthreads();
+        for (int r = threadIdx.x; r < npairs * npb; r += JK_BLOCK) {     // rows carry c' and w = 36/p (eri_eval.cuh)
+            const double p = s_rows[r * PRIM_STRIDE];
+            s_rows[r * PRIM_STRIDE + 4] *= 1.33133536380038971280 * rsqrt(2.0 * p);
+            s_rows[r * PRIM_STRIDE] = 36.0 / p;
+        }
         if (threadIdx.x < npairs) {
             s_Q[threadIdx.x] = g.bra.Q[it.p_begin + threadIdx.x];
             s_base[threadIdx.x] = g.batch_base[it.p_begin + threadIdx.x];
@@ -87,6 +94,7 @@ __global__ void __launch_bounds__(JK_BLOCK) eval_kernel(EvalArgs g)
     const bool active = q < g.ket.n;
     const int qq = active ? q : g.ket.n - 1;
     const double Qq = active ? __ldg(g.ket.Q + qq) : 0.0;
+    const double wcd = __ldg(g.ket.same + qq) ? 0.5 : 1.0;
     const int lane = threadIdx.x & 31;
 
     PrimPair kp[KET_IN_REGS ? KP : 1];
@@ -99,12 +107,17 @@ __global__ void __launch_bounds__(JK_BLOCK) eval_kernel(EvalArgs g)
         const int p = it.p_begin + ip;
         const bool ok = active && (s_Q[ip] * Qq >= g.tau) && (!g.same || p <= q);
         if (!__any_sync(0xffffffffu, ok)) break;          // both conditions only get worse along the bra list
-        if (!ok) continue;
+        // A batch (bra pair, 32 kets = this warp) that exists in the staging map is written in full: lanes whose
+        // quartet is screened out, lies below the diagonal of a same-class segment or beyond the ket list store
+        // zeros, and the degeneracy weights of the 8-fold symmetry that depend on the quartet alone (1/2 if bra
+        // pair == ket pair, 1/2 if the ket pair is diagonal) are folded into the stored values, so the digestion
+        // kernels need no per-lane tests.
         double I[NI];
 #pragma unroll
         for (int i = 0; i < NI; ++i) I[i] = 0.0;
         const double* rows = s_rows + (size_t)ip * npb * PRIM_STRIDE;
-        if (KET_IN_REGS) {
+        if (!ok) {
+        } else if (KET_IN_REGS) {
 #pragma unroll 1
             for (int kb = 0; kb < npb; ++kb) {
                 const PrimPair bp = load_bra_prim_smem(rows + kb * PRIM_STRIDE);
@@ -125,8 +138,9 @@ __global__ void __launch_bounds__(JK_BLOCK) eval_kernel(EvalArgs g)
         }
         const long long batch = s_base[ip] + (q >> 5) - (g.same ? (p >> 5) : 0);
         double* dst = g.buf + (size_t)batch * (NI * 32) + lane;
+        const double w = (g.same && p == q) ? 0.5 * wcd : wcd;
 #pragma unroll
-        for (int i = 0; i < NI; ++i) __stcs(dst + i * 32, I[i]);
+        for (int i = 0; i < NI; ++i) __stcs(dst + i * 32, w * I[i]);
     }
 }
 
@@ -183,9 +197,11 @@ __global__ void schwarz_kernel(int npairs, const int* __restrict__ np, const int
     for (int k = 0; k < NA * NB * NA * NB; ++k) I[k] = 0.0;
     const int n = np[i], o = off[i];
     for (int k1 = 0; k1 < n; ++k1) {
-        const PrimPair b = load_prim_aos(prim + (size_t)(o + k1) * PRIM_STRIDE);
+        PrimPair b = load_prim_aos(prim + (size_t)(o + k1) * PRIM_STRIDE);
+        to_scaled(b);
         for (int k2 = 0; k2 < n; ++k2) {
-            const PrimPair k = load_prim_aos(prim + (size_t)(o + k2) * PRIM_STRIDE);
+            PrimPair k = load_prim_aos(prim + (size_t)(o + k2) * PRIM_STRIDE);
+            to_scaled(k);
             eri_prim_accum<LA, LB, LA, LB>(b, k, boys_tab, I);
         }
     }

@@ -440,7 +440,9 @@ int create_impl(Handle* h, const rttda_basis_t* basis, const double* C_occ, cons
             RT_TRY(upload(h, base, &sg.batch_base));
             // evaluation blocks: JK_BLOCK kets x a run of bra pairs (rows staged in shared memory)
             const int npb = h->tabs.kets[kcb].np;
-            const int G = std::min(JK_BLOCK, EVAL_MAX_ROWS / npb);
+            // at most 32 bra pairs per block: shallow contractions (1 or 3 primitive pairs) would otherwise give a
+            // handful of very long blocks per segment and leave SMs idle
+            const int G = std::min(32, std::min(JK_BLOCK, EVAL_MAX_ROWS / npb));
             std::vector<EvalItem> items;
             for (int k0 = 0; k0 < nk; k0 += JK_BLOCK) {
                 int hi = tau > 0.0 ? count_prod_ge(kcb, hQ[kck][k0]) : nb;     // bra pairs reaching this chunk
