@@ -68,9 +68,11 @@ typedef struct {
 typedef enum { RTTDA_NONE = 0, RTTDA_DELTA = 1, RTTDA_CW = 2, RTTDA_TL = 3, RTTDA_CHIRP = 4,
                RTTDA_SIN2 = 5 } rttda_pulse_t;
 
+#define RTTDA_FIELD_CONTINUE 1   /* flags bit: this call CONTINUES the previous rttda_propagate / _sso call of the handle:
+                                  no delta kick is applied and R(t) stays relative to the reference state of that call */
 typedef struct {
     int32_t type;                               /* rttda_pulse_t */
-    int32_t reserved;
+    int32_t flags;                              /* 0 or RTTDA_FIELD_CONTINUE (setting it in any record marks the call) */
     double E0, omega, t0, sigma, beta, T_env;
     double dir[3];                              /* polarisation d (used as given, not renormalised) */
 } rttda_field_t;
@@ -117,7 +119,9 @@ int rttda_fock(rttda_handle_t h, int32_t nvec, const double* T, double* F, void*
  *   fields host [ntraj]
  *   log    DEVICE or NULL, [nsteps][ntraj][3]: |C|^2, Re R, Im R after each step, R relative to the state
  *          at t_start (after the kick, if any)
- * Re-entrant in time: call again with t_start += nsteps*dt to continue. */
+ * Re-entrant in time: call again with t_start += nsteps*dt to continue; set RTTDA_FIELD_CONTINUE in the field
+ * records of the continued call, otherwise a DELTA field kicks again and R(t) restarts from the state at t_start.
+ * (The state C is the whole checkpoint; the reference state of R(t) lives in the handle until the next fresh call.) */
 int rttda_propagate(rttda_handle_t h, int32_t ntraj, double* C, const rttda_field_t* fields,
                     double t_start, double dt, int32_t nsteps, double* log, void* stream);
 
@@ -203,6 +207,15 @@ int rttda_jk_time(rttda_handle_t h, double* sum_ms, double* count);
  *   pairs, quartets evaluated, 32-ket batches, evaluation ms, digestion ms, evaluation blocks, digestion launches, 0.
  *   *nrows = rows written.  Synchronises.  The Fock workspace of the handle is overwritten. */
 int rttda_profile_pass(rttda_handle_t h, int32_t nvec, double* rows, int32_t cap, int32_t* nrows, void* stream);
+
+/* The FP64 tensor-core (DMMA) GEMM behind the MO<->AO transforms and the field coupling (steps a1, a5, a6; the paper
+ * uses cuBLAS for them), exposed for unit tests and callers:
+ *   C_b(m,n) = alpha * sum_k A_b(m,k) B_b(k,n) + beta * C_b(m,n),  b < batch, element strides in doubles:
+ *   A_b(m,k) = A[b*sabatch + m*sam + k*sak], B_b(k,n) = B[b*sbbatch + k*sbk + n*sbn], C likewise.  All DEVICE.
+ *   beta == 0 does not read C.  K == 0 gives C = beta * C.  Enqueued on `stream`. */
+int rttda_gemm_f64(int32_t M, int32_t N, int32_t K, int32_t batch, double alpha, const double* A, int64_t sam, int64_t sak,
+                   int64_t sabatch, const double* B, int64_t sbk, int64_t sbn, int64_t sbbatch, double beta, double* C,
+                   int64_t scm, int64_t scn, int64_t scbatch, void* stream);
 
 /* Sustained FP64 FMA throughput of the device (TFLOP/s) from a dependent-chain DFMA kernel run for about
  * `seconds`; the roofline denominator of the ALU-bound J/K kernels. */

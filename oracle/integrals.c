@@ -314,6 +314,34 @@ void oracle_eri_tensor(BASIS_ARGS, int nao, double *eri)
         }
 }
 
+/* All integrals (mu nu|lam sig) with (lam, sig) running over the AOs of ONE shell pair (sc, sd):
+ * out[nao][nao][nc][nd], no symmetry used in (mu, nu) except that the shell quartet (sa sb|sc sd) with sa >= sb is
+ * evaluated once and written to both (mu nu) and (nu mu).  Shell quartets with Q_ab Q_cd < tau are left zero
+ * (tau <= 0: none skipped).  Building block of the dense A of the 400-AO configuration (SURVEY 8(c5) route ii). */
+void oracle_eri_pair_block(BASIS_ARGS, int nao, int sc, int sd, double tau, const double *Qs, double *out)
+{
+    basis_t B = BASIS_MK;
+    int nc = 2 * sh_l[sc] + 1, nd = 2 * sh_l[sd] + 1;
+    memset(out, 0, sizeof(double) * (size_t)nao * nao * nc * nd);
+    double qcd = Qs[(size_t)sc * nshells + sd];
+    #pragma omp parallel for schedule(dynamic, 2)
+    for (int sa = 0; sa < nshells; ++sa)
+        for (int sb = 0; sb <= sa; ++sb) {
+            if (tau > 0.0 && Qs[(size_t)sa * nshells + sb] * qcd < tau) continue;
+            double blk[81];
+            shell_quartet(&B, sa, sb, sc, sd, blk);
+            int na = 2 * sh_l[sa] + 1, nb = 2 * sh_l[sb] + 1, idx = 0;
+            for (int ca = 0; ca < na; ++ca)
+            for (int cb = 0; cb < nb; ++cb)
+            for (int cc = 0; cc < nc; ++cc)
+            for (int cd = 0; cd < nd; ++cd, ++idx) {
+                size_t m = ao_off[sa] + ca, n = ao_off[sb] + cb;
+                out[((m * nao + n) * nc + cc) * nd + cd] = blk[idx];
+                out[((n * nao + m) * nc + cc) * nd + cd] = blk[idx];
+            }
+        }
+}
+
 /* Schwarz bounds Q_ab = sqrt(max_{mu in a, nu in b} (mu nu|mu nu)), [nshells][nshells] (R14). */
 void oracle_schwarz(BASIS_ARGS, double *Q)
 {

@@ -112,6 +112,17 @@ class OracleBasis:
         lib().oracle_eri_tensor(*self._args(), ct.c_int(N), eri.ctypes.data_as(_dp))
         return eri
 
+    def eri_pair_block(self, sc: int, sd: int, tau: float = 0.0, Q: np.ndarray | None = None) -> np.ndarray:
+        """(mu nu|lam sig) for all mu, nu and the AOs lam, sig of the shell pair (sc, sd): [N][N][nc][nd]."""
+        nc, nd = 2 * int(self.sh_l[sc]) + 1, 2 * int(self.sh_l[sd]) + 1
+        out = np.zeros((self.nao, self.nao, nc, nd))
+        if Q is None:
+            Q = self.schwarz()
+        Q = np.ascontiguousarray(Q)
+        lib().oracle_eri_pair_block(*self._args(), ct.c_int(self.nao), ct.c_int(sc), ct.c_int(sd), ct.c_double(tau),
+                                    Q.ctypes.data_as(_dp), out.ctypes.data_as(_dp))
+        return out
+
     def schwarz(self) -> np.ndarray:
         Q = np.zeros((self.nshells, self.nshells))
         lib().oracle_schwarz(*self._args(), Q.ctypes.data_as(_dp))

@@ -39,6 +39,48 @@ def build_A(eri, C_o, C_v, eps, cx=1.0):
     return A
 
 
+def build_A_by_pair_blocks(ob, C_o, C_v, eps, cx=1.0, tau=0.0, Q=None, progress=None):
+    """Dense singles block of A (eq. 3 under R1) for systems whose AO tensor does not fit (SURVEY 8(c5) route ii):
+    AO integrals one ket shell pair (lam sig) at a time, half-transformed at once,
+        (ia|lam sig) = sum_{mu nu} C_{mu i} C_{nu a} (mu nu|lam sig),   (ij|lam sig) likewise,
+    stored for all (lam, sig), then the second half transform over (lam, sig).  Same quarter transforms as
+    `mo_eri_blocks`, only ordered so that N^4 doubles never exist at once.  Memory: no*nv*N^2 + no^2*N^2 doubles."""
+    no, nv, N = C_o.shape[1], C_v.shape[1], C_o.shape[0]
+    if Q is None:
+        Q = ob.schwarz()
+    ov = np.zeros((no * nv, N, N))
+    oo = np.zeros((no * no, N, N))
+    for sc in range(ob.nshells):
+        for sd in range(sc + 1):
+            blk = ob.eri_pair_block(sc, sd, tau, Q)                       # [N][N][nc][nd]
+            oc, od = int(ob.ao_off[sc]), int(ob.ao_off[sd])
+            for cc in range(blk.shape[2]):
+                for cd in range(blk.shape[3]):
+                    M = blk[:, :, cc, cd]
+                    half = C_o.T @ M                                        # [no][N]
+                    via = (half @ C_v).reshape(-1)
+                    vij = (half @ C_o).reshape(-1)
+                    ov[:, oc + cc, od + cd] = via
+                    ov[:, od + cd, oc + cc] = via                           # (mu nu|lam sig) = (mu nu|sig lam)
+                    oo[:, oc + cc, od + cd] = vij
+                    oo[:, od + cd, oc + cc] = vij
+        if progress:
+            progress(sc)
+    A = np.empty((no * nv, no * nv))
+    step = max(1, 2 ** 27 // (N * N))                                      # rows of `ov` per chunk (~1 GB)
+    for r0 in range(0, no * nv, step):
+        t = ov[r0:r0 + step] @ C_v                                         # [rows][lam][b]
+        t = np.einsum("rlb,lj->rjb", t, C_o, optimize=True)                # [rows][j][b]
+        A[r0:r0 + step] = 2.0 * t.reshape(t.shape[0], -1)
+    del ov
+    t = oo @ C_v                                                           # [ij][lam][b]
+    oovv = np.einsum("rlb,la->rab", t, C_v, optimize=True).reshape(no, no, nv, nv)   # (ij|ab)
+    A -= cx * np.transpose(oovv, (0, 2, 1, 3)).reshape(no * nv, no * nv)
+    de = (eps[no:][None, :] - eps[:no][:, None]).reshape(-1)
+    A[np.diag_indices(no * nv)] += de
+    return A
+
+
 def extend_A(A):
     """A_ext = diag(A_00 = 0, A), no coupling between element 0 and the singles (R2)."""
     n = A.shape[0]

@@ -18,10 +18,11 @@ INFO = dict(npairs_total=0, npairs_kept=1, nquartets=2, nprim_quartets=3, nquart
             nprim_eval=5, flops_eval=6, flops_digest_per_vec=7, jk_launches=8, kernel_launches=9,
             create_ms=10, qmax=11, nvec_chunk=12, eri_buf_bytes=13, eri_all_bytes=14)
 OPT_INCORE = 1
+FIELD_CONTINUE = 1
 PULSE = dict(none=0, delta=1, cw=2, tl=3, chirp=4, sin2=5)
 EXPORTS = ["rttda_overlap", "rttda_dipole_ao", "rttda_create", "rttda_destroy", "rttda_sigma",
            "rttda_sigma_host", "rttda_fock", "rttda_propagate", "rttda_propagate_sso", "rttda_propagate_host",
-           "rttda_get_info", "rttda_set_option", "rttda_populations", "rttda_spectrum", "rttda_lanczos", "rttda_last_timings", "rttda_jk_time", "rttda_profile_pass", "rttda_fp64_peak", "rttda_last_error",
+           "rttda_get_info", "rttda_set_option", "rttda_populations", "rttda_spectrum", "rttda_lanczos", "rttda_last_timings", "rttda_jk_time", "rttda_profile_pass", "rttda_gemm_f64", "rttda_fp64_peak", "rttda_last_error",
            "rttda_version"]
 
 
@@ -40,7 +41,7 @@ class BasisT(ct.Structure):
 
 
 class FieldT(ct.Structure):
-    _fields_ = [("type", ct.c_int32), ("reserved", ct.c_int32), ("E0", ct.c_double), ("omega", ct.c_double),
+    _fields_ = [("type", ct.c_int32), ("flags", ct.c_int32), ("E0", ct.c_double), ("omega", ct.c_double),
                 ("t0", ct.c_double), ("sigma", ct.c_double), ("beta", ct.c_double), ("T_env", ct.c_double),
                 ("dir", ct.c_double * 3)]
 
@@ -105,7 +106,7 @@ class _BasisHolder:
 
 def make_field(f: dict) -> FieldT:
     d = f.get("dir", (0.0, 0.0, 1.0))
-    return FieldT(PULSE[f.get("type", "none")], 0, float(f.get("E0", 0.0)), float(f.get("omega") or 0.0),
+    return FieldT(PULSE[f.get("type", "none")], FIELD_CONTINUE if f.get("continue") else 0, float(f.get("E0", 0.0)), float(f.get("omega") or 0.0),
                   float(f.get("t0", 0.0)), float(f.get("sigma", 1.0)), float(f.get("beta", 0.0)),
                   float(f.get("T_env", 0.0)), (ct.c_double * 3)(*[float(x) for x in d]))
 
@@ -128,6 +129,17 @@ def rttda_fp64_peak(seconds: float = 1.0, stream=None) -> float:
     out = ct.c_double(0.0)
     _check(lib().rttda_fp64_peak(ct.c_double(seconds), ct.byref(out), _stream(stream)), "rttda_fp64_peak")
     return out.value
+
+
+def rttda_gemm_f64(M, N, K, batch, alpha, A, sa, B, sb, beta, C, sc, stream=None):
+    """C = alpha A B + beta C, strided batched (include/rttda.h); sa = (sam, sak, sabatch), sb = (sbk, sbn, sbbatch),
+    sc = (scm, scn, scbatch) in doubles; A, B, C CUDA tensors (any shape: only the base pointer is used)."""
+    i64 = ct.c_int64
+    _check(lib().rttda_gemm_f64(int(M), int(N), int(K), int(batch), ct.c_double(alpha), ct.c_void_p(A.data_ptr()),
+                                i64(sa[0]), i64(sa[1]), i64(sa[2]), ct.c_void_p(B.data_ptr()), i64(sb[0]), i64(sb[1]),
+                                i64(sb[2]), ct.c_double(beta), ct.c_void_p(C.data_ptr()), i64(sc[0]), i64(sc[1]),
+                                i64(sc[2]), _stream(stream)), "rttda_gemm_f64")
+    return C
 
 
 def rttda_spectrum(R0, log, dt: float, pad: int, omega, intensity, stream=None):

@@ -47,6 +47,9 @@ __global__ void fp64_peak_kernel(double* out, int iters, double a, double b)
 
 using namespace rttda;
 
+// A handle is bound to the device current at rttda_create: every entry point makes that device current.
+#define RT_DEVICE(h) RT_CUDA(cudaSetDevice((h)->device))
+
 extern "C" {
 
 const char* rttda_last_error(void) { return g_err.c_str(); }
@@ -79,7 +82,7 @@ int rttda_create(rttda_handle_t* out, const rttda_basis_t* basis, int32_t nao, i
     }
     Handle* h = new (std::nothrow) Handle();
     if (!h) { set_error("rttda_create: out of host memory"); return RTTDA_ENOMEM; }
-    RT_CUDA(cudaGetDevice(&h->device));
+    if (cudaGetDevice(&h->device) != cudaSuccess) { delete h; set_error("rttda_create: cudaGetDevice failed"); return RTTDA_ECUDA; }
     h->nao = nao; h->nocc = nocc; h->nvirt = nvirt; h->ncsf = nocc * nvirt;
     h->cx = cx; h->tau = schwarz_tau;
     const int r = create_impl(h, basis, C_occ, C_virt, eps, (cudaStream_t)stream);
@@ -92,11 +95,16 @@ int rttda_destroy(rttda_handle_t hh)
 {
     Handle* h = (Handle*)hh;
     if (!h) return RTTDA_OK;
+    cudaSetDevice(h->device);
     cudaDeviceSynchronize();
     for (void* p : h->dev_allocs) cudaFree(p);
-    for (double* p : {h->wsY, h->wsT, h->wsF, h->wsZ, h->wsP, h->prop_ws, h->eri_buf[0], h->eri_buf[1], h->eri_all}) if (p) cudaFree(p);
-    if (h->st_eval) cudaStreamDestroy(h->st_eval);
-    for (cudaEvent_t e : {h->ev_fork, h->ev_E[0], h->ev_E[1], h->ev_D[0], h->ev_D[1]}) if (e) cudaEventDestroy(e);
+    for (double* p : {h->wsY, h->wsT, h->wsF, h->wsZ, h->wsP, h->prop_ws, h->eri_all}) if (p) cudaFree(p);
+    for (int l = 0; l < Handle::MAXLANES; ++l) {
+        if (h->eri_buf[l]) cudaFree(h->eri_buf[l]);
+        if (h->lane_st[l]) cudaStreamDestroy(h->lane_st[l]);
+        if (h->lane_ev[l]) cudaEventDestroy(h->lane_ev[l]);
+    }
+    if (h->ev_fork) cudaEventDestroy(h->ev_fork);
     for (auto& e : h->ev) if (e) cudaEventDestroy(e);
     for (auto& e : h->jk_ev) cudaEventDestroy(e);
     delete h;
@@ -107,6 +115,7 @@ int rttda_sigma(rttda_handle_t hh, int32_t nvec, const double* X, double* sigma,
 {
     Handle* h = (Handle*)hh;
     RT_CHECK(h && X && sigma, "rttda_sigma: NULL pointer");
+    RT_DEVICE(h);
     RT_CHECK(nvec >= 1, "rttda_sigma: nvec < 1");
     RT_CHECK(X != sigma, "rttda_sigma: X and sigma must not alias");
     return sigma_impl(h, nvec, X, h->ncsf, sigma, h->ncsf, (cudaStream_t)stream);
@@ -116,6 +125,7 @@ int rttda_sigma_host(rttda_handle_t hh, int32_t nvec, const double* X, double* s
 {
     Handle* h = (Handle*)hh;
     RT_CHECK(h && X && sigma, "rttda_sigma_host: NULL pointer");
+    RT_DEVICE(h);
     RT_CHECK(nvec >= 1, "rttda_sigma_host: nvec < 1");
     cudaStream_t st = (cudaStream_t)stream;
     const size_t n = (size_t)nvec * h->ncsf;
@@ -131,6 +141,7 @@ int rttda_fock(rttda_handle_t hh, int32_t nvec, const double* T, double* F, void
 {
     Handle* h = (Handle*)hh;
     RT_CHECK(h && T && F, "rttda_fock: NULL pointer");
+    RT_DEVICE(h);
     RT_CHECK(nvec >= 1, "rttda_fock: nvec < 1");
     cudaStream_t st = (cudaStream_t)stream;
     const long long nn = (long long)h->nao * h->nao;
@@ -159,6 +170,7 @@ int rttda_propagate(rttda_handle_t hh, int32_t ntraj, double* C, const rttda_fie
 {
     Handle* h = (Handle*)hh;
     RT_CHECK(h && C && fields, "rttda_propagate: NULL pointer");
+    RT_DEVICE(h);
     RT_CHECK(ntraj >= 1 && ntraj <= 8, "rttda_propagate: ntraj must be in 1..8");
     RT_CHECK(nsteps >= 0, "rttda_propagate: negative step count");
     for (int t = 0; t < ntraj; ++t)
@@ -171,6 +183,7 @@ int rttda_propagate_sso(rttda_handle_t hh, int32_t ntraj, double* C, const rttda
 {
     Handle* h = (Handle*)hh;
     RT_CHECK(h && C && fields, "rttda_propagate_sso: NULL pointer");
+    RT_DEVICE(h);
     RT_CHECK(ntraj >= 1 && ntraj <= 8, "rttda_propagate_sso: ntraj must be in 1..8");
     RT_CHECK(nsteps >= 0, "rttda_propagate_sso: negative step count");
     for (int t = 0; t < ntraj; ++t)
@@ -183,6 +196,7 @@ int rttda_propagate_host(rttda_handle_t hh, int32_t ntraj, double* C, const rttd
 {
     Handle* h = (Handle*)hh;
     RT_CHECK(h && C && fields, "rttda_propagate_host: NULL pointer");
+    RT_DEVICE(h);
     RT_CHECK(ntraj >= 1 && ntraj <= 8 && nsteps >= 0, "rttda_propagate_host: bad ntraj / nsteps");
     cudaStream_t st = (cudaStream_t)stream;
     const size_t ns = (size_t)ntraj * 2 * ((size_t)h->ncsf + 1), nl = (size_t)nsteps * ntraj * 3;
@@ -199,6 +213,7 @@ int rttda_lanczos(rttda_handle_t hh, int32_t m, const double* v0, double* alpha,
 {
     Handle* h = (Handle*)hh;
     RT_CHECK(h && v0 && alpha && beta && V, "rttda_lanczos: NULL pointer");
+    RT_DEVICE(h);
     RT_CHECK(m >= 1 && m < h->ncsf, "rttda_lanczos: need 1 <= m < nocc*nvirt");
     RT_CHECK(v0 < V || v0 >= V + (size_t)(m + 1) * h->ncsf, "rttda_lanczos: v0 must not alias V");
     return lanczos_impl(h, m, v0, alpha, beta, V, (cudaStream_t)stream);
@@ -209,6 +224,7 @@ int rttda_populations(rttda_handle_t hh, int32_t ntraj, const double* C, int32_t
 {
     Handle* h = (Handle*)hh;
     RT_CHECK(h && C && Xs && P, "rttda_populations: NULL pointer");
+    RT_DEVICE(h);
     RT_CHECK(ntraj >= 1 && nstates >= 1, "rttda_populations: ntraj and nstates must be positive");
     return populations_impl(h, ntraj, C, nstates, Xs, P, (cudaStream_t)stream);
 }
@@ -229,6 +245,7 @@ int rttda_set_option(rttda_handle_t hh, int32_t option, double value)
 {
     Handle* h = (Handle*)hh;
     RT_CHECK(h != nullptr, "rttda_set_option: NULL handle");
+    RT_DEVICE(h);
     RT_CHECK(option == RTTDA_OPT_INCORE, "rttda_set_option: unknown option");
     const bool on = value != 0.0;
     if (on && !h->incore) {
@@ -254,6 +271,7 @@ int rttda_last_timings(rttda_handle_t hh, double* ms)
 {
     Handle* h = (Handle*)hh;
     RT_CHECK(h && ms, "rttda_last_timings: NULL pointer");
+    RT_DEVICE(h);
     RT_CHECK(h->ev_valid, "rttda_last_timings: no sigma/fock call yet");
     RT_CUDA(cudaEventSynchronize(h->ev[3]));
     float a = 0, b = 0, c = 0;
@@ -268,6 +286,7 @@ int rttda_jk_time(rttda_handle_t hh, double* sum_ms, double* count)
 {
     Handle* h = (Handle*)hh;
     RT_CHECK(h && sum_ms && count, "rttda_jk_time: NULL pointer");
+    RT_DEVICE(h);
     double tot = 0.0;
     const size_t n = h->jk_ev_used / 2;
     for (size_t i = 0; i < n; ++i) {
@@ -285,6 +304,7 @@ int rttda_profile_pass(rttda_handle_t hh, int32_t nvec, double* rows, int32_t ca
 {
     Handle* h = (Handle*)hh;
     RT_CHECK(h && rows && nrows && cap > 0, "rttda_profile_pass: bad arguments");
+    RT_DEVICE(h);
     RT_CHECK(nvec >= 1, "rttda_profile_pass: nvec < 1");
     const int nvt = padded_nvec(nvec);
     const size_t nn = (size_t)h->nao * h->nao;
@@ -293,6 +313,20 @@ int rttda_profile_pass(rttda_handle_t hh, int32_t nvec, double* rows, int32_t ca
     cudaStream_t st = (cudaStream_t)stream;
     RT_CUDA(cudaMemsetAsync(h->wsF, 0, nn * nvt * sizeof(double), st));
     return jk_profile(h, nvt, (nvec + 1) & ~1, h->wsT, h->wsF, st, rows, cap, nrows);
+}
+
+int rttda_gemm_f64(int32_t M, int32_t N, int32_t K, int32_t batch, double alpha, const double* A, int64_t sam, int64_t sak,
+                   int64_t sabatch, const double* B, int64_t sbk, int64_t sbn, int64_t sbbatch, double beta, double* C,
+                   int64_t scm, int64_t scn, int64_t scbatch, void* stream)
+{
+    RT_CHECK(M >= 0 && N >= 0 && K >= 0 && batch >= 0, "rttda_gemm_f64: negative size");
+    RT_CHECK(A && B && C, "rttda_gemm_f64: NULL pointer");
+    GemmDesc g{};
+    g.M = M; g.N = N; g.K = K; g.batch = batch; g.alpha = alpha; g.beta = beta;
+    g.A = A; g.sam = sam; g.sak = sak; g.sabatch = sabatch;
+    g.B = B; g.sbk = sbk; g.sbn = sbn; g.sbbatch = sbbatch;
+    g.C = C; g.scm = scm; g.scn = scn; g.scbatch = scbatch;
+    return gemm_f64(g, (cudaStream_t)stream);
 }
 
 int rttda_fp64_peak(double seconds, double* tflops, void* stream)

@@ -150,22 +150,34 @@ struct Handle {
     JKTables tabs{};
     std::vector<JKLaunch> launches;
     std::vector<Segment> segments;
-    // HBM staging buffers (double-buffered: evaluation of segment k+1 overlaps digestion of segment k)
-    double* eri_buf[2] = {nullptr, nullptr};
-    size_t eri_buf_n[2] = {0, 0};              // doubles allocated
+    // HBM staging buffers: the segments are dealt to `nlanes` lanes (setup.cu, longest first onto the least loaded
+    // lane); a lane owns one stream and one buffer of the size of its largest segment and runs evaluate -> digest ->
+    // evaluate -> ... for its segments, so kernels of different lanes overlap (the FP64-bound evaluation of one
+    // segment beside the L1/L2-bound digestion of another, and each other's tails).
+    static constexpr int MAXLANES = 8;
+    int nlanes = 0;
+    std::vector<int> lane_segs[MAXLANES];
+    double* eri_buf[MAXLANES] = {nullptr};
+    size_t eri_buf_n[MAXLANES] = {0};          // doubles allocated
+    size_t lane_need[MAXLANES] = {0};          // doubles needed by the lane's largest segment
     size_t eri_buf_need = 0;                   // doubles needed by the largest segment
+    cudaStream_t lane_st[MAXLANES] = {nullptr};
+    cudaEvent_t lane_ev[MAXLANES] = {nullptr};
+    cudaEvent_t ev_fork = nullptr;
     // optional in-core mode (rttda_set_option): all segments' integrals kept in HBM after the first pass
     bool incore = false, incore_valid = false;
     double* eri_all = nullptr;
     size_t eri_all_n = 0, eri_all_need = 0;
-    cudaStream_t st_eval = nullptr;            // evaluation kernels run here, digestion on the caller's stream
-    cudaEvent_t ev_fork = nullptr, ev_E[2] = {nullptr, nullptr}, ev_D[2] = {nullptr, nullptr};
     std::vector<void*> dev_allocs;             // everything to free
     // workspaces (grown on demand)
     double *wsY = nullptr, *wsT = nullptr, *wsF = nullptr, *wsZ = nullptr, *wsP = nullptr;
     size_t wsY_n = 0, wsT_n = 0, wsF_n = 0, wsZ_n = 0, wsP_n = 0;
     double* prop_ws = nullptr;
     size_t prop_ws_n = 0;
+    // propagator state kept across calls: polarisations of the cached D_d matrices, reference state of R(t)
+    bool dd_valid = false;
+    int dd_ntraj = 0, yref_ntraj = 0;
+    double dd_dir[8][3] = {{0}};
     // info
     double info[16] = {0};
     long long kernel_launches = 0;
@@ -176,7 +188,8 @@ struct Handle {
     size_t jk_ev_used = 0;
 };
 
-int jk_mark(Handle* h, cudaStream_t st);   // record the next event of the J/K timing log
+int jk_mark(Handle* h, cudaStream_t st);
+int assign_lanes(Handle* h, int nlanes);   // record the next event of the J/K timing log
 
 // jk_eval.cu / jk_digest.cu
 // F += 2 J[T] - cx K[T] for all nvt (even) interleaved densities; F zeroed by the caller.

@@ -745,15 +745,19 @@ __global__ void symsplit_kernel(int nao, int nvt, const double* __restrict__ T, 
     PP[i] = make_double2(a + b, a - b);
 }
 
-// One ERI pass: for every segment, evaluate its quartets once into a staging buffer (stream st_eval), then digest
-// them for all densities (caller's stream).  Two buffers: the FP64-bound evaluation of segment k+1 overlaps the
-// L1/L2-bound digestion of segment k.  Fq must be zeroed by the caller; densities [0, nvec) of the nvt slots per
+// One ERI pass: every segment is evaluated once into the staging buffer of its lane and then digested for all
+// densities on the lane's stream; the lanes (Handle::lane_*) run side by side and join the caller's stream at the end
+// (the Fock updates are atomic adds, so the lanes need no ordering among themselves).  Small molecules, whose kernels
+// do not fill the GPU, run 8 lanes; large ones run the two-buffer pipeline below.  Fq must be zeroed by the caller; densities [0, nvec) of the nvt slots per
 // element are processed (nvec even, nvt a multiple of 2 with 16-byte aligned slots).
 int jk_build(Handle* h, int nvt, int nvec, const double* Tq, double* Fq, cudaStream_t st)
 {
     RT_CHECK(nvec >= 2 && nvec % 2 == 0 && nvt >= nvec && nvt % 2 == 0, "jk_build: bad density slot counts");
-    if (!h->incore)
-        for (int b = 0; b < 2; ++b) RT_TRY(ensure_ws(h, &h->eri_buf[b], &h->eri_buf_n[b], h->eri_buf_need));
+    if (!h->incore) {
+        for (int l = 0; l < h->nlanes; ++l) RT_TRY(ensure_ws(h, &h->eri_buf[l], &h->eri_buf_n[l], h->lane_need[l]));
+        if (h->nlanes == 0)
+            for (int b = 0; b < 2; ++b) RT_TRY(ensure_ws(h, &h->eri_buf[b], &h->eri_buf_n[b], h->eri_buf_need));
+    }
     {                                   // the exchange kernel gathers {Ps, Pa} pairs: one 16-byte load per (T_mn, T_nm)
         const long long n = (long long)h->nao * h->nao * nvt;
         RT_TRY(ensure_ws(h, &h->wsP, &h->wsP_n, (size_t)2 * n));
@@ -775,20 +779,42 @@ int jk_build(Handle* h, int nvt, int nvec, const double* Tq, double* Fq, cudaStr
         h->incore_valid = true;
         return RTTDA_OK;
     }
+    if (h->nlanes == 0) {
+        // Pipeline mode (large molecules: every kernel fills the GPU on its own, and two kernels of the same kind
+        // running side by side only fight over the FP64 pipe or over L1/L2): segments in order, evaluation of
+        // segment k+1 on lane_st[0] beside the digestion of segment k on the caller's stream, two buffers.
+        cudaStream_t se = h->lane_st[0];
+        cudaEvent_t *evE = h->lane_ev, *evD = h->lane_ev + 2;
+        RT_CUDA(cudaEventRecord(h->ev_fork, st));
+        RT_CUDA(cudaStreamWaitEvent(se, h->ev_fork, 0));
+        int k = 0;
+        for (const Segment& sg : h->segments) {
+            if (sg.nitems == 0) continue;
+            const int b = k & 1;
+            if (k >= 2) RT_CUDA(cudaStreamWaitEvent(se, evD[b], 0));
+            RT_TRY(eval_segment(h, sg, h->eri_buf[b], se));
+            RT_CUDA(cudaEventRecord(evE[b], se));
+            RT_CUDA(cudaStreamWaitEvent(st, evE[b], 0));
+            for (int l = sg.first_launch; l < sg.first_launch + sg.nlaunch; ++l)
+                RT_TRY(digest_launch(h, h->launches[l], sg, h->eri_buf[b], nvt, nvec, Tq, Fq, st));
+            RT_CUDA(cudaEventRecord(evD[b], st));
+            ++k;
+        }
+        return RTTDA_OK;
+    }
     RT_CUDA(cudaEventRecord(h->ev_fork, st));
-    RT_CUDA(cudaStreamWaitEvent(h->st_eval, h->ev_fork, 0));
-    int k = 0;
-    for (const Segment& sg : h->segments) {
-        if (sg.nitems == 0) continue;
-        const int b = k & 1;
-        if (k >= 2) RT_CUDA(cudaStreamWaitEvent(h->st_eval, h->ev_D[b], 0));
-        RT_TRY(eval_segment(h, sg, h->eri_buf[b], h->st_eval));
-        RT_CUDA(cudaEventRecord(h->ev_E[b], h->st_eval));
-        RT_CUDA(cudaStreamWaitEvent(st, h->ev_E[b], 0));
-        for (int l = sg.first_launch; l < sg.first_launch + sg.nlaunch; ++l)
-            RT_TRY(digest_launch(h, h->launches[l], sg, h->eri_buf[b], nvt, nvec, Tq, Fq, st));
-        RT_CUDA(cudaEventRecord(h->ev_D[b], st));
-        ++k;
+    for (int l = 0; l < h->nlanes; ++l) {
+        if (h->lane_segs[l].empty()) continue;
+        cudaStream_t ls = h->lane_st[l];
+        RT_CUDA(cudaStreamWaitEvent(ls, h->ev_fork, 0));
+        for (int si : h->lane_segs[l]) {
+            const Segment& sg = h->segments[si];
+            RT_TRY(eval_segment(h, sg, h->eri_buf[l], ls));
+            for (int k = sg.first_launch; k < sg.first_launch + sg.nlaunch; ++k)
+                RT_TRY(digest_launch(h, h->launches[k], sg, h->eri_buf[l], nvt, nvec, Tq, Fq, ls));
+        }
+        RT_CUDA(cudaEventRecord(h->lane_ev[l], ls));
+        RT_CUDA(cudaStreamWaitEvent(st, h->lane_ev[l], 0));
     }
     return RTTDA_OK;
 }
@@ -799,7 +825,7 @@ int jk_build(Handle* h, int nvt, int nvec, const double* Tq, double* Fq, cudaStr
 // blocks, digestion launches, 0}.
 int jk_profile(Handle* h, int nvt, int nvec, const double* Tq, double* Fq, cudaStream_t st, double* rows, int cap, int* nrows)
 {
-    for (int b = 0; b < 2; ++b) RT_TRY(ensure_ws(h, &h->eri_buf[b], &h->eri_buf_n[b], h->eri_buf_need));
+    RT_TRY(ensure_ws(h, &h->eri_buf[0], &h->eri_buf_n[0], h->eri_buf_need));
     const long long n = (long long)h->nao * h->nao * nvt;
     RT_TRY(ensure_ws(h, &h->wsP, &h->wsP_n, (size_t)2 * n));
     symsplit_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(h->nao, nvt, Tq, reinterpret_cast<double2*>(h->wsP));

@@ -266,46 +266,80 @@ observe_kernel(long long n1, const double* __restrict__ y, const double* __restr
     }
 }
 
-int propagate_impl(Handle* h, int ntraj, double* y, const rttda_field_t* fields, double t_start, double dt,
-                   int nsteps, double* log, cudaStream_t st)
+// Common prologue of both propagators: workspace carving, D_d = sum_k d_k D^k per trajectory (recomputed only when the
+// polarisations change), the linearised delta kick (R8) and the reference state of R(t).  A field record with
+// RTTDA_FIELD_CONTINUE set marks a CONTINUED run: no kick, and R(t) stays relative to the reference state of the
+// previous call on this handle (which must have had the same ntraj).
+struct PropWs {
+    double *ys, *hy, *ksum, *yref, *Dd_oo, *Dd_vv, *Dd_ov;
+    FieldArgs fa;
+    unsigned eg;
+};
+
+static int prop_prologue(Handle* h, int ntraj, double* y, const rttda_field_t* fields, PropWs& w, cudaStream_t st)
 {
     const size_t no = h->nocc, nv = h->nvirt, ncsf = h->ncsf, n1 = ncsf + 1;
     const size_t nstate = (size_t)ntraj * 2 * n1;
     const size_t need = 4 * nstate + (size_t)ntraj * (no * no + nv * nv + no * nv);
+    if (h->prop_ws_n < need) { h->dd_valid = false; h->yref_ntraj = 0; }
     RT_TRY(ensure_ws(h, &h->prop_ws, &h->prop_ws_n, need));
-    double* ys = h->prop_ws;
-    double* hy = ys + nstate;
-    double* ksum = hy + nstate;
-    double* yref = ksum + nstate;
-    double* Dd_oo = yref + nstate;
-    double* Dd_vv = Dd_oo + (size_t)ntraj * no * no;
-    double* Dd_ov = Dd_vv + (size_t)ntraj * nv * nv;
-    FieldArgs fa{};
+    w.ys = h->prop_ws;
+    w.hy = w.ys + nstate;
+    w.ksum = w.hy + nstate;
+    w.yref = w.ksum + nstate;
+    w.Dd_oo = w.yref + nstate;
+    w.Dd_vv = w.Dd_oo + (size_t)ntraj * no * no;
+    w.Dd_ov = w.Dd_vv + (size_t)ntraj * nv * nv;
+    w.fa = FieldArgs{};
+    w.eg = (unsigned)((n1 * ntraj + 255) / 256);
+    bool same_dirs = h->dd_valid && h->dd_ntraj == ntraj;
+    for (int t = 0; t < ntraj && same_dirs; ++t)
+        for (int k = 0; k < 3; ++k) same_dirs = same_dirs && (h->dd_dir[t][k] == fields[t].dir[k]);
     for (int t = 0; t < ntraj; ++t) {
         const double* d = fields[t].dir;
-        fa.D00[t] = d[0] * h->D_00[0] + d[1] * h->D_00[1] + d[2] * h->D_00[2];
+        w.fa.D00[t] = d[0] * h->D_00[0] + d[1] * h->D_00[1] + d[2] * h->D_00[2];
+        if (same_dirs) continue;
         const long long a = no * no, b = nv * nv, c = no * nv;
-        combine3_kernel<<<(unsigned)((a + 255) / 256), 256, 0, st>>>(a, h->D_oo, d[0], d[1], d[2], Dd_oo + t * a);
-        combine3_kernel<<<(unsigned)((b + 255) / 256), 256, 0, st>>>(b, h->D_vv, d[0], d[1], d[2], Dd_vv + t * b);
-        combine3_kernel<<<(unsigned)((c + 255) / 256), 256, 0, st>>>(c, h->D_ov, d[0], d[1], d[2], Dd_ov + t * c);
+        combine3_kernel<<<(unsigned)((a + 255) / 256), 256, 0, st>>>(a, h->D_oo, d[0], d[1], d[2], w.Dd_oo + t * a);
+        combine3_kernel<<<(unsigned)((b + 255) / 256), 256, 0, st>>>(b, h->D_vv, d[0], d[1], d[2], w.Dd_vv + t * b);
+        combine3_kernel<<<(unsigned)((c + 255) / 256), 256, 0, st>>>(c, h->D_ov, d[0], d[1], d[2], w.Dd_ov + t * c);
         h->kernel_launches += 3;
+        for (int k = 0; k < 3; ++k) h->dd_dir[t][k] = d[k];
     }
     RT_CUDA(cudaGetLastError());
-    const unsigned eg = (unsigned)((n1 * ntraj + 255) / 256);
-    // delta kick at t_start (R8)
+    h->dd_valid = true; h->dd_ntraj = ntraj;
+    bool cont = false;
+    for (int t = 0; t < ntraj; ++t) cont = cont || (fields[t].flags & RTTDA_FIELD_CONTINUE);
+    if (cont) {
+        RT_CHECK(h->yref_ntraj == ntraj, "propagate: RTTDA_FIELD_CONTINUE without a previous call of the same ntraj on this handle");
+        return RTTDA_OK;
+    }
     bool any_kick = false;
     for (int t = 0; t < ntraj; ++t) {
-        fa.E[t] = fields[t].type == RTTDA_DELTA ? fields[t].E0 : 0.0;
-        any_kick |= fa.E[t] != 0.0;
+        w.fa.E[t] = fields[t].type == RTTDA_DELTA ? fields[t].E0 : 0.0;
+        any_kick |= w.fa.E[t] != 0.0;
     }
     if (any_kick) {
-        RT_CUDA(cudaMemsetAsync(hy, 0, nstate * sizeof(double), st));
-        RT_TRY(apply_field(h, ntraj, y, hy, Dd_oo, Dd_vv, Dd_ov, fa, st));
-        kick_kernel<<<eg, 256, 0, st>>>((long long)n1, ntraj, hy, y, fa);
+        RT_CUDA(cudaMemsetAsync(w.hy, 0, nstate * sizeof(double), st));
+        RT_TRY(apply_field(h, ntraj, y, w.hy, w.Dd_oo, w.Dd_vv, w.Dd_ov, w.fa, st));
+        kick_kernel<<<w.eg, 256, 0, st>>>((long long)n1, ntraj, w.hy, y, w.fa);
         RT_CUDA(cudaGetLastError());
         h->kernel_launches++;
     }
-    RT_CUDA(cudaMemcpyAsync(yref, y, nstate * sizeof(double), cudaMemcpyDeviceToDevice, st));
+    RT_CUDA(cudaMemcpyAsync(w.yref, y, nstate * sizeof(double), cudaMemcpyDeviceToDevice, st));
+    h->yref_ntraj = ntraj;
+    return RTTDA_OK;
+}
+
+int propagate_impl(Handle* h, int ntraj, double* y, const rttda_field_t* fields, double t_start, double dt,
+                   int nsteps, double* log, cudaStream_t st)
+{
+    const size_t n1 = (size_t)h->ncsf + 1;
+    PropWs w;
+    RT_TRY(prop_prologue(h, ntraj, y, fields, w, st));
+    double *ys = w.ys, *hy = w.hy, *ksum = w.ksum, *yref = w.yref, *Dd_oo = w.Dd_oo, *Dd_vv = w.Dd_vv, *Dd_ov = w.Dd_ov;
+    FieldArgs& fa = w.fa;
+    const unsigned eg = w.eg;
 
     const double ts_off[4] = {0.0, 0.5, 0.5, 1.0};
     const double wgt[4] = {1.0, 2.0, 2.0, 1.0};
@@ -351,40 +385,13 @@ __global__ void plane_axpy_kernel(long long n1, int ntraj, double c, const doubl
 int propagate_sso_impl(Handle* h, int ntraj, double* y, const rttda_field_t* fields, double t_start, double dt,
                        int nsteps, double* log, cudaStream_t st)
 {
-    const size_t no = h->nocc, nv = h->nvirt, ncsf = h->ncsf, n1 = ncsf + 1;
+    const size_t n1 = (size_t)h->ncsf + 1;
     const size_t nstate = (size_t)ntraj * 2 * n1;
-    const size_t need = 4 * nstate + (size_t)ntraj * (no * no + nv * nv + no * nv);
-    RT_TRY(ensure_ws(h, &h->prop_ws, &h->prop_ws_n, need));
-    double* hy = h->prop_ws + nstate;              // same carving as propagate_impl
-    double* yref = h->prop_ws + 3 * nstate;
-    double* Dd_oo = yref + nstate;
-    double* Dd_vv = Dd_oo + (size_t)ntraj * no * no;
-    double* Dd_ov = Dd_vv + (size_t)ntraj * nv * nv;
-    FieldArgs fa{};
-    for (int t = 0; t < ntraj; ++t) {
-        const double* d = fields[t].dir;
-        fa.D00[t] = d[0] * h->D_00[0] + d[1] * h->D_00[1] + d[2] * h->D_00[2];
-        const long long a = no * no, b = nv * nv, c = no * nv;
-        combine3_kernel<<<(unsigned)((a + 255) / 256), 256, 0, st>>>(a, h->D_oo, d[0], d[1], d[2], Dd_oo + t * a);
-        combine3_kernel<<<(unsigned)((b + 255) / 256), 256, 0, st>>>(b, h->D_vv, d[0], d[1], d[2], Dd_vv + t * b);
-        combine3_kernel<<<(unsigned)((c + 255) / 256), 256, 0, st>>>(c, h->D_ov, d[0], d[1], d[2], Dd_ov + t * c);
-        h->kernel_launches += 3;
-    }
-    RT_CUDA(cudaGetLastError());
-    const unsigned eg = (unsigned)((n1 * ntraj + 255) / 256);
-    bool any_kick = false;
-    for (int t = 0; t < ntraj; ++t) {
-        fa.E[t] = fields[t].type == RTTDA_DELTA ? fields[t].E0 : 0.0;
-        any_kick |= fa.E[t] != 0.0;
-    }
-    if (any_kick) {
-        RT_CUDA(cudaMemsetAsync(hy, 0, nstate * sizeof(double), st));
-        RT_TRY(apply_field(h, ntraj, y, hy, Dd_oo, Dd_vv, Dd_ov, fa, st));
-        kick_kernel<<<eg, 256, 0, st>>>((long long)n1, ntraj, hy, y, fa);
-        RT_CUDA(cudaGetLastError());
-        h->kernel_launches++;
-    }
-    RT_CUDA(cudaMemcpyAsync(yref, y, nstate * sizeof(double), cudaMemcpyDeviceToDevice, st));
+    PropWs w;
+    RT_TRY(prop_prologue(h, ntraj, y, fields, w, st));
+    double *hy = w.hy, *yref = w.yref, *Dd_oo = w.Dd_oo, *Dd_vv = w.Dd_vv, *Dd_ov = w.Dd_ov;
+    FieldArgs& fa = w.fa;
+    const unsigned eg = w.eg;
 
     // hy[:, plane, :] = H(t) y[:, plane, :]; the other plane of hy is scratch of the field kernels
     auto apply_H = [&](int plane, double t) -> int {

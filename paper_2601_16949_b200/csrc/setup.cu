@@ -4,6 +4,7 @@
 #include <algorithm>
 #include <chrono>
 #include <cmath>
+#include <cstdlib>
 #include <cstring>
 #include <map>
 #include <numeric>
@@ -42,7 +43,7 @@ void boys_table_host(int L, std::vector<double>& tab)
 // ---------------------------------------------------------------------------------------------- basis
 struct HostBasis {
     int nshells = 0, nao = 0;
-    std::vector<int> l, np, off, ao, center;
+    std::vector<int> l, np, np_true, off, ao, center;   // np: primitives stored (2 is padded to 3), np_true: as given
     std::vector<double> ex, cf;          // cf: final coefficient of the bare primitive
     std::vector<double> xyz;             // [ncenters][3]
 };
@@ -59,7 +60,10 @@ static int load_basis(const rttda_basis_t* b, HostBasis& H)
         RT_CHECK(sh.l == 0 || sh.l == 1, "basis: only s and p shells are supported");
         RT_CHECK(sh.nprim >= 1 && sh.nprim <= RTTDA_MAX_NPRIM, "basis: nprim out of range");
         RT_CHECK(sh.center >= 0 && sh.center < b->ncenters, "basis: bad centre index");
-        H.l.push_back(sh.l); H.np.push_back(sh.nprim); H.off.push_back((int)H.ex.size());
+        // Contraction depths 1 and 3 have their own kernel instantiations; a 2-primitive shell is carried as a
+        // 3-primitive shell whose third primitive has coefficient zero (same integrals, some idle arithmetic).
+        const int np_store = sh.nprim == 2 ? 3 : sh.nprim;
+        H.l.push_back(sh.l); H.np.push_back(np_store); H.np_true.push_back(sh.nprim); H.off.push_back((int)H.ex.size());
         H.center.push_back(sh.center); H.ao.push_back(ao);
         ao += 2 * sh.l + 1;
         // Primitives are taken in order of ascending exponent: the contraction sums do not depend on the order, but
@@ -90,6 +94,7 @@ static int load_basis(const rttda_basis_t* b, HostBasis& H)
             }
         RT_CHECK(self > 0.0, "basis: contracted function has zero norm");
         for (int k = 0; k < sh.nprim; ++k) H.cf.push_back(c[k] / std::sqrt(self));
+        if (np_store != sh.nprim) { H.ex.push_back(H.ex.back()); H.cf.push_back(0.0); }
     }
     H.nao = ao;
     return RTTDA_OK;
@@ -181,9 +186,15 @@ __global__ void shift_diag_kernel(int n, double c, double* __restrict__ A)
     if (i < n) A[(size_t)i * n + i] += c;
 }
 
+struct DevTmp {                   // temporary device allocation, released on scope exit (error paths included)
+    void* p = nullptr;
+    ~DevTmp() { if (p) cudaFree(p); }
+};
+
 struct Pair {
     int s1, s2;          // first (higher l, or larger index at equal l), second
-    int pc, sub, np;     // pair class, contraction sub-class, primitive pairs
+    int pc, sub, np;     // pair class, contraction sub-class, primitive pairs (stored)
+    int np_true;         // primitive pairs as given (2-primitive shells are padded), for the R14 counters
     int row;             // first row in the per-class candidate prim table
     double Q;
     int pos;             // position in its ket class after sorting
@@ -252,10 +263,8 @@ int create_impl(Handle* h, const rttda_basis_t* basis, const double* C_occ, cons
             if (H.l[s2] > H.l[s1]) std::swap(s1, s2);
             Pair P;
             P.s1 = s1; P.s2 = s2; P.pc = H.l[s1] + H.l[s2]; P.np = H.np[s1] * H.np[s2];
-            RT_CHECK(P.np == 1 || P.np == 3 || P.np == 9 || P.np == 2 || P.np == 4 || P.np == 6,
-                     "unsupported contraction depth");
-            RT_CHECK(P.np == 1 || P.np == 3 || P.np == 9,
-                     "contraction depths other than 1 and 3 primitives per shell are not supported yet");
+            P.np_true = H.np_true[s1] * H.np_true[s2];
+            RT_CHECK(P.np == 1 || P.np == 3 || P.np == 9, "unsupported contraction depth");
             P.sub = np_to_sub(P.np);
             const size_t before = rows[P.pc].size();
             prim_rows(H, s1, s2, rows[P.pc]);
@@ -277,12 +286,13 @@ int create_impl(Handle* h, const rttda_basis_t* basis, const double* C_occ, cons
     for (int pc = 0; pc < 3; ++pc) {
         const int n = (int)cand_np[pc].size();
         if (!n) continue;
-        int *d_np = nullptr, *d_off = nullptr;
-        double *d_prim = nullptr, *d_Q = nullptr;
-        RT_CUDA(cudaMalloc(&d_np, n * sizeof(int)));
-        RT_CUDA(cudaMalloc(&d_off, n * sizeof(int)));
-        RT_CUDA(cudaMalloc(&d_prim, rows[pc].size() * sizeof(double)));
-        RT_CUDA(cudaMalloc(&d_Q, n * sizeof(double)));
+        DevTmp t_np, t_off, t_prim, t_Q;                         // freed on every return path
+        RT_CUDA(cudaMalloc(&t_np.p, n * sizeof(int)));
+        RT_CUDA(cudaMalloc(&t_off.p, n * sizeof(int)));
+        RT_CUDA(cudaMalloc(&t_prim.p, rows[pc].size() * sizeof(double)));
+        RT_CUDA(cudaMalloc(&t_Q.p, n * sizeof(double)));
+        int *d_np = (int*)t_np.p, *d_off = (int*)t_off.p;
+        double *d_prim = (double*)t_prim.p, *d_Q = (double*)t_Q.p;
         RT_CUDA(cudaMemcpyAsync(d_np, cand_np[pc].data(), n * sizeof(int), cudaMemcpyHostToDevice, st));
         RT_CUDA(cudaMemcpyAsync(d_off, cand_off[pc].data(), n * sizeof(int), cudaMemcpyHostToDevice, st));
         RT_CUDA(cudaMemcpyAsync(d_prim, rows[pc].data(), rows[pc].size() * sizeof(double), cudaMemcpyHostToDevice, st));
@@ -292,7 +302,6 @@ int create_impl(Handle* h, const rttda_basis_t* basis, const double* C_occ, cons
         RT_CUDA(cudaMemcpyAsync(Q.data(), d_Q, n * sizeof(double), cudaMemcpyDeviceToHost, st));
         RT_CUDA(cudaStreamSynchronize(st));
         for (int k = 0; k < n; ++k) pairs[cand_id[pc][k]].Q = Q[k];
-        cudaFree(d_np); cudaFree(d_off); cudaFree(d_prim); cudaFree(d_Q);
     }
     double Qmax = 0.0;
     for (const Pair& P : pairs) Qmax = std::max(Qmax, P.Q);
@@ -484,6 +493,12 @@ int create_impl(Handle* h, const rttda_basis_t* basis, const double* C_occ, cons
     // ---- R14 counts: unique quartets with Q_ab Q_cd >= tau, and the flop model on them
     {
         double ordered = 0, ordered_prim = 0, diag = 0, diag_prim = 0, fl_ord = 0, fl_diag = 0, nint_ord = 0, nint_diag = 0;
+        // primitive counts as GIVEN (a padded 2-primitive shell counts 2): prefix sums over each sorted class list
+        std::vector<std::vector<double>> pre(NKETCLASS);
+        for (int kc = 0; kc < NKETCLASS; ++kc) {
+            pre[kc].assign(cls[kc].size() + 1, 0.0);
+            for (size_t q = 0; q < cls[kc].size(); ++q) pre[kc][q + 1] = pre[kc][q] + pairs[cls[kc][q]].np_true;
+        }
         for (int kc1 = 0; kc1 < NKETCLASS; ++kc1)
             for (int k : cls[kc1]) {
                 const Pair& P = pairs[k];
@@ -491,15 +506,15 @@ int create_impl(Handle* h, const rttda_basis_t* basis, const double* C_occ, cons
                 for (int kc2 = 0; kc2 < NKETCLASS; ++kc2) {
                     const int n2 = tau > 0.0 ? count_prod_ge(kc2, P.Q) : h->tabs.kets[kc2].n;
                     const int pc2 = kc2 / NSUB, l3 = pc2 >= 1, l4 = pc2 == 2;
-                    const double npq = (double)P.np * h->tabs.kets[kc2].np;
+                    const double npq = (double)P.np_true * pre[kc2][n2];       // primitive quartets of these n2 quartets
                     ordered += n2;
-                    ordered_prim += n2 * npq;
-                    fl_ord += n2 * npq * flops_prim(l1, l2, l3, l4);
+                    ordered_prim += npq;
+                    fl_ord += npq * flops_prim(l1, l2, l3, l4);
                     nint_ord += (double)n2 * (2 * l1 + 1) * (2 * l2 + 1) * (2 * l3 + 1) * (2 * l4 + 1);
                 }
                 if (P.Q * P.Q >= tau) {
-                    diag += 1; diag_prim += (double)P.np * P.np;
-                    fl_diag += (double)P.np * P.np * flops_prim(l1, l2, l1, l2);
+                    diag += 1; diag_prim += (double)P.np_true * P.np_true;
+                    fl_diag += (double)P.np_true * P.np_true * flops_prim(l1, l2, l1, l2);
                     nint_diag += (double)(2 * l1 + 1) * (2 * l2 + 1) * (2 * l1 + 1) * (2 * l2 + 1);
                 }
             }
@@ -541,9 +556,10 @@ int create_impl(Handle* h, const rttda_basis_t* basis, const double* C_occ, cons
     RT_TRY(dalloc(&h->D_oo, 3 * no * no));
     RT_TRY(dalloc(&h->D_vv, 3 * nv * nv));
     RT_TRY(dalloc(&h->D_ov, 3 * no * nv));
-    double* tmp = nullptr;                      // D C_v | D C_o, [3][N][max(no,nv)]
+    DevTmp t_tmp;                               // D C_v | D C_o, [3][N][max(no,nv)]
     const size_t nm = std::max(no, nv);
-    RT_CUDA(cudaMalloc((void**)&tmp, 3 * N * nm * sizeof(double)));
+    RT_CUDA(cudaMalloc(&t_tmp.p, 3 * N * nm * sizeof(double)));
+    double* tmp = (double*)t_tmp.p;
     // tmp = D^k C_v ; D_vv = C_v^T tmp ; D_ov = C_o^T tmp ; then tmp = D^k C_o ; D_oo = C_o^T tmp
     GemmDesc g{};
     g.alpha = 1.0; g.beta = 0.0; g.batch = 3;
@@ -574,7 +590,6 @@ int create_impl(Handle* h, const rttda_basis_t* basis, const double* C_occ, cons
     std::vector<double> doo(3 * no * no);
     RT_CUDA(cudaMemcpyAsync(doo.data(), h->D_oo, doo.size() * sizeof(double), cudaMemcpyDeviceToHost, st));
     RT_CUDA(cudaStreamSynchronize(st));
-    cudaFree(tmp);
     // Dipole origin = electronic centroid of the ground state, c_k = tr(D_oo^k)/n_occ (R6): with orthonormal MOs the
     // shift r -> r - c is D_oo -> D_oo - c 1, D_vv -> D_vv - c 1, D_ov unchanged, and D_00 = 2 tr D_oo (R3: sum
     // over spin orbitals) becomes zero.  Without it D_00 grows with the molecule's distance from the coordinate
@@ -593,14 +608,46 @@ int create_impl(Handle* h, const rttda_basis_t* basis, const double* C_occ, cons
     RT_CUDA(cudaStreamSynchronize(st));
     h->kernel_launches += 6;
     for (auto& e : h->ev) RT_CUDA(cudaEventCreate(&e));
-    RT_CUDA(cudaStreamCreateWithFlags(&h->st_eval, cudaStreamNonBlocking));
     RT_CUDA(cudaEventCreateWithFlags(&h->ev_fork, cudaEventDisableTiming));
-    for (int b = 0; b < 2; ++b) {
-        RT_CUDA(cudaEventCreateWithFlags(&h->ev_E[b], cudaEventDisableTiming));
-        RT_CUDA(cudaEventCreateWithFlags(&h->ev_D[b], cudaEventDisableTiming));
+    for (int l = 0; l < Handle::MAXLANES; ++l) {
+        RT_CUDA(cudaStreamCreateWithFlags(&h->lane_st[l], cudaStreamNonBlocking));
+        RT_CUDA(cudaEventCreateWithFlags(&h->lane_ev[l], cudaEventDisableTiming));
+    }
+    {
+        // all integrals of one pass below 8 GB: the kernels are small, run 8 lanes side by side; else the pipeline
+        const char* e = getenv("RTTDA_LANES");
+        const int nl = e ? atoi(e) : ((double)h->eri_all_need * sizeof(double) < 8e9 ? Handle::MAXLANES : 0);
+        RT_TRY(assign_lanes(h, nl));
     }
     h->info[RTTDA_INFO_CREATE_MS] =
         std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - t0).count();
+    return RTTDA_OK;
+}
+
+// Deal the segments to `nlanes` lanes: longest estimated run time first, each onto the lane with the least work so far
+// (cost model: flop model of the evaluation + 40 flop-equivalents per stored integral for the gather-bound digestion).
+int assign_lanes(Handle* h, int nlanes)
+{
+    RT_CHECK(nlanes >= 0 && nlanes <= Handle::MAXLANES, "lanes must be in 0..8 (0 = two-buffer pipeline)");
+    std::vector<std::pair<double, int>> cost;
+    for (int i = 0; i < (int)h->segments.size(); ++i) {
+        const Segment& sg = h->segments[i];
+        if (sg.nitems == 0) continue;
+        const double npq = (double)sg.nquartets * h->tabs.kets[sg.kc_bra].np * h->tabs.kets[sg.kc_ket].np;
+        cost.push_back({npq * flops_prim(sg.la, sg.lb, sg.lc, sg.ld) + 40.0 * 6.0 * (double)sg.nquartets * sg.ni, i});
+    }
+    std::sort(cost.begin(), cost.end(), [](const auto& a, const auto& b) { return a.first > b.first; });
+    double load[Handle::MAXLANES] = {0};
+    for (int l = 0; l < Handle::MAXLANES; ++l) { h->lane_segs[l].clear(); h->lane_need[l] = 1; }
+    for (const auto& c : cost) {
+        int best = 0;
+        for (int l = 1; l < nlanes; ++l) if (load[l] < load[best]) best = l;
+        load[best] += c.first;
+        h->lane_segs[best].push_back(c.second);
+        const Segment& sg = h->segments[c.second];
+        h->lane_need[best] = std::max(h->lane_need[best], (size_t)sg.nbatch * sg.ni * 32);
+    }
+    h->nlanes = nlanes;
     return RTTDA_OK;
 }
 

@@ -1,0 +1,159 @@
+#!/usr/bin/env python
+"""Writes tests/golden/config{2,3,4}_trajectory_samples.txt: oracle amplitudes of the propagation configs.
+
+Calls only oracle/ and workloads/ (never the CUDA path).  The propagation is the oracle's RK4 (`tda.rk4_propagate`,
+eq. 1 / 14-16, R7) on y' = -i (A_ext + E(t) M_d) y; what differs per config is how A is applied:
+
+  config 2   dense A from the full AO tensor (`tda.build_A`), x/y/z delta kicks (R8), 2000 field-free steps of 0.1 au;
+  config 3   dense A by ket-pair blocks (`tda.build_A_by_pair_blocks`, route ii; 5.2 GB), cw field at the lowest
+             eigenvalue of A (R10: taken from 80 Lanczos steps of the oracle on the dense A, recorded in the file),
+             E0 in {0.005, 0.02}, 4000 steps of 0.05 au; amplitudes stored after steps 3, 400 and 4000;
+  config 4   dense A is 991 GB: ONE RK4 step through the matrix-free route (`tda.sigma_matrix_free`, 4 J/K passes serving
+             the 6 real vectors of the three trajectories, tau_oracle = 1e-14) from seeded random normalised complex
+             states at t = 95 au, i.e. near the maximum of the sin^2 envelope (R9), E0 in {0.01, 0.03, 0.05}, omega = 0.2 Ha
+             (any recorded omega serves parity).  The ground state at t = 0 would make this step trivial (E(0) = 0).
+
+All trajectories of a config advance side by side as columns of one array; the field amplitudes E0 differ per column,
+so E(t) is evaluated for E0 = 1 and the column's E0 is applied inside M_d.
+
+File format: '#' comments; 'meta key value'; 'amp traj step index re im' (index 0 = ground state, 1 + i*nvirt + a = singles);
+'norm traj step |y|^2'.
+
+    python tests/golden/make_trajectory_samples.py <2|3|4> [output file]
+"""
+import os
+import sys
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.dirname(os.path.dirname(os.path.abspath(__file__))))
+sys.path.insert(0, ROOT)
+from oracle import tda                      # noqa: E402
+from oracle.integrals import OracleBasis, num_threads  # noqa: E402
+from workloads import get_config, make_basis, make_mos, make_vectors  # noqa: E402
+
+NSAMP = 160
+
+
+def sample_indices(rng, y):
+    """element 0, NSAMP seeded positions and the 8 largest amplitudes of one column."""
+    top = np.argsort(-np.abs(y))[:8]
+    return np.unique(np.concatenate([[0], rng.integers(0, y.shape[0], size=NSAMP), top]))
+
+
+def write_samples(f, rng, Y, step):
+    for t in range(Y.shape[1]):
+        f.write("norm %d %d %.17e\n" % (t, step, float(np.vdot(Y[:, t], Y[:, t]).real)))
+        for i in sample_indices(rng, Y[:, t]):
+            f.write("amp %d %d %d %.17e %.17e\n" % (t, step, int(i), Y[i, t].real, Y[i, t].imag))
+    f.flush()
+
+
+def dense_apply(A):
+    def apply_A_ext(Z):                                   # real A on the real and imaginary parts of every column
+        nt = Z.shape[1]
+        R = A @ np.concatenate([Z[1:].real, Z[1:].imag], axis=1)
+        out = np.zeros_like(Z)
+        out[1:] = R[:, :nt] + 1j * R[:, nt:]
+        return out
+    return apply_A_ext
+
+
+def field_apply(D, C_o, C_v, fields):
+    """Z [n+1][ntraj] -> column t: E0_t M_{d_t} Z[:, t]  (the caller's pulse has E0 = 1)."""
+    parts = [tda.mo_dipoles(D, C_o, C_v, f["dir"]) for f in fields]
+
+    def apply_Md(Z):
+        return np.stack([fields[t]["E0"] * tda.apply_M(Z[:, t], *parts[t]) for t in range(Z.shape[1])], axis=1)
+    return apply_Md
+
+
+def main():
+    k = int(sys.argv[1])
+    out = sys.argv[2] if len(sys.argv) > 2 else os.path.join(os.path.dirname(os.path.abspath(__file__)),
+                                                             "config%d_trajectory_samples.txt" % k)
+    cfg = get_config(k)
+    basis = make_basis(cfg)
+    ob = OracleBasis(basis)
+    S = ob.overlap()
+    C_o, C_v, eps, cond = make_mos(cfg, S)
+    D = ob.dipole()
+    n = cfg.nocc * cfg.nvirt
+    rng = np.random.default_rng(20260116949 + k)
+    t0 = time.time()
+    f = open(out, "w")
+    f.write("# oracle trajectory samples, config %d, written by tests/golden/make_trajectory_samples.py (oracle only)\n" % k)
+    f.write("# RK4 (R7) on eq. 1 / 14-16 with the field coupling of eq. 16 / 19; see the script's docstring for the route\n")
+    f.write("meta cond_S %.6g\nmeta threads %d\n" % (cond, num_threads()))
+    if k == 2:
+        A = tda.build_A(ob.eri_tensor(), C_o, C_v, eps, 1.0)
+        fields = [dict(x) for x in cfg.fields]
+        cols = []
+        for fl in fields:                                  # linearised kick per trajectory (R8)
+            parts = tda.mo_dipoles(D, C_o, C_v, fl["dir"])
+            y0 = np.zeros(n + 1, dtype=complex); y0[0] = 1.0
+            cols.append(tda.kick(y0, fl, lambda z, p=parts: tda.apply_M(z, *p)))
+        Y = np.stack(cols, axis=1)
+        f.write("meta dt %.17g\nmeta nsteps %d\nmeta route dense_A_full_tensor\n" % (cfg.dt, cfg.nsteps))
+        done = 0
+        for stop in (10, cfg.nsteps):
+            Y, _ = tda.rk4_propagate(dense_apply(A), None, Y, {"type": "none"}, done * cfg.dt, cfg.dt, stop - done, log=False)
+            done = stop
+            write_samples(f, rng, Y, stop)
+    elif k == 3:
+        Q = ob.schwarz()
+        A = tda.build_A_by_pair_blocks(ob, C_o, C_v, eps, 1.0, tau=1e-20, Q=Q,
+                                       progress=lambda sc: print("pair blocks: shell", sc, "%.0f s" % (time.time() - t0), flush=True))
+        dvec = tda.mo_dipoles(D, C_o, C_v, (0.0, 0.0, 1.0))[2].reshape(-1)
+        al, be, _ = tda.lanczos(lambda x: A @ x, dvec, 80)
+        T = np.diag(al) + np.diag(be[:-1], 1) + np.diag(be[:-1], -1)
+        omega = float(np.linalg.eigvalsh(T)[0])
+        fields = [dict(x, omega=omega) for x in cfg.fields]
+        f.write("meta dt %.17g\nmeta nsteps %d\nmeta omega %.17e\nmeta route dense_A_pair_blocks\n" % (cfg.dt, cfg.nsteps, omega))
+        Y = np.zeros((n + 1, len(fields)), dtype=complex); Y[0, :] = 1.0
+        unit = dict(fields[0], E0=1.0)
+        done = 0
+        for stop in (3, 400, cfg.nsteps):
+            Y, _ = tda.rk4_propagate(dense_apply(A), field_apply(D, C_o, C_v, fields), Y, unit, done * cfg.dt, cfg.dt,
+                                     stop - done, log=False)
+            done = stop
+            write_samples(f, rng, Y, stop)
+            print("config 3: step", stop, "%.0f s" % (time.time() - t0), flush=True)
+    elif k == 4:
+        tau, omega, t_start = 1e-14, 0.2, 95.0
+        fields = [dict(x, omega=omega) for x in cfg.fields]
+        Q = ob.schwarz()
+        V = make_vectors(cfg, 2 * len(fields), stream=4).reshape(len(fields), 2, n)
+        g0 = np.random.default_rng(20260116949 + 40).standard_normal((len(fields), 2))
+        Y = np.zeros((n + 1, len(fields)), dtype=complex)
+        for t in range(len(fields)):
+            Y[0, t] = g0[t, 0] + 1j * g0[t, 1]
+            Y[1:, t] = V[t, 0] + 1j * V[t, 1]
+            Y[:, t] /= np.linalg.norm(Y[:, t])
+        f.write("meta dt %.17g\nmeta nsteps 1\nmeta t_start %.17g\nmeta omega %.17e\nmeta tau_oracle %g\n" % (cfg.dt, t_start, omega, tau))
+        f.write("meta route matrix_free_fp64\nmeta start seeded_random_states make_vectors(cfg,6,stream=4)+rng(SEED+40)\n")
+        write_samples(f, rng, Y, 0)                        # the start states themselves (the test regenerates and checks them)
+        npass = [0]
+
+        def apply_A_ext(Z):
+            nt = Z.shape[1]
+            X = np.concatenate([Z[1:].real.T, Z[1:].imag.T])                # [2 ntraj][n]
+            s, _, _ = tda.sigma_matrix_free(ob, X, C_o, C_v, eps, 1.0, tau, Q)
+            npass[0] += 1
+            print("config 4: J/K pass", npass[0], "%.0f s" % (time.time() - t0), flush=True)
+            o = np.zeros_like(Z)
+            o[1:] = (s[:nt] + 1j * s[nt:]).T
+            return o
+        unit = dict(fields[0], E0=1.0)
+        Y, _ = tda.rk4_propagate(apply_A_ext, field_apply(D, C_o, C_v, fields), Y, unit, t_start, cfg.dt, 1, log=False)
+        write_samples(f, rng, Y, 1)
+    else:
+        raise SystemExit("config must be 2, 3 or 4")
+    f.write("meta seconds %.0f\n" % (time.time() - t0))
+    f.close()
+    print("wrote", out, "in %.0f s" % (time.time() - t0))
+
+
+if __name__ == "__main__":
+    main()

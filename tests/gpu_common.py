@@ -48,3 +48,35 @@ def gpu_fock(ctx, T):
 
 def rel_inf(a, b):
     return float(np.max(np.abs(a - b)) / np.max(np.abs(b)))
+
+
+def read_trajectory_samples(k: int):
+    """tests/golden/config{k}_trajectory_samples.txt (oracle-written) -> (meta dict, amp {(traj, step): (idx, values)},
+    norm {(traj, step): |y|^2}) or None if the file has not been generated."""
+    import os
+    path = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "config%d_trajectory_samples.txt" % k)
+    if not os.path.exists(path):
+        return None
+    meta, amp, norm = {}, {}, {}
+    for line in open(path):
+        p = line.split()
+        if not p or p[0].startswith("#"):
+            continue
+        if p[0] == "meta":
+            meta[p[1]] = " ".join(p[2:])
+        elif p[0] == "norm":
+            norm[(int(p[1]), int(p[2]))] = float(p[3])
+        elif p[0] == "amp":
+            amp.setdefault((int(p[1]), int(p[2])), []).append((int(p[3]), complex(float(p[4]), float(p[5]))))
+    if "seconds" not in meta:
+        return None                                   # generator still running / interrupted
+    out = {}
+    for key, lst in amp.items():
+        out[key] = (np.array([i for i, _ in lst]), np.array([v for _, v in lst]))
+    return meta, out, norm
+
+
+def max_amp_err(y_traj, samples):
+    """y_traj [2][1+ncsf] (q, p planes of one trajectory) against stored (indices, complex values)."""
+    idx, val = samples
+    return float(np.max(np.abs((y_traj[0, idx] + 1j * y_traj[1, idx]) - val)))
