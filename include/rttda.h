@@ -37,6 +37,7 @@ extern "C" {
 #define RTTDA_EINVAL -1   /* bad shapes, l > 1, nocc + nvirt != nao, nvec < 1, NULL pointer, ... */
 #define RTTDA_ENOMEM -2
 #define RTTDA_ECUDA  -3   /* CUDA runtime error; string in rttda_last_error() */
+#define RTTDA_ENOCONV -4  /* iterative solver stopped at maxiter; outputs hold the current iterate */
 
 typedef struct rttda_handle_s* rttda_handle_t;   /* opaque; owns all internal device memory */
 
@@ -161,6 +162,16 @@ int rttda_get_info(rttda_handle_t h, int32_t key, double* out);
  *   vectors; must not alias v0).  The Ritz values are the eigenvalues of tridiag(alpha, beta[0..m-2]); the caller
  *   diagonalises that small matrix.  Synchronises `stream` every step (alpha_j, beta_j are read back). */
 int rttda_lanczos(rttda_handle_t h, int32_t m, const double* v0, double* alpha, double* beta, double* V, void* stream);
+
+/* TI-TDA eigenpairs (NEXT-3 of DESIGN.md): the k lowest solutions of A X = omega X (eq. 2; the reference method
+ * the paper compares its spectra with, Table 1) by block Davidson on the singles block: each iteration applies
+ * A to a block of up to max(nblock, k) new directions in ONE multi-vector sigma build; start vectors are unit vectors on
+ * the smallest eps_a - eps_i, the preconditioner is 1 / (theta - (eps_a - eps_i)).
+ *   omega HOST [k] ascending, X DEVICE [k][nocc*nvirt] orthonormal eigenvectors, resid HOST [k] or NULL: |A x - omega x|_2,
+ *   niter / nsigma (may be NULL): iterations and sigma vectors built.  Converged when every residual norm <= tol;
+ *   RTTDA_ENOCONV after maxiter iterations (outputs then hold the current Ritz pairs).  Synchronises `stream`. */
+int rttda_eigs(rttda_handle_t h, int32_t k, int32_t nblock, double tol, int32_t maxiter, double* omega, double* X,
+               double* resid, int32_t* niter, int32_t* nsigma, void* stream);
 
 /* Populations of stationary states (NEXT-2 of DESIGN.md): P[t][i] = |X_i^dagger C_t|^2, eq. 22, the projection
  * of every trajectory's vector onto supplied stationary states (e.g. TI-TDA eigenvectors; the ground state is e_0).

@@ -357,6 +357,49 @@ def lanczos(apply_A, v0, m, reorth=True):
     return alpha, beta, V
 
 
+# ---------------------------------------------------------------- block Davidson on A (NEXT-3: TI-TDA eigenpairs, eq. 2)
+def davidson(apply_A, diag, k, nblock=None, tol=1e-8, maxiter=200):
+    """Lowest k eigenpairs of the singles block A (A X = omega X, eq. 2) by block Davidson:
+        V orthonormal search space (rows), W = A V, H = V W^T, Ritz pairs (theta, y) of H;
+        x_j = y_j V, r_j = y_j W - theta_j x_j; stop when max_j |r_j| <= tol;
+        new directions r_j / (theta_j - diag) for the unconverged roots (|denominator| >= 1e-4), orthonormalised against
+        V by two Gram-Schmidt passes; start = unit vectors on the nblock smallest entries of diag = eps_a - eps_i.
+    `apply_A` maps rows [m][n] -> [m][n].  Returns (omega [k], X [k][n], residual norms [k], iterations)."""
+    n = diag.shape[0]
+    nb = min(max(nblock or k, k), n)
+    V = np.zeros((nb, n))
+    V[np.arange(nb), np.argsort(diag, kind="stable")[:nb]] = 1.0
+    W = apply_A(V)
+    for it in range(1, maxiter + 1):
+        H = V @ W.T
+        th, Y = np.linalg.eigh(0.5 * (H + H.T))
+        kk = min(nb, V.shape[0])
+        X = Y[:, :kk].T @ V
+        R = Y[:, :kk].T @ W - th[:kk, None] * X
+        rn = np.linalg.norm(R, axis=1)
+        if np.max(rn[:k]) <= tol or V.shape[0] >= n:
+            return th[:k], X[:k], rn[:k], it
+        new = []
+        for j in range(kk):
+            if j < k and rn[j] <= tol:
+                continue
+            d = th[j] - diag
+            d = np.where(np.abs(d) < 1e-4, np.where(d < 0, -1e-4, 1e-4), d)
+            t = R[j] / d
+            B = np.vstack([V] + new) if new else V
+            for _ in range(2):
+                t = t - B.T @ (B @ t)
+            nt = np.linalg.norm(t)
+            if nt > 1e-12:
+                new.append((t / nt)[None, :])
+        if not new:
+            return th[:k], X[:k], rn[:k], it
+        Vn = np.vstack(new)
+        V = np.vstack([V, Vn])
+        W = np.vstack([W, apply_A(Vn)])
+    return th[:k], X[:k], rn[:k], maxiter
+
+
 # ---------------------------------------------------------------- spectrum (harness for the pins)
 def spectrum(R, dt, pad=50000):
     """omega * F[R(t)] with mirroring R(-t) = R(t)^*, Hann window, zero padding (eq. 21).

@@ -22,7 +22,7 @@ FIELD_CONTINUE = 1
 PULSE = dict(none=0, delta=1, cw=2, tl=3, chirp=4, sin2=5)
 EXPORTS = ["rttda_overlap", "rttda_dipole_ao", "rttda_create", "rttda_destroy", "rttda_sigma",
            "rttda_sigma_host", "rttda_fock", "rttda_propagate", "rttda_propagate_sso", "rttda_propagate_host",
-           "rttda_get_info", "rttda_set_option", "rttda_populations", "rttda_spectrum", "rttda_lanczos", "rttda_last_timings", "rttda_jk_time", "rttda_profile_pass", "rttda_gemm_f64", "rttda_fp64_peak", "rttda_last_error",
+           "rttda_get_info", "rttda_set_option", "rttda_populations", "rttda_spectrum", "rttda_lanczos", "rttda_eigs", "rttda_last_timings", "rttda_jk_time", "rttda_profile_pass", "rttda_gemm_f64", "rttda_fp64_peak", "rttda_last_error",
            "rttda_version"]
 
 
@@ -223,6 +223,15 @@ class Rttda:
         _check(lib().rttda_lanczos(self._h, int(m), _dptr(v0), _dptr(alpha), _dptr(beta), _dptr(V), _stream(stream)),
                "rttda_lanczos")
         return alpha, beta
+
+    def rttda_eigs(self, k: int, X, nblock: int = 0, tol: float = 1e-8, maxiter: int = 100, stream=None):
+        """Lowest k eigenpairs of A by block Davidson; X CUDA tensor [k][ncsf] receives the vectors.
+        Returns (omega [k], residual norms [k], iterations, sigma vectors built)."""
+        om, rs = np.zeros(k), np.zeros(k)
+        it, ns = ct.c_int32(0), ct.c_int32(0)
+        _check(lib().rttda_eigs(self._h, int(k), int(nblock or k), ct.c_double(tol), int(maxiter), _dptr(om), _dptr(X),
+                                _dptr(rs), ct.byref(it), ct.byref(ns), _stream(stream)), "rttda_eigs")
+        return om, rs, it.value, ns.value
 
     def rttda_populations(self, C, Xs, P, stream=None):
         _check(lib().rttda_populations(self._h, int(C.shape[0]), _dptr(C), int(Xs.shape[0]), _dptr(Xs), _dptr(P),

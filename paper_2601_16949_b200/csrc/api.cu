@@ -219,6 +219,17 @@ int rttda_lanczos(rttda_handle_t hh, int32_t m, const double* v0, double* alpha,
     return lanczos_impl(h, m, v0, alpha, beta, V, (cudaStream_t)stream);
 }
 
+int rttda_eigs(rttda_handle_t hh, int32_t k, int32_t nblock, double tol, int32_t maxiter, double* omega, double* X,
+               double* resid, int32_t* niter, int32_t* nsigma, void* stream)
+{
+    Handle* h = (Handle*)hh;
+    RT_CHECK(h && omega && X, "rttda_eigs: NULL pointer");
+    RT_DEVICE(h);
+    RT_CHECK(k >= 1 && k <= h->ncsf && nblock >= 1, "rttda_eigs: need 1 <= k <= nocc*nvirt and nblock >= 1");
+    RT_CHECK(tol > 0.0 && maxiter >= 1, "rttda_eigs: need tol > 0 and maxiter >= 1");
+    return eigs_impl(h, k, nblock, tol, maxiter, omega, X, resid, niter, nsigma, (cudaStream_t)stream);
+}
+
 int rttda_populations(rttda_handle_t hh, int32_t ntraj, const double* C, int32_t nstates, const double* Xs, double* P,
                       void* stream)
 {

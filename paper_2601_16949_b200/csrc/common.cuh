@@ -224,5 +224,9 @@ int populations_impl(Handle* h, int ntraj, const double* y, int nstates, const d
 int sigma_impl(Handle* h, int nvec, const double* X, long long ldx, double* sigma, long long lds,
                cudaStream_t st);
 int ensure_ws(Handle* h, double** p, size_t* cur, size_t need);
+int project_out(long long n, int nv, const double* V, double* w, double* dots, cudaStream_t st);
+// eigs.cu
+int eigs_impl(Handle* h, int k, int nblock, double tol, int maxiter, double* omega, double* X, double* resid, int* niter,
+              int* nsigma, cudaStream_t st);
 
 }  // namespace rttda

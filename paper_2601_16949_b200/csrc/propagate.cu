@@ -575,6 +575,16 @@ __global__ void multi_axpy_kernel(long long n, int nv, const double* __restrict_
     for (int i = 0; i < nv; ++i) s = fma(-c[i], V[(long long)i * n + e], s);
     w[e] = s;
 }
+// w -= V^T (V w) for the nv rows of V (coefficients through `dots`, DEVICE [nv])
+int project_out(long long n, int nv, const double* V, double* w, double* dots, cudaStream_t st)
+{
+    if (nv <= 0) return RTTDA_OK;
+    multi_dot_kernel<<<nv, 256, 0, st>>>(n, V, w, dots);
+    multi_axpy_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(n, nv, V, dots, w);
+    RT_CUDA(cudaGetLastError());
+    return RTTDA_OK;
+}
+
 __global__ void scale_to_kernel(long long n, double a, const double* __restrict__ in, double* __restrict__ out)
 {
     const long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x;

@@ -219,3 +219,44 @@ def test_gemm_f64_vs_numpy_ragged_strided_batched(shape):
                 torch.cuda.synchronize()
                 scale = max(1.0, float(np.max(np.abs(ref))))
                 assert np.max(np.abs(Cd.cpu().numpy() - ref)) / scale < 1e-13 * max(1, K) ** 0.5
+
+
+@pytest.mark.parametrize("k,nblock", [(1, 1), (4, 4), (5, 8)])
+def test_eigs_block_davidson_tiny_vs_eigh(k, nblock):
+    """rttda_eigs (NEXT-3, eq. 2): lowest k eigenpairs of A through multi-vector sigma builds against eigh of the
+    oracle's dense A: eigenvalues, residual of the returned vectors under the ORACLE's A, orthonormality."""
+    import torch
+    ctx = setup_config(1, dense=True)
+    A, h = ctx["A"], ctx["h"]
+    n = A.shape[0]
+    w = np.linalg.eigvalsh(A)
+    X = torch.zeros((k, n), dtype=torch.float64, device=ctx["dev"])
+    om, rs, it, ns = h.rttda_eigs(k, X, nblock, tol=1e-9, maxiter=100)
+    Xh = X.cpu().numpy()
+    assert np.max(np.abs(om - w[:k])) < 1e-9
+    assert np.max(np.linalg.norm(Xh @ A.T - om[:, None] * Xh, axis=1)) < 2e-9 and np.max(rs) <= 1e-9
+    assert np.max(np.abs(Xh @ Xh.T - np.eye(k))) < 1e-10
+    assert ns <= it * max(nblock, k)
+
+
+def test_eigs_config2_lowest_states_and_populations():
+    """Config 2 (6400 singles): the four lowest TI-TDA states from rttda_eigs (block of 8, one sigma build of up to 8
+    vectors per iteration) against the oracle's block Davidson on its dense A; the vectors feed rttda_populations."""
+    import torch
+    from oracle import tda
+    ctx = setup_config(2, dense=True)
+    A, h, cfg = ctx["A"], ctx["h"], ctx["cfg"]
+    n = A.shape[0]
+    diag = (ctx["eps"][cfg.nocc:][None, :] - ctx["eps"][:cfg.nocc][:, None]).reshape(-1)
+    om_ref, X_ref, rn_ref, _ = tda.davidson(lambda V: V @ A.T, diag, 4, 8, tol=1e-9)
+    X = torch.zeros((4, n), dtype=torch.float64, device=ctx["dev"])
+    om, rs, it, ns = h.rttda_eigs(4, X, 8, tol=1e-8, maxiter=100)
+    Xh = X.cpu().numpy()
+    assert np.max(np.abs(om - om_ref)) < 1e-8
+    assert np.max(np.linalg.norm(Xh @ A.T - om[:, None] * Xh, axis=1)) < 5e-8
+    Xs = np.zeros((5, n + 1)); Xs[0, 0] = 1.0; Xs[1:, 1:] = Xh
+    y = np.zeros((1, 2, n + 1)); y[0, 0, 1:] = Xh[2]                # the third excited state itself
+    P = torch.zeros((1, 5), dtype=torch.float64, device=ctx["dev"])
+    h.rttda_populations(torch.from_numpy(y).to(ctx["dev"]), torch.from_numpy(Xs).to(ctx["dev"]), P)
+    torch.cuda.synchronize()
+    assert np.max(np.abs(P.cpu().numpy()[0] - np.array([0.0, 0.0, 0.0, 1.0, 0.0]))) < 1e-9

@@ -551,3 +551,22 @@ def test_dense_A_by_pair_blocks_equals_tensor_route(tiny):
     blk = tiny["ob"].eri_pair_block(4, 2)
     o4, o2 = int(tiny["ob"].ao_off[4]), int(tiny["ob"].ao_off[2])
     assert np.max(np.abs(blk - tiny["eri"][:, :, o4:o4 + blk.shape[2], o2:o2 + blk.shape[3]])) < 1e-15
+
+
+def test_davidson_lowest_eigenpairs_against_eigh(tiny):
+    """Block Davidson of the oracle (NEXT-3; eq. 2) against LAPACK's eigh of the dense A: eigenvalues, residuals,
+    orthonormality, and the subspace of the lowest roots."""
+    A = tiny["A"]
+    n = A.shape[0]
+    no, nv = tiny["C_o"].shape[1], tiny["C_v"].shape[1]
+    eps = tiny["eps"]
+    diag = (eps[no:][None, :] - eps[:no][:, None]).reshape(-1)
+    w, U = np.linalg.eigh(A)
+    for k, nb in ((1, 1), (4, 4), (6, 9)):
+        om, X, rn, it = tda.davidson(lambda V: V @ A.T, diag, k, nb, tol=1e-9)
+        assert np.max(np.abs(om - w[:k])) < 1e-10
+        assert np.max(rn) <= 1e-9 and np.max(np.abs(X @ A.T - om[:, None] * X)) < 1e-8
+        assert np.max(np.abs(X @ X.T - np.eye(k))) < 1e-10
+        P = U[:, :k] @ U[:, :k].T                                   # projector on the exact lowest-k subspace
+        assert np.max(np.abs(X @ P - X)) < 1e-6
+        assert it < 60
