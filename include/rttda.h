@@ -199,6 +199,11 @@ int rttda_spectrum(int32_t ntraj, int32_t n, const double* R0, const double* log
  * `value`); it is offered because 180 GB of HBM3e can hold what the paper's GPUs could not.  RTTDA_ENOMEM if the
  * store does not fit: the handle then stays in direct mode. */
 #define RTTDA_OPT_INCORE 1
+/* RTTDA_OPT_GRAPH (value != 0 on): rttda_propagate captures ONE RK4 step (4 sigma builds, field coupling, stage
+ * combination, observables; E(t) and the step counter live in device memory) in a CUDA graph and replays it nsteps times.
+ * Default: on for small molecules (whose ERI pass is a few hundred short kernels), off for large ones.  While it is on
+ * the per-pass event timings of rttda_jk_time / rttda_last_timings are not recorded by rttda_propagate. */
+#define RTTDA_OPT_GRAPH 2
 int rttda_set_option(rttda_handle_t h, int32_t option, double value);
 
 /* Time the last rttda_sigma/rttda_fock call spent in the J/K kernels, from CUDA events recorded on its

@@ -105,6 +105,10 @@ int rttda_destroy(rttda_handle_t hh)
         if (h->lane_ev[l]) cudaEventDestroy(h->lane_ev[l]);
     }
     if (h->ev_fork) cudaEventDestroy(h->ev_fork);
+    if (h->step_graph) cudaGraphExecDestroy(h->step_graph);
+    if (h->d_ctl) cudaFree(h->d_ctl);
+    if (h->graph_st) cudaStreamDestroy(h->graph_st);
+    if (h->graph_ev) cudaEventDestroy(h->graph_ev);
     for (auto& e : h->ev) if (e) cudaEventDestroy(e);
     for (auto& e : h->jk_ev) cudaEventDestroy(e);
     delete h;
@@ -257,8 +261,9 @@ int rttda_set_option(rttda_handle_t hh, int32_t option, double value)
     Handle* h = (Handle*)hh;
     RT_CHECK(h != nullptr, "rttda_set_option: NULL handle");
     RT_DEVICE(h);
-    RT_CHECK(option == RTTDA_OPT_INCORE, "rttda_set_option: unknown option");
+    RT_CHECK(option == RTTDA_OPT_INCORE || option == RTTDA_OPT_GRAPH, "rttda_set_option: unknown option");
     const bool on = value != 0.0;
+    if (option == RTTDA_OPT_GRAPH) { h->use_graph = on; return RTTDA_OK; }
     if (on && !h->incore) {
         const int r = ensure_ws(h, &h->eri_all, &h->eri_all_n, h->eri_all_need);
         if (r != RTTDA_OK) return r;                       // not enough HBM: the handle stays in direct mode

@@ -174,6 +174,16 @@ struct Handle {
     size_t wsY_n = 0, wsT_n = 0, wsF_n = 0, wsZ_n = 0, wsP_n = 0;
     double* prop_ws = nullptr;
     size_t prop_ws_n = 0;
+    // CUDA graph of one RK4 step (propagate.cu): device-side control block, cached executable graph and its key
+    void* d_ctl = nullptr;
+    cudaGraphExec_t step_graph = nullptr;
+    cudaStream_t graph_st = nullptr;
+    cudaEvent_t graph_ev = nullptr;
+    struct GraphKey { int ntraj = 0; const double* y = nullptr; unsigned active = 0; int nlanes = -1; long long epoch = -1; } graph_key;
+    long long ws_epoch = 0;                    // bumped whenever a workspace is reallocated
+    long long graph_launches = 0;              // kernels inside one replay of step_graph
+    double graph_dt = 0.0;
+    bool use_graph = false, capturing = false;
     // propagator state kept across calls: polarisations of the cached D_d matrices, reference state of R(t)
     bool dd_valid = false;
     int dd_ntraj = 0, yref_ntraj = 0;
@@ -209,6 +219,7 @@ struct GemmDesc {
     const double* B; long long sbk, sbn, sbbatch;
     double* C;       long long scm, scn, scbatch;
     double alpha, beta;
+    const double* alpha_dev;   // optional DEVICE scalar multiplying alpha (read at run time: CUDA-graph friendly)
 };
 int gemm_f64(const GemmDesc& g, cudaStream_t st);
 
@@ -224,6 +235,7 @@ int populations_impl(Handle* h, int ntraj, const double* y, int nstates, const d
 int sigma_impl(Handle* h, int nvec, const double* X, long long ldx, double* sigma, long long lds,
                cudaStream_t st);
 int ensure_ws(Handle* h, double** p, size_t* cur, size_t need);
+int sigma_reserve(Handle* h, int nvec);
 int project_out(long long n, int nv, const double* V, double* w, double* dots, cudaStream_t st);
 // eigs.cu
 int eigs_impl(Handle* h, int k, int nblock, double tol, int maxiter, double* omega, double* X, double* resid, int* niter,

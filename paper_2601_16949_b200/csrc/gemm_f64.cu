@@ -38,6 +38,7 @@ __global__ void __launch_bounds__(128) gemm_f64_kernel(GemmDesc g)
         for (int j = 0; j < 4; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
 
     const bool a_kfast = (g.sak == 1), b_kfast = (g.sbk == 1);
+    const double alpha = g.alpha_dev ? g.alpha * __ldg(g.alpha_dev) : g.alpha;
     double ra[8], rb[8];                       // register staging of the next tile (BM*BK/128 = 8 each)
 
     auto gload = [&](int k0) {
@@ -98,7 +99,7 @@ __global__ void __launch_bounds__(128) gemm_f64_kernel(GemmDesc g)
                 const int gm = m0 + wm + i * 8 + fr, gn = n0 + wn + j * 8 + 2 * fc + e;
                 if (gm < g.M && gn < g.N) {
                     double* p = C + (long long)gm * g.scm + (long long)gn * g.scn;
-                    const double v = g.alpha * acc[i][j][e];
+                    const double v = alpha * acc[i][j][e];
                     *p = (g.beta == 0.0) ? v : fma(g.beta, *p, v);
                 }
             }

@@ -13,6 +13,7 @@ int ensure_ws(Handle* h, double** p, size_t* cur, size_t need)
     cudaError_t e = cudaMalloc((void**)p, need * sizeof(double));
     if (e != cudaSuccess) { set_error(std::string("workspace cudaMalloc: ") + cudaGetErrorString(e)); return RTTDA_ENOMEM; }
     *cur = need;
+    h->ws_epoch++;                               // pointers baked into a captured graph are stale now
     return RTTDA_OK;
 }
 
@@ -39,15 +40,31 @@ int jk_mark(Handle* h, cudaStream_t st)
     return RTTDA_OK;
 }
 
+// Every workspace a sigma build of nvec vectors needs (must not be grown while a stream is being captured)
+int sigma_reserve(Handle* h, int nvec)
+{
+    const size_t N = h->nao, no = h->nocc;
+    const int nvt = padded_nvec(nvec);
+    RT_TRY(ensure_ws(h, &h->wsY, &h->wsY_n, (size_t)nvec * no * N));
+    RT_TRY(ensure_ws(h, &h->wsT, &h->wsT_n, (size_t)nvt * N * N));
+    RT_TRY(ensure_ws(h, &h->wsF, &h->wsF_n, (size_t)nvt * N * N));
+    RT_TRY(ensure_ws(h, &h->wsP, &h->wsP_n, (size_t)2 * nvt * N * N));
+    if (!h->incore) {
+        for (int l = 0; l < h->nlanes; ++l) RT_TRY(ensure_ws(h, &h->eri_buf[l], &h->eri_buf_n[l], h->lane_need[l]));
+        if (h->nlanes == 0)
+            for (int b = 0; b < 2; ++b) RT_TRY(ensure_ws(h, &h->eri_buf[b], &h->eri_buf_n[b], h->eri_buf_need));
+    }
+    return RTTDA_OK;
+}
+
 int sigma_impl(Handle* h, int nvec, const double* X, long long ldx, double* sigma, long long lds,
                cudaStream_t st)
 {
     const size_t N = h->nao, no = h->nocc, nv = h->nvirt;
     const int nvt = padded_nvec(nvec);          // density slots: 16, 32 or multiples of 64 bytes (sector aligned)
-    RT_TRY(ensure_ws(h, &h->wsY, &h->wsY_n, (size_t)nvec * no * N));
-    RT_TRY(ensure_ws(h, &h->wsT, &h->wsT_n, (size_t)nvt * N * N));
-    RT_TRY(ensure_ws(h, &h->wsF, &h->wsF_n, (size_t)nvt * N * N));
-    RT_CUDA(cudaEventRecord(h->ev[0], st));
+    const bool timed = !h->capturing;           // event timings cannot be taken inside a captured graph
+    if (timed) RT_TRY(sigma_reserve(h, nvec));
+    if (timed) RT_CUDA(cudaEventRecord(h->ev[0], st));
     if (nvt != nvec) RT_CUDA(cudaMemsetAsync(h->wsT, 0, (size_t)nvt * N * N * sizeof(double), st));
     // a1: Y_v = X_v C_v^T  [no][N];  T[mu][nu][v] = sum_j C_o[mu][j] Y_v[j][nu]
     GemmDesc g{};
@@ -62,13 +79,11 @@ int sigma_impl(Handle* h, int nvec, const double* X, long long ldx, double* sigm
     g.B = h->wsY; g.sbk = N; g.sbn = 1; g.sbbatch = no * N;
     g.C = h->wsT; g.scm = N * nvt; g.scn = nvt; g.scbatch = 1;
     RT_TRY(gemm_f64(g, st));
-    RT_CUDA(cudaEventRecord(h->ev[1], st));
-    RT_TRY(jk_mark(h, st));
+    if (timed) { RT_CUDA(cudaEventRecord(h->ev[1], st)); RT_TRY(jk_mark(h, st)); }
     // a3-a4: F = 2 J[T] - cx K[T], interleaved layout; one ERI pass serves all densities
     RT_CUDA(cudaMemsetAsync(h->wsF, 0, (size_t)nvt * N * N * sizeof(double), st));
     RT_TRY(jk_build(h, nvt, (nvec + 1) & ~1, h->wsT, h->wsF, st));
-    RT_TRY(jk_mark(h, st));
-    RT_CUDA(cudaEventRecord(h->ev[2], st));
+    if (timed) { RT_TRY(jk_mark(h, st)); RT_CUDA(cudaEventRecord(h->ev[2], st)); }
     // a5: Z_v = C_o^T F_v [no][N];  sigma_v = deps o X_v + Z_v C_v
     g.M = (int)no; g.N = (int)N; g.K = (int)N; g.batch = nvec;
     g.A = h->C_occ; g.sam = 1; g.sak = no; g.sabatch = 0;
@@ -83,8 +98,7 @@ int sigma_impl(Handle* h, int nvec, const double* X, long long ldx, double* sigm
     g.B = h->C_virt; g.sbk = nv; g.sbn = 1; g.sbbatch = 0;
     g.C = sigma; g.scm = nv; g.scn = 1; g.scbatch = lds;
     RT_TRY(gemm_f64(g, st));
-    RT_CUDA(cudaEventRecord(h->ev[3], st));
-    h->ev_valid = true;
+    if (timed) { RT_CUDA(cudaEventRecord(h->ev[3], st)); h->ev_valid = true; }
     h->kernel_launches += 5;
     return RTTDA_OK;
 }
@@ -188,6 +202,82 @@ static int apply_field(Handle* h, int ntraj, const double* ys, double* hy, const
         h->kernel_launches += 2;
     }
     return RTTDA_OK;
+}
+
+// ---------------------------------------------------------------------------------------------- device-side stepping
+// Control block of a graph-replayed run: pulse parameters, start time, step counter and log pointer live in device
+// memory, so that the captured step holds no per-step host value.
+struct PropCtl {
+    double t_start, dt;
+    double* log;                    // [nsteps][ntraj][3] or NULL
+    int step, ntraj;
+    rttda_field_t f[8];
+    double E[8], mE[8], D00[8];     // E(t) of the current stage, its negative, D_00 along the polarisation
+};
+
+__device__ double field_value_dev(const rttda_field_t& f, double t)
+{
+    switch (f.type) {
+        case RTTDA_CW: return f.E0 * sin(f.omega * t);
+        case RTTDA_TL: {
+            const double s = t - f.t0;
+            return f.E0 * exp(-s * s / (2.0 * f.sigma * f.sigma)) * sin(f.omega * s);
+        }
+        case RTTDA_CHIRP: {
+            const double s = t - f.t0;
+            return f.E0 * exp(-s * s / (2.0 * f.sigma * f.sigma)) * sin((f.omega + 0.5 * f.beta * s) * s);
+        }
+        case RTTDA_SIN2: {
+            if (t < 0.0 || t > f.T_env) return 0.0;
+            const double e = sin(3.14159265358979323846 * t / f.T_env);
+            return f.E0 * e * e * sin(f.omega * t);
+        }
+        default: return 0.0;
+    }
+}
+
+// E(t_stage) of every trajectory, t_stage = t_start + (step + off) dt
+__global__ void field_eval_kernel(PropCtl* c, double off)
+{
+    const int t = threadIdx.x;
+    if (t >= c->ntraj) return;
+    const double ts = c->t_start + ((double)c->step + off) * c->dt;
+    const double E = field_value_dev(c->f[t], ts);
+    c->E[t] = E;
+    c->mE[t] = -E;
+}
+
+__global__ void step_advance_kernel(PropCtl* c) { c->step += 1; }
+
+// field_elem_kernel with E and D_00 read from the control block
+__global__ void __launch_bounds__(1024)
+field_elem_dev_kernel(int ncsf, const double* __restrict__ ys, double* __restrict__ hy,
+                      const double* __restrict__ Dov, const PropCtl* __restrict__ c)
+{
+    const int b = blockIdx.x, traj = b >> 1;
+    const long long n1 = (long long)ncsf + 1;
+    const double* y = ys + b * n1;
+    double* h = hy + b * n1;
+    const double* d = Dov + (long long)traj * ncsf;
+    const double E = c->E[traj], D00 = c->D00[traj], y0 = y[0];
+    const double s2 = 1.41421356237309504880;
+    double dot = 0.0;
+    for (int i = threadIdx.x; i < ncsf; i += blockDim.x) {
+        const double Y = y[1 + i], dv = d[i];
+        dot = fma(dv, Y, dot);
+        h[1 + i] += E * fma(s2 * dv, y0, D00 * Y);
+    }
+    __shared__ double red[32];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) dot += __shfl_xor_sync(0xffffffffu, dot, o);
+    if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = dot;
+    __syncthreads();
+    if (threadIdx.x < 32) {
+        double v = threadIdx.x < (blockDim.x >> 5) ? red[threadIdx.x] : 0.0;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+        if (threadIdx.x == 0) h[0] = E * fma(D00, y0, s2 * v);
+    }
 }
 
 // ---------------------------------------------------------------------------------------------- RK4
@@ -331,12 +421,150 @@ static int prop_prologue(Handle* h, int ntraj, double* y, const rttda_field_t* f
     return RTTDA_OK;
 }
 
+// observe_kernel writing to the control block's log row of the current step (no-op without a log)
+__global__ void __launch_bounds__(1024)
+observe_dev_kernel(long long n1, const double* __restrict__ y, const double* __restrict__ yref, const PropCtl* __restrict__ c)
+{
+    if (c->log == nullptr) return;
+    const int t = blockIdx.x;
+    double* out = c->log + ((long long)c->step * c->ntraj + t) * 3;
+    const double *q = y + 2 * t * n1, *p = q + n1, *qr = yref + 2 * t * n1, *pr = qr + n1;
+    double a = 0, b = 0, cc = 0;
+    for (long long i = threadIdx.x; i < n1; i += blockDim.x) {
+        const double qi = q[i], pi = p[i], qri = qr[i], pri = pr[i];
+        a = fma(qi, qi, fma(pi, pi, a));
+        b = fma(qri, qi, fma(pri, pi, b));
+        cc = fma(qri, pi, fma(-pri, qi, cc));
+    }
+    __shared__ double red[3][32];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        a += __shfl_xor_sync(0xffffffffu, a, o);
+        b += __shfl_xor_sync(0xffffffffu, b, o);
+        cc += __shfl_xor_sync(0xffffffffu, cc, o);
+    }
+    if ((threadIdx.x & 31) == 0) { red[0][threadIdx.x >> 5] = a; red[1][threadIdx.x >> 5] = b; red[2][threadIdx.x >> 5] = cc; }
+    __syncthreads();
+    if (threadIdx.x < 32) {
+        const int nw = blockDim.x >> 5;
+        a = threadIdx.x < nw ? red[0][threadIdx.x] : 0.0;
+        b = threadIdx.x < nw ? red[1][threadIdx.x] : 0.0;
+        cc = threadIdx.x < nw ? red[2][threadIdx.x] : 0.0;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            a += __shfl_xor_sync(0xffffffffu, a, o);
+            b += __shfl_xor_sync(0xffffffffu, b, o);
+            cc += __shfl_xor_sync(0xffffffffu, cc, o);
+        }
+        if (threadIdx.x == 0) { out[0] = a; out[1] = b; out[2] = cc; }
+    }
+}
+
+// One RK4 step with every per-step quantity read from the control block: the body of the captured graph.
+static int rk4_step_dev(Handle* h, int ntraj, double* y, const PropWs& w, unsigned active, double dt, cudaStream_t st)
+{
+    const size_t no = h->nocc, nv = h->nvirt, n1 = (size_t)h->ncsf + 1;
+    PropCtl* c = (PropCtl*)h->d_ctl;
+    const double ts_off[4] = {0.0, 0.5, 0.5, 1.0}, wgt[4] = {1.0, 2.0, 2.0, 1.0}, cnext[4] = {0.5 * dt, 0.5 * dt, dt, 0.0};
+    for (int s = 0; s < 4; ++s) {
+        const double* in = (s == 0) ? y : w.ys;
+        RT_TRY(sigma_impl(h, 2 * ntraj, in + 1, (long long)n1, w.hy + 1, (long long)n1, st));
+        field_eval_kernel<<<1, 32, 0, st>>>(c, ts_off[s]);
+        field_elem_dev_kernel<<<2 * ntraj, 1024, 0, st>>>(h->ncsf, in, w.hy, w.Dd_ov, c);
+        RT_CUDA(cudaGetLastError());
+        h->kernel_launches += 2;
+        for (int t = 0; t < ntraj; ++t) {
+            if (!(active >> t & 1u)) continue;               // NONE / DELTA: E(t) is identically zero
+            GemmDesc g{};
+            g.batch = 2; g.beta = 1.0; g.alpha = 1.0;
+            g.alpha_dev = c->E + t;                           // + E Y D_vv
+            g.M = (int)no; g.N = (int)nv; g.K = (int)nv;
+            g.A = in + (size_t)t * 2 * n1 + 1; g.sam = nv; g.sak = 1; g.sabatch = n1;
+            g.B = w.Dd_vv + (size_t)t * nv * nv; g.sbk = nv; g.sbn = 1; g.sbbatch = 0;
+            g.C = w.hy + (size_t)t * 2 * n1 + 1; g.scm = nv; g.scn = 1; g.scbatch = n1;
+            RT_TRY(gemm_f64(g, st));
+            g.alpha_dev = c->mE + t;                          // - E D_oo Y
+            g.M = (int)no; g.N = (int)nv; g.K = (int)no;
+            g.A = w.Dd_oo + (size_t)t * no * no; g.sam = no; g.sak = 1; g.sabatch = 0;
+            g.B = in + (size_t)t * 2 * n1 + 1; g.sbk = nv; g.sbn = 1; g.sbbatch = n1;
+            RT_TRY(gemm_f64(g, st));
+            h->kernel_launches += 2;
+        }
+        rk4_stage_kernel<<<w.eg, 256, 0, st>>>((long long)n1, ntraj, w.hy, y, w.ys, w.ksum, wgt[s], cnext[s], dt / 6.0,
+                                                s == 0, s == 3);
+        RT_CUDA(cudaGetLastError());
+        h->kernel_launches++;
+    }
+    observe_dev_kernel<<<ntraj, 1024, 0, st>>>((long long)n1, y, w.yref, c);
+    step_advance_kernel<<<1, 1, 0, st>>>(c);
+    RT_CUDA(cudaGetLastError());
+    h->kernel_launches += 2;
+    return RTTDA_OK;
+}
+
+// Graph-replayed RK4 run (RTTDA_OPT_GRAPH): upload the control block, capture one step if the cached graph does not
+// fit (trajectory count, state pointer, set of trajectories with a field, lane layout), replay it nsteps times.
+static int propagate_graph(Handle* h, int ntraj, double* y, const rttda_field_t* fields, double t_start, double dt,
+                           int nsteps, double* log, const PropWs& w, cudaStream_t st)
+{
+    if (!h->d_ctl) RT_CUDA(cudaMalloc(&h->d_ctl, sizeof(PropCtl)));
+    PropCtl hc{};
+    hc.t_start = t_start; hc.dt = dt; hc.log = log; hc.step = 0; hc.ntraj = ntraj;
+    unsigned active = 0;
+    for (int t = 0; t < ntraj; ++t) {
+        hc.f[t] = fields[t];
+        hc.D00[t] = w.fa.D00[t];
+        if (fields[t].type != RTTDA_NONE && fields[t].type != RTTDA_DELTA) active |= 1u << t;
+    }
+    // The legacy default stream cannot be captured, so the step is captured on and replayed from the handle's own stream,
+    // which is ordered after the caller's stream here and joined back into it at the end.
+    cudaStream_t user = st;
+    if (!h->graph_st) {
+        RT_CUDA(cudaStreamCreateWithFlags(&h->graph_st, cudaStreamNonBlocking));
+        RT_CUDA(cudaEventCreateWithFlags(&h->graph_ev, cudaEventDisableTiming));
+    }
+    st = h->graph_st;
+    RT_CUDA(cudaEventRecord(h->graph_ev, user));
+    RT_CUDA(cudaStreamWaitEvent(st, h->graph_ev, 0));
+    RT_CUDA(cudaMemcpyAsync(h->d_ctl, &hc, sizeof(PropCtl), cudaMemcpyHostToDevice, st));   // pageable source: staged before return
+    Handle::GraphKey key;
+    RT_TRY(sigma_reserve(h, 2 * ntraj));
+    key.ntraj = ntraj; key.y = y; key.active = active; key.nlanes = h->nlanes; key.epoch = h->ws_epoch;
+    const Handle::GraphKey& k0 = h->graph_key;
+    if (!h->step_graph || k0.ntraj != key.ntraj || k0.y != key.y || k0.active != key.active || k0.nlanes != key.nlanes ||
+        k0.epoch != key.epoch || h->graph_dt != dt) {
+        if (h->step_graph) { cudaGraphExecDestroy(h->step_graph); h->step_graph = nullptr; }
+        const long long l0 = h->kernel_launches;
+        cudaGraph_t graph = nullptr;
+        RT_CUDA(cudaStreamBeginCapture(st, cudaStreamCaptureModeRelaxed));
+        h->capturing = true;
+        const int rc = rk4_step_dev(h, ntraj, y, w, active, dt, st);
+        h->capturing = false;
+        const cudaError_t e = cudaStreamEndCapture(st, &graph);
+        if (rc != RTTDA_OK) { if (graph) cudaGraphDestroy(graph); return rc; }
+        RT_CUDA(e);
+        const cudaError_t e2 = cudaGraphInstantiate(&h->step_graph, graph, 0);
+        cudaGraphDestroy(graph);
+        RT_CUDA(e2);
+        h->graph_launches = h->kernel_launches - l0;
+        h->kernel_launches = l0;
+        h->graph_key = key;
+        h->graph_dt = dt;
+    }
+    for (int n = 0; n < nsteps; ++n) RT_CUDA(cudaGraphLaunch(h->step_graph, st));
+    RT_CUDA(cudaEventRecord(h->graph_ev, st));
+    RT_CUDA(cudaStreamWaitEvent(user, h->graph_ev, 0));
+    h->kernel_launches += h->graph_launches * nsteps;
+    return RTTDA_OK;
+}
+
 int propagate_impl(Handle* h, int ntraj, double* y, const rttda_field_t* fields, double t_start, double dt,
                    int nsteps, double* log, cudaStream_t st)
 {
     const size_t n1 = (size_t)h->ncsf + 1;
     PropWs w;
     RT_TRY(prop_prologue(h, ntraj, y, fields, w, st));
+    if (h->use_graph && nsteps > 0) return propagate_graph(h, ntraj, y, fields, t_start, dt, nsteps, log, w, st);
     double *ys = w.ys, *hy = w.hy, *ksum = w.ksum, *yref = w.yref, *Dd_oo = w.Dd_oo, *Dd_vv = w.Dd_vv, *Dd_ov = w.Dd_ov;
     FieldArgs& fa = w.fa;
     const unsigned eg = w.eg;

@@ -618,6 +618,7 @@ int create_impl(Handle* h, const rttda_basis_t* basis, const double* C_occ, cons
         const char* e = getenv("RTTDA_LANES");
         const int nl = e ? atoi(e) : ((double)h->eri_all_need * sizeof(double) < 8e9 ? Handle::MAXLANES : 0);
         RT_TRY(assign_lanes(h, nl));
+        h->use_graph = h->nlanes > 0;              // small molecules: launch-bound steps are replayed as a CUDA graph
     }
     h->info[RTTDA_INFO_CREATE_MS] =
         std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - t0).count();
