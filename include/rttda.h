@@ -204,6 +204,14 @@ int rttda_spectrum(int32_t ntraj, int32_t n, const double* R0, const double* log
  * Default: on for small molecules (whose ERI pass is a few hundred short kernels), off for large ones.  While it is on
  * the per-pass event timings of rttda_jk_time / rttda_last_timings are not recorded by rttda_propagate. */
 #define RTTDA_OPT_GRAPH 2
+/* Range-separated exchange (NEXT-4 of DESIGN.md; the paper's functional is CAM-B3LYP):
+ *   A_{ia,jb} = d_ij d_ab (eps_a - eps_i) + 2 (ia|jb) - c_x (ij|ab) - c_x^LR (ij| erf(omega r12)/r12 |ab)
+ * RTTDA_OPT_CX_LR sets c_x^LR (default 0), RTTDA_OPT_RS_OMEGA sets omega in 1/bohr (default 0 = off).  When both are
+ * non-zero every sigma build runs a second ERI pass over the same screened quartets with the integrals of the
+ * attenuated operator (1/r12 with alpha -> alpha omega^2 / (alpha + omega^2)), digested into the exchange part only.
+ * (CAM-B3LYP's exchange kernel is c_x = 0.19, c_x^LR = 0.46, omega = 0.33; its f_xc grid term stays out of scope.) */
+#define RTTDA_OPT_CX_LR 3
+#define RTTDA_OPT_RS_OMEGA 4
 int rttda_set_option(rttda_handle_t h, int32_t option, double value);
 
 /* Time the last rttda_sigma/rttda_fock call spent in the J/K kernels, from CUDA events recorded on its

@@ -173,13 +173,22 @@ void oracle_one_electron(BASIS_ARGS, int nao, const double *O, double *S, double
 /* ---- Hermite Coulomb integrals R^n_{tuv}(alpha, R_PQ) -------------------------------------- */
 /* R^n_{000} = (-2 alpha)^n F_n(alpha |R|^2);
  * R^n_{t+1,u,v} = t R^{n+1}_{t-1,u,v} + X R^{n+1}_{t,u,v}  (same in u with Y, v with Z). */
-static void hermite_R(int L, double alpha, const double *R, double Rt[5][5][5][5] /* [n][t][u][v] */)
+/* Range-separated operator erf(omega r12)/r12 (NEXT-4: the long-range exchange of CAM-type functionals): with
+ * theta^2 = omega^2 / (alpha + omega^2) the Hermite integrals are those of 1/r12 with alpha -> alpha theta^2 and an
+ * overall factor theta:  R^n_{000} = theta (-2 alpha theta^2)^n F_n(alpha theta^2 |R|^2).  omega <= 0 means 1/r12. */
+static void hermite_R(int L, double alpha, double omega, const double *R, double Rt[5][5][5][5] /* [n][t][u][v] */)
 {
     double F[LMAX_TOT + 1];
+    double theta = 1.0;
+    if (omega > 0.0) {
+        double th2 = omega * omega / (alpha + omega * omega);
+        theta = sqrt(th2);
+        alpha *= th2;
+    }
     double T = alpha * (R[0] * R[0] + R[1] * R[1] + R[2] * R[2]);
     oracle_boys(L, T, F);
     memset(Rt, 0, sizeof(double) * 625);
-    double m2a = 1.0;
+    double m2a = theta;
     for (int n = 0; n <= L; ++n) {
         Rt[n][0][0][0] = m2a * F[n];
         m2a *= -2.0 * alpha;
@@ -207,7 +216,7 @@ static void hermite_R(int L, double alpha, const double *R, double Rt[5][5][5][5
 /* ---- contracted shell quartet (ab|cd): out[na][nb][nc][nd] --------------------------------- */
 /* primitive: (ab|cd) = 2 pi^{5/2} / (p q sqrt(p+q)) sum_{tuv} E^{ab}_{tuv}
  *                       sum_{t'u'v'} (-1)^{t'+u'+v'} E^{cd}_{t'u'v'} R^0_{t+t',u+u',v+v'}          */
-static void shell_quartet(const basis_t *B, int sa, int sb, int sc, int sd, double *out)
+static void shell_quartet_op(const basis_t *B, int sa, int sb, int sc, int sd, double omega, double *out)
 {
     int l[4] = {B->sh_l[sa], B->sh_l[sb], B->sh_l[sc], B->sh_l[sd]};
     int n[4] = {2 * l[0] + 1, 2 * l[1] + 1, 2 * l[2] + 1, 2 * l[3] + 1};
@@ -238,7 +247,7 @@ static void shell_quartet(const basis_t *B, int sa, int sb, int sc, int sd, doub
             }
             double alpha = p * q / (p + q);
             double Rt[5][5][5][5];
-            hermite_R(L, alpha, RPQ, Rt);
+            hermite_R(L, alpha, omega, RPQ, Rt);
             double pref = 2.0 * pow(M_PI, 2.5) / (p * q * sqrt(p + q)) * cab * ccd;
             int idx = 0;
             for (int ca = 0; ca < n[0]; ++ca)
@@ -270,6 +279,11 @@ static void shell_quartet(const basis_t *B, int sa, int sb, int sc, int sd, doub
     for (int i = 0; i < ntot; ++i) out[i] = (double)acc[i];
 }
 
+static void shell_quartet(const basis_t *B, int sa, int sb, int sc, int sd, double *out)
+{
+    shell_quartet_op(B, sa, sb, sc, sd, 0.0, out);
+}
+
 void oracle_shell_quartet(BASIS_ARGS, int sa, int sb, int sc, int sd, double *out)
 {
     basis_t B = BASIS_MK;
@@ -290,8 +304,28 @@ void oracle_primitive_eri(const double *ctr /* [4][3] */, const double *ex /* [4
     shell_quartet(&B, 0, 1, 2, 3, out);
 }
 
+/* Same for the operator erf(omega r12)/r12 (omega <= 0: 1/r12). */
+void oracle_primitive_eri_erf(const double *ctr, const double *ex, const int32_t *l4, double omega, double *out)
+{
+    int32_t sh_center[4] = {0, 1, 2, 3}, sh_nprim[4] = {1, 1, 1, 1}, sh_off[4] = {0, 1, 2, 3};
+    int32_t ao_off[4];
+    double ncoef[4] = {1.0, 1.0, 1.0, 1.0};
+    int o = 0;
+    for (int i = 0; i < 4; ++i) { ao_off[i] = o; o += 2 * l4[i] + 1; }
+    basis_t B = mk_basis(4, ctr, sh_center, l4, sh_nprim, sh_off, ao_off, ex, ncoef);
+    shell_quartet_op(&B, 0, 1, 2, 3, omega, out);
+}
+
+void oracle_eri_tensor_erf(BASIS_ARGS, int nao, double omega, double *eri);
+
 /* Full AO tensor (mu nu|lam sig), [nao]^4, NO symmetry used (tiny systems only). */
 void oracle_eri_tensor(BASIS_ARGS, int nao, double *eri)
+{
+    oracle_eri_tensor_erf(nshells, centers, sh_center, sh_l, sh_nprim, sh_off, ao_off, exps, ncoef, nao, 0.0, eri);
+}
+
+/* Full AO tensor of erf(omega r12)/r12 (omega <= 0: 1/r12). */
+void oracle_eri_tensor_erf(BASIS_ARGS, int nao, double omega, double *eri)
 {
     basis_t B = BASIS_MK;
     #pragma omp parallel for schedule(dynamic) collapse(2)
@@ -300,7 +334,7 @@ void oracle_eri_tensor(BASIS_ARGS, int nao, double *eri)
         for (int sc = 0; sc < nshells; ++sc)
         for (int sd = 0; sd < nshells; ++sd) {
             double blk[81];
-            shell_quartet(&B, sa, sb, sc, sd, blk);
+            shell_quartet_op(&B, sa, sb, sc, sd, omega, blk);
             int n0 = 2 * sh_l[sa] + 1, n1 = 2 * sh_l[sb] + 1, n2 = 2 * sh_l[sc] + 1,
                 n3 = 2 * sh_l[sd] + 1, idx = 0;
             for (int ca = 0; ca < n0; ++ca)
@@ -373,9 +407,23 @@ void oracle_schwarz(BASIS_ARGS, double *Q)
 /* oracle_jk_strided visits only the bra pairs ab with ab % ab_stride == ab_phase (all their kets): a
  * BOUNDED SAMPLE of the same loop, used only to time the oracle on workloads whose full pass takes
  * tens of minutes (bench.py cpu_baseline); its J/K are then partial sums.  oracle_jk = stride 1. */
+void oracle_jk_strided_op(BASIS_ARGS, int nao, int nvec, const double *T, double tau, const double *Qs,
+                          int ab_stride, int ab_phase, double omega,
+                          double *J, double *K, int64_t *nquartets, int64_t *nprimq);
+
 void oracle_jk_strided(BASIS_ARGS, int nao, int nvec, const double *T, double tau, const double *Qs,
                        int ab_stride, int ab_phase,
                        double *J, double *K, int64_t *nquartets, int64_t *nprimq)
+{
+    oracle_jk_strided_op(nshells, centers, sh_center, sh_l, sh_nprim, sh_off, ao_off, exps, ncoef, nao, nvec, T, tau, Qs,
+                         ab_stride, ab_phase, 0.0, J, K, nquartets, nprimq);
+}
+
+/* The same loop for the operator erf(omega r12)/r12 (omega <= 0: 1/r12).  The screening bounds Qs stay those of
+ * 1/r12, which dominate the attenuated integrals (erf <= 1). */
+void oracle_jk_strided_op(BASIS_ARGS, int nao, int nvec, const double *T, double tau, const double *Qs,
+                          int ab_stride, int ab_phase, double omega,
+                          double *J, double *K, int64_t *nquartets, int64_t *nprimq)
 {
     basis_t B = BASIS_MK;
     size_t nn = (size_t)nao * nao;
@@ -404,7 +452,7 @@ void oracle_jk_strided(BASIS_ARGS, int nao, int nvec, const double *T, double ta
                 ++nq;
                 npq += (int64_t)sh_nprim[sa] * sh_nprim[sb] * sh_nprim[sc] * sh_nprim[sd];
                 double blk[81];
-                shell_quartet(&B, sa, sb, sc, sd, blk);
+                shell_quartet_op(&B, sa, sb, sc, sd, omega, blk);
                 double w = 1.0;
                 if (sa == sb) w *= 0.5;
                 if (sc == sd) w *= 0.5;

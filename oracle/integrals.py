@@ -112,6 +112,32 @@ class OracleBasis:
         lib().oracle_eri_tensor(*self._args(), ct.c_int(N), eri.ctypes.data_as(_dp))
         return eri
 
+    def eri_tensor_erf(self, omega: float) -> np.ndarray:
+        """Full AO tensor of the attenuated operator erf(omega r12)/r12 (omega <= 0: 1/r12)."""
+        N = self.nao
+        if N > 256:
+            raise ValueError("full N^4 tensor only for small systems (N <= 256)")
+        eri = np.zeros((N, N, N, N))
+        lib().oracle_eri_tensor_erf(*self._args(), ct.c_int(N), ct.c_double(omega), eri.ctypes.data_as(_dp))
+        return eri
+
+    def jk_erf(self, T: np.ndarray, omega: float, tau: float = 0.0, Q: np.ndarray | None = None):
+        """J, K of erf(omega r12)/r12 over the quartets with Q_ab Q_cd >= tau (Q: Schwarz bounds of 1/r12)."""
+        T = np.ascontiguousarray(T, dtype=np.float64)
+        if T.ndim == 2:
+            T = T[None]
+        if Q is None:
+            Q = self.schwarz()
+        Q = np.ascontiguousarray(Q)
+        J = np.zeros_like(T)
+        K = np.zeros_like(T)
+        nq = ct.c_int64(0)
+        npq = ct.c_int64(0)
+        lib().oracle_jk_strided_op(*self._args(), ct.c_int(self.nao), ct.c_int(T.shape[0]), T.ctypes.data_as(_dp),
+                                   ct.c_double(tau), Q.ctypes.data_as(_dp), ct.c_int(1), ct.c_int(0), ct.c_double(omega),
+                                   J.ctypes.data_as(_dp), K.ctypes.data_as(_dp), ct.byref(nq), ct.byref(npq))
+        return J, K, nq.value, npq.value
+
     def eri_pair_block(self, sc: int, sd: int, tau: float = 0.0, Q: np.ndarray | None = None) -> np.ndarray:
         """(mu nu|lam sig) for all mu, nu and the AOs lam, sig of the shell pair (sc, sd): [N][N][nc][nd]."""
         nc, nd = 2 * int(self.sh_l[sc]) + 1, 2 * int(self.sh_l[sd]) + 1
@@ -210,6 +236,16 @@ def primitive_eri(centers4, exps4, l4) -> np.ndarray:
     l, pl = _i(l4)
     out = np.zeros([2 * int(x) + 1 for x in l])
     lib().oracle_primitive_eri(pc, pe, pl, out.ctypes.data_as(_dp))
+    return out
+
+
+def primitive_eri_erf(centers4, exps4, l4, omega: float) -> np.ndarray:
+    """Primitive block of erf(omega r12)/r12 with unit coefficients (omega <= 0: 1/r12), for the pins."""
+    c, pc = _d(np.asarray(centers4).reshape(4, 3))
+    e, pe = _d(exps4)
+    l, pl = _i(l4)
+    out = np.zeros([2 * int(x) + 1 for x in l])
+    lib().oracle_primitive_eri_erf(pc, pe, pl, ct.c_double(omega), out.ctypes.data_as(_dp))
     return out
 
 

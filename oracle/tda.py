@@ -39,6 +39,25 @@ def build_A(eri, C_o, C_v, eps, cx=1.0):
     return A
 
 
+def build_A_rs(eri, eri_lr, C_o, C_v, eps, cx, cx_lr):
+    """Range-separated exchange (NEXT-4; CAM-type functionals):
+    A_{ia,jb} = delta delta (eps_a - eps_i) + 2 (ia|jb) - c_x (ij|ab) - c_x^LR (ij| erf(omega r12)/r12 |ab),
+    `eri_lr` being the AO tensor of the attenuated operator (OracleBasis.eri_tensor_erf)."""
+    no, nv = C_o.shape[1], C_v.shape[1]
+    A = build_A(eri, C_o, C_v, eps, cx)
+    _, oovv_lr = mo_eri_blocks(eri_lr, C_o, C_v)
+    return A - cx_lr * np.transpose(oovv_lr, (0, 2, 1, 3)).reshape(no * nv, no * nv)
+
+
+def sigma_matrix_free_rs(ob, X, C_o, C_v, eps, cx, cx_lr, omega, tau=0.0, Q=None):
+    """sigma for the range-separated A through the matrix-free routes: F = 2 J - c_x K - c_x^LR K_erf."""
+    T = transition_density(X, C_o, C_v)
+    J, K, nq, npq = ob.jk(T, tau=tau, Q=Q)
+    _, K_lr, _, _ = ob.jk_erf(T, omega, tau=tau, Q=Q)
+    return sigma_from_jk(X, J, K + (cx_lr / cx) * K_lr if cx != 0.0 else K, C_o, C_v, eps, cx) if cx != 0.0 else \
+        sigma_from_jk(X, J, K_lr, C_o, C_v, eps, cx_lr), nq, npq
+
+
 def build_A_by_pair_blocks(ob, C_o, C_v, eps, cx=1.0, tau=0.0, Q=None, progress=None):
     """Dense singles block of A (eq. 3 under R1) for systems whose AO tensor does not fit (SURVEY 8(c5) route ii):
     AO integrals one ket shell pair (lam sig) at a time, half-transformed at once,

@@ -4,7 +4,7 @@ The product is the CUDA library librttda.so (csrc/, C-ABI in include/rttda.h); t
 thin binding.  It never imports oracle/ and has no CPU fallback.
 """
 from .binding import (Rttda, RttdaError, rttda_overlap, rttda_dipole_ao, rttda_fp64_peak, lib, LIB_PATH,
-                      EXPORTS, INFO, OPT_INCORE, OPT_GRAPH, make_field)
+                      EXPORTS, INFO, OPT_INCORE, OPT_GRAPH, OPT_CX_LR, OPT_RS_OMEGA, make_field)
 
 __all__ = ["Rttda", "RttdaError", "rttda_overlap", "rttda_dipole_ao", "rttda_fp64_peak", "lib", "LIB_PATH",
-           "EXPORTS", "INFO", "OPT_INCORE", "OPT_GRAPH", "make_field"]
+           "EXPORTS", "INFO", "OPT_INCORE", "OPT_GRAPH", "OPT_CX_LR", "OPT_RS_OMEGA", "make_field"]

@@ -19,6 +19,8 @@ INFO = dict(npairs_total=0, npairs_kept=1, nquartets=2, nprim_quartets=3, nquart
             create_ms=10, qmax=11, nvec_chunk=12, eri_buf_bytes=13, eri_all_bytes=14)
 OPT_INCORE = 1
 OPT_GRAPH = 2
+OPT_CX_LR = 3
+OPT_RS_OMEGA = 4
 FIELD_CONTINUE = 1
 PULSE = dict(none=0, delta=1, cw=2, tl=3, chirp=4, sin2=5)
 EXPORTS = ["rttda_overlap", "rttda_dipole_ao", "rttda_create", "rttda_destroy", "rttda_sigma",

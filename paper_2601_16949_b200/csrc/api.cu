@@ -261,9 +261,16 @@ int rttda_set_option(rttda_handle_t hh, int32_t option, double value)
     Handle* h = (Handle*)hh;
     RT_CHECK(h != nullptr, "rttda_set_option: NULL handle");
     RT_DEVICE(h);
-    RT_CHECK(option == RTTDA_OPT_INCORE || option == RTTDA_OPT_GRAPH, "rttda_set_option: unknown option");
+    RT_CHECK(option == RTTDA_OPT_INCORE || option == RTTDA_OPT_GRAPH || option == RTTDA_OPT_CX_LR || option == RTTDA_OPT_RS_OMEGA,
+             "rttda_set_option: unknown option");
     const bool on = value != 0.0;
     if (option == RTTDA_OPT_GRAPH) { h->use_graph = on; return RTTDA_OK; }
+    if (option == RTTDA_OPT_CX_LR || option == RTTDA_OPT_RS_OMEGA) {
+        RT_CHECK(option == RTTDA_OPT_CX_LR || value >= 0.0, "rttda_set_option: negative range-separation parameter");
+        (option == RTTDA_OPT_CX_LR ? h->cx_lr : h->rs_omega) = value;
+        if (h->step_graph) { cudaGraphExecDestroy(h->step_graph); h->step_graph = nullptr; }   // the captured step has one pass structure
+        return RTTDA_OK;
+    }
     if (on && !h->incore) {
         const int r = ensure_ws(h, &h->eri_all, &h->eri_all_n, h->eri_all_need);
         if (r != RTTDA_OK) return r;                       // not enough HBM: the handle stays in direct mode

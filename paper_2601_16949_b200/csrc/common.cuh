@@ -141,6 +141,12 @@ struct Handle {
     int device = 0;
     int nao = 0, nocc = 0, nvirt = 0, ncsf = 0, nshells = 0;
     double cx = 1.0, tau = 0.0;
+    // range-separated exchange (NEXT-4): A -= cx_lr (ij| erf(omega r12)/r12 |ab); rs_omega <= 0 or cx_lr == 0: off
+    double cx_lr = 0.0, rs_omega = 0.0;
+    // operator and digestion mode of the ERI pass being enqueued (set by jk_build, read by eval_segment / digest_launch)
+    double pass_w_extra = 0.0;                 // 36 / omega^2 added to w = 36/p + 36/q: integrals of erf(omega r)/r
+    double pass_cx = 1.0;                      // exchange factor of this pass
+    bool pass_do_j = true, pass_do_k = true;
     // device-resident inputs
     double *C_occ = nullptr, *C_virt = nullptr, *deps = nullptr;
     double* D_ao = nullptr;                    // [3][nao][nao]

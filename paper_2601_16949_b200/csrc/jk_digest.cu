@@ -657,7 +657,7 @@ static int launch_digest_j(Handle* h, const JKLaunch& L, const Segment& sg, cons
     g.work = L.work;
     g.batch_base = sg.batch_base;
     g.buf = buf;
-    g.Tq = Tq; g.PPq = nullptr; g.Fq = Fq; g.cx = h->cx;
+    g.Tq = Tq; g.PPq = nullptr; g.Fq = Fq; g.cx = h->pass_cx;
     g.ketclass = L.ketclass; g.same = (sg.kc_bra == sg.kc_ket); g.nvt = nvt; g.v0 = v0;
     constexpr int NI = (2 * LA + 1) * (2 * LB + 1) * (2 * LC + 1) * (2 * LD + 1);
     constexpr size_t smem = digest_ring_bytes(NI);
@@ -678,7 +678,7 @@ static int launch_digest(Handle* h, const JKLaunch& L, const Segment& sg, const 
                          const double* Tq, double* Fq, cudaStream_t st)
 {
     constexpr int NC = 2 * LC + 1, ND = 2 * LD + 1;
-    if (LA >= LB) {
+    if (LA >= LB && h->pass_do_j) {
         constexpr int NVJ = (NC * ND <= 3) ? 8 : 4;
         int v0 = 0;
         while (v0 < nvec) {
@@ -693,6 +693,7 @@ static int launch_digest(Handle* h, const JKLaunch& L, const Segment& sg, const 
     constexpr size_t smem = (size_t)2 * NI * 256;
     RT_CUDA(cudaFuncSetAttribute(digest_b_kernel<LA, LB, LC, LD>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     RT_CUDA(cudaFuncSetAttribute(digest_k_kernel<LA, LB, LC, LD>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)digest_k_smem(NI)));
+    if (!h->pass_do_k || h->pass_cx == 0.0) return RTTDA_OK;
     for (int v0 = 0; v0 < nvec; v0 += 8) {
         // lane groups of 2, 4 or 8 densities: a group then never straddles a quarter warp, so one 16-byte gather per
         // lane costs one L1 wavefront per ket (groups of 6 cost ~1.6); lanes beyond the call's densities work on the
@@ -701,7 +702,7 @@ static int launch_digest(Handle* h, const JKLaunch& L, const Segment& sg, const 
         DigestArgs g;
         g.nvleft = left;
         g.tb = h->tabs; g.work = L.work; g.batch_base = sg.batch_base; g.buf = buf;
-        g.Tq = Tq; g.PPq = h->wsP; g.Fq = Fq; g.cx = h->cx;
+        g.Tq = Tq; g.PPq = h->wsP; g.Fq = Fq; g.cx = h->pass_cx;
         g.ketclass = L.ketclass; g.same = (sg.kc_bra == sg.kc_ket); g.nvt = nvt; g.v0 = v0;
         const int KW = 32 / G, nwarps = (32 + KW - 1) / KW;
         // one or three integrals per quartet: the multi-record ring (digest_k_kernel) wins; above that its larger
@@ -765,6 +766,17 @@ int jk_build(Handle* h, int nvt, int nvec, const double* Tq, double* Fq, cudaStr
         RT_CUDA(cudaGetLastError());
         h->kernel_launches++;
     }
+    const bool lr = (h->cx_lr != 0.0 && h->rs_omega > 0.0);
+    RT_CHECK(!(lr && h->incore), "jk_build: the in-core store holds the integrals of ONE operator; switch RTTDA_OPT_INCORE off "
+                                 "when range-separated exchange is on");
+    // ERI passes of this build: the 1/r12 pass (Coulomb + c_x exchange), and, with range-separated exchange, a second
+    // pass over the same quartets with the integrals of erf(omega r12)/r12, digested into the exchange part only
+    const int npass = lr ? 2 : 1;
+    for (int pass = 0; pass < npass; ++pass) {
+    h->pass_w_extra = pass == 0 ? 0.0 : 36.0 / (h->rs_omega * h->rs_omega);
+    h->pass_cx = pass == 0 ? h->cx : h->cx_lr;
+    h->pass_do_j = (pass == 0);
+    h->pass_do_k = true;
     if (h->incore) {
         // In-core mode (optional, off by default): every segment owns its part of one resident store; the first
         // pass fills it, later passes only digest.  This trades 8 bytes of HBM per integral for the evaluation.
@@ -777,7 +789,7 @@ int jk_build(Handle* h, int nvt, int nvec, const double* Tq, double* Fq, cudaStr
                 RT_TRY(digest_launch(h, h->launches[l], sg, buf, nvt, nvec, Tq, Fq, st));
         }
         h->incore_valid = true;
-        return RTTDA_OK;
+        continue;
     }
     if (h->nlanes == 0) {
         // Pipeline mode (large molecules: every kernel fills the GPU on its own, and two kernels of the same kind
@@ -800,7 +812,8 @@ int jk_build(Handle* h, int nvt, int nvec, const double* Tq, double* Fq, cudaStr
             RT_CUDA(cudaEventRecord(evD[b], st));
             ++k;
         }
-        return RTTDA_OK;
+        // the evaluation stream's last kernels were consumed by the digestion above; a following pass reuses the buffers
+        continue;
     }
     RT_CUDA(cudaEventRecord(h->ev_fork, st));
     for (int l = 0; l < h->nlanes; ++l) {
@@ -816,6 +829,8 @@ int jk_build(Handle* h, int nvt, int nvec, const double* Tq, double* Fq, cudaStr
         RT_CUDA(cudaEventRecord(h->lane_ev[l], ls));
         RT_CUDA(cudaStreamWaitEvent(st, h->lane_ev[l], 0));
     }
+    }   // passes
+    h->pass_w_extra = 0.0; h->pass_cx = h->cx; h->pass_do_j = h->pass_do_k = true;
     return RTTDA_OK;
 }
 

@@ -21,6 +21,7 @@ struct EvalArgs {
     const double2* boys;
     double* buf;
     double tau;
+    double w_extra;        // 0 for 1/r12; 36 / omega^2 for erf(omega r12)/r12 (alpha -> alpha omega^2 / (alpha + omega^2))
     int same;
 };
 
@@ -100,7 +101,7 @@ __global__ void __launch_bounds__(JK_BLOCK) eval_kernel(EvalArgs g)
     PrimPair kp[KET_IN_REGS ? KP : 1];
     if (KET_IN_REGS) {
 #pragma unroll
-        for (int k = 0; k < KP; ++k) kp[k] = load_ket_prim<LC, LD>(g.ket.prim, g.ket.n, k, qq);
+        for (int k = 0; k < KP; ++k) { kp[k] = load_ket_prim<LC, LD>(g.ket.prim, g.ket.n, k, qq); kp[k].p += g.w_extra; }
     }
 
     for (int ip = 0; ip < npairs; ++ip) {
@@ -128,7 +129,8 @@ __global__ void __launch_bounds__(JK_BLOCK) eval_kernel(EvalArgs g)
             // ket primitive outermost: it is loaded once (coalesced, L1) and meets every bra primitive (shared memory)
 #pragma unroll 1
             for (int kk = 0; kk < KP; ++kk) {
-                const PrimPair k1 = load_ket_prim<LC, LD>(g.ket.prim, g.ket.n, kk, qq);
+                PrimPair k1 = load_ket_prim<LC, LD>(g.ket.prim, g.ket.n, kk, qq);
+                k1.p += g.w_extra;
 #pragma unroll 1
                 for (int kb = 0; kb < npb; ++kb) {
                     const PrimPair bp = load_bra_prim_smem(rows + kb * PRIM_STRIDE);
@@ -155,6 +157,7 @@ static int launch_eval(Handle* h, const Segment& sg, double* buf, cudaStream_t s
     g.boys = h->tabs.boys[LA + LB + LC + LD];
     g.buf = buf;
     g.tau = h->tabs.tau;
+    g.w_extra = h->pass_w_extra;
     g.same = (sg.kc_bra == sg.kc_ket);
     dim3 grid(sg.nitems), block(JK_BLOCK);
     switch (g.ket.np) {

@@ -260,3 +260,34 @@ def test_eigs_config2_lowest_states_and_populations():
     h.rttda_populations(torch.from_numpy(y).to(ctx["dev"]), torch.from_numpy(Xs).to(ctx["dev"]), P)
     torch.cuda.synchronize()
     assert np.max(np.abs(P.cpu().numpy()[0] - np.array([0.0, 0.0, 0.0, 1.0, 0.0]))) < 1e-9
+
+
+@pytest.mark.parametrize("cx,cx_lr,omega", [(0.19, 0.46, 0.33), (0.0, 1.0, 0.5), (1.0, 0.3, 2.0)])
+def test_range_separated_exchange_tiny_dense_and_config2(cx, cx_lr, omega):
+    """NEXT-4: A with the long-range exchange term - c_x^LR (ij|erf(omega r12)/r12|ab) (RTTDA_OPT_CX_LR / _RS_OMEGA: a
+    second ERI pass with attenuated integrals) against the oracle's dense A on config 1 and its matrix-free route on
+    config 2; switching the option off again restores the plain operator."""
+    import paper_2601_16949_b200 as R
+    from workloads import make_vectors
+    from oracle import tda
+    ctx = setup_config(1, dense=True)
+    ob = ctx["ob"]
+    A = tda.build_A_rs(ob.eri_tensor(), ob.eri_tensor_erf(omega), ctx["C_o"], ctx["C_v"], ctx["eps"], cx, cx_lr)
+    X = make_vectors(ctx["cfg"], 5)
+    h = _handle(ctx, cx, 1e-12)
+    plain = _sigma(h, X, ctx["dev"])
+    h.rttda_set_option(R.OPT_CX_LR, cx_lr)
+    h.rttda_set_option(R.OPT_RS_OMEGA, omega)
+    assert rel_inf(_sigma(h, X, ctx["dev"]), tda.sigma_dense(A, X)) < 1e-12
+    h.rttda_set_option(R.OPT_CX_LR, 0.0)
+    assert np.array_equal(_sigma(h, X, ctx["dev"]), plain) or rel_inf(_sigma(h, X, ctx["dev"]), plain) < 1e-14
+    h.close()
+    ctx2 = setup_config(2)
+    X = make_vectors(ctx2["cfg"], 6)
+    ref, _, _ = tda.sigma_matrix_free_rs(ctx2["ob"], X, ctx2["C_o"], ctx2["C_v"], ctx2["eps"], cx, cx_lr, omega, tau=1e-20)
+    h = _handle(ctx2, cx, 1e-12)
+    h.rttda_set_option(R.OPT_CX_LR, cx_lr)
+    h.rttda_set_option(R.OPT_RS_OMEGA, omega)
+    got = _sigma(h, X, ctx2["dev"])
+    h.close()
+    assert rel_inf(got, ref) < SIGMA_TOL

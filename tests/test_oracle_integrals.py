@@ -260,3 +260,66 @@ def test_schwarz_screening_error_is_bounded(tiny):
         assert nq <= n0 and err <= tau * np.sum(np.abs(T)) * 8
         assert err >= prev - 1e-15
         prev = err
+
+
+# ------------------------------------------------------------------------------------ erf-attenuated ERIs (NEXT-4)
+def test_erf_attenuated_ssss_against_gaussian_geminal_quadrature():
+    """erf(w r)/r = (2/sqrt(pi)) int_0^w exp(-s^2 r^2) ds, and the s-type integral of a Gaussian geminal has the closed form
+      (ab| exp(-s^2 r12^2) |cd) = K_ab K_cd (pi^2 / (pq + s^2 (p+q)))^(3/2) exp(-pq s^2 / (pq + s^2 (p+q)) |PQ|^2),
+    so (ss|erf(w r12)/r12|ss) is a one-dimensional quadrature of elementary functions (scipy.integrate.quad): no Boys
+    function, no theta prefactor, nothing the oracle's Hermite route uses."""
+    from scipy.integrate import quad
+    from oracle.integrals import primitive_eri_erf
+    rng = np.random.default_rng(17)
+    for omega in (0.2, 0.33, 1.0, 4.0):
+        for _ in range(5):
+            ctr = rng.uniform(-1.5, 1.5, size=(4, 3))
+            a, b, c, d = ex = np.exp(rng.uniform(np.log(0.1), np.log(10), size=4))
+            p, q = a + b, c + d
+            P = (a * ctr[0] + b * ctr[1]) / p
+            Q = (c * ctr[2] + d * ctr[3]) / q
+            K = np.exp(-a * b / p * np.sum((ctr[0] - ctr[1]) ** 2)) * np.exp(-c * d / q * np.sum((ctr[2] - ctr[3]) ** 2))
+            R2 = float(np.sum((P - Q) ** 2))
+
+            def geminal(s):
+                den = p * q + s * s * (p + q)
+                return (np.pi ** 2 / den) ** 1.5 * np.exp(-p * q * s * s / den * R2)
+            ref = 2.0 / np.sqrt(np.pi) * quad(geminal, 0.0, omega, epsabs=1e-15, epsrel=1e-13)[0] * K
+            val = primitive_eri_erf(ctr, ex, [0, 0, 0, 0], omega).item()
+            assert abs(val - ref) < 1e-11 * max(1.0, abs(ref))
+
+
+@pytest.mark.parametrize("l4", [(0, 0, 0, 0), (1, 0, 0, 0), (1, 1, 0, 0), (1, 0, 1, 0), (1, 1, 1, 0), (1, 1, 1, 1)])
+def test_erf_attenuated_limits_and_bounds(l4):
+    """omega -> infinity recovers 1/r12; omega -> 0 gives (2 omega / sqrt(pi)) <a|b> <c|d> (erf(x) ~ 2x/sqrt(pi));
+    omega <= 0 means the Coulomb operator; and for the positive (ss|ss) integrand the value grows with omega."""
+    from oracle.integrals import primitive_eri_erf
+    rng = np.random.default_rng(23)
+    ctr = rng.uniform(-1.0, 1.0, size=(4, 3))
+    ex = np.array([0.7, 1.3, 0.45, 0.9])
+    full = primitive_eri(ctr, ex, l4)
+    assert np.array_equal(primitive_eri_erf(ctr, ex, l4, 0.0), full)
+    assert np.max(np.abs(primitive_eri_erf(ctr, ex, l4, 1e6) - full)) < 1e-10 * np.max(np.abs(full))
+    w = 1e-4
+    Sab = _raw_1e(ctr[0], l4[0], ex[0], ctr[1], l4[1], ex[1])
+    Scd = _raw_1e(ctr[2], l4[2], ex[2], ctr[3], l4[3], ex[3])
+    lim = 2.0 * w / np.sqrt(np.pi) * np.einsum("ab,cd->abcd", Sab, Scd)
+    got = primitive_eri_erf(ctr, ex, l4, w)
+    assert np.max(np.abs(got - lim)) < 1e-6 * np.max(np.abs(lim)) + 1e-18
+    if sum(l4) == 0:
+        vals = [primitive_eri_erf(ctr, ex, l4, x).item() for x in (0.1, 0.3, 1.0, 3.0, 30.0)]
+        assert all(0.0 < u < v for u, v in zip(vals, vals[1:])) and vals[-1] < full.item()
+
+
+def test_erf_attenuated_tensor_symmetry_and_jk_route(tiny):
+    """The attenuated AO tensor keeps the 8-fold symmetry, is dominated by the Coulomb Schwarz bounds, and the matrix-free
+    J/K route with the operator switch equals the plain contraction of that tensor."""
+    ob, N = tiny["ob"], tiny["ob"].nao
+    e = ob.eri_tensor_erf(0.33)
+    assert np.max(np.abs(e - e.transpose(1, 0, 2, 3))) < 1e-14 and np.max(np.abs(e - e.transpose(2, 3, 0, 1))) < 1e-14
+    diag = np.sqrt(np.einsum("mnmn->mn", tiny["eri"]))
+    assert np.all(np.abs(e) <= diag[:, :, None, None] * diag[None, None, :, :] + 1e-14)
+    T = np.random.default_rng(3).standard_normal((2, N, N))
+    J, K, _, _ = ob.jk_erf(T, 0.33, tau=0.0)
+    assert np.max(np.abs(J - np.einsum("mnls,vls->vmn", e, T))) < 1e-12
+    assert np.max(np.abs(K - np.einsum("mnls,vns->vml", e, T))) < 1e-12

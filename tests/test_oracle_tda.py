@@ -570,3 +570,24 @@ def test_davidson_lowest_eigenpairs_against_eigh(tiny):
         P = U[:, :k] @ U[:, :k].T                                   # projector on the exact lowest-k subspace
         assert np.max(np.abs(X @ P - X)) < 1e-6
         assert it < 60
+
+
+def test_range_separated_A_limits_and_matrix_free_route(tiny):
+    """A with range-separated exchange (NEXT-4): omega -> infinity turns c_x^LR into ordinary exchange
+    (A(c_x, c_x^LR, inf) = A(c_x + c_x^LR)), c_x^LR = 0 changes nothing, the long-range block is symmetric PSD, and the
+    matrix-free route equals the dense one."""
+    ob, C_o, C_v, eps = tiny["ob"], tiny["C_o"], tiny["C_v"], tiny["eps"]
+    e_inf = ob.eri_tensor_erf(1e7)
+    A = tda.build_A_rs(tiny["eri"], e_inf, C_o, C_v, eps, 0.19, 0.46)
+    assert np.max(np.abs(A - tda.build_A(tiny["eri"], C_o, C_v, eps, 0.65))) < 1e-9
+    e = ob.eri_tensor_erf(0.33)
+    assert np.array_equal(tda.build_A_rs(tiny["eri"], e, C_o, C_v, eps, 0.4, 0.0), tda.build_A(tiny["eri"], C_o, C_v, eps, 0.4))
+    A = tda.build_A_rs(tiny["eri"], e, C_o, C_v, eps, 0.19, 0.46)
+    assert np.max(np.abs(A - A.T)) < 1e-13
+    Klr = (tda.build_A(tiny["eri"], C_o, C_v, eps, 0.19) - A) / 0.46          # (ij|erf|ab) as a matrix in (ia),(jb)
+    assert np.linalg.eigvalsh(0.5 * (Klr + Klr.T))[0] > -1e-12
+    X = make_vectors(tiny["cfg"], 3)
+    for cx in (0.19, 0.0):
+        Ad = tda.build_A_rs(tiny["eri"], e, C_o, C_v, eps, cx, 0.46)
+        s, _, _ = tda.sigma_matrix_free_rs(ob, X, C_o, C_v, eps, cx, 0.46, 0.33, tau=0.0)
+        assert np.max(np.abs(s - tda.sigma_dense(Ad, X))) < 1e-12
