@@ -227,13 +227,17 @@ class Rttda:
                "rttda_lanczos")
         return alpha, beta
 
-    def rttda_eigs(self, k: int, X, nblock: int = 0, tol: float = 1e-8, maxiter: int = 100, stream=None):
+    def rttda_eigs(self, k: int, X, nblock: int = 0, tol: float = 1e-8, maxiter: int = 100, stream=None,
+                   allow_nonconverged: bool = False):
         """Lowest k eigenpairs of A by block Davidson; X CUDA tensor [k][ncsf] receives the vectors.
-        Returns (omega [k], residual norms [k], iterations, sigma vectors built)."""
+        Returns (omega [k], residual norms [k], iterations, sigma vectors built).  RTTDA_ENOCONV raises unless
+        allow_nonconverged (the outputs then hold the current Ritz pairs and their residuals)."""
         om, rs = np.zeros(k), np.zeros(k)
         it, ns = ct.c_int32(0), ct.c_int32(0)
-        _check(lib().rttda_eigs(self._h, int(k), int(nblock or k), ct.c_double(tol), int(maxiter), _dptr(om), _dptr(X),
-                                _dptr(rs), ct.byref(it), ct.byref(ns), _stream(stream)), "rttda_eigs")
+        rc = lib().rttda_eigs(self._h, int(k), int(nblock or k), ct.c_double(tol), int(maxiter), _dptr(om), _dptr(X),
+                              _dptr(rs), ct.byref(it), ct.byref(ns), _stream(stream))
+        if not (allow_nonconverged and rc == -4):
+            _check(rc, "rttda_eigs")
         return om, rs, it.value, ns.value
 
     def rttda_populations(self, C, Xs, P, stream=None):
