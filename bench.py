@@ -56,6 +56,10 @@ def parse():
     ap.add_argument("--parity-tau", type=float, default=1e-14,
                     help="second, tighter threshold at which config 4 is also timed: the largest tau of the sweep at which "
                          "sigma meets the 1e-10 oracle tolerance at 1280 AO (tests/test_gpu_parity.py, DESIGN.md section 11); 0 = skip")
+    ap.add_argument("--omega", type=float, default=0.0, help="carrier frequency in Ha (0 = from rttda_eigs, see run_b200)")
+    ap.add_argument("--sweep-point", nargs=2, metavar=("NVEC", "TAU"), default=None,
+                    help="config 5, ONE point: 2 warm rttda_sigma calls, then one call between cudaProfilerStart/Stop "
+                         "(for `ncu --profile-from-start off`: FP64 pipe utilisation per point, profiles/README.md)")
     ap.add_argument("--sweep", action="store_true", help="run the config-5 sigma sweep (nvec x tau) instead of the step bench -> gpurun_out/sweep.json")
     return ap.parse_args()
 
@@ -270,18 +274,23 @@ def run_b200(args):
     D = R.rttda_dipole_ao(basis)
     dz = (C_o.T @ D[2] @ C_v).reshape(-1)
     nst = 1 if k == 3 else 6
-    Xe = torch.zeros((nst, ncsf), dtype=torch.float64, device=dev)
+    if args.omega > 0:
+        nst = 0
+    Xe = torch.zeros((max(nst, 1), ncsf), dtype=torch.float64, device=dev)
     t_e = time.perf_counter()
-    om_e, res_e, it_e, nsig_e = h.rttda_eigs(nst, Xe, max(nst, 6), tol=1e-4, maxiter=40 if k != 4 else 12, stream=st,
-                                             allow_nonconverged=True)
-    torch.cuda.synchronize()
-    eigs_s = time.perf_counter() - t_e
-    wts = (Xe.cpu().numpy() @ dz) ** 2
-    bright = int(np.argmax(wts))
-    omega = float(om_e[0]) if k != 4 else 0.5 * float(om_e[bright])
-    eigs_info = {"omega_states": [float(x) for x in om_e], "residuals": [float(x) for x in res_e], "iterations": it_e,
-                 "sigma_vectors": nsig_e, "seconds": eigs_s, "bright_state": bright,
-                 "dipole_weights": [float(x) for x in wts]}
+    if nst:
+        om_e, res_e, it_e, nsig_e = h.rttda_eigs(nst, Xe, max(nst, 6), tol=1e-4, maxiter=40 if k != 4 else 12, stream=st,
+                                                 allow_nonconverged=True)
+        torch.cuda.synchronize()
+        eigs_s = time.perf_counter() - t_e
+        wts = (Xe.cpu().numpy() @ dz) ** 2
+        bright = int(np.argmax(wts))
+        omega = float(om_e[0]) if k != 4 else 0.5 * float(om_e[bright])
+        eigs_info = {"omega_states": [float(x) for x in om_e], "residuals": [float(x) for x in res_e], "iterations": it_e,
+                     "sigma_vectors": nsig_e, "seconds": eigs_s, "bright_state": bright,
+                     "dipole_weights": [float(x) for x in wts]}
+    else:
+        omega, eigs_info = args.omega, "--omega given"
     fields = fields_for(cfg, args.ntraj, omega)
     ntraj = len(fields)
     nvec = 2 * ntraj
@@ -466,6 +475,33 @@ def run_b200(args):
         torch.distributed.destroy_process_group()
 
 
+# ------------------------------------------------------------------------------------------ config 5, one point under ncu
+def run_sweep_point(args):
+    import torch
+    import paper_2601_16949_b200 as R
+    from workloads import make_vectors
+    nvec, tau = int(args.sweep_point[0]), float(args.sweep_point[1])
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(0)
+    cfg, basis, C_o, C_v, eps, cond, bump = build_inputs(4, R.rttda_overlap)
+    st = torch.cuda.current_stream()
+    h = R.Rttda(basis, torch.from_numpy(C_o).to(dev), torch.from_numpy(C_v).to(dev), eps, 1.0, tau, st)
+    X = torch.from_numpy(make_vectors(cfg, nvec)).to(dev)
+    out = torch.empty_like(X)
+    for _ in range(2):
+        h.rttda_sigma(X, out, st)
+    torch.cuda.synchronize()
+    torch.cuda.cudart().cudaProfilerStart()
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    a.record(st); h.rttda_sigma(X, out, st); b.record(st)
+    torch.cuda.synchronize()
+    torch.cuda.cudart().cudaProfilerStop()
+    info = h.info()
+    print(json.dumps({"nvec": nvec, "tau": tau, "ms": a.elapsed_time(b), "unique_shell_quartets": info["nquartets"],
+                      "primitive_quartets": info["nprim_quartets"]}))
+    h.close()
+
+
 # ------------------------------------------------------------------------------------------ config 5 sweep
 def run_sweep(args):
     """BJ:configs[4]: batched sigma microbenchmark at the 1280-AO molecule, nvec x tau; 3 warm-ups + 10 timed
@@ -522,7 +558,9 @@ def run_sweep(args):
 
 if __name__ == "__main__":
     a = parse()
-    if a.sweep:
+    if a.sweep_point:
+        run_sweep_point(a)
+    elif a.sweep:
         run_sweep(a)
     elif a.impl == "reference":
         run_reference(a)

@@ -144,8 +144,10 @@ int rttda_propagate_host(rttda_handle_t h, int32_t ntraj, double* C, const rttda
 #define RTTDA_INFO_NQUARTETS         2   /* unique shell quartets with Q_ab Q_cd >= tau (R14) */
 #define RTTDA_INFO_NPRIM_QUARTETS    3   /* primitive quartets inside those */
 #define RTTDA_INFO_NQUARTETS_EVAL    4   /* contracted quartet evaluations the kernels perform per ERI pass */
-#define RTTDA_INFO_NPRIM_EVAL        5   /* primitive quartet evaluations per ERI pass */
-#define RTTDA_INFO_FLOPS_EVAL        6   /* FP64 flop model of one ERI pass, evaluation part */
+#define RTTDA_INFO_NPRIM_EVAL        5   /* primitive quartet evaluations per ERI pass (after primitive-pair screening:
+                                            primitive pairs whose own bound q_k has q_k Q_max < 1e-3 tau are dropped) */
+#define RTTDA_INFO_FLOPS_EVAL        6   /* FP64 flop model of one ERI pass, evaluation part: on the primitive quartets
+                                            actually evaluated (RTTDA_INFO_NPRIM_EVAL) */
 #define RTTDA_INFO_FLOPS_DIGEST_PER_VEC 7 /* FP64 flop model, digestion per density */
 #define RTTDA_INFO_JK_LAUNCHES       8   /* kernel launches of one ERI pass */
 #define RTTDA_INFO_KERNEL_LAUNCHES   9   /* kernels launched by this handle so far (all entry points) */

@@ -43,10 +43,11 @@ void set_error(const std::string& msg);
 // so that c_bra * c_ket / sqrt(p+q) = 2 pi^(5/2) / (p q sqrt(p+q)) * K_ab K_cd * coefficients.
 constexpr int PRIM_STRIDE = 12;
 
-// Pair classes: 0 = ss, 1 = ps (p first), 2 = pp; contraction sub-class by number of primitive pairs.
-constexpr int NSUB = 3;                       // nprim pairs in {1, 3, 9}
+// Pair classes: 0 = ss, 1 = ps (p first), 2 = pp; contraction sub-class by number of primitive pairs kept after
+// primitive screening (setup.cu), rounded up to 1, 3, 6 or 9.
+constexpr int NSUB = 4;                       // primitive pairs stored per shell pair: {1, 3, 6, 9}
 constexpr int NKETCLASS = 3 * NSUB;           // ket class id = pairclass * NSUB + sub
-__host__ __device__ inline int sub_to_np(int sub) { return sub == 0 ? 1 : (sub == 1 ? 3 : 9); }
+__host__ __device__ inline int sub_to_np(int sub) { return sub == 0 ? 1 : (sub == 1 ? 3 : (sub == 2 ? 6 : 9)); }
 
 // Unique (unordered) pairs of one pair class (pair type x contraction sub-class), sorted by Schwarz bound
 // descending.  The same list serves as the BRA list of the evaluation kernels (block-uniform side, AoS rows

@@ -163,6 +163,7 @@ static int launch_eval(Handle* h, const Segment& sg, double* buf, cudaStream_t s
     switch (g.ket.np) {
         case 1: eval_kernel<LA, LB, LC, LD, 1><<<grid, block, 0, st>>>(g); break;
         case 3: eval_kernel<LA, LB, LC, LD, 3><<<grid, block, 0, st>>>(g); break;
+        case 6: eval_kernel<LA, LB, LC, LD, 6><<<grid, block, 0, st>>>(g); break;
         default: eval_kernel<LA, LB, LC, LD, 9><<<grid, block, 0, st>>>(g); break;
     }
     h->kernel_launches++;

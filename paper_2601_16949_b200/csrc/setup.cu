@@ -195,6 +195,7 @@ struct Pair {
     int s1, s2;          // first (higher l, or larger index at equal l), second
     int pc, sub, np;     // pair class, contraction sub-class, primitive pairs (stored)
     int np_true;         // primitive pairs as given (2-primitive shells are padded), for the R14 counters
+    std::vector<int> sel; // the primitive rows kept (offsets from `row`, ascending), np of them
     int row;             // first row in the per-class candidate prim table
     double Q;
     int pos;             // position in its ket class after sorting
@@ -212,7 +213,7 @@ static int upload(Handle* h, const std::vector<T>& v, const T** out)
     return RTTDA_OK;
 }
 
-static int np_to_sub(int np) { return np == 1 ? 0 : (np == 3 ? 1 : 2); }
+static int np_to_sub(int np) { return np == 1 ? 0 : (np == 3 ? 1 : (np == 6 ? 2 : 3)); }
 
 // Flop model of one primitive quartet of total angular momentum L, bra/ket split irrelevant at this
 // granularity: geometry + prefactor, Boys, R recursion, operator stages.
@@ -283,6 +284,7 @@ int create_impl(Handle* h, const rttda_basis_t* basis, const double* C_occ, cons
         }
 
     // ---- Schwarz bounds on the device
+    std::vector<double> qprim[3];
     for (int pc = 0; pc < 3; ++pc) {
         const int n = (int)cand_np[pc].size();
         if (!n) continue;
@@ -302,11 +304,51 @@ int create_impl(Handle* h, const rttda_basis_t* basis, const double* C_occ, cons
         RT_CUDA(cudaMemcpyAsync(Q.data(), d_Q, n * sizeof(double), cudaMemcpyDeviceToHost, st));
         RT_CUDA(cudaStreamSynchronize(st));
         for (int k = 0; k < n; ++k) pairs[cand_id[pc][k]].Q = Q[k];
+        // primitive-level bounds: every primitive pair as a shell pair of its own, q_k = sqrt(max (kk|kk))
+        const int nrow = (int)(rows[pc].size() / PRIM_STRIDE);
+        std::vector<int> one(nrow, 1), idx(nrow);
+        std::iota(idx.begin(), idx.end(), 0);
+        DevTmp t_np1, t_off1, t_Q1;
+        RT_CUDA(cudaMalloc(&t_np1.p, nrow * sizeof(int)));
+        RT_CUDA(cudaMalloc(&t_off1.p, nrow * sizeof(int)));
+        RT_CUDA(cudaMalloc(&t_Q1.p, nrow * sizeof(double)));
+        RT_CUDA(cudaMemcpyAsync(t_np1.p, one.data(), nrow * sizeof(int), cudaMemcpyHostToDevice, st));
+        RT_CUDA(cudaMemcpyAsync(t_off1.p, idx.data(), nrow * sizeof(int), cudaMemcpyHostToDevice, st));
+        RT_TRY(schwarz_device(pc, nrow, (int*)t_np1.p, (int*)t_off1.p, d_prim, h->tabs.boys[2 * pc], (double*)t_Q1.p, st));
+        h->kernel_launches++;
+        qprim[pc].resize(nrow);
+        RT_CUDA(cudaMemcpyAsync(qprim[pc].data(), t_Q1.p, nrow * sizeof(double), cudaMemcpyDeviceToHost, st));
+        RT_CUDA(cudaStreamSynchronize(st));
     }
     double Qmax = 0.0;
     for (const Pair& P : pairs) Qmax = std::max(Qmax, P.Q);
     RT_CHECK(Qmax > 0.0 && std::isfinite(Qmax), "Schwarz bounds are not finite/positive");
     const double tau = h->tau;
+
+    // ---- primitive screening: a primitive pair k whose own bound q_k cannot lift any integral above tau_p = 1e-3 tau
+    // (q_k Q_max < tau_p; |(k.|cd)| <= q_k Q_cd) is dropped from its shell pair, and the pair moves to the contraction
+    // sub-class of what is left (9 -> 6 -> 3 -> 1 primitive pairs; kept rows stay in exponent order).  The Schwarz bound Q
+    // of the shell pair, hence the R14 quartet set, is untouched; the neglected primitive quartets are a thousand
+    // times smaller than what the shell-level screening drops.  tau = 0 keeps every primitive.
+    const double tau_p = 1e-3 * tau;
+    for (Pair& P : pairs) {
+        std::vector<int> order(P.np);
+        std::iota(order.begin(), order.end(), 0);
+        std::stable_sort(order.begin(), order.end(), [&](int x, int y) { return qprim[P.pc][P.row + x] > qprim[P.pc][P.row + y]; });
+        int neff = 0;
+        for (int k = 0; k < P.np; ++k) neff += (qprim[P.pc][P.row + k] * Qmax >= tau_p) ? 1 : 0;
+        neff = std::max(neff, 1);
+        const int nstore = neff <= 1 ? 1 : (neff <= 3 ? 3 : (neff <= 6 ? 6 : 9));
+        if (nstore < P.np) {
+            order.resize(nstore);
+            std::sort(order.begin(), order.end());
+            P.np = nstore;
+            P.sub = np_to_sub(nstore);
+        } else {
+            std::iota(order.begin(), order.end(), 0);
+        }
+        P.sel = order;
+    }
 
     // ---- keep, classify, sort by bound
     std::vector<int> cls[NKETCLASS];
@@ -337,8 +379,8 @@ int create_impl(Handle* h, const rttda_basis_t* basis, const double* C_occ, cons
             for (int k = 0; k < np; ++k)
                 for (int f = 0; f < PRIM_STRIDE; ++f)
                 {
-                    soa[((size_t)k * PRIM_STRIDE + f) * n + q] = rows[pc][(size_t)(P.row + k) * PRIM_STRIDE + f];
-                    aos[((size_t)q * np + k) * PRIM_STRIDE + f] = rows[pc][(size_t)(P.row + k) * PRIM_STRIDE + f];
+                    soa[((size_t)k * PRIM_STRIDE + f) * n + q] = rows[pc][(size_t)(P.row + P.sel[k]) * PRIM_STRIDE + f];
+                    aos[((size_t)q * np + k) * PRIM_STRIDE + f] = rows[pc][(size_t)(P.row + P.sel[k]) * PRIM_STRIDE + f];
                 }
         }
         KetClass& K = h->tabs.kets[kc];
@@ -411,7 +453,7 @@ int create_impl(Handle* h, const rttda_basis_t* basis, const double* C_occ, cons
     auto nkets_of = [&](int kc_ket, double Qp) {    // kets q (a prefix of the list) with Qp Q_q >= tau
         return tau > 0.0 ? count_prod_ge(kc_ket, Qp) : h->tabs.kets[kc_ket].n;
     };
-    double n_eval = 0, nprim_eval = 0;
+    double n_eval = 0, nprim_eval = 0, fl_eval = 0;
     size_t buf_need = 1;
     h->launches.clear();
     h->segments.clear();
@@ -443,6 +485,7 @@ int create_impl(Handle* h, const rttda_basis_t* basis, const double* C_occ, cons
             if (nquart == 0) continue;
             n_eval += (double)nquart;
             nprim_eval += (double)nquart * h->tabs.kets[kcb].np * h->tabs.kets[kck].np;
+            fl_eval += (double)nquart * h->tabs.kets[kcb].np * h->tabs.kets[kck].np * flops_prim(sg.la, sg.lb, sg.lc, sg.ld);
             buf_need = std::max(buf_need, (size_t)nbatch * sg.ni * 32);
             sg.incore_off = h->eri_all_need;
             h->eri_all_need += (size_t)nbatch * sg.ni * 32;
@@ -520,7 +563,8 @@ int create_impl(Handle* h, const rttda_basis_t* basis, const double* C_occ, cons
             }
         h->info[RTTDA_INFO_NQUARTETS] = 0.5 * (ordered + diag);
         h->info[RTTDA_INFO_NPRIM_QUARTETS] = 0.5 * (ordered_prim + diag_prim);
-        h->info[RTTDA_INFO_FLOPS_EVAL] = 0.5 * (fl_ord + fl_diag);
+        (void)fl_ord; (void)fl_diag;
+        h->info[RTTDA_INFO_FLOPS_EVAL] = fl_eval;   // on the primitive quartets the kernels evaluate (after primitive screening)
         h->info[RTTDA_INFO_FLOPS_DIGEST_PER_VEC] = 20.0 * 0.5 * (nint_ord + nint_diag);
     }
     h->info[RTTDA_INFO_NPAIRS_TOTAL] = (double)npairs_total;
