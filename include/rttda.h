@@ -144,8 +144,10 @@ int rttda_propagate_host(rttda_handle_t h, int32_t ntraj, double* C, const rttda
 #define RTTDA_INFO_NQUARTETS         2   /* unique shell quartets with Q_ab Q_cd >= tau (R14) */
 #define RTTDA_INFO_NPRIM_QUARTETS    3   /* primitive quartets inside those */
 #define RTTDA_INFO_NQUARTETS_EVAL    4   /* contracted quartet evaluations the kernels perform per ERI pass */
-#define RTTDA_INFO_NPRIM_EVAL        5   /* primitive quartet evaluations per ERI pass (after primitive-pair screening:
-                                            primitive pairs whose own bound q_k has q_k Q_max < 1e-3 tau are dropped) */
+#define RTTDA_INFO_NPRIM_EVAL        5   /* primitive quartets evaluated by the LAST ERI build, counted on the device (after
+                                            primitive screening: a primitive quartet (kb, kk) of a shell quartet is
+                                            evaluated iff q_kb Q_ket >= tau_p and q_kk Q_bra >= tau_p, tau_p = min(1e-3 tau, 1e-15), q_k the
+                                            primitive pair's own Schwarz bound); synchronises the device */
 #define RTTDA_INFO_FLOPS_EVAL        6   /* FP64 flop model of one ERI pass, evaluation part: on the primitive quartets
                                             actually evaluated (RTTDA_INFO_NPRIM_EVAL) */
 #define RTTDA_INFO_FLOPS_DIGEST_PER_VEC 7 /* FP64 flop model, digestion per density */

@@ -287,6 +287,17 @@ int rttda_get_info(rttda_handle_t hh, int32_t key, double* out)
     RT_CHECK(h && out, "rttda_get_info: NULL pointer");
     RT_CHECK(key >= 0 && key < 16, "rttda_get_info: unknown key");
     *out = (key == RTTDA_INFO_KERNEL_LAUNCHES) ? (double)h->kernel_launches : h->info[key];
+    if (key == RTTDA_INFO_NPRIM_EVAL || key == RTTDA_INFO_FLOPS_EVAL) {
+        // counted by the evaluation kernels of the last ERI build (all its passes); before the first build the
+        // host-side count of the stored primitive pairs stands in (an upper bound)
+        RT_DEVICE(h);
+        unsigned long long c[8];
+        RT_CUDA(cudaDeviceSynchronize());
+        RT_CUDA(cudaMemcpy(c, h->d_primcount, sizeof c, cudaMemcpyDeviceToHost));
+        double n = 0.0, fl = 0.0;
+        for (int L = 0; L <= 4; ++L) { n += (double)c[L]; fl += (double)c[L] * flops_prim_L(L); }
+        if (n > 0.0) *out = (key == RTTDA_INFO_NPRIM_EVAL) ? n : fl;
+    }
     return RTTDA_OK;
 }
 
@@ -335,6 +346,7 @@ int rttda_profile_pass(rttda_handle_t hh, int32_t nvec, double* rows, int32_t ca
              "rttda_profile_pass: call rttda_sigma / rttda_fock with the same nvec first (its densities are reused)");
     cudaStream_t st = (cudaStream_t)stream;
     RT_CUDA(cudaMemsetAsync(h->wsF, 0, nn * nvt * sizeof(double), st));
+    RT_CUDA(cudaMemsetAsync(h->d_primcount, 0, 8 * sizeof(unsigned long long), st));
     return jk_profile(h, nvt, (nvec + 1) & ~1, h->wsT, h->wsF, st, rows, cap, nrows);
 }
 

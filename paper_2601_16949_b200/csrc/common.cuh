@@ -62,6 +62,8 @@ struct KetClass {
     const int* same;       // [n] 1 if both shells are the same shell
     const double* prim;    // [np][PRIM_STRIDE][n]
     const double* prim_aos;// [n][np][PRIM_STRIDE]
+    const float* qp;       // [np][n]  primitive-pair bounds q_k = sqrt(max (kk|kk)), rounded up, descending in k
+    const float* qp_aos;   // [n][np]
 };
 
 // Ordered bra record of the digestion kernels (block-uniform side): shell a fixed by the list, partner b varies.
@@ -141,6 +143,7 @@ void boys_table_host(int L, std::vector<double>& tab);
 struct Handle {
     int device = 0;
     int nao = 0, nocc = 0, nvirt = 0, ncsf = 0, nshells = 0;
+    unsigned long long* d_primcount = nullptr; // [8] primitive quartets evaluated in the last ERI pass, per total L (jk_eval.cu)
     double cx = 1.0, tau = 0.0;
     // range-separated exchange (NEXT-4): A -= cx_lr (ij| erf(omega r12)/r12 |ab); rs_omega <= 0 or cx_lr == 0: off
     double cx_lr = 0.0, rs_omega = 0.0;
@@ -206,7 +209,11 @@ struct Handle {
 };
 
 int jk_mark(Handle* h, cudaStream_t st);
-int assign_lanes(Handle* h, int nlanes);   // record the next event of the J/K timing log
+int assign_lanes(Handle* h, int nlanes);
+// Primitive-level screening threshold: three orders below the shell-level one, and never looser than 1e-15, so that its
+// error stays far below both the shell screening error and the 1e-10 sigma tolerance at any tau.
+inline double prim_threshold(double tau) { return tau * 1e-3 < 1e-15 ? tau * 1e-3 : 1e-15; }
+double flops_prim_L(int L);                // flop model of one primitive quartet of total angular momentum L   // record the next event of the J/K timing log
 
 // jk_eval.cu / jk_digest.cu
 // F += 2 J[T] - cx K[T] for all nvt (even) interleaved densities; F zeroed by the caller.

@@ -766,6 +766,7 @@ int jk_build(Handle* h, int nvt, int nvec, const double* Tq, double* Fq, cudaStr
         RT_CUDA(cudaGetLastError());
         h->kernel_launches++;
     }
+    RT_CUDA(cudaMemsetAsync(h->d_primcount, 0, 8 * sizeof(unsigned long long), st));   // counters of THIS build
     const bool lr = (h->cx_lr != 0.0 && h->rs_omega > 0.0);
     RT_CHECK(!(lr && h->incore), "jk_build: the in-core store holds the integrals of ONE operator; switch RTTDA_OPT_INCORE off "
                                  "when range-separated exchange is on");

@@ -21,6 +21,8 @@ struct EvalArgs {
     const double2* boys;
     double* buf;
     double tau;
+    double tau_p;          // primitive-quartet threshold (prim_threshold(tau)): (kb, kk) is evaluated iff q_kb Q_ket >= tau_p and q_kk Q_bra >= tau_p
+    unsigned long long* primcount;   // primitive quartets evaluated (lane level), one counter per total angular momentum
     double w_extra;        // 0 for 1/r12; 36 / omega^2 for erf(omega r12)/r12 (alpha -> alpha omega^2 / (alpha + omega^2))
     int same;
 };
@@ -69,6 +71,7 @@ __global__ void __launch_bounds__(JK_BLOCK) eval_kernel(EvalArgs g)
     __shared__ __align__(16) double s_rows[EVAL_MAX_ROWS * PRIM_STRIDE];
     __shared__ double s_Q[JK_BLOCK];
     __shared__ long long s_base[JK_BLOCK];
+    __shared__ float s_qp[EVAL_MAX_ROWS];
 
     const EvalItem it = g.items[blockIdx.x];
     const int npb = g.bra.np, npairs = it.p_end - it.p_begin;
@@ -78,6 +81,7 @@ __global__ void __launch_bounds__(JK_BLOCK) eval_kernel(EvalArgs g)
         double2* dst = reinterpret_cast<double2*>(s_rows);
         const int n2 = npairs * npb * (PRIM_STRIDE / 2);
         for (int i = threadIdx.x; i < n2; i += JK_BLOCK) dst[i] = src[i];
+        for (int i = threadIdx.x; i < npairs * npb; i += JK_BLOCK) s_qp[i] = g.bra.qp_aos[(size_t)it.p_begin * npb + i];
         __syncthreads();
         for (int r = threadIdx.x; r < npairs * npb; r += JK_BLOCK) {     // rows carry c' and w = 36/p (eri_eval.cuh)
             const double p = s_rows[r * PRIM_STRIDE];
@@ -98,6 +102,10 @@ __global__ void __launch_bounds__(JK_BLOCK) eval_kernel(EvalArgs g)
     const double wcd = __ldg(g.ket.same + qq) ? 0.5 : 1.0;
     const int lane = threadIdx.x & 31;
 
+    float kq[KP];                                           // bounds of this ket's primitive pairs, descending
+#pragma unroll
+    for (int k = 0; k < KP; ++k) kq[k] = __ldg(g.ket.qp + (size_t)k * g.ket.n + qq);
+    unsigned long long nprim_done = 0;
     PrimPair kp[KET_IN_REGS ? KP : 1];
     if (KET_IN_REGS) {
 #pragma unroll
@@ -117,22 +125,37 @@ __global__ void __launch_bounds__(JK_BLOCK) eval_kernel(EvalArgs g)
 #pragma unroll
         for (int i = 0; i < NI; ++i) I[i] = 0.0;
         const double* rows = s_rows + (size_t)ip * npb * PRIM_STRIDE;
+        // Primitive-quartet screening (both lists are sorted by descending bound, so the primitives a quartet needs are
+        // prefixes): bra primitive kb matters to this lane iff q_kb Q_ket >= tau_p, ket primitive kk iff q_kk Q_bra >=
+        // tau_p.  The warp runs the longest prefix any of its lanes needs; kets of a warp are neighbours in the
+        // Schwarz-sorted list, so the prefixes are nearly uniform.
+        const float* qb = s_qp + ip * npb;
+        int nkb_l = 0, nkk_l = 0;
+        if (ok) {
+            for (int kb = 0; kb < npb; ++kb) nkb_l += ((double)qb[kb] * Qq >= g.tau_p) ? 1 : 0;
+#pragma unroll
+            for (int kk = 0; kk < KP; ++kk) nkk_l += ((double)kq[kk] * s_Q[ip] >= g.tau_p) ? 1 : 0;
+            nkb_l = max(nkb_l, 1); nkk_l = max(nkk_l, 1);
+        }
+        const int nkb = __reduce_max_sync(0xffffffffu, nkb_l), nkk = __reduce_max_sync(0xffffffffu, nkk_l);
+        if (ok) nprim_done += (unsigned)(nkb * nkk);
         if (!ok) {
         } else if (KET_IN_REGS) {
 #pragma unroll 1
-            for (int kb = 0; kb < npb; ++kb) {
+            for (int kb = 0; kb < nkb; ++kb) {
                 const PrimPair bp = load_bra_prim_smem(rows + kb * PRIM_STRIDE);
 #pragma unroll
-                for (int kk = 0; kk < KP; ++kk) eri_prim_accum<LA, LB, LC, LD>(bp, kp[kk], s_boys, I);
+                for (int kk = 0; kk < KP; ++kk)
+                    if (kk < nkk) eri_prim_accum<LA, LB, LC, LD>(bp, kp[kk], s_boys, I);
             }
         } else {
             // ket primitive outermost: it is loaded once (coalesced, L1) and meets every bra primitive (shared memory)
 #pragma unroll 1
-            for (int kk = 0; kk < KP; ++kk) {
+            for (int kk = 0; kk < nkk; ++kk) {
                 PrimPair k1 = load_ket_prim<LC, LD>(g.ket.prim, g.ket.n, kk, qq);
                 k1.p += g.w_extra;
 #pragma unroll 1
-                for (int kb = 0; kb < npb; ++kb) {
+                for (int kb = 0; kb < nkb; ++kb) {
                     const PrimPair bp = load_bra_prim_smem(rows + kb * PRIM_STRIDE);
                     eri_prim_accum<LA, LB, LC, LD>(bp, k1, s_boys, I);
                 }
@@ -144,6 +167,10 @@ __global__ void __launch_bounds__(JK_BLOCK) eval_kernel(EvalArgs g)
 #pragma unroll
         for (int i = 0; i < NI; ++i) __stcs(dst + i * 32, w * I[i]);
     }
+    // primitive quartets evaluated by this block (feeds the flop model of the roofline figure)
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) nprim_done += __shfl_xor_sync(0xffffffffu, nprim_done, o);
+    if (lane == 0 && nprim_done) atomicAdd(g.primcount + L, nprim_done);
 }
 
 template <int LA, int LB, int LC, int LD>
@@ -157,6 +184,8 @@ static int launch_eval(Handle* h, const Segment& sg, double* buf, cudaStream_t s
     g.boys = h->tabs.boys[LA + LB + LC + LD];
     g.buf = buf;
     g.tau = h->tabs.tau;
+    g.tau_p = prim_threshold(h->tabs.tau);
+    g.primcount = h->d_primcount;
     g.w_extra = h->pass_w_extra;
     g.same = (sg.kc_bra == sg.kc_ket);
     dim3 grid(sg.nitems), block(JK_BLOCK);

@@ -233,6 +233,12 @@ static double flops_prim(int la, int lb, int lc, int ld)
     return 2.0 * fma + other;
 }
 
+double flops_prim_L(int L)
+{
+    static const int cls[5][4] = {{0, 0, 0, 0}, {1, 0, 0, 0}, {1, 0, 1, 0}, {1, 1, 1, 0}, {1, 1, 1, 1}};
+    return flops_prim(cls[L][0], cls[L][1], cls[L][2], cls[L][3]);
+}
+
 int create_impl(Handle* h, const rttda_basis_t* basis, const double* C_occ, const double* C_virt,
                 const double* eps, cudaStream_t st)
 {
@@ -325,12 +331,12 @@ int create_impl(Handle* h, const rttda_basis_t* basis, const double* C_occ, cons
     RT_CHECK(Qmax > 0.0 && std::isfinite(Qmax), "Schwarz bounds are not finite/positive");
     const double tau = h->tau;
 
-    // ---- primitive screening: a primitive pair k whose own bound q_k cannot lift any integral above tau_p = 1e-3 tau
-    // (q_k Q_max < tau_p; |(k.|cd)| <= q_k Q_cd) is dropped from its shell pair, and the pair moves to the contraction
-    // sub-class of what is left (9 -> 6 -> 3 -> 1 primitive pairs; kept rows stay in exponent order).  The Schwarz bound Q
+    // ---- primitive screening: a primitive pair k whose own bound q_k cannot lift any integral above tau_p
+    // (q_k Q_max < tau_p, tau_p = min(1e-3 tau, 1e-15); |(k.|cd)| <= q_k Q_cd) is dropped from its shell pair, and the pair moves to the contraction
+    // sub-class of what is left (9 -> 6 -> 3 -> 1 primitive pairs; kept rows in order of descending bound).  The Schwarz bound Q
     // of the shell pair, hence the R14 quartet set, is untouched; the neglected primitive quartets are a thousand
     // times smaller than what the shell-level screening drops.  tau = 0 keeps every primitive.
-    const double tau_p = 1e-3 * tau;
+    const double tau_p = prim_threshold(tau);
     for (Pair& P : pairs) {
         std::vector<int> order(P.np);
         std::iota(order.begin(), order.end(), 0);
@@ -341,13 +347,10 @@ int create_impl(Handle* h, const rttda_basis_t* basis, const double* C_occ, cons
         const int nstore = neff <= 1 ? 1 : (neff <= 3 ? 3 : (neff <= 6 ? 6 : 9));
         if (nstore < P.np) {
             order.resize(nstore);
-            std::sort(order.begin(), order.end());
             P.np = nstore;
             P.sub = np_to_sub(nstore);
-        } else {
-            std::iota(order.begin(), order.end(), 0);
         }
-        P.sel = order;
+        P.sel = order;                      // most significant primitive first: quartet-level prefixes (jk_eval.cu)
     }
 
     // ---- keep, classify, sort by bound
@@ -370,12 +373,19 @@ int create_impl(Handle* h, const rttda_basis_t* basis, const double* C_occ, cons
         std::vector<double> soa((size_t)np * PRIM_STRIDE * std::max(n, 1), 0.0);
         std::vector<double> aos((size_t)np * PRIM_STRIDE * std::max(n, 1), 0.0);
         std::vector<int> aoc(std::max(n, 1), 0), aod(std::max(n, 1), 0), same(std::max(n, 1), 0);
+        std::vector<float> qsoa((size_t)np * std::max(n, 1), 0.f), qaos((size_t)np * std::max(n, 1), 0.f);
         hQ[kc].assign(std::max(n, 1), 0.0);
         for (int q = 0; q < n; ++q) {
             Pair& P = pairs[v[q]];
             P.pos = q;
             hQ[kc][q] = P.Q;
             aoc[q] = H.ao[P.s1]; aod[q] = H.ao[P.s2]; same[q] = (P.s1 == P.s2);
+            for (int k = 0; k < np; ++k) {
+                // float is enough for a screening bound; rounded up so that it never under-estimates
+                const float qf = std::nextafter((float)(qprim[pc][P.row + P.sel[k]] * (1.0 + 1e-6)), INFINITY);
+                qsoa[(size_t)k * n + q] = qf;
+                qaos[(size_t)q * np + k] = qf;
+            }
             for (int k = 0; k < np; ++k)
                 for (int f = 0; f < PRIM_STRIDE; ++f)
                 {
@@ -391,6 +401,8 @@ int create_impl(Handle* h, const rttda_basis_t* basis, const double* C_occ, cons
         RT_TRY(upload(h, same, &K.same));
         RT_TRY(upload(h, soa, &K.prim));
         RT_TRY(upload(h, aos, &K.prim_aos));
+        RT_TRY(upload(h, qsoa, &K.qp));
+        RT_TRY(upload(h, qaos, &K.qp_aos));
     }
 
     // ---- ordered bra records grouped into a-lists keyed by (shell a, l_b, sub)
@@ -652,6 +664,9 @@ int create_impl(Handle* h, const rttda_basis_t* basis, const double* C_occ, cons
     RT_CUDA(cudaStreamSynchronize(st));
     h->kernel_launches += 6;
     for (auto& e : h->ev) RT_CUDA(cudaEventCreate(&e));
+    RT_CUDA(cudaMalloc((void**)&h->d_primcount, 8 * sizeof(unsigned long long)));
+    h->dev_allocs.push_back(h->d_primcount);
+    RT_CUDA(cudaMemsetAsync(h->d_primcount, 0, 8 * sizeof(unsigned long long), st));
     RT_CUDA(cudaEventCreateWithFlags(&h->ev_fork, cudaEventDisableTiming));
     for (int l = 0; l < Handle::MAXLANES; ++l) {
         RT_CUDA(cudaStreamCreateWithFlags(&h->lane_st[l], cudaStreamNonBlocking));
