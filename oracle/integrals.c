@@ -376,6 +376,137 @@ void oracle_eri_pair_block(BASIS_ARGS, int nao, int sc, int sd, double tau, cons
         }
 }
 
+/* ---- the same shell quartet with EVERY intermediate in x87 long double --------------------------------------
+ * (Boys function, Hermite E and R recursions, contraction; same formulas, same order as shell_quartet_op with
+ * omega = 0).  Used to measure the rounding noise of the FP64 integral values themselves: at cond(S) ~ 1e4-1e5 the
+ * back transform C_o^T F C_v amplifies per-integral relative errors of 1e-15 to the 1e-10 level of the sigma
+ * tolerance. */
+static void boys_ld(int nmax, long double T, long double *F)
+{
+    if (T <= 35.0L) {
+        long double term = 1.0L / (2 * nmax + 1), sum = term;
+        for (int k = 1; k < 4000; ++k) {
+            term *= 2.0L * T / (2 * nmax + 2 * k + 1);
+            sum += term;
+            if (term < 1e-21L * sum) break;
+        }
+        long double emt = expl(-T), f = emt * sum;
+        F[nmax] = f;
+        for (int n = nmax; n >= 1; --n) { f = (2.0L * T * f + emt) / (2 * n - 1); F[n - 1] = f; }
+    } else {
+        long double emt = expl(-T), f = 0.5L * sqrtl(M_PIl / T) * erfl(sqrtl(T));
+        F[0] = f;
+        for (int n = 0; n < nmax; ++n) { f = ((2 * n + 1) * f - emt) / (2.0L * T); F[n + 1] = f; }
+    }
+}
+
+static void hermite_E_ld(long double a, long double b, long double Ax, long double Bx, long double E[2][2][3])
+{
+    long double p = a + b, mu = a * b / p, XAB = Ax - Bx;
+    long double Px = (a * Ax + b * Bx) / p, XPA = Px - Ax, XPB = Px - Bx;
+    for (int i = 0; i < 12; ++i) ((long double *)E)[i] = 0.0L;
+    E[0][0][0] = expl(-mu * XAB * XAB);
+    for (int t = 0; t <= 1; ++t) {
+        long double em = (t - 1 >= 0) ? E[0][0][t - 1] : 0.0L, e0 = E[0][0][t];
+        E[1][0][t] = em / (2 * p) + XPA * e0;
+    }
+    for (int i = 0; i <= 1; ++i)
+        for (int t = 0; t <= i + 1; ++t) {
+            long double em = (t - 1 >= 0) ? E[i][0][t - 1] : 0.0L;
+            long double e0 = (t <= i) ? E[i][0][t] : 0.0L;
+            long double ep = (t + 1 <= i) ? E[i][0][t + 1] : 0.0L;
+            E[i][1][t] = em / (2 * p) + XPB * e0 + (t + 1) * ep;
+        }
+}
+
+static void shell_quartet_ld(const basis_t *B, int sa, int sb, int sc, int sd, long double *out)
+{
+    int l[4] = {B->sh_l[sa], B->sh_l[sb], B->sh_l[sc], B->sh_l[sd]};
+    int n[4] = {2 * l[0] + 1, 2 * l[1] + 1, 2 * l[2] + 1, 2 * l[3] + 1};
+    int L = l[0] + l[1] + l[2] + l[3];
+    const double *A = B->centers + 3 * B->sh_center[sa], *Bc = B->centers + 3 * B->sh_center[sb];
+    const double *C = B->centers + 3 * B->sh_center[sc], *D = B->centers + 3 * B->sh_center[sd];
+    int ntot = n[0] * n[1] * n[2] * n[3];
+    for (int i = 0; i < ntot; ++i) out[i] = 0.0L;
+    for (int ka = 0; ka < B->sh_nprim[sa]; ++ka)
+    for (int kb = 0; kb < B->sh_nprim[sb]; ++kb) {
+        long double a = B->exps[B->sh_off[sa] + ka], b = B->exps[B->sh_off[sb] + kb];
+        long double cab = (long double)B->ncoef[B->sh_off[sa] + ka] * B->ncoef[B->sh_off[sb] + kb];
+        long double p = a + b, P[3], Eab[3][2][2][3];
+        for (int x = 0; x < 3; ++x) { P[x] = (a * A[x] + b * Bc[x]) / p; hermite_E_ld(a, b, A[x], Bc[x], Eab[x]); }
+        for (int kc = 0; kc < B->sh_nprim[sc]; ++kc)
+        for (int kd = 0; kd < B->sh_nprim[sd]; ++kd) {
+            long double c = B->exps[B->sh_off[sc] + kc], d = B->exps[B->sh_off[sd] + kd];
+            long double ccd = (long double)B->ncoef[B->sh_off[sc] + kc] * B->ncoef[B->sh_off[sd] + kd];
+            long double q = c + d, Q[3], Ecd[3][2][2][3], R[3];
+            for (int x = 0; x < 3; ++x) { Q[x] = (c * C[x] + d * D[x]) / q; hermite_E_ld(c, d, C[x], D[x], Ecd[x]); R[x] = P[x] - Q[x]; }
+            long double alpha = p * q / (p + q), F[LMAX_TOT + 1];
+            boys_ld(L, alpha * (R[0] * R[0] + R[1] * R[1] + R[2] * R[2]), F);
+            static __thread long double Rt[5][5][5][5];
+            for (int i = 0; i < 625; ++i) ((long double *)Rt)[i] = 0.0L;
+            long double m2a = 1.0L;
+            for (int nn = 0; nn <= L; ++nn) { Rt[nn][0][0][0] = m2a * F[nn]; m2a *= -2.0L * alpha; }
+            for (int N = 1; N <= L; ++N)
+                for (int t = 0; t <= N; ++t)
+                    for (int u = 0; u <= N - t; ++u) {
+                        int v = N - t - u;
+                        for (int nn = 0; nn <= L - N; ++nn) {
+                            long double val;
+                            if (t > 0) val = (t - 1 > 0 ? (t - 1) * Rt[nn + 1][t - 2][u][v] : 0.0L) + R[0] * Rt[nn + 1][t - 1][u][v];
+                            else if (u > 0) val = (u - 1 > 0 ? (u - 1) * Rt[nn + 1][t][u - 2][v] : 0.0L) + R[1] * Rt[nn + 1][t][u - 1][v];
+                            else val = (v - 1 > 0 ? (v - 1) * Rt[nn + 1][t][u][v - 2] : 0.0L) + R[2] * Rt[nn + 1][t][u][v - 1];
+                            Rt[nn][t][u][v] = val;
+                        }
+                    }
+            long double pref = 2.0L * powl(M_PIl, 2.5L) / (p * q * sqrtl(p + q)) * cab * ccd;
+            int idx = 0;
+            for (int ca = 0; ca < n[0]; ++ca)
+            for (int cb = 0; cb < n[1]; ++cb)
+            for (int cc = 0; cc < n[2]; ++cc)
+            for (int cd = 0; cd < n[3]; ++cd, ++idx) {
+                int pa[3], pb[3], pc[3], pd[3];
+                cart_pow(l[0], ca, pa); cart_pow(l[1], cb, pb); cart_pow(l[2], cc, pc); cart_pow(l[3], cd, pd);
+                long double s = 0.0L;
+                for (int t = 0; t <= pa[0] + pb[0]; ++t)
+                for (int u = 0; u <= pa[1] + pb[1]; ++u)
+                for (int v = 0; v <= pa[2] + pb[2]; ++v) {
+                    long double eab = Eab[0][pa[0]][pb[0]][t] * Eab[1][pa[1]][pb[1]][u] * Eab[2][pa[2]][pb[2]][v];
+                    for (int t2 = 0; t2 <= pc[0] + pd[0]; ++t2)
+                    for (int u2 = 0; u2 <= pc[1] + pd[1]; ++u2)
+                    for (int v2 = 0; v2 <= pc[2] + pd[2]; ++v2) {
+                        long double ecd = Ecd[0][pc[0]][pd[0]][t2] * Ecd[1][pc[1]][pd[1]][u2] * Ecd[2][pc[2]][pd[2]][v2];
+                        long double sgn = ((t2 + u2 + v2) & 1) ? -1.0L : 1.0L;
+                        s += eab * sgn * ecd * Rt[0][t + t2][u + u2][v + v2];
+                    }
+                }
+                out[idx] += pref * s;
+            }
+        }
+    }
+}
+
+/* Full AO tensor in long double, [nao]^4 (small systems only: 16 bytes per element). */
+void oracle_eri_tensor_ld(BASIS_ARGS, int nao, long double *eri)
+{
+    basis_t B = BASIS_MK;
+    #pragma omp parallel for schedule(dynamic) collapse(2)
+    for (int sa = 0; sa < nshells; ++sa)
+    for (int sb = 0; sb < nshells; ++sb)
+        for (int sc = 0; sc < nshells; ++sc)
+        for (int sd = 0; sd < nshells; ++sd) {
+            long double blk[81];
+            shell_quartet_ld(&B, sa, sb, sc, sd, blk);
+            int n0 = 2 * sh_l[sa] + 1, n1 = 2 * sh_l[sb] + 1, n2 = 2 * sh_l[sc] + 1, n3 = 2 * sh_l[sd] + 1, idx = 0;
+            for (int ca = 0; ca < n0; ++ca)
+            for (int cb = 0; cb < n1; ++cb)
+            for (int cc = 0; cc < n2; ++cc)
+            for (int cd = 0; cd < n3; ++cd, ++idx) {
+                size_t m = ao_off[sa] + ca, nu = ao_off[sb] + cb, la = ao_off[sc] + cc, si = ao_off[sd] + cd;
+                eri[((m * nao + nu) * nao + la) * nao + si] = blk[idx];
+            }
+        }
+}
+
 /* Schwarz bounds Q_ab = sqrt(max_{mu in a, nu in b} (mu nu|mu nu)), [nshells][nshells] (R14). */
 void oracle_schwarz(BASIS_ARGS, double *Q)
 {

@@ -112,6 +112,15 @@ class OracleBasis:
         lib().oracle_eri_tensor(*self._args(), ct.c_int(N), eri.ctypes.data_as(_dp))
         return eri
 
+    def eri_tensor_ld(self) -> np.ndarray:
+        """Full AO tensor with every intermediate of the integral evaluation in x87 long double (np.longdouble [N]^4)."""
+        N = self.nao
+        if N > 128:
+            raise ValueError("long-double N^4 tensor only for N <= 128 (16 bytes per element)")
+        eri = np.zeros((N, N, N, N), dtype=np.longdouble)
+        lib().oracle_eri_tensor_ld(*self._args(), ct.c_int(N), ct.c_void_p(eri.ctypes.data))
+        return eri
+
     def eri_tensor_erf(self, omega: float) -> np.ndarray:
         """Full AO tensor of the attenuated operator erf(omega r12)/r12 (omega <= 0: 1/r12)."""
         N = self.nao

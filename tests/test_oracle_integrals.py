@@ -323,3 +323,18 @@ def test_erf_attenuated_tensor_symmetry_and_jk_route(tiny):
     J, K, _, _ = ob.jk_erf(T, 0.33, tau=0.0)
     assert np.max(np.abs(J - np.einsum("mnls,vls->vmn", e, T))) < 1e-12
     assert np.max(np.abs(K - np.einsum("mnls,vns->vml", e, T))) < 1e-12
+
+
+def test_fp64_integral_values_against_long_double_evaluation(tiny):
+    """Rounding noise of the oracle's FP64 integral VALUES: the whole AO tensor of config 1 against the same formulas
+    evaluated with every intermediate in x87 long double (oracle_eri_tensor_ld).  Absolute errors of a few 1e-16 (the
+    Hermite sums cancel, so small integrals carry the absolute error of the large intermediates); this is the noise that
+    cond(S) = 4.5e4 amplifies to the 1e-10 level of the sigma tolerance at 1280 AO."""
+    e64, eld = tiny["eri"], tiny["ob"].eri_tensor_ld()
+    assert eld.dtype == np.longdouble
+    d = np.abs(e64 - eld.astype(np.float64))
+    rms = float(np.sqrt(np.mean(d ** 2)))
+    print("FP64 integral values vs long-double evaluation: max abs %.2e, rms %.2e" % (d.max(), rms))
+    assert d.max() < 1e-14 and rms < 5e-17
+    # and the long-double tensor obeys the same symmetry and the closed form as the FP64 one
+    assert np.max(np.abs(eld - eld.transpose(2, 3, 0, 1))) < 1e-17
