@@ -332,6 +332,8 @@ def run_b200(args):
     ms = [a.elapsed_time(b) for a, b in ev]
     total_ms = float(sum(ms))
     jk_ms, jk_n = h.rttda_jk_time()
+    info["flops_eval"] = h.rttda_get_info("flops_eval")      # counted by the kernels of the last timed ERI pass
+    info["nprim_eval"] = h.rttda_get_info("nprim_eval")
     launches = int(h.rttda_get_info("kernel_launches") - l0)
     total_ms = reduce_max(total_ms, world, dev)
     ms_per_step = total_ms / args.steps
@@ -375,7 +377,8 @@ def run_b200(args):
             incore = {"unavailable": str(e)}
         finally:
             h.rttda_set_option(R.OPT_INCORE, 0)
-    # roofline of the dominant kernel group (the J/K ERI pass): algorithmic flops / measured device time
+    # roofline of the dominant kernel group (the J/K ERI pass): algorithmic flops / measured device time.  The evaluation
+    # part is counted by the kernels themselves (primitive quartets actually evaluated in the last ERI pass).
     flops_pass = info["flops_eval"] + nvec * info["flops_digest_per_vec"]
     jk_src = "CUDA events around every ERI pass of the timed steps (rttda_jk_time)"
     if jk_n == 0:
@@ -423,8 +426,14 @@ def run_b200(args):
                "setup_s": setup_s, "create_ms": info["create_ms"],
                "jk_ms_per_pass": jk_avg_ms, "jk_ms_source": jk_src,
                "jk_share_of_step": 4.0 * jk_avg_ms / ms_per_step if not sso else None,
-               "roofline": {"bound": "alu", "kernel": "eval_kernel<*> + digest_j_kernel<*> + digest_b_kernel<*> (all launches of one ERI pass)",
+               "roofline": {"bound": "alu", "kernel": "eval_kernel<*> + digest_j_kernel<*> + digest_k/b_kernel<*> (all launches of one ERI pass)",
                             "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
+                            "flop_model": "evaluation: per-class minimal McMurchie-Davidson count x primitive quartets the kernels "
+                                          "EVALUATED (device counters, after primitive screening); digestion: 20 flops per "
+                                          "integral value per density.  Round 1 counted every primitive quartet of the R14 "
+                                          "quartets; on that count this pass reads %.3f" % (
+                                              (info["nprim_quartets"] / max(info["nprim_eval"], 1.0) * info["flops_eval"]
+                                               + nvec * info["flops_digest_per_vec"]) / (jk_avg_ms * 1e-3) / 1e12 / peak),
                             "traffic": traffic, "traffic_source": "NOT measured in this run: profiles/r2_traffic_per_pass.txt (ncu "
                             "dram__bytes_read+write summed over the launches of one ERI pass of this same command, config 4, "
                             "nvec 6)" if traffic else None,
@@ -450,7 +459,7 @@ def run_b200(args):
         torch.cuda.synchronize()
         ms_p = a.elapsed_time(b) / args.steps
         jk_p, jk_pn = h.rttda_jk_time()
-        ip = h.info()
+        ip = h.info()                                    # after the timed passes: device-counted evaluation work
         fl_p = ip["flops_eval"] + nvec * ip["flops_digest_per_vec"]
         at_parity = {"tau": args.parity_tau, "sigma_vectors_per_s": 8.0 * ntraj / (ms_p * 1e-3), "ms_per_step": ms_p,
                      "jk_ms_per_pass": jk_p / max(jk_pn, 1), "unique_shell_quartets": ip["nquartets"],
@@ -540,8 +549,8 @@ def run_sweep(args):
             if tau == 1e-14:
                 ref[nvec] = res
             err = float(np.max(np.abs(res - ref[nvec])) / np.max(np.abs(ref[nvec])))
-            flops = info["flops_eval"] + nvec * info["flops_digest_per_vec"]
-            points.append({"tau": tau, "nvec": nvec, "ms_median": float(np.median(ms)), "ms_min": float(min(ms)),
+            flops = h.rttda_get_info("flops_eval") + nvec * info["flops_digest_per_vec"]     # counted by the last pass
+            points.append({"tau": tau, "nvec": nvec, "primitive_quartets_evaluated": h.rttda_get_info("nprim_eval"), "ms_median": float(np.median(ms)), "ms_min": float(min(ms)),
                            "sigma_vectors_per_s": nvec / (float(np.median(ms)) * 1e-3),
                            "eri_quartets_per_s": info["nquartets"] / (jk * 1e-3), "jk_ms": jk,
                            "unique_shell_quartets": info["nquartets"], "primitive_quartets": info["nprim_quartets"],
