@@ -278,7 +278,7 @@ def test_sigma_config4_vs_stored_oracle_samples():
     for tau in (1e-12, 1e-14):
         h = ctx["h"] if tau == ctx["tau"] else R.Rttda(ctx["basis"], torch.from_numpy(ctx["C_o"]).to(ctx["dev"]),
                                                          torch.from_numpy(ctx["C_v"]).to(ctx["dev"]), ctx["eps"], 1.0, tau)
-        for nvec in (32, 2):
+        for nvec in (32, 8, 2):
             Xd = torch.from_numpy(np.ascontiguousarray(X32[:nvec])).to(ctx["dev"])
             out = torch.empty_like(Xd)
             h.rttda_sigma(Xd, out)
