@@ -1,13 +1,16 @@
 /* ORACLE -- test infrastructure, NOT the product.  Plain, slow, CPU-only McMurchie-Davidson
- * integrals for contracted Cartesian s/p Gaussians, written from the textbook definitions the
+ * integrals for contracted Cartesian s/p/d Gaussians, written from the textbook definitions the
  * paper cites (refs 88-91) and DESIGN.md section "Oracle".  Shares no code with
  * paper_2601_16949_b200/csrc.  Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline /
  * --impl reference legs may call it.
  *
- * Conventions: AO order = shell order, p components x, y, z.  `ncoef[k]` are the FINAL
+ * Conventions: AO order = shell order, p components x, y, z; d components (Cartesian, 6 per shell, SURVEY 8(f)
+ * NEXT-4, "6-31G*") xx, xy, xz, yy, yz, zz.  `ncoef[k]` are the FINAL
  * coefficients multiplying the bare primitive  x^i y^j z^k exp(-a r^2)  (primitive norm,
  * contraction coefficient and the contracted-shell renormalisation already folded in by
- * oracle/integrals.py, which computes them from this file's own overlap routine).
+ * oracle/integrals.py, which computes them from this file's own overlap routine).  Reading R11 for d shells:
+ * EVERY Cartesian component is normalised, <phi|phi> = 1; ncoef normalises xx (and yy, zz, which share its norm),
+ * and xy, xz, yz carry the extra factor sqrt(3) = sqrt(<xx|xx> / <xy|xy>) (cart_norm below).
  *
  * Every function follows the definitions step by step; there is no blocking or reordering.
  */
@@ -20,7 +23,12 @@
 #include <omp.h>
 #endif
 
-#define LMAX_TOT 4 /* l_a+l_b+l_c+l_d <= 4 for s/p */
+#define LMAX 2       /* highest shell angular momentum: s, p, d */
+#define LMAX_TOT 8   /* l_a+l_b+l_c+l_d */
+#define NR (LMAX_TOT + 1)
+#define NCART(l) (((l) + 1) * ((l) + 2) / 2)
+#define NCMAX 6      /* NCART(LMAX) */
+#define NQMAX 1296   /* NCMAX^4 */
 
 typedef struct {
     int nshells;
@@ -60,38 +68,49 @@ void oracle_boys(int nmax, double T, double *F)
     }
 }
 
-/* ---- 1-D Hermite expansion coefficients E_t^{ij}, i,j <= 1, t <= 2 ------------------------ */
+/* ---- 1-D Hermite expansion coefficients E_t^{ij}, i,j <= LMAX, t <= i+j ------------------- */
 /* E_0^{00} = exp(-mu X_AB^2);
  * E_t^{i+1,j} = E_{t-1}^{ij}/(2p) + X_PA E_t^{ij} + (t+1) E_{t+1}^{ij}
  * E_t^{i,j+1} = E_{t-1}^{ij}/(2p) + X_PB E_t^{ij} + (t+1) E_{t+1}^{ij};  E_t = 0 for t<0, t>i+j */
-static void hermite_E(double a, double b, double Ax, double Bx, double E[2][2][3])
+static void hermite_E(double a, double b, double Ax, double Bx, double E[LMAX + 1][LMAX + 1][2 * LMAX + 1])
 {
     double p = a + b, mu = a * b / p, XAB = Ax - Bx;
     double Px = (a * Ax + b * Bx) / p, XPA = Px - Ax, XPB = Px - Bx;
-    memset(E, 0, sizeof(double) * 12);
+    memset(E, 0, sizeof(double) * (LMAX + 1) * (LMAX + 1) * (2 * LMAX + 1));
     E[0][0][0] = exp(-mu * XAB * XAB);
-    /* i: 0 -> 1 at j = 0 */
-    for (int t = 0; t <= 1; ++t) {
-        double em = (t - 1 >= 0) ? E[0][0][t - 1] : 0.0;
-        double e0 = E[0][0][t];
-        double ep = (t + 1 <= 0) ? E[0][0][t + 1] : 0.0; /* E_t^{00} = 0 for t > 0 */
-        E[1][0][t] = em / (2 * p) + XPA * e0 + (t + 1) * ep;
-    }
-    /* j: 0 -> 1 at i = 0 and i = 1 */
-    for (int i = 0; i <= 1; ++i)
+    /* i -> i+1 at j = 0 */
+    for (int i = 0; i < LMAX; ++i)
         for (int t = 0; t <= i + 1; ++t) {
             double em = (t - 1 >= 0) ? E[i][0][t - 1] : 0.0;
             double e0 = (t <= i) ? E[i][0][t] : 0.0;
             double ep = (t + 1 <= i) ? E[i][0][t + 1] : 0.0;
-            E[i][1][t] = em / (2 * p) + XPB * e0 + (t + 1) * ep;
+            E[i + 1][0][t] = em / (2 * p) + XPA * e0 + (t + 1) * ep;
         }
+    /* j -> j+1 at every i */
+    for (int i = 0; i <= LMAX; ++i)
+        for (int j = 0; j < LMAX; ++j)
+            for (int t = 0; t <= i + j + 1; ++t) {
+                double em = (t - 1 >= 0) ? E[i][j][t - 1] : 0.0;
+                double e0 = (t <= i + j) ? E[i][j][t] : 0.0;
+                double ep = (t + 1 <= i + j) ? E[i][j][t + 1] : 0.0;
+                E[i][j + 1][t] = em / (2 * p) + XPB * e0 + (t + 1) * ep;
+            }
 }
 
-/* Cartesian powers of component c of a shell with angular momentum l (s: 000; p: x, y, z). */
+/* Cartesian powers of component c of a shell with angular momentum l (s: 000; p: x, y, z; d: xx, xy, xz, yy, yz, zz). */
 static void cart_pow(int l, int c, int pw[3])
 {
+    static const int dpow[6][3] = {{2, 0, 0}, {1, 1, 0}, {1, 0, 1}, {0, 2, 0}, {0, 1, 1}, {0, 0, 2}};
     pw[0] = pw[1] = pw[2] = 0;
     if (l == 1) pw[c] = 1;
+    if (l == 2) { pw[0] = dpow[c][0]; pw[1] = dpow[c][1]; pw[2] = dpow[c][2]; }
+}
+
+/* Norm of component c relative to component 0 of its shell (R11 for d shells, see the header): for one radial part
+ * int x^4 e^{-2ar^2} = 3 int x^2 y^2 e^{-2ar^2}, so xy, xz, yz need sqrt(3) to reach <phi|phi> = 1. */
+static double cart_norm(int l, int c)
+{
+    return (l == 2 && (c == 1 || c == 2 || c == 4)) ? sqrt(3.0) : 1.0;
 }
 
 /* ---- one-electron: overlap and dipole (origin O) for one shell pair ----------------------- */
@@ -100,7 +119,7 @@ static void cart_pow(int l, int c, int pw[3])
 static void shell_pair_1e(const basis_t *B, int sa, int sb, const double *O,
                           double *S, double *D /* [3][na*nb] or NULL */)
 {
-    int la = B->sh_l[sa], lb = B->sh_l[sb], na = 2 * la + 1, nb = 2 * lb + 1;
+    int la = B->sh_l[sa], lb = B->sh_l[sb], na = NCART(la), nb = NCART(lb);
     const double *A = B->centers + 3 * B->sh_center[sa], *Bc = B->centers + 3 * B->sh_center[sb];
     for (int i = 0; i < na * nb; ++i) {
         S[i] = 0.0;
@@ -111,7 +130,7 @@ static void shell_pair_1e(const basis_t *B, int sa, int sb, const double *O,
             double a = B->exps[B->sh_off[sa] + ka], b = B->exps[B->sh_off[sb] + kb];
             double cc = B->ncoef[B->sh_off[sa] + ka] * B->ncoef[B->sh_off[sb] + kb];
             double p = a + b, pref = pow(M_PI / p, 1.5);
-            double E[3][2][2][3], P[3];
+            double E[3][LMAX + 1][LMAX + 1][2 * LMAX + 1], P[3];
             for (int x = 0; x < 3; ++x) {
                 hermite_E(a, b, A[x], Bc[x], E[x]);
                 P[x] = (a * A[x] + b * Bc[x]) / p;
@@ -126,12 +145,13 @@ static void shell_pair_1e(const basis_t *B, int sa, int sb, const double *O,
                         e0[x] = E[x][pa[x]][pb[x]][0];
                         e1[x] = E[x][pa[x]][pb[x]][1];
                     }
-                    S[ca * nb + cb] += cc * pref * e0[0] * e0[1] * e0[2];
+                    double cn = cart_norm(la, ca) * cart_norm(lb, cb);
+                    S[ca * nb + cb] += cn * (cc * pref * e0[0] * e0[1] * e0[2]);
                     if (D)
                         for (int x = 0; x < 3; ++x) {
                             double m = e1[x] + (P[x] - O[x]) * e0[x];
                             int y = (x + 1) % 3, z = (x + 2) % 3;
-                            D[x * na * nb + ca * nb + cb] += cc * pref * m * e0[y] * e0[z];
+                            D[x * na * nb + ca * nb + cb] += cn * (cc * pref * m * e0[y] * e0[z]);
                         }
                 }
         }
@@ -156,8 +176,8 @@ void oracle_one_electron(BASIS_ARGS, int nao, const double *O, double *S, double
     basis_t B = BASIS_MK;
     for (int sa = 0; sa < nshells; ++sa)
         for (int sb = 0; sb < nshells; ++sb) {
-            double s[9], d[27];
-            int na = 2 * sh_l[sa] + 1, nb = 2 * sh_l[sb] + 1;
+            double s[NCMAX * NCMAX], d[3 * NCMAX * NCMAX];
+            int na = NCART(sh_l[sa]), nb = NCART(sh_l[sb]);
             shell_pair_1e(&B, sa, sb, O, s, D ? d : NULL);
             for (int ca = 0; ca < na; ++ca)
                 for (int cb = 0; cb < nb; ++cb) {
@@ -176,7 +196,7 @@ void oracle_one_electron(BASIS_ARGS, int nao, const double *O, double *S, double
 /* Range-separated operator erf(omega r12)/r12 (NEXT-4: the long-range exchange of CAM-type functionals): with
  * theta^2 = omega^2 / (alpha + omega^2) the Hermite integrals are those of 1/r12 with alpha -> alpha theta^2 and an
  * overall factor theta:  R^n_{000} = theta (-2 alpha theta^2)^n F_n(alpha theta^2 |R|^2).  omega <= 0 means 1/r12. */
-static void hermite_R(int L, double alpha, double omega, const double *R, double Rt[5][5][5][5] /* [n][t][u][v] */)
+static void hermite_R(int L, double alpha, double omega, const double *R, double Rt[NR][NR][NR][NR] /* [n][t][u][v] */)
 {
     double F[LMAX_TOT + 1];
     double theta = 1.0;
@@ -187,7 +207,10 @@ static void hermite_R(int L, double alpha, double omega, const double *R, double
     }
     double T = alpha * (R[0] * R[0] + R[1] * R[1] + R[2] * R[2]);
     oracle_boys(L, T, F);
-    memset(Rt, 0, sizeof(double) * 625);
+    for (int n = 0; n <= L; ++n)        /* only n, t, u, v <= L are ever touched */
+        for (int t = 0; t <= L; ++t)
+            for (int u = 0; u <= L; ++u)
+                for (int v = 0; v <= L; ++v) Rt[n][t][u][v] = 0.0;
     double m2a = theta;
     for (int n = 0; n <= L; ++n) {
         Rt[n][0][0][0] = m2a * F[n];
@@ -219,18 +242,18 @@ static void hermite_R(int L, double alpha, double omega, const double *R, double
 static void shell_quartet_op(const basis_t *B, int sa, int sb, int sc, int sd, double omega, double *out)
 {
     int l[4] = {B->sh_l[sa], B->sh_l[sb], B->sh_l[sc], B->sh_l[sd]};
-    int n[4] = {2 * l[0] + 1, 2 * l[1] + 1, 2 * l[2] + 1, 2 * l[3] + 1};
+    int n[4] = {NCART(l[0]), NCART(l[1]), NCART(l[2]), NCART(l[3])};
     int L = l[0] + l[1] + l[2] + l[3];
     const double *A = B->centers + 3 * B->sh_center[sa], *Bc = B->centers + 3 * B->sh_center[sb];
     const double *C = B->centers + 3 * B->sh_center[sc], *D = B->centers + 3 * B->sh_center[sd];
     int ntot = n[0] * n[1] * n[2] * n[3];
-    long double acc[81];
+    long double acc[NQMAX];
     for (int i = 0; i < ntot; ++i) acc[i] = 0.0L;
     for (int ka = 0; ka < B->sh_nprim[sa]; ++ka)
     for (int kb = 0; kb < B->sh_nprim[sb]; ++kb) {
         double a = B->exps[B->sh_off[sa] + ka], b = B->exps[B->sh_off[sb] + kb];
         double cab = B->ncoef[B->sh_off[sa] + ka] * B->ncoef[B->sh_off[sb] + kb];
-        double p = a + b, P[3], Eab[3][2][2][3];
+        double p = a + b, P[3], Eab[3][LMAX + 1][LMAX + 1][2 * LMAX + 1];
         for (int x = 0; x < 3; ++x) {
             P[x] = (a * A[x] + b * Bc[x]) / p;
             hermite_E(a, b, A[x], Bc[x], Eab[x]);
@@ -239,14 +262,14 @@ static void shell_quartet_op(const basis_t *B, int sa, int sb, int sc, int sd, d
         for (int kd = 0; kd < B->sh_nprim[sd]; ++kd) {
             double c = B->exps[B->sh_off[sc] + kc], d = B->exps[B->sh_off[sd] + kd];
             double ccd = B->ncoef[B->sh_off[sc] + kc] * B->ncoef[B->sh_off[sd] + kd];
-            double q = c + d, Q[3], Ecd[3][2][2][3], RPQ[3];
+            double q = c + d, Q[3], Ecd[3][LMAX + 1][LMAX + 1][2 * LMAX + 1], RPQ[3];
             for (int x = 0; x < 3; ++x) {
                 Q[x] = (c * C[x] + d * D[x]) / q;
                 hermite_E(c, d, C[x], D[x], Ecd[x]);
                 RPQ[x] = P[x] - Q[x];
             }
             double alpha = p * q / (p + q);
-            double Rt[5][5][5][5];
+            double Rt[NR][NR][NR][NR];
             hermite_R(L, alpha, omega, RPQ, Rt);
             double pref = 2.0 * pow(M_PI, 2.5) / (p * q * sqrt(p + q)) * cab * ccd;
             int idx = 0;
@@ -272,7 +295,8 @@ static void shell_quartet_op(const basis_t *B, int sa, int sb, int sc, int sd, d
                         s += eab * sgn * ecd * Rt[0][t + t2][u + u2][v + v2];
                     }
                 }
-                acc[idx] += (long double)(pref * s);
+                double cn = cart_norm(l[0], ca) * cart_norm(l[1], cb) * cart_norm(l[2], cc) * cart_norm(l[3], cd);
+                acc[idx] += (long double)(cn * (pref * s));
             }
         }
     }
@@ -299,7 +323,7 @@ void oracle_primitive_eri(const double *ctr /* [4][3] */, const double *ex /* [4
     int32_t ao_off[4];
     double ncoef[4] = {1.0, 1.0, 1.0, 1.0};
     int o = 0;
-    for (int i = 0; i < 4; ++i) { ao_off[i] = o; o += 2 * l4[i] + 1; }
+    for (int i = 0; i < 4; ++i) { ao_off[i] = o; o += NCART(l4[i]); }
     basis_t B = mk_basis(4, ctr, sh_center, l4, sh_nprim, sh_off, ao_off, ex, ncoef);
     shell_quartet(&B, 0, 1, 2, 3, out);
 }
@@ -311,7 +335,7 @@ void oracle_primitive_eri_erf(const double *ctr, const double *ex, const int32_t
     int32_t ao_off[4];
     double ncoef[4] = {1.0, 1.0, 1.0, 1.0};
     int o = 0;
-    for (int i = 0; i < 4; ++i) { ao_off[i] = o; o += 2 * l4[i] + 1; }
+    for (int i = 0; i < 4; ++i) { ao_off[i] = o; o += NCART(l4[i]); }
     basis_t B = mk_basis(4, ctr, sh_center, l4, sh_nprim, sh_off, ao_off, ex, ncoef);
     shell_quartet_op(&B, 0, 1, 2, 3, omega, out);
 }
@@ -333,10 +357,10 @@ void oracle_eri_tensor_erf(BASIS_ARGS, int nao, double omega, double *eri)
     for (int sb = 0; sb < nshells; ++sb)
         for (int sc = 0; sc < nshells; ++sc)
         for (int sd = 0; sd < nshells; ++sd) {
-            double blk[81];
+            double blk[NQMAX];
             shell_quartet_op(&B, sa, sb, sc, sd, omega, blk);
-            int n0 = 2 * sh_l[sa] + 1, n1 = 2 * sh_l[sb] + 1, n2 = 2 * sh_l[sc] + 1,
-                n3 = 2 * sh_l[sd] + 1, idx = 0;
+            int n0 = NCART(sh_l[sa]), n1 = NCART(sh_l[sb]), n2 = NCART(sh_l[sc]),
+                n3 = NCART(sh_l[sd]), idx = 0;
             for (int ca = 0; ca < n0; ++ca)
             for (int cb = 0; cb < n1; ++cb)
             for (int cc = 0; cc < n2; ++cc)
@@ -355,16 +379,16 @@ void oracle_eri_tensor_erf(BASIS_ARGS, int nao, double omega, double *eri)
 void oracle_eri_pair_block(BASIS_ARGS, int nao, int sc, int sd, double tau, const double *Qs, double *out)
 {
     basis_t B = BASIS_MK;
-    int nc = 2 * sh_l[sc] + 1, nd = 2 * sh_l[sd] + 1;
+    int nc = NCART(sh_l[sc]), nd = NCART(sh_l[sd]);
     memset(out, 0, sizeof(double) * (size_t)nao * nao * nc * nd);
     double qcd = Qs[(size_t)sc * nshells + sd];
     #pragma omp parallel for schedule(dynamic, 2)
     for (int sa = 0; sa < nshells; ++sa)
         for (int sb = 0; sb <= sa; ++sb) {
             if (tau > 0.0 && Qs[(size_t)sa * nshells + sb] * qcd < tau) continue;
-            double blk[81];
+            double blk[NQMAX];
             shell_quartet(&B, sa, sb, sc, sd, blk);
-            int na = 2 * sh_l[sa] + 1, nb = 2 * sh_l[sb] + 1, idx = 0;
+            int na = NCART(sh_l[sa]), nb = NCART(sh_l[sb]), idx = 0;
             for (int ca = 0; ca < na; ++ca)
             for (int cb = 0; cb < nb; ++cb)
             for (int cc = 0; cc < nc; ++cc)
@@ -400,29 +424,34 @@ static void boys_ld(int nmax, long double T, long double *F)
     }
 }
 
-static void hermite_E_ld(long double a, long double b, long double Ax, long double Bx, long double E[2][2][3])
+static void hermite_E_ld(long double a, long double b, long double Ax, long double Bx,
+                         long double E[LMAX + 1][LMAX + 1][2 * LMAX + 1])
 {
     long double p = a + b, mu = a * b / p, XAB = Ax - Bx;
     long double Px = (a * Ax + b * Bx) / p, XPA = Px - Ax, XPB = Px - Bx;
-    for (int i = 0; i < 12; ++i) ((long double *)E)[i] = 0.0L;
+    for (int i = 0; i < (LMAX + 1) * (LMAX + 1) * (2 * LMAX + 1); ++i) ((long double *)E)[i] = 0.0L;
     E[0][0][0] = expl(-mu * XAB * XAB);
-    for (int t = 0; t <= 1; ++t) {
-        long double em = (t - 1 >= 0) ? E[0][0][t - 1] : 0.0L, e0 = E[0][0][t];
-        E[1][0][t] = em / (2 * p) + XPA * e0;
-    }
-    for (int i = 0; i <= 1; ++i)
+    for (int i = 0; i < LMAX; ++i)
         for (int t = 0; t <= i + 1; ++t) {
             long double em = (t - 1 >= 0) ? E[i][0][t - 1] : 0.0L;
             long double e0 = (t <= i) ? E[i][0][t] : 0.0L;
             long double ep = (t + 1 <= i) ? E[i][0][t + 1] : 0.0L;
-            E[i][1][t] = em / (2 * p) + XPB * e0 + (t + 1) * ep;
+            E[i + 1][0][t] = em / (2 * p) + XPA * e0 + (t + 1) * ep;
         }
+    for (int i = 0; i <= LMAX; ++i)
+        for (int j = 0; j < LMAX; ++j)
+            for (int t = 0; t <= i + j + 1; ++t) {
+                long double em = (t - 1 >= 0) ? E[i][j][t - 1] : 0.0L;
+                long double e0 = (t <= i + j) ? E[i][j][t] : 0.0L;
+                long double ep = (t + 1 <= i + j) ? E[i][j][t + 1] : 0.0L;
+                E[i][j + 1][t] = em / (2 * p) + XPB * e0 + (t + 1) * ep;
+            }
 }
 
 static void shell_quartet_ld(const basis_t *B, int sa, int sb, int sc, int sd, long double *out)
 {
     int l[4] = {B->sh_l[sa], B->sh_l[sb], B->sh_l[sc], B->sh_l[sd]};
-    int n[4] = {2 * l[0] + 1, 2 * l[1] + 1, 2 * l[2] + 1, 2 * l[3] + 1};
+    int n[4] = {NCART(l[0]), NCART(l[1]), NCART(l[2]), NCART(l[3])};
     int L = l[0] + l[1] + l[2] + l[3];
     const double *A = B->centers + 3 * B->sh_center[sa], *Bc = B->centers + 3 * B->sh_center[sb];
     const double *C = B->centers + 3 * B->sh_center[sc], *D = B->centers + 3 * B->sh_center[sd];
@@ -432,18 +461,21 @@ static void shell_quartet_ld(const basis_t *B, int sa, int sb, int sc, int sd, l
     for (int kb = 0; kb < B->sh_nprim[sb]; ++kb) {
         long double a = B->exps[B->sh_off[sa] + ka], b = B->exps[B->sh_off[sb] + kb];
         long double cab = (long double)B->ncoef[B->sh_off[sa] + ka] * B->ncoef[B->sh_off[sb] + kb];
-        long double p = a + b, P[3], Eab[3][2][2][3];
+        long double p = a + b, P[3], Eab[3][LMAX + 1][LMAX + 1][2 * LMAX + 1];
         for (int x = 0; x < 3; ++x) { P[x] = (a * A[x] + b * Bc[x]) / p; hermite_E_ld(a, b, A[x], Bc[x], Eab[x]); }
         for (int kc = 0; kc < B->sh_nprim[sc]; ++kc)
         for (int kd = 0; kd < B->sh_nprim[sd]; ++kd) {
             long double c = B->exps[B->sh_off[sc] + kc], d = B->exps[B->sh_off[sd] + kd];
             long double ccd = (long double)B->ncoef[B->sh_off[sc] + kc] * B->ncoef[B->sh_off[sd] + kd];
-            long double q = c + d, Q[3], Ecd[3][2][2][3], R[3];
+            long double q = c + d, Q[3], Ecd[3][LMAX + 1][LMAX + 1][2 * LMAX + 1], R[3];
             for (int x = 0; x < 3; ++x) { Q[x] = (c * C[x] + d * D[x]) / q; hermite_E_ld(c, d, C[x], D[x], Ecd[x]); R[x] = P[x] - Q[x]; }
             long double alpha = p * q / (p + q), F[LMAX_TOT + 1];
             boys_ld(L, alpha * (R[0] * R[0] + R[1] * R[1] + R[2] * R[2]), F);
-            static __thread long double Rt[5][5][5][5];
-            for (int i = 0; i < 625; ++i) ((long double *)Rt)[i] = 0.0L;
+            static __thread long double Rt[NR][NR][NR][NR];
+            for (int nn = 0; nn <= L; ++nn)
+                for (int t = 0; t <= L; ++t)
+                    for (int u = 0; u <= L; ++u)
+                        for (int v = 0; v <= L; ++v) Rt[nn][t][u][v] = 0.0L;
             long double m2a = 1.0L;
             for (int nn = 0; nn <= L; ++nn) { Rt[nn][0][0][0] = m2a * F[nn]; m2a *= -2.0L * alpha; }
             for (int N = 1; N <= L; ++N)
@@ -479,7 +511,10 @@ static void shell_quartet_ld(const basis_t *B, int sa, int sb, int sc, int sd, l
                         s += eab * sgn * ecd * Rt[0][t + t2][u + u2][v + v2];
                     }
                 }
-                out[idx] += pref * s;
+                long double cn = 1.0L;     /* sqrt(3) per mixed d component, in long double */
+                { int pw[4][3]; cart_pow(l[0], ca, pw[0]); cart_pow(l[1], cb, pw[1]); cart_pow(l[2], cc, pw[2]); cart_pow(l[3], cd, pw[3]);
+                  for (int k = 0; k < 4; ++k) if (l[k] == 2 && pw[k][0] < 2 && pw[k][1] < 2 && pw[k][2] < 2) cn *= sqrtl(3.0L); }
+                out[idx] += cn * (pref * s);
             }
         }
     }
@@ -494,9 +529,9 @@ void oracle_eri_tensor_ld(BASIS_ARGS, int nao, long double *eri)
     for (int sb = 0; sb < nshells; ++sb)
         for (int sc = 0; sc < nshells; ++sc)
         for (int sd = 0; sd < nshells; ++sd) {
-            long double blk[81];
+            long double blk[NQMAX];
             shell_quartet_ld(&B, sa, sb, sc, sd, blk);
-            int n0 = 2 * sh_l[sa] + 1, n1 = 2 * sh_l[sb] + 1, n2 = 2 * sh_l[sc] + 1, n3 = 2 * sh_l[sd] + 1, idx = 0;
+            int n0 = NCART(sh_l[sa]), n1 = NCART(sh_l[sb]), n2 = NCART(sh_l[sc]), n3 = NCART(sh_l[sd]), idx = 0;
             for (int ca = 0; ca < n0; ++ca)
             for (int cb = 0; cb < n1; ++cb)
             for (int cc = 0; cc < n2; ++cc)
@@ -514,9 +549,9 @@ void oracle_schwarz(BASIS_ARGS, double *Q)
     #pragma omp parallel for schedule(dynamic)
     for (int sa = 0; sa < nshells; ++sa)
         for (int sb = 0; sb <= sa; ++sb) {
-            double blk[81];
+            double blk[NQMAX];
             shell_quartet(&B, sa, sb, sa, sb, blk);
-            int na = 2 * sh_l[sa] + 1, nb = 2 * sh_l[sb] + 1;
+            int na = NCART(sh_l[sa]), nb = NCART(sh_l[sb]);
             double m = 0.0;
             for (int ca = 0; ca < na; ++ca)
                 for (int cb = 0; cb < nb; ++cb) {
@@ -582,14 +617,14 @@ void oracle_jk_strided_op(BASIS_ARGS, int nao, int nvec, const double *T, double
                 if (tau > 0.0 && qab * Qs[(size_t)sc * nshells + sd] < tau) continue;
                 ++nq;
                 npq += (int64_t)sh_nprim[sa] * sh_nprim[sb] * sh_nprim[sc] * sh_nprim[sd];
-                double blk[81];
+                double blk[NQMAX];
                 shell_quartet_op(&B, sa, sb, sc, sd, omega, blk);
                 double w = 1.0;
                 if (sa == sb) w *= 0.5;
                 if (sc == sd) w *= 0.5;
                 if (ab == cd) w *= 0.5;
-                int n0 = 2 * sh_l[sa] + 1, n1 = 2 * sh_l[sb] + 1, n2 = 2 * sh_l[sc] + 1,
-                    n3 = 2 * sh_l[sd] + 1, idx = 0;
+                int n0 = NCART(sh_l[sa]), n1 = NCART(sh_l[sb]), n2 = NCART(sh_l[sc]),
+                    n3 = NCART(sh_l[sd]), idx = 0;
                 for (int ca = 0; ca < n0; ++ca)
                 for (int cb = 0; cb < n1; ++cb)
                 for (int cc = 0; cc < n2; ++cc)
@@ -665,14 +700,14 @@ void oracle_jk_ld(BASIS_ARGS, int nao, int nvec, const long double *T, double ta
                 if (tau > 0.0 && qab * Qs[(size_t)sc * nshells + sd] < tau) continue;
                 ++nq;
                 npq += (int64_t)sh_nprim[sa] * sh_nprim[sb] * sh_nprim[sc] * sh_nprim[sd];
-                double blk[81];
+                double blk[NQMAX];
                 shell_quartet(&B, sa, sb, sc, sd, blk);
                 long double w = 1.0L;
                 if (sa == sb) w *= 0.5L;
                 if (sc == sd) w *= 0.5L;
                 if (ab == cd) w *= 0.5L;
-                int n0 = 2 * sh_l[sa] + 1, n1 = 2 * sh_l[sb] + 1, n2 = 2 * sh_l[sc] + 1,
-                    n3 = 2 * sh_l[sd] + 1, idx = 0;
+                int n0 = NCART(sh_l[sa]), n1 = NCART(sh_l[sb]), n2 = NCART(sh_l[sc]),
+                    n3 = NCART(sh_l[sd]), idx = 0;
                 for (int ca = 0; ca < n0; ++ca)
                 for (int cb = 0; cb < n1; ++cb)
                 for (int cc = 0; cc < n2; ++cc)
@@ -717,19 +752,19 @@ void oracle_jk_samples(BASIS_ARGS, int nao, int nvec, const double *T, int nsamp
     size_t nn = (size_t)nao * nao;
     int32_t *ao2sh = malloc(sizeof(int32_t) * nao);
     for (int s = 0; s < nshells; ++s)
-        for (int c = 0; c < 2 * sh_l[s] + 1; ++c) ao2sh[ao_off[s] + c] = s;
+        for (int c = 0; c < NCART(sh_l[s]); ++c) ao2sh[ao_off[s] + c] = s;
     #pragma omp parallel for schedule(dynamic)
     for (int smp = 0; smp < nsamp; ++smp) {
         int mu = smu[smp], nu = snu[smp], sa = ao2sh[mu], sb = ao2sh[nu];
         int ca = mu - ao_off[sa], cb = nu - ao_off[sb];
-        int na = 2 * sh_l[sa] + 1, nb = 2 * sh_l[sb] + 1;
+        int na = NCART(sh_l[sa]), nb = NCART(sh_l[sb]);
         (void)na;
         long double Jacc[64], Kacc[64];
         for (int v = 0; v < nvec; ++v) Jacc[v] = Kacc[v] = 0.0L;
         for (int sc = 0; sc < nshells; ++sc)
             for (int sd = 0; sd < nshells; ++sd) {
-                int nc = 2 * sh_l[sc] + 1, nd = 2 * sh_l[sd] + 1;
-                double bj[81], bk[81];
+                int nc = NCART(sh_l[sc]), nd = NCART(sh_l[sd]);
+                double bj[NQMAX], bk[NQMAX];
                 shell_quartet(&B, sa, sb, sc, sd, bj); /* (mu nu|lam sig) */
                 shell_quartet(&B, sa, sc, sb, sd, bk); /* (mu lam|nu sig) */
                 for (int cc = 0; cc < nc; ++cc)

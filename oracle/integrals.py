@@ -48,11 +48,19 @@ def boys(nmax: int, T: float) -> np.ndarray:
     return F
 
 
+def ncart(l):
+    """Cartesian components of a shell: 1 (s), 3 (p), 6 (d: xx, xy, xz, yy, yz, zz)."""
+    l = np.asarray(l)
+    return (l + 1) * (l + 2) // 2
+
+
 def primitive_norm(a, l):
-    """N(a,0) = (2a/pi)^(3/4); N(a,1) = (2a/pi)^(3/4) 2 sqrt(a)  (definitions)."""
+    """N(a,0) = (2a/pi)^(3/4); N(a,1) = N(a,0) 2 sqrt(a); N(a,2) = N(a,0) 4a / sqrt(3), the norm of the xx
+    component (xy, xz, yz carry sqrt(3) more inside integrals.c)  (definitions)."""
     a = np.asarray(a, dtype=np.float64)
+    l = np.asarray(l)
     n = (2.0 * a / np.pi) ** 0.75
-    return n * np.where(np.asarray(l) == 1, 2.0 * np.sqrt(a), 1.0)
+    return n * np.where(l == 1, 2.0 * np.sqrt(a), np.where(l == 2, 4.0 * a / np.sqrt(3.0), 1.0))
 
 
 class OracleBasis:
@@ -66,7 +74,7 @@ class OracleBasis:
         self.sh_nprim, self._pn = _i(basis.sh_nprim)
         self.sh_off, self._po = _i(basis.sh_off)
         self.nshells = int(self.sh_l.shape[0])
-        n = 2 * self.sh_l.astype(np.int64) + 1
+        n = ncart(self.sh_l.astype(np.int64))
         self.ao_off, self._pa = _i(np.concatenate([[0], np.cumsum(n)[:-1]]))
         self.nao = int(n.sum())
         self.exps, self._pe = _d(basis.exps)
@@ -75,7 +83,7 @@ class OracleBasis:
         self.ncoef, self._pk = _d(raw)
         S = self.overlap()
         scale = 1.0 / np.sqrt(np.diag(S))
-        sh_scale = scale[self.ao_off]          # x, y, z of a p shell share the radial part
+        sh_scale = scale[self.ao_off]          # first component (x of p, xx of d): the shell's radial part
         self.ncoef, self._pk = _d(raw * np.repeat(sh_scale, self.sh_nprim))
 
     def _args(self):
@@ -98,7 +106,7 @@ class OracleBasis:
         return D
 
     def shell_quartet(self, a, b, c, d) -> np.ndarray:
-        n = [2 * int(self.sh_l[s]) + 1 for s in (a, b, c, d)]
+        n = [int(ncart(int(self.sh_l[s]))) for s in (a, b, c, d)]
         out = np.zeros(n)
         lib().oracle_shell_quartet(*self._args(), ct.c_int(a), ct.c_int(b), ct.c_int(c),
                                    ct.c_int(d), out.ctypes.data_as(_dp))
@@ -149,7 +157,7 @@ class OracleBasis:
 
     def eri_pair_block(self, sc: int, sd: int, tau: float = 0.0, Q: np.ndarray | None = None) -> np.ndarray:
         """(mu nu|lam sig) for all mu, nu and the AOs lam, sig of the shell pair (sc, sd): [N][N][nc][nd]."""
-        nc, nd = 2 * int(self.sh_l[sc]) + 1, 2 * int(self.sh_l[sd]) + 1
+        nc, nd = int(ncart(int(self.sh_l[sc]))), int(ncart(int(self.sh_l[sd])))
         out = np.zeros((self.nao, self.nao, nc, nd))
         if Q is None:
             Q = self.schwarz()
@@ -243,7 +251,7 @@ def primitive_eri(centers4, exps4, l4) -> np.ndarray:
     c, pc = _d(np.asarray(centers4).reshape(4, 3))
     e, pe = _d(exps4)
     l, pl = _i(l4)
-    out = np.zeros([2 * int(x) + 1 for x in l])
+    out = np.zeros([int(ncart(int(x))) for x in l])
     lib().oracle_primitive_eri(pc, pe, pl, out.ctypes.data_as(_dp))
     return out
 
@@ -253,7 +261,7 @@ def primitive_eri_erf(centers4, exps4, l4, omega: float) -> np.ndarray:
     c, pc = _d(np.asarray(centers4).reshape(4, 3))
     e, pe = _d(exps4)
     l, pl = _i(l4)
-    out = np.zeros([2 * int(x) + 1 for x in l])
+    out = np.zeros([int(ncart(int(x))) for x in l])
     lib().oracle_primitive_eri_erf(pc, pe, pl, ct.c_double(omega), out.ctypes.data_as(_dp))
     return out
 

@@ -104,7 +104,8 @@ class _BasisHolder:
         dp = ct.POINTER(ct.c_double)
         self.c = BasisT(self.centers.ctypes.data_as(dp), int(self.centers.shape[0]), n, self.shells,
                         self.exps.ctypes.data_as(dp), self.coefs.ctypes.data_as(dp))
-        self.nao = int(np.sum(2 * np.asarray(basis.sh_l) + 1))
+        _l = np.asarray(basis.sh_l, dtype=np.int64)
+        self.nao = int(np.sum((_l + 1) * (_l + 2) // 2))
 
 
 def make_field(f: dict) -> FieldT:

@@ -72,6 +72,9 @@ __device__ __forceinline__ int warp_reduce_owner_index(int lane)
 }
 
 constexpr int REC_TILE = 256;
+#ifndef RTTDA_K_MAXNI
+#define RTTDA_K_MAXNI 3
+#endif
 #ifndef RTTDA_K_PP_MAXNI
 #define RTTDA_K_PP_MAXNI 27
 #endif
@@ -707,7 +710,7 @@ static int launch_digest(Handle* h, const JKLaunch& L, const Segment& sg, const 
         const int KW = 32 / G, nwarps = (32 + KW - 1) / KW;
         // one or three integrals per quartet: the multi-record ring (digest_k_kernel) wins; above that its larger
         // register footprint costs more occupancy than the saved barriers bring (profiles/README.md)
-        if (NI > 3) digest_b_kernel<LA, LB, LC, LD><<<dim3(4 * L.nwork), dim3(32 * nwarps), smem, st>>>(g, G, KW);
+        if (NI > RTTDA_K_MAXNI) digest_b_kernel<LA, LB, LC, LD><<<dim3(4 * L.nwork), dim3(32 * nwarps), smem, st>>>(g, G, KW);
         else digest_k_kernel<LA, LB, LC, LD><<<dim3(4 * L.nwork), dim3(32 * nwarps), digest_k_smem(NI), st>>>(g, G, KW);
         h->kernel_launches++;
         RT_CUDA(cudaGetLastError());

@@ -4,6 +4,7 @@ Recipe = BASELINE.json `configs` (BJ:configs[0..4]) under DESIGN.md readings:
   R11 contraction coefficients d_k ~ U[0.2, 1.0] on normalised primitives (each side renormalises
       the contracted function itself);
   R12 config-4 heavy centre = s(3), s(3), s(1), p(3), p(1) (9 AOs), H-like = s(3), s(1) (2 AOs);
+      the d-shell test molecule ("tiny-d", key 6): heavy = s(3), s(1), p(3), p(1), d(1) (14 AOs, Cartesian d);
   R13 box edge L = 8 (n_centres/6)^(1/3) bohr, rejection sampling for the 1.8 bohr minimum;
   R17 trial vectors iid N(0,1), scaled to unit 2-norm;
   R18 C = S^-1/2 Q, Q = sign-fixed QR of an N x N N(0,1) matrix; eps_occ ~ U[-1,-0.3],
@@ -22,7 +23,7 @@ SEED = 260116949
 class Basis:
     centers: np.ndarray      # [ncenters][3] float64, bohr
     sh_center: np.ndarray    # [nshells] int32
-    sh_l: np.ndarray         # [nshells] int32, 0 = s, 1 = p (x, y, z)
+    sh_l: np.ndarray         # [nshells] int32, 0 = s, 1 = p (x, y, z), 2 = d (xx, xy, xz, yy, yz, zz)
     sh_nprim: np.ndarray     # [nshells] int32
     sh_off: np.ndarray       # [nshells] int32, offset into exps / coefs
     exps: np.ndarray         # [sum nprim] float64
@@ -38,11 +39,13 @@ class Basis:
 
     @property
     def nao(self) -> int:
-        return int(np.sum(2 * self.sh_l + 1))
+        l = self.sh_l.astype(np.int64)
+        return int(np.sum((l + 1) * (l + 2) // 2))
 
     @property
     def ao_off(self) -> np.ndarray:
-        n = 2 * self.sh_l.astype(np.int64) + 1
+        l = self.sh_l.astype(np.int64)
+        n = (l + 1) * (l + 2) // 2
         return np.concatenate([[0], np.cumsum(n)[:-1]]).astype(np.int32)
 
 
@@ -73,6 +76,7 @@ class Config:
 _SP5 = ((0, 3), (0, 1), (1, 1))                      # BJ:configs[0]: 2 s shells (3, 1 prims) + p(1)
 _HEAVY9 = ((0, 3), (0, 3), (0, 1), (1, 3), (1, 1))   # R12
 _H2 = ((0, 3), (0, 1))
+_SPD14 = ((0, 3), (0, 1), (1, 3), (1, 1), (2, 1))    # 6-31G*-like heavy centre with one Cartesian d shell (NEXT-4)
 
 CONFIGS = {
     1: Config("tiny", 6, 0, _SP5, (), 5, 25, 1e-12, 0.05, 10,
@@ -87,6 +91,9 @@ CONFIGS = {
               tuple({"type": "sin2", "E0": e, "omega": None, "T_env": 200.0,
                      "dir": (0.0, 0.0, 1.0)} for e in (0.01, 0.03, 0.05)), 4),
     5: Config("sigma-microbench", 120, 100, _HEAVY9, _H2, 400, 880, 1e-12, 0.0, 0, (), 4),
+    # not a BASELINE.json config: the small d-shell molecule of the NEXT-4 tests (4 heavy centres + 2 H-like, 60 AOs)
+    6: Config("tiny-d", 4, 2, _SPD14, _H2, 10, 50, 1e-12, 0.05, 10,
+              ({"type": "cw", "E0": 0.01, "omega": 0.3, "dir": (0.0, 0.0, 1.0)},), 6),
 }
 
 
@@ -121,7 +128,7 @@ def make_basis(cfg: Config, bump: int = 0) -> Basis:
     sh_center, sh_l, sh_nprim, exps, coefs = [], [], [], [], []
     for c in range(n):
         for (l, nprim) in (cfg.h_shells if kinds[c] else cfg.heavy_shells):
-            lo, hi = (0.1, 20.0) if l == 0 else (0.2, 2.0)
+            lo, hi = (0.1, 20.0) if l == 0 else ((0.2, 2.0) if l == 1 else (0.3, 1.5))
             e = np.exp(rng.uniform(np.log(lo), np.log(hi), size=nprim))
             d = rng.uniform(0.2, 1.0, size=nprim)
             sh_center.append(c)
