@@ -296,6 +296,7 @@ int rttda_get_info(rttda_handle_t hh, int32_t key, double* out)
         RT_CUDA(cudaMemcpy(c, h->d_primcount, sizeof c, cudaMemcpyDeviceToHost));
         double n = 0.0, fl = 0.0;
         for (int L = 0; L <= 4; ++L) { n += (double)c[L]; fl += (double)c[L] * flops_prim_L(L); }
+        n += (double)c[5]; fl += (double)c[6];              // classes with a d shell (eri_generic.cu)
         if (n > 0.0) *out = (key == RTTDA_INFO_NPRIM_EVAL) ? n : fl;
     }
     return RTTDA_OK;

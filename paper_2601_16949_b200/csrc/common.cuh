@@ -43,10 +43,15 @@ void set_error(const std::string& msg);
 // so that c_bra * c_ket / sqrt(p+q) = 2 pi^(5/2) / (p q sqrt(p+q)) * K_ab K_cd * coefficients.
 constexpr int PRIM_STRIDE = 12;
 
-// Pair classes: 0 = ss, 1 = ps (p first), 2 = pp; contraction sub-class by number of primitive pairs kept after
-// primitive screening (setup.cu), rounded up to 1, 3, 6 or 9.
+// Pair classes (higher l first): 0 = ss, 1 = ps, 2 = pp, 3 = ds, 4 = dp, 5 = dd; contraction sub-class by number of
+// primitive pairs kept after primitive screening (setup.cu), rounded up to 1, 3, 6 or 9.
 constexpr int NSUB = 4;                       // primitive pairs stored per shell pair: {1, 3, 6, 9}
-constexpr int NKETCLASS = 3 * NSUB;           // ket class id = pairclass * NSUB + sub
+constexpr int NPAIRCLASS = 6;
+constexpr int NKETCLASS = NPAIRCLASS * NSUB;  // ket class id = pairclass * NSUB + sub
+__host__ __device__ inline int ncart(int l) { return (l + 1) * (l + 2) / 2; }     // Cartesian components of a shell
+inline int pairclass_of(int l1, int l2) { return l1 * (l1 + 1) / 2 + l2; }       // l1 >= l2
+inline int pairclass_l1(int pc) { return pc >= 3 ? 2 : (pc >= 1 ? 1 : 0); }
+inline int pairclass_l2(int pc) { return pc - pairclass_l1(pc) * (pairclass_l1(pc) + 1) / 2; }
 __host__ __device__ inline int sub_to_np(int sub) { return sub == 0 ? 1 : (sub == 1 ? 3 : (sub == 2 ? 6 : 9)); }
 
 // Unique (unordered) pairs of one pair class (pair type x contraction sub-class), sorted by Schwarz bound
@@ -143,7 +148,8 @@ void boys_table_host(int L, std::vector<double>& tab);
 struct Handle {
     int device = 0;
     int nao = 0, nocc = 0, nvirt = 0, ncsf = 0, nshells = 0;
-    unsigned long long* d_primcount = nullptr; // [8] primitive quartets evaluated in the last ERI pass, per total L (jk_eval.cu)
+    unsigned long long* d_primcount = nullptr; // [8] primitive quartets evaluated in the last ERI pass: [0..4] s/p classes by total L
+                                               // (jk_eval.cu), [5] all classes of the general path (eri_generic.cu), [6] their model flops
     double cx = 1.0, tau = 0.0;
     // range-separated exchange (NEXT-4): A -= cx_lr (ij| erf(omega r12)/r12 |ab); rs_omega <= 0 or cx_lr == 0: off
     double cx_lr = 0.0, rs_omega = 0.0;
@@ -213,6 +219,7 @@ int assign_lanes(Handle* h, int nlanes);
 // Primitive-level screening threshold: three orders below the shell-level one, and never looser than 1e-15, so that its
 // error stays far below both the shell screening error and the 1e-10 sigma tolerance at any tau.
 inline double prim_threshold(double tau) { return tau * 1e-3 < 1e-15 ? tau * 1e-3 : 1e-15; }
+double flops_prim(int la, int lb, int lc, int ld);
 double flops_prim_L(int L);                // flop model of one primitive quartet of total angular momentum L   // record the next event of the J/K timing log
 
 // jk_eval.cu / jk_digest.cu
@@ -220,11 +227,21 @@ double flops_prim_L(int L);                // flop model of one primitive quarte
 int jk_build(Handle* h, int nvt, int nvec, const double* Tq, double* Fq, cudaStream_t st);
 int jk_profile(Handle* h, int nvt, int nvec, const double* Tq, double* Fq, cudaStream_t st, double* rows, int cap, int* nrows);
 int eval_segment(Handle* h, const Segment& sg, double* buf, cudaStream_t st);
-int digest_launch(Handle* h, const JKLaunch& L, const Segment& sg, const double* buf, int nvt, const double* Tq,
+int digest_launch(Handle* h, const JKLaunch& L, const Segment& sg, const double* buf, int nvt, int nvec, const double* Tq,
                   double* Fq, cudaStream_t st);
 inline int padded_nvec(int nvec) { return nvec <= 2 ? 2 : (nvec <= 4 ? 4 : ((nvec + 7) & ~7)); }
 int schwarz_device(int pairclass, int npairs, const int* d_np, const int* d_off, const double* d_prim,
                    const double2* d_boys /* table for L = 2 * pairclass */, double* d_Q, cudaStream_t st);
+// eri_generic.cu: the general-angular-momentum path (classes with a d shell)
+bool segment_is_general(const Segment& sg);
+int eval_segment_general(Handle* h, const Segment& sg, double* buf, cudaStream_t st);
+int digest_segment_general(Handle* h, const Segment& sg, const double* buf, int nvt, int nvec, const double* Tq, double* Fq,
+                           cudaStream_t st);
+int schwarz_general(int la, int lb, int npairs, const int* d_np, const int* d_off, const double* d_prim, double* d_Q,
+                    cudaStream_t st);
+// evaluate + digest one segment (fast or general path)
+int digest_segment(Handle* h, const Segment& sg, const double* buf, int nvt, int nvec, const double* Tq, double* Fq,
+                   cudaStream_t st);
 
 // gemm_f64.cu: C(m,n) = alpha * sum_k A(m,k) B(k,n) + beta * C(m,n), fully strided, batched.
 struct GemmDesc {

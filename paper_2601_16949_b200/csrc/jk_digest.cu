@@ -718,6 +718,16 @@ static int launch_digest(Handle* h, const JKLaunch& L, const Segment& sg, const 
     return RTTDA_OK;
 }
 
+// All digestion work of one segment: the a-list launches of the s/p classes, or the general-path kernel.
+int digest_segment(Handle* h, const Segment& sg, const double* buf, int nvt, int nvec, const double* Tq, double* Fq,
+                   cudaStream_t st)
+{
+    if (segment_is_general(sg)) return digest_segment_general(h, sg, buf, nvt, nvec, Tq, Fq, st);
+    for (int l = sg.first_launch; l < sg.first_launch + sg.nlaunch; ++l)
+        RT_TRY(digest_launch(h, h->launches[l], sg, buf, nvt, nvec, Tq, Fq, st));
+    return RTTDA_OK;
+}
+
 int digest_launch(Handle* h, const JKLaunch& L, const Segment& sg, const double* buf, int nvt, int nvec,
                   const double* Tq, double* Fq, cudaStream_t st)
 {
@@ -789,8 +799,7 @@ int jk_build(Handle* h, int nvt, int nvec, const double* Tq, double* Fq, cudaStr
             if (sg.nitems == 0) continue;
             double* buf = h->eri_all + sg.incore_off;
             if (!h->incore_valid) RT_TRY(eval_segment(h, sg, buf, st));
-            for (int l = sg.first_launch; l < sg.first_launch + sg.nlaunch; ++l)
-                RT_TRY(digest_launch(h, h->launches[l], sg, buf, nvt, nvec, Tq, Fq, st));
+            RT_TRY(digest_segment(h, sg, buf, nvt, nvec, Tq, Fq, st));
         }
         h->incore_valid = true;
         continue;
@@ -811,8 +820,7 @@ int jk_build(Handle* h, int nvt, int nvec, const double* Tq, double* Fq, cudaStr
             RT_TRY(eval_segment(h, sg, h->eri_buf[b], se));
             RT_CUDA(cudaEventRecord(evE[b], se));
             RT_CUDA(cudaStreamWaitEvent(st, evE[b], 0));
-            for (int l = sg.first_launch; l < sg.first_launch + sg.nlaunch; ++l)
-                RT_TRY(digest_launch(h, h->launches[l], sg, h->eri_buf[b], nvt, nvec, Tq, Fq, st));
+            RT_TRY(digest_segment(h, sg, h->eri_buf[b], nvt, nvec, Tq, Fq, st));
             RT_CUDA(cudaEventRecord(evD[b], st));
             ++k;
         }
@@ -827,8 +835,7 @@ int jk_build(Handle* h, int nvt, int nvec, const double* Tq, double* Fq, cudaStr
         for (int si : h->lane_segs[l]) {
             const Segment& sg = h->segments[si];
             RT_TRY(eval_segment(h, sg, h->eri_buf[l], ls));
-            for (int k = sg.first_launch; k < sg.first_launch + sg.nlaunch; ++k)
-                RT_TRY(digest_launch(h, h->launches[k], sg, h->eri_buf[l], nvt, nvec, Tq, Fq, ls));
+            RT_TRY(digest_segment(h, sg, h->eri_buf[l], nvt, nvec, Tq, Fq, ls));
         }
         RT_CUDA(cudaEventRecord(h->lane_ev[l], ls));
         RT_CUDA(cudaStreamWaitEvent(st, h->lane_ev[l], 0));
@@ -858,8 +865,7 @@ int jk_profile(Handle* h, int nvt, int nvec, const double* Tq, double* Fq, cudaS
         RT_CUDA(cudaEventRecord(e[0], st));
         RT_TRY(eval_segment(h, sg, h->eri_buf[0], st));
         RT_CUDA(cudaEventRecord(e[1], st));
-        for (int l = sg.first_launch; l < sg.first_launch + sg.nlaunch; ++l)
-            RT_TRY(digest_launch(h, h->launches[l], sg, h->eri_buf[0], nvt, nvec, Tq, Fq, st));
+        RT_TRY(digest_segment(h, sg, h->eri_buf[0], nvt, nvec, Tq, Fq, st));
         RT_CUDA(cudaEventRecord(e[2], st));
         RT_CUDA(cudaEventSynchronize(e[2]));
         float me = 0, md = 0;

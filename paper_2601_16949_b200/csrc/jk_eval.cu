@@ -203,6 +203,7 @@ static int launch_eval(Handle* h, const Segment& sg, double* buf, cudaStream_t s
 int eval_segment(Handle* h, const Segment& sg, double* buf, cudaStream_t st)
 {
     if (sg.nitems == 0) return RTTDA_OK;
+    if (segment_is_general(sg)) return eval_segment_general(h, sg, buf, st);
     const int key = sg.la * 8 + sg.lb * 4 + sg.lc * 2 + sg.ld;
     switch (key) {
         case 0:  return launch_eval<0, 0, 0, 0>(h, sg, buf, st);

@@ -57,7 +57,7 @@ static int load_basis(const rttda_basis_t* b, HostBasis& H)
     int ao = 0;
     for (int s = 0; s < b->nshells; ++s) {
         const rttda_shell_t& sh = b->shells[s];
-        RT_CHECK(sh.l == 0 || sh.l == 1, "basis: only s and p shells are supported");
+        RT_CHECK(sh.l >= 0 && sh.l <= 2, "basis: only s, p and (Cartesian) d shells are supported");
         RT_CHECK(sh.nprim >= 1 && sh.nprim <= RTTDA_MAX_NPRIM, "basis: nprim out of range");
         RT_CHECK(sh.center >= 0 && sh.center < b->ncenters, "basis: bad centre index");
         // Contraction depths 1 and 3 have their own kernel instantiations; a 2-primitive shell is carried as a
@@ -65,7 +65,7 @@ static int load_basis(const rttda_basis_t* b, HostBasis& H)
         const int np_store = sh.nprim == 2 ? 3 : sh.nprim;
         H.l.push_back(sh.l); H.np.push_back(np_store); H.np_true.push_back(sh.nprim); H.off.push_back((int)H.ex.size());
         H.center.push_back(sh.center); H.ao.push_back(ao);
-        ao += 2 * sh.l + 1;
+        ao += ncart(sh.l);
         // Primitives are taken in order of ascending exponent: the contraction sums do not depend on the order, but
         // with every shell sorted the same way a primitive-pair index means "diffuse x diffuse" ... "tight x tight"
         // for all kets of a warp alike, which makes the near-field / far-field Boys branch of the evaluation kernels
@@ -80,16 +80,18 @@ static int load_basis(const rttda_basis_t* b, HostBasis& H)
             RT_CHECK(a > 0.0, "basis: non-positive exponent");
             double nrm = std::pow(2.0 * a / M_PI, 0.75);
             if (sh.l == 1) nrm *= 2.0 * std::sqrt(a);
+            if (sh.l == 2) nrm *= 4.0 * a / std::sqrt(3.0);          // the xx component; xy, xz, yz carry sqrt(3) more (R11)
             c[k] = b->coefs[sh.prim_off + order[k]] * nrm;
             H.ex.push_back(a);
         }
-        // self overlap of the contracted function: s: sum c c (pi/p)^1.5 ; p: sum c c (pi/p)^1.5 / (2p)
+        // self overlap of the contracted function: s: sum c c (pi/p)^1.5 ; p: ... / (2p) ; d (xx): ... * 3 / (4 p^2)
         double self = 0.0;
         for (int k = 0; k < sh.nprim; ++k)
             for (int m = 0; m < sh.nprim; ++m) {
                 const double p = H.ex[H.off.back() + k] + H.ex[H.off.back() + m];   // sorted order, as c[]
                 double t = c[k] * c[m] * std::pow(M_PI / p, 1.5);
                 if (sh.l == 1) t /= 2.0 * p;
+                if (sh.l == 2) t *= 0.75 / (p * p);
                 self += t;
             }
         RT_CHECK(self > 0.0, "basis: contracted function has zero norm");
@@ -100,41 +102,53 @@ static int load_basis(const rttda_basis_t* b, HostBasis& H)
     return RTTDA_OK;
 }
 
-// One-electron block of a shell pair: S[na*nb] and D[3][na*nb] (origin 0).
+// One-electron block of a shell pair: S[na*nb] and D[3][na*nb] (origin 0), from the 1-D Hermite coefficients
+// E_0 (overlap) and E_1 + P E_0 (first moment) of every primitive pair; Gaussian-product factor in `base`.
 static void pair_1e(const HostBasis& H, int sa, int sb, double* S, double* D)
 {
-    const int la = H.l[sa], lb = H.l[sb], na = 2 * la + 1, nb = 2 * lb + 1;
+    const int la = H.l[sa], lb = H.l[sb], na = ncart(la), nb = ncart(lb);
     const double* A = &H.xyz[3 * H.center[sa]];
     const double* B = &H.xyz[3 * H.center[sb]];
     std::fill(S, S + na * nb, 0.0);
     std::fill(D, D + 3 * na * nb, 0.0);
     const double ab2 = (A[0] - B[0]) * (A[0] - B[0]) + (A[1] - B[1]) * (A[1] - B[1]) + (A[2] - B[2]) * (A[2] - B[2]);
+    auto powers = [](int l, int c, int* pw) {              // s; x y z; xx xy xz yy yz zz
+        pw[0] = pw[1] = pw[2] = 0;
+        if (l == 1) pw[c] = 1;
+        if (l == 2) { const int f = c < 3 ? 0 : (c < 5 ? 1 : 2), g = c < 3 ? c : (c < 5 ? c - 2 : 2); pw[f] += 1; pw[g] += 1; }
+    };
+    auto cnorm = [](int l, int c) { return (l == 2 && (c == 1 || c == 2 || c == 4)) ? std::sqrt(3.0) : 1.0; };
     for (int ka = 0; ka < H.np[sa]; ++ka)
         for (int kb = 0; kb < H.np[sb]; ++kb) {
             const double a = H.ex[H.off[sa] + ka], b = H.ex[H.off[sb] + kb], p = a + b;
             const double base = H.cf[H.off[sa] + ka] * H.cf[H.off[sb] + kb] * std::pow(M_PI / p, 1.5) *
                                 std::exp(-a * b / p * ab2);
-            double P[3], e0[3][2][2], e1[3][2][2];   // [axis][i][j]: Hermite E_0 and E_1 (K factored out)
+            double P[3], E[3][3][3][6];                     // [axis][i][j][t], t <= i + j (+1 slack)
             for (int x = 0; x < 3; ++x) {
                 P[x] = (a * A[x] + b * B[x]) / p;
                 const double xa = P[x] - A[x], xb = P[x] - B[x], h = 0.5 / p;
-                e0[x][0][0] = 1.0;            e1[x][0][0] = 0.0;
-                e0[x][1][0] = xa;             e1[x][1][0] = h;
-                e0[x][0][1] = xb;             e1[x][0][1] = h;
-                e0[x][1][1] = xa * xb + h;    e1[x][1][1] = (xa + xb) * h;
+                for (int i = 0; i < 3; ++i) for (int j = 0; j < 3; ++j) for (int t = 0; t < 6; ++t) E[x][i][j][t] = 0.0;
+                E[x][0][0][0] = 1.0;
+                for (int i = 0; i < la; ++i)
+                    for (int t = 0; t <= i + 1; ++t)
+                        E[x][i + 1][0][t] = (t > 0 ? h * E[x][i][0][t - 1] : 0.0) + xa * E[x][i][0][t] + (t + 1) * E[x][i][0][t + 1];
+                for (int i = 0; i <= la; ++i)
+                    for (int j = 0; j < lb; ++j)
+                        for (int t = 0; t <= i + j + 1; ++t)
+                            E[x][i][j + 1][t] = (t > 0 ? h * E[x][i][j][t - 1] : 0.0) + xb * E[x][i][j][t] + (t + 1) * E[x][i][j][t + 1];
             }
             for (int ca = 0; ca < na; ++ca)
                 for (int cb = 0; cb < nb; ++cb) {
-                    int pa[3] = {0, 0, 0}, pb[3] = {0, 0, 0};
-                    if (la) pa[ca] = 1;
-                    if (lb) pb[cb] = 1;
-                    const double f0 = e0[0][pa[0]][pb[0]], f1 = e0[1][pa[1]][pb[1]], f2 = e0[2][pa[2]][pb[2]];
-                    S[ca * nb + cb] += base * f0 * f1 * f2;
-                    const double m0 = e1[0][pa[0]][pb[0]] + P[0] * f0, m1 = e1[1][pa[1]][pb[1]] + P[1] * f1,
-                                 m2 = e1[2][pa[2]][pb[2]] + P[2] * f2;
-                    D[0 * na * nb + ca * nb + cb] += base * m0 * f1 * f2;
-                    D[1 * na * nb + ca * nb + cb] += base * f0 * m1 * f2;
-                    D[2 * na * nb + ca * nb + cb] += base * f0 * f1 * m2;
+                    int pa[3], pb[3];
+                    powers(la, ca, pa); powers(lb, cb, pb);
+                    const double cn = base * cnorm(la, ca) * cnorm(lb, cb);
+                    const double f0 = E[0][pa[0]][pb[0]][0], f1 = E[1][pa[1]][pb[1]][0], f2 = E[2][pa[2]][pb[2]][0];
+                    S[ca * nb + cb] += cn * f0 * f1 * f2;
+                    const double m0 = E[0][pa[0]][pb[0]][1] + P[0] * f0, m1 = E[1][pa[1]][pb[1]][1] + P[1] * f1,
+                                 m2 = E[2][pa[2]][pb[2]][1] + P[2] * f2;
+                    D[0 * na * nb + ca * nb + cb] += cn * m0 * f1 * f2;
+                    D[1 * na * nb + ca * nb + cb] += cn * f0 * m1 * f2;
+                    D[2 * na * nb + ca * nb + cb] += cn * f0 * f1 * m2;
                 }
         }
 }
@@ -144,9 +158,9 @@ static void one_electron_host(const HostBasis& H, double* S, double* D)
     const size_t N = H.nao;
     for (int sa = 0; sa < H.nshells; ++sa)
         for (int sb = 0; sb < H.nshells; ++sb) {
-            double s[9], d[27];
+            double s[36], d[108];
             pair_1e(H, sa, sb, s, d);
-            const int na = 2 * H.l[sa] + 1, nb = 2 * H.l[sb] + 1;
+            const int na = ncart(H.l[sa]), nb = ncart(H.l[sb]);
             for (int ca = 0; ca < na; ++ca)
                 for (int cb = 0; cb < nb; ++cb) {
                     const size_t idx = (size_t)(H.ao[sa] + ca) * N + H.ao[sb] + cb;
@@ -217,7 +231,7 @@ static int np_to_sub(int np) { return np == 1 ? 0 : (np == 3 ? 1 : (np == 6 ? 2 
 
 // Flop model of one primitive quartet of total angular momentum L, bra/ket split irrelevant at this
 // granularity: geometry + prefactor, Boys, R recursion, operator stages.
-static double flops_prim(int la, int lb, int lc, int ld)
+double flops_prim(int la, int lb, int lc, int ld)
 {
     const int L = la + lb + lc + ld;
     auto nh = [](int n) { return (n + 1) * (n + 2) * (n + 3) / 6; };
@@ -229,7 +243,7 @@ static double flops_prim(int la, int lb, int lc, int ld)
     int ord = L, blk = 1;
     const int ls[4] = {ld, lc, lb, la};
     for (int s = 0; s < 4; ++s)
-        if (ls[s]) { ord -= 1; fma += 2.0 * 3 * blk * nh(ord) * 0.75; blk *= 3; }
+        for (int k = 0; k < ls[s]; ++k) { ord -= 1; fma += 2.0 * 3 * blk * nh(ord) * 0.75; blk *= 3; }   // d: two operator stages [est.]
     return 2.0 * fma + other;
 }
 
@@ -260,8 +274,8 @@ int create_impl(Handle* h, const rttda_basis_t* basis, const double* C_occ, cons
 
     // ---- candidate pairs and their primitive rows (canonical orientation), per pair class
     std::vector<Pair> pairs;
-    std::vector<double> rows[3];
-    std::vector<int> cand_np[3], cand_off[3], cand_id[3];
+    std::vector<double> rows[NPAIRCLASS];
+    std::vector<int> cand_np[NPAIRCLASS], cand_off[NPAIRCLASS], cand_id[NPAIRCLASS];
     long long npairs_total = 0;
     for (int i = 0; i < H.nshells; ++i)
         for (int j = 0; j <= i; ++j) {
@@ -269,7 +283,7 @@ int create_impl(Handle* h, const rttda_basis_t* basis, const double* C_occ, cons
             int s1 = i, s2 = j;
             if (H.l[s2] > H.l[s1]) std::swap(s1, s2);
             Pair P;
-            P.s1 = s1; P.s2 = s2; P.pc = H.l[s1] + H.l[s2]; P.np = H.np[s1] * H.np[s2];
+            P.s1 = s1; P.s2 = s2; P.pc = pairclass_of(H.l[s1], H.l[s2]); P.np = H.np[s1] * H.np[s2];
             P.np_true = H.np_true[s1] * H.np_true[s2];
             RT_CHECK(P.np == 1 || P.np == 3 || P.np == 9, "unsupported contraction depth");
             P.sub = np_to_sub(P.np);
@@ -290,8 +304,8 @@ int create_impl(Handle* h, const rttda_basis_t* basis, const double* C_occ, cons
         }
 
     // ---- Schwarz bounds on the device
-    std::vector<double> qprim[3];
-    for (int pc = 0; pc < 3; ++pc) {
+    std::vector<double> qprim[NPAIRCLASS];
+    for (int pc = 0; pc < NPAIRCLASS; ++pc) {
         const int n = (int)cand_np[pc].size();
         if (!n) continue;
         DevTmp t_np, t_off, t_prim, t_Q;                         // freed on every return path
@@ -304,7 +318,10 @@ int create_impl(Handle* h, const rttda_basis_t* basis, const double* C_occ, cons
         RT_CUDA(cudaMemcpyAsync(d_np, cand_np[pc].data(), n * sizeof(int), cudaMemcpyHostToDevice, st));
         RT_CUDA(cudaMemcpyAsync(d_off, cand_off[pc].data(), n * sizeof(int), cudaMemcpyHostToDevice, st));
         RT_CUDA(cudaMemcpyAsync(d_prim, rows[pc].data(), rows[pc].size() * sizeof(double), cudaMemcpyHostToDevice, st));
-        RT_TRY(schwarz_device(pc, n, d_np, d_off, d_prim, h->tabs.boys[2 * pc], d_Q, st));
+        // pairs with a d shell take the general path (eri_generic.cu), which needs no Boys table
+        const int pl1 = pairclass_l1(pc), pl2 = pairclass_l2(pc);
+        if (pl1 > 1) RT_TRY(schwarz_general(pl1, pl2, n, d_np, d_off, d_prim, d_Q, st));
+        else RT_TRY(schwarz_device(pc, n, d_np, d_off, d_prim, h->tabs.boys[2 * pc], d_Q, st));
         h->kernel_launches++;
         std::vector<double> Q(n);
         RT_CUDA(cudaMemcpyAsync(Q.data(), d_Q, n * sizeof(double), cudaMemcpyDeviceToHost, st));
@@ -320,7 +337,8 @@ int create_impl(Handle* h, const rttda_basis_t* basis, const double* C_occ, cons
         RT_CUDA(cudaMalloc(&t_Q1.p, nrow * sizeof(double)));
         RT_CUDA(cudaMemcpyAsync(t_np1.p, one.data(), nrow * sizeof(int), cudaMemcpyHostToDevice, st));
         RT_CUDA(cudaMemcpyAsync(t_off1.p, idx.data(), nrow * sizeof(int), cudaMemcpyHostToDevice, st));
-        RT_TRY(schwarz_device(pc, nrow, (int*)t_np1.p, (int*)t_off1.p, d_prim, h->tabs.boys[2 * pc], (double*)t_Q1.p, st));
+        if (pl1 > 1) RT_TRY(schwarz_general(pl1, pl2, nrow, (int*)t_np1.p, (int*)t_off1.p, d_prim, (double*)t_Q1.p, st));
+        else RT_TRY(schwarz_device(pc, nrow, (int*)t_np1.p, (int*)t_off1.p, d_prim, h->tabs.boys[2 * pc], (double*)t_Q1.p, st));
         h->kernel_launches++;
         qprim[pc].resize(nrow);
         RT_CUDA(cudaMemcpyAsync(qprim[pc].data(), t_Q1.p, nrow * sizeof(double), cudaMemcpyDeviceToHost, st));
@@ -479,8 +497,8 @@ int create_impl(Handle* h, const rttda_basis_t* basis, const double* C_occ, cons
             const bool same = (kcb == kck);
             Segment sg{};
             sg.kc_bra = kcb; sg.kc_ket = kck;
-            sg.la = pcb >= 1; sg.lb = pcb == 2; sg.lc = pck >= 1; sg.ld = pck == 2;
-            sg.ni = (2 * sg.la + 1) * (2 * sg.lb + 1) * (2 * sg.lc + 1) * (2 * sg.ld + 1);
+            sg.la = pairclass_l1(pcb); sg.lb = pairclass_l2(pcb); sg.lc = pairclass_l1(pck); sg.ld = pairclass_l2(pck);
+            sg.ni = ncart(sg.la) * ncart(sg.lb) * ncart(sg.lc) * ncart(sg.ld);
             // staging map: pair p owns the 32-ket batches covering kets [same ? p : 0, nk_p)
             std::vector<long long> base(nb, 0);
             long long nbatch = 0, nquart = 0;
@@ -506,11 +524,16 @@ int create_impl(Handle* h, const rttda_basis_t* basis, const double* C_occ, cons
             const int npb = h->tabs.kets[kcb].np;
             // at most 32 bra pairs per block: shallow contractions (1 or 3 primitive pairs) would otherwise give a
             // handful of very long blocks per segment and leave SMs idle
-            const int G = std::min(32, std::min(JK_BLOCK, EVAL_MAX_ROWS / npb));
+            // general path (classes with a d shell, eri_generic.cu): a block is 32 kets x 4 component workers and walks
+            // few bra pairs, so that even a handful of d shells spreads over many blocks (at most ~2e5 blocks per segment)
+            const bool general = segment_is_general(sg);
+            const int kstep = general ? 32 : JK_BLOCK;
+            const int G = general ? (int)std::max<long long>(1, ((long long)nb * ((nk + 31) / 32) + 199999) / 200000)
+                                  : std::min(32, std::min(JK_BLOCK, EVAL_MAX_ROWS / npb));
             std::vector<EvalItem> items;
-            for (int k0 = 0; k0 < nk; k0 += JK_BLOCK) {
+            for (int k0 = 0; k0 < nk; k0 += kstep) {
                 int hi = tau > 0.0 ? count_prod_ge(kcb, hQ[kck][k0]) : nb;     // bra pairs reaching this chunk
-                if (same) hi = std::min(hi, std::min(nb, k0 + JK_BLOCK));
+                if (same) hi = std::min(hi, std::min(nb, k0 + kstep));
                 for (int p0 = 0; p0 < hi; p0 += G) items.push_back(EvalItem{k0, p0, std::min(hi, p0 + G)});
             }
             sg.nitems = (int)items.size();
@@ -518,6 +541,7 @@ int create_impl(Handle* h, const rttda_basis_t* basis, const double* C_occ, cons
             // digestion launches: ordered bra classes (a-lists) of this bra pair class against the ket class
             sg.first_launch = (int)h->launches.size();
             for (int orient = 0; orient < 2; ++orient) {
+                if (segment_is_general(sg)) break;                 // classes with a d shell: one kernel digests the whole segment
                 if (orient == 1 && sg.la == sg.lb) break;          // ss and pp pairs: one ordered class
                 const int la = orient == 0 ? sg.la : sg.lb, lb = orient == 0 ? sg.lb : sg.la;
                 std::vector<std::pair<double, WorkItem>> witems;
@@ -557,20 +581,20 @@ int create_impl(Handle* h, const rttda_basis_t* basis, const double* C_occ, cons
         for (int kc1 = 0; kc1 < NKETCLASS; ++kc1)
             for (int k : cls[kc1]) {
                 const Pair& P = pairs[k];
-                const int l1 = P.pc >= 1, l2 = P.pc == 2;
+                const int l1 = pairclass_l1(P.pc), l2 = pairclass_l2(P.pc);
                 for (int kc2 = 0; kc2 < NKETCLASS; ++kc2) {
                     const int n2 = tau > 0.0 ? count_prod_ge(kc2, P.Q) : h->tabs.kets[kc2].n;
-                    const int pc2 = kc2 / NSUB, l3 = pc2 >= 1, l4 = pc2 == 2;
+                    const int pc2 = kc2 / NSUB, l3 = pairclass_l1(pc2), l4 = pairclass_l2(pc2);
                     const double npq = (double)P.np_true * pre[kc2][n2];       // primitive quartets of these n2 quartets
                     ordered += n2;
                     ordered_prim += npq;
                     fl_ord += npq * flops_prim(l1, l2, l3, l4);
-                    nint_ord += (double)n2 * (2 * l1 + 1) * (2 * l2 + 1) * (2 * l3 + 1) * (2 * l4 + 1);
+                    nint_ord += (double)n2 * ncart(l1) * ncart(l2) * ncart(l3) * ncart(l4);
                 }
                 if (P.Q * P.Q >= tau) {
                     diag += 1; diag_prim += (double)P.np_true * P.np_true;
                     fl_diag += (double)P.np_true * P.np_true * flops_prim(l1, l2, l1, l2);
-                    nint_diag += (double)(2 * l1 + 1) * (2 * l2 + 1) * (2 * l1 + 1) * (2 * l2 + 1);
+                    nint_diag += (double)ncart(l1) * ncart(l2) * ncart(l1) * ncart(l2);
                 }
             }
         h->info[RTTDA_INFO_NQUARTETS] = 0.5 * (ordered + diag);

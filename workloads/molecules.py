@@ -63,6 +63,7 @@ class Config:
     nsteps: int
     fields: tuple = field(default_factory=tuple)   # tuple of dicts, one per trajectory
     k: int = 0               # 1-based config number (seed offset)
+    bump: int = 0            # default re-draw index of make_basis / make_mos (R18: a draw with a too ill-conditioned S is re-drawn)
 
     @property
     def ncenters(self) -> int:
@@ -93,7 +94,7 @@ CONFIGS = {
     5: Config("sigma-microbench", 120, 100, _HEAVY9, _H2, 400, 880, 1e-12, 0.0, 0, (), 4),
     # not a BASELINE.json config: the small d-shell molecule of the NEXT-4 tests (4 heavy centres + 2 H-like, 60 AOs)
     6: Config("tiny-d", 4, 2, _SPD14, _H2, 10, 50, 1e-12, 0.05, 10,
-              ({"type": "cw", "E0": 0.01, "omega": 0.3, "dir": (0.0, 0.0, 1.0)},), 6),
+              ({"type": "cw", "E0": 0.01, "omega": 0.3, "dir": (0.0, 0.0, 1.0)},), 6, 2),   # draw 2: cond(S) = 144
 }
 
 
@@ -116,8 +117,9 @@ def _place_centers(rng: np.random.Generator, n: int, L: float, dmin: float = 1.8
     return pts
 
 
-def make_basis(cfg: Config, bump: int = 0) -> Basis:
+def make_basis(cfg: Config, bump: int | None = None) -> Basis:
     """Centres, shell table, exponents and coefficients of config `cfg` (seed stream 0)."""
+    bump = cfg.bump if bump is None else bump
     rng = _rng(cfg.k, 0, bump)
     n = cfg.ncenters
     centers = _place_centers(rng, n, cfg.box)
@@ -151,7 +153,7 @@ def orthonormalizer(S: np.ndarray):
     return (U / np.sqrt(w)) @ U.T, float(w[-1] / w[0])
 
 
-def make_mos(cfg: Config, S: np.ndarray, bump: int = 0):
+def make_mos(cfg: Config, S: np.ndarray, bump: int | None = None):
     """Synthetic MOs C = S^-1/2 Q (seed stream 1) and orbital energies (seed stream 2).
 
     Returns (C_occ [N][nocc], C_virt [N][nvirt], eps [nocc+nvirt], cond(S)).  The caller rejects
@@ -159,6 +161,7 @@ def make_mos(cfg: Config, S: np.ndarray, bump: int = 0):
     """
     N = S.shape[0]
     assert N == cfg.nocc + cfg.nvirt
+    bump = cfg.bump if bump is None else bump
     X, cond = orthonormalizer(S)
     g = _rng(cfg.k, 1, bump).standard_normal((N, N))
     Q, R = np.linalg.qr(g)
