@@ -187,3 +187,20 @@ def test_random_molecules_with_contracted_d_shells(seed):
         assert rel_inf(_fock(h, T), 2 * J - K) < 1e-12
         assert int(h.rttda_get_info("nquartets")) == nq and int(h.rttda_get_info("nprim_quartets")) == npq
         h.close()
+
+
+def test_d320_sigma_vs_matrix_free_oracle():
+    """320 basis functions with d shells (the size of the paper's smallest Table-3 molecule; workloads key 7):
+    sigma for two vectors against the oracle's matrix-free route (screened at 1e-16), 13.9 M unique shell quartets in
+    every class from (ss|ss) to (dd|dd), several evaluation blocks and ragged 32-ket batches per class."""
+    from workloads import make_vectors
+    from oracle import tda
+    ctx = setup_config(7, tau=1e-14)
+    assert ctx["basis"].nao == 320
+    X = make_vectors(ctx["cfg"], 2)
+    ref, nq, _ = tda.sigma_matrix_free(ctx["ob"], X, ctx["C_o"], ctx["C_v"], ctx["eps"], 1.0, tau=1e-16)
+    got = gpu_sigma(ctx, X)
+    err = rel_inf(got, ref)
+    print("d-320: sigma rel err %.2e (%d oracle quartets)" % (err, nq))
+    assert err < SIGMA_TOL
+    assert abs(X[0] @ got[1] - X[1] @ got[0]) < 1e-11                 # A is symmetric

@@ -95,6 +95,10 @@ CONFIGS = {
     # not a BASELINE.json config: the small d-shell molecule of the NEXT-4 tests (4 heavy centres + 2 H-like, 60 AOs)
     6: Config("tiny-d", 4, 2, _SPD14, _H2, 10, 50, 1e-12, 0.05, 10,
               ({"type": "cw", "E0": 0.01, "omega": 0.3, "dir": (0.0, 0.0, 1.0)},), 6, 2),   # draw 2: cond(S) = 144
+    # 320 basis functions with d shells: the size of the paper's smallest Table-3 molecule (320 BF, 6-31G*),
+    # 20 heavy centres (14 AOs) + 20 H-like (2 AOs); measurement and parity case of the d-shell path
+    7: Config("d-320", 20, 20, _SPD14, _H2, 60, 260, 1e-12, 0.05, 100,
+              ({"type": "cw", "E0": 0.01, "omega": 0.3, "dir": (0.0, 0.0, 1.0)},), 7, 1),       # draw 1: cond(S) = 1.9e3
 }
 
 
