@@ -41,10 +41,12 @@ extern "C" {
 
 typedef struct rttda_handle_s* rttda_handle_t;   /* opaque; owns all internal device memory */
 
-/* One contracted Cartesian Gaussian shell: l = 0 (s) or 1 (p: components x, y, z).  AO order = shell order. */
+/* One contracted Cartesian Gaussian shell: l = 0 (s), 1 (p: components x, y, z) or 2 (d: the six Cartesian components
+ * xx, xy, xz, yy, yz, zz, each normalised to <phi|phi> = 1, "6-31G*").  AO order = shell
+ * order, so nao = sum over shells of (l+1)(l+2)/2.  Classes with a d shell run on a general (slower) kernel path. */
 typedef struct {
     int32_t center;     /* index into centers */
-    int32_t l;          /* 0 or 1 */
+    int32_t l;          /* 0, 1 or 2 */
     int32_t nprim;      /* 1..RTTDA_MAX_NPRIM */
     int32_t prim_off;   /* offset of this shell's primitives in exps / coefs */
 } rttda_shell_t;
