@@ -322,10 +322,49 @@ struct GenDigestArgs {
     int same, nvt, nvec, nao, la, lb, lc, ld, do_j, do_k;
 };
 
-// block = one stored batch (bra pair x 32 kets), lane = ket, the warps share the batch's components; every stored value
-// goes through the eight index images (mn|ls) (nm|ls) (mn|sl) (nm|sl) (ls|mn) (sl|mn) (ls|nm) (sl|nm):
-//   F[i0][i1] += 2 I T[i2][i3]  (Coulomb),  F[i0][i2] -= cx I T[i1][i3]  (exchange),
-// I carrying 1/2 per coincidence (a == b, c == d, ab == cd) - the last two are folded into the stored value.
+// block = one stored batch (bra pair (m n) x 32 kets (l s)), lane = ket, GEN_DV densities per sweep.  Every stored value I
+// stands for its eight index images (mn|ls) (nm|ls) (mn|sl) (nm|sl) (ls|mn) (sl|mn) (ls|nm) (sl|nm), with 1/2 per
+// coincidence (a == b here; c == d and ab == cd are folded into the stored value):
+//   Coulomb   F[mn], F[nm] += 2 sum_{ls} I (T_ls + T_sl)        F[ls], F[sl] += 2 sum_{mn} I (T_mn + T_nm)
+//   exchange  F[ml] -= cx sum_{ns} I T_ns   F[lm] -= cx sum I T_sn     F[nl] -= cx sum_{ms} I T_ms   F[ln] -= cx sum I T_sm
+//             F[ms] -= cx sum_{nl} I T_nl   F[sm] -= cx sum I T_ln     F[ns] -= cx sum_{ml} I T_ml   F[sn] -= cx sum I T_lm
+// Each line is one sweep over the batch: the warps split the OUTPUT index pair, a lane sums over the other two indices
+// in registers and issues one atomic per output element and density (the F[mn] sums go through a warp reduction first).
+constexpr int GEN_DV = 4;
+template <bool OUT_A, bool OUT_C>
+__device__ __forceinline__ void gen_exchange_sweep(const GenDigestArgs& g, const double* __restrict__ src, int NA, int NB, int NC,
+                                                   int ND, int aoA, int aoB, int aoC, int aoD, double scale, int v0, int nv,
+                                                   int warp, int nwarp, bool live)
+{
+    // output pair (o1, o2): o1 from the bra (a if OUT_A else b), o2 from the ket (c if OUT_C else d); summed pair (r1, r2)
+    const int NO1 = OUT_A ? NA : NB, NO2 = OUT_C ? NC : ND, NR1 = OUT_A ? NB : NA, NR2 = OUT_C ? ND : NC;
+    const int aoO1 = OUT_A ? aoA : aoB, aoO2 = OUT_C ? aoC : aoD, aoR1 = OUT_A ? aoB : aoA, aoR2 = OUT_C ? aoD : aoC;
+    const size_t nvt = g.nvt, rs = (size_t)g.nao * nvt;
+    for (int o = warp; o < NO1 * NO2; o += nwarp) {
+        const int o1 = o % NO1, o2 = o / NO1;
+        double acc1[GEN_DV], acc2[GEN_DV];
+        for (int v = 0; v < GEN_DV; ++v) acc1[v] = acc2[v] = 0.0;
+        for (int r2 = 0; r2 < NR2; ++r2)
+            for (int r1 = 0; r1 < NR1; ++r1) {
+                const int a = OUT_A ? o1 : r1, b = OUT_A ? r1 : o1, c = OUT_C ? o2 : r2, d = OUT_C ? r2 : o2;
+                const double x = src[(size_t)(((d * NC + c) * NB + b) * NA + a) * 32];
+                const double* T12 = g.Tq + (size_t)(aoR1 + r1) * rs + (size_t)(aoR2 + r2) * nvt + v0;
+                const double* T21 = g.Tq + (size_t)(aoR2 + r2) * rs + (size_t)(aoR1 + r1) * nvt + v0;
+                for (int v = 0; v < GEN_DV; ++v)
+                    if (v < nv) { acc1[v] = fma(x, T12[v], acc1[v]); acc2[v] = fma(x, T21[v], acc2[v]); }
+            }
+        if (live) {
+            double* F12 = g.Fq + (size_t)(aoO1 + o1) * rs + (size_t)(aoO2 + o2) * nvt + v0;
+            double* F21 = g.Fq + (size_t)(aoO2 + o2) * rs + (size_t)(aoO1 + o1) * nvt + v0;
+            for (int v = 0; v < GEN_DV; ++v)
+                if (v < nv) {
+                    if (acc1[v] != 0.0) atomicAdd(F12 + v, scale * acc1[v]);
+                    if (acc2[v] != 0.0) atomicAdd(F21 + v, scale * acc2[v]);
+                }
+        }
+    }
+}
+
 __global__ void __launch_bounds__(128) digest_generic_kernel(GenDigestArgs g)
 {
     const long long batch = blockIdx.x;
@@ -339,30 +378,71 @@ __global__ void __launch_bounds__(128) digest_generic_kernel(GenDigestArgs g)
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarp = blockDim.x >> 5;
     const long long kbi = batch - g.batch_base[p] + (g.same ? (p >> 5) : 0);
     const long long q = kbi * 32 + lane;
-    if (q >= g.ket.n) return;
+    const bool live = q < g.ket.n;                         // lanes beyond the ket list hold zeros; they only help to reduce
+    const long long qq = live ? q : g.ket.n - 1;
     const int NA = gen_ncart(g.la), NB = gen_ncart(g.lb), NC = gen_ncart(g.lc), ND = gen_ncart(g.ld);
-    const int NI = NA * NB * NC * ND;
-    const int aoA = g.bra.ao_c[p], aoB = g.bra.ao_d[p], aoC = g.ket.ao_c[q], aoD = g.ket.ao_d[q];
+    const int NAB = NA * NB, NCD = NC * ND, NI = NAB * NCD;
+    const int aoA = g.bra.ao_c[p], aoB = g.bra.ao_d[p], aoC = g.ket.ao_c[qq], aoD = g.ket.ao_d[qq];
     const double wab = g.bra.same[p] ? 0.5 : 1.0;
     const size_t nvt = g.nvt, rs = (size_t)g.nao * nvt;
     const double* src = g.buf + (size_t)batch * ((size_t)NI * 32) + lane;
-    for (int i = warp; i < NI; i += nwarp) {
-        const double x = wab * src[(size_t)i * 32];
-        if (x == 0.0) continue;
-        const int a = i % NA, b = (i / NA) % NB, c = (i / (NA * NB)) % NC, d = i / (NA * NB * NC);
-        const int m = aoA + a, n = aoB + b, l = aoC + c, s = aoD + d;
-        const int im[8][4] = {{m, n, l, s}, {n, m, l, s}, {m, n, s, l}, {n, m, s, l},
-                              {l, s, m, n}, {s, l, m, n}, {l, s, n, m}, {s, l, n, m}};
-        for (int k = 0; k < 8; ++k) {
-            const int i0 = im[k][0], i1 = im[k][1], i2 = im[k][2], i3 = im[k][3];
-            const double* Tj = g.Tq + (size_t)i2 * rs + (size_t)i3 * nvt;
-            const double* Tk = g.Tq + (size_t)i1 * rs + (size_t)i3 * nvt;
-            double* Fj = g.Fq + (size_t)i0 * rs + (size_t)i1 * nvt;
-            double* Fk = g.Fq + (size_t)i0 * rs + (size_t)i2 * nvt;
-            for (int v = 0; v < g.nvec; ++v) {
-                if (g.do_j) atomicAdd(Fj + v, 2.0 * x * Tj[v]);
-                if (g.do_k) atomicAdd(Fk + v, -g.cx * x * Tk[v]);
+    for (int v0 = 0; v0 < g.nvec; v0 += GEN_DV) {
+        const int nv = min(GEN_DV, g.nvec - v0);
+        if (g.do_j) {
+            // F[mn], F[nm] += 2 w sum_{ls} I (T_ls + T_sl), summed over the kets of the batch by a warp reduction
+            for (int ab = warp; ab < NAB; ab += nwarp) {
+                double acc[GEN_DV];
+                for (int v = 0; v < GEN_DV; ++v) acc[v] = 0.0;
+                for (int cd = 0; cd < NCD; ++cd) {
+                    const int c = cd % NC, d = cd / NC;
+                    const double x = src[(size_t)(cd * NAB + ab) * 32];
+                    const double* Tls = g.Tq + (size_t)(aoC + c) * rs + (size_t)(aoD + d) * nvt + v0;
+                    const double* Tsl = g.Tq + (size_t)(aoD + d) * rs + (size_t)(aoC + c) * nvt + v0;
+                    for (int v = 0; v < GEN_DV; ++v)
+                        if (v < nv) acc[v] = fma(x, Tls[v] + Tsl[v], acc[v]);
+                }
+                for (int v = 0; v < GEN_DV; ++v)
+                    for (int o = 16; o > 0; o >>= 1) acc[v] += __shfl_xor_sync(0xffffffffu, acc[v], o);
+                if (lane == 0) {
+                    const int a = ab % NA, b = ab / NA;
+                    double* Fmn = g.Fq + (size_t)(aoA + a) * rs + (size_t)(aoB + b) * nvt + v0;
+                    double* Fnm = g.Fq + (size_t)(aoB + b) * rs + (size_t)(aoA + a) * nvt + v0;
+                    for (int v = 0; v < nv; ++v) {
+                        atomicAdd(Fmn + v, 2.0 * wab * acc[v]);
+                        atomicAdd(Fnm + v, 2.0 * wab * acc[v]);
+                    }
+                }
             }
+            // F[ls], F[sl] += 2 w sum_{mn} I (T_mn + T_nm)
+            for (int cd = warp; cd < NCD; cd += nwarp) {
+                const int c = cd % NC, d = cd / NC;
+                double acc[GEN_DV];
+                for (int v = 0; v < GEN_DV; ++v) acc[v] = 0.0;
+                for (int ab = 0; ab < NAB; ++ab) {
+                    const int a = ab % NA, b = ab / NA;
+                    const double x = src[(size_t)(cd * NAB + ab) * 32];
+                    const double* Tmn = g.Tq + (size_t)(aoA + a) * rs + (size_t)(aoB + b) * nvt + v0;
+                    const double* Tnm = g.Tq + (size_t)(aoB + b) * rs + (size_t)(aoA + a) * nvt + v0;
+                    for (int v = 0; v < GEN_DV; ++v)
+                        if (v < nv) acc[v] = fma(x, Tmn[v] + Tnm[v], acc[v]);
+                }
+                if (live) {
+                    double* Fls = g.Fq + (size_t)(aoC + c) * rs + (size_t)(aoD + d) * nvt + v0;
+                    double* Fsl = g.Fq + (size_t)(aoD + d) * rs + (size_t)(aoC + c) * nvt + v0;
+                    for (int v = 0; v < nv; ++v)
+                        if (acc[v] != 0.0) {
+                            atomicAdd(Fls + v, 2.0 * wab * acc[v]);
+                            atomicAdd(Fsl + v, 2.0 * wab * acc[v]);
+                        }
+                }
+            }
+        }
+        if (g.do_k) {
+            const double sc = -g.cx * wab;
+            gen_exchange_sweep<true, true>(g, src, NA, NB, NC, ND, aoA, aoB, aoC, aoD, sc, v0, nv, warp, nwarp, live);
+            gen_exchange_sweep<false, true>(g, src, NA, NB, NC, ND, aoA, aoB, aoC, aoD, sc, v0, nv, warp, nwarp, live);
+            gen_exchange_sweep<true, false>(g, src, NA, NB, NC, ND, aoA, aoB, aoC, aoD, sc, v0, nv, warp, nwarp, live);
+            gen_exchange_sweep<false, false>(g, src, NA, NB, NC, ND, aoA, aoB, aoC, aoD, sc, v0, nv, warp, nwarp, live);
         }
     }
 }
