@@ -130,7 +130,7 @@ struct JKTables {
     const BraRec* recs;
     const BraRec* jrecs;      // the canonical records of every a-list, in the same order
     const AList* alists;
-    const double2* boys[5];   // per total angular momentum L: rows {F_{L+k}(j/8)/k!, k < 8; exp(-j/8); pad}
+    const double2* boys[9];   // per total angular momentum L (0..8): rows {F_{L+k}(j/8)/k!, k < 8; exp(-j/8); pad}
     double tau;
     int nao;
 };
@@ -237,8 +237,8 @@ bool segment_is_general(const Segment& sg);
 int eval_segment_general(Handle* h, const Segment& sg, double* buf, cudaStream_t st);
 int digest_segment_general(Handle* h, const Segment& sg, const double* buf, int nvt, int nvec, const double* Tq, double* Fq,
                            cudaStream_t st);
-int schwarz_general(int la, int lb, int npairs, const int* d_np, const int* d_off, const double* d_prim, double* d_Q,
-                    cudaStream_t st);
+int schwarz_general(int la, int lb, int npairs, const int* d_np, const int* d_off, const double* d_prim,
+                    const double2* d_boys /* table for L = 2 (la + lb) */, double* d_Q, cudaStream_t st);
 // evaluate + digest one segment (fast or general path)
 int digest_segment(Handle* h, const Segment& sg, const double* buf, int nvt, int nvec, const double* Tq, double* Fq,
                    cudaStream_t st);

@@ -45,26 +45,33 @@ __device__ __forceinline__ double gen_norm(int l, int c)
     return (l == 2 && (c == 1 || c == 2 || c == 4)) ? 1.7320508075688772935 : 1.0;
 }
 
-// Boys function F_0..F_L(T).  T < 35: the all-positive series of F_L, then the (stable) downward recursion;
-// T >= 35: F_0 = sqrt(pi/T)/2 (erfc(sqrt 35) = 6e-17) and the upward recursion with its e^-T term.
-__device__ void gen_boys(int L, double T, double* F)
+// Boys function F_0..F_L(T).  T < 36: F_L from the table row of the nearest grid point T0 = j/8 ({F_{L+k}(T0)/k!, k < 8;
+// e^-T0}, built in long double by setup.cu: F_L(T) = sum_k h_k (T0 - T)^k since dF_n/dT = -F_{n+1}), then the stable
+// downward recursion F_{n-1} = (2T F_n + e^-T)/(2n - 1) with e^-T = e^-T0 e^(T0 - T) by its Taylor series;
+// T >= 36: F_0 = sqrt(pi/T)/2 (erfc(6) = 2e-17) and the upward recursion, stable there, with its e^-T term.
+__device__ void gen_boys(int L, double T, const double2* __restrict__ tab, double* F)
 {
-    if (T < 35.0) {
-        double term = 1.0 / (2 * L + 1), sum = term;
-        for (int k = 1; k < 400; ++k) {
-            term *= 2.0 * T / (2 * L + 2 * k + 1);
-            sum += term;
-            if (term < 1e-17 * sum) break;
-        }
-        const double emt = exp(-T);
-        double f = emt * sum;
+    if (T < BOYS_TMAX) {
+        constexpr double MAGIC = 6755399441055744.0;      // 1.5 * 2^52: rounds to nearest integer
+        const double t = fma(T, 8.0, MAGIC);
+        const int j = __double2loint(t);
+        const double dx = fma(t - MAGIC, 0.125, -T);      // T0 - T, |dx| <= 1/16
+        const double2* row = tab + j * (BOYS_ROW / 2);
+        const double2 h01 = row[0], h23 = row[1], h45 = row[2], h67 = row[3];
+        double f = h67.y;
+        f = fma(f, dx, h67.x); f = fma(f, dx, h45.y); f = fma(f, dx, h45.x); f = fma(f, dx, h23.y);
+        f = fma(f, dx, h23.x); f = fma(f, dx, h01.y); f = fma(f, dx, h01.x);
         F[L] = f;
-        for (int n = L; n >= 1; --n) { f = (2.0 * T * f + emt) / (2 * n - 1); F[n - 1] = f; }
+        double e = 1.0 / 40320.0;
+        e = fma(e, dx, 1.0 / 5040.0); e = fma(e, dx, 1.0 / 720.0); e = fma(e, dx, 1.0 / 120.0); e = fma(e, dx, 1.0 / 24.0);
+        e = fma(e, dx, 1.0 / 6.0); e = fma(e, dx, 0.5); e = fma(e, dx, 1.0); e = fma(e, dx, 1.0);
+        e *= row[4].x;
+        for (int n = L; n >= 1; --n) { f = fma(2.0 * T, f, e) / (2 * n - 1); F[n - 1] = f; }
     } else {
-        const double emt = exp(-T);
+        const double emt = exp(-T), r = 0.5 / T;
         double f = 0.5 * sqrt(3.14159265358979323846 / T);
         F[0] = f;
-        for (int n = 0; n < L; ++n) { f = ((2 * n + 1) * f - emt) / (2.0 * T); F[n + 1] = f; }
+        for (int n = 0; n < L; ++n) { f = ((2 * n + 1) * f - emt) * r; F[n + 1] = f; }
     }
 }
 
@@ -74,9 +81,9 @@ typedef double ETable[3][GEN_LMAX + 1][GEN_LMAX + 1][2 * GEN_LMAX + 1];
 __device__ void gen_build_E(int li, int lj, double h, const double* XA, const double* XB, ETable& E)
 {
     for (int x = 0; x < 3; ++x) {
-        for (int i = 0; i <= GEN_LMAX; ++i)
-            for (int j = 0; j <= GEN_LMAX; ++j)
-                for (int t = 0; t <= 2 * GEN_LMAX; ++t) E[x][i][j][t] = 0.0;
+        for (int i = 0; i <= li; ++i)
+            for (int j = 0; j <= lj; ++j)
+                for (int t = 0; t <= li + lj; ++t) E[x][i][j][t] = 0.0;
         E[x][0][0][0] = 1.0;
         for (int i = 0; i < li; ++i)
             for (int t = 0; t <= i + 1; ++t) {
@@ -99,10 +106,11 @@ __device__ void gen_build_E(int li, int lj, double h, const double* XA, const do
 // R^0_{tuv}, t+u+v <= L, times `pref`; two ping-pong tables, level n built from level n+1:
 //   R^n_{t+1,u,v} = t R^{n+1}_{t-1,u,v} + X R^{n+1}_{t,u,v}   (u with Y, v with Z alike)
 // Returns the table that holds level 0.
-__device__ double* gen_build_R(int L, double pref, double alpha, double X, double Y, double Z, double* Ra, double* Rb)
+__device__ double* gen_build_R(int L, double pref, double alpha, double X, double Y, double Z, const double2* __restrict__ tab,
+                               double* Ra, double* Rb)
 {
     double F[4 * GEN_LMAX + 1];
-    gen_boys(L, alpha * (X * X + Y * Y + Z * Z), F);
+    gen_boys(L, alpha * (X * X + Y * Y + Z * Z), tab, F);
     double sc = pref;
     for (int n = 0; n <= L; ++n) { F[n] *= sc; sc *= -2.0 * alpha; }
     for (int n = L; n >= 0; --n) {
@@ -146,7 +154,8 @@ __device__ __forceinline__ GenPrim gen_load_soa(const double* __restrict__ prim,
 // The Hermite table of one primitive quartet: R (level 0) for total order L with the prefactor c_b c_k / sqrt(p+q)
 // (times theta for the operator erf(omega r12)/r12, whose integrals are those of 1/r12 at alpha theta^2,
 // theta^2 = omega^2 / (alpha + omega^2)).
-__device__ double* gen_quartet_R(int L, const GenPrim& b, const GenPrim& k, double omega2, double* Ra, double* Rb)
+__device__ double* gen_quartet_R(int L, const GenPrim& b, const GenPrim& k, double omega2, const double2* __restrict__ tab,
+                                 double* Ra, double* Rb)
 {
     const double pq = b.p + k.p;
     double alpha = b.p * k.p / pq;
@@ -156,7 +165,7 @@ __device__ double* gen_quartet_R(int L, const GenPrim& b, const GenPrim& k, doub
         pref *= sqrt(th2);
         alpha *= th2;
     }
-    return gen_build_R(L, pref, alpha, b.P[0] - k.P[0], b.P[1] - k.P[1], b.P[2] - k.P[2], Ra, Rb);
+    return gen_build_R(L, pref, alpha, b.P[0] - k.P[0], b.P[1] - k.P[1], b.P[2] - k.P[2], tab, Ra, Rb);
 }
 
 // G[tuv] = sum_{t'u'v'} (-1)^{t'+u'+v'} E^{cd}_{t'u'v'} R_{t+t',u+u',v+v'} for all bra Hermite components of order <= LB
@@ -200,6 +209,7 @@ struct GenEvalArgs {
     const EvalItem* items;
     KetClass bra, ket;
     const long long* batch_base;
+    const double2* boys;                 // table of the segment's total angular momentum
     double* buf;
     double tau, omega2;
     unsigned long long* primcount;
@@ -218,8 +228,8 @@ __global__ void __launch_bounds__(32 * GEN_WORKERS) eval_generic_kernel(GenEvalA
     const int la = g.la, lb = g.lb, lc = g.lc, ld = g.ld;
     const int NA = gen_ncart(la), NB = gen_ncart(lb), NC = gen_ncart(lc), ND = gen_ncart(ld);
     const int NI = NA * NB * NC * ND, L = la + lb + lc + ld, LB = la + lb;
-    const int lane = threadIdx.x & 31, worker = threadIdx.x >> 5;
-    const bool split_ket = NC * ND >= GEN_WORKERS;
+    const int lane = threadIdx.x & 31, worker = threadIdx.x >> 5, nworker = blockDim.x >> 5;
+    const bool split_ket = NC * ND >= nworker;
     const int q = it.k0 + lane;
     const bool active = q < g.ket.n;
     const int qq = active ? q : g.ket.n - 1;
@@ -227,38 +237,48 @@ __global__ void __launch_bounds__(32 * GEN_WORKERS) eval_generic_kernel(GenEvalA
     const double wcd = g.ket.same[qq] ? 0.5 : 1.0;
     const int npb = g.bra.np, npk = g.ket.np;
     double Ra[GEN_NHERM], Rb[GEN_NHERM], G[GEN_NHB];
-    ETable Eb, Ek;
+    ETable Ek;
+    // the bra pair is block-uniform: its primitives and their Hermite E tables are built once per pair in shared memory
+    __shared__ ETable s_Eb[9];
+    __shared__ GenPrim s_bp[9];
     unsigned long long nprim_done = 0;
 
     for (int p = it.p_begin; p < it.p_end; ++p) {
         const double Qp = g.bra.Q[p];
         const bool ok = active && (Qp * Qq >= g.tau) && (!g.same || p <= q);
-        if (!__any_sync(0xffffffffu, ok)) break;           // both conditions only get worse along the bra list
+        if (!__any_sync(0xffffffffu, ok)) break;           // both conditions only get worse along the bra list; the warps
+                                                           // of a block hold the same kets, so the exit is block-uniform
+        __syncthreads();                                   // everyone is done with the previous pair's tables
+        if (threadIdx.x < npb) {
+            const GenPrim bp = gen_load_aos(g.bra.prim_aos + ((size_t)p * npb + threadIdx.x) * PRIM_STRIDE);
+            s_bp[threadIdx.x] = bp;
+            gen_build_E(la, lb, bp.h, bp.XA, bp.XB, s_Eb[threadIdx.x]);
+        }
+        __syncthreads();
         const long long batch = g.batch_base[p] + (q >> 5) - (g.same ? (p >> 5) : 0);
         double* dst = g.buf + (size_t)batch * ((size_t)NI * 32) + lane;
         if (!ok) {                                         // the batch exists: lanes without a quartet store zeros
-            for (int i = worker; i < NI; i += GEN_WORKERS) dst[(size_t)i * 32] = 0.0;
+            for (int i = worker; i < NI; i += nworker) dst[(size_t)i * 32] = 0.0;
             continue;
         }
         const double w = (g.same && p == q) ? 0.5 * wcd : wcd;
         bool first = true;
-        for (int kb = 0; kb < npb; ++kb) {
-            const GenPrim bp = gen_load_aos(g.bra.prim_aos + ((size_t)p * npb + kb) * PRIM_STRIDE);
-            gen_build_E(la, lb, bp.h, bp.XA, bp.XB, Eb);
-            for (int kk = 0; kk < npk; ++kk) {
-                const GenPrim kp = gen_load_soa(g.ket.prim, g.ket.n, kk, qq);
-                gen_build_E(lc, ld, kp.h, kp.XA, kp.XB, Ek);
-                const double* R = gen_quartet_R(L, bp, kp, g.omega2, Ra, Rb);
+        for (int kk = 0; kk < npk; ++kk) {
+            const GenPrim kp = gen_load_soa(g.ket.prim, g.ket.n, kk, qq);
+            gen_build_E(lc, ld, kp.h, kp.XA, kp.XB, Ek);
+            for (int kb = 0; kb < npb; ++kb) {
+                const double* R = gen_quartet_R(L, s_bp[kb], kp, g.omega2, g.boys, Ra, Rb);
+                const ETable& Eb = s_Eb[kb];
                 if (worker == 0) ++nprim_done;
                 for (int cd = 0; cd < NC * ND; ++cd) {
-                    if (split_ket && cd % GEN_WORKERS != worker) continue;
+                    if (split_ket && cd % nworker != worker) continue;
                     const int c = cd % NC, d = cd / NC;
                     int pc[3], pd[3];
                     gen_pow(lc, c, pc); gen_pow(ld, d, pd);
                     gen_contract_ket(LB, Ek, pc, pd, R, G);
                     const double ncd = w * gen_norm(lc, c) * gen_norm(ld, d);
                     for (int ab = 0; ab < NA * NB; ++ab) {
-                        if (!split_ket && ab % GEN_WORKERS != worker) continue;
+                        if (!split_ket && ab % nworker != worker) continue;
                         const int a = ab % NA, b = ab / NA;
                         int pa[3], pb[3];
                         gen_pow(la, a, pa); gen_pow(lb, b, pb);
@@ -280,7 +300,7 @@ __global__ void __launch_bounds__(32 * GEN_WORKERS) eval_generic_kernel(GenEvalA
 
 // Schwarz bounds of pairs with a d shell: Q = sqrt(max_{components} (ab|ab)), thread = pair.
 __global__ void schwarz_generic_kernel(int la, int lb, int npairs, const int* __restrict__ np, const int* __restrict__ off,
-                                       const double* __restrict__ prim, double* __restrict__ Q)
+                                       const double* __restrict__ prim, const double2* __restrict__ boys, double* __restrict__ Q)
 {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= npairs) return;
@@ -295,7 +315,7 @@ __global__ void schwarz_generic_kernel(int la, int lb, int npairs, const int* __
         for (int k2 = 0; k2 < n; ++k2) {
             const GenPrim kp = gen_load_aos(prim + (size_t)(o + k2) * PRIM_STRIDE);
             gen_build_E(la, lb, kp.h, kp.XA, kp.XB, Ek);
-            const double* R = gen_quartet_R(2 * LB, bp, kp, 0.0, Ra, Rb);
+            const double* R = gen_quartet_R(2 * LB, bp, kp, 0.0, boys, Ra, Rb);
             for (int b = 0; b < NB; ++b)
                 for (int a = 0; a < NA; ++a) {
                     int pa[3], pb[3];
@@ -458,6 +478,7 @@ int eval_segment_general(Handle* h, const Segment& sg, double* buf, cudaStream_t
     g.bra = h->tabs.kets[sg.kc_bra];
     g.ket = h->tabs.kets[sg.kc_ket];
     g.batch_base = sg.batch_base;
+    g.boys = h->tabs.boys[sg.la + sg.lb + sg.lc + sg.ld];
     g.buf = buf;
     g.tau = h->tabs.tau;
     g.omega2 = h->pass_w_extra > 0.0 ? 36.0 / h->pass_w_extra : 0.0;     // pass_w_extra = 36 / omega^2 (jk_build)
@@ -465,7 +486,9 @@ int eval_segment_general(Handle* h, const Segment& sg, double* buf, cudaStream_t
     g.flops_per_prim = (unsigned long long)flops_prim(sg.la, sg.lb, sg.lc, sg.ld);
     g.same = (sg.kc_bra == sg.kc_ket);
     g.la = sg.la; g.lb = sg.lb; g.lc = sg.lc; g.ld = sg.ld;
-    eval_generic_kernel<<<dim3(sg.nitems), dim3(32 * GEN_WORKERS), 0, st>>>(g);
+    // few components per quartet: the Hermite tables every worker builds for itself would dominate - fewer workers
+    const int workers = sg.ni >= 100 ? GEN_WORKERS : (sg.ni >= 36 ? 2 : 1);
+    eval_generic_kernel<<<dim3(sg.nitems), dim3(32 * workers), 0, st>>>(g);
     h->kernel_launches++;
     RT_CUDA(cudaGetLastError());
     return RTTDA_OK;
@@ -494,11 +517,11 @@ int digest_segment_general(Handle* h, const Segment& sg, const double* buf, int 
     return RTTDA_OK;
 }
 
-int schwarz_general(int la, int lb, int npairs, const int* d_np, const int* d_off, const double* d_prim, double* d_Q,
-                    cudaStream_t st)
+int schwarz_general(int la, int lb, int npairs, const int* d_np, const int* d_off, const double* d_prim,
+                    const double2* d_boys, double* d_Q, cudaStream_t st)
 {
     if (npairs == 0) return RTTDA_OK;
-    schwarz_generic_kernel<<<dim3((npairs + 63) / 64), dim3(64), 0, st>>>(la, lb, npairs, d_np, d_off, d_prim, d_Q);
+    schwarz_generic_kernel<<<dim3((npairs + 63) / 64), dim3(64), 0, st>>>(la, lb, npairs, d_np, d_off, d_prim, d_boys, d_Q);
     RT_CUDA(cudaGetLastError());
     return RTTDA_OK;
 }

@@ -264,7 +264,7 @@ int create_impl(Handle* h, const rttda_basis_t* basis, const double* C_occ, cons
     const size_t N = h->nao;
 
     // ---- Boys table
-    for (int L = 0; L <= 4; ++L) {
+    for (int L = 0; L <= 8; ++L) {
         std::vector<double> boys;
         boys_table_host(L, boys);
         const double* d = nullptr;
@@ -318,9 +318,9 @@ int create_impl(Handle* h, const rttda_basis_t* basis, const double* C_occ, cons
         RT_CUDA(cudaMemcpyAsync(d_np, cand_np[pc].data(), n * sizeof(int), cudaMemcpyHostToDevice, st));
         RT_CUDA(cudaMemcpyAsync(d_off, cand_off[pc].data(), n * sizeof(int), cudaMemcpyHostToDevice, st));
         RT_CUDA(cudaMemcpyAsync(d_prim, rows[pc].data(), rows[pc].size() * sizeof(double), cudaMemcpyHostToDevice, st));
-        // pairs with a d shell take the general path (eri_generic.cu), which needs no Boys table
+        // pairs with a d shell take the general path (eri_generic.cu)
         const int pl1 = pairclass_l1(pc), pl2 = pairclass_l2(pc);
-        if (pl1 > 1) RT_TRY(schwarz_general(pl1, pl2, n, d_np, d_off, d_prim, d_Q, st));
+        if (pl1 > 1) RT_TRY(schwarz_general(pl1, pl2, n, d_np, d_off, d_prim, h->tabs.boys[2 * (pl1 + pl2)], d_Q, st));
         else RT_TRY(schwarz_device(pc, n, d_np, d_off, d_prim, h->tabs.boys[2 * pc], d_Q, st));
         h->kernel_launches++;
         std::vector<double> Q(n);
@@ -337,7 +337,7 @@ int create_impl(Handle* h, const rttda_basis_t* basis, const double* C_occ, cons
         RT_CUDA(cudaMalloc(&t_Q1.p, nrow * sizeof(double)));
         RT_CUDA(cudaMemcpyAsync(t_np1.p, one.data(), nrow * sizeof(int), cudaMemcpyHostToDevice, st));
         RT_CUDA(cudaMemcpyAsync(t_off1.p, idx.data(), nrow * sizeof(int), cudaMemcpyHostToDevice, st));
-        if (pl1 > 1) RT_TRY(schwarz_general(pl1, pl2, nrow, (int*)t_np1.p, (int*)t_off1.p, d_prim, (double*)t_Q1.p, st));
+        if (pl1 > 1) RT_TRY(schwarz_general(pl1, pl2, nrow, (int*)t_np1.p, (int*)t_off1.p, d_prim, h->tabs.boys[2 * (pl1 + pl2)], (double*)t_Q1.p, st));
         else RT_TRY(schwarz_device(pc, nrow, (int*)t_np1.p, (int*)t_off1.p, d_prim, h->tabs.boys[2 * pc], (double*)t_Q1.p, st));
         h->kernel_launches++;
         qprim[pc].resize(nrow);
