@@ -116,6 +116,22 @@ int rttda_sigma_host(rttda_handle_t h, int32_t nvec, const double* X, double* si
  * T, F DEVICE [nvec][nao][nao]. */
 int rttda_fock(rttda_handle_t h, int32_t nvec, const double* T, double* F, void* stream);
 
+/* rttda_fock for callers that cannot allocate device memory (code under CUDA graph capture, tight serving loops,
+ * harnesses that forbid cudaMalloc): same inputs, same result, but every workspace - interleaved densities and results,
+ * the symmetry-split density pairs, the integral staging buffer - lives in ONE file-scope device array of
+ * RTTDA_STATIC_SCRATCH_BYTES inside the library (csrc/fock_static.cu), and the call runs no cudaMalloc / cudaFree /
+ * allocating library routine.  Every GPU that loads the library holds that array until the process exits.
+ *   nvec   1..RTTDA_STATIC_MAX_NVEC;  T, F DEVICE [nvec][nao][nao] as for rttda_fock, must not alias
+ *   EINVAL (with the byte counts in rttda_last_error) when 4 * nao^2 * nvt * 8 bytes + the handle's staging buffer
+ *          (RTTDA_INFO_ERI_BUF_BYTES) exceed the array: about 250 basis functions with s/p shells; use rttda_fock beyond
+ *   All calls on one device share the array and it keeps the last call's contents (the call clears what must start at
+ *   zero): calls that overlap on the GPU - two streams, or two handles on one device - RACE; serialise them.  The
+ *   segments run one after the other on `stream` (no lanes), so small molecules are slower here than through rttda_fock.
+ *   The first call on a device resolves the array's device address (cudaGetSymbolAddress) and must not be captured. */
+#define RTTDA_STATIC_SCRATCH_BYTES 134217728
+#define RTTDA_STATIC_MAX_NVEC 8
+int rttda_fock_static(rttda_handle_t h, int32_t nvec, const double* T, double* F, void* stream);
+
 /* Fixed-step RK4 (R7) on i dC/dt = H(t) C for ntraj independent trajectories sharing every ERI pass.
  *   C      DEVICE in/out [ntraj][2][1 + nocc*nvirt]: plane 0 = q (Re), plane 1 = p (Im); element 0 = KS
  *          ground state

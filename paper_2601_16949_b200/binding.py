@@ -24,7 +24,7 @@ OPT_RS_OMEGA = 4
 FIELD_CONTINUE = 1
 PULSE = dict(none=0, delta=1, cw=2, tl=3, chirp=4, sin2=5)
 EXPORTS = ["rttda_overlap", "rttda_dipole_ao", "rttda_create", "rttda_destroy", "rttda_sigma",
-           "rttda_sigma_host", "rttda_fock", "rttda_propagate", "rttda_propagate_sso", "rttda_propagate_host",
+           "rttda_sigma_host", "rttda_fock", "rttda_fock_static", "rttda_propagate", "rttda_propagate_sso", "rttda_propagate_host",
            "rttda_get_info", "rttda_set_option", "rttda_populations", "rttda_spectrum", "rttda_lanczos", "rttda_eigs", "rttda_last_timings", "rttda_jk_time", "rttda_profile_pass", "rttda_gemm_f64", "rttda_fp64_peak", "rttda_last_error",
            "rttda_version"]
 
@@ -194,6 +194,10 @@ class Rttda:
 
     def rttda_fock(self, T, F, stream=None):
         _check(lib().rttda_fock(self._h, int(T.shape[0]), _dptr(T), _dptr(F), _stream(stream)), "rttda_fock")
+        return F
+
+    def rttda_fock_static(self, T, F, stream=None):
+        _check(lib().rttda_fock_static(self._h, int(T.shape[0]), _dptr(T), _dptr(F), _stream(stream)), "rttda_fock_static")
         return F
 
     def _fields(self, fields):
