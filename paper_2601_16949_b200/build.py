@@ -9,7 +9,7 @@ from concurrent.futures import ThreadPoolExecutor
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "librttda.so")
-SOURCES = ["api.cu", "setup.cu", "jk_eval.cu", "jk_digest.cu", "eri_generic.cu", "fock_static.cu", "gemm_f64.cu", "propagate.cu", "eigs.cu"]
+SOURCES = ["api.cu", "setup.cu", "jk_eval.cu", "jk_digest.cu", "eri_generic.cu", "jk_eval_d.cu", "fock_static.cu", "gemm_f64.cu", "propagate.cu", "eigs.cu"]
 HEADERS = ["common.cuh", "eri_eval.cuh", "tma.cuh", os.path.join("..", "..", "include", "rttda.h")]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",

@@ -235,6 +235,8 @@ int schwarz_device(int pairclass, int npairs, const int* d_np, const int* d_off,
 // eri_generic.cu: the general-angular-momentum path (classes with a d shell)
 bool segment_is_general(const Segment& sg);
 int eval_segment_general(Handle* h, const Segment& sg, double* buf, cudaStream_t st);
+// jk_eval_d.cu: unrolled kernels for the d classes up to L = 5 (*handled = false: not one of them)
+int eval_segment_d(Handle* h, const Segment& sg, double* buf, cudaStream_t st, bool* handled);
 int digest_segment_general(Handle* h, const Segment& sg, const double* buf, int nvt, int nvec, const double* Tq, double* Fq,
                            cudaStream_t st);
 int schwarz_general(int la, int lb, int npairs, const int* d_np, const int* d_off, const double* d_prim,

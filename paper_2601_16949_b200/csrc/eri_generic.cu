@@ -10,6 +10,7 @@
 //   (ab|cd) = c_b c_k / sqrt(p+q) sum_{tuv} E^{ab}_{tuv} sum_{t'u'v'} (-1)^{t'+u'+v'} E^{cd}_{t'u'v'} R_{t+t',u+u',v+v'}
 // with E_0^{00} = 1 (the Gaussian-product factors sit in the row entry c), R^n_{000} = (-2 alpha)^n F_n(alpha |PQ|^2).
 // d components: xx, xy, xz, yy, yz, zz, each normalised (reading R11: xy, xz, yz carry sqrt(3)).
+#include <cstdlib>
 #include "common.cuh"
 
 namespace rttda {
@@ -473,6 +474,11 @@ bool segment_is_general(const Segment& sg) { return sg.la > 1 || sg.lb > 1 || sg
 
 int eval_segment_general(Handle* h, const Segment& sg, double* buf, cudaStream_t st)
 {
+    if (!getenv("RTTDA_GENERIC_ONLY")) {               // classes up to L = 5 have unrolled kernels (jk_eval_d.cu)
+        bool handled = false;
+        RT_TRY(eval_segment_d(h, sg, buf, st, &handled));
+        if (handled) return RTTDA_OK;
+    }
     GenEvalArgs g;
     g.items = sg.items;
     g.bra = h->tabs.kets[sg.kc_bra];

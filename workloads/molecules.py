@@ -77,6 +77,7 @@ class Config:
 _SP5 = ((0, 3), (0, 1), (1, 1))                      # BJ:configs[0]: 2 s shells (3, 1 prims) + p(1)
 _HEAVY9 = ((0, 3), (0, 3), (0, 1), (1, 3), (1, 1))   # R12
 _H2 = ((0, 3), (0, 1))
+_SPD15 = ((0, 3), (0, 3), (0, 1), (1, 3), (1, 1), (2, 1))   # 6-31G*-like heavy centre: 3 s + 2 p + 1 Cartesian d shell = 15 BF
 _SPD14 = ((0, 3), (0, 1), (1, 3), (1, 1), (2, 1))    # 6-31G*-like heavy centre with one Cartesian d shell (NEXT-4)
 
 CONFIGS = {
@@ -99,6 +100,10 @@ CONFIGS = {
     # 20 heavy centres (14 AOs) + 20 H-like (2 AOs); measurement and parity case of the d-shell path
     7: Config("d-320", 20, 20, _SPD14, _H2, 60, 260, 1e-12, 0.05, 100,
               ({"type": "cw", "E0": 0.01, "omega": 0.3, "dir": (0.0, 0.0, 1.0)},), 7, 1),       # draw 1: cond(S) = 1.9e3
+    # the SHAPE of the paper's largest molecule (Table 3: F-Coronene C108 H42 N12, 120 heavy atoms x 15 BF +
+    # 42 H x 2 BF = 1884 BF, 387 occupied orbitals); synthetic centres and exponents as everywhere
+    8: Config("d-1884", 120, 42, _SPD15, _H2, 387, 1497, 1e-12, 0.1, 0,
+              ({"type": "cw", "E0": 0.01, "omega": 0.3, "dir": (0.0, 0.0, 1.0)},), 8, 2),   # draw 2: cond(S) = 5.5e4
 }
 
 
