@@ -3,6 +3,7 @@
 #include <cuda_runtime.h>
 #include <cstdint>
 #include <cstdio>
+#include <cstdlib>
 #include <string>
 #include <vector>
 #include "../../include/rttda.h"
@@ -48,7 +49,7 @@ constexpr int PRIM_STRIDE = 12;
 constexpr int NSUB = 4;                       // primitive pairs stored per shell pair: {1, 3, 6, 9}
 constexpr int NPAIRCLASS = 6;
 constexpr int NKETCLASS = NPAIRCLASS * NSUB;  // ket class id = pairclass * NSUB + sub
-__host__ __device__ inline int ncart(int l) { return (l + 1) * (l + 2) / 2; }     // Cartesian components of a shell
+__host__ __device__ constexpr int ncart(int l) { return (l + 1) * (l + 2) / 2; }     // Cartesian components of a shell
 inline int pairclass_of(int l1, int l2) { return l1 * (l1 + 1) / 2 + l2; }       // l1 >= l2
 inline int pairclass_l1(int pc) { return pc >= 3 ? 2 : (pc >= 1 ? 1 : 0); }
 inline int pairclass_l2(int pc) { return pc - pairclass_l1(pc) * (pairclass_l1(pc) + 1) / 2; }
@@ -234,6 +235,17 @@ int schwarz_device(int pairclass, int npairs, const int* d_np, const int* d_off,
                    const double2* d_boys /* table for L = 2 * pairclass */, double* d_Q, cudaStream_t st);
 // eri_generic.cu: the general-angular-momentum path (classes with a d shell)
 bool segment_is_general(const Segment& sg);
+// the a-list digestion kernels (jk_digest.cu) are instantiated for the s/p classes and for these d classes
+inline bool digest_has_alist_kernels(const Segment& sg)
+{
+    if (sg.la <= 1) return true;                                   // s/p (canonical order: la is the largest)
+    if (getenv("RTTDA_GENERIC_DIGEST")) return false;
+    const int bra = sg.la * 3 + sg.lb, ket = sg.lc * 3 + sg.ld;    // (2,0) = 6, (2,1) = 7, (2,2) = 8
+    if (bra == 6) return ket == 0 || ket == 3 || ket == 4 || ket == 6;
+    if (bra == 7) return ket == 0 || ket == 3 || ket == 4 || ket == 6;
+    if (bra == 8) return ket == 0 || ket == 3 || ket == 4;
+    return false;
+}
 int eval_segment_general(Handle* h, const Segment& sg, double* buf, cudaStream_t st);
 // jk_eval_d.cu: unrolled kernels for the d classes up to L = 5 (*handled = false: not one of them)
 int eval_segment_d(Handle* h, const Segment& sg, double* buf, cudaStream_t st, bool* handled);

@@ -124,7 +124,7 @@ template <int LA, int LB, int LC, int LD, int NV>
 __global__ void __launch_bounds__(JK_BLOCK)
 digest_j_kernel(DigestArgs g)
 {
-    constexpr int NA = 2 * LA + 1, NB = 2 * LB + 1, NC = 2 * LC + 1, ND = 2 * LD + 1;
+    constexpr int NA = ncart(LA), NB = ncart(LB), NC = ncart(LC), ND = ncart(LD);
     constexpr int NI = NA * NB * NC * ND;
     constexpr bool USE_TMA = digest_uses_tma(NI);
     const JKTables& tb = g.tb;
@@ -307,7 +307,7 @@ template <int LA, int LB, int LC, int LD>
 __global__ void __launch_bounds__(256)
 digest_b_kernel(DigestArgs g, int G, int KW)
 {
-    constexpr int NA = 2 * LA + 1, NB = 2 * LB + 1, NC = 2 * LC + 1, ND = 2 * LD + 1;
+    constexpr int NA = ncart(LA), NB = ncart(LB), NC = ncart(LC), ND = ncart(LD);
     constexpr int NI = NA * NB * NC * ND;
     const JKTables& tb = g.tb;
     const WorkItem wi = g.work[blockIdx.x >> 2];
@@ -486,7 +486,7 @@ template <int LA, int LB, int LC, int LD>
 __global__ void __launch_bounds__(256)
 digest_k_kernel(DigestArgs g, int G, int KW)
 {
-    constexpr int NA = 2 * LA + 1, NB = 2 * LB + 1, NC = 2 * LC + 1, ND = 2 * LD + 1;
+    constexpr int NA = ncart(LA), NB = ncart(LB), NC = ncart(LC), ND = ncart(LD);
     constexpr int NI = NA * NB * NC * ND;
     constexpr int NAB = NA * NB;
     constexpr int KR = digest_k_recs(NI);
@@ -662,7 +662,7 @@ static int launch_digest_j(Handle* h, const JKLaunch& L, const Segment& sg, cons
     g.buf = buf;
     g.Tq = Tq; g.PPq = nullptr; g.Fq = Fq; g.cx = h->pass_cx;
     g.ketclass = L.ketclass; g.same = (sg.kc_bra == sg.kc_ket); g.nvt = nvt; g.v0 = v0;
-    constexpr int NI = (2 * LA + 1) * (2 * LB + 1) * (2 * LC + 1) * (2 * LD + 1);
+    constexpr int NI = (ncart(LA)) * (ncart(LB)) * (ncart(LC)) * (ncart(LD));
     constexpr size_t smem = digest_ring_bytes(NI);
     if (smem > 0)     // per launch: the attribute belongs to the current device's context, not to the process
         RT_CUDA(cudaFuncSetAttribute(digest_j_kernel<LA, LB, LC, LD, NV>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
@@ -680,9 +680,9 @@ template <int LA, int LB, int LC, int LD>
 static int launch_digest(Handle* h, const JKLaunch& L, const Segment& sg, const double* buf, int nvt, int nvec,
                          const double* Tq, double* Fq, cudaStream_t st)
 {
-    constexpr int NC = 2 * LC + 1, ND = 2 * LD + 1;
+    constexpr int NC = ncart(LC), ND = ncart(LD);
     if (LA >= LB && h->pass_do_j) {
-        constexpr int NVJ = (NC * ND <= 3) ? 8 : 4;
+        constexpr int NVJ = (NC * ND <= 3) ? 8 : (NC * ND <= 9 ? 4 : 2);      // Scd and Jcd hold NC ND NVJ doubles each
         int v0 = 0;
         while (v0 < nvec) {
             const int left = nvec - v0;
@@ -692,10 +692,12 @@ static int launch_digest(Handle* h, const JKLaunch& L, const Segment& sg, const 
             else { RT_TRY((launch_digest_j<LA, LB, LC, LD, 2>(h, L, sg, buf, nvt, v0, Tq, Fq, st))); v0 += 2; }
         }
     }
-    constexpr int NI = (2 * LA + 1) * (2 * LB + 1) * (2 * LC + 1) * (2 * LD + 1);
+    constexpr int NI = (ncart(LA)) * (ncart(LB)) * (ncart(LC)) * (ncart(LD));
     constexpr size_t smem = (size_t)2 * NI * 256;
-    RT_CUDA(cudaFuncSetAttribute(digest_b_kernel<LA, LB, LC, LD>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    RT_CUDA(cudaFuncSetAttribute(digest_k_kernel<LA, LB, LC, LD>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)digest_k_smem(NI)));
+    if constexpr (NI > RTTDA_K_MAXNI)
+        RT_CUDA(cudaFuncSetAttribute(digest_b_kernel<LA, LB, LC, LD>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    else
+        RT_CUDA(cudaFuncSetAttribute(digest_k_kernel<LA, LB, LC, LD>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)digest_k_smem(NI)));
     if (!h->pass_do_k || h->pass_cx == 0.0) return RTTDA_OK;
     for (int v0 = 0; v0 < nvec; v0 += 8) {
         // lane groups of 2, 4 or 8 densities: a group then never straddles a quarter warp, so one 16-byte gather per
@@ -710,7 +712,7 @@ static int launch_digest(Handle* h, const JKLaunch& L, const Segment& sg, const 
         const int KW = 32 / G, nwarps = (32 + KW - 1) / KW;
         // one or three integrals per quartet: the multi-record ring (digest_k_kernel) wins; above that its larger
         // register footprint costs more occupancy than the saved barriers bring (profiles/README.md)
-        if (NI > RTTDA_K_MAXNI) digest_b_kernel<LA, LB, LC, LD><<<dim3(4 * L.nwork), dim3(32 * nwarps), smem, st>>>(g, G, KW);
+        if constexpr (NI > RTTDA_K_MAXNI) digest_b_kernel<LA, LB, LC, LD><<<dim3(4 * L.nwork), dim3(32 * nwarps), smem, st>>>(g, G, KW);
         else digest_k_kernel<LA, LB, LC, LD><<<dim3(4 * L.nwork), dim3(32 * nwarps), digest_k_smem(NI), st>>>(g, G, KW);
         h->kernel_launches++;
         RT_CUDA(cudaGetLastError());
@@ -722,7 +724,7 @@ static int launch_digest(Handle* h, const JKLaunch& L, const Segment& sg, const 
 int digest_segment(Handle* h, const Segment& sg, const double* buf, int nvt, int nvec, const double* Tq, double* Fq,
                    cudaStream_t st)
 {
-    if (segment_is_general(sg)) return digest_segment_general(h, sg, buf, nvt, nvec, Tq, Fq, st);
+    if (sg.nlaunch == 0) return digest_segment_general(h, sg, buf, nvt, nvec, Tq, Fq, st);   // no a-list launches: general kernel
     for (int l = sg.first_launch; l < sg.first_launch + sg.nlaunch; ++l)
         RT_TRY(digest_launch(h, h->launches[l], sg, buf, nvt, nvec, Tq, Fq, st));
     return RTTDA_OK;
@@ -732,18 +734,20 @@ int digest_launch(Handle* h, const JKLaunch& L, const Segment& sg, const double*
                   const double* Tq, double* Fq, cudaStream_t st)
 {
     if (L.nwork == 0) return RTTDA_OK;
-    const int key = L.la * 8 + L.lb * 4 + L.lc * 2 + L.ld;
-    switch (key) {
-        case 0:  return launch_digest<0, 0, 0, 0>(h, L, sg, buf, nvt, nvec, Tq, Fq, st);
-        case 8:  return launch_digest<1, 0, 0, 0>(h, L, sg, buf, nvt, nvec, Tq, Fq, st);
-        case 4:  return launch_digest<0, 1, 0, 0>(h, L, sg, buf, nvt, nvec, Tq, Fq, st);
-        case 10: return launch_digest<1, 0, 1, 0>(h, L, sg, buf, nvt, nvec, Tq, Fq, st);
-        case 6:  return launch_digest<0, 1, 1, 0>(h, L, sg, buf, nvt, nvec, Tq, Fq, st);
-        case 12: return launch_digest<1, 1, 0, 0>(h, L, sg, buf, nvt, nvec, Tq, Fq, st);
-        case 14: return launch_digest<1, 1, 1, 0>(h, L, sg, buf, nvt, nvec, Tq, Fq, st);
-        case 15: return launch_digest<1, 1, 1, 1>(h, L, sg, buf, nvt, nvec, Tq, Fq, st);
+#define RT_DIGEST_CASE(A, B, C, D) \
+    case ((A * 3 + B) * 3 + C) * 3 + D: return launch_digest<A, B, C, D>(h, L, sg, buf, nvt, nvec, Tq, Fq, st);
+    switch (((L.la * 3 + L.lb) * 3 + L.lc) * 3 + L.ld) {
+        RT_DIGEST_CASE(0, 0, 0, 0) RT_DIGEST_CASE(1, 0, 0, 0) RT_DIGEST_CASE(0, 1, 0, 0) RT_DIGEST_CASE(1, 0, 1, 0)
+        RT_DIGEST_CASE(0, 1, 1, 0) RT_DIGEST_CASE(1, 1, 0, 0) RT_DIGEST_CASE(1, 1, 1, 0) RT_DIGEST_CASE(1, 1, 1, 1)
+        // classes with a d shell (both orientations of the bra pair) up to DIGEST_ALIST_MAXNI integrals per quartet
+        RT_DIGEST_CASE(2, 0, 0, 0) RT_DIGEST_CASE(0, 2, 0, 0) RT_DIGEST_CASE(2, 0, 1, 0) RT_DIGEST_CASE(0, 2, 1, 0)
+        RT_DIGEST_CASE(2, 0, 1, 1) RT_DIGEST_CASE(0, 2, 1, 1) RT_DIGEST_CASE(2, 0, 2, 0) RT_DIGEST_CASE(0, 2, 2, 0)
+        RT_DIGEST_CASE(2, 1, 0, 0) RT_DIGEST_CASE(1, 2, 0, 0) RT_DIGEST_CASE(2, 1, 1, 0) RT_DIGEST_CASE(1, 2, 1, 0)
+        RT_DIGEST_CASE(2, 1, 1, 1) RT_DIGEST_CASE(1, 2, 1, 1) RT_DIGEST_CASE(2, 1, 2, 0) RT_DIGEST_CASE(1, 2, 2, 0)
+        RT_DIGEST_CASE(2, 2, 0, 0) RT_DIGEST_CASE(2, 2, 1, 0) RT_DIGEST_CASE(2, 2, 1, 1)
         default: set_error("digest: unsupported class"); return RTTDA_EINVAL;
     }
+#undef RT_DIGEST_CASE
 }
 
 // PP[mu][nu][v] = {T[mu][nu][v] + T[nu][mu][v], T[mu][nu][v] - T[nu][mu][v]}  (step a2 of DESIGN.md)

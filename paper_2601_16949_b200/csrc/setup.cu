@@ -541,7 +541,7 @@ int create_impl(Handle* h, const rttda_basis_t* basis, const double* C_occ, cons
             // digestion launches: ordered bra classes (a-lists) of this bra pair class against the ket class
             sg.first_launch = (int)h->launches.size();
             for (int orient = 0; orient < 2; ++orient) {
-                if (segment_is_general(sg)) break;                 // classes with a d shell: one kernel digests the whole segment
+                if (!digest_has_alist_kernels(sg)) break;          // large d classes: one general kernel digests the whole segment
                 if (orient == 1 && sg.la == sg.lb) break;          // ss and pp pairs: one ordered class
                 const int la = orient == 0 ? sg.la : sg.lb, lb = orient == 0 ? sg.lb : sg.la;
                 std::vector<std::pair<double, WorkItem>> witems;
