@@ -242,8 +242,8 @@ inline bool digest_has_alist_kernels(const Segment& sg)
     if (getenv("RTTDA_GENERIC_DIGEST")) return false;
     const int bra = sg.la * 3 + sg.lb, ket = sg.lc * 3 + sg.ld;    // (2,0) = 6, (2,1) = 7, (2,2) = 8
     if (bra == 6) return ket == 0 || ket == 3 || ket == 4 || ket == 6;
-    if (bra == 7) return ket == 0 || ket == 3 || ket == 4 || ket == 6;
-    if (bra == 8) return ket == 0 || ket == 3 || ket == 4;
+    if (bra == 7) return ket == 0 || ket == 3 || ket == 4 || ket == 6 || ket == 7;
+    if (bra == 8) return ket == 0 || ket == 3 || ket == 4 || ket == 6 || ket == 7;
     return false;
 }
 int eval_segment_general(Handle* h, const Segment& sg, double* buf, cudaStream_t st);

@@ -82,6 +82,9 @@ constexpr int REC_TILE = 256;
 constexpr bool digest_uses_tma(int ni) { return ni <= 27; }
 constexpr size_t digest_ring_bytes(int ni) { return digest_uses_tma(ni) ? (size_t)(JK_BLOCK / 32) * 2 * ni * 256 : 0; }      // a-list records staged in shared memory at a time
 
+// ring stages of digest_b_kernel: two (the copy of record r+1 flies while record r is digested) while they fit in shared
+// memory, one for the largest classes (648 integrals per quartet = 166 KB per stage)
+constexpr int digest_b_stages(int ni) { return (size_t)2 * ni * 256 <= 200 * 1024 ? 2 : 1; }
 constexpr int next_pow2(int n) { return n <= 1 ? 1 : (n <= 2 ? 2 : (n <= 4 ? 4 : (n <= 8 ? 8 : (n <= 16 ? 16 : 32)))); }
 
 struct DigestArgs {
@@ -406,7 +409,8 @@ digest_b_kernel(DigestArgs g, int G, int KW)
             const BraRec br = s_rec[ir];
             const bool more = (ir + 1 < nrec) && reaches(ir + 1);
             __syncthreads();                              // every warp is done with the stage refilled next
-            if (more) issue(ir + 1, stage ^ 1);
+            if constexpr (digest_b_stages(NI) == 2) { if (more) issue(ir + 1, stage ^ 1); }
+            else { if (ir > 0) issue(ir, 0); }            // single stage: the copy cannot overlap the previous record
             if (stage == 0) { mbar_wait(&s_bar[0], phase0); phase0 ^= 1; }
             else { mbar_wait(&s_bar[1], phase1); phase1 ^= 1; }
             const double* src = s_dyn + (size_t)stage * (NI * 32) + (kb & 31);
@@ -439,7 +443,7 @@ digest_b_kernel(DigestArgs g, int G, int KW)
                     }
                 }
             }
-            stage ^= 1;
+            if constexpr (digest_b_stages(NI) == 2) stage ^= 1;
             if (!more) { if (ir + 1 < nrec) done = true; break; }
             ok_cur = lane_ok(ir + 1);
             gather(ir + 1, ok_cur, cur_bd, cur_bc);
@@ -693,7 +697,7 @@ static int launch_digest(Handle* h, const JKLaunch& L, const Segment& sg, const 
         }
     }
     constexpr int NI = (ncart(LA)) * (ncart(LB)) * (ncart(LC)) * (ncart(LD));
-    constexpr size_t smem = (size_t)2 * NI * 256;
+    constexpr size_t smem = (size_t)digest_b_stages(NI) * NI * 256;
     if constexpr (NI > RTTDA_K_MAXNI)
         RT_CUDA(cudaFuncSetAttribute(digest_b_kernel<LA, LB, LC, LD>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     else
@@ -745,6 +749,7 @@ int digest_launch(Handle* h, const JKLaunch& L, const Segment& sg, const double*
         RT_DIGEST_CASE(2, 1, 0, 0) RT_DIGEST_CASE(1, 2, 0, 0) RT_DIGEST_CASE(2, 1, 1, 0) RT_DIGEST_CASE(1, 2, 1, 0)
         RT_DIGEST_CASE(2, 1, 1, 1) RT_DIGEST_CASE(1, 2, 1, 1) RT_DIGEST_CASE(2, 1, 2, 0) RT_DIGEST_CASE(1, 2, 2, 0)
         RT_DIGEST_CASE(2, 2, 0, 0) RT_DIGEST_CASE(2, 2, 1, 0) RT_DIGEST_CASE(2, 2, 1, 1)
+        RT_DIGEST_CASE(2, 1, 2, 1) RT_DIGEST_CASE(1, 2, 2, 1) RT_DIGEST_CASE(2, 2, 2, 0) RT_DIGEST_CASE(2, 2, 2, 1)
         default: set_error("digest: unsupported class"); return RTTDA_EINVAL;
     }
 #undef RT_DIGEST_CASE

@@ -1,6 +1,6 @@
-// Unrolled evaluation kernels for the shell-quartet classes with a d shell and total angular momentum L <= 5
-// ((ds|ss) ... (dp|pp), (dp|ds), (dd|ps)).  Same block shape, staging layout, screening rules and
-// weights as eval_generic_kernel (eri_generic.cu), which keeps the classes above L = 5; what differs is that every
+// Unrolled evaluation kernels for the shell-quartet classes with a d shell up to (dd|dp), L <= 7.
+// Same block shape, staging layout, screening rules and weights as eval_generic_kernel (eri_generic.cu), which keeps
+// (dd|dd); what differs is that every
 // angular-momentum quantity is a template parameter, so all loops unroll, every Hermite index is a constant and the
 // tables are registers (or local memory at fixed offsets) instead of run-time indexed arrays.
 //
@@ -268,6 +268,10 @@ int eval_segment_d(Handle* h, const Segment& sg, double* buf, cudaStream_t st, b
         case ((2 * 3 + 1) * 3 + 1) * 3 + 1: return launch_eval_d<2, 1, 1, 1, 3>(h, sg, buf, st);
         case ((2 * 3 + 1) * 3 + 2) * 3 + 0: return launch_eval_d<2, 1, 2, 0, 3>(h, sg, buf, st);
         case ((2 * 3 + 2) * 3 + 1) * 3 + 0: return launch_eval_d<2, 2, 1, 0, 3>(h, sg, buf, st);
+        case ((2 * 3 + 1) * 3 + 2) * 3 + 1: return launch_eval_d<2, 1, 2, 1, 6>(h, sg, buf, st);
+        case ((2 * 3 + 2) * 3 + 1) * 3 + 1: return launch_eval_d<2, 2, 1, 1, 3>(h, sg, buf, st);
+        case ((2 * 3 + 2) * 3 + 2) * 3 + 0: return launch_eval_d<2, 2, 2, 0, 6>(h, sg, buf, st);
+        case ((2 * 3 + 2) * 3 + 2) * 3 + 1: return launch_eval_d<2, 2, 2, 1, 6>(h, sg, buf, st);
         default: *handled = false; return RTTDA_OK;
     }
 }
