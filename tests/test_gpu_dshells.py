@@ -204,3 +204,34 @@ def test_d320_sigma_vs_matrix_free_oracle():
     print("d-320: sigma rel err %.2e (%d oracle quartets)" % (err, nq))
     assert err < SIGMA_TOL
     assert abs(X[0] @ got[1] - X[1] @ got[0]) < 1e-11                 # A is symmetric
+
+
+def test_d1884_fock_sampled_elements_and_properties():
+    """1884 basis functions in the shape of the paper's largest molecule (Table 3: 120 heavy centres x 15 BF
+    with one Cartesian d shell each + 42 H-like x 2 BF; workloads key 8), 1.56e9 unique shell quartets, every kernel of
+    the d path at full size (pipeline mode, unrolled evaluation, a-list digestion, (dd|dd) on the general kernels):
+    F elements at sampled AO pairs - d, p and s functions - against the oracle's definition-level J and K (no screening,
+    no symmetry), plus properties that hold at any size."""
+    ctx = setup_config(8)
+    ob, basis = ctx["ob"], ctx["basis"]
+    N = basis.nao
+    assert N == 1884
+    rng = np.random.default_rng(8)
+    X = rng.standard_normal((2, ctx["cfg"].nocc, ctx["cfg"].nvirt))
+    X /= np.linalg.norm(X.reshape(2, -1), axis=1)[:, None, None]
+    T = np.stack([ctx["C_o"] @ x @ ctx["C_v"].T for x in X])              # transition densities, non-symmetric
+    F = gpu_fock(ctx, T)
+    off = basis.ao_off
+    d_sh = [s for s in range(basis.nshells) if basis.sh_l[s] == 2]
+    p_sh = [s for s in range(basis.nshells) if basis.sh_l[s] == 1]
+    mu = np.array([off[d_sh[3]] + 1, off[d_sh[50]] + 3, off[p_sh[7]] + 2, 0, off[d_sh[100]] + 5])
+    nu = np.array([off[d_sh[3]] + 4, off[p_sh[90]] + 1, off[d_sh[77]] + 0, N - 1, off[d_sh[100]] + 5])
+    J, K = ob.jk_samples(T, mu, nu)
+    got = F[:, mu, nu].T
+    scale = np.max(np.abs(F))
+    err = np.max(np.abs(got - (2 * J - K))) / scale
+    print("d-1884: sampled Fock elements, max error / max|F| = %.2e" % err)
+    assert err < SIGMA_TOL
+    F2 = gpu_fock(ctx, np.stack([T[0] + T[0].T, 2.0 * T[1] - 0.5 * T[0]]))
+    assert np.max(np.abs(F2[0] - (F[0] + F[0].T))) / scale < SIGMA_TOL     # F[T^T] = F[T]^T
+    assert np.max(np.abs(F2[1] - (2.0 * F[1] - 0.5 * F[0]))) / scale < SIGMA_TOL
