@@ -43,7 +43,7 @@ typedef struct rttda_handle_s* rttda_handle_t;   /* opaque; owns all internal de
 
 /* One contracted Cartesian Gaussian shell: l = 0 (s), 1 (p: components x, y, z) or 2 (d: the six Cartesian components
  * xx, xy, xz, yy, yz, zz, each normalised to <phi|phi> = 1, "6-31G*").  AO order = shell
- * order, so nao = sum over shells of (l+1)(l+2)/2.  Classes with a d shell run on a general (slower) kernel path. */
+ * order, so nao = sum over shells of (l+1)(l+2)/2. */
 typedef struct {
     int32_t center;     /* index into centers */
     int32_t l;          /* 0, 1 or 2 */
