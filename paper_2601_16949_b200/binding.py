@@ -271,9 +271,9 @@ class Rttda:
 
     def rttda_profile_pass(self, nvec: int, stream=None) -> np.ndarray:
         """One extra ERI pass with per-segment CUDA-event timings; rows as documented in include/rttda.h."""
-        rows = np.zeros((128, 16))
+        rows = np.zeros((512, 16))                    # at most 24 x 25 / 2 = 300 segments (6 pair types x 4 contraction sub-classes)
         n = ct.c_int32(0)
-        _check(lib().rttda_profile_pass(self._h, int(nvec), _dptr(rows), 128, ct.byref(n), _stream(stream)),
+        _check(lib().rttda_profile_pass(self._h, int(nvec), _dptr(rows), 512, ct.byref(n), _stream(stream)),
                "rttda_profile_pass")
         return rows[: n.value]
 
