@@ -53,6 +53,9 @@ def parse():
                     help="rk4 (BASELINE.json configs; 8 sigma-vectors per trajectory and step) or the paper's SSO "
                          "(NEXT-1; 2 per trajectory and step)")
     ap.add_argument("--tau", type=float, default=0.0, help="Schwarz threshold (0 = the config's: 1e-12, reading R15)")
+    ap.add_argument("--exchange", default="1,0,0", metavar="CX,CX_LR,OMEGA",
+                    help="exchange kernel of A: -cx (ij|ab) - cx_lr (ij|erf(omega r)/r|ab); default 1,0,0 = the exchange-only "
+                         "headline (BASELINE.json); 0.19,0.46,0.33 = the exchange part of the paper's CAM-B3LYP (second ERI pass)")
     ap.add_argument("--parity-tau", type=float, default=1e-14,
                     help="second, tighter threshold at which config 4 is also timed: the largest tau of the sweep at which "
                          "sigma meets the 1e-10 oracle tolerance at 1280 AO (tests/test_gpu_parity.py, DESIGN.md section 11); 0 = skip")
@@ -261,7 +264,11 @@ def run_b200(args):
     st = torch.cuda.current_stream()
     tau = args.tau if args.tau > 0 else cfg.tau
     Co_d, Cv_d = torch.from_numpy(C_o).to(dev), torch.from_numpy(C_v).to(dev)
-    h = R.Rttda(basis, Co_d, Cv_d, eps, 1.0, tau, st)
+    cx, cx_lr, rs_omega = (float(x) for x in args.exchange.split(","))
+    h = R.Rttda(basis, Co_d, Cv_d, eps, cx, tau, st)
+    if cx_lr != 0.0 and rs_omega > 0.0:
+        h.rttda_set_option(R.OPT_CX_LR, cx_lr)
+        h.rttda_set_option(R.OPT_RS_OMEGA, rs_omega)
     torch.cuda.synchronize()
     setup_s = time.perf_counter() - t0
     info = h.info()
@@ -412,6 +419,8 @@ def run_b200(args):
                                       "+ 16 GEMM launches + field + combine" % (k, cfg.name, h.nao, h.nocc, h.nvirt,
                                                                                ncsf, ntraj, nvec, tau, dt),
                           "l2": "256 MiB buffer written between timed steps (L2 flush)",
+                          "exchange": {"cx": cx, "cx_lr": cx_lr, "rs_omega": rs_omega,
+                                       "eri_passes_per_sigma": 2 if (cx_lr != 0.0 and rs_omega > 0.0) else 1},
                           "parallelism": "replicas" if world > 1 else "1 GPU", "omega": omega,
                           "propagator": args.propagator + (" (one call per step: H(t0) q is recomputed, 3 sigma builds "
                                                            "of ntraj vectors per timed step)" if sso else ""),
