@@ -26,6 +26,8 @@
 #define LMAX 2       /* highest shell angular momentum: s, p, d */
 #define LMAX_TOT 8   /* l_a+l_b+l_c+l_d */
 #define NR (LMAX_TOT + 1)
+/* Hermite table R^n_{tuv}, n, t, u, v <= L, stored compactly with stride L + 1 (the variable L of the enclosing function) */
+#define RT(n, t, u, v) Rt[((((n) * (L + 1)) + (t)) * (L + 1) + (u)) * (L + 1) + (v)]
 #define NCART(l) (((l) + 1) * ((l) + 2) / 2)
 #define NCMAX 6      /* NCART(LMAX) */
 #define NQMAX 1296   /* NCMAX^4 */
@@ -71,15 +73,16 @@ void oracle_boys(int nmax, double T, double *F)
 /* ---- 1-D Hermite expansion coefficients E_t^{ij}, i,j <= LMAX, t <= i+j ------------------- */
 /* E_0^{00} = exp(-mu X_AB^2);
  * E_t^{i+1,j} = E_{t-1}^{ij}/(2p) + X_PA E_t^{ij} + (t+1) E_{t+1}^{ij}
- * E_t^{i,j+1} = E_{t-1}^{ij}/(2p) + X_PB E_t^{ij} + (t+1) E_{t+1}^{ij};  E_t = 0 for t<0, t>i+j */
-static void hermite_E(double a, double b, double Ax, double Bx, double E[LMAX + 1][LMAX + 1][2 * LMAX + 1])
+ * E_t^{i,j+1} = E_{t-1}^{ij}/(2p) + X_PB E_t^{ij} + (t+1) E_{t+1}^{ij};  E_t = 0 for t<0, t>i+j;
+ * filled for i <= li, j <= lj (the shells' angular momenta), zero beyond */
+static void hermite_E(int li, int lj, double a, double b, double Ax, double Bx, double E[LMAX + 1][LMAX + 1][2 * LMAX + 1])
 {
     double p = a + b, mu = a * b / p, XAB = Ax - Bx;
     double Px = (a * Ax + b * Bx) / p, XPA = Px - Ax, XPB = Px - Bx;
     memset(E, 0, sizeof(double) * (LMAX + 1) * (LMAX + 1) * (2 * LMAX + 1));
     E[0][0][0] = exp(-mu * XAB * XAB);
     /* i -> i+1 at j = 0 */
-    for (int i = 0; i < LMAX; ++i)
+    for (int i = 0; i < li; ++i)
         for (int t = 0; t <= i + 1; ++t) {
             double em = (t - 1 >= 0) ? E[i][0][t - 1] : 0.0;
             double e0 = (t <= i) ? E[i][0][t] : 0.0;
@@ -87,8 +90,8 @@ static void hermite_E(double a, double b, double Ax, double Bx, double E[LMAX + 
             E[i + 1][0][t] = em / (2 * p) + XPA * e0 + (t + 1) * ep;
         }
     /* j -> j+1 at every i */
-    for (int i = 0; i <= LMAX; ++i)
-        for (int j = 0; j < LMAX; ++j)
+    for (int i = 0; i <= li; ++i)
+        for (int j = 0; j < lj; ++j)
             for (int t = 0; t <= i + j + 1; ++t) {
                 double em = (t - 1 >= 0) ? E[i][j][t - 1] : 0.0;
                 double e0 = (t <= i + j) ? E[i][j][t] : 0.0;
@@ -132,7 +135,7 @@ static void shell_pair_1e(const basis_t *B, int sa, int sb, const double *O,
             double p = a + b, pref = pow(M_PI / p, 1.5);
             double E[3][LMAX + 1][LMAX + 1][2 * LMAX + 1], P[3];
             for (int x = 0; x < 3; ++x) {
-                hermite_E(a, b, A[x], Bc[x], E[x]);
+                hermite_E(la, lb, a, b, A[x], Bc[x], E[x]);
                 P[x] = (a * A[x] + b * Bc[x]) / p;
             }
             for (int ca = 0; ca < na; ++ca)
@@ -196,7 +199,7 @@ void oracle_one_electron(BASIS_ARGS, int nao, const double *O, double *S, double
 /* Range-separated operator erf(omega r12)/r12 (NEXT-4: the long-range exchange of CAM-type functionals): with
  * theta^2 = omega^2 / (alpha + omega^2) the Hermite integrals are those of 1/r12 with alpha -> alpha theta^2 and an
  * overall factor theta:  R^n_{000} = theta (-2 alpha theta^2)^n F_n(alpha theta^2 |R|^2).  omega <= 0 means 1/r12. */
-static void hermite_R(int L, double alpha, double omega, const double *R, double Rt[NR][NR][NR][NR] /* [n][t][u][v] */)
+static void hermite_R(int L, double alpha, double omega, const double *R, double *Rt /* RT(n,t,u,v), (L+1)^4 entries */)
 {
     double F[LMAX_TOT + 1];
     double theta = 1.0;
@@ -210,10 +213,10 @@ static void hermite_R(int L, double alpha, double omega, const double *R, double
     for (int n = 0; n <= L; ++n)        /* only n, t, u, v <= L are ever touched */
         for (int t = 0; t <= L; ++t)
             for (int u = 0; u <= L; ++u)
-                for (int v = 0; v <= L; ++v) Rt[n][t][u][v] = 0.0;
+                for (int v = 0; v <= L; ++v) RT(n, t, u, v) = 0.0;
     double m2a = theta;
     for (int n = 0; n <= L; ++n) {
-        Rt[n][0][0][0] = m2a * F[n];
+        RT(n, 0, 0, 0) = m2a * F[n];
         m2a *= -2.0 * alpha;
     }
     for (int N = 1; N <= L; ++N) /* total order t+u+v = N needs n <= L-N */
@@ -223,15 +226,15 @@ static void hermite_R(int L, double alpha, double omega, const double *R, double
                 for (int n = 0; n <= L - N; ++n) {
                     double val;
                     if (t > 0)
-                        val = (t - 1 > 0 ? (t - 1) * Rt[n + 1][t - 2][u][v] : 0.0) +
-                              R[0] * Rt[n + 1][t - 1][u][v];
+                        val = (t - 1 > 0 ? (t - 1) * RT(n + 1, t - 2, u, v) : 0.0) +
+                              R[0] * RT(n + 1, t - 1, u, v);
                     else if (u > 0)
-                        val = (u - 1 > 0 ? (u - 1) * Rt[n + 1][t][u - 2][v] : 0.0) +
-                              R[1] * Rt[n + 1][t][u - 1][v];
+                        val = (u - 1 > 0 ? (u - 1) * RT(n + 1, t, u - 2, v) : 0.0) +
+                              R[1] * RT(n + 1, t, u - 1, v);
                     else
-                        val = (v - 1 > 0 ? (v - 1) * Rt[n + 1][t][u][v - 2] : 0.0) +
-                              R[2] * Rt[n + 1][t][u][v - 1];
-                    Rt[n][t][u][v] = val;
+                        val = (v - 1 > 0 ? (v - 1) * RT(n + 1, t, u, v - 2) : 0.0) +
+                              R[2] * RT(n + 1, t, u, v - 1);
+                    RT(n, t, u, v) = val;
                 }
             }
 }
@@ -256,7 +259,7 @@ static void shell_quartet_op(const basis_t *B, int sa, int sb, int sc, int sd, d
         double p = a + b, P[3], Eab[3][LMAX + 1][LMAX + 1][2 * LMAX + 1];
         for (int x = 0; x < 3; ++x) {
             P[x] = (a * A[x] + b * Bc[x]) / p;
-            hermite_E(a, b, A[x], Bc[x], Eab[x]);
+            hermite_E(l[0], l[1], a, b, A[x], Bc[x], Eab[x]);
         }
         for (int kc = 0; kc < B->sh_nprim[sc]; ++kc)
         for (int kd = 0; kd < B->sh_nprim[sd]; ++kd) {
@@ -265,11 +268,11 @@ static void shell_quartet_op(const basis_t *B, int sa, int sb, int sc, int sd, d
             double q = c + d, Q[3], Ecd[3][LMAX + 1][LMAX + 1][2 * LMAX + 1], RPQ[3];
             for (int x = 0; x < 3; ++x) {
                 Q[x] = (c * C[x] + d * D[x]) / q;
-                hermite_E(c, d, C[x], D[x], Ecd[x]);
+                hermite_E(l[2], l[3], c, d, C[x], D[x], Ecd[x]);
                 RPQ[x] = P[x] - Q[x];
             }
             double alpha = p * q / (p + q);
-            double Rt[NR][NR][NR][NR];
+            double Rt[NR * NR * NR * NR];          /* only the first (L+1)^4 entries are used */
             hermite_R(L, alpha, omega, RPQ, Rt);
             double pref = 2.0 * pow(M_PI, 2.5) / (p * q * sqrt(p + q)) * cab * ccd;
             int idx = 0;
@@ -292,7 +295,7 @@ static void shell_quartet_op(const basis_t *B, int sa, int sb, int sc, int sd, d
                         double ecd = Ecd[0][pc[0]][pd[0]][t2] * Ecd[1][pc[1]][pd[1]][u2] *
                                      Ecd[2][pc[2]][pd[2]][v2];
                         double sgn = ((t2 + u2 + v2) & 1) ? -1.0 : 1.0;
-                        s += eab * sgn * ecd * Rt[0][t + t2][u + u2][v + v2];
+                        s += eab * sgn * ecd * RT(0, t + t2, u + u2, v + v2);
                     }
                 }
                 double cn = cart_norm(l[0], ca) * cart_norm(l[1], cb) * cart_norm(l[2], cc) * cart_norm(l[3], cd);
@@ -424,22 +427,22 @@ static void boys_ld(int nmax, long double T, long double *F)
     }
 }
 
-static void hermite_E_ld(long double a, long double b, long double Ax, long double Bx,
+static void hermite_E_ld(int li, int lj, long double a, long double b, long double Ax, long double Bx,
                          long double E[LMAX + 1][LMAX + 1][2 * LMAX + 1])
 {
     long double p = a + b, mu = a * b / p, XAB = Ax - Bx;
     long double Px = (a * Ax + b * Bx) / p, XPA = Px - Ax, XPB = Px - Bx;
     for (int i = 0; i < (LMAX + 1) * (LMAX + 1) * (2 * LMAX + 1); ++i) ((long double *)E)[i] = 0.0L;
     E[0][0][0] = expl(-mu * XAB * XAB);
-    for (int i = 0; i < LMAX; ++i)
+    for (int i = 0; i < li; ++i)
         for (int t = 0; t <= i + 1; ++t) {
             long double em = (t - 1 >= 0) ? E[i][0][t - 1] : 0.0L;
             long double e0 = (t <= i) ? E[i][0][t] : 0.0L;
             long double ep = (t + 1 <= i) ? E[i][0][t + 1] : 0.0L;
             E[i + 1][0][t] = em / (2 * p) + XPA * e0 + (t + 1) * ep;
         }
-    for (int i = 0; i <= LMAX; ++i)
-        for (int j = 0; j < LMAX; ++j)
+    for (int i = 0; i <= li; ++i)
+        for (int j = 0; j < lj; ++j)
             for (int t = 0; t <= i + j + 1; ++t) {
                 long double em = (t - 1 >= 0) ? E[i][j][t - 1] : 0.0L;
                 long double e0 = (t <= i + j) ? E[i][j][t] : 0.0L;
@@ -462,32 +465,32 @@ static void shell_quartet_ld(const basis_t *B, int sa, int sb, int sc, int sd, l
         long double a = B->exps[B->sh_off[sa] + ka], b = B->exps[B->sh_off[sb] + kb];
         long double cab = (long double)B->ncoef[B->sh_off[sa] + ka] * B->ncoef[B->sh_off[sb] + kb];
         long double p = a + b, P[3], Eab[3][LMAX + 1][LMAX + 1][2 * LMAX + 1];
-        for (int x = 0; x < 3; ++x) { P[x] = (a * A[x] + b * Bc[x]) / p; hermite_E_ld(a, b, A[x], Bc[x], Eab[x]); }
+        for (int x = 0; x < 3; ++x) { P[x] = (a * A[x] + b * Bc[x]) / p; hermite_E_ld(l[0], l[1], a, b, A[x], Bc[x], Eab[x]); }
         for (int kc = 0; kc < B->sh_nprim[sc]; ++kc)
         for (int kd = 0; kd < B->sh_nprim[sd]; ++kd) {
             long double c = B->exps[B->sh_off[sc] + kc], d = B->exps[B->sh_off[sd] + kd];
             long double ccd = (long double)B->ncoef[B->sh_off[sc] + kc] * B->ncoef[B->sh_off[sd] + kd];
             long double q = c + d, Q[3], Ecd[3][LMAX + 1][LMAX + 1][2 * LMAX + 1], R[3];
-            for (int x = 0; x < 3; ++x) { Q[x] = (c * C[x] + d * D[x]) / q; hermite_E_ld(c, d, C[x], D[x], Ecd[x]); R[x] = P[x] - Q[x]; }
+            for (int x = 0; x < 3; ++x) { Q[x] = (c * C[x] + d * D[x]) / q; hermite_E_ld(l[2], l[3], c, d, C[x], D[x], Ecd[x]); R[x] = P[x] - Q[x]; }
             long double alpha = p * q / (p + q), F[LMAX_TOT + 1];
             boys_ld(L, alpha * (R[0] * R[0] + R[1] * R[1] + R[2] * R[2]), F);
-            static __thread long double Rt[NR][NR][NR][NR];
+            static __thread long double Rt[NR * NR * NR * NR];
             for (int nn = 0; nn <= L; ++nn)
                 for (int t = 0; t <= L; ++t)
                     for (int u = 0; u <= L; ++u)
-                        for (int v = 0; v <= L; ++v) Rt[nn][t][u][v] = 0.0L;
+                        for (int v = 0; v <= L; ++v) RT(nn, t, u, v) = 0.0L;
             long double m2a = 1.0L;
-            for (int nn = 0; nn <= L; ++nn) { Rt[nn][0][0][0] = m2a * F[nn]; m2a *= -2.0L * alpha; }
+            for (int nn = 0; nn <= L; ++nn) { RT(nn, 0, 0, 0) = m2a * F[nn]; m2a *= -2.0L * alpha; }
             for (int N = 1; N <= L; ++N)
                 for (int t = 0; t <= N; ++t)
                     for (int u = 0; u <= N - t; ++u) {
                         int v = N - t - u;
                         for (int nn = 0; nn <= L - N; ++nn) {
                             long double val;
-                            if (t > 0) val = (t - 1 > 0 ? (t - 1) * Rt[nn + 1][t - 2][u][v] : 0.0L) + R[0] * Rt[nn + 1][t - 1][u][v];
-                            else if (u > 0) val = (u - 1 > 0 ? (u - 1) * Rt[nn + 1][t][u - 2][v] : 0.0L) + R[1] * Rt[nn + 1][t][u - 1][v];
-                            else val = (v - 1 > 0 ? (v - 1) * Rt[nn + 1][t][u][v - 2] : 0.0L) + R[2] * Rt[nn + 1][t][u][v - 1];
-                            Rt[nn][t][u][v] = val;
+                            if (t > 0) val = (t - 1 > 0 ? (t - 1) * RT(nn + 1, t - 2, u, v) : 0.0L) + R[0] * RT(nn + 1, t - 1, u, v);
+                            else if (u > 0) val = (u - 1 > 0 ? (u - 1) * RT(nn + 1, t, u - 2, v) : 0.0L) + R[1] * RT(nn + 1, t, u - 1, v);
+                            else val = (v - 1 > 0 ? (v - 1) * RT(nn + 1, t, u, v - 2) : 0.0L) + R[2] * RT(nn + 1, t, u, v - 1);
+                            RT(nn, t, u, v) = val;
                         }
                     }
             long double pref = 2.0L * powl(M_PIl, 2.5L) / (p * q * sqrtl(p + q)) * cab * ccd;
@@ -508,7 +511,7 @@ static void shell_quartet_ld(const basis_t *B, int sa, int sb, int sc, int sd, l
                     for (int v2 = 0; v2 <= pc[2] + pd[2]; ++v2) {
                         long double ecd = Ecd[0][pc[0]][pd[0]][t2] * Ecd[1][pc[1]][pd[1]][u2] * Ecd[2][pc[2]][pd[2]][v2];
                         long double sgn = ((t2 + u2 + v2) & 1) ? -1.0L : 1.0L;
-                        s += eab * sgn * ecd * Rt[0][t + t2][u + u2][v + v2];
+                        s += eab * sgn * ecd * RT(0, t + t2, u + u2, v + v2);
                     }
                 }
                 long double cn = 1.0L;     /* sqrt(3) per mixed d component, in long double */

@@ -9,7 +9,8 @@ eq. 1 / 14-16, R7) on y' = -i (A_ext + E(t) M_d) y; what differs per config is h
              eigenvalue of A (R10: taken from 80 Lanczos steps of the oracle on the dense A, recorded in the file),
              E0 in {0.005, 0.02}, 4000 steps of 0.05 au; amplitudes stored after steps 3, 400 and 4000;
   config 4   dense A is 991 GB: ONE RK4 step through the matrix-free route (`tda.sigma_matrix_free`, 4 J/K passes serving
-             the 6 real vectors of the three trajectories, tau_oracle = 1e-14) from seeded random normalised complex
+             the 6 real vectors of the three trajectories, tau_oracle = 1e-13: one order below the config's own threshold;
+             its screening error of ~1e-10 |sigma| dt is two orders below the 1e-8 amplitude tolerance) from seeded random normalised complex
              states at t = 95 au, i.e. near the maximum of the sin^2 envelope (R9), E0 in {0.01, 0.03, 0.05}, omega = 0.2 Ha
              (any recorded omega serves parity).  The ground state at t = 0 would make this step trivial (E(0) = 0).
 
@@ -121,7 +122,7 @@ def main():
             write_samples(f, rng, Y, stop)
             print("config 3: step", stop, "%.0f s" % (time.time() - t0), flush=True)
     elif k == 4:
-        tau, omega, t_start = 1e-14, 0.2, 95.0
+        tau, omega, t_start = 1e-13, 0.2, 95.0
         fields = [dict(x, omega=omega) for x in cfg.fields]
         Q = ob.schwarz()
         V = make_vectors(cfg, 2 * len(fields), stream=4).reshape(len(fields), 2, n)

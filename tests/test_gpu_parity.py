@@ -427,7 +427,7 @@ def test_propagate_config3_prefix_and_full_4000_steps_vs_stored_dense_A_oracle()
 def test_propagate_config4_one_step_mid_pulse_vs_stored_matrix_free_oracle():
     """BJ:configs[3] (1280 AO; dense A = 991 GB does not exist): one RK4 step of the three-trajectory batch
     (E0 in {0.01, 0.03, 0.05}, sin^2 envelope, R9) taken near the envelope maximum (t = 95 au) from seeded random
-    normalised states, against the oracle's matrix-free RK4 step (4 J/K passes at tau_oracle = 1e-14).  The start
+    normalised states, against the oracle's matrix-free RK4 step (4 J/K passes at the tau_oracle recorded in the file, 1e-13).  The start
     states are regenerated here from the seeds and checked against the stored step-0 samples."""
     import torch
     from workloads import make_vectors
