@@ -9,6 +9,10 @@
 
 namespace rttda {
 
+#ifndef RTTDA_SCALED_STAGES
+#define RTTDA_SCALED_STAGES 1
+#endif
+
 __host__ __device__ constexpr int nherm(int L) { return (L + 1) * (L + 2) * (L + 3) / 6; }
 // index of Hermite component (t,u,v): ordered by total order N, then s = N - t, then v
 __host__ __device__ constexpr int hidx(int t, int u, int v)
@@ -84,9 +88,12 @@ __device__ __forceinline__ double rsqrt_fast(double x)
     return fma(y * e, fma(0.375, e, 0.5), y);
 }
 
-template <int L>
+// SCALED: the table is returned as gs^(t+u+v) R_{tuv} (the operator stages of eri_prim_accum then need no multiply by
+// their 1/2p: see apply_p); the powers of gs ride along the recursion, r~^n_{t+1,u,v} = (gs X) r~^{n+1}_{tuv} +
+// (t gs^2) r~^{n+1}_{t-1,u,v}, at the price of five multiplies per primitive quartet.
+template <int L, bool SCALED = false>
 __device__ __forceinline__ void hermite_R(double cc, double wb, double wk, double X, double Y, double Z,
-                                          const double2* __restrict__ tab, double (&R0)[nherm(L)])
+                                          const double2* __restrict__ tab, double (&R0)[nherm(L)], double gs = 1.0)
 {
     double r[L + 1][nherm(L)];
     const double R2 = fma(X, X, fma(Y, Y, Z * Z));
@@ -109,6 +116,8 @@ __device__ __forceinline__ void hermite_R(double cc, double wb, double wk, doubl
 #pragma unroll
         for (int n = 0; n < L; ++n) r[n + 1][0] = ((2 * n + 1) * wn) * r[n][0];
     }
+    if (SCALED) { X *= gs; Y *= gs; Z *= gs; }
+    const double g2 = SCALED ? gs * gs : 1.0;                // multiplies the (t-1) factors below
 #pragma unroll
     for (int N = 1; N <= L; ++N)
 #pragma unroll
@@ -121,13 +130,13 @@ __device__ __forceinline__ void hermite_R(double cc, double wb, double wk, doubl
                     double val;
                     if (t > 0) {
                         val = X * r[n + 1][hidx(t - 1, u, v)];
-                        if (t > 1) val = fma((double)(t - 1), r[n + 1][hidx(t - 2, u, v)], val);
+                        if (t > 1) val = fma((double)(t - 1) * g2, r[n + 1][hidx(t - 2, u, v)], val);
                     } else if (u > 0) {
                         val = Y * r[n + 1][hidx(t, u - 1, v)];
-                        if (u > 1) val = fma((double)(u - 1), r[n + 1][hidx(t, u - 2, v)], val);
+                        if (u > 1) val = fma((double)(u - 1) * g2, r[n + 1][hidx(t, u - 2, v)], val);
                     } else {
                         val = Z * r[n + 1][hidx(t, u, v - 1)];
-                        if (v > 1) val = fma((double)(v - 1), r[n + 1][hidx(t, u, v - 2)], val);
+                        if (v > 1) val = fma((double)(v - 1) * g2, r[n + 1][hidx(t, u, v - 2)], val);
                     }
                     r[n][hidx(t, u, v)] = val;
                 }
@@ -137,7 +146,9 @@ __device__ __forceinline__ void hermite_R(double cc, double wb, double wk, doubl
 
 // One operator application: out[c][h] = X[c] * in[h] + g * in[h + e_c] for |h| <= LOUT (g = +1/2p for bra
 // functions, -1/2q for ket functions).  NC = 1 means "s function": plain copy of the first nherm(LOUT).
-template <int NC, int LOUT, int NBLK>
+// SCALED: the tables carry g^(order) (hermite_R<L, true>, rescale_orders), so that g * in[h + e_c] is in[h + e_c] itself
+// and a stage is one FMA per output.
+template <int NC, int LOUT, int NBLK, bool SCALED = false>
 __device__ __forceinline__ void apply_p(const double (&in)[NBLK][nherm(LOUT + (NC == 3 ? 1 : 0))],
                                         const double* X, double g, double (&out)[NBLK * NC][nherm(LOUT)])
 {
@@ -156,7 +167,7 @@ __device__ __forceinline__ void apply_p(const double (&in)[NBLK][nherm(LOUT + (N
 #pragma unroll
                         for (int v = LOUT - t - u; v >= 0; --v)
                             out[b * 3 + c][hidx(t, u, v)] =
-                                fma(X[c], in[b][hidx(t, u, v)], g * in[b][hidx_plus(t, u, v, c)]);
+                                fma(X[c], in[b][hidx(t, u, v)], SCALED ? in[b][hidx_plus(t, u, v, c)] : g * in[b][hidx_plus(t, u, v, c)]);
         }
     }
 }
@@ -165,12 +176,14 @@ __device__ __forceinline__ void apply_p(const double (&in)[NBLK][nherm(LOUT + (N
 // w = 36/p and c' = c pi^(1/4)/sqrt(2p) (see hermite_R) once to_scaled() has been applied to a table row.
 struct PrimPair {
     double p, Px, Py, Pz, c, inv2p;
+    double two_p;   // 2p = 1 / inv2p (set by to_scaled; used for kets only)
     double XA[3];   // P - (first centre)
     double XB[3];   // P - (second centre)
 };
 
 __device__ __forceinline__ void to_scaled(PrimPair& r)
 {
+    r.two_p = 2.0 * r.p;
     r.c *= 1.33133536380038971280 * rsqrt(2.0 * r.p);        // pi^(1/4)
     r.p = 36.0 / r.p;
 }
@@ -185,12 +198,18 @@ __device__ __forceinline__ void eri_prim_accum(const PrimPair& br, const PrimPai
 {
     constexpr int L = LA + LB + LC + LD;
     constexpr int NA = 2 * LA + 1, NB = 2 * LB + 1, NC = 2 * LC + 1, ND = 2 * LD + 1;
+    // Scaled stages (RTTDA_SCALED_STAGES): the Hermite tables carry g^(order), g = -1/2q while the ket operators are
+    // applied and +1/2p for the bra operators, so that a stage costs one FMA per output instead of a multiply and an
+    // FMA; between the two phases the (few) remaining entries are rescaled by (g_bra / g_ket)^(order).
+    constexpr bool SC = RTTDA_SCALED_STAGES && L >= 2;
+    constexpr bool KET_PHASE = LC + LD > 0, BRA_PHASE = LA + LB > 0;
+    const double gk = -kt.inv2p, gb = br.inv2p;
     double V0[1][nherm(L)];
-    hermite_R<L>(br.c * kt.c, br.p, kt.p, br.Px - kt.Px, br.Py - kt.Py, br.Pz - kt.Pz, tab, V0[0]);
+    hermite_R<L, SC>(br.c * kt.c, br.p, kt.p, br.Px - kt.Px, br.Py - kt.Py, br.Pz - kt.Pz, tab, V0[0], KET_PHASE ? gk : gb);
     double VD[ND][nherm(L - LD)];
-    apply_p<ND, L - LD, 1>(V0, kt.XB, -kt.inv2p, VD);
+    apply_p<ND, L - LD, 1, SC>(V0, kt.XB, gk, VD);
     double VC[ND * NC][nherm(L - LD - LC)];
-    apply_p<NC, L - LD - LC, ND>(VD, kt.XA, -kt.inv2p, VC);
+    apply_p<NC, L - LD - LC, ND, SC>(VD, kt.XA, gk, VC);
     // The operators above treat X_QC, X_QD as constants; two p functions on one pair with the SAME Cartesian
     // component pick up the extra term of E_0^{11} = X_PA X_PB + 1/2p (x_P Lambda_1 = Lambda_2/2p + Lambda_0).
     if constexpr (LC == 1 && LD == 1) {
@@ -200,10 +219,17 @@ __device__ __forceinline__ void eri_prim_accum(const PrimPair& br, const PrimPai
             for (int hh = 0; hh < nherm(L - LD - LC); ++hh)
                 VC[c * NC + c][hh] = fma(kt.inv2p, V0[0][hh], VC[c * NC + c][hh]);
     }
+    if constexpr (SC && KET_PHASE && BRA_PHASE) {              // g_ket^(order) -> g_bra^(order)
+        const double rho = -(br.inv2p * kt.two_p), rho2 = rho * rho;
+#pragma unroll
+        for (int dc = 0; dc < ND * NC; ++dc)
+#pragma unroll
+            for (int hh = 1; hh < nherm(LA + LB); ++hh) VC[dc][hh] *= (hh < nherm(1) ? rho : rho2);
+    }
     double VB[ND * NC * NB][nherm(LA)];
-    apply_p<NB, LA, ND * NC>(VC, br.XB, br.inv2p, VB);
+    apply_p<NB, LA, ND * NC, SC>(VC, br.XB, gb, VB);
     double VA[ND * NC * NB * NA][1];
-    apply_p<NA, 0, ND * NC * NB>(VB, br.XA, br.inv2p, VA);
+    apply_p<NA, 0, ND * NC * NB, SC>(VB, br.XA, gb, VA);
     if constexpr (LA == 1 && LB == 1) {
 #pragma unroll
         for (int dc = 0; dc < ND * NC; ++dc)

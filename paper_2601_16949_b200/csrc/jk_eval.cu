@@ -55,7 +55,7 @@ __device__ __forceinline__ PrimPair load_bra_prim_smem(const double* row)
     PrimPair r;
     const double2* r2 = reinterpret_cast<const double2*>(row);
     const double2 a = r2[0], b = r2[1], c = r2[2], d = r2[3], e = r2[4], f = r2[5];
-    r.p = a.x; r.Px = a.y; r.Py = b.x; r.Pz = b.y; r.c = c.x; r.inv2p = c.y;
+    r.p = a.x; r.Px = a.y; r.Py = b.x; r.Pz = b.y; r.c = c.x; r.inv2p = c.y; r.two_p = 0.0;   // two_p: kets only
     r.XA[0] = d.x; r.XA[1] = d.y; r.XA[2] = e.x; r.XB[0] = e.y; r.XB[1] = f.x; r.XB[2] = f.y;
     return r;
 }
