@@ -98,8 +98,10 @@ __device__ __forceinline__ void hermite_R(double cc, double wb, double wk, doubl
     double r[L + 1][nherm(L)];
     const double R2 = fma(X, X, fma(Y, Y, Z * Z));
     const double w = wb + wk;
-    if (R2 < w) {
-        const double rw = rsqrt_fast(w);
+    const bool near = R2 < w;
+    const double rs = rsqrt_fast(near ? w : R2);             // one rsqrt serves both branches of a mixed warp
+    if (near) {
+        const double rw = rs;
         const double alpha = 36.0 * (rw * rw);
         double F[L + 1];
         boys_near<L>(alpha * R2, tab, F);
@@ -110,7 +112,7 @@ __device__ __forceinline__ void hermite_R(double cc, double wb, double wk, doubl
             sc *= -2.0 * alpha;
         }
     } else {
-        const double u = rsqrt_fast(R2);
+        const double u = rs;
         r[0][0] = cc * u;
         const double wn = -(u * u);                          // -1/R^2
 #pragma unroll
