@@ -272,7 +272,7 @@ int eval_segment_d(Handle* h, const Segment& sg, double* buf, cudaStream_t st, b
         case ((2 * 3 + 1) * 3 + 2) * 3 + 0: return launch_eval_d<2, 1, 2, 0, 2>(h, sg, buf, st);
         case ((2 * 3 + 2) * 3 + 1) * 3 + 0: return launch_eval_d<2, 2, 1, 0, 3>(h, sg, buf, st);
         case ((2 * 3 + 1) * 3 + 2) * 3 + 1: return launch_eval_d<2, 1, 2, 1, 3>(h, sg, buf, st);
-        case ((2 * 3 + 2) * 3 + 1) * 3 + 1: return launch_eval_d<2, 2, 1, 1, 1>(h, sg, buf, st);
+        case ((2 * 3 + 2) * 3 + 1) * 3 + 1: return launch_eval_d<2, 2, 1, 1, 2>(h, sg, buf, st);
         case ((2 * 3 + 2) * 3 + 2) * 3 + 0: return launch_eval_d<2, 2, 2, 0, 2>(h, sg, buf, st);
         case ((2 * 3 + 2) * 3 + 2) * 3 + 1: return launch_eval_d<2, 2, 2, 1, 2>(h, sg, buf, st);
         default: *handled = false; return RTTDA_OK;
