@@ -235,3 +235,30 @@ def test_d1884_fock_sampled_elements_and_properties():
     F2 = gpu_fock(ctx, np.stack([T[0] + T[0].T, 2.0 * T[1] - 0.5 * T[0]]))
     assert np.max(np.abs(F2[0] - (F[0] + F[0].T))) / scale < SIGMA_TOL     # F[T^T] = F[T]^T
     assert np.max(np.abs(F2[1] - (2.0 * F[1] - 0.5 * F[0]))) / scale < SIGMA_TOL
+
+
+def test_d_molecule_eigenpairs_and_sso_step_vs_dense_oracle():
+    """The other consumers of the sigma build on a basis with d shells: the lowest TI-TDA eigenpairs (rttda_eigs) against
+    eigh of the oracle's dense A, and 10 steps of the paper's split-operator propagator against the oracle's."""
+    import torch
+    from oracle import tda
+    ctx = setup_config(6, dense=True)
+    A, h, cfg = ctx["A"], ctx["h"], ctx["cfg"]
+    n = A.shape[0]
+    w = np.linalg.eigvalsh(A)
+    X = torch.zeros((4, n), dtype=torch.float64, device=ctx["dev"])
+    om, rs, it, ns = h.rttda_eigs(4, X, 8, tol=1e-9, maxiter=100)
+    Xh = X.cpu().numpy()
+    assert np.max(np.abs(om - w[:4])) < 1e-8           # tau = 1e-12 in A's integrals: eigenvalues move by ~1e-11
+    assert np.max(np.linalg.norm(Xh @ A.T - om[:, None] * Xh, axis=1)) < 5e-8
+    fld = dict(cfg.fields[0])
+    D = ctx["ob"].dipole()
+    Doo, Dvv, Dov, D00 = tda.mo_dipoles(D, ctx["C_o"], ctx["C_v"], fld["dir"])
+    y0 = np.zeros(n + 1, dtype=complex); y0[0] = 1.0
+    yref, _ = tda.sso_dense(A, Doo, Dvv, Dov, D00, y0, fld, 0.0, cfg.dt, cfg.nsteps)
+    y = torch.zeros((1, 2, n + 1), dtype=torch.float64, device=ctx["dev"])
+    y[:, 0, 0] = 1.0
+    h.rttda_propagate_sso(y, [fld], 0.0, cfg.dt, cfg.nsteps, None)
+    torch.cuda.synchronize()
+    yy = y.cpu().numpy()
+    assert np.max(np.abs((yy[0, 0] + 1j * yy[0, 1]) - yref)) < AMP_TOL
