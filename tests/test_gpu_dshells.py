@@ -138,7 +138,7 @@ def test_d_molecule_range_separated_exchange(cx, cx_lr, omega):
     h.close()
 
 
-@pytest.mark.parametrize("seed", [1, 2, 3, 4])
+@pytest.mark.parametrize("seed", [1, 2, 3, 4, 5, 6, 7, 8])
 def test_random_molecules_with_contracted_d_shells(seed):
     """Random centres, s/p/d shells with contraction depths 1..3 on the d shells too, tau in {0, 1e-10}."""
     import paper_2601_16949_b200 as R
