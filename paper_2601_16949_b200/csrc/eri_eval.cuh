@@ -12,6 +12,9 @@ namespace rttda {
 #ifndef RTTDA_SCALED_STAGES
 #define RTTDA_SCALED_STAGES 1
 #endif
+#ifndef RTTDA_FUSED_L1
+#define RTTDA_FUSED_L1 1
+#endif
 
 __host__ __device__ constexpr int nherm(int L) { return (L + 1) * (L + 2) * (L + 3) / 6; }
 // index of Hermite component (t,u,v): ordered by total order N, then s = N - t, then v
@@ -88,6 +91,32 @@ __device__ __forceinline__ double rsqrt_fast(double x)
     return fma(y * e, fma(0.375, e, 0.5), y);
 }
 
+// The seeds of the recursion alone: s[n] = pref (-2 alpha)^n F_n(T), n <= L (see hermite_R for the two branches).
+template <int L>
+__device__ __forceinline__ void hermite_seeds(double cc, double wb, double wk, double R2, const double2* __restrict__ tab,
+                                              double (&s)[L + 1])
+{
+    const double w = wb + wk;
+    const bool near = R2 < w;
+    const double rs = rsqrt_fast(near ? w : R2);             // one rsqrt serves both branches of a mixed warp
+    if (near) {
+        const double alpha = 36.0 * (rs * rs);
+        double F[L + 1];
+        boys_near<L>(alpha * R2, tab, F);
+        double sc = cc * 6.77027500257307544338 * rs;        // 12 / sqrt(pi)
+#pragma unroll
+        for (int n = 0; n <= L; ++n) {
+            s[n] = sc * F[n];
+            sc *= -2.0 * alpha;
+        }
+    } else {
+        s[0] = cc * rs;
+        const double wn = -(rs * rs);                        // -1/R^2
+#pragma unroll
+        for (int n = 0; n < L; ++n) s[n + 1] = ((2 * n + 1) * wn) * s[n];
+    }
+}
+
 // SCALED: the table is returned as gs^(t+u+v) R_{tuv} (the operator stages of eri_prim_accum then need no multiply by
 // their 1/2p: see apply_p); the powers of gs ride along the recursion, r~^n_{t+1,u,v} = (gs X) r~^{n+1}_{tuv} +
 // (t gs^2) r~^{n+1}_{t-1,u,v}, at the price of five multiplies per primitive quartet.
@@ -97,27 +126,10 @@ __device__ __forceinline__ void hermite_R(double cc, double wb, double wk, doubl
 {
     double r[L + 1][nherm(L)];
     const double R2 = fma(X, X, fma(Y, Y, Z * Z));
-    const double w = wb + wk;
-    const bool near = R2 < w;
-    const double rs = rsqrt_fast(near ? w : R2);             // one rsqrt serves both branches of a mixed warp
-    if (near) {
-        const double rw = rs;
-        const double alpha = 36.0 * (rw * rw);
-        double F[L + 1];
-        boys_near<L>(alpha * R2, tab, F);
-        double sc = cc * 6.77027500257307544338 * rw;        // 12 / sqrt(pi)
+    double seeds[L + 1];
+    hermite_seeds<L>(cc, wb, wk, R2, tab, seeds);
 #pragma unroll
-        for (int n = 0; n <= L; ++n) {
-            r[n][0] = sc * F[n];
-            sc *= -2.0 * alpha;
-        }
-    } else {
-        const double u = rs;
-        r[0][0] = cc * u;
-        const double wn = -(u * u);                          // -1/R^2
-#pragma unroll
-        for (int n = 0; n < L; ++n) r[n + 1][0] = ((2 * n + 1) * wn) * r[n][0];
-    }
+    for (int n = 0; n <= L; ++n) r[n][0] = seeds[n];
     if (SCALED) { X *= gs; Y *= gs; Z *= gs; }
     const double g2 = SCALED ? gs * gs : 1.0;                // multiplies the (t-1) factors below
 #pragma unroll
@@ -203,6 +215,18 @@ __device__ __forceinline__ void eri_prim_accum(const PrimPair& br, const PrimPai
     // Scaled stages (RTTDA_SCALED_STAGES): the Hermite tables carry g^(order), g = -1/2q while the ket operators are
     // applied and +1/2p for the bra operators, so that a stage costs one FMA per output instead of a multiply and an
     // FMA; between the two phases the (few) remaining entries are rescaled by (g_bra / g_ket)^(order).
+    if constexpr (RTTDA_FUSED_L1 && LA == 1 && LB + LC + LD == 0) {
+        // (ps|ss): (a_c b|cd) = X_PA,c R_000 + (1/2p) R_{e_c}, R_{e_c} = (P-Q)_c r^1_000: two FMAs per component straight
+        // into the accumulators, no table
+        const double X = br.Px - kt.Px, Y = br.Py - kt.Py, Z = br.Pz - kt.Pz;
+        double sd[2];
+        hermite_seeds<1>(br.c * kt.c, br.p, kt.p, fma(X, X, fma(Y, Y, Z * Z)), tab, sd);
+        const double q = br.inv2p * sd[1];
+        I[0] = fma(X, q, fma(br.XA[0], sd[0], I[0]));
+        I[1] = fma(Y, q, fma(br.XA[1], sd[0], I[1]));
+        I[2] = fma(Z, q, fma(br.XA[2], sd[0], I[2]));
+        return;
+    }
     constexpr bool SC = RTTDA_SCALED_STAGES && L >= 2;
     constexpr bool KET_PHASE = LC + LD > 0, BRA_PHASE = LA + LB > 0;
     const double gk = -kt.inv2p, gb = br.inv2p;
